@@ -1,0 +1,144 @@
+/* jenga.h -- C-ABI of the B200-native batched Jenga rigid-body step.
+ *
+ * The operation is the time step of arxiv/paper_2606_28394 (§4 "Rigid-body dynamics",
+ * §6 "Collision detection", §7 "Contact solver"), batched over independent tower episodes
+ * ("envs"), in the canonical order fixed by SURVEY.md §8(c) S0-S7 / DESIGN.md §2:
+ *
+ *   S1 predict      v += h (g + f/m), w += h Iw^-1 tau              Eq. 4-5,
+ *   S2 broadphase   world-AABB overlap with margin eps              Eq. 10-11
+ *   S3 narrowphase  15-axis OBB SAT + face/edge manifold (<=4 pts)  §6.2,
+ *   S4 setup        r_A, r_B, tangent basis, effective masses       Eq. 12-13
+ *   S5 PGS          normal rows clamped >= 0, friction rows boxed   Eq. 14-15 + Listing 1
+ *   S6 integrate    x += h v, q <- normalise(q + h/2 [0,w] q),      Eq. 2, 6, 16
+ *                   Baumgarte position correction per colliding pair
+ *
+ * Everything below is plain C: POD structs, raw pointers, sizes.  All buffer pointers are
+ * DEVICE pointers owned by the caller (the Python binding allocates them as torch tensors);
+ * the library never allocates or frees device memory, never synchronises and never touches
+ * the default stream: every call enqueues kernels on the `cuda_stream` it is given
+ * (a cudaStream_t passed as void*) and returns.  Return value: 0 = OK, negative = error
+ * (JENGA_E_*); data-dependent conditions (capacity overflow, non-finite state) are
+ * reported per env in `status[]`, with deterministic truncation (lowest pair indices kept).
+ *
+ * Indices.  Bodies 0..n_bodies-1; the ground plane z = 0 is body -1 (static).
+ * Canonical pair index: ground-body b -> b; bodies i<j -> B + i(2B-i-1)/2 + (j-i-1).
+ * In a pair, A is the lower id (ground first), the normal points from A to B
+ * (Listing 1: a loses the impulse, b gains it).
+ */
+#ifndef JENGA_H_
+#define JENGA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define JENGA_OK            0
+#define JENGA_E_ARG        -1   /* bad argument: NULL / misaligned pointer, capacity out of range */
+#define JENGA_E_CUDA       -2   /* CUDA error on launch; text via jenga_strerror(JENGA_E_CUDA) */
+#define JENGA_E_DEVICE     -3   /* device is not sm_100 (the kernels are compiled for sm_100a only) */
+
+/* status[env] bit flags */
+#define JENGA_ST_PAIR_OVERFLOW    1u   /* more broadphase candidates than max_pairs          */
+#define JENGA_ST_CONTACT_OVERFLOW 2u   /* more colliding pairs than max_contacts/4           */
+#define JENGA_ST_COLOUR_OVERFLOW  4u   /* greedy colouring needed more than 64 colours       */
+#define JENGA_ST_NONFINITE        8u   /* a position or velocity became inf/NaN              */
+
+#define JENGA_AXIS_GROUND 15           /* SAT axis id of a ground contact; 0-2 = A's face axes,
+                                          3-5 = B's, 6+3i+j = a_i x b_j  */
+
+/* counters[] slots (uint64, accumulated with atomics by jenga_step) */
+enum { JENGA_CNT_ENV_STEPS = 0, JENGA_CNT_BODY_STEPS, JENGA_CNT_CANDIDATES, JENGA_CNT_COLLIDING,
+       JENGA_CNT_CONTACTS, JENGA_CNT_CONTACT_ITERS, JENGA_CNT_COLOURS, JENGA_CNT_RESERVED, JENGA_N_COUNTERS };
+
+typedef struct jenga_world jenga_world;   /* opaque host-side handle; owns nothing on the device */
+
+typedef struct {
+  uint32_t struct_size;                 /* = sizeof(jenga_world_desc), checked                         */
+  int32_t  n_envs, n_bodies;            /* E, B                                                        */
+  int32_t  body_stride;                 /* S >= B, multiple of 4 (16-byte rows)                        */
+  float    dt;                          /* 1/240                                        */
+  int32_t  n_substeps;                  /* each substep = S1..S7 at h = dt/n_substeps   */
+  int32_t  pgs_iters;                   /* PGS sweeps per substep (paper: 14)            */
+  float    gravity[3];                  /* (0,0,-9.81)                                  */
+  float    restitution;                 /* e of Eq. 14                                  */
+  float    aabb_margin;                 /* eps of Eq. 10, 0.002                     */
+  float    baumgarte_beta, slop;        /* Eq. 16: 0.35, 4e-4                           */
+  float    edge_bias_rel, edge_bias_abs;/* face preference: edge axis iff dE < rel*dF - abs*/
+  float    par_eps;                     /* cross axes with |a x b|^2 < par_eps are skipped             */
+  float    tie_eps;                     /* an axis replaces the incumbent only if smaller by > tie_eps */
+  float    match_tol;                   /* warm-start contact-point matching radius [m]    */
+  int32_t  warm_start;                  /* 1: carry (jn,jt1,jt2) between steps                         */
+  int32_t  gyroscopic;                  /* 1: add -h Iw^-1 (w x Iw w) in S1 (Eq. 4); default 0         */
+  int32_t  max_pairs;                   /* candidate-pair capacity per env                             */
+  int32_t  max_contacts;                /* contact capacity per env; colliding pairs <= max_contacts/4;
+                                           32 <= max_contacts/4 <= 512                                 */
+  int32_t  materialise;                 /* 1: jenga_step also writes pairs/contacts/lambda of its last
+                                           substep (debug / parity); 0: they stay on chip              */
+  int32_t  device;                      /* CUDA device ordinal the buffers live on                     */
+} jenga_world_desc;
+
+/* All DEVICE pointers, caller-owned, 16-byte aligned.  PC = max_contacts/4. */
+typedef struct {
+  float       *state;      /* [E][13][S]  px py pz qw qx qy qz vx vy vz wx wy wz  */
+  const float *props;      /* [E][8][S]   inv_m invIx invIy invIz hx hy hz active(0/1); I_body diagonal,
+                                          Eq. 3; h* = half extents along body x,y,z       */
+  const float *mu;         /* [E]         static friction mu_s per env          */
+  const float *f_ext;      /* [E][6][S]   world force(3) + torque(3) applied in every substep of the
+                                          call; may be NULL                                            */
+  int32_t     *pairs;      /* [E][max_pairs]  ascending canonical pair indices (S2 output)             */
+  int32_t     *n_pairs;    /* [E]                                                                      */
+  float       *contacts;   /* [E][max_contacts][8]: nx ny nz depth px py pz tag, ordered (pair, slot);
+                              tag (int bits) = position of the pair in pairs[] (bits 0-15)
+                              | slot 0..3 (bits 16-17) | SAT axis id 0..15 (bits 20-23)                */
+  int32_t     *n_contacts; /* [E]                                                                      */
+  float       *lambda;     /* [E][max_contacts][3]  jn jt1 jt2 in contact order (S5 output)            */
+  int32_t     *cache_key;  /* [E][PC][2]  warm-start cache: canonical pair index, (axis<<8 | n_points) */
+  float       *cache_lam;  /* [E][PC][4][3] accumulated impulses of the previous substep               */
+  float       *cache_pt;   /* [E][PC][4][3] world contact points of the previous substep               */
+  int32_t     *n_cache;    /* [E]  number of valid cache pairs (0 = cold)                              */
+  uint32_t    *status;     /* [E]  JENGA_ST_* flags, OR-ed in                                          */
+  unsigned long long *counters; /* [JENGA_N_COUNTERS], may be NULL                                     */
+} jenga_buffers;
+
+/* Validates desc/buffers (sizes, alignment, device arch) and returns a host handle. */
+int jenga_world_create(const jenga_world_desc *desc, const jenga_buffers *bufs, jenga_world **out);
+
+/* S2 on the current poses: state, props -> pairs, n_pairs.  Eq. 10.
+ * Decisions are bit-exact with an fp64 evaluation of Eq. 10 on the same fp32 inputs
+ * (near-threshold tests are re-evaluated in fp64 on the device).                                      */
+int jenga_broadphase(jenga_world *w, void *cuda_stream);
+
+/* S3: state, props, pairs, n_pairs -> contacts, n_contacts.  PAPER.md:261-280.                        */
+int jenga_narrowphase(jenga_world *w, void *cuda_stream);
+
+/* S4+S5 on the velocities it is given (no predict): state(v,w), contacts, pairs [, cache] ->
+ * state(v,w), lambda.  `iters` overrides desc.pgs_iters when > 0.  Uses the warm-start cache
+ * (read only) when desc.warm_start = 1 and n_cache[env] > 0.  Eq. 13-15, Listing 1.                   */
+int jenga_pgs_solve(jenga_world *w, int iters, void *cuda_stream);
+
+/* n_steps advances of dt (each n_substeps fused substeps S1..S7), one launch; state, cache,
+ * status and counters are updated in place.                                                           */
+int jenga_step(jenga_world *w, int n_steps, void *cuda_stream);
+
+/* Replaces bufs.f_ext for subsequent calls (NULL = no external load); takes effect for launches
+ * enqueued after it returns.  Used to switch a push on and off between jenga_step calls.            */
+int jenga_set_f_ext(jenga_world *w, const float *f_ext);
+
+/* Frees the host handle (nothing on the device belongs to it). */
+int jenga_world_destroy(jenga_world *w);
+
+/* Dynamic shared memory per CTA the kernels need for this descriptor (0 if invalid). */
+size_t jenga_smem_bytes(const jenga_world_desc *desc);
+
+/* Threads per CTA (= one env) the kernels are launched with for this descriptor. */
+int jenga_block_threads(const jenga_world_desc *desc);
+
+const char *jenga_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JENGA_H_ */

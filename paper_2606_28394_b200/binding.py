@@ -1,0 +1,184 @@
+"""Thin Python binding of csrc/libjenga.so (include/jenga.h): argument marshalling only.
+
+PyTorch allocates the device buffers and supplies the stream; every step of the method
+runs inside the library's CUDA kernels.  There is no CPU fallback: if the library is
+missing or the device is not a B200-class (sm_100) GPU the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "csrc", "libjenga.so")
+_lib = None
+
+N_COUNTERS = 8
+COUNTER_NAMES = ("env_steps", "body_steps", "candidates", "colliding", "contacts", "contact_iters", "colours", "reserved")
+ST_PAIR_OVERFLOW, ST_CONTACT_OVERFLOW, ST_COLOUR_OVERFLOW, ST_NONFINITE = 1, 2, 4, 8
+AXIS_GROUND = 15
+
+
+class JengaError(RuntimeError):
+    pass
+
+
+class WorldDesc(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_envs", C.c_int32), ("n_bodies", C.c_int32), ("body_stride", C.c_int32),
+                ("dt", C.c_float), ("n_substeps", C.c_int32), ("pgs_iters", C.c_int32), ("gravity", C.c_float * 3),
+                ("restitution", C.c_float), ("aabb_margin", C.c_float), ("baumgarte_beta", C.c_float), ("slop", C.c_float),
+                ("edge_bias_rel", C.c_float), ("edge_bias_abs", C.c_float), ("par_eps", C.c_float), ("tie_eps", C.c_float),
+                ("match_tol", C.c_float), ("warm_start", C.c_int32), ("gyroscopic", C.c_int32), ("max_pairs", C.c_int32),
+                ("max_contacts", C.c_int32), ("materialise", C.c_int32), ("device", C.c_int32)]
+
+
+class Buffers(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("state", "props", "mu", "f_ext", "pairs", "n_pairs", "contacts", "n_contacts",
+                                          "lambda_", "cache_key", "cache_lam", "cache_pt", "n_cache", "status", "counters")]
+
+
+def lib():
+    """Load csrc/libjenga.so; build it first if it is absent and nvcc is here.  Raises if neither works."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            from . import build as _build
+            try:
+                _build.build()
+            except Exception as exc:  # no silent fallback
+                raise JengaError(f"libjenga.so is missing and could not be built: {exc}") from exc
+        L = C.CDLL(_LIB_PATH)
+        L.jenga_world_create.argtypes = [C.POINTER(WorldDesc), C.POINTER(Buffers), C.POINTER(C.c_void_p)]
+        L.jenga_world_destroy.argtypes = [C.c_void_p]
+        L.jenga_broadphase.argtypes = [C.c_void_p, C.c_void_p]
+        L.jenga_narrowphase.argtypes = [C.c_void_p, C.c_void_p]
+        L.jenga_pgs_solve.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.jenga_step.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.jenga_set_f_ext.argtypes = [C.c_void_p, C.c_void_p]
+        L.jenga_smem_bytes.argtypes = [C.POINTER(WorldDesc)]
+        L.jenga_smem_bytes.restype = C.c_size_t
+        L.jenga_block_threads.argtypes = [C.POINTER(WorldDesc)]
+        L.jenga_strerror.argtypes = [C.c_int]
+        L.jenga_strerror.restype = C.c_char_p
+        for f in ("jenga_world_create", "jenga_world_destroy", "jenga_broadphase", "jenga_narrowphase", "jenga_pgs_solve",
+                  "jenga_step", "jenga_set_f_ext", "jenga_block_threads"):
+            getattr(L, f).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(code: int, what: str):
+    if code != 0:
+        raise JengaError(f"{what} failed ({code}): {lib().jenga_strerror(code).decode()}")
+
+
+def make_desc(wp, materialise: bool = False, device: int = 0) -> WorldDesc:
+    """wp: any object with the fields of workloads.WorldParams."""
+    d = WorldDesc()
+    d.struct_size = C.sizeof(WorldDesc)
+    d.n_envs, d.n_bodies, d.body_stride = wp.n_envs, wp.n_bodies, wp.body_stride
+    d.dt, d.n_substeps, d.pgs_iters = wp.dt, wp.n_substeps, wp.pgs_iters
+    d.gravity[:] = list(wp.gravity)
+    d.restitution, d.aabb_margin = wp.restitution, wp.aabb_margin
+    d.baumgarte_beta, d.slop = wp.baumgarte_beta, wp.slop
+    d.edge_bias_rel, d.edge_bias_abs, d.par_eps, d.tie_eps = wp.edge_bias_rel, wp.edge_bias_abs, wp.par_eps, wp.tie_eps
+    d.match_tol, d.warm_start, d.gyroscopic = wp.match_tol, wp.warm_start, wp.gyroscopic
+    d.max_pairs, d.max_contacts = wp.max_pairs, wp.max_contacts
+    d.materialise, d.device = int(materialise), device
+    return d
+
+
+class World:
+    """Device buffers of one batch of envs plus the library handle.
+
+    state/props/mu are host arrays (numpy or torch, fp32) in the tile layout of include/jenga.h;
+    they are copied to the device once here.  All methods enqueue on torch's current stream.
+    """
+
+    def __init__(self, wp, state, props, mu, materialise: bool = False, device: int = 0):
+        if not torch.cuda.is_available():
+            raise JengaError("no CUDA device: the Jenga step has no CPU path")
+        self.wp = wp
+        self.dev = torch.device("cuda", device)
+        E, S = wp.n_envs, wp.body_stride
+        pc = wp.max_contacts // 4
+        t = lambda a, dt: torch.as_tensor(a, dtype=dt).contiguous().to(self.dev)
+        self.state = t(state, torch.float32)
+        self.props = t(props, torch.float32)
+        self.mu = t(mu, torch.float32)
+        assert self.state.shape == (E, 13, S) and self.props.shape == (E, 8, S) and self.mu.shape == (E,)
+        z = lambda shape, dt: torch.zeros(shape, dtype=dt, device=self.dev)
+        self.f_ext = None
+        self.pairs = z((E, wp.max_pairs), torch.int32)
+        self.n_pairs = z((E,), torch.int32)
+        self.contacts = z((E, wp.max_contacts, 8), torch.float32)
+        self.n_contacts = z((E,), torch.int32)
+        self.lam = z((E, wp.max_contacts, 3), torch.float32)
+        self.cache_key = z((E, pc, 2), torch.int32)
+        self.cache_lam = z((E, pc, 4, 3), torch.float32)
+        self.cache_pt = z((E, pc, 4, 3), torch.float32)
+        self.n_cache = z((E,), torch.int32)
+        self.status = z((E,), torch.int32)
+        self.counters = z((N_COUNTERS,), torch.int64)
+        self.desc = make_desc(wp, materialise, device)
+        b = Buffers()
+        b.state, b.props, b.mu, b.f_ext = self.state.data_ptr(), self.props.data_ptr(), self.mu.data_ptr(), None
+        b.pairs, b.n_pairs = self.pairs.data_ptr(), self.n_pairs.data_ptr()
+        b.contacts, b.n_contacts, b.lambda_ = self.contacts.data_ptr(), self.n_contacts.data_ptr(), self.lam.data_ptr()
+        b.cache_key, b.cache_lam, b.cache_pt = self.cache_key.data_ptr(), self.cache_lam.data_ptr(), self.cache_pt.data_ptr()
+        b.n_cache, b.status, b.counters = self.n_cache.data_ptr(), self.status.data_ptr(), self.counters.data_ptr()
+        self.bufs = b
+        self.handle = C.c_void_p()
+        _check(lib().jenga_world_create(C.byref(self.desc), C.byref(b), C.byref(self.handle)), "jenga_world_create")
+
+    # -- the C-ABI calls, same names ------------------------------------------------------
+    def _stream(self):
+        return C.c_void_p(torch.cuda.current_stream(self.dev).cuda_stream)
+
+    def jenga_broadphase(self):
+        _check(lib().jenga_broadphase(self.handle, self._stream()), "jenga_broadphase")
+
+    def jenga_narrowphase(self):
+        _check(lib().jenga_narrowphase(self.handle, self._stream()), "jenga_narrowphase")
+
+    def jenga_pgs_solve(self, iters: int = 0):
+        _check(lib().jenga_pgs_solve(self.handle, int(iters), self._stream()), "jenga_pgs_solve")
+
+    def jenga_step(self, n_steps: int = 1):
+        _check(lib().jenga_step(self.handle, int(n_steps), self._stream()), "jenga_step")
+
+    def jenga_set_f_ext(self, f_ext):
+        """f_ext: None or an [E][6][S] fp32 array/tensor (copied to the device, kept alive here)."""
+        if f_ext is None:
+            self.f_ext = None
+            _check(lib().jenga_set_f_ext(self.handle, None), "jenga_set_f_ext")
+        else:
+            self.f_ext = torch.as_tensor(f_ext, dtype=torch.float32).contiguous().to(self.dev)
+            assert self.f_ext.shape == (self.wp.n_envs, 6, self.wp.body_stride)
+            _check(lib().jenga_set_f_ext(self.handle, C.c_void_p(self.f_ext.data_ptr())), "jenga_set_f_ext")
+
+    def jenga_world_destroy(self):
+        if self.handle:
+            _check(lib().jenga_world_destroy(self.handle), "jenga_world_destroy")
+            self.handle = C.c_void_p()
+
+    broadphase, narrowphase, pgs_solve, step, set_f_ext, destroy = (
+        jenga_broadphase, jenga_narrowphase, jenga_pgs_solve, jenga_step, jenga_set_f_ext, jenga_world_destroy)
+
+    def __del__(self):
+        try:
+            self.jenga_world_destroy()
+        except Exception:
+            pass
+
+    # -- helpers ---------------------------------------------------------------------------
+    def reset_cache(self):
+        self.n_cache.zero_()
+
+    def counters_dict(self):
+        return dict(zip(COUNTER_NAMES, self.counters.tolist()))
+
+    def launch_info(self):
+        return dict(threads=lib().jenga_block_threads(C.byref(self.desc)), smem_bytes=lib().jenga_smem_bytes(C.byref(self.desc)))

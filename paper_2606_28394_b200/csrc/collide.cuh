@@ -1,0 +1,230 @@
+// collide.cuh -- per-thread narrowphase of the batched Jenga step (fp32, sm_100a).
+//
+// S3 of DESIGN.md §2: 15-axis OBB-OBB separating-axis test (§6.2) and the
+// contact manifold (§6.2.1, read as reference/incident face clipping with
+// per-point depth, DESIGN.md §3 reading A8), plus box-vs-ground-plane corners (reading A9).
+// One thread handles one candidate pair; all state is in registers / thread-local arrays.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace jenga {
+
+struct Vec3 { float x, y, z; };
+
+__device__ __forceinline__ Vec3 v3(float x, float y, float z) { Vec3 r; r.x = x; r.y = y; r.z = z; return r; }
+__device__ __forceinline__ Vec3 operator+(Vec3 a, Vec3 b) { return v3(a.x + b.x, a.y + b.y, a.z + b.z); }
+__device__ __forceinline__ Vec3 operator-(Vec3 a, Vec3 b) { return v3(a.x - b.x, a.y - b.y, a.z - b.z); }
+__device__ __forceinline__ Vec3 operator-(Vec3 a) { return v3(-a.x, -a.y, -a.z); }
+__device__ __forceinline__ Vec3 operator*(float s, Vec3 a) { return v3(s * a.x, s * a.y, s * a.z); }
+__device__ __forceinline__ float dot(Vec3 a, Vec3 b) { return fmaf(a.x, b.x, fmaf(a.y, b.y, a.z * b.z)); }
+__device__ __forceinline__ Vec3 cross(Vec3 a, Vec3 b) {
+  return v3(fmaf(a.y, b.z, -a.z * b.y), fmaf(a.z, b.x, -a.x * b.z), fmaf(a.x, b.y, -a.y * b.x));
+}
+__device__ __forceinline__ Vec3 madd(Vec3 a, float s, Vec3 b) {      // a + s b
+  return v3(fmaf(s, b.x, a.x), fmaf(s, b.y, a.y), fmaf(s, b.z, a.z));
+}
+__device__ __forceinline__ float comp(Vec3 a, int k) { return k == 0 ? a.x : (k == 1 ? a.y : a.z); }
+
+// An oriented box: centre, the three body axes in world coordinates (columns of R, Eq. 1
+// PAPER.md:147) and the half extents along them.
+struct Box {
+  Vec3 c;
+  Vec3 ax[3];
+  float he[3];
+};
+
+struct Manifold {
+  int   np;        // 0 = not colliding
+  int   axis;      // SAT axis id 0..14, 15 = ground
+  Vec3  n;         // A -> B
+  Vec3  p[4];
+  float d[4];
+};
+
+struct CollideParams {
+  float edge_bias_rel, edge_bias_abs, par_eps, tie_eps;
+};
+
+// ---------------------------------------------------------------- ground plane (reading A9)
+// Corners below z = 0 are contacts: n = +z, depth = -z, point at mid-surface (cx, cy, z/2).
+// More than four: drop the shallowest (ties: the higher corner id goes) until four remain.
+__device__ inline void collide_ground(const Box& b, Manifold& m) {
+  float cz[8]; float cx[8], cy[8];
+  unsigned ok = 0; int nq = 0;
+#pragma unroll
+  for (int id = 0; id < 8; ++id) {
+    float sx = (id & 1) ? b.he[0] : -b.he[0], sy = (id & 2) ? b.he[1] : -b.he[1], sz = (id & 4) ? b.he[2] : -b.he[2];
+    Vec3 o = madd(madd(sx * b.ax[0], sy, b.ax[1]), sz, b.ax[2]);
+    cx[id] = b.c.x + o.x; cy[id] = b.c.y + o.y; cz[id] = b.c.z + o.z;
+    if (cz[id] < 0.0f) { ok |= 1u << id; ++nq; }
+  }
+  while (nq > 4) {
+    int worst = -1; float wd = 0.0f;
+#pragma unroll
+    for (int id = 0; id < 8; ++id)
+      if ((ok >> id) & 1u) { float dd = -cz[id]; if (worst < 0 || dd <= wd) { worst = id; wd = dd; } }
+    ok &= ~(1u << worst); --nq;
+  }
+  m.np = 0; m.axis = 15; m.n = v3(0.0f, 0.0f, 1.0f);
+#pragma unroll
+  for (int id = 0; id < 8; ++id)
+    if ((ok >> id) & 1u) {
+      int k = m.np++;
+      m.p[k] = v3(cx[id], cy[id], 0.5f * cz[id]);
+      m.d[k] = -cz[id];
+    }
+}
+
+// Sutherland-Hodgman against the half-space  s * ((P - c) . axis) <= e.
+__device__ inline int clip_halfspace(const Vec3* in, int nin, Vec3* out, Vec3 c, Vec3 axis, float s, float e) {
+  int nout = 0;
+  Vec3 P = in[0];
+  float dP = e - s * dot(P - c, axis);
+  for (int i = 0; i < nin; ++i) {
+    Vec3 Q = in[(i + 1 == nin) ? 0 : i + 1];
+    float dQ = e - s * dot(Q - c, axis);
+    if (dP >= 0.0f) {
+      out[nout++] = P;
+      if (dQ < 0.0f) { float t = dP / (dP - dQ); out[nout++] = madd(P, t, Q - P); }
+    } else if (dQ >= 0.0f) {
+      float t = dP / (dP - dQ); out[nout++] = madd(P, t, Q - P);
+    }
+    P = Q; dP = dQ;
+  }
+  return nout;
+}
+
+// ---------------------------------------------------------------- box vs box
+__device__ inline void collide_boxes(const CollideParams& cp, const Box& A, const Box& B, Manifold& m) {
+  m.np = 0;
+  const Vec3 t = B.c - A.c;
+  // 15 axes: overlap delta = rA + rB - |t.L|; any delta <= 0 separates.
+  float bestF = 0.0f, bestE = 0.0f; int iF = -1, iE = -1;
+  Vec3 LF = v3(0, 0, 0), LE = v3(0, 0, 0);
+  // cij = a_i . b_j reused by the face axes
+  float c[3][3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) c[i][j] = dot(A.ax[i], B.ax[j]);
+  const float ta[3] = { dot(t, A.ax[0]), dot(t, A.ax[1]), dot(t, A.ax[2]) };
+  const float tb[3] = { dot(t, B.ax[0]), dot(t, B.ax[1]), dot(t, B.ax[2]) };
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {            // A's face axes, ids 0..2
+    float rB = B.he[0] * fabsf(c[k][0]) + B.he[1] * fabsf(c[k][1]) + B.he[2] * fabsf(c[k][2]);
+    float dl = A.he[k] + rB - fabsf(ta[k]);
+    if (dl <= 0.0f) return;
+    if (iF < 0 || dl < bestF - cp.tie_eps) { iF = k; bestF = dl; LF = A.ax[k]; }
+  }
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {            // B's face axes, ids 3..5
+    float rA = A.he[0] * fabsf(c[0][k]) + A.he[1] * fabsf(c[1][k]) + A.he[2] * fabsf(c[2][k]);
+    float dl = rA + B.he[k] - fabsf(tb[k]);
+    if (dl <= 0.0f) return;
+    if (dl < bestF - cp.tie_eps) { iF = 3 + k; bestF = dl; LF = B.ax[k]; }
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {          // edge axes a_i x b_j, ids 6..14
+      Vec3 u = cross(A.ax[i], B.ax[j]);
+      float l2 = dot(u, u);
+      if (l2 < cp.par_eps) continue;
+      float inv = 1.0f / sqrtf(l2);
+      u = inv * u;
+      float rA = A.he[0] * fabsf(dot(A.ax[0], u)) + A.he[1] * fabsf(dot(A.ax[1], u)) + A.he[2] * fabsf(dot(A.ax[2], u));
+      float rB = B.he[0] * fabsf(dot(B.ax[0], u)) + B.he[1] * fabsf(dot(B.ax[1], u)) + B.he[2] * fabsf(dot(B.ax[2], u));
+      float dl = rA + rB - fabsf(dot(t, u));
+      if (dl <= 0.0f) return;
+      if (iE < 0 || dl < bestE - cp.tie_eps) { iE = 6 + 3 * i + j; bestE = dl; LE = u; }
+    }
+  // face preference (DESIGN §3 reading A7)
+  int ax = iF; Vec3 n = LF; float delta = bestF;
+  if (iE >= 0 && bestE < cp.edge_bias_rel * bestF - cp.edge_bias_abs) { ax = iE; n = LE; delta = bestE; }
+  if (dot(n, t) < 0.0f) n = -n;
+  m.axis = ax; m.n = n;
+
+  if (ax >= 6) {                            // edge-edge: closest points of the two support edges
+    const int i = (ax - 6) / 3, j = (ax - 6) % 3;
+    Vec3 pa = A.c, pb = B.c;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      if (k != i) { float s = dot(A.ax[k], n) >= 0.0f ? 1.0f : -1.0f; pa = madd(pa, s * A.he[k], A.ax[k]); }
+      if (k != j) { float s = dot(B.ax[k], n) >= 0.0f ? 1.0f : -1.0f; pb = madd(pb, -s * B.he[k], B.ax[k]); }
+    }
+    const Vec3 ai = A.ax[i], bj = B.ax[j], r = pa - pb;
+    const float bb = dot(ai, bj), cc = dot(ai, r), ff = dot(bj, r), den = 1.0f - bb * bb;
+    float sA = (bb * ff - cc) / den, sB = (ff - bb * cc) / den;
+    sA = fminf(fmaxf(sA, -A.he[i]), A.he[i]);
+    sB = fminf(fmaxf(sB, -B.he[j]), B.he[j]);
+    m.p[0] = 0.5f * (madd(pa, sA, ai) + madd(pb, sB, bj));
+    m.d[0] = delta; m.np = 1;
+    return;
+  }
+
+  // face case: X owns the axis (reference), Y is the other (incident)
+  const bool refA = ax < 3; const int r = ax % 3;
+  const Box& X = refA ? A : B; const Box& Y = refA ? B : A;
+  const Vec3 nref = refA ? n : -n;
+  int mi = 0; float sg = -1.0f, best = 3.0e38f;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    float dk = dot(Y.ax[k], nref);
+    if (-dk < best) { best = -dk; mi = k; sg = -1.0f; }
+    if (dk < best) { best = dk; mi = k; sg = 1.0f; }
+  }
+  const int iu = (mi == 0) ? 1 : 0, iv = (mi == 2) ? 1 : 2;
+  Vec3 poly0[8], poly1[8], inc[4];
+  {
+    const Vec3 fc = madd(Y.c, sg * Y.he[mi], Y.ax[mi]);
+    const Vec3 eu = Y.he[iu] * Y.ax[iu], ev = Y.he[iv] * Y.ax[iv];
+    poly0[0] = fc - eu - ev; poly0[1] = fc + eu - ev; poly0[2] = fc + eu + ev; poly0[3] = fc - eu + ev;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) inc[k] = poly0[k];
+  }
+  const int u = (r == 0) ? 1 : 0, v = (r == 2) ? 1 : 2;
+  int np = clip_halfspace(poly0, 4, poly1, X.c, X.ax[u], 1.0f, X.he[u]);
+  if (np) np = clip_halfspace(poly1, np, poly0, X.c, X.ax[u], -1.0f, X.he[u]);
+  if (np) np = clip_halfspace(poly0, np, poly1, X.c, X.ax[v], 1.0f, X.he[v]);
+  if (np) np = clip_halfspace(poly1, np, poly0, X.c, X.ax[v], -1.0f, X.he[v]);
+  Vec3 cpt[8]; float cd[8]; int nc = 0;
+  for (int k = 0; k < np; ++k) {
+    float d = X.he[r] - dot(poly0[k] - X.c, nref);
+    if (d >= 0.0f) { cpt[nc] = madd(poly0[k], 0.5f * d, nref); cd[nc] = d; ++nc; }
+  }
+  if (nc == 0) {                            // fallback: deepest incident vertex, SAT depth
+    int bi = 0; float bd = -3.0e38f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      float d = X.he[r] - dot(inc[k] - X.c, nref);
+      if (d > bd) { bd = d; bi = k; }
+    }
+    m.p[0] = madd(inc[bi], 0.5f * delta, nref); m.d[0] = delta; m.np = 1;
+    return;
+  }
+  unsigned keep = (1u << nc) - 1u;
+  if (nc > 4) {                             // <= 4 reduction (DESIGN §2 S3)
+    int i0 = 0, i1 = -1, i2 = -1, i3 = -1; float far2 = -1.0f, amax = 0.0f, amin = 0.0f;
+    for (int k = 1; k < nc; ++k) if (cd[k] > cd[i0]) i0 = k;
+    for (int k = 0; k < nc; ++k) if (k != i0) {
+      Vec3 d = cpt[k] - cpt[i0]; float dd = dot(d, d);
+      if (dd > far2) { far2 = dd; i1 = k; }
+    }
+    const Vec3 e01 = cpt[i1] - cpt[i0];
+    for (int k = 0; k < nc; ++k) {
+      if (k == i0 || k == i1) continue;
+      float area = dot(cross(e01, cpt[k] - cpt[i0]), n);
+      if (area > amax) { amax = area; i2 = k; }
+      if (area < amin) { amin = area; i3 = k; }
+    }
+    keep = (1u << i0) | (1u << i1);
+    if (i2 >= 0) keep |= 1u << i2;
+    if (i3 >= 0) keep |= 1u << i3;
+  }
+  int no = 0;
+  for (int k = 0; k < nc; ++k) if ((keep >> k) & 1u) { m.p[no] = cpt[k]; m.d[no] = cd[k]; ++no; }
+  m.np = no;
+}
+
+}  // namespace jenga

@@ -1,0 +1,318 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by
+element on the same seeded fp32 inputs.  Tolerances are BASELINE.json north_star's:
+  broadphase pair lists bit-exact; contact normals 1e-4 rad, depths/points 1e-6 m (on decisions
+  with margin >= 1e-5 m); PGS impulses 1e-4 relative + 1e-7 N*s; single-step pose 1e-6 m / 1e-5 rad.
+"""
+import numpy as np
+import pytest
+
+from paper_2606_28394_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_PT = 1e-6          # m
+TOL_NRM = 1e-4         # rad
+TOL_LAM_REL, TOL_LAM_ABS = 1e-4, 1e-7
+TOL_POS, TOL_ANG = 1e-6, 1e-5
+MARGIN = 1e-5          # decisions closer than this to their threshold are excluded (and counted)
+
+
+@pytest.fixture(scope="module")
+def J():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2606_28394_b200 import binding
+    binding.lib()
+    return binding
+
+
+# ----------------------------------------------------------------------------- helpers
+def oracle_mid_state(orc, wl, n_steps):
+    """Advance the workload n_steps with the oracle and return it re-rounded to fp32 tiles
+    (the common input of both sides) plus the oracle's warm-start cache at that point."""
+    P = orc.make_params(wl.params)
+    bod = orc.unpack_tiles(wl.state, wl.props, wl.params.n_bodies)
+    cache = orc.Cache(bod.E, wl.params.max_contacts)
+    orc.rollout(P, bod, wl.mu.astype(np.float64), n_steps, cache=cache)
+    st = orc.pack_state(bod, wl.params.body_stride).astype(np.float32)
+    return st, cache
+
+
+def angle_between(a, b):
+    c = np.clip(np.sum(a * b, axis=-1) / (np.linalg.norm(a, axis=-1) * np.linalg.norm(b, axis=-1)), -1, 1)
+    return np.arccos(c)
+
+
+def gpu_contacts(world, e):
+    n = int(world.n_contacts[e].item())
+    c = world.contacts[e, :n].cpu().numpy()
+    tag = c[:, 7].copy().view(np.int32)
+    return dict(n=n, nrm=c[:, 0:3].astype(np.float64), depth=c[:, 3].astype(np.float64), pt=c[:, 4:7].astype(np.float64),
+                cand=tag & 0xffff, slot=(tag >> 16) & 3, axis=(tag >> 20) & 0xf)
+
+
+def load_oracle_contacts(world, e, pairs, oc):
+    """Write an oracle contact list (dict of arrays) into the GPU buffers of env e."""
+    import torch
+    n = len(oc["pair"])
+    pos = {int(p): k for k, p in enumerate(pairs)}
+    buf = np.zeros((n, 8), np.float32)
+    buf[:, 0:3] = oc["nrm"]; buf[:, 3] = oc["depth"]; buf[:, 4:7] = oc["pt"]
+    tag = np.array([pos[int(p)] | (int(s) << 16) | (int(a) << 20) for p, s, a in zip(oc["pair"], oc["slot"], oc["axis"])], np.int32)
+    buf[:, 7] = tag.view(np.float32)
+    world.pairs[e, :len(pairs)] = torch.as_tensor(np.asarray(pairs, np.int32)).to(world.dev)
+    world.n_pairs[e] = len(pairs)
+    world.contacts[e, :n] = torch.as_tensor(buf).to(world.dev)
+    world.n_contacts[e] = n
+
+
+def workloads_small():
+    out = [("cfg1", W.make_config(1), 0), ("cfg2", W.make_config(2, n_envs=6), 0),
+           ("cfg3", W.make_config(3, n_envs=4), 0), ("cfg4", W.make_config(4, n_envs=2), 0)]
+    return out
+
+
+# ----------------------------------------------------------------------------- S2 broadphase
+@pytest.mark.parametrize("steps", [0, 45])
+def test_broadphase_bit_exact(orc, J, steps):
+    """Pair lists bit-exact, no exclusions (north_star), on step-0 and mid-rollout states."""
+    import torch
+    for name, wl, _ in workloads_small() + [("cfg3b", W.make_config(3, n_envs=3, env_offset=100), 0)]:
+        if steps and name == "cfg4":
+            continue
+        state = wl.state if steps == 0 else oracle_mid_state(orc, wl, steps if name != "cfg3b" else 260)[0]
+        world = J.World(wl.params, state, wl.props, wl.mu)
+        world.broadphase(); torch.cuda.synchronize()
+        P = orc.make_params(wl.params)
+        bod = orc.unpack_tiles(state, wl.props, wl.params.n_bodies)
+        for e in range(wl.params.n_envs):
+            ref, st = orc.broadphase(P, bod, e)
+            n = int(world.n_pairs[e].item())
+            got = world.pairs[e, :n].cpu().numpy()
+            assert n == len(ref) and np.array_equal(got, ref), f"{name} env {e}: pair list differs"
+            assert int(world.status[e].item()) == st
+        world.destroy()
+
+
+def test_broadphase_threshold_cases_use_fp64(orc, J):
+    """Bodies placed so that Eq. 10's slack is within a few fp32 ulps of zero on either side."""
+    import torch
+    rng = np.random.default_rng(7)
+    bodies = []
+    for k in range(24):
+        bodies.append(dict(pos=(0.2 * k, 0.0, 0.05), size=(W.BLOCK_L, W.BLOCK_W, W.BLOCK_H), mass=W.BLOCK_MASS))
+        gap = W.BLOCK_L + 0.002 + rng.uniform(-3e-8, 3e-8)       # |dx| = ex_i + ex_j + eps +- tiny
+        yaw = rng.uniform(-1e-4, 1e-4)
+        bodies.append(dict(pos=(0.2 * k + gap, 0.0, 0.05), quat=(np.cos(yaw / 2), 0, 0, np.sin(yaw / 2)),
+                           size=(W.BLOCK_L, W.BLOCK_W, W.BLOCK_H), mass=W.BLOCK_MASS))
+    wl = W.make_custom(bodies)
+    world = J.World(wl.params, wl.state, wl.props, wl.mu)
+    world.broadphase(); torch.cuda.synchronize()
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(wl.state, wl.props, wl.params.n_bodies)
+    ref, _ = orc.broadphase(P, bod, 0)
+    got = world.pairs[0, :int(world.n_pairs[0].item())].cpu().numpy()
+    assert np.array_equal(got, ref)
+    assert 3 < len(ref) < 24 + 20          # some of the near-threshold pairs are in, some out
+
+
+def test_broadphase_overflow_truncates_lowest(orc, J):
+    import torch
+    wl = W.make_config(3, n_envs=2)
+    wl.params.max_pairs = 16
+    world = J.World(wl.params, wl.state, wl.props, wl.mu)
+    world.broadphase(); torch.cuda.synchronize()
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(wl.state, wl.props, wl.params.n_bodies)
+    for e in range(2):
+        ref, st = orc.broadphase(P, bod, e)
+        assert st & 1 and int(world.status[e].item()) & J.ST_PAIR_OVERFLOW
+        assert np.array_equal(world.pairs[e, :16].cpu().numpy(), ref) and int(world.n_pairs[e].item()) == 16
+
+
+# ----------------------------------------------------------------------------- S3 narrowphase
+def compare_contacts(orc, world, P, bod, e, pairs, stats):
+    mg = orc.OrcMargins(); mg.reset()
+    cont, st = orc.narrowphase(P, bod, pairs, e, margins=mg)
+    ref = cont.trimmed(); got = gpu_contacts(world, e)
+    m = mg.as_dict()
+    risky = min(m["sat_sign"], m["axis_choice"], m["incident"], m["clip"], m["reduce"]) < MARGIN
+    if risky:
+        # compare pair by pair, skipping pairs whose own decisions are near a threshold
+        stats["envs_near_threshold"] += 1
+    ref_pairs = ref["pair"]; got_pairs = np.asarray(pairs)[got["cand"]] if got["n"] else np.zeros(0, np.int64)
+    for p in np.union1d(np.unique(ref_pairs), np.unique(got_pairs)):
+        i, j = orc.pair_bodies(bod.B, int(p))
+        pm = orc.OrcMargins(); pm.reset()
+        if i < 0:
+            orc.collide_ground(bod.x[e, j], bod.q[e, j], bod.he[e, j], margins=pm)
+        else:
+            orc.collide_boxes(P, bod.x[e, i], bod.q[e, i], bod.he[e, i], bod.x[e, j], bod.q[e, j], bod.he[e, j], margins=pm)
+        d = pm.as_dict()
+        stats["pairs"] += 1
+        if min(d["sat_sign"], d["axis_choice"], d["incident"], d["clip"], d["reduce"]) < MARGIN:
+            stats["pairs_excluded"] += 1
+            continue
+        r = ref_pairs == p; g = got_pairs == p
+        assert r.sum() == g.sum(), f"env {e} pair {p}: {r.sum()} vs {g.sum()} contacts (margins {d})"
+        assert np.array_equal(ref["axis"][r], got["axis"][g]) and np.array_equal(ref["slot"][r], got["slot"][g])
+        assert np.all(angle_between(ref["nrm"][r], got["nrm"][g]) < TOL_NRM)
+        assert np.max(np.abs(ref["depth"][r] - got["depth"][g])) < TOL_PT, (e, p, ref["depth"][r], got["depth"][g])
+        assert np.max(np.abs(ref["pt"][r] - got["pt"][g])) < TOL_PT, (e, p)
+        stats["contacts"] += int(r.sum())
+
+
+@pytest.mark.parametrize("name,cfg,E,steps", [("cfg1", 1, 1, 30), ("cfg2", 2, 6, 40), ("cfg3", 3, 4, 200), ("cfg3late", 3, 3, 420),
+                                              ("cfg4", 4, 2, 20)])
+def test_narrowphase_matches_oracle(orc, J, name, cfg, E, steps):
+    import torch
+    wl = W.make_config(cfg, n_envs=E)
+    state, _ = oracle_mid_state(orc, wl, steps)
+    world = J.World(wl.params, state, wl.props, wl.mu)
+    world.broadphase(); world.narrowphase(); torch.cuda.synchronize()
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(state, wl.props, wl.params.n_bodies)
+    stats = dict(pairs=0, pairs_excluded=0, contacts=0, envs_near_threshold=0)
+    for e in range(E):
+        pairs, _ = orc.broadphase(P, bod, e)
+        compare_contacts(orc, world, P, bod, e, pairs, stats)
+    print(f"\n[{name}] narrowphase parity: {stats}")
+    assert stats["contacts"] > 0 and stats["pairs_excluded"] <= 0.05 * stats["pairs"] + 2
+
+
+def test_narrowphase_box_soup(orc, J):
+    """2^13 random box pairs (one pair per env, ~50 % overlapping), the stage-test soup of DESIGN §5."""
+    import torch
+    n = 8192
+    xA, qA, hA, xB, qB, hB = W.random_box_pairs(n)
+    state, props, S = W.empty_tiles(n, 2)
+    for b, (x, q, h) in enumerate(((xA, qA, hA), (xB, qB, hB))):
+        state[:, 0:3, b] = x; state[:, 3:7, b] = q
+        props[:, 0, b] = 1.0; props[:, 1:4, b] = 1.0; props[:, 4:7, b] = h; props[:, 7, b] = 1.0
+    wp = W.WorldParams(n_envs=n, n_bodies=2, body_stride=S, max_pairs=8, max_contacts=128)
+    state = state.astype(np.float32); props = props.astype(np.float32)
+    world = J.World(wp, state, props, np.full(n, 0.4, np.float32))
+    world.pairs[:, 0] = 2; world.n_pairs[:] = 1           # the body pair (0,1) has canonical index B + 0 = 2
+    world.narrowphase(); torch.cuda.synchronize()
+    P = orc.make_params(wp); bod = orc.unpack_tiles(state, props, 2)
+    nc = world.n_contacts.cpu().numpy(); cont = world.contacts.cpu().numpy()
+    n_cmp = n_excl = n_hit = 0
+    for e in range(n):
+        mg = orc.OrcMargins(); mg.reset()
+        r = orc.collide_boxes(P, bod.x[e, 0], bod.q[e, 0], bod.he[e, 0], bod.x[e, 1], bod.q[e, 1], bod.he[e, 1], margins=mg)
+        d = mg.as_dict()
+        if min(d["sat_sign"], d["axis_choice"], d["incident"], d["clip"], d["reduce"]) < MARGIN:
+            n_excl += 1
+            continue
+        n_cmp += 1
+        assert nc[e] == r["npts"], (e, nc[e], r["npts"], d)
+        if r["npts"]:
+            n_hit += 1
+            c = cont[e, :nc[e]]
+            tag = c[:, 7].copy().view(np.int32)
+            assert np.all(((tag >> 20) & 0xf) == r["axis"])
+            assert np.all(angle_between(c[:, 0:3].astype(np.float64), r["n"][None, :]) < TOL_NRM)
+            assert np.max(np.abs(c[:, 3] - r["depths"])) < TOL_PT and np.max(np.abs(c[:, 4:7] - r["pts"])) < TOL_PT
+    print(f"\n[soup] compared {n_cmp} pairs ({n_hit} colliding), excluded {n_excl} near-threshold")
+    assert n_hit > n // 5 and n_excl < 0.05 * n
+
+
+# ----------------------------------------------------------------------------- S4+S5 PGS
+@pytest.mark.parametrize("name,cfg,E,steps,warm", [("cfg1", 1, 1, 30, True), ("cfg2", 2, 6, 70, True), ("cfg2cold", 2, 3, 40, False),
+                                                   ("cfg3", 3, 4, 300, True), ("cfg4", 4, 2, 30, True)])
+def test_pgs_matches_oracle(orc, J, name, cfg, E, steps, warm):
+    """Stage isolation: both sides solve the oracle's contact list from the same velocities
+    (gravity pre-added), the same warm-start cache and the canonical colour order."""
+    import torch
+    wl = W.make_config(cfg, n_envs=E)
+    wl.params.warm_start = int(warm)
+    state, cache = oracle_mid_state(orc, wl, steps)
+    h = wl.params.dt
+    dyn = (wl.props[:, 7, :] != 0) & (wl.props[:, 0, :] != 0)
+    state[:, 9, :] += np.float32(h * wl.params.gravity[2]) * dyn           # pre-add h*g (S1)
+    world = J.World(wl.params, state, wl.props, wl.mu)
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(state, wl.props, wl.params.n_bodies)
+    if warm:
+        # the cache the GPU sees is the oracle's, rounded to fp32; the oracle re-reads the rounded values
+        cache.lam[:] = cache.lam.astype(np.float32); cache.pt[:] = cache.pt.astype(np.float32)
+        key = np.stack([cache.key_pair, cache.key_meta], axis=-1)
+        world.cache_key[:, :, :] = torch.as_tensor(key).to(world.dev)
+        world.cache_lam[:] = torch.as_tensor(cache.lam.astype(np.float32)).to(world.dev)
+        world.cache_pt[:] = torch.as_tensor(cache.pt.astype(np.float32)).to(world.dev)
+        world.n_cache[:] = torch.as_tensor(cache.n_keys).to(world.dev)
+    refs = []
+    for e in range(E):
+        pairs, _ = orc.broadphase(P, bod, e)
+        cont, _ = orc.narrowphase(P, bod, pairs, e)
+        oc = cont.trimmed()
+        for k in ("nrm", "pt", "depth"):                                   # both sides see fp32-rounded contacts
+            oc[k] = oc[k].astype(np.float32).astype(np.float64)
+        c2 = orc.Contacts.from_arrays(oc["pair"], oc["slot"], oc["axis"], oc["nrm"], oc["pt"], oc["depth"])
+        load_oracle_contacts(world, e, pairs, oc)
+        lam, col, _ = orc.solve(P, bod, c2, float(wl.mu[e]), e=e, cache=cache if warm else None)
+        refs.append(lam)
+    world.pgs_solve(); torch.cuda.synchronize()
+    gstate = world.state.cpu().numpy().astype(np.float64)
+    worst = 0.0
+    for e in range(E):
+        n = len(refs[e])
+        got = world.lam[e, :n].cpu().numpy().astype(np.float64)
+        err = np.abs(got - refs[e]); tol = TOL_LAM_REL * np.abs(refs[e]) + TOL_LAM_ABS
+        worst = max(worst, float(np.max(err / tol)) if n else 0.0)
+        assert np.all(err <= tol), f"{name} env {e}: impulse error {err.max():.3e} (worst ratio {np.max(err / tol):.2f})"
+        B = wl.params.n_bodies
+        v = np.transpose(gstate[e, 7:10, :B]); w = np.transpose(gstate[e, 10:13, :B])
+        assert np.max(np.abs(v - bod.v[e])) < 1e-6 and np.max(np.abs(w - bod.w[e])) < 1e-4
+    print(f"\n[{name}] PGS parity: worst impulse error = {worst:.3f} of tolerance")
+
+
+# ----------------------------------------------------------------------------- whole step
+@pytest.mark.parametrize("name,cfg,E,steps", [("cfg1", 1, 1, 20), ("cfg2", 2, 6, 60), ("cfg3", 3, 4, 250), ("cfg4", 4, 2, 10)])
+def test_single_step_pose(orc, J, name, cfg, E, steps):
+    """One fused jenga_step from a common fp32 state and warm-start cache vs one oracle step."""
+    import torch
+    wl = W.make_config(cfg, n_envs=E)
+    state, cache = oracle_mid_state(orc, wl, steps)
+    world = J.World(wl.params, state, wl.props, wl.mu, materialise=True)
+    cache.lam[:] = cache.lam.astype(np.float32); cache.pt[:] = cache.pt.astype(np.float32)
+    world.cache_key[:, :, :] = torch.as_tensor(np.stack([cache.key_pair, cache.key_meta], axis=-1)).to(world.dev)
+    world.cache_lam[:] = torch.as_tensor(cache.lam.astype(np.float32)).to(world.dev)
+    world.cache_pt[:] = torch.as_tensor(cache.pt.astype(np.float32)).to(world.dev)
+    world.n_cache[:] = torch.as_tensor(cache.n_keys).to(world.dev)
+    fext = wl.fext_at(steps)
+    if fext is not None:
+        world.set_f_ext(fext)
+    world.step(1); torch.cuda.synchronize()
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(state, wl.props, wl.params.n_bodies)
+    f64 = orc.unpack_fext(fext, wl.params.n_bodies)
+    g = world.state.cpu().numpy().astype(np.float64)
+    n_ok = 0
+    for e in range(E):
+        tr = orc.step_env(P, bod, float(wl.mu[e]), e=e, fext=f64, cache=cache, trace=True)
+        m = tr["margins"]
+        if min(m["aabb"], m["sat_sign"], m["axis_choice"], m["incident"], m["clip"], m["reduce"]) < MARGIN:
+            continue                                   # a discrete decision sat on its threshold: not a pose-parity case
+        n_ok += 1
+        B = wl.params.n_bodies
+        assert int(world.n_pairs[e].item()) == len(tr["pairs"]) and int(world.n_contacts[e].item()) == tr["contacts"].n
+        x = np.transpose(g[e, 0:3, :B]); q = np.transpose(g[e, 3:7, :B])
+        assert np.max(np.abs(x - bod.x[e])) < TOL_POS, f"{name} env {e}: position error {np.max(np.abs(x - bod.x[e])):.3e}"
+        ang = 2 * np.arccos(np.clip(np.abs(np.sum(q * bod.q[e], axis=1)), 0, 1))
+        assert np.max(ang) < TOL_ANG, f"{name} env {e}: orientation error {ang.max():.3e} rad"
+        assert int(world.status[e].item()) == tr["status"]
+    print(f"\n[{name}] single-step pose parity on {n_ok}/{E} envs (rest had a decision within {MARGIN} of its threshold)")
+    assert n_ok >= max(1, E // 2)
+
+
+def test_counters_and_multi_step_equivalence(J):
+    """jenga_step(n) in one launch == n launches of jenga_step(1), bit for bit; counters add up."""
+    import torch
+    wl = W.make_config(2, n_envs=5)
+    a = J.World(wl.params, wl.state, wl.props, wl.mu); b = J.World(wl.params, wl.state, wl.props, wl.mu)
+    a.step(12)
+    for _ in range(12):
+        b.step(1)
+    torch.cuda.synchronize()
+    assert torch.equal(a.state, b.state) and torch.equal(a.cache_lam, b.cache_lam)
+    ca, cb = a.counters_dict(), b.counters_dict()
+    assert ca == cb and ca["env_steps"] == 5 * 12 and ca["contacts"] > 0 and ca["contact_iters"] == 20 * ca["contacts"]
+    active = int((wl.props[:, 7, :] != 0).sum())
+    assert ca["body_steps"] == 12 * active
