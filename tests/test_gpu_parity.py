@@ -14,7 +14,15 @@ TOL_PT = 1e-6          # m
 TOL_NRM = 1e-4         # rad
 TOL_LAM_REL, TOL_LAM_ABS = 1e-4, 1e-7
 TOL_POS, TOL_ANG = 1e-6, 1e-5
-MARGIN = 1e-5          # decisions closer than this to their threshold are excluded (and counted)
+MARGIN = 1e-5          # overlap sign: north_star compares narrowphase on |penetration| >= 1e-5 m
+MARGIN_OTHER = 2e-6    # other discrete decisions (axis choice, incident face, clip in/out, >4 reduction): a few
+                       # fp32 ulps of the 0.05-0.5 m quantities they compare.  A pair is EXCUSED only if the two
+                       # sides actually disagree AND one of its decisions lies inside these bands; excused pairs
+                       # are counted and must stay a small fraction.
+
+
+def near_threshold(d):
+    return d["sat_sign"] < MARGIN or min(d["axis_choice"], d["incident"], d["clip"], d["reduce"]) < MARGIN_OTHER
 
 
 @pytest.fixture(scope="module")
@@ -42,6 +50,14 @@ def oracle_mid_state(orc, wl, n_steps):
 def angle_between(a, b):
     c = np.clip(np.sum(a * b, axis=-1) / (np.linalg.norm(a, axis=-1) * np.linalg.norm(b, axis=-1)), -1, 1)
     return np.arccos(c)
+
+
+def rotation_angle(qa, qb):
+    """angle of the relative rotation qa (x) conj(qb), from its vector part (well conditioned near 0;
+    2*acos(|qa.qb|) is not: fp32 rounding of a unit quaternion alone moves it by ~5e-4 rad)."""
+    wa, va = qa[:, 0:1], qa[:, 1:4]; wb, vb = qb[:, 0:1], qb[:, 1:4]
+    vec = -wa * vb + wb * va - np.cross(va, vb)
+    return 2 * np.arcsin(np.clip(np.linalg.norm(vec, axis=1), 0, 1))
 
 
 def gpu_contacts(world, e):
@@ -106,7 +122,7 @@ def test_broadphase_threshold_cases_use_fp64(orc, J):
         yaw = rng.uniform(-1e-4, 1e-4)
         bodies.append(dict(pos=(0.2 * k + gap, 0.0, 0.05), quat=(np.cos(yaw / 2), 0, 0, np.sin(yaw / 2)),
                            size=(W.BLOCK_L, W.BLOCK_W, W.BLOCK_H), mass=W.BLOCK_MASS))
-    wl = W.make_custom(bodies)
+    wl = W.make_custom(bodies, max_pairs=2048, max_contacts=1024)
     world = J.World(wl.params, wl.state, wl.props, wl.mu)
     world.broadphase(); torch.cuda.synchronize()
     P = orc.make_params(wl.params); bod = orc.unpack_tiles(wl.state, wl.props, wl.params.n_bodies)
@@ -130,35 +146,41 @@ def test_broadphase_overflow_truncates_lowest(orc, J):
 
 
 # ----------------------------------------------------------------------------- S3 narrowphase
+def contacts_agree(ref, r, got, g):
+    if r.sum() != g.sum():
+        return f"{r.sum()} vs {g.sum()} contacts"
+    if not (np.array_equal(ref["axis"][r], got["axis"][g]) and np.array_equal(ref["slot"][r], got["slot"][g])):
+        return "axis / slot ids differ"
+    if r.sum() == 0:
+        return None
+    if not np.all(angle_between(ref["nrm"][r], got["nrm"][g]) < TOL_NRM):
+        return "normal differs"
+    if np.max(np.abs(ref["depth"][r] - got["depth"][g])) >= TOL_PT:
+        return f"depth differs by {np.max(np.abs(ref['depth'][r] - got['depth'][g])):.2e}"
+    if np.max(np.abs(ref["pt"][r] - got["pt"][g])) >= TOL_PT:
+        return f"point differs by {np.max(np.abs(ref['pt'][r] - got['pt'][g])):.2e}"
+    return None
+
+
 def compare_contacts(orc, world, P, bod, e, pairs, stats):
-    mg = orc.OrcMargins(); mg.reset()
-    cont, st = orc.narrowphase(P, bod, pairs, e, margins=mg)
+    cont, st = orc.narrowphase(P, bod, pairs, e)
     ref = cont.trimmed(); got = gpu_contacts(world, e)
-    m = mg.as_dict()
-    risky = min(m["sat_sign"], m["axis_choice"], m["incident"], m["clip"], m["reduce"]) < MARGIN
-    if risky:
-        # compare pair by pair, skipping pairs whose own decisions are near a threshold
-        stats["envs_near_threshold"] += 1
     ref_pairs = ref["pair"]; got_pairs = np.asarray(pairs)[got["cand"]] if got["n"] else np.zeros(0, np.int64)
     for p in np.union1d(np.unique(ref_pairs), np.unique(got_pairs)):
+        stats["pairs"] += 1
+        r = ref_pairs == p; g = got_pairs == p
+        why = contacts_agree(ref, r, got, g)
+        if why is None:
+            stats["contacts"] += int(r.sum())
+            continue
         i, j = orc.pair_bodies(bod.B, int(p))
         pm = orc.OrcMargins(); pm.reset()
         if i < 0:
             orc.collide_ground(bod.x[e, j], bod.q[e, j], bod.he[e, j], margins=pm)
         else:
             orc.collide_boxes(P, bod.x[e, i], bod.q[e, i], bod.he[e, i], bod.x[e, j], bod.q[e, j], bod.he[e, j], margins=pm)
-        d = pm.as_dict()
-        stats["pairs"] += 1
-        if min(d["sat_sign"], d["axis_choice"], d["incident"], d["clip"], d["reduce"]) < MARGIN:
-            stats["pairs_excluded"] += 1
-            continue
-        r = ref_pairs == p; g = got_pairs == p
-        assert r.sum() == g.sum(), f"env {e} pair {p}: {r.sum()} vs {g.sum()} contacts (margins {d})"
-        assert np.array_equal(ref["axis"][r], got["axis"][g]) and np.array_equal(ref["slot"][r], got["slot"][g])
-        assert np.all(angle_between(ref["nrm"][r], got["nrm"][g]) < TOL_NRM)
-        assert np.max(np.abs(ref["depth"][r] - got["depth"][g])) < TOL_PT, (e, p, ref["depth"][r], got["depth"][g])
-        assert np.max(np.abs(ref["pt"][r] - got["pt"][g])) < TOL_PT, (e, p)
-        stats["contacts"] += int(r.sum())
+        assert near_threshold(pm.as_dict()), f"env {e} pair {p}: {why}; margins {pm.as_dict()}"
+        stats["pairs_excused"] += 1
 
 
 @pytest.mark.parametrize("name,cfg,E,steps", [("cfg1", 1, 1, 30), ("cfg2", 2, 6, 40), ("cfg3", 3, 4, 200), ("cfg3late", 3, 3, 420),
@@ -170,12 +192,12 @@ def test_narrowphase_matches_oracle(orc, J, name, cfg, E, steps):
     world = J.World(wl.params, state, wl.props, wl.mu)
     world.broadphase(); world.narrowphase(); torch.cuda.synchronize()
     P = orc.make_params(wl.params); bod = orc.unpack_tiles(state, wl.props, wl.params.n_bodies)
-    stats = dict(pairs=0, pairs_excluded=0, contacts=0, envs_near_threshold=0)
+    stats = dict(pairs=0, pairs_excused=0, contacts=0)
     for e in range(E):
         pairs, _ = orc.broadphase(P, bod, e)
         compare_contacts(orc, world, P, bod, e, pairs, stats)
     print(f"\n[{name}] narrowphase parity: {stats}")
-    assert stats["contacts"] > 0 and stats["pairs_excluded"] <= 0.05 * stats["pairs"] + 2
+    assert stats["contacts"] > 0 and stats["pairs_excused"] <= 0.01 * stats["pairs"] + 1
 
 
 def test_narrowphase_box_soup(orc, J):
@@ -194,25 +216,25 @@ def test_narrowphase_box_soup(orc, J):
     world.narrowphase(); torch.cuda.synchronize()
     P = orc.make_params(wp); bod = orc.unpack_tiles(state, props, 2)
     nc = world.n_contacts.cpu().numpy(); cont = world.contacts.cpu().numpy()
-    n_cmp = n_excl = n_hit = 0
+    n_cmp = n_excused = n_hit = 0
     for e in range(n):
         mg = orc.OrcMargins(); mg.reset()
         r = orc.collide_boxes(P, bod.x[e, 0], bod.q[e, 0], bod.he[e, 0], bod.x[e, 1], bod.q[e, 1], bod.he[e, 1], margins=mg)
-        d = mg.as_dict()
-        if min(d["sat_sign"], d["axis_choice"], d["incident"], d["clip"], d["reduce"]) < MARGIN:
-            n_excl += 1
+        c = cont[e, :nc[e]]
+        tag = c[:, 7].copy().view(np.int32)
+        ok = nc[e] == r["npts"]
+        if ok and r["npts"]:
+            ok = (np.all(((tag >> 20) & 0xf) == r["axis"])
+                  and np.all(angle_between(c[:, 0:3].astype(np.float64), r["n"][None, :]) < TOL_NRM)
+                  and np.max(np.abs(c[:, 3] - r["depths"])) < TOL_PT and np.max(np.abs(c[:, 4:7] - r["pts"])) < TOL_PT)
+        if not ok:
+            assert near_threshold(mg.as_dict()), (e, nc[e], r, mg.as_dict())
+            n_excused += 1
             continue
         n_cmp += 1
-        assert nc[e] == r["npts"], (e, nc[e], r["npts"], d)
-        if r["npts"]:
-            n_hit += 1
-            c = cont[e, :nc[e]]
-            tag = c[:, 7].copy().view(np.int32)
-            assert np.all(((tag >> 20) & 0xf) == r["axis"])
-            assert np.all(angle_between(c[:, 0:3].astype(np.float64), r["n"][None, :]) < TOL_NRM)
-            assert np.max(np.abs(c[:, 3] - r["depths"])) < TOL_PT and np.max(np.abs(c[:, 4:7] - r["pts"])) < TOL_PT
-    print(f"\n[soup] compared {n_cmp} pairs ({n_hit} colliding), excluded {n_excl} near-threshold")
-    assert n_hit > n // 5 and n_excl < 0.05 * n
+        n_hit += int(r["npts"] > 0)
+    print(f"\n[soup] {n_cmp} pairs agree ({n_hit} colliding), {n_excused} excused (a decision within fp32 rounding of its threshold)")
+    assert n_hit > n // 5 and n_excused < 0.01 * n
 
 
 # ----------------------------------------------------------------------------- S4+S5 PGS
@@ -287,19 +309,19 @@ def test_single_step_pose(orc, J, name, cfg, E, steps):
     n_ok = 0
     for e in range(E):
         tr = orc.step_env(P, bod, float(wl.mu[e]), e=e, fext=f64, cache=cache, trace=True)
-        m = tr["margins"]
-        if min(m["aabb"], m["sat_sign"], m["axis_choice"], m["incident"], m["clip"], m["reduce"]) < MARGIN:
-            continue                                   # a discrete decision sat on its threshold: not a pose-parity case
-        n_ok += 1
         B = wl.params.n_bodies
-        assert int(world.n_pairs[e].item()) == len(tr["pairs"]) and int(world.n_contacts[e].item()) == tr["contacts"].n
+        if int(world.n_contacts[e].item()) != tr["contacts"].n:
+            assert near_threshold(tr["margins"]), (name, e, tr["margins"])   # a manifold decision sat on its threshold
+            continue
+        n_ok += 1
+        assert int(world.n_pairs[e].item()) == len(tr["pairs"])
         x = np.transpose(g[e, 0:3, :B]); q = np.transpose(g[e, 3:7, :B])
         assert np.max(np.abs(x - bod.x[e])) < TOL_POS, f"{name} env {e}: position error {np.max(np.abs(x - bod.x[e])):.3e}"
-        ang = 2 * np.arccos(np.clip(np.abs(np.sum(q * bod.q[e], axis=1)), 0, 1))
+        ang = rotation_angle(q, bod.q[e])
         assert np.max(ang) < TOL_ANG, f"{name} env {e}: orientation error {ang.max():.3e} rad"
         assert int(world.status[e].item()) == tr["status"]
-    print(f"\n[{name}] single-step pose parity on {n_ok}/{E} envs (rest had a decision within {MARGIN} of its threshold)")
-    assert n_ok >= max(1, E // 2)
+    print(f"\n[{name}] single-step pose parity on {n_ok}/{E} envs (rest: a contact-count decision on its threshold)")
+    assert n_ok >= max(1, (3 * E) // 4)
 
 
 def test_counters_and_multi_step_equivalence(J):
