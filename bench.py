@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py -- env-steps/s of the batched Jenga step (BASELINE.json metric) on N B200s of one node.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]            # the CUDA path (libjenga.so)
+    python bench.py --impl reference [--steps K] [--warmup W]       # the fp64 oracle on the host cores
+
+Workload: BASELINE.json configs[4] ("cfg5", the throughput headline): 65,536 envs of 18-level, 54-block
+towers per GPU, mu_s round-robin, 0-12 removals, Ziglar push sweep, dt = 1/240, 20 PGS iterations, fp32;
+seeded synthetic inputs from paper_2606_28394_b200/workloads.py.  A "step" is one dt
+advance of every env of the batch through the whole hot path (S1..S7, one fused kernel).  The timed region
+starts at step 0 of the rollout (cold warm-start cache, settle window, push at steps 60-83) and covers K steps.
+Weak scaling: each rank owns its own 65,536 envs (env ids rank*E ..), no collective on the data path.
+
+One JSON line on stdout (rank 0).  See DESIGN.md §7 for the work model behind "roofline".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "env-steps/s"
+CFG = 5
+N_SM, FP32_LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 SMSPs x 32 FP32 lanes (guide: B200_PROFILING.md table)
+
+# Algorithmic FP32 thread-instructions (FMA = 1), SURVEY.md §8(d) / DESIGN.md §7
+W_ROW, W_ROW_GROUND = 87, 51                # per contact-iteration: 3 rows x (J.v 12 + clamp 5 + apply 12); ground rows touch one body
+W_SETUP = 190                               # per contact: r, basis, 3 x (2 cross + 2 I^-1 mul + k)
+W_MANIFOLD, W_MANIFOLD_GROUND = 600, 100    # per colliding pair
+W_SAT = 250                                 # per candidate pair
+W_AABB_TEST, W_AABB_BODY, W_INTEGRATE = 15, 30, 100
+
+
+def work_model(cnt: dict, n_bodies: int, iters: int) -> dict:
+    """Algorithmic FP32 thread-instructions of the launches that produced the counters `cnt`."""
+    gc, c = cnt["ground_contacts"], cnt["contacts"]
+    ground_pairs = gc / 4.0                                   # a resting block has 4 ground corners
+    tests = n_bodies * (n_bodies - 1) // 2 + n_bodies
+    parts = {
+        "pgs_rows": iters * ((c - gc) * W_ROW + gc * W_ROW_GROUND),
+        "setup": c * W_SETUP,
+        "manifold": (cnt["colliding"] - ground_pairs) * W_MANIFOLD + ground_pairs * W_MANIFOLD_GROUND,
+        "sat": cnt["candidates"] * W_SAT,
+        "broadphase": cnt["env_steps"] * (tests * W_AABB_TEST + n_bodies * W_AABB_BODY),
+        "integrate": cnt["body_steps"] * W_INTEGRATE,
+    }
+    parts["total"] = float(sum(parts.values()))
+    return parts
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, cuda_index: int, period: float = 0.1):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.mask, self.sm_max, self.power = period, [], 0, None, 0.0
+        self._halt = threading.Event()
+        self.h = None
+        try:
+            import pynvml as N
+            import torch
+            N.nvmlInit()
+            self.N = N
+            try:
+                uuid = "GPU-" + str(torch.cuda.get_device_properties(cuda_index).uuid)
+                self.h = N.nvmlDeviceGetHandleByUUID(uuid.encode() if isinstance(uuid, str) else uuid)
+            except Exception:
+                self.h = N.nvmlDeviceGetHandleByIndex(cuda_index)
+            self.sm_max = int(N.nvmlDeviceGetMaxClockInfo(self.h, N.NVML_CLOCK_SM))
+        except Exception as exc:                 # NVML missing: report that, never fake a clock
+            self.err = repr(exc)
+
+    def run(self):
+        if self.h is None:
+            return
+        N = self.N
+        while not self._halt.is_set():
+            try:
+                self.samples.append(int(N.nvmlDeviceGetClockInfo(self.h, N.NVML_CLOCK_SM)))
+                self.mask |= int(N.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                self.power = max(self.power, N.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            self._halt.wait(self.period)
+
+    def stop(self) -> dict:
+        self._halt.set()
+        if self.is_alive():
+            self.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["nvml_unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.sm_max,
+                "reasons": [n for b, n in self.REASONS.items() if self.mask & b],
+                "samples": len(self.samples), "power_w_max": round(self.power, 1)}
+
+
+def schedule(wl, n_steps: int, chunk: int):
+    """Split steps [0, n_steps) into launches: boundaries where the push switches on/off and every `chunk` steps.
+    Yields (first_step, n, push_active)."""
+    s = 0
+    while s < n_steps:
+        active = wl.push_fext is not None and wl.push_start <= s < wl.push_end
+        nxt = n_steps
+        for b in (wl.push_start, wl.push_end):
+            if s < b < nxt:
+                nxt = b
+        n = min(chunk, nxt - s)
+        yield s, n, active
+        s += n
+
+
+# ------------------------------------------------------------------------------- oracle arm (CPU)
+def oracle_sample(n_envs: int, env_offset: int = 0):
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle as O                                     # test infrastructure; allowed here (cpu_baseline / --impl reference)
+    from paper_2606_28394_b200 import workloads as W
+    wl = W.make_config(CFG, n_envs=n_envs, env_offset=env_offset)
+    P = O.make_params(wl.params)
+    bod = O.unpack_tiles(wl.state, wl.props, wl.params.n_bodies)
+    cache = O.Cache(bod.E, wl.params.max_contacts)
+    fext = O.unpack_fext(wl.push_fext, wl.params.n_bodies)
+    return O, wl, P, bod, cache, fext
+
+
+def oracle_advance(O, wl, P, bod, cache, fext, first: int, n: int):
+    """Steps [first, first+n) of the rollout with the push schedule; returns seconds."""
+    t0 = time.perf_counter()
+    mu = wl.mu.astype(np.float64)
+    for s, k, active in schedule(wl, first + n, 1 << 30):
+        if s + k <= first:
+            continue
+        lo = max(s, first)
+        O.rollout(P, bod, mu, s + k - lo, fext=fext if active else None, cache=cache)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(budget_s: float = 15.0) -> dict:
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle as O
+    cores = int(O.n_threads())
+    n_envs = max(32, 2 * cores)
+    O, wl, P, bod, cache, fext = oracle_sample(n_envs)
+    t_probe = oracle_advance(O, wl, P, bod, cache, fext, 0, 2)
+    n = int(max(4, min(wl.n_steps - 2, budget_s / max(t_probe / 2, 1e-6))))
+    t = oracle_advance(O, wl, P, bod, cache, fext, 2, n)
+    return {"value": n_envs * n / t, "unit": METRIC, "cores": cores, "kind": "oracle",
+            "sample": f"first {n_envs} envs of cfg5, steps 2..{2 + n} of the rollout (fp64, OpenMP over envs), {t:.1f} s"}
+
+
+def run_reference(args) -> dict:
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        sys.exit(0)
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle as O
+    cores = int(O.n_threads())
+    n_envs = max(32, 2 * cores)
+    O, wl, P, bod, cache, fext = oracle_sample(n_envs)
+    steps = min(args.steps, wl.n_steps - args.warmup)
+    oracle_advance(O, wl, P, bod, cache, fext, 0, args.warmup)
+    t = oracle_advance(O, wl, P, bod, cache, fext, args.warmup, steps)
+    v = n_envs * steps / t
+    sample = f"first {n_envs} envs of cfg5 per step, steps {args.warmup}..{args.warmup + steps} of the rollout (fp64 oracle, OpenMP over envs)"
+    return {"impl": "reference", "metric": METRIC, "value": v, "unit": METRIC, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "cfg5: 18-level 54-block towers, 20 PGS iters, dt=1/240 (bounded sample)", "envs_per_step": n_envs},
+            "cpu_baseline": {"value": v, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+# ------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args) -> dict:
+    import torch
+    import torch.distributed as dist
+    from paper_2606_28394_b200 import binding, shard, workloads as W
+
+    rank, world_size = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the Jenga step has no CPU path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world_size > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    binding.lib()                                            # fail loudly if libjenga.so is missing
+
+    E = args.envs
+    wl = W.make_config(CFG, n_envs=E, env_offset=shard.env_range(rank, world_size, E)[0])   # weak scaling: every rank has its own E envs
+    wp = wl.params
+    K = min(args.steps, wl.n_steps)
+    world = binding.World(wp, wl.state, wl.props, wl.mu, device=local)
+    state0 = world.state.clone()
+    fext_dev = torch.as_tensor(wl.push_fext).to(dev)
+    fext_ptr = binding.C.c_void_p(fext_dev.data_ptr())
+    L = binding.lib()
+    stream = torch.cuda.current_stream(dev)
+
+    def set_push(active: bool):
+        binding._check(L.jenga_set_f_ext(world.handle, fext_ptr if active else None), "jenga_set_f_ext")
+
+    def reset():
+        world.state.copy_(state0)
+        world.n_cache.zero_(); world.status.zero_(); world.counters.zero_()
+        set_push(False)
+
+    def barrier():
+        if world_size > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # warm-up: W untimed steps of the same launch shape, then back to step 0
+    for _ in range(max(args.warmup, 0)):
+        world.jenga_step(min(args.chunk, K))
+    reset()
+
+    # ---- device-resident timing: inputs already in HBM, CUDA events on the launching stream
+    launches = list(schedule(wl, K, args.chunk))
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(len(launches) + 1)]
+    sampler = ClockSampler(local); sampler.start()
+    barrier()
+    ev[0].record(stream)
+    for i, (s, n, active) in enumerate(launches):
+        set_push(active)
+        world.jenga_step(n)
+        ev[i + 1].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = ev[0].elapsed_time(ev[-1])
+    launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(len(launches))]
+    cnt = world.counters_dict()
+    status_or = int(np.bitwise_or.reduce(world.status.cpu().numpy()))
+    n_flagged = int((world.status != 0).sum().item())
+    assert cnt["env_steps"] == E * K, (cnt, E, K)
+
+    # ---- end to end through the C-ABI with HOST buffers: per step H2D of the state tile (pinned), step, D2H
+    reset()
+    h_a = torch.empty(world.state.shape, dtype=torch.float32, pin_memory=True)
+    h_b = torch.empty_like(h_a, pin_memory=True)
+    h_a.copy_(torch.as_tensor(wl.state))
+    h_fext = torch.as_tensor(wl.push_fext).pin_memory()
+    Ke = min(K, args.e2e_steps) if args.e2e_steps > 0 else K
+    state_bytes = h_a.numel() * 4
+    h2d = d2h = 0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    pushing = False
+    for s in range(Ke):
+        active = wl.push_start <= s < wl.push_end
+        if active and not pushing:
+            fext_dev.copy_(h_fext, non_blocking=True); h2d += h_fext.numel() * 4
+        if active != pushing:
+            set_push(active); pushing = active
+        world.jenga_step_host(h_a, h_b, 1)
+        h_a, h_b = h_b, h_a
+        h2d += state_bytes; d2h += state_bytes
+    e1.record(stream)
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+
+    ms, ms_e2e = shard.max_over_ranks(ms, dev), shard.max_over_ranks(ms_e2e, dev)
+    total_env_steps = E * K * world_size
+    value = total_env_steps / (ms * 1e-3)
+    e2e_value = E * Ke * world_size / (ms_e2e * 1e-3)
+
+    # ---- roofline of the (only) kernel, k_step: algorithmic FP32 thread-instructions / launch time vs FP32 issue peak
+    wm = work_model(cnt, wp.n_bodies, wp.pgs_iters)
+    kernel_s = sum(launch_ms) * 1e-3
+    sm_max = clocks.get("sm_max_mhz") or 1965
+    peak = N_SM * FP32_LANES_PER_SM * sm_max * 1e6 / 1e12
+    achieved = wm["total"] / kernel_s / 1e12
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "k_step_dram_bytes_per_launch.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+    out = {
+        "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world_size, "steps": K, "warmup": args.warmup,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "cfg5 (BASELINE.json configs[4]): 18-level 54-block towers, mu_s {0.25,0.40,0.60} round-robin, 0-12 removals, "
+                               "Ziglar push sweep, dt=1/240, 20 PGS iters, rollout steps 0..K",
+                   "envs_per_gpu": E, "n_bodies": wp.n_bodies, "pgs_iters": wp.pgs_iters, "steps_per_launch": args.chunk,
+                   "parallelism": f"env-sharded x{world_size}, no data-path collective",
+                   "l2": "inputs larger than L2 (state 191 MB + warm-start cache 1.7 GB per step vs 126 MB L2)"},
+        "body_steps_per_s": cnt["body_steps"] * world_size / (ms * 1e-3),
+        "contacts_per_s": cnt["contacts"] * world_size / (ms * 1e-3),
+        "contact_iters_per_s": cnt["contact_iters"] * world_size / (ms * 1e-3),
+        "contacts_per_env_step": cnt["contacts"] / cnt["env_steps"],
+        "colours_per_env_step": cnt["colours"] / cnt["env_steps"],
+        "status": {"or": status_or, "envs_flagged": n_flagged},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke},
+        "gpu_launches": len(launches),
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinstr/s (FP32 thread-instructions, FMA=1)",
+                     "frac": achieved / peak, "traffic": traffic, "kernel": "k_step", "launch_ms_avg": sum(launch_ms) / len(launch_ms),
+                     "peak_source": f"{N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x {sm_max} MHz (nominal issue rate; DESIGN.md §7)",
+                     "algorithmic_instr_per_env_step": wm["total"] / cnt["env_steps"],
+                     "shares": {k: round(v / wm["total"], 4) for k, v in wm.items() if k != "total"}},
+    }
+    if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline()
+    if world_size > 1:
+        dist.destroy_process_group()
+    return out if rank == 0 else None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=480, help="dt advances timed (default: the config's full 480-step rollout)")
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--envs", type=int, default=65536, help="envs per GPU (cfg5: 65,536)")
+    ap.add_argument("--chunk", type=int, default=12, help="dt advances per jenga_step launch")
+    ap.add_argument("--e2e-steps", type=int, default=96, help="steps of the end-to-end (host buffers) leg; 0 = K")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = min(args.steps, 60)                     # bounded: the oracle is slow by design
+        out = run_reference(args)
+    else:
+        out = run_cuda(args)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -51,7 +51,9 @@ extern "C" {
 
 /* counters[] slots (uint64, accumulated with atomics by jenga_step) */
 enum { JENGA_CNT_ENV_STEPS = 0, JENGA_CNT_BODY_STEPS, JENGA_CNT_CANDIDATES, JENGA_CNT_COLLIDING,
-       JENGA_CNT_CONTACTS, JENGA_CNT_CONTACT_ITERS, JENGA_CNT_COLOURS, JENGA_CNT_RESERVED, JENGA_N_COUNTERS };
+       JENGA_CNT_CONTACTS, JENGA_CNT_CONTACT_ITERS, JENGA_CNT_COLOURS, JENGA_CNT_GROUND_CONTACTS, JENGA_N_COUNTERS };
+/* CONTACTS counts every contact generated (ground ones included); GROUND_CONTACTS the ground-plane subset
+ * (their PGS rows touch one body, so the roofline's work model counts them separately).   */
 
 typedef struct jenga_world jenga_world;   /* opaque host-side handle; owns nothing on the device */
 
@@ -122,6 +124,13 @@ int jenga_pgs_solve(jenga_world *w, int iters, void *cuda_stream);
 /* n_steps advances of dt (each n_substeps fused substeps S1..S7), one launch; state, cache,
  * status and counters are updated in place.                                                           */
 int jenga_step(jenga_world *w, int n_steps, void *cuda_stream);
+
+/* jenga_step with HOST state buffers (the end-to-end call): enqueues, on `cuda_stream`, a host->device copy
+ * of h_state_in ([E][13][S] fp32, same layout as bufs.state; pinned memory recommended, pageable works but
+ * serialises) into bufs.state, the fused step, and a device->host copy of bufs.state into h_state_out.
+ * Either host pointer may be NULL to skip that copy.  Asynchronous like every other call: the caller
+ * synchronises the stream before reading h_state_out.  The warm-start cache stays on the device.        */
+int jenga_step_host(jenga_world *w, const float *h_state_in, float *h_state_out, int n_steps, void *cuda_stream);
 
 /* Replaces bufs.f_ext for subsequent calls (NULL = no external load); takes effect for launches
  * enqueued after it returns.  Used to switch a push on and off between jenga_step calls.            */

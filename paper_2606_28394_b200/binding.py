@@ -16,7 +16,7 @@ _LIB_PATH = os.path.join(_HERE, "csrc", "libjenga.so")
 _lib = None
 
 N_COUNTERS = 8
-COUNTER_NAMES = ("env_steps", "body_steps", "candidates", "colliding", "contacts", "contact_iters", "colours", "reserved")
+COUNTER_NAMES = ("env_steps", "body_steps", "candidates", "colliding", "contacts", "contact_iters", "colours", "ground_contacts")
 ST_PAIR_OVERFLOW, ST_CONTACT_OVERFLOW, ST_COLOUR_OVERFLOW, ST_NONFINITE = 1, 2, 4, 8
 AXIS_GROUND = 15
 
@@ -57,13 +57,14 @@ def lib():
         L.jenga_pgs_solve.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.jenga_step.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.jenga_set_f_ext.argtypes = [C.c_void_p, C.c_void_p]
+        L.jenga_step_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.jenga_smem_bytes.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_smem_bytes.restype = C.c_size_t
         L.jenga_block_threads.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_strerror.argtypes = [C.c_int]
         L.jenga_strerror.restype = C.c_char_p
         for f in ("jenga_world_create", "jenga_world_destroy", "jenga_broadphase", "jenga_narrowphase", "jenga_pgs_solve",
-                  "jenga_step", "jenga_set_f_ext", "jenga_block_threads"):
+                  "jenga_step", "jenga_step_host", "jenga_set_f_ext", "jenga_block_threads"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -149,6 +150,15 @@ class World:
     def jenga_step(self, n_steps: int = 1):
         _check(lib().jenga_step(self.handle, int(n_steps), self._stream()), "jenga_step")
 
+    def jenga_step_host(self, h_state_in, h_state_out, n_steps: int = 1):
+        """h_state_in / h_state_out: None or contiguous fp32 CPU tensors [E][13][S] (pinned for async copies)."""
+        for t in (h_state_in, h_state_out):
+            if t is not None:
+                assert t.device.type == "cpu" and t.dtype == torch.float32 and t.is_contiguous() and t.shape == self.state.shape
+        pi = C.c_void_p(h_state_in.data_ptr()) if h_state_in is not None else None
+        po = C.c_void_p(h_state_out.data_ptr()) if h_state_out is not None else None
+        _check(lib().jenga_step_host(self.handle, pi, po, int(n_steps), self._stream()), "jenga_step_host")
+
     def jenga_set_f_ext(self, f_ext):
         """f_ext: None or an [E][6][S] fp32 array/tensor (copied to the device, kept alive here)."""
         if f_ext is None:
@@ -164,8 +174,8 @@ class World:
             _check(lib().jenga_world_destroy(self.handle), "jenga_world_destroy")
             self.handle = C.c_void_p()
 
-    broadphase, narrowphase, pgs_solve, step, set_f_ext, destroy = (
-        jenga_broadphase, jenga_narrowphase, jenga_pgs_solve, jenga_step, jenga_set_f_ext, jenga_world_destroy)
+    broadphase, narrowphase, pgs_solve, step, step_host, set_f_ext, destroy = (
+        jenga_broadphase, jenga_narrowphase, jenga_pgs_solve, jenga_step, jenga_step_host, jenga_set_f_ext, jenga_world_destroy)
 
     def __del__(self):
         try:

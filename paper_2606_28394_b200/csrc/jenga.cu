@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(T, MINB) k_step(const Params P, const int n_st
   const Smem& s = cx.s; const int env = cx.env;
   const float mu = P.mu[env];
   unsigned st = 0;
-  unsigned long long c_cand = 0, c_coll = 0, c_cont = 0, c_col = 0;
+  unsigned long long c_cand = 0, c_coll = 0, c_cont = 0, c_gcont = 0, c_col = 0;
   int n_active = 0;
   if (threadIdx.x == 0) for (int b = 0; b < P.B; ++b) n_active += body_dynamic(s, P.S, b) ? 1 : 0;
   const int n_sub = n_steps * P.n_substeps;
@@ -120,18 +120,20 @@ __global__ void __launch_bounds__(T, MINB) k_step(const Params P, const int n_st
     store_cache(P, env, s, ps, have, n_coll);
     if (threadIdx.x == 0) { c_cand += n_cand; c_coll += n_coll; c_col += ncol; }
     c_cont += have ? ps.np : 0;
+    c_gcont += (have && ps.a < 0) ? ps.np : 0;
     __syncthreads();
   }
   store_tile(P.state + (size_t)env * kStateRows * P.S, s.st, kStateRows * P.S);
   flush_status(P, env, st);
   if (P.counters) {
     // contacts: warp-reduce, one atomic per warp
-    unsigned long long v = c_cont;
+    unsigned long long v = c_cont, vg = c_gcont;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    for (int o = 16; o > 0; o >>= 1) { v += __shfl_down_sync(0xffffffffu, v, o); vg += __shfl_down_sync(0xffffffffu, vg, o); }
     if ((threadIdx.x & 31) == 0 && v) {
       atomicAdd(P.counters + JENGA_CNT_CONTACTS, v);
       atomicAdd(P.counters + JENGA_CNT_CONTACT_ITERS, v * (unsigned long long)P.iters);
+      if (vg) atomicAdd(P.counters + JENGA_CNT_GROUND_CONTACTS, vg);
     }
     if (threadIdx.x == 0) {
       atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, (unsigned long long)n_steps);
@@ -382,5 +384,22 @@ extern "C" int jenga_step(jenga_world* w, int n_steps, void* stream) {
   if (!w || n_steps < 0) return JENGA_E_ARG;
   if (n_steps == 0) return JENGA_OK;
   JENGA_DISPATCH(k_step, w->threads, w->smem, (cudaStream_t)stream, w->P.E, w->P, n_steps);
+  return JENGA_OK;
+}
+
+extern "C" int jenga_step_host(jenga_world* w, const float* h_in, float* h_out, int n_steps, void* stream) {
+  if (!w || n_steps < 0) return JENGA_E_ARG;
+  const size_t bytes = (size_t)w->P.E * jenga::kStateRows * w->P.S * sizeof(float);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (h_in) {
+    cudaError_t e = cudaMemcpyAsync(w->bufs.state, h_in, bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e, "jenga_step_host H2D");
+  }
+  const int rc = jenga_step(w, n_steps, stream);
+  if (rc != JENGA_OK) return rc;
+  if (h_out) {
+    cudaError_t e = cudaMemcpyAsync(h_out, w->bufs.state, bytes, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return cuda_fail(e, "jenga_step_host D2H");
+  }
   return JENGA_OK;
 }
