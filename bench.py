@@ -145,17 +145,20 @@ def oracle_advance(O, wl, P, bod, cache, fext, first: int, n: int):
 
 
 def cpu_baseline(budget_s: float = 15.0) -> dict:
-    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload:
+    the whole 480-step rollout of the first n envs, n sized from a probe so that the run takes ~budget_s."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import oracle as O
     cores = int(O.n_threads())
-    n_envs = max(32, 2 * cores)
+    O, wl, P, bod, cache, fext = oracle_sample(2 * cores)
+    oracle_advance(O, wl, P, bod, cache, fext, 0, 2)                      # page in, spin up the OpenMP team
+    t_probe = oracle_advance(O, wl, P, bod, cache, fext, 2, 10)
+    rate = 2 * cores * 10 / t_probe                                        # env-steps/s
+    n_envs = int(min(4096, max(cores, round(budget_s * rate / wl.n_steps / cores) * cores)))
     O, wl, P, bod, cache, fext = oracle_sample(n_envs)
-    t_probe = oracle_advance(O, wl, P, bod, cache, fext, 0, 2)
-    n = int(max(4, min(wl.n_steps - 2, budget_s / max(t_probe / 2, 1e-6))))
-    t = oracle_advance(O, wl, P, bod, cache, fext, 2, n)
-    return {"value": n_envs * n / t, "unit": METRIC, "cores": cores, "kind": "oracle",
-            "sample": f"first {n_envs} envs of cfg5, steps 2..{2 + n} of the rollout (fp64, OpenMP over envs), {t:.1f} s"}
+    t = oracle_advance(O, wl, P, bod, cache, fext, 0, wl.n_steps)
+    return {"value": n_envs * wl.n_steps / t, "unit": METRIC, "cores": cores, "kind": "oracle",
+            "sample": f"first {n_envs} envs of cfg5, all {wl.n_steps} steps of the rollout (fp64, OpenMP over envs), {t:.1f} s"}
 
 
 def run_reference(args) -> dict:
@@ -282,10 +285,12 @@ def run_cuda(args) -> dict:
     sm_max = clocks.get("sm_max_mhz") or 1965
     peak = N_SM * FP32_LANES_PER_SM * sm_max * 1e6 / 1e12
     achieved = wm["total"] / kernel_s / 1e12
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "k_step_dram_bytes_per_launch.json")
+    traffic = None                                           # ncu dram__bytes per env-step (profiles/) x env-steps per launch
+    tpath = os.path.join(ROOT, "profiles", "k_step_traffic.csv")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+        import csv
+        row = next(csv.DictReader(open(tpath)))
+        traffic = float(row["dram_bytes_per_env_step"]) * cnt["env_steps"] / len(launches)
     out = {
         "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world_size, "steps": K, "warmup": args.warmup,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
