@@ -306,6 +306,8 @@ def run_cuda(args) -> dict:
         "contacts_per_env_step": cnt["contacts"] / cnt["env_steps"],
         "colours_per_env_step": cnt["colours"] / cnt["env_steps"],
         "status": {"or": status_or, "envs_flagged": n_flagged},
+        "maxima": {k: cnt[k] for k in ("max_candidates", "max_colliding", "max_colours")},
+        "capacity": {"max_pairs": wp.max_pairs, "max_contacts": wp.max_contacts, "smem_bytes_per_env": world.launch_info()["smem_bytes"]},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke},
         "gpu_launches": len(launches),

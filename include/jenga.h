@@ -51,9 +51,11 @@ extern "C" {
 
 /* counters[] slots (uint64, accumulated with atomics by jenga_step) */
 enum { JENGA_CNT_ENV_STEPS = 0, JENGA_CNT_BODY_STEPS, JENGA_CNT_CANDIDATES, JENGA_CNT_COLLIDING,
-       JENGA_CNT_CONTACTS, JENGA_CNT_CONTACT_ITERS, JENGA_CNT_COLOURS, JENGA_CNT_GROUND_CONTACTS, JENGA_N_COUNTERS };
+       JENGA_CNT_CONTACTS, JENGA_CNT_CONTACT_ITERS, JENGA_CNT_COLOURS, JENGA_CNT_GROUND_CONTACTS,
+       JENGA_CNT_MAX_CANDIDATES, JENGA_CNT_MAX_COLLIDING, JENGA_CNT_MAX_COLOURS, JENGA_CNT_RESERVED, JENGA_N_COUNTERS };
 /* CONTACTS counts every contact generated (ground ones included); GROUND_CONTACTS the ground-plane subset
- * (their PGS rows touch one body, so the roofline's work model counts them separately).   */
+ * (their PGS rows touch one body, so the roofline's work model counts them separately).
+ * MAX_* are running maxima per env and substep (capacity sizing: max_pairs, max_contacts/4, 64 colours).  */
 
 typedef struct jenga_world jenga_world;   /* opaque host-side handle; owns nothing on the device */
 

@@ -15,8 +15,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "csrc", "libjenga.so")
 _lib = None
 
-N_COUNTERS = 8
-COUNTER_NAMES = ("env_steps", "body_steps", "candidates", "colliding", "contacts", "contact_iters", "colours", "ground_contacts")
+N_COUNTERS = 12
+COUNTER_NAMES = ("env_steps", "body_steps", "candidates", "colliding", "contacts", "contact_iters", "colours", "ground_contacts",
+                 "max_candidates", "max_colliding", "max_colours", "reserved")
 ST_PAIR_OVERFLOW, ST_CONTACT_OVERFLOW, ST_COLOUR_OVERFLOW, ST_NONFINITE = 1, 2, 4, 8
 AXIS_GROUND = 15
 

@@ -96,13 +96,20 @@ __device__ inline int clip_halfspace(const Vec3* in, int nin, Vec3* out, Vec3 c,
 }
 
 // ---------------------------------------------------------------- box vs box
-__device__ inline void collide_boxes(const CollideParams& cp, const Box& A, const Box& B, Manifold& m) {
-  m.np = 0;
+struct SatResult { int axis; Vec3 n; float delta; };
+
+__device__ __forceinline__ float absdot3(const float* he, float a, float b, float c) {
+  return fmaf(he[2], fabsf(c), fmaf(he[1], fabsf(b), he[0] * fabsf(a)));
+}
+
+// 15-axis SAT: overlap delta = rA + rB - |t.L|; any delta <= 0 separates.
+// Returns false if separated; otherwise the chosen axis (face preference, DESIGN §3 R-bias),
+// the normal A -> B and the overlap on it.  Every multiply-add is an explicit fmaf so that the
+// two places that call it (colliding-pair detection, manifold pass) take identical decisions.
+__device__ __forceinline__ bool sat_boxes(const CollideParams& cp, const Box& A, const Box& B, SatResult& r) {
   const Vec3 t = B.c - A.c;
-  // 15 axes: overlap delta = rA + rB - |t.L|; any delta <= 0 separates.
   float bestF = 0.0f, bestE = 0.0f; int iF = -1, iE = -1;
   Vec3 LF = v3(0, 0, 0), LE = v3(0, 0, 0);
-  // cij = a_i . b_j reused by the face axes
   float c[3][3];
 #pragma unroll
   for (int i = 0; i < 3; ++i)
@@ -112,16 +119,16 @@ __device__ inline void collide_boxes(const CollideParams& cp, const Box& A, cons
   const float tb[3] = { dot(t, B.ax[0]), dot(t, B.ax[1]), dot(t, B.ax[2]) };
 #pragma unroll
   for (int k = 0; k < 3; ++k) {            // A's face axes, ids 0..2
-    float rB = B.he[0] * fabsf(c[k][0]) + B.he[1] * fabsf(c[k][1]) + B.he[2] * fabsf(c[k][2]);
-    float dl = A.he[k] + rB - fabsf(ta[k]);
-    if (dl <= 0.0f) return;
+    const float rB = absdot3(B.he, c[k][0], c[k][1], c[k][2]);
+    const float dl = A.he[k] + rB - fabsf(ta[k]);
+    if (dl <= 0.0f) return false;
     if (iF < 0 || dl < bestF - cp.tie_eps) { iF = k; bestF = dl; LF = A.ax[k]; }
   }
 #pragma unroll
   for (int k = 0; k < 3; ++k) {            // B's face axes, ids 3..5
-    float rA = A.he[0] * fabsf(c[0][k]) + A.he[1] * fabsf(c[1][k]) + A.he[2] * fabsf(c[2][k]);
-    float dl = rA + B.he[k] - fabsf(tb[k]);
-    if (dl <= 0.0f) return;
+    const float rA = absdot3(A.he, c[0][k], c[1][k], c[2][k]);
+    const float dl = rA + B.he[k] - fabsf(tb[k]);
+    if (dl <= 0.0f) return false;
     if (dl < bestF - cp.tie_eps) { iF = 3 + k; bestF = dl; LF = B.ax[k]; }
   }
 #pragma unroll
@@ -129,21 +136,41 @@ __device__ inline void collide_boxes(const CollideParams& cp, const Box& A, cons
 #pragma unroll
     for (int j = 0; j < 3; ++j) {          // edge axes a_i x b_j, ids 6..14
       Vec3 u = cross(A.ax[i], B.ax[j]);
-      float l2 = dot(u, u);
+      const float l2 = dot(u, u);
       if (l2 < cp.par_eps) continue;
-      float inv = 1.0f / sqrtf(l2);
+      const float inv = 1.0f / sqrtf(l2);
       u = inv * u;
-      float rA = A.he[0] * fabsf(dot(A.ax[0], u)) + A.he[1] * fabsf(dot(A.ax[1], u)) + A.he[2] * fabsf(dot(A.ax[2], u));
-      float rB = B.he[0] * fabsf(dot(B.ax[0], u)) + B.he[1] * fabsf(dot(B.ax[1], u)) + B.he[2] * fabsf(dot(B.ax[2], u));
-      float dl = rA + rB - fabsf(dot(t, u));
-      if (dl <= 0.0f) return;
+      const float rA = absdot3(A.he, dot(A.ax[0], u), dot(A.ax[1], u), dot(A.ax[2], u));
+      const float rB = absdot3(B.he, dot(B.ax[0], u), dot(B.ax[1], u), dot(B.ax[2], u));
+      const float dl = rA + rB - fabsf(dot(t, u));
+      if (dl <= 0.0f) return false;
       if (iE < 0 || dl < bestE - cp.tie_eps) { iE = 6 + 3 * i + j; bestE = dl; LE = u; }
     }
-  // face preference (DESIGN §3 reading A7)
   int ax = iF; Vec3 n = LF; float delta = bestF;
-  if (iE >= 0 && bestE < cp.edge_bias_rel * bestF - cp.edge_bias_abs) { ax = iE; n = LE; delta = bestE; }
+  if (iE >= 0 && bestE < fmaf(cp.edge_bias_rel, bestF, -cp.edge_bias_abs)) { ax = iE; n = LE; delta = bestE; }
   if (dot(n, t) < 0.0f) n = -n;
-  m.axis = ax; m.n = n;
+  r.axis = ax; r.n = n; r.delta = delta;
+  return true;
+}
+
+// Ground: colliding iff a corner lies below z = 0 (reading A9).
+__device__ __forceinline__ bool ground_hit(const Box& b) {
+  // lowest corner z = c.z - sum_k |ax_k.z| he_k  is NOT used: the per-corner sums below are the ones
+  // collide_ground evaluates, so the decision is identical.
+  bool hit = false;
+#pragma unroll
+  for (int id = 0; id < 8; ++id) {
+    const float sx = (id & 1) ? b.he[0] : -b.he[0], sy = (id & 2) ? b.he[1] : -b.he[1], sz = (id & 4) ? b.he[2] : -b.he[2];
+    const Vec3 o = madd(madd(sx * b.ax[0], sy, b.ax[1]), sz, b.ax[2]);
+    hit = hit || (b.c.z + o.z < 0.0f);
+  }
+  return hit;
+}
+
+// Contact manifold for an overlapping pair (PAPER.md:273-280 read as A8).
+__device__ inline void manifold_boxes(const Box& A, const Box& B, const SatResult& sr, Manifold& m) {
+  const int ax = sr.axis; const Vec3 n = sr.n; const float delta = sr.delta;
+  m.axis = ax; m.n = n; m.np = 0;
 
   if (ax >= 6) {                            // edge-edge: closest points of the two support edges
     const int i = (ax - 6) / 3, j = (ax - 6) % 3;
@@ -225,6 +252,11 @@ __device__ inline void collide_boxes(const CollideParams& cp, const Box& A, cons
   int no = 0;
   for (int k = 0; k < nc; ++k) if ((keep >> k) & 1u) { m.p[no] = cpt[k]; m.d[no] = cd[k]; ++no; }
   m.np = no;
+}
+
+__device__ inline void collide_boxes(const CollideParams& cp, const Box& A, const Box& B, Manifold& m) {
+  SatResult sr; m.np = 0;
+  if (sat_boxes(cp, A, B, sr)) manifold_boxes(A, B, sr, m);
 }
 
 }  // namespace jenga

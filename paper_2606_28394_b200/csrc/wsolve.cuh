@@ -1,0 +1,467 @@
+// wsolve.cuh -- colliding-pair detection, canonical colouring, contact setup, coloured PGS sweeps,
+// integration and warm-start cache for one env per warp (see wenv.cuh for the mapping).
+#pragma once
+#include "wenv.cuh"
+
+namespace jenga {
+
+__device__ __forceinline__ Box load_box(const Smem& s, int S, int b) {
+  Box X;
+  const float4 x = bd4(s, b, 0);
+  X.c = v3(x.x, x.y, x.z);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) X.ax[k] = v3(s.R[k * S + b], s.R[(3 + k) * S + b], s.R[(6 + k) * S + b]);
+  X.he[0] = s.pr[4 * S + b]; X.he[1] = s.pr[5 * S + b]; X.he[2] = s.pr[6 * S + b];
+  return X;
+}
+
+// cab word of a colliding pair: (a+1) bits 0-10 | A dynamic bit 11 | b bits 16-26 | B dynamic bit 27
+__device__ __forceinline__ unsigned pack_ab(const Smem& s, int a, int b) {
+  unsigned w = (unsigned)(a + 1) | ((unsigned)b << 16);
+  if (a >= 0 && s.bd[a * kBd + 3] != 0.0f) w |= 1u << 11;
+  if (s.bd[b * kBd + 3] != 0.0f) w |= 1u << 27;
+  return w;
+}
+__device__ __forceinline__ int ab_a(unsigned w) { return (int)(w & 0x7ffu) - 1; }
+__device__ __forceinline__ int ab_b(unsigned w) { return (int)((w >> 16) & 0x7ffu); }
+
+// S3, first half: which candidates collide (15-axis SAT / a ground corner below z = 0).  Lane k of a
+// round takes candidate base+k; the colliding ones are compacted in ascending pair index into
+// s.cpair[cur] / s.cab.  Returns the number kept (<= pc); sets CONTACT_OVERFLOW.
+__device__ inline int find_colliding(const Smem& s, const Params& P, int n_cand, int cur, unsigned* status) {
+  const int S = P.S, lane = lane_id();
+  const unsigned below = (1u << lane) - 1u;
+  int n = 0;
+  for (int base = 0; base < n_cand; base += 32) {
+    const int k = base + lane;
+    bool hit = false; int idx = 0, i = -1, j = 0;
+    if (k < n_cand) {
+      idx = s.cand[k];
+      pair_bodies(P.B, idx, i, j);
+      const Box Bj = load_box(s, S, j);
+      if (i < 0) hit = ground_hit(Bj);
+      else { const Box Bi = load_box(s, S, i); SatResult sr; hit = sat_boxes(P.cp, Bi, Bj, sr); }
+    }
+    const unsigned bal = __ballot_sync(kFull, hit);
+    const int rank = n + __popc(bal & below);
+    if (hit && rank < P.pc) { s.cpair[cur][rank] = (unsigned short)idx; s.cab[rank] = pack_ab(s, i, j); }
+    n += __popc(bal);
+  }
+  if (n > P.pc) { *status |= JENGA_ST_CONTACT_OVERFLOW; n = P.pc; }
+  __syncwarp();
+  return n;
+}
+
+// Canonical order (north_star (d), DESIGN §2 S4): visit the colliding pairs in ascending pair index;
+// colour = lowest colour not used by an earlier pair sharing a dynamic body.  Then pos[]/order[] =
+// pairs sorted by (colour, pair index) and ph[] = the phase chunks (<= 32 pairs of one colour each).
+// The walk is sequential by definition (lane 0, one 64-bit mask per body); when the colliding-pair
+// list equals the previous substep's the previous colouring is the same function of the same input
+// and is kept.
+__device__ inline void colour_pairs(const Smem& s, const Params& P, int n_coll, int cur, unsigned* status) {
+  const int lane = lane_id();
+  bool same = n_coll == s.misc[MiNprev];
+  if (same)
+    for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[cur][r] == s.cpair[cur ^ 1][r]);
+  same = __all_sync(kFull, same);
+  if (same) return;
+  for (int b = lane; b < P.B; b += 32) s.used[b] = 0ull;
+  for (int c = lane; c < kMaxColours; c += 32) s.ccount[c] = 0;
+  __syncwarp();
+  if (lane == 0) {
+    int ncol = 0; unsigned st = 0;
+    for (int r = 0; r < n_coll; ++r) {
+      const unsigned w = s.cab[r];
+      const int a = ab_a(w), b = ab_b(w);
+      unsigned long long m = 0ull;
+      if (w & (1u << 11)) m |= s.used[a];
+      if (w & (1u << 27)) m |= s.used[b];
+      int c = __ffsll((long long)~m) - 1;
+      if (c < 0) { c = kMaxColours - 1; st |= JENGA_ST_COLOUR_OVERFLOW; }
+      if (a >= 0) s.used[a] |= 1ull << c;
+      s.used[b] |= 1ull << c;
+      s.colour[r] = (unsigned char)c;
+      const int k = s.ccount[c];
+      s.wrank[r] = (unsigned short)k; s.ccount[c] = k + 1;
+      if (c + 1 > ncol) ncol = c + 1;
+    }
+    int acc = 0, nph = 0;
+    for (int c = 0; c < ncol; ++c) {
+      const int n = s.ccount[c];
+      s.cstart[c] = acc;
+      for (int off = 0; off < n; off += 32) s.ph[nph++] = (acc + off) | (min(32, n - off) << 16);
+      acc += n;
+    }
+    s.misc[MiNcol] = ncol; s.misc[MiNph] = nph;
+    if (st) *status |= st;
+  }
+  __syncwarp();
+  for (int r = lane; r < n_coll; r += 32) {
+    const int k = s.cstart[s.colour[r]] + s.wrank[r];
+    s.pos[r] = (unsigned short)k; s.order[k] = (unsigned short)r;
+  }
+  __syncwarp();
+}
+
+// ---------------------------------------------------------------- pair slots (colour-sorted solver constants)
+// float4 fields of slot k (s.slot[f * pcA + k]):
+//   0: a, b, meta = np | axis << 8 | pair index << 16 (int bits), 1/|e_k - n (n.e_k)| (tangent normalisation)
+//   1: n.x n.y n.z, Baumgarte corr = beta max(0, depth_max - slop) / (imA + imB)     (Eq. 16)
+//   2+3c: p.x p.y p.z, (1+e)/K_nn          3+3c: 1/K_t1t1, 1/K_t2t2, K_n,t1, K_n,t2
+//   4+3c: K_t1,t2, jn, jt1, jt2             (K_dd: Eq. 13, for d = n, t1, t2)
+__device__ __forceinline__ float4& slot4(const Smem& s, int f, int k) { return s.slot[f * s.pcA + k]; }
+
+struct Frame { Vec3 n, t1, t2; };
+
+// t1 = normalise(e_k - n (n.e_k)), k = x unless |n_x| > 1/sqrt(2), then y;  t2 = n x t1   (DESIGN §3 R-basis)
+__device__ __forceinline__ void tangent_raw(Vec3 n, Vec3& u) {
+  const bool usey = fabsf(n.x) > 0.70710678118654752f;
+  const float d = usey ? n.y : n.x;
+  u = v3(fmaf(-d, n.x, usey ? 0.0f : 1.0f), fmaf(-d, n.y, usey ? 1.0f : 0.0f), -d * n.z);
+}
+__device__ __forceinline__ Frame make_frame(Vec3 n, float il) {
+  Frame F; F.n = n;
+  Vec3 u; tangent_raw(n, u);
+  F.t1 = il * u;
+  F.t2 = cross(n, F.t1);
+  return F;
+}
+
+struct Body5 { float4 x, v, w, i0, i1; };     // x.w = inverse mass (0: static / inactive / ground)
+
+__device__ __forceinline__ void load_body(const Smem& s, int b, Body5& o, bool with_vel) {
+  if (b >= 0) {
+    o.x = bd4(s, b, 0); o.i0 = bd4(s, b, 3); o.i1 = bd4(s, b, 4);
+    if (with_vel) { o.v = bd4(s, b, 1); o.w = bd4(s, b, 2); }
+  } else {
+    o.x = o.v = o.w = o.i0 = o.i1 = make_float4(0, 0, 0, 0);
+  }
+}
+__device__ __forceinline__ Vec3 imul(const Body5& B, Vec3 a) {      // Iw^-1 a
+  return v3(fmaf(B.i0.z, a.z, fmaf(B.i0.y, a.y, B.i0.x * a.x)),
+            fmaf(B.i1.x, a.z, fmaf(B.i0.w, a.y, B.i0.y * a.x)),
+            fmaf(B.i1.y, a.z, fmaf(B.i1.x, a.y, B.i0.z * a.x)));
+}
+__device__ __forceinline__ Vec3 xyz(float4 v) { return v3(v.x, v.y, v.z); }
+
+// S4 for one colliding pair: writes slot k from the pair's manifold.  Warm start (DESIGN §3 R-warm): a new
+// contact inherits (jn,jt1,jt2) of the nearest not yet taken previous contact point of the same pair
+// within match_tol; slots ascending.
+__device__ inline void setup_slot(const Smem& s, const Params& P, int env, int k, int a, int b, int pair,
+                                  const Manifold& m) {
+  Body5 A, Bb; load_body(s, a, A, false); load_body(s, b, Bb, false);
+  const Vec3 n = m.n;
+  Vec3 u; tangent_raw(n, u);
+  const float il = rsqrtf(dot(u, u));
+  const Frame F = make_frame(n, il);
+  const Vec3 dir[3] = { F.n, F.t1, F.t2 };
+  const float im = A.x.w + Bb.x.w;
+  float lam[4][3]; Vec3 pt[4];
+  float dmax = 0.0f;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) { lam[c][0] = lam[c][1] = lam[c][2] = 0.0f; pt[c] = v3(0, 0, 0); }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) if (c < m.np) { pt[c] = m.p[c]; dmax = fmaxf(dmax, m.d[c]); }
+
+  if (P.warm_start) {
+    const int nk = P.n_cache[env];
+    const int* keys = P.cache_key + (size_t)env * P.pc * 2;
+    int lo = 0, hi = nk;
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (keys[2 * mid] < pair) lo = mid + 1; else hi = mid; }
+    if (lo < nk && keys[2 * lo] == pair) {
+      const int ocnt = keys[2 * lo + 1] & 0xff;
+      const float* ol = P.cache_lam + ((size_t)env * P.pc + lo) * 12;
+      const float* op = P.cache_pt + ((size_t)env * P.pc + lo) * 12;
+      Vec3 q[4]; float l[4][3];
+#pragma unroll
+      for (int o = 0; o < 4; ++o) {
+        q[o] = v3(0, 0, 0); l[o][0] = l[o][1] = l[o][2] = 0.0f;
+        if (o < ocnt) { q[o] = v3(op[3 * o], op[3 * o + 1], op[3 * o + 2]); l[o][0] = ol[3 * o]; l[o][1] = ol[3 * o + 1]; l[o][2] = ol[3 * o + 2]; }
+      }
+      unsigned taken = 0;
+      const float tol2 = P.match_tol * P.match_tol;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        if (c < m.np) {
+          int bo = -1; float bdist = tol2;
+#pragma unroll
+          for (int o = 0; o < 4; ++o)
+            if (o < ocnt && !((taken >> o) & 1u)) {
+              const Vec3 d = pt[c] - q[o]; const float dd = dot(d, d);
+              if (dd < bdist) { bdist = dd; bo = o; }
+            }
+#pragma unroll
+          for (int o = 0; o < 4; ++o)
+            if (o == bo) { taken |= 1u << o; lam[c][0] = l[o][0]; lam[c][1] = l[o][1]; lam[c][2] = l[o][2]; }
+        }
+      }
+    }
+  }
+
+  const int meta = m.np | (m.axis << 8) | (pair << 16);
+  slot4(s, 0, k) = make_float4(__int_as_float(a), __int_as_float(b), __int_as_float(meta), il);
+  slot4(s, 1, k) = make_float4(n.x, n.y, n.z, im > 0.0f ? P.beta * fmaxf(0.0f, dmax - P.slop) / im : 0.0f);
+  const float e1 = 1.0f + P.restitution;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    float ik[3] = { 0, 0, 0 }, ko[3] = { 0, 0, 0 };
+    if (c < m.np) {
+      const Vec3 rA = a >= 0 ? pt[c] - xyz(A.x) : v3(0, 0, 0), rB = pt[c] - xyz(Bb.x);
+      Vec3 uA[3], uB[3], wA[3], wB[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        uA[d] = cross(rA, dir[d]); uB[d] = cross(rB, dir[d]);
+        wA[d] = imul(A, uA[d]); wB[d] = imul(Bb, uB[d]);
+      }
+#pragma unroll
+      for (int d = 0; d < 3; ++d) ik[d] = 1.0f / (im + dot(uA[d], wA[d]) + dot(uB[d], wB[d]));
+      ik[0] *= e1;
+      ko[0] = dot(uA[0], wA[1]) + dot(uB[0], wB[1]);
+      ko[1] = dot(uA[0], wA[2]) + dot(uB[0], wB[2]);
+      ko[2] = dot(uA[1], wA[2]) + dot(uB[1], wB[2]);
+    }
+    slot4(s, 2 + 3 * c, k) = make_float4(pt[c].x, pt[c].y, pt[c].z, ik[0]);
+    slot4(s, 3 + 3 * c, k) = make_float4(ik[1], ik[2], ko[0], ko[1]);
+    slot4(s, 4 + 3 * c, k) = make_float4(ko[2], lam[c][0], lam[c][1], lam[c][2]);
+  }
+}
+
+// S3 second half + S4: lane l of a round takes colour-sorted position base+l, computes the pair's manifold
+// (same SAT code as find_colliding -> same decisions) and writes its slot.
+__device__ inline void setup_pairs(const Smem& s, const Params& P, int env, int n_coll, int cur) {
+  const int S = P.S, lane = lane_id();
+  for (int base = 0; base < n_coll; base += 32) {
+    const int k = base + lane;
+    if (k < n_coll) {
+      const int r = s.order[k];
+      const unsigned w = s.cab[r];
+      const int a = ab_a(w), b = ab_b(w);
+      Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
+      const Box Bj = load_box(s, S, b);
+      if (a < 0) collide_ground(Bj, m);
+      else { const Box Bi = load_box(s, S, a); collide_boxes(P.cp, Bi, Bj, m); }
+      setup_slot(s, P, env, k, a, b, s.cpair[cur][r], m);
+    }
+  }
+  __syncwarp();
+}
+
+// a loses the impulse, b gains it (Listing 1, PAPER.md:335-336 + the angular lines, reading A11)
+__device__ __forceinline__ void apply_impulse(Body5& A, Body5& B, Vec3 rA, Vec3 rB, Vec3 Pi) {
+  A.v.x = fmaf(-A.x.w, Pi.x, A.v.x); A.v.y = fmaf(-A.x.w, Pi.y, A.v.y); A.v.z = fmaf(-A.x.w, Pi.z, A.v.z);
+  B.v.x = fmaf(B.x.w, Pi.x, B.v.x);  B.v.y = fmaf(B.x.w, Pi.y, B.v.y);  B.v.z = fmaf(B.x.w, Pi.z, B.v.z);
+  const Vec3 cA = cross(Pi, rA), cB = cross(rB, Pi);        // -(rA x Pi), +(rB x Pi)
+  A.w.x = fmaf(A.i0.z, cA.z, fmaf(A.i0.y, cA.y, fmaf(A.i0.x, cA.x, A.w.x)));
+  A.w.y = fmaf(A.i1.x, cA.z, fmaf(A.i0.w, cA.y, fmaf(A.i0.y, cA.x, A.w.y)));
+  A.w.z = fmaf(A.i1.y, cA.z, fmaf(A.i1.x, cA.y, fmaf(A.i0.z, cA.x, A.w.z)));
+  B.w.x = fmaf(B.i0.z, cB.z, fmaf(B.i0.y, cB.y, fmaf(B.i0.x, cB.x, B.w.x)));
+  B.w.y = fmaf(B.i1.x, cB.z, fmaf(B.i0.w, cB.y, fmaf(B.i0.y, cB.x, B.w.y)));
+  B.w.z = fmaf(B.i1.y, cB.z, fmaf(B.i1.x, cB.y, fmaf(B.i0.z, cB.x, B.w.z)));
+}
+
+// One colour chunk of the warm-start application (S4) or of a Gauss-Seidel sweep (S5).  Lane l takes the pair
+// at colour-sorted position start+l: slots ascending; per contact the normal row (Eq. 14, clamp >= 0), then
+// t1, then t2 (Eq. 15, each clipped to +-mu_s jn) -- Listing 1.  The three rows of a contact
+// act on the same two bodies: the relative velocity of the contact point is read once, advanced between rows
+// with the contact-space couplings K_ij (exactly the change the applied impulse causes), and the summed
+// impulse is applied once (DESIGN §3 R-couple).  Pairs of one colour share no dynamic body.
+template <bool WARM>
+__device__ __forceinline__ void solve_chunk(const Smem& s, int start, int count, float mu) {
+  const int lane = lane_id();
+  if (lane < count) {
+    const int k = start + lane;
+    const float4 h = slot4(s, 0, k), nn = slot4(s, 1, k);
+    const int a = __float_as_int(h.x), b = __float_as_int(h.y), np = __float_as_int(h.z) & 0xff;
+    Body5 A, B; load_body(s, a, A, true); load_body(s, b, B, true);
+    const Frame F = make_frame(xyz(nn), h.w);
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+      if (c < np) {
+        const float4 p4 = slot4(s, 2 + 3 * c, k), k4 = slot4(s, 3 + 3 * c, k);
+        float4 l4 = slot4(s, 4 + 3 * c, k);
+        const Vec3 p = xyz(p4), rA = p - xyz(A.x), rB = p - xyz(B.x);
+        Vec3 Pi;
+        if (WARM) {
+          Pi = madd(madd(l4.y * F.n, l4.z, F.t1), l4.w, F.t2);
+        } else {
+          const Vec3 vr = (xyz(B.v) + cross(xyz(B.w), rB)) - (xyz(A.v) + cross(xyz(A.w), rA));
+          const float u0 = dot(vr, F.n);
+          float u1 = dot(vr, F.t1), u2 = dot(vr, F.t2);
+          const float nw = fmaxf(fmaf(-u0, p4.w, l4.y), 0.0f);
+          const float d0 = nw - l4.y;
+          u1 = fmaf(k4.z, d0, u1); u2 = fmaf(k4.w, d0, u2);
+          const float lim = mu * nw;
+          const float n1 = fminf(fmaxf(fmaf(-u1, k4.x, l4.z), -lim), lim);
+          const float d1 = n1 - l4.z;
+          u2 = fmaf(l4.x, d1, u2);
+          const float n2 = fminf(fmaxf(fmaf(-u2, k4.y, l4.w), -lim), lim);
+          const float d2 = n2 - l4.w;
+          l4.y = nw; l4.z = n1; l4.w = n2;
+          slot4(s, 4 + 3 * c, k) = l4;
+          Pi = madd(madd(d0 * F.n, d1, F.t1), d2, F.t2);
+        }
+        apply_impulse(A, B, rA, rB, Pi);
+      }
+    if (a >= 0) { bd4(s, a, 1) = A.v; bd4(s, a, 2) = A.w; }
+    bd4(s, b, 1) = B.v; bd4(s, b, 2) = B.w;
+  }
+  __syncwarp();
+}
+
+// S4 (warm-start application) + S5: the phase chunks in canonical order, `iters` sweeps.
+__device__ inline void pgs_sweeps(const Smem& s, const Params& P, int iters, float mu) {
+  const int nph = s.misc[MiNph];
+  if (P.warm_start)
+    for (int j = 0; j < nph; ++j) { const int w = s.ph[j]; solve_chunk<true>(s, w & 0xffff, w >> 16, mu); }
+  for (int it = 0; it < iters; ++it)
+    for (int j = 0; j < nph; ++j) { const int w = s.ph[j]; solve_chunk<false>(s, w & 0xffff, w >> 16, mu); }
+}
+
+// S6: x += h v (Eq. 6); q <- normalise(q + h/2 [0,w] (x) q) (Eq. 2, world-frame
+// reading A3); then Eq. 16 (reading A14) once per colliding pair, colour by colour.
+__device__ inline void integrate(const Smem& s, const Params& P, unsigned* status) {
+  const int S = P.S, lane = lane_id(); const float h = P.h;
+  for (int b = lane; b < P.B; b += 32) {
+    float4 x = bd4(s, b, 0);
+    if (x.w == 0.0f) continue;                                   // static or inactive
+    const float4 v = bd4(s, b, 1), om = bd4(s, b, 2);
+    x.x += h * v.x; x.y += h * v.y; x.z += h * v.z;
+    bd4(s, b, 0) = x;
+    const float qw = s.q[b], qx = s.q[S + b], qy = s.q[2 * S + b], qz = s.q[3 * S + b];
+    const float dw = -(om.x * qx + om.y * qy + om.z * qz);
+    const float dx = om.x * qw + om.y * qz - om.z * qy;
+    const float dy = om.y * qw + om.z * qx - om.x * qz;
+    const float dz = om.z * qw + om.x * qy - om.y * qx;
+    const float hh = 0.5f * h;
+    const float nw = qw + hh * dw, nx = qx + hh * dx, ny = qy + hh * dy, nz = qz + hh * dz;
+    const float il = 1.0f / sqrtf(nw * nw + nx * nx + ny * ny + nz * nz);
+    s.q[b] = nw * il; s.q[S + b] = nx * il; s.q[2 * S + b] = ny * il; s.q[3 * S + b] = nz * il;
+    if (!(isfinite(x.x) && isfinite(x.y) && isfinite(x.z) && isfinite(v.x) && isfinite(v.y) && isfinite(v.z)))
+      *status |= JENGA_ST_NONFINITE;
+  }
+  __syncwarp();
+  const int nph = s.misc[MiNph];
+  for (int j = 0; j < nph; ++j) {
+    const int w = s.ph[j], k = (w & 0xffff) + lane;
+    float4 nn = make_float4(0, 0, 0, 0);
+    if (lane < (w >> 16)) nn = slot4(s, 1, k);
+    if (__any_sync(kFull, nn.w > 0.0f)) {
+      if (nn.w > 0.0f) {
+        const float4 hd = slot4(s, 0, k);
+        const int a = __float_as_int(hd.x), b = __float_as_int(hd.y);
+        float4 xb = bd4(s, b, 0);
+        if (xb.w != 0.0f) {
+          const float f = xb.w * nn.w;
+          xb.x += f * nn.x; xb.y += f * nn.y; xb.z += f * nn.z;
+          bd4(s, b, 0) = xb;
+        }
+        if (a >= 0) {
+          float4 xa = bd4(s, a, 0);
+          if (xa.w != 0.0f) {
+            const float f = xa.w * nn.w;
+            xa.x -= f * nn.x; xa.y -= f * nn.y; xa.z -= f * nn.z;
+            bd4(s, a, 0) = xa;
+          }
+        }
+      }
+      __syncwarp();
+    }
+  }
+}
+
+// S7: every pair's impulses and contact points become the next substep's warm-start cache, in ascending
+// pair order (cache entry r = pair rank r).  Returns the lane's (contacts, ground contacts) for the counters.
+__device__ inline int2 store_cache(const Smem& s, const Params& P, int env, int n_coll) {
+  const int lane = lane_id();
+  int nc = 0, ng = 0;
+  for (int base = 0; base < n_coll; base += 32) {
+    const int k = base + lane;
+    if (k < n_coll) {
+      const int r = s.order[k];
+      const float4 hd = slot4(s, 0, k);
+      const int meta = __float_as_int(hd.z), np = meta & 0xff;
+      nc += np; if (__float_as_int(hd.x) < 0) ng += np;
+      int* key = P.cache_key + ((size_t)env * P.pc + r) * 2;
+      key[0] = (int)((unsigned)meta >> 16); key[1] = meta & 0xfff;
+      float* ol = P.cache_lam + ((size_t)env * P.pc + r) * 12;
+      float* op = P.cache_pt + ((size_t)env * P.pc + r) * 12;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const float4 p4 = slot4(s, 2 + 3 * c, k), l4 = slot4(s, 4 + 3 * c, k);
+        const bool on = c < np;
+        ol[3 * c] = on ? l4.y : 0.0f; ol[3 * c + 1] = on ? l4.z : 0.0f; ol[3 * c + 2] = on ? l4.w : 0.0f;
+        op[3 * c] = p4.x; op[3 * c + 1] = p4.y; op[3 * c + 2] = p4.z;
+      }
+    }
+  }
+  if (lane == 0) P.n_cache[env] = n_coll;
+  __syncwarp();
+  return make_int2(nc, ng);
+}
+
+// ---------------------------------------------------------------- materialised outputs (stage calls / parity)
+__device__ inline void write_pairs(const Smem& s, const Params& P, int env, int n_cand) {
+  int* out = P.pairs + (size_t)env * P.max_pairs;
+  for (int k = lane_id(); k < n_cand; k += 32) out[k] = s.cand[k];
+  if (lane_id() == 0) P.n_pairs[env] = n_cand;
+}
+
+__device__ __forceinline__ int warp_excl_scan(int v, int* total) {
+  const int lane = lane_id();
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += t; }
+  *total = __shfl_sync(kFull, inc, 31);
+  return inc - v;
+}
+
+// Contact list in (pair, slot) order: the manifolds are recomputed from the (unchanged) poses in ascending
+// pair order, so nothing has to be kept on chip for the debug output.  Leaves s.wrank[r] = contact offset.
+__device__ inline int write_contacts(const Smem& s, const Params& P, int env, int n_cand, int n_coll, int cur) {
+  const int S = P.S, lane = lane_id();
+  int off0 = 0;
+  for (int base = 0; base < n_coll; base += 32) {
+    const int r = base + lane;
+    Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
+    int idx = 0;
+    if (r < n_coll) {
+      const unsigned w = s.cab[r];
+      const int a = ab_a(w), b = ab_b(w);
+      idx = s.cpair[cur][r];
+      const Box Bj = load_box(s, S, b);
+      if (a < 0) collide_ground(Bj, m);
+      else { const Box Bi = load_box(s, S, a); collide_boxes(P.cp, Bi, Bj, m); }
+    }
+    int tot; const int off = off0 + warp_excl_scan(m.np, &tot);
+    if (r < n_coll) {
+      s.wrank[r] = (unsigned short)off;
+      int lo = 0, hi = n_cand;                                   // position of the pair in the candidate list
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if (s.cand[mid] < idx) lo = mid + 1; else hi = mid; }
+      float4* out = reinterpret_cast<float4*>(P.contacts + ((size_t)env * P.max_contacts + off) * 8);
+      for (int c = 0; c < m.np; ++c) {
+        const int tag = (lo & 0xffff) | (c << 16) | (m.axis << 20);
+        out[2 * c] = make_float4(m.n.x, m.n.y, m.n.z, m.d[c]);
+        out[2 * c + 1] = make_float4(m.p[c].x, m.p[c].y, m.p[c].z, __int_as_float(tag));
+      }
+    }
+    off0 += tot;
+  }
+  if (lane == 0) P.n_contacts[env] = off0;
+  __syncwarp();
+  return off0;
+}
+
+// lambda in contact order; needs s.wrank[r] = contact offset of pair r.
+__device__ inline void write_lambda(const Smem& s, const Params& P, int env, int n_coll) {
+  for (int r = lane_id(); r < n_coll; r += 32) {
+    const int k = s.pos[r];
+    const int np = __float_as_int(slot4(s, 0, k).z) & 0xff;
+    float* out = P.lambda + ((size_t)env * P.max_contacts + s.wrank[r]) * 3;
+    for (int c = 0; c < np; ++c) {
+      const float4 l4 = slot4(s, 4 + 3 * c, k);
+      out[3 * c] = l4.y; out[3 * c + 1] = l4.z; out[3 * c + 2] = l4.w;
+    }
+  }
+}
+
+}  // namespace jenga
