@@ -203,6 +203,10 @@ def run_cuda(args) -> dict:
     E = args.envs
     wl = W.make_config(CFG, n_envs=E, env_offset=shard.env_range(rank, world_size, E)[0])   # weak scaling: every rank has its own E envs
     wp = wl.params
+    if args.max_contacts:
+        wp.max_contacts = args.max_contacts
+    if args.max_pairs:
+        wp.max_pairs = args.max_pairs
     K = min(args.steps, wl.n_steps)
     world = binding.World(wp, wl.state, wl.props, wl.mu, device=local)
     state0 = world.state.clone()
@@ -334,6 +338,8 @@ def main():
     ap.add_argument("--chunk", type=int, default=12, help="dt advances per jenga_step launch")
     ap.add_argument("--e2e-steps", type=int, default=96, help="steps of the end-to-end (host buffers) leg; 0 = K")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--max-contacts", type=int, default=0, help="override the workload's contact capacity per env")
+    ap.add_argument("--max-pairs", type=int, default=0, help="override the workload's candidate capacity per env")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = min(args.steps, 60)                     # bounded: the oracle is slow by design

@@ -25,8 +25,7 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
 
 // ---------------------------------------------------------------- fused step
 __global__ void __launch_bounds__(32) k_step(const Params P, const int n_steps) {
-  extern __shared__ __align__(16) float smem_base[];
-  const Smem s = carve(smem_base, P.S, P.max_pairs, P.pc);
+  const Smem s = carve(P.S, P.max_pairs, P.pc);
   const int env = blockIdx.x, lane = lane_id();
   load_env(s, P, env);
   if (lane == 0) { s.misc[MiNprev] = -1; s.misc[MiNph] = 0; s.misc[MiNcol] = 0; }
@@ -84,8 +83,7 @@ __global__ void __launch_bounds__(32) k_step(const Params P, const int n_steps) 
 
 // ---------------------------------------------------------------- stage kernels
 __global__ void __launch_bounds__(32) k_broadphase(const Params P) {
-  extern __shared__ __align__(16) float smem_base[];
-  const Smem s = carve(smem_base, P.S, P.max_pairs, P.pc);
+  const Smem s = carve(P.S, P.max_pairs, P.pc);
   const int env = blockIdx.x;
   unsigned st = 0;
   load_env(s, P, env);
@@ -104,8 +102,7 @@ __device__ inline int load_candidates(const Smem& s, const Params& P, int env) {
 }
 
 __global__ void __launch_bounds__(32) k_narrowphase(const Params P) {
-  extern __shared__ __align__(16) float smem_base[];
-  const Smem s = carve(smem_base, P.S, P.max_pairs, P.pc);
+  const Smem s = carve(P.S, P.max_pairs, P.pc);
   const int env = blockIdx.x;
   unsigned st = 0;
   load_env(s, P, env);
@@ -143,8 +140,7 @@ __device__ inline int pairs_from_contacts(const Smem& s, const Params& P, int en
 }
 
 __global__ void __launch_bounds__(32) k_pgs(const Params P, const int iters) {
-  extern __shared__ __align__(16) float smem_base[];
-  const Smem s = carve(smem_base, P.S, P.max_pairs, P.pc);
+  const Smem s = carve(P.S, P.max_pairs, P.pc);
   const int env = blockIdx.x, lane = lane_id();
   unsigned st = 0;
   load_env(s, P, env);
@@ -153,7 +149,7 @@ __global__ void __launch_bounds__(32) k_pgs(const Params P, const int iters) {
   const int n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
   const int n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
   // contact offsets survive the colouring (which reuses s.wrank) in the previous-list buffer, free in this kernel
-  unsigned short* keep = s.cpair[1];
+  const SP<unsigned short> keep = s.cpair[1];
   for (int r = lane; r < n_coll; r += 32) keep[r] = s.wrank[r];
   __syncwarp();
   colour_pairs(s, P, n_coll, 0, &st);

@@ -38,25 +38,35 @@ struct Params {
   unsigned* status; unsigned long long* counters;
 };
 
+// Every shared array is addressed as an offset into the one extern shared array, so that the compiler knows the
+// address space (LDS/STS with 32-bit addresses; pointers carried in a struct degrade to generic LD/ST).
+extern __shared__ __align__(16) float smem_f[];
+template <typename T> struct SP {
+  int off;                                                   // in 4-byte words
+  __device__ __forceinline__ T* ptr() const { return reinterpret_cast<T*>(smem_f + off); }
+  __device__ __forceinline__ T& operator[](int i) const { return reinterpret_cast<T*>(smem_f + off)[i]; }
+  __device__ __forceinline__ T* operator+(int i) const { return reinterpret_cast<T*>(smem_f + off) + i; }
+};
+
 struct Smem {
-  float4* slot;               // [kSlotF4][pcA]
-  float*  bd;                 // [S][kBd]
-  float*  q;                  // [4][S]
-  float*  pr;                 // [8][S]  inv_m invIx invIy invIz hx hy hz active
-  float*  R;                  // [9][S]  element (r,c) at R[(3r+c)*S + b]
-  float*  ext;                // [3][S]
-  unsigned long long* used;   // [S] colour masks per body
-  unsigned* cab;              // [pcA] (a+1) | b << 16 of colliding pair r (ascending pair order)
-  unsigned short* cand;       // [mpA] candidate pair indices, ascending
-  unsigned short* cpair[2];   // [pcA] colliding pair indices: [cur], [prev]
-  unsigned short* pos;        // [pcA] colour-sorted position of pair r
-  unsigned short* order;      // [pcA] pair r at colour-sorted position k
-  unsigned short* wrank;      // [pcA] rank inside its colour / contact offset
-  unsigned char* colour;      // [pcA]
-  int* ph;                    // [kMaxColours + pcA/32 + 2] phase chunks: start | count << 16
-  int* ccount;                // [64]
-  int* cstart;                // [64]
-  int* misc;                  // [16]
+  SP<float4> slot;              // [kSlotF4][pcA]
+  SP<float> bd;                // [S][kBd]
+  SP<float> q;                  // [4][S]
+  SP<float> pr;                // [8][S]  inv_m invIx invIy invIz hx hy hz active
+  SP<float> R;                  // [9][S]  element (r,c) at R[(3r+c)*S + b]
+  SP<float> ext;               // [3][S]
+  SP<unsigned long long> used;  // [S] colour masks per body
+  SP<unsigned> cab;             // [pcA] (a+1) | b << 16 of colliding pair r (ascending pair order)
+  SP<unsigned short> cand;      // [mpA] candidate pair indices, ascending
+  SP<unsigned short> cpair[2];  // [pcA] colliding pair indices: [cur], [prev]
+  SP<unsigned short> pos;       // [pcA] colour-sorted position of pair r
+  SP<unsigned short> order;     // [pcA] pair r at colour-sorted position k
+  SP<unsigned short> wrank;     // [pcA] rank inside its colour / contact offset
+  SP<unsigned char> colour;     // [pcA]
+  SP<int> ph;                   // [kMaxColours + pcA/32 + 2] phase chunks: start | count << 16
+  SP<int> ccount;               // [64]
+  SP<int> cstart;               // [64]
+  SP<int> misc;                 // [16]
   int pcA;
 };
 
@@ -64,12 +74,19 @@ enum { MiNph = 0, MiNcol = 1, MiNprev = 2, MiCur = 3 };
 
 __host__ __device__ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
+// The slot region is dead between S7 of one substep and the setup pass of the next, which is when the candidate
+// list (S2 -> first half of S3) and the colouring masks (S4) live: they alias it.
+__host__ __device__ inline int slot_region_words(int S, int max_pairs, int pc) {
+  const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8);
+  const int a = kSlotF4 * 4 * pcA, b = mpA / 2 + 2 * S;
+  return round_up(a > b ? a : b, 4);
+}
+
 __host__ __device__ inline size_t smem_words(int S, int max_pairs, int pc) {
-  const int pcA = round_up(pc, 32), mpA = round_up(max_pairs, 8);
-  size_t w = (size_t)kSlotF4 * 4 * pcA;
-  w += (size_t)(kBd + 4 + 8 + 9 + 3 + 2) * S;
+  const int pcA = round_up(pc, 8);
+  size_t w = slot_region_words(S, max_pairs, pc);
+  w += (size_t)(kBd + 4 + 8 + 9 + 3) * S;
   w += pcA;                        // cab
-  w += mpA / 2;                    // cand (u16)
   w += 5 * (size_t)(pcA / 2);      // cpair x2, pos, order, wrank (u16)
   w += pcA / 4;                    // colour (u8)
   w += kMaxColours + pcA / 32 + 4; // ph
@@ -77,36 +94,35 @@ __host__ __device__ inline size_t smem_words(int S, int max_pairs, int pc) {
   return round_up((int)w, 4);
 }
 
-__device__ inline Smem carve(float* base, int S, int max_pairs, int pc) {
+__device__ inline Smem carve(int S, int max_pairs, int pc) {
   Smem s;
-  const int pcA = round_up(pc, 32), mpA = round_up(max_pairs, 8);
+  const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8);
   s.pcA = pcA;
-  float* p = base;
-  s.slot = reinterpret_cast<float4*>(p); p += (size_t)kSlotF4 * 4 * pcA;
-  s.bd = p;  p += kBd * S;
-  s.q = p;   p += 4 * S;
-  s.pr = p;  p += 8 * S;
-  s.R = p;   p += 9 * S;
-  s.ext = p; p += 3 * S;
-  s.used = reinterpret_cast<unsigned long long*>(p); p += 2 * S;
-  s.cab = reinterpret_cast<unsigned*>(p); p += pcA;
-  s.cand = reinterpret_cast<unsigned short*>(p); p += mpA / 2;
-  s.cpair[0] = reinterpret_cast<unsigned short*>(p); p += pcA / 2;
-  s.cpair[1] = reinterpret_cast<unsigned short*>(p); p += pcA / 2;
-  s.pos = reinterpret_cast<unsigned short*>(p); p += pcA / 2;
-  s.order = reinterpret_cast<unsigned short*>(p); p += pcA / 2;
-  s.wrank = reinterpret_cast<unsigned short*>(p); p += pcA / 2;
-  s.colour = reinterpret_cast<unsigned char*>(p); p += pcA / 4;
-  s.ph = reinterpret_cast<int*>(p); p += kMaxColours + pcA / 32 + 4;
-  s.ccount = reinterpret_cast<int*>(p); p += kMaxColours;
-  s.cstart = reinterpret_cast<int*>(p); p += kMaxColours;
-  s.misc = reinterpret_cast<int*>(p);
+  int p = 0;
+  s.slot.off = 0; s.cand.off = 0; s.used.off = mpA / 2;
+  p += slot_region_words(S, max_pairs, pc);
+  s.bd.off = p;  p += kBd * S;
+  s.q.off = p;   p += 4 * S;
+  s.pr.off = p;  p += 8 * S;
+  s.R.off = p;   p += 9 * S;
+  s.ext.off = p; p += 3 * S;
+  s.cab.off = p; p += pcA;
+  s.cpair[0].off = p; p += pcA / 2;
+  s.cpair[1].off = p; p += pcA / 2;
+  s.pos.off = p; p += pcA / 2;
+  s.order.off = p; p += pcA / 2;
+  s.wrank.off = p; p += pcA / 2;
+  s.colour.off = p; p += pcA / 4;
+  s.ph.off = p; p += kMaxColours + pcA / 32 + 4;
+  s.ccount.off = p; p += kMaxColours;
+  s.cstart.off = p; p += kMaxColours;
+  s.misc.off = p;
   return s;
 }
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
 
-__device__ __forceinline__ float4& bd4(const Smem& s, int b, int k) { return reinterpret_cast<float4*>(s.bd + b * kBd)[k]; }
+__device__ __forceinline__ float4& bd4(const Smem& s, int b, int k) { return reinterpret_cast<float4*>(smem_f + s.bd.off + b * kBd)[k]; }
 
 __device__ __forceinline__ bool body_dynamic(const Smem& s, int S, int b) {
   return s.pr[7 * S + b] != 0.0f && s.pr[b] != 0.0f;
@@ -130,7 +146,7 @@ __device__ inline void load_env(const Smem& s, const Params& P, int env) {
     }
   }
   const float4* p4 = reinterpret_cast<const float4*>(P.props + (size_t)env * kPropRows * S);
-  float4* d4 = reinterpret_cast<float4*>(s.pr);
+  float4* d4 = reinterpret_cast<float4*>(s.pr.ptr());
   for (int i = lane; i < kPropRows * S / 4; i += 32) d4[i] = p4[i];
   __syncwarp();
   for (int b = lane; b < S; b += 32) {

@@ -284,7 +284,11 @@ __device__ __forceinline__ void solve_chunk(const Smem& s, int start, int count,
         if (WARM) {
           Pi = madd(madd(l4.y * F.n, l4.z, F.t1), l4.w, F.t2);
         } else {
-          const Vec3 vr = (xyz(B.v) + cross(xyz(B.w), rB)) - (xyz(A.v) + cross(xyz(A.w), rA));
+          // vr = (vB + wB x rB) - (vA + wA x rA), each component one subtraction and four fused multiply-adds
+          const Vec3 vr = v3(
+            fmaf(A.w.z, rA.y, fmaf(-A.w.y, rA.z, fmaf(-B.w.z, rB.y, fmaf(B.w.y, rB.z, B.v.x - A.v.x)))),
+            fmaf(A.w.x, rA.z, fmaf(-A.w.z, rA.x, fmaf(-B.w.x, rB.z, fmaf(B.w.z, rB.x, B.v.y - A.v.y)))),
+            fmaf(A.w.y, rA.x, fmaf(-A.w.x, rA.y, fmaf(-B.w.y, rB.x, fmaf(B.w.x, rB.y, B.v.z - A.v.z)))));
           const float u0 = dot(vr, F.n);
           float u1 = dot(vr, F.t1), u2 = dot(vr, F.t2);
           const float nw = fmaxf(fmaf(-u0, p4.w, l4.y), 0.0f);
@@ -404,6 +408,7 @@ __device__ inline void write_pairs(const Smem& s, const Params& P, int env, int 
   int* out = P.pairs + (size_t)env * P.max_pairs;
   for (int k = lane_id(); k < n_cand; k += 32) out[k] = s.cand[k];
   if (lane_id() == 0) P.n_pairs[env] = n_cand;
+  __syncwarp();
 }
 
 __device__ __forceinline__ int warp_excl_scan(int v, int* total) {
@@ -435,8 +440,9 @@ __device__ inline int write_contacts(const Smem& s, const Params& P, int env, in
     int tot; const int off = off0 + warp_excl_scan(m.np, &tot);
     if (r < n_coll) {
       s.wrank[r] = (unsigned short)off;
-      int lo = 0, hi = n_cand;                                   // position of the pair in the candidate list
-      while (lo < hi) { const int mid = (lo + hi) >> 1; if (s.cand[mid] < idx) lo = mid + 1; else hi = mid; }
+      const int* gp = P.pairs + (size_t)env * P.max_pairs;      // position of the pair in the candidate list (the
+      int lo = 0, hi = n_cand;                                   // on-chip copy may already be overwritten by the slots)
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if (gp[mid] < idx) lo = mid + 1; else hi = mid; }
       float4* out = reinterpret_cast<float4*>(P.contacts + ((size_t)env * P.max_contacts + off) * 8);
       for (int c = 0; c < m.np; ++c) {
         const int tag = (lo & 0xffff) | (c << 16) | (m.axis << 20);

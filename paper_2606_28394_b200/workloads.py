@@ -223,8 +223,8 @@ def make_tower(cfg: int, n_envs: Optional[int] = None, env_offset: int = 0, jitt
             fext[e, 0:3, b] = F * d
             push_body[e], push_k[e], push_kthr[e] = b, k, kthr
     params = WorldParams(n_envs=E, n_bodies=B, body_stride=S, pgs_iters=c["iters"],
-                         max_pairs=512 if B <= 54 else 768,
-                         max_contacts=1024 if B <= 54 else 1536)
+                         max_pairs=768,
+                         max_contacts=704 if B <= 54 else 1536)    # 54 blocks: 156 standing pairs, <= 171 seen in collapses
     return Workload(
         name=f"cfg{cfg}", params=params,
         state=state.astype(np.float32), props=props.astype(np.float32), mu=mu.astype(np.float32),
