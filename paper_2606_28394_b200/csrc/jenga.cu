@@ -23,68 +23,105 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
   return v;
 }
 
+// ---------------------------------------------------------------- warp / TMEM set-up
+// TM kernels: CTA = 4 warps = 4 envs, 256 TMEM columns per CTA (2 CTAs per SM), warp w uses TMEM lanes 32 w .. 32 w + 31.
+template <bool TM>
+__device__ __forceinline__ Smem begin_warp(const Params& P, int& env) {
+  __shared__ unsigned tm_base_s;
+  const int warp = threadIdx.x >> 5;
+  env = blockIdx.x * (TM ? 4 : 1) + warp;
+  Smem s = carve(P.S, P.max_pairs, P.pc, TM, warp * (int)smem_words(P.S, P.max_pairs, P.pc, TM));
+  if (TM) {
+    if (warp == 0) {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                   :: "r"((unsigned)__cvta_generic_to_shared(&tm_base_s)), "n"(kTmCols) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    s.tm = tm_base_s + ((unsigned)(warp * 32) << 16);
+  }
+  return s;
+}
+
+template <bool TM>
+__device__ __forceinline__ void end_warp(const Smem& s) {
+  if (TM) {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if ((threadIdx.x >> 5) == 0)
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s.tm), "n"(kTmCols) : "memory");   // warp 0: s.tm = base
+  }
+}
+
 // ---------------------------------------------------------------- fused step
-__global__ void __launch_bounds__(32) k_step(const Params P, const int n_steps) {
-  const Smem s = carve(P.S, P.max_pairs, P.pc);
-  const int env = blockIdx.x, lane = lane_id();
-  load_env(s, P, env);
-  if (lane == 0) { s.misc[MiNprev] = -1; s.misc[MiNph] = 0; s.misc[MiNcol] = 0; }
-  __syncwarp();
-  const float mu = P.mu[env];
-  unsigned st = 0;
-  unsigned long long c_cand = 0, c_coll = 0, c_cont = 0, c_gcont = 0, c_col = 0;
-  int m_cand = 0, m_coll = 0, m_col = 0, cur = 0;
-  const int n_sub = n_steps * P.n_substeps;
-  for (int sub = 0; sub < n_sub; ++sub) {
-    pose_and_predict(s, P, env, true);
-    const int n_cand = broadphase(s, P, &st);
-    const int n_coll = find_colliding(s, P, n_cand, cur, &st);
-    colour_pairs(s, P, n_coll, cur, &st);
-    setup_pairs(s, P, env, n_coll, cur);
-    pgs_sweeps(s, P, P.iters, mu);
-    if (P.materialise && sub == n_sub - 1) {
-      write_pairs(s, P, env, n_cand);
-      write_contacts(s, P, env, n_cand, n_coll, cur);
-      write_lambda(s, P, env, n_coll);
-    }
-    integrate(s, P, &st);
-    const int2 cc = store_cache(s, P, env, n_coll);
-    c_cont += cc.x; c_gcont += cc.y;
-    const int ncol = s.misc[MiNcol];
-    c_cand += n_cand; c_coll += n_coll; c_col += ncol;
-    m_cand = max(m_cand, n_cand); m_coll = max(m_coll, n_coll); m_col = max(m_col, ncol);
+template <bool TM>
+__global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const int n_steps) {
+  int env;
+  const Smem s = begin_warp<TM>(P, env);
+  const int lane = lane_id();
+  if (env < P.E) {
+    load_env(s, P, env);
+    if (lane == 0) { s.misc[MiNprev] = -1; s.misc[MiNph] = 0; s.misc[MiNcol] = 0; }
     __syncwarp();
-    if (lane == 0) s.misc[MiNprev] = n_coll;
-    cur ^= 1;
-    __syncwarp();
-  }
-  store_env(s, P, env);
-  flush_status(P, env, st);
-  if (P.counters) {
-    const unsigned long long v = warp_sum(c_cont), vg = warp_sum(c_gcont);
-    int n_active = 0;
-    for (int b = lane; b < P.B; b += 32) n_active += s.bd[b * kBd + 3] != 0.0f ? 1 : 0;
-    n_active = __reduce_add_sync(kFull, n_active);
-    if (lane == 0) {
-      atomicAdd(P.counters + JENGA_CNT_CONTACTS, v);
-      atomicAdd(P.counters + JENGA_CNT_CONTACT_ITERS, v * (unsigned long long)P.iters);
-      atomicAdd(P.counters + JENGA_CNT_GROUND_CONTACTS, vg);
-      atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, (unsigned long long)n_steps);
-      atomicAdd(P.counters + JENGA_CNT_BODY_STEPS, (unsigned long long)n_steps * n_active);
-      atomicAdd(P.counters + JENGA_CNT_CANDIDATES, c_cand);
-      atomicAdd(P.counters + JENGA_CNT_COLLIDING, c_coll);
-      atomicAdd(P.counters + JENGA_CNT_COLOURS, c_col);
-      atomicMax(P.counters + JENGA_CNT_MAX_CANDIDATES, (unsigned long long)m_cand);
-      atomicMax(P.counters + JENGA_CNT_MAX_COLLIDING, (unsigned long long)m_coll);
-      atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)m_col);
+    const float mu = P.mu[env];
+    unsigned st = 0;
+    unsigned long long c_cand = 0, c_coll = 0, c_cont = 0, c_gcont = 0, c_col = 0;
+    int m_cand = 0, m_coll = 0, m_col = 0, cur = 0;
+    const int n_sub = n_steps * P.n_substeps;
+    for (int sub = 0; sub < n_sub; ++sub) {
+      pose_and_predict(s, P, env, true);
+      const int n_cand = broadphase(s, P, &st);
+      const int n_coll = find_colliding(s, P, n_cand, cur, &st);
+      colour_pairs<TM>(s, P, n_coll, cur, &st);
+      setup_pairs<TM>(s, P, env, n_coll, cur);
+      pgs_sweeps<TM>(s, P, P.iters, mu);
+      if (P.materialise && sub == n_sub - 1) {
+        write_pairs(s, P, env, n_cand);
+        write_contacts(s, P, env, n_cand, n_coll, cur);
+        write_lambda<TM>(s, P, env, n_coll);
+      }
+      integrate(s, P, &st);
+      const int2 cc = store_cache<TM>(s, P, env, n_coll);
+      c_cont += cc.x; c_gcont += cc.y;
+      const int ncol = s.misc[MiNcol];
+      c_cand += n_cand; c_coll += n_coll; c_col += ncol;
+      m_cand = max(m_cand, n_cand); m_coll = max(m_coll, n_coll); m_col = max(m_col, ncol);
+      __syncwarp();
+      if (lane == 0) s.misc[MiNprev] = n_coll;
+      cur ^= 1;
+      __syncwarp();
+    }
+    store_env(s, P, env);
+    flush_status(P, env, st);
+    if (P.counters) {
+      const unsigned long long v = warp_sum(c_cont), vg = warp_sum(c_gcont);
+      int n_active = 0;
+      for (int b = lane; b < P.B; b += 32) n_active += s.bd[b * kBd + 3] != 0.0f ? 1 : 0;
+      n_active = __reduce_add_sync(kFull, n_active);
+      if (lane == 0) {
+        atomicAdd(P.counters + JENGA_CNT_CONTACTS, v);
+        atomicAdd(P.counters + JENGA_CNT_CONTACT_ITERS, v * (unsigned long long)P.iters);
+        atomicAdd(P.counters + JENGA_CNT_GROUND_CONTACTS, vg);
+        atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, (unsigned long long)n_steps);
+        atomicAdd(P.counters + JENGA_CNT_BODY_STEPS, (unsigned long long)n_steps * n_active);
+        atomicAdd(P.counters + JENGA_CNT_CANDIDATES, c_cand);
+        atomicAdd(P.counters + JENGA_CNT_COLLIDING, c_coll);
+        atomicAdd(P.counters + JENGA_CNT_COLOURS, c_col);
+        atomicMax(P.counters + JENGA_CNT_MAX_CANDIDATES, (unsigned long long)m_cand);
+        atomicMax(P.counters + JENGA_CNT_MAX_COLLIDING, (unsigned long long)m_coll);
+        atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)m_col);
+      }
     }
   }
+  end_warp<TM>(s);
 }
 
 // ---------------------------------------------------------------- stage kernels
 __global__ void __launch_bounds__(32) k_broadphase(const Params P) {
-  const Smem s = carve(P.S, P.max_pairs, P.pc);
-  const int env = blockIdx.x;
+  int env;
+  const Smem s = begin_warp<false>(P, env);
   unsigned st = 0;
   load_env(s, P, env);
   pose_and_predict(s, P, env, false);
@@ -102,8 +139,8 @@ __device__ inline int load_candidates(const Smem& s, const Params& P, int env) {
 }
 
 __global__ void __launch_bounds__(32) k_narrowphase(const Params P) {
-  const Smem s = carve(P.S, P.max_pairs, P.pc);
-  const int env = blockIdx.x;
+  int env;
+  const Smem s = begin_warp<false>(P, env);
   unsigned st = 0;
   load_env(s, P, env);
   pose_and_predict(s, P, env, false);
@@ -139,46 +176,55 @@ __device__ inline int pairs_from_contacts(const Smem& s, const Params& P, int en
   return n;
 }
 
-__global__ void __launch_bounds__(32) k_pgs(const Params P, const int iters) {
-  const Smem s = carve(P.S, P.max_pairs, P.pc);
-  const int env = blockIdx.x, lane = lane_id();
-  unsigned st = 0;
-  load_env(s, P, env);
-  if (lane == 0) { s.misc[MiNprev] = -1; s.misc[MiNph] = 0; s.misc[MiNcol] = 0; }
-  pose_and_predict(s, P, env, false);
-  const int n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
-  const int n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
-  // contact offsets survive the colouring (which reuses s.wrank) in the previous-list buffer, free in this kernel
-  const SP<unsigned short> keep = s.cpair[1];
-  for (int r = lane; r < n_coll; r += 32) keep[r] = s.wrank[r];
-  __syncwarp();
-  colour_pairs(s, P, n_coll, 0, &st);
-  for (int r = lane; r < n_coll; r += 32) s.wrank[r] = keep[r];
-  __syncwarp();
-  const float4* in = reinterpret_cast<const float4*>(P.contacts + (size_t)env * P.max_contacts * 8);
-  for (int base = 0; base < n_coll; base += 32) {
-    const int k = base + lane;
-    if (k < n_coll) {
-      const int r = s.order[k];
-      const int c0 = s.wrank[r], c1 = r + 1 < n_coll ? s.wrank[r + 1] : n_cont;
-      const unsigned w = s.cab[r];
-      Manifold m; m.np = min(4, c1 - c0);
-      const float4 f0 = in[2 * c0];
-      m.n = v3(f0.x, f0.y, f0.z);
-      m.axis = (__float_as_int(in[2 * c0 + 1].w) >> 20) & 0xf;
+template <bool TM>
+__global__ void __launch_bounds__(TM ? 128 : 32) k_pgs(const Params P, const int iters) {
+  int env;
+  const Smem s = begin_warp<TM>(P, env);
+  const int lane = lane_id();
+  if (env < P.E) {
+    unsigned st = 0;
+    load_env(s, P, env);
+    if (lane == 0) { s.misc[MiNprev] = -1; s.misc[MiNph] = 0; s.misc[MiNcol] = 0; }
+    pose_and_predict(s, P, env, false);
+    const int n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
+    const int n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
+    // contact offsets survive the colouring (which reuses s.wrank) in the previous-list buffer, free in this kernel
+    const SP<unsigned short> keep = s.cpair[1];
+    for (int r = lane; r < n_coll; r += 32) keep[r] = s.wrank[r];
+    __syncwarp();
+    colour_pairs<TM>(s, P, n_coll, 0, &st);
+    for (int r = lane; r < n_coll; r += 32) s.wrank[r] = keep[r];
+    __syncwarp();
+    const float4* in = reinterpret_cast<const float4*>(P.contacts + (size_t)env * P.max_contacts * 8);
+    for (int j = 0; 32 * j < n_coll; ++j) {
+      const int k = 32 * j + lane;
+      PairC pc;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        m.p[c] = v3(0, 0, 0); m.d[c] = 0.0f;
-        if (c < m.np) { const float4 a4 = in[2 * (c0 + c)], b4 = in[2 * (c0 + c) + 1]; m.p[c] = v3(b4.x, b4.y, b4.z); m.d[c] = a4.w; }
+      for (int t = 0; t < 48; ++t) pc.v[t] = 0.0f;
+      if (k < n_coll) {
+        const int r = s.order[k];
+        const int c0 = s.wrank[r], c1 = r + 1 < n_coll ? s.wrank[r + 1] : n_cont;
+        const unsigned w = s.cab[r];
+        Manifold m; m.np = min(4, c1 - c0);
+        const float4 f0 = in[2 * c0];
+        m.n = v3(f0.x, f0.y, f0.z);
+        m.axis = (__float_as_int(in[2 * c0 + 1].w) >> 20) & 0xf;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          m.p[c] = v3(0, 0, 0); m.d[c] = 0.0f;
+          if (c < m.np) { const float4 a4 = in[2 * (c0 + c)], b4 = in[2 * (c0 + c) + 1]; m.p[c] = v3(b4.x, b4.y, b4.z); m.d[c] = a4.w; }
+        }
+        setup_slot(s, P, env, k, ab_a(w), ab_b(w), s.cpair[0][r], m, pc);
       }
-      setup_slot(s, P, env, k, ab_a(w), ab_b(w), s.cpair[0][r], m);
+      round_store<TM>(s, j, n_coll, pc);
     }
+    __syncwarp();
+    pgs_sweeps<TM>(s, P, iters, P.mu[env]);
+    write_lambda<TM>(s, P, env, n_coll);
+    store_env(s, P, env);
+    flush_status(P, env, st);
   }
-  __syncwarp();
-  pgs_sweeps(s, P, iters, P.mu[env]);
-  write_lambda(s, P, env, n_coll);
-  store_env(s, P, env);
-  flush_status(P, env, st);
+  end_warp<TM>(s);
 }
 
 }  // namespace jenga
@@ -190,8 +236,9 @@ struct jenga_world {
   jenga_world_desc desc;
   jenga_buffers bufs;
   Params P;
-  int threads;
-  size_t smem;
+  bool tm;                 // step / solve kernels keep the first 160 pairs' contact constants in TMEM (4 envs per CTA)
+  size_t smem_step;        // dynamic shared memory per CTA of k_step / k_pgs
+  size_t smem_stage;       // ... of k_broadphase / k_narrowphase (one warp per CTA, no TMEM)
 };
 
 static char g_err[512] = "no error";
@@ -203,18 +250,30 @@ static bool desc_ok(const jenga_world_desc* d) {
   if (d->n_substeps <= 0 || d->pgs_iters < 0 || !(d->dt > 0.0f)) return false;
   if (d->max_pairs <= 0 || d->max_pairs > 65535) return false;
   if (d->max_contacts < 4 || (d->max_contacts & 3) || d->max_contacts > 65532) return false;
-  if (4 * jenga::smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4) > 227 * 1024) return false;
+  if (4 * jenga::smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, false) > 227 * 1024) return false;
   return true;
+}
+
+static size_t env_bytes(const jenga_world_desc* d, bool tm) {
+  return 4 * jenga::smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, tm);
+}
+
+/* The TMEM kernel pays off when two 4-env CTAs fit one SM (8 envs instead of <= 4); JENGA_NO_TMEM=1 forces the
+ * all-shared-memory kernel (used by the tests to cover both). */
+static bool use_tmem(const jenga_world_desc* d) {
+  const char* off = getenv("JENGA_NO_TMEM");
+  if (off && off[0] == '1') return false;
+  return 2 * (4 * env_bytes(d, true) + 1024 + 16) <= 227 * 1024;
 }
 
 extern "C" size_t jenga_smem_bytes(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
-  return 4 * jenga::smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4);
+  return use_tmem(d) ? 4 * env_bytes(d, true) : env_bytes(d, false);
 }
 
 extern "C" int jenga_block_threads(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
-  return 32;   /* one warp per env */
+  return use_tmem(d) ? 128 : 32;   /* one warp per env; 4 envs per CTA in the TMEM kernel */
 }
 
 extern "C" const char* jenga_strerror(int code) {
@@ -234,9 +293,6 @@ static int cuda_fail(cudaError_t e, const char* what) {
 
 static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; }
 
-template <typename Kern, typename... Args>
-static int launch(const char* name, Kern k, jenga_world* w, void* stream, Args... args);
-
 extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers* b, jenga_world** out) {
   if (!out) return JENGA_E_ARG;
   *out = nullptr;
@@ -254,7 +310,7 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   if (smem > (size_t)prop.sharedMemPerBlockOptin) return JENGA_E_ARG;
   jenga_world* w = (jenga_world*)calloc(1, sizeof(jenga_world));
   if (!w) return JENGA_E_ARG;
-  w->desc = *d; w->bufs = *b; w->smem = smem; w->threads = 32;
+  w->desc = *d; w->bufs = *b; w->tm = use_tmem(d); w->smem_step = smem; w->smem_stage = env_bytes(d, false);
   Params& P = w->P;
   P.E = d->n_envs; P.B = d->n_bodies; P.S = d->body_stride;
   P.h = d->dt / (float)d->n_substeps; P.n_substeps = d->n_substeps; P.iters = d->pgs_iters;
@@ -267,20 +323,20 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.pairs = b->pairs; P.n_pairs = b->n_pairs; P.contacts = b->contacts; P.n_contacts = b->n_contacts; P.lambda = b->lambda;
   P.cache_key = b->cache_key; P.cache_lam = b->cache_lam; P.cache_pt = b->cache_pt; P.n_cache = b->n_cache;
   P.status = b->status; P.counters = b->counters;
-  const void* kernels[] = { (const void*)jenga::k_step, (const void*)jenga::k_broadphase, (const void*)jenga::k_narrowphase,
-                            (const void*)jenga::k_pgs };
-  for (const void* k : kernels) {
-    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  struct { const void* k; size_t smem; } kernels[] = {
+    { w->tm ? (const void*)jenga::k_step<true> : (const void*)jenga::k_step<false>, w->smem_step },
+    { w->tm ? (const void*)jenga::k_pgs<true> : (const void*)jenga::k_pgs<false>, w->smem_step },
+    { (const void*)jenga::k_broadphase, w->smem_stage }, { (const void*)jenga::k_narrowphase, w->smem_stage } };
+  for (auto& kn : kernels) {
+    e = cudaFuncSetAttribute(kn.k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kn.smem);
     if (e != cudaSuccess) { free(w); return cuda_fail(e, "cudaFuncSetAttribute"); }
-    cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(kn.k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   }
   *out = w;
   return JENGA_OK;
 }
 
-template <typename Kern, typename... Args>
-static int launch(const char* name, Kern k, jenga_world* w, void* stream, Args... args) {
-  k<<<w->P.E, 32, w->smem, (cudaStream_t)stream>>>(w->P, args...);
+static int launched(const char* name) {
   const cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? JENGA_OK : cuda_fail(e, name);
 }
@@ -299,24 +355,30 @@ extern "C" int jenga_set_f_ext(jenga_world* w, const float* f_ext) {
 
 extern "C" int jenga_broadphase(jenga_world* w, void* stream) {
   if (!w) return JENGA_E_ARG;
-  return launch("k_broadphase", jenga::k_broadphase, w, stream);
+  jenga::k_broadphase<<<w->P.E, 32, w->smem_stage, (cudaStream_t)stream>>>(w->P);
+  return launched("k_broadphase");
 }
 
 extern "C" int jenga_narrowphase(jenga_world* w, void* stream) {
   if (!w) return JENGA_E_ARG;
-  return launch("k_narrowphase", jenga::k_narrowphase, w, stream);
+  jenga::k_narrowphase<<<w->P.E, 32, w->smem_stage, (cudaStream_t)stream>>>(w->P);
+  return launched("k_narrowphase");
 }
 
 extern "C" int jenga_pgs_solve(jenga_world* w, int iters, void* stream) {
   if (!w || iters < 0) return JENGA_E_ARG;
   const int it = iters > 0 ? iters : w->P.iters;
-  return launch("k_pgs", jenga::k_pgs, w, stream, it);
+  if (w->tm) jenga::k_pgs<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, it);
+  else jenga::k_pgs<false><<<w->P.E, 32, w->smem_step, (cudaStream_t)stream>>>(w->P, it);
+  return launched("k_pgs");
 }
 
 extern "C" int jenga_step(jenga_world* w, int n_steps, void* stream) {
   if (!w || n_steps < 0) return JENGA_E_ARG;
   if (n_steps == 0) return JENGA_OK;
-  return launch("k_step", jenga::k_step, w, stream, n_steps);
+  if (w->tm) jenga::k_step<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps);
+  else jenga::k_step<false><<<w->P.E, 32, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps);
+  return launched("k_step");
 }
 
 extern "C" int jenga_step_host(jenga_world* w, const float* h_in, float* h_out, int n_steps, void* stream) {

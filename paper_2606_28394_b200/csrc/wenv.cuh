@@ -20,7 +20,11 @@ namespace jenga {
 constexpr int kStateRows = 13, kPropRows = 8, kFextRows = 6;
 constexpr int kMaxColours = 64;
 constexpr int kBd = 20;        // floats per body record: x y z im | vx vy vz - | wx wy wz - | Ixx Ixy Ixz Iyy | Iyz Izz - -
-constexpr int kSlotF4 = 14;    // float4 per pair slot: header, normal+corr, 4 contacts x 3
+constexpr int kHdrF4 = 2;      // float4 per pair header: (a, b, meta, 1/|t1 raw|), (n.xyz, Baumgarte corr)
+constexpr int kCsF4 = 12;      // float4 of contact constants per pair: 36 read-only words + 12 impulses
+constexpr int kTmBlocks = 5;   // TMEM tier: the first 5 x 32 colour-sorted positions keep their contact constants in
+constexpr int kTmPos = 32 * kTmBlocks;   // tensor memory (48 columns per block of 32 pairs, lane = position % 32)
+constexpr int kTmCols = 256;   // columns allocated per CTA of 4 warps (4 envs); 2 CTAs per SM
 constexpr unsigned kFull = 0xffffffffu;
 
 struct Params {
@@ -49,7 +53,8 @@ template <typename T> struct SP {
 };
 
 struct Smem {
-  SP<float4> slot;              // [kSlotF4][pcA]
+  SP<float4> hdr;               // [kHdrF4][pcA] pair headers, colour-sorted position
+  SP<float4> cs;                // [kCsF4][capS] contact constants of the positions kept in shared memory
   SP<float> bd;                // [S][kBd]
   SP<float> q;                  // [4][S]
   SP<float> pr;                // [8][S]  inv_m invIx invIy invIz hx hy hz active
@@ -67,40 +72,46 @@ struct Smem {
   SP<int> ccount;               // [64]
   SP<int> cstart;               // [64]
   SP<int> misc;                 // [16]
-  int pcA;
+  int pcA, capS, pos0;          // pos0: first colour-sorted position held in cs (0, or kTmPos in the TMEM kernel)
+  unsigned tm;                  // TMEM address of this warp's lanes, column 0 (TMEM kernel)
 };
 
 enum { MiNph = 0, MiNcol = 1, MiNprev = 2, MiCur = 3 };
 
 __host__ __device__ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
-// The slot region is dead between S7 of one substep and the setup pass of the next, which is when the candidate
-// list (S2 -> first half of S3) and the colouring masks (S4) live: they alias it.
-__host__ __device__ inline int slot_region_words(int S, int max_pairs, int pc) {
+// The header + contact-constant region is dead between S7 of one substep and the setup pass of the next, which is
+// when the candidate list (S2 -> first half of S3) and the colouring masks (S4) live: they alias it.
+__host__ __device__ inline int cap_smem_pairs(int pc, bool tm) {
+  const int pcA = round_up(pc, 8);
+  return tm ? (pcA > kTmPos ? pcA - kTmPos : 8) : pcA;
+}
+__host__ __device__ inline int slot_region_words(int S, int max_pairs, int pc, bool tm) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8);
-  const int a = kSlotF4 * 4 * pcA, b = mpA / 2 + 2 * S;
+  const int a = 4 * (kHdrF4 * pcA + kCsF4 * cap_smem_pairs(pc, tm)), b = mpA / 2 + 2 * S;
   return round_up(a > b ? a : b, 4);
 }
 
-__host__ __device__ inline size_t smem_words(int S, int max_pairs, int pc) {
+__host__ __device__ inline size_t smem_words(int S, int max_pairs, int pc, bool tm) {
   const int pcA = round_up(pc, 8);
-  size_t w = slot_region_words(S, max_pairs, pc);
+  size_t w = slot_region_words(S, max_pairs, pc, tm);
   w += (size_t)(kBd + 4 + 8 + 9 + 3) * S;
   w += pcA;                        // cab
   w += 5 * (size_t)(pcA / 2);      // cpair x2, pos, order, wrank (u16)
   w += pcA / 4;                    // colour (u8)
-  w += kMaxColours + pcA / 32 + 4; // ph
+  w += kMaxColours + pcA / 32 + 8; // ph
   w += 2 * kMaxColours + 16;       // ccount, cstart, misc
   return round_up((int)w, 4);
 }
 
-__device__ inline Smem carve(int S, int max_pairs, int pc) {
+// base: word offset of this env's arena inside the CTA's dynamic shared memory
+__device__ inline Smem carve(int S, int max_pairs, int pc, bool tm, int base) {
   Smem s;
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8);
-  s.pcA = pcA;
-  int p = 0;
-  s.slot.off = 0; s.cand.off = 0; s.used.off = mpA / 2;
-  p += slot_region_words(S, max_pairs, pc);
+  s.pcA = pcA; s.capS = cap_smem_pairs(pc, tm); s.pos0 = tm ? kTmPos : 0; s.tm = 0;
+  int p = base;
+  s.hdr.off = p; s.cs.off = p + 4 * kHdrF4 * pcA; s.cand.off = p; s.used.off = p + mpA / 2;
+  p += slot_region_words(S, max_pairs, pc, tm);
   s.bd.off = p;  p += kBd * S;
   s.q.off = p;   p += 4 * S;
   s.pr.off = p;  p += 8 * S;
@@ -113,7 +124,7 @@ __device__ inline Smem carve(int S, int max_pairs, int pc) {
   s.order.off = p; p += pcA / 2;
   s.wrank.off = p; p += pcA / 2;
   s.colour.off = p; p += pcA / 4;
-  s.ph.off = p; p += kMaxColours + pcA / 32 + 4;
+  s.ph.off = p; p += kMaxColours + pcA / 32 + 8;
   s.ccount.off = p; p += kMaxColours;
   s.cstart.off = p; p += kMaxColours;
   s.misc.off = p;

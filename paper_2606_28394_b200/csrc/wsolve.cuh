@@ -58,6 +58,7 @@ __device__ inline int find_colliding(const Smem& s, const Params& P, int n_cand,
 // The walk is sequential by definition (lane 0, one 64-bit mask per body); when the colliding-pair
 // list equals the previous substep's the previous colouring is the same function of the same input
 // and is kept.
+template <bool TM>
 __device__ inline void colour_pairs(const Smem& s, const Params& P, int n_coll, int cur, unsigned* status) {
   const int lane = lane_id();
   bool same = n_coll == s.misc[MiNprev];
@@ -89,7 +90,12 @@ __device__ inline void colour_pairs(const Smem& s, const Params& P, int n_coll, 
     for (int c = 0; c < ncol; ++c) {
       const int n = s.ccount[c];
       s.cstart[c] = acc;
-      for (int off = 0; off < n; off += 32) s.ph[nph++] = (acc + off) | (min(32, n - off) << 16);
+      for (int st0 = acc; st0 < acc + n; ) {                     // chunks of <= 32 pairs; none straddles the TMEM boundary
+        int lim = min(acc + n, st0 + 32);
+        if (TM && st0 < kTmPos && lim > kTmPos) lim = kTmPos;
+        s.ph[nph++] = st0 | ((lim - st0) << 16);
+        st0 = lim;
+      }
       acc += n;
     }
     s.misc[MiNcol] = ncol; s.misc[MiNph] = nph;
@@ -104,12 +110,77 @@ __device__ inline void colour_pairs(const Smem& s, const Params& P, int n_coll, 
 }
 
 // ---------------------------------------------------------------- pair slots (colour-sorted solver constants)
-// float4 fields of slot k (s.slot[f * pcA + k]):
+// Header of position k (shared memory, s.hdr[f * pcA + k]):
 //   0: a, b, meta = np | axis << 8 | pair index << 16 (int bits), 1/|e_k - n (n.e_k)| (tangent normalisation)
 //   1: n.x n.y n.z, Baumgarte corr = beta max(0, depth_max - slop) / (imA + imB)     (Eq. 16)
-//   2+3c: p.x p.y p.z, (1+e)/K_nn          3+3c: 1/K_t1t1, 1/K_t2t2, K_n,t1, K_n,t2
-//   4+3c: K_t1,t2, jn, jt1, jt2             (K_dd: Eq. 13, for d = n, t1, t2)
-__device__ __forceinline__ float4& slot4(const Smem& s, int f, int k) { return s.slot[f * s.pcA + k]; }
+// Contact constants of position k: 48 words, PairC.  ro[9c..9c+8] = p.xyz, (1+e)/K_nn, 1/K_t1t1, 1/K_t2t2,
+// K_n,t1, K_n,t2, K_t1,t2 of contact c (K_dd: Eq. 13, for d = n, t1, t2); lam[3c..3c+2] = jn, jt1, jt2.
+// They live in shared memory (field-major float4 [12][capS], position k - pos0) or, in the TMEM kernel for
+// positions < kTmPos, in tensor memory: block j = k / 32 at columns [48 j, 48 j + 48) of lane k % 32.
+__device__ __forceinline__ float4& hdr4(const Smem& s, int f, int k) { return s.hdr[f * s.pcA + k]; }
+
+struct PairC { float v[48]; };      // v[0..35] read-only constants, v[36..47] impulses
+constexpr int kLam = 36;
+
+__device__ __forceinline__ void tm_ld16(unsigned a, float* r) {
+  unsigned* u = reinterpret_cast<unsigned*>(r);
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+               : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]), "=r"(u[6]), "=r"(u[7]),
+                 "=r"(u[8]), "=r"(u[9]), "=r"(u[10]), "=r"(u[11]), "=r"(u[12]), "=r"(u[13]), "=r"(u[14]), "=r"(u[15]) : "r"(a));
+}
+__device__ __forceinline__ void tm_st16(unsigned a, const float* r) {
+  const unsigned* u = reinterpret_cast<const unsigned*>(r);
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+               :: "r"(a), "r"(u[0]), "r"(u[1]), "r"(u[2]), "r"(u[3]), "r"(u[4]), "r"(u[5]), "r"(u[6]), "r"(u[7]),
+                  "r"(u[8]), "r"(u[9]), "r"(u[10]), "r"(u[11]), "r"(u[12]), "r"(u[13]), "r"(u[14]), "r"(u[15]) : "memory");
+}
+__device__ __forceinline__ void tm_st4(unsigned a, const float* r) {
+  const unsigned* u = reinterpret_cast<const unsigned*>(r);
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" :: "r"(a), "r"(u[0]), "r"(u[1]), "r"(u[2]), "r"(u[3]) : "memory");
+}
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// whole block j (all 32 lanes take part; lane l gets position 32 j + l)
+__device__ __forceinline__ void tm_load_block(const Smem& s, int j, PairC& c) {
+  const unsigned a = s.tm + 48u * (unsigned)j;
+  tm_ld16(a, c.v); tm_ld16(a + 16, c.v + 16); tm_ld16(a + 32, c.v + 32);
+}
+__device__ __forceinline__ void tm_store_block(const Smem& s, int j, const PairC& c) {
+  const unsigned a = s.tm + 48u * (unsigned)j;
+  tm_st16(a, c.v); tm_st16(a + 16, c.v + 16); tm_st16(a + 32, c.v + 32);
+}
+__device__ __forceinline__ void tm_store_lam(const Smem& s, int j, const float* lam) {
+  const unsigned a = s.tm + 48u * (unsigned)j + 36u;
+  tm_st4(a, lam); tm_st4(a + 4, lam + 4); tm_st4(a + 8, lam + 8);
+}
+// shared-memory tier: position k >= pos0
+__device__ __forceinline__ void sm_load_pair(const Smem& s, int k, PairC& c) {
+  const int i = k - s.pos0;
+#pragma unroll
+  for (int f = 0; f < kCsF4; ++f) { const float4 t = s.cs[f * s.capS + i]; c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
+}
+__device__ __forceinline__ void sm_store_pair(const Smem& s, int k, const PairC& c) {
+  const int i = k - s.pos0;
+#pragma unroll
+  for (int f = 0; f < kCsF4; ++f) s.cs[f * s.capS + i] = make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]);
+}
+__device__ __forceinline__ void sm_store_lam(const Smem& s, int k, const float* lam) {
+  const int i = k - s.pos0;
+#pragma unroll
+  for (int f = 0; f < 3; ++f) s.cs[(9 + f) * s.capS + i] = make_float4(lam[4 * f], lam[4 * f + 1], lam[4 * f + 2], lam[4 * f + 3]);
+}
+// aligned round: lane l <-> position 32 j + l (setup, cache store, lambda output).  All lanes call these.
+template <bool TM>
+__device__ __forceinline__ void round_load(const Smem& s, int j, int n_valid, PairC& c) {
+  if (TM && j < kTmBlocks) { tm_load_block(s, j, c); tm_wait_ld(); }
+  else if (32 * j + lane_id() < n_valid) sm_load_pair(s, 32 * j + lane_id(), c);
+}
+template <bool TM>
+__device__ __forceinline__ void round_store(const Smem& s, int j, int n_valid, const PairC& c) {
+  if (TM && j < kTmBlocks) { tm_store_block(s, j, c); tm_wait_st(); }
+  else if (32 * j + lane_id() < n_valid) sm_store_pair(s, 32 * j + lane_id(), c);
+}
 
 struct Frame { Vec3 n, t1, t2; };
 
@@ -148,7 +219,7 @@ __device__ __forceinline__ Vec3 xyz(float4 v) { return v3(v.x, v.y, v.z); }
 // contact inherits (jn,jt1,jt2) of the nearest not yet taken previous contact point of the same pair
 // within match_tol; slots ascending.
 __device__ inline void setup_slot(const Smem& s, const Params& P, int env, int k, int a, int b, int pair,
-                                  const Manifold& m) {
+                                  const Manifold& m, PairC& out) {
   Body5 A, Bb; load_body(s, a, A, false); load_body(s, b, Bb, false);
   const Vec3 n = m.n;
   Vec3 u; tangent_raw(n, u);
@@ -199,8 +270,8 @@ __device__ inline void setup_slot(const Smem& s, const Params& P, int env, int k
   }
 
   const int meta = m.np | (m.axis << 8) | (pair << 16);
-  slot4(s, 0, k) = make_float4(__int_as_float(a), __int_as_float(b), __int_as_float(meta), il);
-  slot4(s, 1, k) = make_float4(n.x, n.y, n.z, im > 0.0f ? P.beta * fmaxf(0.0f, dmax - P.slop) / im : 0.0f);
+  hdr4(s, 0, k) = make_float4(__int_as_float(a), __int_as_float(b), __int_as_float(meta), il);
+  hdr4(s, 1, k) = make_float4(n.x, n.y, n.z, im > 0.0f ? P.beta * fmaxf(0.0f, dmax - P.slop) / im : 0.0f);
   const float e1 = 1.0f + P.restitution;
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
@@ -220,18 +291,22 @@ __device__ inline void setup_slot(const Smem& s, const Params& P, int env, int k
       ko[1] = dot(uA[0], wA[2]) + dot(uB[0], wB[2]);
       ko[2] = dot(uA[1], wA[2]) + dot(uB[1], wB[2]);
     }
-    slot4(s, 2 + 3 * c, k) = make_float4(pt[c].x, pt[c].y, pt[c].z, ik[0]);
-    slot4(s, 3 + 3 * c, k) = make_float4(ik[1], ik[2], ko[0], ko[1]);
-    slot4(s, 4 + 3 * c, k) = make_float4(ko[2], lam[c][0], lam[c][1], lam[c][2]);
+    float* o = out.v + 9 * c;
+    o[0] = pt[c].x; o[1] = pt[c].y; o[2] = pt[c].z; o[3] = ik[0]; o[4] = ik[1]; o[5] = ik[2]; o[6] = ko[0]; o[7] = ko[1]; o[8] = ko[2];
+    out.v[kLam + 3 * c] = lam[c][0]; out.v[kLam + 3 * c + 1] = lam[c][1]; out.v[kLam + 3 * c + 2] = lam[c][2];
   }
 }
 
-// S3 second half + S4: lane l of a round takes colour-sorted position base+l, computes the pair's manifold
-// (same SAT code as find_colliding -> same decisions) and writes its slot.
+// S3 second half + S4: lane l of round j takes colour-sorted position 32 j + l, computes the pair's manifold
+// (same SAT code as find_colliding -> same decisions) and writes its header and contact constants.
+template <bool TM>
 __device__ inline void setup_pairs(const Smem& s, const Params& P, int env, int n_coll, int cur) {
   const int S = P.S, lane = lane_id();
-  for (int base = 0; base < n_coll; base += 32) {
-    const int k = base + lane;
+  for (int j = 0; 32 * j < n_coll; ++j) {
+    const int k = 32 * j + lane;
+    PairC c;
+#pragma unroll
+    for (int t = 0; t < 48; ++t) c.v[t] = 0.0f;
     if (k < n_coll) {
       const int r = s.order[k];
       const unsigned w = s.cab[r];
@@ -240,8 +315,9 @@ __device__ inline void setup_pairs(const Smem& s, const Params& P, int env, int 
       const Box Bj = load_box(s, S, b);
       if (a < 0) collide_ground(Bj, m);
       else { const Box Bi = load_box(s, S, a); collide_boxes(P.cp, Bi, Bj, m); }
-      setup_slot(s, P, env, k, a, b, s.cpair[cur][r], m);
+      setup_slot(s, P, env, k, a, b, s.cpair[cur][r], m, c);
     }
+    round_store<TM>(s, j, n_coll, c);
   }
   __syncwarp();
 }
@@ -259,30 +335,51 @@ __device__ __forceinline__ void apply_impulse(Body5& A, Body5& B, Vec3 rA, Vec3 
   B.w.z = fmaf(B.i1.y, cB.z, fmaf(B.i1.x, cB.y, fmaf(B.i0.z, cB.x, B.w.z)));
 }
 
-// One colour chunk of the warm-start application (S4) or of a Gauss-Seidel sweep (S5).  Lane l takes the pair
-// at colour-sorted position start+l: slots ascending; per contact the normal row (Eq. 14, clamp >= 0), then
-// t1, then t2 (Eq. 15, each clipped to +-mu_s jn) -- Listing 1.  The three rows of a contact
-// act on the same two bodies: the relative velocity of the contact point is read once, advanced between rows
-// with the contact-space couplings K_ij (exactly the change the applied impulse causes), and the summed
-// impulse is applied once (DESIGN §3 R-couple).  Pairs of one colour share no dynamic body.
-template <bool WARM>
+// One colour chunk of the warm-start application (S4) or of a Gauss-Seidel sweep (S5).  Lane l takes the pair at
+// colour-sorted position k = start + ((l - start) mod 32), i.e. lane = k mod 32 (the lane that owns the pair's
+// TMEM row): slots ascending; per contact the normal row (Eq. 14, clamp >= 0), then t1, then t2 (Eq. 15, each
+// clipped to +-mu_s jn) -- Listing 1.  The three rows of a contact act on the same two bodies:
+// the relative velocity of the contact point is read once, advanced between rows with the contact-space couplings
+// K_ij (exactly the change the applied impulse causes), and the summed impulse is applied once (DESIGN §3
+// R-couple).  Pairs of one colour share no dynamic body.
+template <bool TM, bool WARM>
 __device__ __forceinline__ void solve_chunk(const Smem& s, int start, int count, float mu) {
   const int lane = lane_id();
-  if (lane < count) {
-    const int k = start + lane;
-    const float4 h = slot4(s, 0, k), nn = slot4(s, 1, k);
+  const int k = start + ((lane - start) & 31);
+  const bool active = k < start + count;
+  const int jA = start >> 5;
+  const bool in_tm = TM && start < kTmPos;                       // chunks never straddle kTmPos
+  const bool span = (start & 31) + count > 32;
+  PairC c;
+  float keepA[12], keepB[12];                                    // impulses of the lanes that are not in this chunk
+  if (in_tm) {
+    tm_load_block(s, jA, c);
+    PairC o;
+    if (span) tm_load_block(s, jA + 1, o);
+    tm_wait_ld();
+    const bool mineB = (k >> 5) != jA;
+#pragma unroll
+    for (int t = 0; t < 12; ++t) { keepA[t] = c.v[kLam + t]; keepB[t] = span ? o.v[kLam + t] : 0.0f; }
+    if (span) {
+#pragma unroll
+      for (int t = 0; t < 48; ++t) c.v[t] = mineB ? o.v[t] : c.v[t];
+    }
+  } else if (active) {
+    sm_load_pair(s, k, c);
+  }
+  if (active) {
+    const float4 h = hdr4(s, 0, k), nn = hdr4(s, 1, k);
     const int a = __float_as_int(h.x), b = __float_as_int(h.y), np = __float_as_int(h.z) & 0xff;
     Body5 A, B; load_body(s, a, A, true); load_body(s, b, B, true);
     const Frame F = make_frame(xyz(nn), h.w);
 #pragma unroll
-    for (int c = 0; c < 4; ++c)
-      if (c < np) {
-        const float4 p4 = slot4(s, 2 + 3 * c, k), k4 = slot4(s, 3 + 3 * c, k);
-        float4 l4 = slot4(s, 4 + 3 * c, k);
-        const Vec3 p = xyz(p4), rA = p - xyz(A.x), rB = p - xyz(B.x);
+    for (int ci = 0; ci < 4; ++ci)
+      if (ci < np) {
+        const float* r = c.v + 9 * ci; float* l = c.v + kLam + 3 * ci;
+        const Vec3 p = v3(r[0], r[1], r[2]), rA = p - xyz(A.x), rB = p - xyz(B.x);
         Vec3 Pi;
         if (WARM) {
-          Pi = madd(madd(l4.y * F.n, l4.z, F.t1), l4.w, F.t2);
+          Pi = madd(madd(l[0] * F.n, l[1], F.t1), l[2], F.t2);
         } else {
           // vr = (vB + wB x rB) - (vA + wA x rA), each component one subtraction and four fused multiply-adds
           const Vec3 vr = v3(
@@ -291,34 +388,47 @@ __device__ __forceinline__ void solve_chunk(const Smem& s, int start, int count,
             fmaf(A.w.y, rA.x, fmaf(-A.w.x, rA.y, fmaf(-B.w.y, rB.x, fmaf(B.w.x, rB.y, B.v.z - A.v.z)))));
           const float u0 = dot(vr, F.n);
           float u1 = dot(vr, F.t1), u2 = dot(vr, F.t2);
-          const float nw = fmaxf(fmaf(-u0, p4.w, l4.y), 0.0f);
-          const float d0 = nw - l4.y;
-          u1 = fmaf(k4.z, d0, u1); u2 = fmaf(k4.w, d0, u2);
+          const float nw = fmaxf(fmaf(-u0, r[3], l[0]), 0.0f);
+          const float d0 = nw - l[0];
+          u1 = fmaf(r[6], d0, u1); u2 = fmaf(r[7], d0, u2);
           const float lim = mu * nw;
-          const float n1 = fminf(fmaxf(fmaf(-u1, k4.x, l4.z), -lim), lim);
-          const float d1 = n1 - l4.z;
-          u2 = fmaf(l4.x, d1, u2);
-          const float n2 = fminf(fmaxf(fmaf(-u2, k4.y, l4.w), -lim), lim);
-          const float d2 = n2 - l4.w;
-          l4.y = nw; l4.z = n1; l4.w = n2;
-          slot4(s, 4 + 3 * c, k) = l4;
+          const float n1 = fminf(fmaxf(fmaf(-u1, r[4], l[1]), -lim), lim);
+          const float d1 = n1 - l[1];
+          u2 = fmaf(r[8], d1, u2);
+          const float n2 = fminf(fmaxf(fmaf(-u2, r[5], l[2]), -lim), lim);
+          const float d2 = n2 - l[2];
+          l[0] = nw; l[1] = n1; l[2] = n2;
           Pi = madd(madd(d0 * F.n, d1, F.t1), d2, F.t2);
         }
         apply_impulse(A, B, rA, rB, Pi);
       }
     if (a >= 0) { bd4(s, a, 1) = A.v; bd4(s, a, 2) = A.w; }
     bd4(s, b, 1) = B.v; bd4(s, b, 2) = B.w;
+    if (!WARM && !in_tm) sm_store_lam(s, k, c.v + kLam);
+  }
+  if (!WARM && in_tm) {                                          // all lanes: rows outside the chunk get their old values back
+    const bool mineB = (k >> 5) != jA;
+#pragma unroll
+    for (int t = 0; t < 12; ++t) {
+      const float mine = c.v[kLam + t];
+      keepA[t] = (active && !mineB) ? mine : keepA[t];
+      keepB[t] = (active && mineB) ? mine : keepB[t];
+    }
+    tm_store_lam(s, jA, keepA);
+    if (span) tm_store_lam(s, jA + 1, keepB);
+    tm_wait_st();
   }
   __syncwarp();
 }
 
 // S4 (warm-start application) + S5: the phase chunks in canonical order, `iters` sweeps.
+template <bool TM>
 __device__ inline void pgs_sweeps(const Smem& s, const Params& P, int iters, float mu) {
   const int nph = s.misc[MiNph];
   if (P.warm_start)
-    for (int j = 0; j < nph; ++j) { const int w = s.ph[j]; solve_chunk<true>(s, w & 0xffff, w >> 16, mu); }
+    for (int j = 0; j < nph; ++j) { const int w = s.ph[j]; solve_chunk<TM, true>(s, w & 0xffff, w >> 16, mu); }
   for (int it = 0; it < iters; ++it)
-    for (int j = 0; j < nph; ++j) { const int w = s.ph[j]; solve_chunk<false>(s, w & 0xffff, w >> 16, mu); }
+    for (int j = 0; j < nph; ++j) { const int w = s.ph[j]; solve_chunk<TM, false>(s, w & 0xffff, w >> 16, mu); }
 }
 
 // S6: x += h v (Eq. 6); q <- normalise(q + h/2 [0,w] (x) q) (Eq. 2, world-frame
@@ -348,10 +458,10 @@ __device__ inline void integrate(const Smem& s, const Params& P, unsigned* statu
   for (int j = 0; j < nph; ++j) {
     const int w = s.ph[j], k = (w & 0xffff) + lane;
     float4 nn = make_float4(0, 0, 0, 0);
-    if (lane < (w >> 16)) nn = slot4(s, 1, k);
+    if (lane < (w >> 16)) nn = hdr4(s, 1, k);
     if (__any_sync(kFull, nn.w > 0.0f)) {
       if (nn.w > 0.0f) {
-        const float4 hd = slot4(s, 0, k);
+        const float4 hd = hdr4(s, 0, k);
         const int a = __float_as_int(hd.x), b = __float_as_int(hd.y);
         float4 xb = bd4(s, b, 0);
         if (xb.w != 0.0f) {
@@ -375,14 +485,16 @@ __device__ inline void integrate(const Smem& s, const Params& P, unsigned* statu
 
 // S7: every pair's impulses and contact points become the next substep's warm-start cache, in ascending
 // pair order (cache entry r = pair rank r).  Returns the lane's (contacts, ground contacts) for the counters.
+template <bool TM>
 __device__ inline int2 store_cache(const Smem& s, const Params& P, int env, int n_coll) {
   const int lane = lane_id();
   int nc = 0, ng = 0;
-  for (int base = 0; base < n_coll; base += 32) {
-    const int k = base + lane;
+  for (int j = 0; 32 * j < n_coll; ++j) {
+    const int k = 32 * j + lane;
+    PairC c; round_load<TM>(s, j, n_coll, c);
     if (k < n_coll) {
       const int r = s.order[k];
-      const float4 hd = slot4(s, 0, k);
+      const float4 hd = hdr4(s, 0, k);
       const int meta = __float_as_int(hd.z), np = meta & 0xff;
       nc += np; if (__float_as_int(hd.x) < 0) ng += np;
       int* key = P.cache_key + ((size_t)env * P.pc + r) * 2;
@@ -390,11 +502,10 @@ __device__ inline int2 store_cache(const Smem& s, const Params& P, int env, int 
       float* ol = P.cache_lam + ((size_t)env * P.pc + r) * 12;
       float* op = P.cache_pt + ((size_t)env * P.pc + r) * 12;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const float4 p4 = slot4(s, 2 + 3 * c, k), l4 = slot4(s, 4 + 3 * c, k);
-        const bool on = c < np;
-        ol[3 * c] = on ? l4.y : 0.0f; ol[3 * c + 1] = on ? l4.z : 0.0f; ol[3 * c + 2] = on ? l4.w : 0.0f;
-        op[3 * c] = p4.x; op[3 * c + 1] = p4.y; op[3 * c + 2] = p4.z;
+      for (int ci = 0; ci < 4; ++ci) {
+        const bool on = ci < np;
+#pragma unroll
+        for (int t = 0; t < 3; ++t) { ol[3 * ci + t] = on ? c.v[kLam + 3 * ci + t] : 0.0f; op[3 * ci + t] = c.v[9 * ci + t]; }
       }
     }
   }
@@ -458,14 +569,18 @@ __device__ inline int write_contacts(const Smem& s, const Params& P, int env, in
 }
 
 // lambda in contact order; needs s.wrank[r] = contact offset of pair r.
+template <bool TM>
 __device__ inline void write_lambda(const Smem& s, const Params& P, int env, int n_coll) {
-  for (int r = lane_id(); r < n_coll; r += 32) {
-    const int k = s.pos[r];
-    const int np = __float_as_int(slot4(s, 0, k).z) & 0xff;
-    float* out = P.lambda + ((size_t)env * P.max_contacts + s.wrank[r]) * 3;
-    for (int c = 0; c < np; ++c) {
-      const float4 l4 = slot4(s, 4 + 3 * c, k);
-      out[3 * c] = l4.y; out[3 * c + 1] = l4.z; out[3 * c + 2] = l4.w;
+  for (int j = 0; 32 * j < n_coll; ++j) {
+    const int k = 32 * j + lane_id();
+    PairC c; round_load<TM>(s, j, n_coll, c);
+    if (k < n_coll) {
+      const int r = s.order[k];
+      const int np = __float_as_int(hdr4(s, 0, k).z) & 0xff;
+      float* out = P.lambda + ((size_t)env * P.max_contacts + s.wrank[r]) * 3;
+#pragma unroll
+      for (int ci = 0; ci < 4; ++ci)
+        if (ci < np) { out[3 * ci] = c.v[kLam + 3 * ci]; out[3 * ci + 1] = c.v[kLam + 3 * ci + 1]; out[3 * ci + 2] = c.v[kLam + 3 * ci + 2]; }
     }
   }
 }
