@@ -153,6 +153,36 @@ __device__ __forceinline__ bool sat_boxes(const CollideParams& cp, const Box& A,
   return true;
 }
 
+__device__ __forceinline__ Vec3 pick3(const Vec3* a, int k) { return k == 0 ? a[0] : (k == 1 ? a[1] : a[2]); }
+__device__ __forceinline__ float pickf(const float* a, int k) { return k == 0 ? a[0] : (k == 1 ? a[1] : a[2]); }
+
+// Normal and overlap of ONE axis of a pair that sat_boxes found overlapping with this axis chosen: the same
+// expressions as in sat_boxes (same fused multiply-adds), so the values are identical bit for bit.
+__device__ __forceinline__ void sat_axis(const Box& A, const Box& B, int axis, SatResult& r) {
+  const Vec3 t = B.c - A.c;
+  Vec3 n; float delta;
+  if (axis < 3) {
+    n = pick3(A.ax, axis);
+    const float rB = absdot3(B.he, dot(n, B.ax[0]), dot(n, B.ax[1]), dot(n, B.ax[2]));
+    delta = pickf(A.he, axis) + rB - fabsf(dot(t, n));
+  } else if (axis < 6) {
+    n = pick3(B.ax, axis - 3);
+    const float rA = absdot3(A.he, dot(A.ax[0], n), dot(A.ax[1], n), dot(A.ax[2], n));
+    delta = rA + pickf(B.he, axis - 3) - fabsf(dot(t, n));
+  } else {
+    const int i = (axis - 6) / 3, j = (axis - 6) - 3 * i;
+    Vec3 u = cross(pick3(A.ax, i), pick3(B.ax, j));
+    const float inv = 1.0f / sqrtf(dot(u, u));
+    u = inv * u;
+    const float rA = absdot3(A.he, dot(A.ax[0], u), dot(A.ax[1], u), dot(A.ax[2], u));
+    const float rB = absdot3(B.he, dot(B.ax[0], u), dot(B.ax[1], u), dot(B.ax[2], u));
+    delta = rA + rB - fabsf(dot(t, u));
+    n = u;
+  }
+  if (dot(n, t) < 0.0f) n = -n;
+  r.axis = axis; r.n = n; r.delta = delta;
+}
+
 // Ground: colliding iff a corner lies below z = 0 (reading A9).
 __device__ __forceinline__ bool ground_hit(const Box& b) {
   // lowest corner z = c.z - sum_k |ax_k.z| he_k  is NOT used: the per-corner sums below are the ones
@@ -211,14 +241,18 @@ __device__ inline void manifold_boxes(const Box& A, const Box& B, const SatResul
     for (int k = 0; k < 4; ++k) inc[k] = poly0[k];
   }
   const int u = (r == 0) ? 1 : 0, v = (r == 2) ? 1 : 2;
-  int np = clip_halfspace(poly0, 4, poly1, X.c, X.ax[u], 1.0f, X.he[u]);
-  if (np) np = clip_halfspace(poly1, np, poly0, X.c, X.ax[u], -1.0f, X.he[u]);
-  if (np) np = clip_halfspace(poly0, np, poly1, X.c, X.ax[v], 1.0f, X.he[v]);
-  if (np) np = clip_halfspace(poly1, np, poly0, X.c, X.ax[v], -1.0f, X.he[v]);
+  int np = 4;
+  Vec3 *pin = poly0, *pout = poly1;
+#pragma unroll 1
+  for (int pl = 0; pl < 4 && np; ++pl) {      // side planes +u, -u, +v, -v of the reference face (one copy of the clip code)
+    const int w = pl < 2 ? u : v;
+    np = clip_halfspace(pin, np, pout, X.c, X.ax[w], (pl & 1) ? -1.0f : 1.0f, X.he[w]);
+    Vec3* t = pin; pin = pout; pout = t;
+  }
   Vec3 cpt[8]; float cd[8]; int nc = 0;
   for (int k = 0; k < np; ++k) {
-    float d = X.he[r] - dot(poly0[k] - X.c, nref);
-    if (d >= 0.0f) { cpt[nc] = madd(poly0[k], 0.5f * d, nref); cd[nc] = d; ++nc; }
+    float d = X.he[r] - dot(pin[k] - X.c, nref);
+    if (d >= 0.0f) { cpt[nc] = madd(pin[k], 0.5f * d, nref); cd[nc] = d; ++nc; }
   }
   if (nc == 0) {                            // fallback: deepest incident vertex, SAT depth
     int bi = 0; float bd = -3.0e38f;

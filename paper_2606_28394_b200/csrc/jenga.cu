@@ -56,27 +56,43 @@ __device__ __forceinline__ void end_warp(const Smem& s) {
 }
 
 // ---------------------------------------------------------------- fused step
+// The 4 warps of a TMEM-kernel CTA meet at a CTA barrier before and after the PGS sweeps of every substep: they then
+// run the same code region at the same time, which keeps the instruction working set of an SM (32 KB L1.5 I-cache)
+// to two regions instead of eight (profiles/r1d: `no_instruction` was the top stall with 8 free-running warps).
 template <bool TM>
 __global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const int n_steps) {
   int env;
   const Smem s = begin_warp<TM>(P, env);
   const int lane = lane_id();
-  if (env < P.E) {
+  const bool valid = env < P.E;
+  float mu = 0.0f;
+  if (valid) {
     load_env(s, P, env);
     if (lane == 0) { s.misc[MiNprev] = -1; s.misc[MiNph] = 0; s.misc[MiNcol] = 0; }
     __syncwarp();
-    const float mu = P.mu[env];
-    unsigned st = 0;
-    unsigned long long c_cand = 0, c_coll = 0, c_cont = 0, c_gcont = 0, c_col = 0;
-    int m_cand = 0, m_coll = 0, m_col = 0, cur = 0;
-    const int n_sub = n_steps * P.n_substeps;
-    for (int sub = 0; sub < n_sub; ++sub) {
+    mu = P.mu[env];
+  }
+  unsigned st = 0;
+  unsigned long long c_cand = 0, c_coll = 0, c_cont = 0, c_gcont = 0, c_col = 0;
+  int m_cand = 0, m_coll = 0, m_col = 0, cur = 0;
+  const int n_sub = n_steps * P.n_substeps;
+  for (int sub = 0; sub < n_sub; ++sub) {
+    int n_cand = 0, n_coll = 0;
+    if (valid) {
       pose_and_predict(s, P, env, true);
-      const int n_cand = broadphase(s, P, &st);
-      const int n_coll = find_colliding(s, P, n_cand, cur, &st);
+      n_cand = broadphase(s, P, &st);
+    }
+    if (TM) __syncthreads();
+    if (valid) {
+      n_coll = find_colliding(s, P, n_cand, cur, &st);
       colour_pairs<TM>(s, P, n_coll, cur, &st);
-      setup_pairs<TM>(s, P, env, n_coll, cur);
-      pgs_sweeps<TM>(s, P, P.iters, mu);
+    }
+    if (TM) __syncthreads();
+    if (valid) setup_pairs<TM>(s, P, env, n_coll, cur);
+    if (TM) __syncthreads();
+    if (valid) pgs_sweeps<TM>(s, P, P.iters, mu);
+    if (TM) __syncthreads();
+    if (valid) {
       if (P.materialise && sub == n_sub - 1) {
         write_pairs(s, P, env, n_cand);
         write_contacts(s, P, env, n_cand, n_coll, cur);
@@ -93,6 +109,8 @@ __global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const in
       cur ^= 1;
       __syncwarp();
     }
+  }
+  if (valid) {
     store_env(s, P, env);
     flush_status(P, env, st);
     if (P.counters) {
@@ -167,7 +185,7 @@ __device__ inline int pairs_from_contacts(const Smem& s, const Params& P, int en
     if (first && rank < P.pc) {
       const int idx = pairs[tag & 0xffff];
       int i, j; pair_bodies(P.B, idx, i, j);
-      s.cpair[0][rank] = (unsigned short)idx; s.cab[rank] = pack_ab(s, i, j); s.wrank[rank] = (unsigned short)c;
+      s.cpair[0][rank] = (unsigned short)idx; s.cab[rank] = pack_ab(s, i, j, (tag >> 20) & 0xf); s.wrank[rank] = (unsigned short)c;
     }
     n += __popc(bal);
   }

@@ -15,15 +15,25 @@ __device__ __forceinline__ Box load_box(const Smem& s, int S, int b) {
   return X;
 }
 
-// cab word of a colliding pair: (a+1) bits 0-10 | A dynamic bit 11 | b bits 16-26 | B dynamic bit 27
-__device__ __forceinline__ unsigned pack_ab(const Smem& s, int a, int b) {
-  unsigned w = (unsigned)(a + 1) | ((unsigned)b << 16);
+// cab word of a colliding pair: (a+1) bits 0-10 | A dynamic bit 11 | SAT axis bits 12-15 | b bits 16-26 | B dynamic bit 27
+__device__ __forceinline__ unsigned pack_ab(const Smem& s, int a, int b, int axis) {
+  unsigned w = (unsigned)(a + 1) | ((unsigned)axis << 12) | ((unsigned)b << 16);
   if (a >= 0 && s.bd[a * kBd + 3] != 0.0f) w |= 1u << 11;
   if (s.bd[b * kBd + 3] != 0.0f) w |= 1u << 27;
   return w;
 }
 __device__ __forceinline__ int ab_a(unsigned w) { return (int)(w & 0x7ffu) - 1; }
 __device__ __forceinline__ int ab_b(unsigned w) { return (int)((w >> 16) & 0x7ffu); }
+__device__ __forceinline__ int ab_axis(unsigned w) { return (int)((w >> 12) & 0xfu); }
+
+// Manifold of colliding pair (a, b) whose SAT axis is known (find_colliding stored it).
+__device__ __forceinline__ void pair_manifold(const Smem& s, int S, int a, int b, int axis, Manifold& m) {
+  const Box Bj = load_box(s, S, b);
+  if (a < 0) { collide_ground(Bj, m); return; }
+  const Box Bi = load_box(s, S, a);
+  SatResult sr; sat_axis(Bi, Bj, axis, sr);
+  manifold_boxes(Bi, Bj, sr, m);
+}
 
 // S3, first half: which candidates collide (15-axis SAT / a ground corner below z = 0).  Lane k of a
 // round takes candidate base+k; the colliding ones are compacted in ascending pair index into
@@ -34,17 +44,17 @@ __device__ inline int find_colliding(const Smem& s, const Params& P, int n_cand,
   int n = 0;
   for (int base = 0; base < n_cand; base += 32) {
     const int k = base + lane;
-    bool hit = false; int idx = 0, i = -1, j = 0;
+    bool hit = false; int idx = 0, i = -1, j = 0, axis = JENGA_AXIS_GROUND;
     if (k < n_cand) {
       idx = s.cand[k];
       pair_bodies(P.B, idx, i, j);
       const Box Bj = load_box(s, S, j);
       if (i < 0) hit = ground_hit(Bj);
-      else { const Box Bi = load_box(s, S, i); SatResult sr; hit = sat_boxes(P.cp, Bi, Bj, sr); }
+      else { const Box Bi = load_box(s, S, i); SatResult sr; sr.axis = 0; hit = sat_boxes(P.cp, Bi, Bj, sr); axis = sr.axis; }
     }
     const unsigned bal = __ballot_sync(kFull, hit);
     const int rank = n + __popc(bal & below);
-    if (hit && rank < P.pc) { s.cpair[cur][rank] = (unsigned short)idx; s.cab[rank] = pack_ab(s, i, j); }
+    if (hit && rank < P.pc) { s.cpair[cur][rank] = (unsigned short)idx; s.cab[rank] = pack_ab(s, i, j, axis); }
     n += __popc(bal);
   }
   if (n > P.pc) { *status |= JENGA_ST_CONTACT_OVERFLOW; n = P.pc; }
@@ -312,9 +322,7 @@ __device__ inline void setup_pairs(const Smem& s, const Params& P, int env, int 
       const unsigned w = s.cab[r];
       const int a = ab_a(w), b = ab_b(w);
       Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
-      const Box Bj = load_box(s, S, b);
-      if (a < 0) collide_ground(Bj, m);
-      else { const Box Bi = load_box(s, S, a); collide_boxes(P.cp, Bi, Bj, m); }
+      pair_manifold(s, S, a, b, ab_axis(w), m);
       setup_slot(s, P, env, k, a, b, s.cpair[cur][r], m, c);
     }
     round_store<TM>(s, j, n_coll, c);
@@ -544,9 +552,7 @@ __device__ inline int write_contacts(const Smem& s, const Params& P, int env, in
       const unsigned w = s.cab[r];
       const int a = ab_a(w), b = ab_b(w);
       idx = s.cpair[cur][r];
-      const Box Bj = load_box(s, S, b);
-      if (a < 0) collide_ground(Bj, m);
-      else { const Box Bi = load_box(s, S, a); collide_boxes(P.cp, Bi, Bj, m); }
+      pair_manifold(s, S, a, b, ab_axis(w), m);
     }
     int tot; const int off = off0 + warp_excl_scan(m.np, &tot);
     if (r < n_coll) {
