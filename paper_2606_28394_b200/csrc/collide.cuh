@@ -198,84 +198,98 @@ __device__ __forceinline__ bool ground_hit(const Box& b) {
 }
 
 // Contact manifold for an overlapping pair (PAPER.md:273-280 read as A8).
+__device__ __forceinline__ Vec3 sel3(bool c, Vec3 a, Vec3 b) { return v3(c ? a.x : b.x, c ? a.y : b.y, c ? a.z : b.z); }
+
+// Only the clip polygons and the candidate points are indexed dynamically (thread-local arrays); the boxes, the
+// reference / incident frames and the result stay in registers (axis choices go through select chains).
 __device__ inline void manifold_boxes(const Box& A, const Box& B, const SatResult& sr, Manifold& m) {
   const int ax = sr.axis; const Vec3 n = sr.n; const float delta = sr.delta;
   m.axis = ax; m.n = n; m.np = 0;
 
   if (ax >= 6) {                            // edge-edge: closest points of the two support edges
-    const int i = (ax - 6) / 3, j = (ax - 6) % 3;
+    const int i = (ax - 6) / 3, j = (ax - 6) - 3 * i;
     Vec3 pa = A.c, pb = B.c;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-      if (k != i) { float s = dot(A.ax[k], n) >= 0.0f ? 1.0f : -1.0f; pa = madd(pa, s * A.he[k], A.ax[k]); }
-      if (k != j) { float s = dot(B.ax[k], n) >= 0.0f ? 1.0f : -1.0f; pb = madd(pb, -s * B.he[k], B.ax[k]); }
+      const float sa = dot(A.ax[k], n) >= 0.0f ? 1.0f : -1.0f, sb = dot(B.ax[k], n) >= 0.0f ? 1.0f : -1.0f;
+      const Vec3 qa = madd(pa, sa * A.he[k], A.ax[k]), qb = madd(pb, -sb * B.he[k], B.ax[k]);
+      pa = sel3(k != i, qa, pa); pb = sel3(k != j, qb, pb);
     }
-    const Vec3 ai = A.ax[i], bj = B.ax[j], r = pa - pb;
+    const Vec3 ai = pick3(A.ax, i), bj = pick3(B.ax, j), r = pa - pb;
+    const float hi = pickf(A.he, i), hj = pickf(B.he, j);
     const float bb = dot(ai, bj), cc = dot(ai, r), ff = dot(bj, r), den = 1.0f - bb * bb;
     float sA = (bb * ff - cc) / den, sB = (ff - bb * cc) / den;
-    sA = fminf(fmaxf(sA, -A.he[i]), A.he[i]);
-    sB = fminf(fmaxf(sB, -B.he[j]), B.he[j]);
+    sA = fminf(fmaxf(sA, -hi), hi);
+    sB = fminf(fmaxf(sB, -hj), hj);
     m.p[0] = 0.5f * (madd(pa, sA, ai) + madd(pb, sB, bj));
     m.d[0] = delta; m.np = 1;
     return;
   }
 
   // face case: X owns the axis (reference), Y is the other (incident)
-  const bool refA = ax < 3; const int r = ax % 3;
-  const Box& X = refA ? A : B; const Box& Y = refA ? B : A;
+  const bool refA = ax < 3; const int r = refA ? ax : ax - 3;
+  Vec3 Xax[3], Yax[3]; float Xhe[3], Yhe[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    Xax[k] = sel3(refA, A.ax[k], B.ax[k]); Yax[k] = sel3(refA, B.ax[k], A.ax[k]);
+    Xhe[k] = refA ? A.he[k] : B.he[k];     Yhe[k] = refA ? B.he[k] : A.he[k];
+  }
+  const Vec3 Xc = sel3(refA, A.c, B.c), Yc = sel3(refA, B.c, A.c);
   const Vec3 nref = refA ? n : -n;
   int mi = 0; float sg = -1.0f, best = 3.0e38f;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    float dk = dot(Y.ax[k], nref);
+    float dk = dot(Yax[k], nref);
     if (-dk < best) { best = -dk; mi = k; sg = -1.0f; }
     if (dk < best) { best = dk; mi = k; sg = 1.0f; }
   }
   const int iu = (mi == 0) ? 1 : 0, iv = (mi == 2) ? 1 : 2;
   Vec3 poly0[8], poly1[8], inc[4];
   {
-    const Vec3 fc = madd(Y.c, sg * Y.he[mi], Y.ax[mi]);
-    const Vec3 eu = Y.he[iu] * Y.ax[iu], ev = Y.he[iv] * Y.ax[iv];
-    poly0[0] = fc - eu - ev; poly0[1] = fc + eu - ev; poly0[2] = fc + eu + ev; poly0[3] = fc - eu + ev;
+    const Vec3 fc = madd(Yc, sg * pickf(Yhe, mi), pick3(Yax, mi));
+    const Vec3 eu = pickf(Yhe, iu) * pick3(Yax, iu), ev = pickf(Yhe, iv) * pick3(Yax, iv);
+    inc[0] = fc - eu - ev; inc[1] = fc + eu - ev; inc[2] = fc + eu + ev; inc[3] = fc - eu + ev;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) inc[k] = poly0[k];
+    for (int k = 0; k < 4; ++k) poly0[k] = inc[k];
   }
   const int u = (r == 0) ? 1 : 0, v = (r == 2) ? 1 : 2;
+  const Vec3 xu = pick3(Xax, u), xv = pick3(Xax, v);
+  const float hu = pickf(Xhe, u), hv = pickf(Xhe, v), hr = pickf(Xhe, r);
   int np = 4;
   Vec3 *pin = poly0, *pout = poly1;
 #pragma unroll 1
   for (int pl = 0; pl < 4 && np; ++pl) {      // side planes +u, -u, +v, -v of the reference face (one copy of the clip code)
-    const int w = pl < 2 ? u : v;
-    np = clip_halfspace(pin, np, pout, X.c, X.ax[w], (pl & 1) ? -1.0f : 1.0f, X.he[w]);
+    np = clip_halfspace(pin, np, pout, Xc, pl < 2 ? xu : xv, (pl & 1) ? -1.0f : 1.0f, pl < 2 ? hu : hv);
     Vec3* t = pin; pin = pout; pout = t;
   }
   Vec3 cpt[8]; float cd[8]; int nc = 0;
   for (int k = 0; k < np; ++k) {
-    float d = X.he[r] - dot(pin[k] - X.c, nref);
+    float d = hr - dot(pin[k] - Xc, nref);
     if (d >= 0.0f) { cpt[nc] = madd(pin[k], 0.5f * d, nref); cd[nc] = d; ++nc; }
   }
   if (nc == 0) {                            // fallback: deepest incident vertex, SAT depth
-    int bi = 0; float bd = -3.0e38f;
+    Vec3 bp = inc[0]; float bd = -3.0e38f;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      float d = X.he[r] - dot(inc[k] - X.c, nref);
-      if (d > bd) { bd = d; bi = k; }
+      float d = hr - dot(inc[k] - Xc, nref);
+      if (d > bd) { bd = d; bp = inc[k]; }
     }
-    m.p[0] = madd(inc[bi], 0.5f * delta, nref); m.d[0] = delta; m.np = 1;
+    m.p[0] = madd(bp, 0.5f * delta, nref); m.d[0] = delta; m.np = 1;
     return;
   }
   unsigned keep = (1u << nc) - 1u;
   if (nc > 4) {                             // <= 4 reduction (DESIGN §2 S3)
     int i0 = 0, i1 = -1, i2 = -1, i3 = -1; float far2 = -1.0f, amax = 0.0f, amin = 0.0f;
     for (int k = 1; k < nc; ++k) if (cd[k] > cd[i0]) i0 = k;
+    const Vec3 p0 = cpt[i0];
     for (int k = 0; k < nc; ++k) if (k != i0) {
-      Vec3 d = cpt[k] - cpt[i0]; float dd = dot(d, d);
+      Vec3 d = cpt[k] - p0; float dd = dot(d, d);
       if (dd > far2) { far2 = dd; i1 = k; }
     }
-    const Vec3 e01 = cpt[i1] - cpt[i0];
+    const Vec3 e01 = cpt[i1] - p0;
     for (int k = 0; k < nc; ++k) {
       if (k == i0 || k == i1) continue;
-      float area = dot(cross(e01, cpt[k] - cpt[i0]), n);
+      float area = dot(cross(e01, cpt[k] - p0), n);
       if (area > amax) { amax = area; i2 = k; }
       if (area < amin) { amin = area; i3 = k; }
     }
@@ -283,8 +297,10 @@ __device__ inline void manifold_boxes(const Box& A, const Box& B, const SatResul
     if (i2 >= 0) keep |= 1u << i2;
     if (i3 >= 0) keep |= 1u << i3;
   }
-  int no = 0;
-  for (int k = 0; k < nc; ++k) if ((keep >> k) & 1u) { m.p[no] = cpt[k]; m.d[no] = cd[k]; ++no; }
+  const int no = __popc(keep);              // survivors in ascending clip-output index; static output slots
+#pragma unroll
+  for (int o = 0; o < 4; ++o)
+    if (o < no) { const int k = __fns(keep, 0, o + 1); m.p[o] = cpt[k]; m.d[o] = cd[k]; }
   m.np = no;
 }
 

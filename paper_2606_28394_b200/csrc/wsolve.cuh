@@ -229,7 +229,7 @@ __device__ __forceinline__ Vec3 xyz(float4 v) { return v3(v.x, v.y, v.z); }
 // contact inherits (jn,jt1,jt2) of the nearest not yet taken previous contact point of the same pair
 // within match_tol; slots ascending.
 __device__ inline void setup_slot(const Smem& s, const Params& P, int env, int k, int a, int b, int pair,
-                                  const Manifold& m, PairC& out) {
+                                  const Manifold& m, PairC& out, int prev_buf = 0) {
   Body5 A, Bb; load_body(s, a, A, false); load_body(s, b, Bb, false);
   const Vec3 n = m.n;
   Vec3 u; tangent_raw(n, u);
@@ -245,11 +245,21 @@ __device__ inline void setup_slot(const Smem& s, const Params& P, int env, int k
   for (int c = 0; c < 4; ++c) if (c < m.np) { pt[c] = m.p[c]; dmax = fmaxf(dmax, m.d[c]); }
 
   if (P.warm_start) {
-    const int nk = P.n_cache[env];
+    // cache entry = rank of the pair in the previous substep's colliding list: that list is still in shared memory
+    // (s.cpair[prev]) inside a launch; at the first substep of a launch the keys are read from HBM.
     const int* keys = P.cache_key + (size_t)env * P.pc * 2;
-    int lo = 0, hi = nk;
-    while (lo < hi) { const int mid = (lo + hi) >> 1; if (keys[2 * mid] < pair) lo = mid + 1; else hi = mid; }
-    if (lo < nk && keys[2 * lo] == pair) {
+    const int nprev = s.misc[MiNprev];
+    int nk, lo = 0; bool found;
+    if (nprev >= 0) {
+      nk = nprev; int hi = nk;
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)s.cpair[prev_buf][mid] < pair) lo = mid + 1; else hi = mid; }
+      found = lo < nk && (int)s.cpair[prev_buf][lo] == pair;
+    } else {
+      nk = P.n_cache[env]; int hi = nk;
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if (keys[2 * mid] < pair) lo = mid + 1; else hi = mid; }
+      found = lo < nk && keys[2 * lo] == pair;
+    }
+    if (found) {
       const int ocnt = keys[2 * lo + 1] & 0xff;
       const float* ol = P.cache_lam + ((size_t)env * P.pc + lo) * 12;
       const float* op = P.cache_pt + ((size_t)env * P.pc + lo) * 12;
@@ -323,7 +333,7 @@ __device__ inline void setup_pairs(const Smem& s, const Params& P, int env, int 
       const int a = ab_a(w), b = ab_b(w);
       Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
       pair_manifold(s, S, a, b, ab_axis(w), m);
-      setup_slot(s, P, env, k, a, b, s.cpair[cur][r], m, c);
+      setup_slot(s, P, env, k, a, b, s.cpair[cur][r], m, c, cur ^ 1);
     }
     round_store<TM>(s, j, n_coll, c);
   }
