@@ -81,6 +81,7 @@ __global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const in
     if (valid) {
       pose_and_predict(s, P, env, true);
       n_cand = broadphase(s, P, &st);
+      if (P.materialise && sub == n_sub - 1) write_pairs(s, P, env, n_cand);   // before the slots overwrite the list
     }
     if (TM) __syncthreads();
     if (valid) {
@@ -94,7 +95,6 @@ __global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const in
     if (TM) __syncthreads();
     if (valid) {
       if (P.materialise && sub == n_sub - 1) {
-        write_pairs(s, P, env, n_cand);
         write_contacts(s, P, env, n_cand, n_coll, cur);
         write_lambda<TM>(s, P, env, n_coll);
       }

@@ -315,6 +315,9 @@ def test_single_step_pose(orc, J, name, cfg, E, steps):
             continue
         n_ok += 1
         assert int(world.n_pairs[e].item()) == len(tr["pairs"])
+        assert np.array_equal(world.pairs[e, :len(tr["pairs"])].cpu().numpy(), tr["pairs"])      # materialised outputs of the fused step
+        gc = gpu_contacts(world, e); rc = tr["contacts"].trimmed()
+        assert np.array_equal(np.asarray(tr["pairs"])[gc["cand"]], rc["pair"]) and np.array_equal(gc["slot"], rc["slot"])
         x = np.transpose(g[e, 0:3, :B]); q = np.transpose(g[e, 3:7, :B])
         assert np.max(np.abs(x - bod.x[e])) < TOL_POS, f"{name} env {e}: position error {np.max(np.abs(x - bod.x[e])):.3e}"
         ang = rotation_angle(q, bod.q[e])
@@ -412,3 +415,99 @@ def test_rollout_collapse_agreement(orc, J):
     # the same rate under a 1e-7 m input change.  The test holds the CUDA path to the oracle's own sensitivity.
     assert agree[far].mean() >= 0.975
     assert agree[far].mean() >= self_agree[far].mean() - 0.01
+
+
+# ----------------------------------------------------------------------------- full size, edge cases, untested parameters
+def test_full_size_cfg5_sampled_envs(orc, J):
+    """BASELINE.json configs[4] at its full size, in the launch shape bench.py times (65,536 envs, jenga_step(12) is
+    n x jenga_step(1) bit for bit, see above): one step from the seeded initial state, poses of sampled envs against
+    the oracle within the single-step tolerance; every env keeps a clean status and every active body stays finite."""
+    import torch
+    E = 65536
+    wl = W.make_config(5, n_envs=E)
+    world = J.World(wl.params, wl.state, wl.props, wl.mu)
+    assert world.launch_info()["threads"] in (32, 128)
+    world.step(1); torch.cuda.synchronize()
+    assert int(world.status.max().item()) == 0 and bool(torch.isfinite(world.state).all().item())
+    cnt = world.counters_dict()
+    assert cnt["env_steps"] == E and cnt["body_steps"] == int((wl.props[:, 7, :] != 0).sum())
+    sample = np.unique(np.concatenate([[0, 1, E - 1, E - 2], np.random.default_rng(11).integers(0, E, 28)]))
+    g = world.state[torch.as_tensor(sample).to(world.dev)].cpu().numpy().astype(np.float64)
+    B = wl.params.n_bodies
+    wp = W.make_config(5, n_envs=1).params
+    P = orc.make_params(wp)
+    for n, e in enumerate(sample):
+        bod = orc.unpack_tiles(wl.state[e:e + 1], wl.props[e:e + 1], B)
+        orc.step_env(P, bod, float(wl.mu[e]), e=0, cache=orc.Cache(1, wp.max_contacts))
+        x = np.transpose(g[n, 0:3, :B]); q = np.transpose(g[n, 3:7, :B])
+        assert np.max(np.abs(x - bod.x[0])) < TOL_POS, f"env {e}: position error {np.max(np.abs(x - bod.x[0])):.3e}"
+        assert np.max(rotation_angle(q, bod.q[0])) < TOL_ANG
+    world.destroy()
+
+
+def test_empty_and_single_body_envs(orc, J):
+    """Degenerate envs: all bodies inactive (nothing moves, no pairs), and one free block that falls and lands."""
+    import torch
+    wl = W.make_config(2, n_envs=3)
+    wl.props[1, 7, :] = 0.0                                    # env 1: every body removed
+    world = J.World(wl.params, wl.state, wl.props, wl.mu, materialise=True)
+    world.step(5); torch.cuda.synchronize()
+    assert torch.equal(world.state[1].cpu(), torch.as_tensor(wl.state[1]))
+    assert int(world.n_pairs[1].item()) == 0 and int(world.n_contacts[1].item()) == 0 and int(world.n_cache[1].item()) == 0
+    assert int(world.status.max().item()) == 0
+    one = W.make_custom([dict(pos=(0, 0, 0.0076), size=(W.BLOCK_L, W.BLOCK_W, W.BLOCK_H), mass=W.BLOCK_MASS)])
+    w1 = J.World(one.params, one.state, one.props, one.mu)
+    P = orc.make_params(one.params); bod = orc.unpack_tiles(one.state, one.props, 1); cache = orc.Cache(1, one.params.max_contacts)
+    for _ in range(30):
+        w1.step(1); orc.step_env(P, bod, 0.4, e=0, cache=cache)
+    torch.cuda.synchronize()
+    g = w1.state.cpu().numpy().astype(np.float64)
+    assert abs(g[0, 2, 0] - bod.x[0, 0, 2]) < 5e-6 and abs(g[0, 2, 0] - 0.0075) < 5e-4      # resting on the ground
+
+
+def test_contact_overflow_truncates_like_the_oracle(orc, J):
+    """max_contacts/4 colliding pairs kept (lowest pair indices), CONTACT_OVERFLOW set, on both sides."""
+    import torch
+    wl = W.make_config(2, n_envs=2)
+    wl.params.max_contacts = 128                                # 32 pair slots < ~150 colliding pairs
+    world = J.World(wl.params, wl.state, wl.props, wl.mu, materialise=True)
+    world.step(1); torch.cuda.synchronize()
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(wl.state, wl.props, wl.params.n_bodies)
+    for e in range(2):
+        tr = orc.step_env(P, bod, float(wl.mu[e]), e=e, cache=orc.Cache(2, 128), trace=True)
+        assert tr["status"] & 2 and int(world.status[e].item()) == tr["status"]
+        got = gpu_contacts(world, e)
+        ref = tr["contacts"].trimmed()
+        assert got["n"] == len(ref["pair"]) and np.array_equal(np.asarray(tr["pairs"])[got["cand"]], ref["pair"])
+        B = wl.params.n_bodies
+        x = np.transpose(world.state[e, 0:3, :B].cpu().numpy().astype(np.float64))
+        assert np.max(np.abs(x - bod.x[e])) < TOL_POS
+
+
+def test_paper_parameter_set_single_step(orc, J):
+    """The paper's own parameters (Table 6): 81 x 26 x 18 mm blocks of 19.6 g, e = 0.10, three
+    substeps, 14 PGS iterations -- the parts of the step definition the five configs never touch (restitution,
+    n_substeps > 1).  A 4-level tower plus a block dropped onto it with 0.4 m/s, 10 steps, step by step."""
+    import torch
+    l, w, h, m = 0.081, 0.026, 0.018, 0.0196
+    bodies = []
+    for lv in range(4):
+        for sl in range(3):
+            off = (sl - 1) * (w + 0.0015)
+            pos = (0.0, off, h / 2 - 1e-4 + lv * (h - 1e-4)) if lv % 2 == 0 else (off, 0.0, h / 2 - 1e-4 + lv * (h - 1e-4))
+            yaw = 0.0 if lv % 2 == 0 else np.pi / 2
+            bodies.append(dict(pos=pos, quat=(np.cos(yaw / 2), 0, 0, np.sin(yaw / 2)), size=(l, w, h), mass=m))
+    bodies.append(dict(pos=(0.01, 0.005, 4 * h + 0.02), quat=(0.98, 0.1, 0.12, 0.08) / np.linalg.norm((0.98, 0.1, 0.12, 0.08)),
+                       size=(l, w, h), mass=m, vel=(0, 0, -0.4)))
+    wl = W.make_custom(bodies, mu=0.40, restitution=0.10, n_substeps=3, pgs_iters=14, max_pairs=256, max_contacts=512)
+    world = J.World(wl.params, wl.state, wl.props, wl.mu)
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(wl.state, wl.props, len(bodies)); cache = orc.Cache(1, 512)
+    worst = 0.0
+    for step in range(10):
+        world.step(1); orc.step_env(P, bod, 0.40, e=0, cache=cache)
+        torch.cuda.synchronize()
+        g = world.state.cpu().numpy().astype(np.float64)
+        x = np.transpose(g[0, 0:3, :len(bodies)])
+        worst = max(worst, float(np.max(np.abs(x - bod.x[0]))))
+    print(f"\n[paper params] 10 steps x 3 substeps, e = 0.10: max position difference {worst:.2e} m")
+    assert worst < 2e-5 and int(world.status.max().item()) == 0          # 30 substeps of accumulated fp32 rounding
