@@ -82,6 +82,8 @@ typedef struct {
   int32_t  materialise;                 /* 1: jenga_step also writes pairs/contacts/lambda of its last
                                            substep (debug / parity); 0: they stay on chip              */
   int32_t  device;                      /* CUDA device ordinal the buffers live on                     */
+  float    collapse_length;             /* block length l of Eq. 18; latch off if <= 0 */
+  float    collapse_fd, collapse_ek, collapse_theta;   /* f_d = 0.5, eps_k = 5e-5 J, theta_th = 30 deg in rad   */
 } jenga_world_desc;
 
 /* All DEVICE pointers, caller-owned, 16-byte aligned.  PC = max_contacts/4. */
@@ -105,6 +107,12 @@ typedef struct {
   int32_t     *n_cache;    /* [E]  number of valid cache pairs (0 = cold)                              */
   uint32_t    *status;     /* [E]  JENGA_ST_* flags, OR-ed in                                          */
   unsigned long long *counters; /* [JENGA_N_COUNTERS], may be NULL                                     */
+  /* Collapse latch (Eq. 18, reading A17), evaluated by jenga_step after every dt
+   * advance; all three may be NULL (latch off).                                                        */
+  const float *ref_pose;   /* [E][7][S]  px py pz qw qx qy qz of the reference (initial) pose           */
+  int32_t     *collapsed;  /* [E]  OR-latched: 1 once dx_max > f_d l, theta_max > theta_th and E_k > eps_k
+                                   held at the same step                                                */
+  float       *collapse_stats; /* [E][4] of the last step: dx_max [m], E_k [J], theta_max [rad], 0     */
 } jenga_buffers;
 
 /* Validates desc/buffers (sizes, alignment, device arch) and returns a host handle. */

@@ -32,12 +32,14 @@ class WorldDesc(C.Structure):
                 ("restitution", C.c_float), ("aabb_margin", C.c_float), ("baumgarte_beta", C.c_float), ("slop", C.c_float),
                 ("edge_bias_rel", C.c_float), ("edge_bias_abs", C.c_float), ("par_eps", C.c_float), ("tie_eps", C.c_float),
                 ("match_tol", C.c_float), ("warm_start", C.c_int32), ("gyroscopic", C.c_int32), ("max_pairs", C.c_int32),
-                ("max_contacts", C.c_int32), ("materialise", C.c_int32), ("device", C.c_int32)]
+                ("max_contacts", C.c_int32), ("materialise", C.c_int32), ("device", C.c_int32),
+                ("collapse_length", C.c_float), ("collapse_fd", C.c_float), ("collapse_ek", C.c_float), ("collapse_theta", C.c_float)]
 
 
 class Buffers(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("state", "props", "mu", "f_ext", "pairs", "n_pairs", "contacts", "n_contacts",
-                                          "lambda_", "cache_key", "cache_lam", "cache_pt", "n_cache", "status", "counters")]
+                                          "lambda_", "cache_key", "cache_lam", "cache_pt", "n_cache", "status", "counters",
+                                          "ref_pose", "collapsed", "collapse_stats")]
 
 
 def lib():
@@ -89,6 +91,8 @@ def make_desc(wp, materialise: bool = False, device: int = 0) -> WorldDesc:
     d.match_tol, d.warm_start, d.gyroscopic = wp.match_tol, wp.warm_start, wp.gyroscopic
     d.max_pairs, d.max_contacts = wp.max_pairs, wp.max_contacts
     d.materialise, d.device = int(materialise), device
+    d.collapse_length = getattr(wp, "collapse_length", 0.0)
+    d.collapse_fd, d.collapse_ek, d.collapse_theta = 0.5, 5.0e-5, 0.5235987755982988      # Eq. 18: f_d, eps_k [J], 30 deg
     return d
 
 
@@ -99,7 +103,7 @@ class World:
     they are copied to the device once here.  All methods enqueue on torch's current stream.
     """
 
-    def __init__(self, wp, state, props, mu, materialise: bool = False, device: int = 0):
+    def __init__(self, wp, state, props, mu, materialise: bool = False, device: int = 0, collapse_length: float = 0.0):
         if not torch.cuda.is_available():
             raise JengaError("no CUDA device: the Jenga step has no CPU path")
         self.wp = wp
@@ -125,12 +129,19 @@ class World:
         self.status = z((E,), torch.int32)
         self.counters = z((N_COUNTERS,), torch.int64)
         self.desc = make_desc(wp, materialise, device)
+        self.desc.collapse_length = float(collapse_length)
         b = Buffers()
         b.state, b.props, b.mu, b.f_ext = self.state.data_ptr(), self.props.data_ptr(), self.mu.data_ptr(), None
         b.pairs, b.n_pairs = self.pairs.data_ptr(), self.n_pairs.data_ptr()
         b.contacts, b.n_contacts, b.lambda_ = self.contacts.data_ptr(), self.n_contacts.data_ptr(), self.lam.data_ptr()
         b.cache_key, b.cache_lam, b.cache_pt = self.cache_key.data_ptr(), self.cache_lam.data_ptr(), self.cache_pt.data_ptr()
         b.n_cache, b.status, b.counters = self.n_cache.data_ptr(), self.status.data_ptr(), self.counters.data_ptr()
+        self.ref_pose = self.collapsed = self.collapse_stats = None
+        if collapse_length > 0.0:                      # Eq. 18 latch against the pose the world starts from
+            self.ref_pose = self.state[:, 0:7, :].contiguous()
+            self.collapsed = z((E,), torch.int32)
+            self.collapse_stats = z((E, 4), torch.float32)
+            b.ref_pose, b.collapsed, b.collapse_stats = self.ref_pose.data_ptr(), self.collapsed.data_ptr(), self.collapse_stats.data_ptr()
         self.bufs = b
         self.handle = C.c_void_p()
         _check(lib().jenga_world_create(C.byref(self.desc), C.byref(b), C.byref(self.handle)), "jenga_world_create")

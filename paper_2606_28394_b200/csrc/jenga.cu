@@ -99,6 +99,7 @@ __global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const in
         write_lambda<TM>(s, P, env, n_coll);
       }
       integrate(s, P, &st);
+      if (P.collapsed && (sub + 1) % P.n_substeps == 0) collapse_latch(s, P, env);
       const int2 cc = store_cache<TM>(s, P, env, n_coll);
       c_cont += cc.x; c_gcont += cc.y;
       const int ncol = s.misc[MiNcol];
@@ -341,6 +342,10 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.pairs = b->pairs; P.n_pairs = b->n_pairs; P.contacts = b->contacts; P.n_contacts = b->n_contacts; P.lambda = b->lambda;
   P.cache_key = b->cache_key; P.cache_lam = b->cache_lam; P.cache_pt = b->cache_pt; P.n_cache = b->n_cache;
   P.status = b->status; P.counters = b->counters;
+  const bool latch = d->collapse_length > 0.0f && b->ref_pose && b->collapsed;
+  P.ref_pose = latch ? b->ref_pose : nullptr; P.collapsed = latch ? b->collapsed : nullptr;
+  P.collapse_stats = latch ? b->collapse_stats : nullptr;
+  P.collapse_dx = d->collapse_fd * d->collapse_length; P.collapse_ek = d->collapse_ek; P.collapse_theta = d->collapse_theta;
   struct { const void* k; size_t smem; } kernels[] = {
     { w->tm ? (const void*)jenga::k_step<true> : (const void*)jenga::k_step<false>, w->smem_step },
     { w->tm ? (const void*)jenga::k_pgs<true> : (const void*)jenga::k_pgs<false>, w->smem_step },

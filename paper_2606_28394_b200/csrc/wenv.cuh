@@ -40,6 +40,8 @@ struct Params {
   int* pairs; int* n_pairs; float* contacts; int* n_contacts; float* lambda;
   int* cache_key; float* cache_lam; float* cache_pt; int* n_cache;
   unsigned* status; unsigned long long* counters;
+  const float* ref_pose; int* collapsed; float* collapse_stats;
+  float collapse_dx, collapse_ek, collapse_theta;           // f_d * l, eps_k, theta_th
 };
 
 // Every shared array is addressed as an offset into the one extern shared array, so that the compiler knows the

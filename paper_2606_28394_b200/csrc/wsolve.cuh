@@ -501,6 +501,41 @@ __device__ inline void integrate(const Smem& s, const Params& P, unsigned* statu
   }
 }
 
+// Collapse latch (Eq. 18, reading A17) after a dt advance: dx_max = max_b |x_b - x_b(0)|,
+// theta_max = max_b 2 acos|q_b . q_b(0)|, E_k = sum_b 1/2 m |v|^2 + 1/2 w . I_w w (body frame: R^T w against the
+// principal moments); collapsed |= all three above their thresholds at this step.
+__device__ inline void collapse_latch(const Smem& s, const Params& P, int env) {
+  const int S = P.S, lane = lane_id();
+  const float* ref = P.ref_pose + (size_t)env * 7 * S;
+  float dxm = 0.0f, thm = 0.0f, ek = 0.0f;
+  for (int b = lane; b < P.B; b += 32) {
+    const float4 x = bd4(s, b, 0);
+    if (x.w == 0.0f) continue;
+    const float dx = x.x - ref[b], dy = x.y - ref[S + b], dz = x.z - ref[2 * S + b];
+    dxm = fmaxf(dxm, sqrtf(dx * dx + dy * dy + dz * dz));
+    const float qw = s.q[b], qx = s.q[S + b], qy = s.q[2 * S + b], qz = s.q[3 * S + b];
+    const float c = fminf(fabsf(qw * ref[3 * S + b] + qx * ref[4 * S + b] + qy * ref[5 * S + b] + qz * ref[6 * S + b]), 1.0f);
+    thm = fmaxf(thm, 2.0f * acosf(c));
+    const float4 v = bd4(s, b, 1), w = bd4(s, b, 2);
+    // R^T w with R from the new q (Eq. 1)
+    const float r00 = 1.0f - 2.0f * (qy * qy + qz * qz), r01 = 2.0f * (qx * qy - qz * qw), r02 = 2.0f * (qx * qz + qy * qw);
+    const float r10 = 2.0f * (qx * qy + qz * qw), r11 = 1.0f - 2.0f * (qx * qx + qz * qz), r12 = 2.0f * (qy * qz - qx * qw);
+    const float r20 = 2.0f * (qx * qz - qy * qw), r21 = 2.0f * (qy * qz + qx * qw), r22 = 1.0f - 2.0f * (qx * qx + qy * qy);
+    const float w0 = r00 * w.x + r10 * w.y + r20 * w.z, w1 = r01 * w.x + r11 * w.y + r21 * w.z, w2 = r02 * w.x + r12 * w.y + r22 * w.z;
+    ek += 0.5f * (v.x * v.x + v.y * v.y + v.z * v.z) / x.w
+        + 0.5f * (w0 * w0 / s.pr[S + b] + w1 * w1 / s.pr[2 * S + b] + w2 * w2 / s.pr[3 * S + b]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    dxm = fmaxf(dxm, __shfl_xor_sync(kFull, dxm, o)); thm = fmaxf(thm, __shfl_xor_sync(kFull, thm, o));
+    ek += __shfl_xor_sync(kFull, ek, o);
+  }
+  if (lane == 0) {
+    if (dxm > P.collapse_dx && ek > P.collapse_ek && thm > P.collapse_theta) P.collapsed[env] = 1;
+    if (P.collapse_stats) *reinterpret_cast<float4*>(P.collapse_stats + (size_t)env * 4) = make_float4(dxm, ek, thm, 0.0f);
+  }
+}
+
 // S7: every pair's impulses and contact points become the next substep's warm-start cache, in ascending
 // pair order (cache entry r = pair rank r).  Returns the lane's (contacts, ground contacts) for the counters.
 template <bool TM>

@@ -402,10 +402,24 @@ def test_rollout_collapse_agreement(orc, J):
         world.step(1)
         got |= collapse_flags(world.state.cpu().numpy(), state, props, B)
     assert int(world.status.max().item()) == 0
+    # the kernel-side latch (jenga_step epilogue, NEXT-1) on the same trajectory, launched 12 steps at a time
+    w2 = J.World(wl.params, state, props, mu, collapse_length=W.BLOCK_L)
+    for lo, hi, f in ((0, wl.push_start, None), (wl.push_start, wl.push_end, fext), (wl.push_end, wl.n_steps, None)):
+        w2.set_f_ext(f)
+        for s0 in range(lo, hi, 12):
+            w2.step(min(12, hi - s0))
+    torch.cuda.synchronize()
+    assert torch.equal(w2.state, world.state)                       # n launches of 1 step == launches of 12, bit for bit
+    klatch = w2.collapsed.cpu().numpy() != 0
+    stats = w2.collapse_stats.cpu().numpy()
+    assert np.isfinite(stats).all() and (klatch == got).mean() >= 0.995, (klatch != got).sum()
+    last = collapse_flags(world.state.cpu().numpy(), state, props, B)          # stats are those of the last step
+    assert np.all(klatch >= last)
     far = np.abs(k - kthr) / kthr >= 0.1
     agree = (got == (ref != 0))
     for e in np.nonzero(~agree)[0]:
         print(f"  disagree: env {e} mu {mu[e]:.2f} k {k[e]:.3f} k_thr {kthr[e]:.0f} oracle {int(ref[e] != 0)} cuda {int(got[e])}")
+    print(f"[rollout] kernel latch vs harness latch on the CUDA trajectory: {int((klatch != got).sum())} of {E} differ")
     print(f"\n[rollout] {E} episodes, {int(far.sum())} with |k-k_thr|/k_thr >= 0.1: oracle collapses {int((ref != 0)[far].sum())}, "
           f"CUDA {int(got[far].sum())}, agreement {agree[far].mean():.3f} (all episodes: {agree.mean():.3f})")
     self_agree = ((ref != 0) == (ref2 != 0))
