@@ -252,31 +252,50 @@ def run_cuda(args) -> dict:
     n_flagged = int((world.status != 0).sum().item())
     assert cnt["env_steps"] == E * K, (cnt, E, K)
 
-    # ---- end to end through the C-ABI with HOST buffers: per step H2D of the state tile (pinned), step, D2H
-    reset()
-    h_a = torch.empty(world.state.shape, dtype=torch.float32, pin_memory=True)
-    h_b = torch.empty_like(h_a, pin_memory=True)
-    h_a.copy_(torch.as_tensor(wl.state))
-    h_fext = torch.as_tensor(wl.push_fext).pin_memory()
+    # ---- end to end through the C-ABI with HOST buffers: every step, for every env, H2D of the state tile (pinned
+    # memory), the step, D2H of the result (jenga_step_host).  The batch is served as `--e2e-split` worlds of E/split
+    # envs on their own streams, so that one part's copies overlap the other part's kernel (what a user of the
+    # library would do with a PCIe-bound call); the result of step s is the host input of step s+1.
+    linfo = world.launch_info()
+    world.destroy(); del world
+    torch.cuda.empty_cache()
+    n_split = max(1, min(args.e2e_split, E))
+    bounds = [(i * E // n_split, (i + 1) * E // n_split) for i in range(n_split)]
+    parts = []
+    for lo, hi in bounds:
+        wpi = W.WorldParams(**{**wp.__dict__, "n_envs": hi - lo})
+        wi = binding.World(wpi, wl.state[lo:hi], wl.props[lo:hi], wl.mu[lo:hi], device=local)
+        h_a = torch.empty(wi.state.shape, dtype=torch.float32, pin_memory=True)
+        h_b = torch.empty_like(h_a, pin_memory=True)
+        h_a.copy_(torch.as_tensor(wl.state[lo:hi]))
+        parts.append(dict(w=wi, st=torch.cuda.Stream(dev), h_a=h_a, h_b=h_b, h_fext=torch.as_tensor(wl.push_fext[lo:hi]).pin_memory(),
+                          fdev=torch.zeros((hi - lo, 6, wp.body_stride), dtype=torch.float32, device=dev)))
     Ke = min(K, args.e2e_steps) if args.e2e_steps > 0 else K
-    state_bytes = h_a.numel() * 4
     h2d = d2h = 0
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(stream)
+    for p in parts:
+        p["st"].wait_event(e0)
     pushing = False
     for s in range(Ke):
         active = wl.push_start <= s < wl.push_end
-        if active and not pushing:
-            fext_dev.copy_(h_fext, non_blocking=True); h2d += h_fext.numel() * 4
-        if active != pushing:
-            set_push(active); pushing = active
-        world.jenga_step_host(h_a, h_b, 1)
-        h_a, h_b = h_b, h_a
-        h2d += state_bytes; d2h += state_bytes
+        for p in parts:
+            with torch.cuda.stream(p["st"]):
+                if active and not pushing:
+                    p["fdev"].copy_(p["h_fext"], non_blocking=True); h2d += p["h_fext"].numel() * 4
+                if active != pushing:
+                    binding._check(L.jenga_set_f_ext(p["w"].handle, binding.C.c_void_p(p["fdev"].data_ptr()) if active else None), "jenga_set_f_ext")
+                p["w"].jenga_step_host(p["h_a"], p["h_b"], 1)
+                p["h_a"], p["h_b"] = p["h_b"], p["h_a"]
+                h2d += p["h_a"].numel() * 4; d2h += p["h_a"].numel() * 4
+        pushing = active
+    for p in parts:
+        ev = torch.cuda.Event(); ev.record(p["st"]); stream.wait_event(ev)
     e1.record(stream)
     barrier()
     ms_e2e = e0.elapsed_time(e1)
+    e2e_launches = Ke * n_split
 
     ms, ms_e2e = shard.max_over_ranks(ms, dev), shard.max_over_ranks(ms_e2e, dev)
     total_env_steps = E * K * world_size
@@ -311,9 +330,11 @@ def run_cuda(args) -> dict:
         "colours_per_env_step": cnt["colours"] / cnt["env_steps"],
         "status": {"or": status_or, "envs_flagged": n_flagged},
         "maxima": {k: cnt[k] for k in ("max_candidates", "max_colliding", "max_colours")},
-        "capacity": {"max_pairs": wp.max_pairs, "max_contacts": wp.max_contacts, "smem_bytes_per_env": world.launch_info()["smem_bytes"]},
+        "capacity": {"max_pairs": wp.max_pairs, "max_contacts": wp.max_contacts, "smem_bytes_per_cta": linfo["smem_bytes"],
+                     "threads_per_cta": linfo["threads"], "envs_per_cta": linfo["threads"] // 32},
         "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke},
+        "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke,
+                "split": n_split, "launches": e2e_launches},
         "gpu_launches": len(launches),
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinstr/s (FP32 thread-instructions, FMA=1)",
                      "frac": achieved / peak, "traffic": traffic, "kernel": "k_step", "launch_ms_avg": sum(launch_ms) / len(launch_ms),
@@ -337,6 +358,7 @@ def main():
     ap.add_argument("--envs", type=int, default=65536, help="envs per GPU (cfg5: 65,536)")
     ap.add_argument("--chunk", type=int, default=12, help="dt advances per jenga_step launch")
     ap.add_argument("--e2e-steps", type=int, default=96, help="steps of the end-to-end (host buffers) leg; 0 = K")
+    ap.add_argument("--e2e-split", type=int, default=2, help="worlds (streams) the e2e leg serves the batch with")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--max-contacts", type=int, default=0, help="override the workload's contact capacity per env")
     ap.add_argument("--max-pairs", type=int, default=0, help="override the workload's candidate capacity per env")
