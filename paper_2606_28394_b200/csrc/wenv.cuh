@@ -1,14 +1,21 @@
 // wenv.cuh -- warp-per-env layout of the batched Jenga step (sm_100a) and stages S1, S2.
 //
-// Mapping (kernel "v2"): ONE WARP owns one env for the whole launch (CTA = 32 threads), so
-// every synchronisation is a __syncwarp().  Shared memory per env holds
+// Mapping: ONE WARP owns one env for the whole launch, so every synchronisation inside an env is a
+// __syncwarp().  Two kernel flavours share this code (template <bool TM>):
+//   TM = false  CTA = 1 warp; all solver constants in shared memory.
+//   TM = true   CTA = 4 warps = 4 envs, 2 CTAs per SM; the 48 contact-constant words of the first 160
+//               colour-sorted pairs of each env live in tensor memory (tcgen05.ld/st, lane = position mod 32,
+//               block j = position / 32 at columns [48 j, 48 j + 48)), which frees enough shared memory for 8 envs
+//               per SM.  The CTA's warps meet at a CTA barrier between the stages of a substep so that they run
+//               the same code region (instruction-cache locality), nothing else is shared between them.
+// Shared memory per env holds
 //   * the body records (position, inverse mass, velocities, world inverse inertia: 20 floats per body,
 //     read and written with 128-bit accesses by the solver),
 //   * orientation, properties, rotation matrices and AABB extents as [row][S] arrays,
-//   * the candidate list, the colliding-pair list (current and previous substep), colours and the
-//     colour-sorted order,
-//   * the solver constants of every colliding pair in COLOUR-SORTED order as 14 float4 per pair
-//     (field-major: lane l of a colour chunk reads consecutive 16-byte words -> conflict-free LDS.128).
+//   * the colliding-pair list (current and previous substep), colours, the colour-sorted order, the phase chunks,
+//   * per colour-sorted position a 2-float4 header (bodies, meta, normal, Baumgarte term) and, for the positions not
+//     in TMEM, the 12 float4 of contact constants, field-major (lane l of a chunk reads consecutive 16-byte words:
+//     conflict-free LDS.128).  The candidate list and the colouring masks alias that region (dead before setup).
 // A colour phase of the PGS is one warp instruction stream over the <= 32 pairs of a chunk; lanes are
 // re-assigned to pairs every phase, so no lane idles because "its" pair has another colour.
 #pragma once
