@@ -201,7 +201,9 @@ def run_cuda(args) -> dict:
     binding.lib()                                            # fail loudly if libjenga.so is missing
 
     E = args.envs
-    wl = W.make_config(CFG, n_envs=E, env_offset=shard.env_range(rank, world_size, E)[0])   # weak scaling: every rank has its own E envs
+    wl = W.make_config(args.cfg, n_envs=E, env_offset=shard.env_range(rank, world_size, E)[0])
+    if wl.push_fext is None:
+        wl.push_fext = np.zeros((E, 6, wl.params.body_stride), np.float32); wl.push_start = wl.push_end = 0   # weak scaling: every rank has its own E envs
     wp = wl.params
     if args.max_contacts:
         wp.max_contacts = args.max_contacts
@@ -319,7 +321,7 @@ def run_cuda(args) -> dict:
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "cfg5 (BASELINE.json configs[4]): 18-level 54-block towers, mu_s {0.25,0.40,0.60} round-robin, 0-12 removals, "
-                               "Ziglar push sweep, dt=1/240, 20 PGS iters, rollout steps 0..K",
+                               "Ziglar push sweep, dt=1/240, 20 PGS iters, rollout steps 0..K" if args.cfg == CFG else f"cfg{args.cfg} (manual run, not the bench workload)",
                    "envs_per_gpu": E, "n_bodies": wp.n_bodies, "pgs_iters": wp.pgs_iters, "steps_per_launch": args.chunk,
                    "parallelism": f"env-sharded x{world_size}, no data-path collective",
                    "l2": "inputs larger than L2 (state 191 MB + warm-start cache 1.7 GB per step vs 126 MB L2)"},
@@ -359,6 +361,7 @@ def main():
     ap.add_argument("--chunk", type=int, default=12, help="dt advances per jenga_step launch")
     ap.add_argument("--e2e-steps", type=int, default=96, help="steps of the end-to-end (host buffers) leg; 0 = K")
     ap.add_argument("--e2e-split", type=int, default=2, help="worlds (streams) the e2e leg serves the batch with")
+    ap.add_argument("--cfg", type=int, default=CFG, help="BASELINE.json config number (5 = the bench workload; others: manual runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--max-contacts", type=int, default=0, help="override the workload's contact capacity per env")
     ap.add_argument("--max-pairs", type=int, default=0, help="override the workload's candidate capacity per env")

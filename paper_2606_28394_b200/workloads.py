@@ -223,8 +223,8 @@ def make_tower(cfg: int, n_envs: Optional[int] = None, env_offset: int = 0, jitt
             fext[e, 0:3, b] = F * d
             push_body[e], push_k[e], push_kthr[e] = b, k, kthr
     params = WorldParams(n_envs=E, n_bodies=B, body_stride=S, pgs_iters=c["iters"],
-                         max_pairs=768,
-                         max_contacts=704 if B <= 54 else 1536)    # 54 blocks: 156 standing pairs, <= 171 seen in collapses
+                         max_pairs=768 if B <= 54 else 1536,       # 54 blocks: <= 570 candidates / 171 colliding pairs seen in
+                         max_contacts=704 if B <= 54 else 1216)    # collapses (156 standing); 90 blocks: > 768 / 269 (264 standing)
     return Workload(
         name=f"cfg{cfg}", params=params,
         state=state.astype(np.float32), props=props.astype(np.float32), mu=mu.astype(np.float32),
@@ -254,7 +254,7 @@ def make_debris(n_envs: int = 4096, env_offset: int = 0, n_bodies: int = 54) -> 
         props[e, 1, :B], props[e, 2, :B], props[e, 3, :B] = inv_I
         props[e, 4, :B], props[e, 5, :B], props[e, 6, :B] = BLOCK_L / 2, BLOCK_W / 2, BLOCK_H / 2
         props[e, 7, :B] = 1.0
-    params = WorldParams(n_envs=E, n_bodies=B, body_stride=S, pgs_iters=20, max_pairs=768, max_contacts=1536)
+    params = WorldParams(n_envs=E, n_bodies=B, body_stride=S, pgs_iters=20, max_pairs=512, max_contacts=704)   # seen: 235 candidates, 111 colliding pairs
     mu = np.full(E, 0.40)
     return Workload(name="cfg3", params=params, state=state.astype(np.float32), props=props.astype(np.float32),
                     mu=mu.astype(np.float32), n_steps=720, meta=dict(cfg=3, env_offset=env_offset))
