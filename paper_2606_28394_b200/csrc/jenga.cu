@@ -24,17 +24,19 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
 }
 
 // ---------------------------------------------------------------- warp / TMEM set-up
-// TM kernels: CTA = 4 warps = 4 envs, 256 TMEM columns per CTA (2 CTAs per SM), warp w uses TMEM lanes 32 w .. 32 w + 31.
+// TM kernels: CTA = 4 warps = 4 envs; 256 TMEM columns per CTA and 2 CTAs per SM (tmb = 5) or 512 columns and 1 CTA
+// per SM (tmb = 10); warp w uses TMEM lanes 32 w .. 32 w + 31.
 template <bool TM>
 __device__ __forceinline__ Smem begin_warp(const Params& P, int& env) {
   __shared__ unsigned tm_base_s;
   const int warp = threadIdx.x >> 5;
   env = blockIdx.x * (TM ? 4 : 1) + warp;
-  Smem s = carve(P.S, P.max_pairs, P.pc, TM, warp * (int)smem_words(P.S, P.max_pairs, P.pc, TM));
+  const int tmb = TM ? P.tmb : 0, cols = tmb > 5 ? 512 : 256;
+  Smem s = carve(P.S, P.max_pairs, P.pc, tmb, warp * (int)smem_words(P.S, P.max_pairs, P.pc, tmb));
   if (TM) {
     if (warp == 0) {
       asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                   :: "r"((unsigned)__cvta_generic_to_shared(&tm_base_s)), "n"(kTmCols) : "memory");
+                   :: "r"((unsigned)__cvta_generic_to_shared(&tm_base_s)), "r"(cols) : "memory");
       asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -48,10 +50,11 @@ __device__ __forceinline__ Smem begin_warp(const Params& P, int& env) {
 template <bool TM>
 __device__ __forceinline__ void end_warp(const Smem& s) {
   if (TM) {
+    const int cols = s.pos0 > 160 ? 512 : 256;
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if ((threadIdx.x >> 5) == 0)
-      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s.tm), "n"(kTmCols) : "memory");   // warp 0: s.tm = base
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s.tm), "r"(cols) : "memory");   // warp 0: s.tm = base
   }
 }
 
@@ -255,7 +258,7 @@ struct jenga_world {
   jenga_world_desc desc;
   jenga_buffers bufs;
   Params P;
-  bool tm;                 // step / solve kernels keep the first 160 pairs' contact constants in TMEM (4 envs per CTA)
+  int tmb;                 // TMEM blocks per env of the step / solve kernels: 5, 10 or 0 (no TMEM, 1 warp per CTA)
   size_t smem_step;        // dynamic shared memory per CTA of k_step / k_pgs
   size_t smem_stage;       // ... of k_broadphase / k_narrowphase (one warp per CTA, no TMEM)
 };
@@ -269,30 +272,34 @@ static bool desc_ok(const jenga_world_desc* d) {
   if (d->n_substeps <= 0 || d->pgs_iters < 0 || !(d->dt > 0.0f)) return false;
   if (d->max_pairs <= 0 || d->max_pairs > 65535) return false;
   if (d->max_contacts < 4 || (d->max_contacts & 3) || d->max_contacts > 65532) return false;
-  if (4 * jenga::smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, false) > 227 * 1024) return false;
+  if (4 * jenga::smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, 0) > 227 * 1024) return false;
   return true;
 }
 
-static size_t env_bytes(const jenga_world_desc* d, bool tm) {
-  return 4 * jenga::smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, tm);
+static size_t env_bytes(const jenga_world_desc* d, int tmb) {
+  return 4 * jenga::smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, tmb);
 }
 
-/* The TMEM kernel pays off when two 4-env CTAs fit one SM (8 envs instead of <= 4); JENGA_NO_TMEM=1 forces the
- * all-shared-memory kernel (used by the tests to cover both). */
-static bool use_tmem(const jenga_world_desc* d) {
+/* TMEM blocks per env.  5 (256 columns per 4-env CTA) when two such CTAs fit one SM: 8 envs per SM; else 10 (512
+ * columns) when one 4-env CTA fits: 4 envs per SM; else 0: the all-shared-memory kernel, one warp per CTA.
+ * JENGA_NO_TMEM=1 forces 0 (the tests use it to cover both kernels). */
+static int pick_tmb(const jenga_world_desc* d) {
   const char* off = getenv("JENGA_NO_TMEM");
-  if (off && off[0] == '1') return false;
-  return 2 * (4 * env_bytes(d, true) + 1024 + 16) <= 227 * 1024;
+  if (off && off[0] == '1') return 0;
+  if (2 * (4 * env_bytes(d, 5) + 1024 + 16) <= 227 * 1024) return 5;
+  if (4 * env_bytes(d, 10) + 1024 + 16 <= 227 * 1024 && env_bytes(d, 0) + 1024 > 227 * 1024 / 4) return 10;
+  return 0;
 }
 
 extern "C" size_t jenga_smem_bytes(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
-  return use_tmem(d) ? 4 * env_bytes(d, true) : env_bytes(d, false);
+  const int tmb = pick_tmb(d);
+  return tmb ? 4 * env_bytes(d, tmb) : env_bytes(d, 0);
 }
 
 extern "C" int jenga_block_threads(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
-  return use_tmem(d) ? 128 : 32;   /* one warp per env; 4 envs per CTA in the TMEM kernel */
+  return pick_tmb(d) ? 128 : 32;   /* one warp per env; 4 envs per CTA in the TMEM kernel */
 }
 
 extern "C" const char* jenga_strerror(int code) {
@@ -329,7 +336,7 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   if (smem > (size_t)prop.sharedMemPerBlockOptin) return JENGA_E_ARG;
   jenga_world* w = (jenga_world*)calloc(1, sizeof(jenga_world));
   if (!w) return JENGA_E_ARG;
-  w->desc = *d; w->bufs = *b; w->tm = use_tmem(d); w->smem_step = smem; w->smem_stage = env_bytes(d, false);
+  w->desc = *d; w->bufs = *b; w->tmb = pick_tmb(d); w->smem_step = smem; w->smem_stage = env_bytes(d, 0);
   Params& P = w->P;
   P.E = d->n_envs; P.B = d->n_bodies; P.S = d->body_stride;
   P.h = d->dt / (float)d->n_substeps; P.n_substeps = d->n_substeps; P.iters = d->pgs_iters;
@@ -337,7 +344,7 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.restitution = d->restitution; P.aabb_margin = d->aabb_margin; P.beta = d->baumgarte_beta; P.slop = d->slop;
   P.cp.edge_bias_rel = d->edge_bias_rel; P.cp.edge_bias_abs = d->edge_bias_abs; P.cp.par_eps = d->par_eps; P.cp.tie_eps = d->tie_eps;
   P.match_tol = d->match_tol; P.warm_start = d->warm_start; P.gyroscopic = d->gyroscopic;
-  P.max_pairs = d->max_pairs; P.max_contacts = d->max_contacts; P.pc = d->max_contacts / 4; P.materialise = d->materialise;
+  P.max_pairs = d->max_pairs; P.max_contacts = d->max_contacts; P.pc = d->max_contacts / 4; P.materialise = d->materialise; P.tmb = w->tmb;
   P.state = b->state; P.props = b->props; P.mu = b->mu; P.f_ext = b->f_ext;
   P.pairs = b->pairs; P.n_pairs = b->n_pairs; P.contacts = b->contacts; P.n_contacts = b->n_contacts; P.lambda = b->lambda;
   P.cache_key = b->cache_key; P.cache_lam = b->cache_lam; P.cache_pt = b->cache_pt; P.n_cache = b->n_cache;
@@ -347,8 +354,8 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.collapse_stats = latch ? b->collapse_stats : nullptr;
   P.collapse_dx = d->collapse_fd * d->collapse_length; P.collapse_ek = d->collapse_ek; P.collapse_theta = d->collapse_theta;
   struct { const void* k; size_t smem; } kernels[] = {
-    { w->tm ? (const void*)jenga::k_step<true> : (const void*)jenga::k_step<false>, w->smem_step },
-    { w->tm ? (const void*)jenga::k_pgs<true> : (const void*)jenga::k_pgs<false>, w->smem_step },
+    { w->tmb ? (const void*)jenga::k_step<true> : (const void*)jenga::k_step<false>, w->smem_step },
+    { w->tmb ? (const void*)jenga::k_pgs<true> : (const void*)jenga::k_pgs<false>, w->smem_step },
     { (const void*)jenga::k_broadphase, w->smem_stage }, { (const void*)jenga::k_narrowphase, w->smem_stage } };
   for (auto& kn : kernels) {
     e = cudaFuncSetAttribute(kn.k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kn.smem);
@@ -391,7 +398,7 @@ extern "C" int jenga_narrowphase(jenga_world* w, void* stream) {
 extern "C" int jenga_pgs_solve(jenga_world* w, int iters, void* stream) {
   if (!w || iters < 0) return JENGA_E_ARG;
   const int it = iters > 0 ? iters : w->P.iters;
-  if (w->tm) jenga::k_pgs<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, it);
+  if (w->tmb) jenga::k_pgs<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, it);
   else jenga::k_pgs<false><<<w->P.E, 32, w->smem_step, (cudaStream_t)stream>>>(w->P, it);
   return launched("k_pgs");
 }
@@ -399,7 +406,7 @@ extern "C" int jenga_pgs_solve(jenga_world* w, int iters, void* stream) {
 extern "C" int jenga_step(jenga_world* w, int n_steps, void* stream) {
   if (!w || n_steps < 0) return JENGA_E_ARG;
   if (n_steps == 0) return JENGA_OK;
-  if (w->tm) jenga::k_step<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps);
+  if (w->tmb) jenga::k_step<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps);
   else jenga::k_step<false><<<w->P.E, 32, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps);
   return launched("k_step");
 }

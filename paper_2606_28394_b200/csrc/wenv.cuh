@@ -29,9 +29,9 @@ constexpr int kMaxColours = 64;
 constexpr int kBd = 20;        // floats per body record: x y z im | vx vy vz - | wx wy wz - | Ixx Ixy Ixz Iyy | Iyz Izz - -
 constexpr int kHdrF4 = 2;      // float4 per pair header: (a, b, meta, 1/|t1 raw|), (n.xyz, Baumgarte corr)
 constexpr int kCsF4 = 12;      // float4 of contact constants per pair: 36 read-only words + 12 impulses
-constexpr int kTmBlocks = 5;   // TMEM tier: the first 5 x 32 colour-sorted positions keep their contact constants in
-constexpr int kTmPos = 32 * kTmBlocks;   // tensor memory (48 columns per block of 32 pairs, lane = position % 32)
-constexpr int kTmCols = 256;   // columns allocated per CTA of 4 warps (4 envs); 2 CTAs per SM
+// TMEM tier: the first 32 * tmb colour-sorted positions keep their contact constants in tensor memory (48 columns per
+// block of 32 pairs, lane = position % 32).  tmb = 5: 256 columns per CTA of 4 warps, 2 CTAs per SM (8 envs per SM);
+// tmb = 10: 512 columns, 1 CTA per SM (4 envs per SM; large configs); tmb = 0: no TMEM (1 warp per CTA).
 constexpr unsigned kFull = 0xffffffffu;
 
 struct Params {
@@ -42,7 +42,7 @@ struct Params {
   float restitution, aabb_margin, beta, slop;
   CollideParams cp;
   float match_tol;
-  int warm_start, gyroscopic, max_pairs, max_contacts, pc, materialise;
+  int warm_start, gyroscopic, max_pairs, max_contacts, pc, materialise, tmb;
   float* state; const float* props; const float* mu; const float* f_ext;
   int* pairs; int* n_pairs; float* contacts; int* n_contacts; float* lambda;
   int* cache_key; float* cache_lam; float* cache_pt; int* n_cache;
@@ -81,7 +81,7 @@ struct Smem {
   SP<int> ccount;               // [64]
   SP<int> cstart;               // [64]
   SP<int> misc;                 // [16]
-  int pcA, capS, pos0;          // pos0: first colour-sorted position held in cs (0, or kTmPos in the TMEM kernel)
+  int pcA, capS, pos0;          // pos0 = 32 * tmb: first colour-sorted position held in cs
   unsigned tm;                  // TMEM address of this warp's lanes, column 0 (TMEM kernel)
 };
 
@@ -91,19 +91,19 @@ __host__ __device__ inline int round_up(int v, int m) { return (v + m - 1) / m *
 
 // The header + contact-constant region is dead between S7 of one substep and the setup pass of the next, which is
 // when the candidate list (S2 -> first half of S3) and the colouring masks (S4) live: they alias it.
-__host__ __device__ inline int cap_smem_pairs(int pc, bool tm) {
+__host__ __device__ inline int cap_smem_pairs(int pc, int tmb) {
   const int pcA = round_up(pc, 8);
-  return tm ? (pcA > kTmPos ? pcA - kTmPos : 8) : pcA;
+  return tmb ? (pcA > 32 * tmb ? pcA - 32 * tmb : 8) : pcA;
 }
-__host__ __device__ inline int slot_region_words(int S, int max_pairs, int pc, bool tm) {
+__host__ __device__ inline int slot_region_words(int S, int max_pairs, int pc, int tmb) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8);
-  const int a = 4 * (kHdrF4 * pcA + kCsF4 * cap_smem_pairs(pc, tm)), b = mpA / 2 + 2 * S;
+  const int a = 4 * (kHdrF4 * pcA + kCsF4 * cap_smem_pairs(pc, tmb)), b = mpA / 2 + 2 * S;
   return round_up(a > b ? a : b, 4);
 }
 
-__host__ __device__ inline size_t smem_words(int S, int max_pairs, int pc, bool tm) {
+__host__ __device__ inline size_t smem_words(int S, int max_pairs, int pc, int tmb) {
   const int pcA = round_up(pc, 8);
-  size_t w = slot_region_words(S, max_pairs, pc, tm);
+  size_t w = slot_region_words(S, max_pairs, pc, tmb);
   w += (size_t)(kBd + 4 + 8 + 9 + 3) * S;
   w += pcA;                        // cab
   w += 5 * (size_t)(pcA / 2);      // cpair x2, pos, order, wrank (u16)
@@ -114,13 +114,13 @@ __host__ __device__ inline size_t smem_words(int S, int max_pairs, int pc, bool 
 }
 
 // base: word offset of this env's arena inside the CTA's dynamic shared memory
-__device__ inline Smem carve(int S, int max_pairs, int pc, bool tm, int base) {
+__device__ inline Smem carve(int S, int max_pairs, int pc, int tmb, int base) {
   Smem s;
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8);
-  s.pcA = pcA; s.capS = cap_smem_pairs(pc, tm); s.pos0 = tm ? kTmPos : 0; s.tm = 0;
+  s.pcA = pcA; s.capS = cap_smem_pairs(pc, tmb); s.pos0 = 32 * tmb; s.tm = 0;
   int p = base;
   s.hdr.off = p; s.cs.off = p + 4 * kHdrF4 * pcA; s.cand.off = p; s.used.off = p + mpA / 2;
-  p += slot_region_words(S, max_pairs, pc, tm);
+  p += slot_region_words(S, max_pairs, pc, tmb);
   s.bd.off = p;  p += kBd * S;
   s.q.off = p;   p += 4 * S;
   s.pr.off = p;  p += 8 * S;

@@ -102,7 +102,7 @@ __device__ inline void colour_pairs(const Smem& s, const Params& P, int n_coll, 
       s.cstart[c] = acc;
       for (int st0 = acc; st0 < acc + n; ) {                     // chunks of <= 32 pairs; none straddles the TMEM boundary
         int lim = min(acc + n, st0 + 32);
-        if (TM && st0 < kTmPos && lim > kTmPos) lim = kTmPos;
+        if (TM && st0 < s.pos0 && lim > s.pos0) lim = s.pos0;
         s.ph[nph++] = st0 | ((lim - st0) << 16);
         st0 = lim;
       }
@@ -126,7 +126,7 @@ __device__ inline void colour_pairs(const Smem& s, const Params& P, int n_coll, 
 // Contact constants of position k: 48 words, PairC.  ro[9c..9c+8] = p.xyz, (1+e)/K_nn, 1/K_t1t1, 1/K_t2t2,
 // K_n,t1, K_n,t2, K_t1,t2 of contact c (K_dd: Eq. 13, for d = n, t1, t2); lam[3c..3c+2] = jn, jt1, jt2.
 // They live in shared memory (field-major float4 [12][capS], position k - pos0) or, in the TMEM kernel for
-// positions < kTmPos, in tensor memory: block j = k / 32 at columns [48 j, 48 j + 48) of lane k % 32.
+// positions < pos0 = 32 * tmb, in tensor memory: block j = k / 32 at columns [48 j, 48 j + 48) of lane k % 32.
 __device__ __forceinline__ float4& hdr4(const Smem& s, int f, int k) { return s.hdr[f * s.pcA + k]; }
 
 struct PairC { float v[48]; };      // v[0..35] read-only constants, v[36..47] impulses
@@ -183,12 +183,12 @@ __device__ __forceinline__ void sm_store_lam(const Smem& s, int k, const float* 
 // aligned round: lane l <-> position 32 j + l (setup, cache store, lambda output).  All lanes call these.
 template <bool TM>
 __device__ __forceinline__ void round_load(const Smem& s, int j, int n_valid, PairC& c) {
-  if (TM && j < kTmBlocks) { tm_load_block(s, j, c); tm_wait_ld(); }
+  if (TM && 32 * j < s.pos0) { tm_load_block(s, j, c); tm_wait_ld(); }
   else if (32 * j + lane_id() < n_valid) sm_load_pair(s, 32 * j + lane_id(), c);
 }
 template <bool TM>
 __device__ __forceinline__ void round_store(const Smem& s, int j, int n_valid, const PairC& c) {
-  if (TM && j < kTmBlocks) { tm_store_block(s, j, c); tm_wait_st(); }
+  if (TM && 32 * j < s.pos0) { tm_store_block(s, j, c); tm_wait_st(); }
   else if (32 * j + lane_id() < n_valid) sm_store_pair(s, 32 * j + lane_id(), c);
 }
 
@@ -366,7 +366,7 @@ __device__ __forceinline__ void solve_chunk(const Smem& s, int start, int count,
   const int k = start + ((lane - start) & 31);
   const bool active = k < start + count;
   const int jA = start >> 5;
-  const bool in_tm = TM && start < kTmPos;                       // chunks never straddle kTmPos
+  const bool in_tm = TM && start < s.pos0;                       // chunks never straddle pos0
   const bool span = (start & 31) + count > 32;
   PairC c;
   float keepA[12], keepB[12];                                    // impulses of the lanes that are not in this chunk
