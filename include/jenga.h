@@ -113,6 +113,7 @@ typedef struct {
   int32_t     *collapsed;  /* [E]  OR-latched: 1 once dx_max > f_d l, theta_max > theta_th and E_k > eps_k
                                    held at the same step                                                */
   float       *collapse_stats; /* [E][4] of the last step: dx_max [m], E_k [J], theta_max [rad], 0     */
+  int32_t     *rest_steps; /* [E]  steps taken by the last jenga_simulate_until_rest; may be NULL      */
 } jenga_buffers;
 
 /* Validates desc/buffers (sizes, alignment, device arch) and returns a host handle. */
@@ -134,6 +135,14 @@ int jenga_pgs_solve(jenga_world *w, int iters, void *cuda_stream);
 /* n_steps advances of dt (each n_substeps fused substeps S1..S7), one launch; state, cache,
  * status and counters are updated in place.                                                           */
 int jenga_step(jenga_world *w, int n_steps, void *cuda_stream);
+
+/* simulate_until_rest (§8.3): every env advances dt by dt until its total kinetic energy
+ * E_k = sum_b 1/2 m |v|^2 + 1/2 w . I w, evaluated after every step, is below ek_rest, at most max_steps steps
+ * (the paper: 400 steps, 1e-7 J); bufs.rest_steps[env] = steps taken (>= 1).  One launch: an env at rest stops
+ * costing arithmetic, and its CTA retires as soon as all of the CTA's envs rest, which frees the SM for the next
+ * CTA -- the grid scheduler does the active-env compaction.  f_ext, the warm-start cache and the collapse latch
+ * behave as in jenga_step; counters add the steps actually taken.                                         */
+int jenga_simulate_until_rest(jenga_world *w, int max_steps, float ek_rest, void *cuda_stream);
 
 /* jenga_step with HOST state buffers (the end-to-end call): enqueues, on `cuda_stream`, a host->device copy
  * of h_state_in ([E][13][S] fp32, same layout as bufs.state; pinned memory recommended, pageable works but

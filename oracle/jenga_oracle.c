@@ -798,6 +798,33 @@ void orc_rollout(const orc_params *P, int32_t E, int32_t B, int32_t n_steps,
   }
 }
 
+/* simulate_until_rest (§8.3): advance env by env until the total kinetic energy
+ * E_k = sum_b 1/2 m |v|^2 + 1/2 w . I w, evaluated after every step, falls below ek_rest, at most max_steps
+ * steps (the paper: 400, 1e-7 J).  steps_out[e] = steps taken (>= 1).  Same arrays as orc_rollout. */
+void orc_rollout_until_rest(const orc_params *P, int32_t E, int32_t B, int32_t max_steps, double ek_rest,
+                            double *x, double *q, double *v, double *w,
+                            const double *inv_m, const double *inv_I, const double *he, const int32_t *active,
+                            const double *mu,
+                            int32_t *key_pair, int32_t *key_meta, int32_t *n_keys, double *lam, double *cpt,
+                            uint32_t *status, int32_t *steps_out, double *ek_out) {
+  const int32_t pc = P->max_contacts / 4;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int32_t e = 0; e < E; ++e) {
+    orc_cache cache = { n_keys[e], key_pair + (size_t)e*pc, key_meta + (size_t)e*pc, lam + (size_t)e*pc*12, cpt + (size_t)e*pc*12 };
+    size_t o3 = (size_t)e*B*3, o4 = (size_t)e*B*4, o1 = (size_t)e*B;
+    int32_t s = 0; double out3[3] = { 0, 0, 0 };
+    while (s < max_steps) {
+      status[e] |= orc_step_env(P, B, x+o3, q+o4, v+o3, w+o3, inv_m+o1, inv_I+o3, he+o3, active+o1,
+                                mu[e], NULL, &cache, NULL);
+      ++s;
+      orc_collapse_test(B, x+o3, q+o4, v+o3, w+o3, x+o3, q+o4, inv_m+o1, inv_I+o3, active+o1, 1.0, out3);
+      if (out3[1] < ek_rest) break;
+    }
+    n_keys[e] = cache.n_pairs;
+    steps_out[e] = s; if (ek_out) ek_out[e] = out3[1];
+  }
+}
+
 int32_t orc_max_threads(void) {
 #ifdef _OPENMP
   extern int omp_get_max_threads(void);

@@ -319,6 +319,21 @@ def rollout(P, bod: Bodies, mu, n_steps, fext=None, cache: Cache = None, x0=None
     return status
 
 
+def rollout_until_rest(P, bod: Bodies, mu, max_steps=400, ek_rest=1e-7, cache: Cache = None):
+    """per env, steps until E_k < ek_rest (checked after every step), at most max_steps.
+    Returns (steps [E], E_k at exit [E], status [E])."""
+    E, B = bod.E, bod.B
+    if cache is None:
+        cache = Cache(E, P.max_contacts)
+    status = np.zeros(E, np.uint32); steps = np.zeros(E, np.int32); ek = np.zeros(E)
+    mu = np.ascontiguousarray(mu, np.float64)
+    lib().orc_rollout_until_rest(C.byref(P), C.c_int32(E), C.c_int32(B), C.c_int32(max_steps), C.c_double(ek_rest),
+                                 dp(bod.x), dp(bod.q), dp(bod.v), dp(bod.w), dp(bod.inv_m), dp(bod.inv_I), dp(bod.he),
+                                 ip(bod.active), dp(mu), ip(cache.key_pair), ip(cache.key_meta), ip(cache.n_keys),
+                                 dp(cache.lam), dp(cache.pt), status.ctypes.data_as(c_up), ip(steps), dp(ek))
+    return steps, ek, status
+
+
 def collapse_test(bod: Bodies, x0, q0, e=0, length=0.075):
     out = np.zeros(3)
     r = lib().orc_collapse_test(C.c_int32(bod.B), dp(bod.x[e]), dp(bod.q[e]), dp(bod.v[e]), dp(bod.w[e]), dp(x0), dp(q0),

@@ -39,7 +39,7 @@ class WorldDesc(C.Structure):
 class Buffers(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("state", "props", "mu", "f_ext", "pairs", "n_pairs", "contacts", "n_contacts",
                                           "lambda_", "cache_key", "cache_lam", "cache_pt", "n_cache", "status", "counters",
-                                          "ref_pose", "collapsed", "collapse_stats")]
+                                          "ref_pose", "collapsed", "collapse_stats", "rest_steps")]
 
 
 def lib():
@@ -59,6 +59,7 @@ def lib():
         L.jenga_narrowphase.argtypes = [C.c_void_p, C.c_void_p]
         L.jenga_pgs_solve.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.jenga_step.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.jenga_simulate_until_rest.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_void_p]
         L.jenga_set_f_ext.argtypes = [C.c_void_p, C.c_void_p]
         L.jenga_step_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.jenga_smem_bytes.argtypes = [C.POINTER(WorldDesc)]
@@ -67,7 +68,7 @@ def lib():
         L.jenga_strerror.argtypes = [C.c_int]
         L.jenga_strerror.restype = C.c_char_p
         for f in ("jenga_world_create", "jenga_world_destroy", "jenga_broadphase", "jenga_narrowphase", "jenga_pgs_solve",
-                  "jenga_step", "jenga_step_host", "jenga_set_f_ext", "jenga_block_threads"):
+                  "jenga_step", "jenga_step_host", "jenga_simulate_until_rest", "jenga_set_f_ext", "jenga_block_threads"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -137,6 +138,8 @@ class World:
         b.cache_key, b.cache_lam, b.cache_pt = self.cache_key.data_ptr(), self.cache_lam.data_ptr(), self.cache_pt.data_ptr()
         b.n_cache, b.status, b.counters = self.n_cache.data_ptr(), self.status.data_ptr(), self.counters.data_ptr()
         self.ref_pose = self.collapsed = self.collapse_stats = None
+        self.rest_steps = z((E,), torch.int32)
+        b.rest_steps = self.rest_steps.data_ptr()
         if collapse_length > 0.0:                      # Eq. 18 latch against the pose the world starts from
             self.ref_pose = self.state[:, 0:7, :].contiguous()
             self.collapsed = z((E,), torch.int32)
@@ -162,6 +165,9 @@ class World:
     def jenga_step(self, n_steps: int = 1):
         _check(lib().jenga_step(self.handle, int(n_steps), self._stream()), "jenga_step")
 
+    def jenga_simulate_until_rest(self, max_steps: int = 400, ek_rest: float = 1.0e-7):
+        _check(lib().jenga_simulate_until_rest(self.handle, int(max_steps), C.c_float(ek_rest), self._stream()), "jenga_simulate_until_rest")
+
     def jenga_step_host(self, h_state_in, h_state_out, n_steps: int = 1):
         """h_state_in / h_state_out: None or contiguous fp32 CPU tensors [E][13][S] (pinned for async copies)."""
         for t in (h_state_in, h_state_out):
@@ -186,8 +192,9 @@ class World:
             _check(lib().jenga_world_destroy(self.handle), "jenga_world_destroy")
             self.handle = C.c_void_p()
 
-    broadphase, narrowphase, pgs_solve, step, step_host, set_f_ext, destroy = (
-        jenga_broadphase, jenga_narrowphase, jenga_pgs_solve, jenga_step, jenga_step_host, jenga_set_f_ext, jenga_world_destroy)
+    broadphase, narrowphase, pgs_solve, step, step_host, simulate_until_rest, set_f_ext, destroy = (
+        jenga_broadphase, jenga_narrowphase, jenga_pgs_solve, jenga_step, jenga_step_host, jenga_simulate_until_rest,
+        jenga_set_f_ext, jenga_world_destroy)
 
     def __del__(self):
         try:

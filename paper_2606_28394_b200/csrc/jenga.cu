@@ -63,11 +63,13 @@ __device__ __forceinline__ void end_warp(const Smem& s) {
 // run the same code region at the same time, which keeps the instruction working set of an SM (32 KB L1.5 I-cache)
 // to two regions instead of eight (profiles/r1d: `no_instruction` was the top stall with 8 free-running warps).
 template <bool TM>
-__global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const int n_steps) {
+__global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const int n_steps, const float rest_ek) {
   int env;
   const Smem s = begin_warp<TM>(P, env);
   const int lane = lane_id();
-  const bool valid = env < P.E;
+  bool valid = env < P.E;            // false also once the env is at rest (jenga_simulate_until_rest)
+  const bool in_range = valid;
+  int steps_done = 0;
   float mu = 0.0f;
   if (valid) {
     load_env(s, P, env);
@@ -112,9 +114,19 @@ __global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const in
       if (lane == 0) s.misc[MiNprev] = n_coll;
       cur ^= 1;
       __syncwarp();
+      if ((sub + 1) % P.n_substeps == 0) {
+        ++steps_done;
+        if (rest_ek > 0.0f && env_kinetic_energy(s, P) < rest_ek) valid = false;
+      }
+    }
+    if (rest_ek > 0.0f) {                                           // the CTA retires when all of its envs rest
+      const bool all_rest = TM ? (__syncthreads_and(!valid) != 0) : !valid;
+      if (all_rest) break;
     }
   }
+  valid = in_range;
   if (valid) {
+    if (rest_ek > 0.0f && P.rest_steps && lane == 0) P.rest_steps[env] = steps_done;
     store_env(s, P, env);
     flush_status(P, env, st);
     if (P.counters) {
@@ -126,8 +138,8 @@ __global__ void __launch_bounds__(TM ? 128 : 32) k_step(const Params P, const in
         atomicAdd(P.counters + JENGA_CNT_CONTACTS, v);
         atomicAdd(P.counters + JENGA_CNT_CONTACT_ITERS, v * (unsigned long long)P.iters);
         atomicAdd(P.counters + JENGA_CNT_GROUND_CONTACTS, vg);
-        atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, (unsigned long long)n_steps);
-        atomicAdd(P.counters + JENGA_CNT_BODY_STEPS, (unsigned long long)n_steps * n_active);
+        atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, (unsigned long long)steps_done);
+        atomicAdd(P.counters + JENGA_CNT_BODY_STEPS, (unsigned long long)steps_done * n_active);
         atomicAdd(P.counters + JENGA_CNT_CANDIDATES, c_cand);
         atomicAdd(P.counters + JENGA_CNT_COLLIDING, c_coll);
         atomicAdd(P.counters + JENGA_CNT_COLOURS, c_col);
@@ -352,6 +364,7 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   const bool latch = d->collapse_length > 0.0f && b->ref_pose && b->collapsed;
   P.ref_pose = latch ? b->ref_pose : nullptr; P.collapsed = latch ? b->collapsed : nullptr;
   P.collapse_stats = latch ? b->collapse_stats : nullptr;
+  P.rest_steps = b->rest_steps;
   P.collapse_dx = d->collapse_fd * d->collapse_length; P.collapse_ek = d->collapse_ek; P.collapse_theta = d->collapse_theta;
   struct { const void* k; size_t smem; } kernels[] = {
     { w->tmb ? (const void*)jenga::k_step<true> : (const void*)jenga::k_step<false>, w->smem_step },
@@ -406,9 +419,16 @@ extern "C" int jenga_pgs_solve(jenga_world* w, int iters, void* stream) {
 extern "C" int jenga_step(jenga_world* w, int n_steps, void* stream) {
   if (!w || n_steps < 0) return JENGA_E_ARG;
   if (n_steps == 0) return JENGA_OK;
-  if (w->tmb) jenga::k_step<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps);
-  else jenga::k_step<false><<<w->P.E, 32, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps);
+  if (w->tmb) jenga::k_step<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps, 0.0f);
+  else jenga::k_step<false><<<w->P.E, 32, w->smem_step, (cudaStream_t)stream>>>(w->P, n_steps, 0.0f);
   return launched("k_step");
+}
+
+extern "C" int jenga_simulate_until_rest(jenga_world* w, int max_steps, float ek_rest, void* stream) {
+  if (!w || max_steps <= 0 || !(ek_rest > 0.0f)) return JENGA_E_ARG;
+  if (w->tmb) jenga::k_step<true><<<(w->P.E + 3) / 4, 128, w->smem_step, (cudaStream_t)stream>>>(w->P, max_steps, ek_rest);
+  else jenga::k_step<false><<<w->P.E, 32, w->smem_step, (cudaStream_t)stream>>>(w->P, max_steps, ek_rest);
+  return launched("k_step (until rest)");
 }
 
 extern "C" int jenga_step_host(jenga_world* w, const float* h_in, float* h_out, int n_steps, void* stream) {

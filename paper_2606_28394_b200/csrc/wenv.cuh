@@ -47,7 +47,7 @@ struct Params {
   int* pairs; int* n_pairs; float* contacts; int* n_contacts; float* lambda;
   int* cache_key; float* cache_lam; float* cache_pt; int* n_cache;
   unsigned* status; unsigned long long* counters;
-  const float* ref_pose; int* collapsed; float* collapse_stats;
+  const float* ref_pose; int* collapsed; float* collapse_stats; int* rest_steps;
   float collapse_dx, collapse_ek, collapse_theta;           // f_d * l, eps_k, theta_th
 };
 

@@ -536,6 +536,27 @@ __device__ inline void collapse_latch(const Smem& s, const Params& P, int env) {
   }
 }
 
+// Total kinetic energy of the env: sum_b 1/2 m |v|^2 + 1/2 w . I w, I in the body frame.
+__device__ inline float env_kinetic_energy(const Smem& s, const Params& P) {
+  const int S = P.S;
+  float ek = 0.0f;
+  for (int b = lane_id(); b < P.B; b += 32) {
+    const float4 x = bd4(s, b, 0);
+    if (x.w == 0.0f) continue;
+    const float4 v = bd4(s, b, 1), w = bd4(s, b, 2);
+    const float qw = s.q[b], qx = s.q[S + b], qy = s.q[2 * S + b], qz = s.q[3 * S + b];
+    const float r00 = 1.0f - 2.0f * (qy * qy + qz * qz), r01 = 2.0f * (qx * qy - qz * qw), r02 = 2.0f * (qx * qz + qy * qw);
+    const float r10 = 2.0f * (qx * qy + qz * qw), r11 = 1.0f - 2.0f * (qx * qx + qz * qz), r12 = 2.0f * (qy * qz - qx * qw);
+    const float r20 = 2.0f * (qx * qz - qy * qw), r21 = 2.0f * (qy * qz + qx * qw), r22 = 1.0f - 2.0f * (qx * qx + qy * qy);
+    const float w0 = r00 * w.x + r10 * w.y + r20 * w.z, w1 = r01 * w.x + r11 * w.y + r21 * w.z, w2 = r02 * w.x + r12 * w.y + r22 * w.z;
+    ek += 0.5f * (v.x * v.x + v.y * v.y + v.z * v.z) / x.w
+        + 0.5f * (w0 * w0 / s.pr[S + b] + w1 * w1 / s.pr[2 * S + b] + w2 * w2 / s.pr[3 * S + b]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) ek += __shfl_xor_sync(kFull, ek, o);
+  return ek;
+}
+
 // S7: every pair's impulses and contact points become the next substep's warm-start cache, in ascending
 // pair order (cache entry r = pair rank r).  Returns the lane's (contacts, ground contacts) for the counters.
 template <bool TM>

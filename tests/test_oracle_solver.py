@@ -275,3 +275,23 @@ def test_P10_resting_tower_drift(orc):
         st = orc.rollout(P, bod, wl.mu, 480, cache=cache)
         assert st[0] == 0
         assert np.linalg.norm(bod.x - x60, axis=2).max() < lim
+
+
+def test_until_rest_sliding_block_closed_form(orc):
+    """simulate_until_rest: a block sliding on the ground with speed v0 decelerates with mu g, so
+    it is at rest (E_k < 1e-7 J) after ceil(v0 / (mu g h)) steps up to the E_k threshold; a block already at rest
+    takes exactly one step; an airborne block runs into the step limit."""
+    mu, v0 = 0.4, 0.30
+    h = W.f32(1.0 / 240.0)
+    wl = W.make_custom([dict(pos=(0, 0, W.BLOCK_H / 2 - 1e-4), size=(W.BLOCK_L, W.BLOCK_W, W.BLOCK_H), mass=W.BLOCK_MASS, vel=(v0, 0, 0))], mu=mu)
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(wl.state, wl.props, 1)
+    steps, ek, _ = orc.rollout_until_rest(P, bod, wl.mu, max_steps=400, ek_rest=1e-7)
+    n_stop = v0 / (mu * 9.81 * h)                      # steps until Coulomb friction has removed v0
+    assert abs(steps[0] - n_stop) <= 3 and ek[0] < 1e-7, (steps, n_stop, ek)
+    assert abs(bod.x[0, 0, 0] - v0 * v0 / (2 * mu * 9.81)) < 2e-3       # stopping distance v0^2 / (2 mu g)
+    steps2, ek2, _ = orc.rollout_until_rest(P, bod, wl.mu, max_steps=400, ek_rest=1e-7)   # now at rest
+    assert steps2[0] == 1 and ek2[0] < 1e-7
+    air = W.make_custom([dict(pos=(0, 0, 5.0), size=(W.BLOCK_L, W.BLOCK_W, W.BLOCK_H), mass=W.BLOCK_MASS)])
+    b3 = orc.unpack_tiles(air.state, air.props, 1)
+    steps3, ek3, _ = orc.rollout_until_rest(orc.make_params(air.params), b3, air.mu, max_steps=50, ek_rest=1e-7)
+    assert steps3[0] == 50 and abs(ek3[0] - 0.5 * W.BLOCK_MASS * (9.81 * 50 * h) ** 2) < 1e-4 * ek3[0] + 1e-9
