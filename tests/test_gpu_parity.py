@@ -571,3 +571,19 @@ def test_until_rest_matches_oracle(orc, J):
     # the step at which E_k crosses 1e-7 J depends on rounding for towers that are still rocking: measured on B200
     # 71 % equal, 92 % within 5 steps
     assert np.mean(d == 0) >= 0.5 and np.mean(d <= 5) >= 0.8
+
+
+def test_step_host_equals_step(J):
+    """jenga_step_host (host buffers: H2D, fused step, D2H on the caller's stream) gives the state jenga_step gives."""
+    import torch
+    wl = W.make_config(2, n_envs=5)
+    a = J.World(wl.params, wl.state, wl.props, wl.mu); b = J.World(wl.params, wl.state, wl.props, wl.mu)
+    h_in = torch.as_tensor(wl.state).clone().pin_memory(); h_out = torch.empty_like(h_in).pin_memory()
+    for _ in range(4):
+        a.step(1)
+        b.step_host(h_in, h_out, 1)
+        torch.cuda.synchronize()
+        h_in, h_out = h_out, h_in
+    assert torch.equal(a.state.cpu(), h_in) and torch.equal(a.state, b.state)
+    b.step_host(None, h_out, 2); a.step(2); torch.cuda.synchronize()      # NULL input: continue from the device state
+    assert torch.equal(a.state.cpu(), h_out)
