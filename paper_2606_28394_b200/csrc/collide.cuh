@@ -304,9 +304,4 @@ __device__ inline void manifold_boxes(const Box& A, const Box& B, const SatResul
   m.np = no;
 }
 
-__device__ inline void collide_boxes(const CollideParams& cp, const Box& A, const Box& B, Manifold& m) {
-  SatResult sr; m.np = 0;
-  if (sat_boxes(cp, A, B, sr)) manifold_boxes(A, B, sr, m);
-}
-
 }  // namespace jenga

@@ -85,7 +85,7 @@ struct Smem {
   unsigned tm;                  // TMEM address of this warp's lanes, column 0 (TMEM kernel)
 };
 
-enum { MiNph = 0, MiNcol = 1, MiNprev = 2, MiCur = 3 };
+enum { MiNph = 0, MiNcol = 1, MiNprev = 2 };
 
 __host__ __device__ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 

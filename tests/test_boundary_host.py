@@ -34,6 +34,15 @@ def test_library_is_sm100a_only():
     assert "sm_100a" in out and "sm_90" not in out and "sm_80" not in out
 
 
+def test_library_uses_tensor_memory_and_shared_window_loads():
+    """SASS evidence that the kernels are Blackwell-native: tcgen05.ld/st compile to LDTM/STTM, and the shared-memory
+    arrays are addressed with LDS/STS (not generic LD/ST)."""
+    from paper_2606_28394_b200 import build
+    sass = subprocess.run(["cuobjdump", "-sass", build.LIB], capture_output=True, text=True).stdout
+    assert sass.count("LDTM") >= 10 and sass.count("STTM") >= 5
+    assert sass.count("LDS") > 500 and " LD.E" not in sass
+
+
 def test_descriptor_validation_and_launch_shape(L):
     from paper_2606_28394_b200 import binding, workloads as W
     wp = W.make_config(2, n_envs=2).params
