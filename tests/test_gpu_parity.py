@@ -587,3 +587,47 @@ def test_step_host_equals_step(J):
     assert torch.equal(a.state.cpu(), h_in) and torch.equal(a.state, b.state)
     b.step_host(None, h_out, 2); a.step(2); torch.cuda.synchronize()      # NULL input: continue from the device state
     assert torch.equal(a.state.cpu(), h_out)
+
+
+def test_in_rollout_block_removal(orc, J):
+    """NEXT-4 (the game loop's withdrawal): props are caller-owned and read at every launch, so a
+    block is removed mid-episode by clearing its `active` flag between two jenga_step calls.  From a common settled
+    state: remove one block per env, then 5 steps on both sides; the removed block stays put, its pairs disappear
+    from the pair list and the cached impulses of the other pairs are still found."""
+    import torch
+    E = 4
+    wl = W.make_config(2, n_envs=E)
+    state, cache = oracle_mid_state(orc, wl, 40)
+    B = wl.params.n_bodies
+    world = J.World(wl.params, state, wl.props, wl.mu, materialise=True)
+    cache.lam[:] = cache.lam.astype(np.float32); cache.pt[:] = cache.pt.astype(np.float32)
+    world.cache_key[:, :, :] = torch.as_tensor(np.stack([cache.key_pair, cache.key_meta], axis=-1)).to(world.dev)
+    world.cache_lam[:] = torch.as_tensor(cache.lam.astype(np.float32)).to(world.dev)
+    world.cache_pt[:] = torch.as_tensor(cache.pt.astype(np.float32)).to(world.dev)
+    world.n_cache[:] = torch.as_tensor(cache.n_keys).to(world.dev)
+    props = wl.props.copy()
+    victims = []
+    for e in range(E):
+        b = next(b for b in (3 * 6 + 1, 3 * 7 + 1, 3 * 8 + 1, 3 * 9 + 1) if props[e, 7, b] != 0 and props[e, 7, b - 1] != 0 and props[e, 7, b + 1] != 0)
+        props[e, 7, b] = 0.0; victims.append(b)
+    world.props.copy_(torch.as_tensor(props))                     # the caller's buffer: visible to the next launch
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(state, props, B)
+    for step in range(5):
+        world.step(1)
+        trs = [orc.step_env(P, bod, float(wl.mu[e]), e=e, cache=cache, trace=True) for e in range(E)]
+        if step == 0:
+            torch.cuda.synchronize()
+            g = world.state.cpu().numpy().astype(np.float64)
+            for e in range(E):
+                got = world.pairs[e, :int(world.n_pairs[e].item())].cpu().numpy()
+                assert np.array_equal(got, trs[e]["pairs"])
+                assert all(victims[e] not in orc.pair_bodies(B, int(p)) for p in got)
+                x = np.transpose(g[e, 0:3, :B])
+                assert np.max(np.abs(x - bod.x[e])) < TOL_POS
+                assert np.array_equal(g[e, 0:7, victims[e]], state[e, 0:7, victims[e]].astype(np.float64))
+    torch.cuda.synchronize()
+    g = world.state.cpu().numpy().astype(np.float64)
+    for e in range(E):
+        x = np.transpose(g[e, 0:3, :B])
+        assert np.max(np.abs(x - bod.x[e])) < 5e-6                 # 5 steps of accumulated fp32 rounding
+    assert int(world.status.max().item()) == 0
