@@ -166,6 +166,15 @@ int jenga_block_threads(const jenga_world_desc *desc);
 
 const char *jenga_strerror(int code);
 
+/* Measured roofline denominators of this device: two micro-benchmarks on all SMs,
+ * out[0] = FP32 thread-instructions per second (dependent-free FFMA streams, FMA = 1 instruction),
+ * out[1] = shared-memory bytes per second (conflict-free LDS.128 streams), out[2] = SM count,
+ * out[3], out[4] = seconds of the two timed runs, out[5] = the FFMA rate with three register operands (out[0] has
+ * one uniform-register operand).  `out` is a HOST array of 6 doubles; `scratch` a DEVICE
+ * buffer of jenga_peaks_scratch_bytes() bytes.  Unlike the step calls this one synchronises the stream.  */
+int jenga_measure_peaks(double *out, void *scratch, void *cuda_stream);
+size_t jenga_peaks_scratch_bytes(void);
+
 #ifdef __cplusplus
 }
 #endif

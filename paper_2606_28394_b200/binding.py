@@ -66,6 +66,9 @@ def lib():
         L.jenga_smem_bytes.restype = C.c_size_t
         L.jenga_block_threads.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_strerror.argtypes = [C.c_int]
+        L.jenga_measure_peaks.argtypes = [C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
+        L.jenga_measure_peaks.restype = C.c_int
+        L.jenga_peaks_scratch_bytes.restype = C.c_size_t
         L.jenga_strerror.restype = C.c_char_p
         for f in ("jenga_world_create", "jenga_world_destroy", "jenga_broadphase", "jenga_narrowphase", "jenga_pgs_solve",
                   "jenga_step", "jenga_step_host", "jenga_simulate_until_rest", "jenga_set_f_ext", "jenga_block_threads"):
@@ -95,6 +98,20 @@ def make_desc(wp, materialise: bool = False, device: int = 0) -> WorldDesc:
     d.collapse_length = getattr(wp, "collapse_length", 0.0)
     d.collapse_fd, d.collapse_ek, d.collapse_theta = 0.5, 5.0e-5, 0.5235987755982988      # Eq. 18: f_d, eps_k [J], 30 deg
     return d
+
+
+def jenga_measure_peaks(device: int = 0) -> dict:
+    """FP32 issue rate and shared-memory bandwidth of the device, measured by the library's micro-benchmarks."""
+    if not torch.cuda.is_available():
+        raise JengaError("no CUDA device")
+    L = lib()
+    dev = torch.device("cuda", device)
+    scratch = torch.empty(L.jenga_peaks_scratch_bytes(), dtype=torch.uint8, device=dev)
+    out = (C.c_double * 6)()
+    with torch.cuda.device(dev):
+        _check(L.jenga_measure_peaks(out, C.c_void_p(scratch.data_ptr()), C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)),
+               "jenga_measure_peaks")
+    return dict(fp32_instr_per_s=out[0], smem_bytes_per_s=out[1], n_sm=int(out[2]), ffma_s=out[3], lds_s=out[4], fp32_instr_per_s_3reg=out[5])
 
 
 class World:
