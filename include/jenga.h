@@ -84,6 +84,10 @@ typedef struct {
   int32_t  device;                      /* CUDA device ordinal the buffers live on                     */
   float    collapse_length;             /* block length l of Eq. 18; latch off if <= 0 */
   float    collapse_fd, collapse_ek, collapse_theta;   /* f_d = 0.5, eps_k = 5e-5 J, theta_th = 30 deg in rad   */
+  int32_t  solver_tier;                 /* where the PGS kernel keeps the contact constants: 0 = auto (the fastest tier
+                                           that fits), 1 = shared memory only (one warp per CTA), 2 = tensor memory,
+                                           256 columns per 4-env CTA (two CTAs per SM), 3 = tensor memory, 512 columns
+                                           (one CTA per SM).  A tier that does not fit the sizes is JENGA_E_ARG.       */
 } jenga_world_desc;
 
 /* All DEVICE pointers, caller-owned, 16-byte aligned.  PC = max_contacts/4. */
@@ -114,9 +118,15 @@ typedef struct {
                                    held at the same step                                                */
   float       *collapse_stats; /* [E][4] of the last step: dx_max [m], E_k [J], theta_max [rad], 0     */
   int32_t     *rest_steps; /* [E]  steps taken by the last jenga_simulate_until_rest; may be NULL      */
+  void        *scratch;    /* jenga_scratch_bytes(desc) bytes, 16-byte aligned, ZERO-FILLED by the caller before the
+                              first call: the hand-off between the two kernels of a substep (pair headers, solver
+                              constants and colour chunks of every env) plus per-env bookkeeping (the colouring of the
+                              last pair list, the rest flag).  Contents are private to the library.              */
+  size_t       scratch_bytes;
 } jenga_buffers;
 
-/* Validates desc/buffers (sizes, alignment, device arch) and returns a host handle. */
+/* Validates desc/buffers (sizes, alignment, device arch) and returns a host handle.  desc.device must be the current
+ * CUDA device here and in every later call on the handle (JENGA_E_DEVICE otherwise).                    */
 int jenga_world_create(const jenga_world_desc *desc, const jenga_buffers *bufs, jenga_world **out);
 
 /* S2 on the current poses: state, props -> pairs, n_pairs.  Eq. 10.
@@ -132,16 +142,16 @@ int jenga_narrowphase(jenga_world *w, void *cuda_stream);
  * (read only) when desc.warm_start = 1 and n_cache[env] > 0.  Eq. 13-15, Listing 1.                   */
 int jenga_pgs_solve(jenga_world *w, int iters, void *cuda_stream);
 
-/* n_steps advances of dt (each n_substeps fused substeps S1..S7), one launch; state, cache,
- * status and counters are updated in place.                                                           */
+/* n_steps advances of dt (each n_substeps substeps S1..S7 = two kernel launches: detection + setup, then solve +
+ * integrate), all enqueued by this one call; state, cache, status and counters are updated in place.  */
 int jenga_step(jenga_world *w, int n_steps, void *cuda_stream);
 
 /* simulate_until_rest (§8.3): every env advances dt by dt until its total kinetic energy
  * E_k = sum_b 1/2 m |v|^2 + 1/2 w . I w, evaluated after every step, is below ek_rest, at most max_steps steps
- * (the paper: 400 steps, 1e-7 J); bufs.rest_steps[env] = steps taken (>= 1).  One launch: an env at rest stops
- * costing arithmetic, and its CTA retires as soon as all of the CTA's envs rest, which frees the SM for the next
- * CTA -- the grid scheduler does the active-env compaction.  f_ext, the warm-start cache and the collapse latch
- * behave as in jenga_step; counters add the steps actually taken.                                         */
+ * (the paper: 400 steps, 1e-7 J); bufs.rest_steps[env] = steps taken (>= 1).  The launches of max_steps steps are
+ * enqueued at once; an env at rest is flagged on the device and its warp leaves every later launch at once, so it
+ * stops costing arithmetic without a host round trip.  f_ext, the warm-start cache and the collapse latch behave
+ * as in jenga_step; counters add the steps actually taken.                                                */
 int jenga_simulate_until_rest(jenga_world *w, int max_steps, float ek_rest, void *cuda_stream);
 
 /* jenga_step with HOST state buffers (the end-to-end call): enqueues, on `cuda_stream`, a host->device copy
@@ -158,11 +168,14 @@ int jenga_set_f_ext(jenga_world *w, const float *f_ext);
 /* Frees the host handle (nothing on the device belongs to it). */
 int jenga_world_destroy(jenga_world *w);
 
-/* Dynamic shared memory per CTA the kernels need for this descriptor (0 if invalid). */
+/* Dynamic shared memory per CTA of the PGS kernel for this descriptor (0 if invalid). */
 size_t jenga_smem_bytes(const jenga_world_desc *desc);
 
-/* Threads per CTA (= one env) the kernels are launched with for this descriptor. */
+/* Threads per CTA of the PGS kernel (one warp per env: 128 = 4 envs per CTA in the tensor-memory tiers, 32 else). */
 int jenga_block_threads(const jenga_world_desc *desc);
+
+/* Size of jenga_buffers.scratch for this descriptor (0 if invalid). */
+size_t jenga_scratch_bytes(const jenga_world_desc *desc);
 
 const char *jenga_strerror(int code);
 

@@ -33,13 +33,17 @@ class WorldDesc(C.Structure):
                 ("edge_bias_rel", C.c_float), ("edge_bias_abs", C.c_float), ("par_eps", C.c_float), ("tie_eps", C.c_float),
                 ("match_tol", C.c_float), ("warm_start", C.c_int32), ("gyroscopic", C.c_int32), ("max_pairs", C.c_int32),
                 ("max_contacts", C.c_int32), ("materialise", C.c_int32), ("device", C.c_int32),
-                ("collapse_length", C.c_float), ("collapse_fd", C.c_float), ("collapse_ek", C.c_float), ("collapse_theta", C.c_float)]
+                ("collapse_length", C.c_float), ("collapse_fd", C.c_float), ("collapse_ek", C.c_float), ("collapse_theta", C.c_float),
+                ("solver_tier", C.c_int32)]
 
 
 class Buffers(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("state", "props", "mu", "f_ext", "pairs", "n_pairs", "contacts", "n_contacts",
                                           "lambda_", "cache_key", "cache_lam", "cache_pt", "n_cache", "status", "counters",
-                                          "ref_pose", "collapsed", "collapse_stats", "rest_steps")]
+                                          "ref_pose", "collapsed", "collapse_stats", "rest_steps", "scratch")] + [("scratch_bytes", C.c_size_t)]
+
+
+TIERS = {"auto": 0, "smem": 1, "tmem256": 2, "tmem512": 3}
 
 
 def lib():
@@ -65,6 +69,8 @@ def lib():
         L.jenga_smem_bytes.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_smem_bytes.restype = C.c_size_t
         L.jenga_block_threads.argtypes = [C.POINTER(WorldDesc)]
+        L.jenga_scratch_bytes.argtypes = [C.POINTER(WorldDesc)]
+        L.jenga_scratch_bytes.restype = C.c_size_t
         L.jenga_strerror.argtypes = [C.c_int]
         L.jenga_measure_peaks.argtypes = [C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
         L.jenga_measure_peaks.restype = C.c_int
@@ -82,7 +88,7 @@ def _check(code: int, what: str):
         raise JengaError(f"{what} failed ({code}): {lib().jenga_strerror(code).decode()}")
 
 
-def make_desc(wp, materialise: bool = False, device: int = 0) -> WorldDesc:
+def make_desc(wp, materialise: bool = False, device: int = 0, tier: str = "auto") -> WorldDesc:
     """wp: any object with the fields of workloads.WorldParams."""
     d = WorldDesc()
     d.struct_size = C.sizeof(WorldDesc)
@@ -97,6 +103,7 @@ def make_desc(wp, materialise: bool = False, device: int = 0) -> WorldDesc:
     d.materialise, d.device = int(materialise), device
     d.collapse_length = getattr(wp, "collapse_length", 0.0)
     d.collapse_fd, d.collapse_ek, d.collapse_theta = 0.5, 5.0e-5, 0.5235987755982988      # Eq. 18: f_d, eps_k [J], 30 deg
+    d.solver_tier = TIERS[tier]
     return d
 
 
@@ -121,7 +128,8 @@ class World:
     they are copied to the device once here.  All methods enqueue on torch's current stream.
     """
 
-    def __init__(self, wp, state, props, mu, materialise: bool = False, device: int = 0, collapse_length: float = 0.0):
+    def __init__(self, wp, state, props, mu, materialise: bool = False, device: int = 0, collapse_length: float = 0.0,
+                 tier: str = "auto"):
         if not torch.cuda.is_available():
             raise JengaError("no CUDA device: the Jenga step has no CPU path")
         self.wp = wp
@@ -146,8 +154,12 @@ class World:
         self.n_cache = z((E,), torch.int32)
         self.status = z((E,), torch.int32)
         self.counters = z((N_COUNTERS,), torch.int64)
-        self.desc = make_desc(wp, materialise, device)
+        self.desc = make_desc(wp, materialise, device, tier)
         self.desc.collapse_length = float(collapse_length)
+        n_scr = lib().jenga_scratch_bytes(C.byref(self.desc))
+        if n_scr == 0:
+            raise JengaError("jenga_scratch_bytes: the world descriptor is out of range")
+        self.scratch = z((n_scr,), torch.uint8)
         b = Buffers()
         b.state, b.props, b.mu, b.f_ext = self.state.data_ptr(), self.props.data_ptr(), self.mu.data_ptr(), None
         b.pairs, b.n_pairs = self.pairs.data_ptr(), self.n_pairs.data_ptr()
@@ -157,8 +169,9 @@ class World:
         self.ref_pose = self.collapsed = self.collapse_stats = None
         self.rest_steps = z((E,), torch.int32)
         b.rest_steps = self.rest_steps.data_ptr()
+        b.scratch, b.scratch_bytes = self.scratch.data_ptr(), n_scr
         if collapse_length > 0.0:                      # Eq. 18 latch against the pose the world starts from
-            self.ref_pose = self.state[:, 0:7, :].contiguous()
+            self.ref_pose = self.state[:, 0:7, :].clone()      # a copy also when E = 1 (contiguous() would alias the live state)
             self.collapsed = z((E,), torch.int32)
             self.collapse_stats = z((E, 4), torch.float32)
             b.ref_pose, b.collapsed, b.collapse_stats = self.ref_pose.data_ptr(), self.collapsed.data_ptr(), self.collapse_stats.data_ptr()

@@ -1,0 +1,658 @@
+// kcollide.cuh -- first kernel of a substep, one env per warp: S1 predict, S2 broadphase, S3 narrowphase, S4 contact
+// setup (effective masses, warm-start lookup) and the canonical colouring; its products go to the scratch buffer
+// (layout.cuh) for k_solve.
+#pragma once
+#include "layout.cuh"
+
+namespace jenga {
+
+// ---------------------------------------------------------------- shared-memory arena of one env
+struct CSm {
+  SP<float> cb;                 // [S][kCb] collision body records
+  SP<float> ext;                // [3][S]   world AABB half extents
+  SP<unsigned long long> used;  // [S]      colour masks per body
+  SP<unsigned> cab;             // [pcA]    (a+1) | A dynamic << 11 | axis << 12 | b << 16 | B dynamic << 27
+  SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending
+  SP<unsigned short> cpair;     // [pcA]    colliding pair indices, ascending
+  SP<unsigned short> cprev;     // [pcA]    pair indices of the warm-start cache (previous substep), ascending
+  SP<unsigned short> pos;       // [pcA]    position of pair r
+  SP<unsigned short> wrank;     // [pcA]    rank inside its colour / contact offset
+  SP<unsigned char> colour;     // [pcA]
+  SP<int> ph;                   // [ph_max] chunk descriptors in canonical order
+  SP<int> chc;                  // [ph_max] colour | first rank-in-colour << 8 of each chunk
+  SP<int> ccount;               // [64]
+  SP<int> cfirst;               // [64] first chunk of the colour
+  SP<int> fill;                 // [nblk] lanes taken in each block (packing)
+  SP<int> misc;                 // [8]
+};
+enum { MiNph = 0, MiNcol = 1, MiNblk = 2 };
+
+__host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc) {
+  const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc);
+  size_t w = (size_t)kCb * S + 3 * S + 2 * S;            // cb, ext, used
+  w += pcA;                                              // cab
+  w += mpA / 2;                                          // cand
+  w += 4 * (size_t)(pcA / 2);                            // cpair, cprev, pos, wrank
+  w += pcA / 4;                                          // colour
+  w += 2 * round_up(ph_max(nblk), 4);                    // ph, chc
+  w += 2 * kMaxColours + round_up(nblk, 4) + 8;          // ccount, cfirst, fill, misc
+  return round_up((int)w, 4);
+}
+
+__device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base) {
+  const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc), phw = round_up(ph_max(nblk), 4);
+  CSm s; int p = base;
+  s.cb.off = p;     p += kCb * S;
+  s.ext.off = p;    p += 3 * S;
+  if (p & 1) ++p;
+  s.used.off = p;   p += 2 * S;
+  s.cab.off = p;    p += pcA;
+  s.cand.off = p;   p += mpA / 2;
+  s.cpair.off = p;  p += pcA / 2;
+  s.cprev.off = p;  p += pcA / 2;
+  s.pos.off = p;    p += pcA / 2;
+  s.wrank.off = p;  p += pcA / 2;
+  s.colour.off = p; p += pcA / 4;
+  s.ph.off = p;     p += phw;
+  s.chc.off = p;    p += phw;
+  s.ccount.off = p; p += kMaxColours;
+  s.cfirst.off = p; p += kMaxColours;
+  s.fill.off = p;   p += round_up(nblk, 4);
+  s.misc.off = p;
+  return s;
+}
+
+__device__ __forceinline__ float4& cb4(const CSm& s, int b, int k) { return reinterpret_cast<float4*>(smem_f + s.cb.off + b * kCb)[k]; }
+
+__device__ __forceinline__ Box load_box(const CSm& s, int b) {
+  Box X;
+  const float4 x = cb4(s, b, 0), a0 = cb4(s, b, 1), a1 = cb4(s, b, 2), a2 = cb4(s, b, 3);
+  X.c = v3(x.x, x.y, x.z);
+  X.ax[0] = v3(a0.x, a0.y, a0.z); X.ax[1] = v3(a1.x, a1.y, a1.z); X.ax[2] = v3(a2.x, a2.y, a2.z);
+  X.he[0] = a0.w; X.he[1] = a1.w; X.he[2] = a2.w;
+  return X;
+}
+
+// ---------------------------------------------------------------- S1: load, R, Iw^-1, AABB extents, velocity predict
+// state [13][S] and props [8][S] of one env are contiguous in HBM; lane b reads column b of every row (coalesced).
+// Eq. 1, I_world^-1 = R diag(I_body^-1) R^T, e'_k = sum_j |R_kj| e_j;
+// v += h (g + f/m), w += h Iw^-1 (tau [- w x Iw w]) (Eq. 5; reading A2): written back to `state`.
+__device__ inline void load_predict(const CSm& s, const Params& P, int env, bool predict) {
+  const int S = P.S;
+  float* st = P.state + (size_t)env * kStateRows * S;
+  const float* pr = P.props + (size_t)env * kPropRows * S;
+  for (int b = lane_id(); b < P.B; b += 32) {
+    const float px = st[b], py = st[S + b], pz = st[2 * S + b];
+    const float w = st[3 * S + b], x = st[4 * S + b], y = st[5 * S + b], z = st[6 * S + b];
+    const float im = pr[b], i0r = pr[S + b], i1r = pr[2 * S + b], i2r = pr[3 * S + b];
+    const float hx = pr[4 * S + b], hy = pr[5 * S + b], hz = pr[6 * S + b];
+    const bool act = pr[7 * S + b] != 0.0f, dyn = act && im != 0.0f;
+    float R[9]; quat_to_R(w, x, y, z, R);
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+      s.ext[k * S + b] = fabsf(R[3 * k]) * hx + fabsf(R[3 * k + 1]) * hy + fabsf(R[3 * k + 2]) * hz;
+    float I6[6];
+    world_inv_inertia(R, dyn ? i0r : 0.0f, dyn ? i1r : 0.0f, dyn ? i2r : 0.0f, I6);
+    cb4(s, b, 0) = make_float4(px, py, pz, dyn ? im : 0.0f);
+    cb4(s, b, 1) = make_float4(R[0], R[3], R[6], hx);        // body axis k = column k of R
+    cb4(s, b, 2) = make_float4(R[1], R[4], R[7], hy);
+    cb4(s, b, 3) = make_float4(R[2], R[5], R[8], hz);
+    cb4(s, b, 4) = make_float4(I6[0], I6[1], I6[2], I6[3]);
+    cb4(s, b, 5) = make_float4(I6[4], I6[5], act ? 1.0f : 0.0f, dyn ? 1.0f : 0.0f);
+    cb4(s, b, 6) = make_float4(w, x, y, z);
+    if (!predict || !dyn) continue;
+    float f[6] = { 0, 0, 0, 0, 0, 0 };
+    if (P.f_ext) {
+      const float* fe = P.f_ext + (size_t)env * kFextRows * S;
+#pragma unroll
+      for (int k = 0; k < 6; ++k) f[k] = fe[k * S + b];
+    }
+    float vx = st[7 * S + b], vy = st[8 * S + b], vz = st[9 * S + b];
+    const Vec3 wv = v3(st[10 * S + b], st[11 * S + b], st[12 * S + b]);
+    vx += P.h * (P.g[0] + im * f[0]); vy += P.h * (P.g[1] + im * f[1]); vz += P.h * (P.g[2] + im * f[2]);
+    Vec3 tau = v3(f[3], f[4], f[5]);
+    if (P.gyroscopic) {                  // I_world w = R diag(I_body) R^T w
+      const float wb0 = R[0] * wv.x + R[3] * wv.y + R[6] * wv.z, wb1 = R[1] * wv.x + R[4] * wv.y + R[7] * wv.z,
+                  wb2 = R[2] * wv.x + R[5] * wv.y + R[8] * wv.z;
+      const float l0 = wb0 / i0r, l1 = wb1 / i1r, l2 = wb2 / i2r;
+      const Vec3 Lw = v3(R[0] * l0 + R[1] * l1 + R[2] * l2, R[3] * l0 + R[4] * l1 + R[5] * l2, R[6] * l0 + R[7] * l1 + R[8] * l2);
+      tau = tau - cross(wv, Lw);
+    }
+    const Vec3 dw = sym_mul(I6, tau);
+    st[7 * S + b] = vx; st[8 * S + b] = vy; st[9 * S + b] = vz;
+    st[10 * S + b] = wv.x + P.h * dw.x; st[11 * S + b] = wv.y + P.h * dw.y; st[12 * S + b] = wv.z + P.h * dw.z;
+  }
+  __syncwarp();
+}
+
+// fp64 re-evaluation of one Eq. 10 test, every operation rounded separately (no FMA), in the order
+// R from q (Eq. 1), e'_k = |R_k0| e_0 + |R_k1| e_1 + |R_k2| e_2, slack_k = (e'_i,k + e'_j,k + eps) - |x_i,k - x_j,k|.
+// Used only when the fp32 slack is within 1e-5 m of zero, so that the pair list equals the fp64 definition.
+#define DM(a, b) __dmul_rn((a), (b))
+#define DA(a, b) __dadd_rn((a), (b))
+#define DS(a, b) __dsub_rn((a), (b))
+__device__ __noinline__ void ext_f64(const CSm& s, int b, double* e3) {
+  const float4 q4 = cb4(s, b, 6);
+  const double w = q4.x, x = q4.y, y = q4.z, z = q4.w;
+  const double hx = cb4(s, b, 1).w, hy = cb4(s, b, 2).w, hz = cb4(s, b, 3).w;
+  double R[9];
+  R[0] = DS(1.0, DM(2.0, DA(DM(y, y), DM(z, z)))); R[1] = DM(2.0, DS(DM(x, y), DM(z, w))); R[2] = DM(2.0, DA(DM(x, z), DM(y, w)));
+  R[3] = DM(2.0, DA(DM(x, y), DM(z, w))); R[4] = DS(1.0, DM(2.0, DA(DM(x, x), DM(z, z)))); R[5] = DM(2.0, DS(DM(y, z), DM(x, w)));
+  R[6] = DM(2.0, DS(DM(x, z), DM(y, w))); R[7] = DM(2.0, DA(DM(y, z), DM(x, w))); R[8] = DS(1.0, DM(2.0, DA(DM(x, x), DM(y, y))));
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+    e3[k] = DA(DA(DM(fabs(R[3 * k]), hx), DM(fabs(R[3 * k + 1]), hy)), DM(fabs(R[3 * k + 2]), hz));
+}
+
+__device__ __noinline__ bool aabb_test_f64(const CSm& s, const Params& P, int i, int j) {
+  const double eps = (double)P.aabb_margin;
+  double ej[3]; ext_f64(s, j, ej);
+  const float4 xj = cb4(s, j, 0);
+  if (i < 0) return DS(eps, DS((double)xj.z, ej[2])) >= 0.0;
+  double ei[3]; ext_f64(s, i, ei);
+  const float4 xi = cb4(s, i, 0);
+  const double ci[3] = { xi.x, xi.y, xi.z }, cj[3] = { xj.x, xj.y, xj.z };
+  double smin = 1e300;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const double slack = DS(DA(DA(ei[k], ej[k]), eps), fabs(DS(ci[k], cj[k])));
+    if (slack < smin) smin = slack;
+  }
+  return smin >= 0.0;
+}
+#undef DM
+#undef DA
+#undef DS
+
+// S2: ground tests, then all body pairs, in ascending canonical pair index; 32 tests per round, hits
+// compacted with __ballot_sync/__popc into s.cand (Eq. 10; ground test reading A6).
+// Returns the number of candidates kept (<= max_pairs); sets PAIR_OVERFLOW in *status.
+__device__ inline int broadphase(const CSm& s, const Params& P, unsigned* status) {
+  const int B = P.B, S = P.S, lane = lane_id();
+  const float eps = P.aabb_margin;
+  const unsigned below = (1u << lane) - 1u;
+  int n = 0;
+  for (int base = 0; base < B; base += 32) {               // ground: pair index = b
+    const int j = base + lane;
+    bool hit = false;
+    if (j < B && cb4(s, j, 5).w != 0.0f) {
+      const float sl = eps - (cb4(s, j, 0).z - s.ext[2 * S + j]);
+      hit = sl >= 0.0f;
+      if (fabsf(sl) < 1.0e-5f) hit = aabb_test_f64(s, P, -1, j);
+    }
+    const unsigned bal = __ballot_sync(kFull, hit);
+    const int rank = n + __popc(bal & below);
+    if (hit && rank < P.max_pairs) s.cand[rank] = (unsigned short)j;
+    n += __popc(bal);
+  }
+  const int n_bp = B * (B - 1) / 2;
+  int i = 0, col = lane;                                   // lane's pair: row i, column col (j = i + 1 + col)
+  for (int base = 0; base < n_bp; base += 32) {
+    while (i < B - 1 && col >= B - 1 - i) { col -= B - 1 - i; ++i; }
+    bool hit = false;
+    const int j = i + 1 + col;
+    if (i < B - 1) {
+      const float4 xi = cb4(s, i, 0), xj = cb4(s, j, 0);
+      const bool consider = cb4(s, i, 5).z != 0.0f && cb4(s, j, 5).z != 0.0f && (xi.w != 0.0f || xj.w != 0.0f);
+      if (consider) {
+        const float s0 = (s.ext[i] + s.ext[j] + eps) - fabsf(xi.x - xj.x);
+        const float s1 = (s.ext[S + i] + s.ext[S + j] + eps) - fabsf(xi.y - xj.y);
+        const float s2 = (s.ext[2 * S + i] + s.ext[2 * S + j] + eps) - fabsf(xi.z - xj.z);
+        const float smin = fminf(s0, fminf(s1, s2));
+        hit = smin >= 0.0f;
+        if (fabsf(smin) < 1.0e-5f) hit = aabb_test_f64(s, P, i, j);
+      }
+    }
+    const unsigned bal = __ballot_sync(kFull, hit);
+    const int rank = n + __popc(bal & below);
+    if (hit && rank < P.max_pairs) s.cand[rank] = (unsigned short)(B + i * (2 * B - i - 1) / 2 + col);
+    n += __popc(bal);
+    col += 32;
+  }
+  if (n > P.max_pairs) { *status |= JENGA_ST_PAIR_OVERFLOW; n = P.max_pairs; }
+  __syncwarp();
+  return n;
+}
+
+// cab word of a colliding pair: (a+1) bits 0-10 | A dynamic bit 11 | SAT axis bits 12-15 | b bits 16-26 | B dynamic bit 27
+__device__ __forceinline__ unsigned pack_ab(const CSm& s, int a, int b, int axis) {
+  unsigned w = (unsigned)(a + 1) | ((unsigned)axis << 12) | ((unsigned)b << 16);
+  if (a >= 0 && cb4(s, a, 0).w != 0.0f) w |= 1u << 11;
+  if (cb4(s, b, 0).w != 0.0f) w |= 1u << 27;
+  return w;
+}
+__device__ __forceinline__ int ab_a(unsigned w) { return (int)(w & 0x7ffu) - 1; }
+__device__ __forceinline__ int ab_b(unsigned w) { return (int)((w >> 16) & 0x7ffu); }
+__device__ __forceinline__ int ab_axis(unsigned w) { return (int)((w >> 12) & 0xfu); }
+
+// Manifold of colliding pair (a, b) whose SAT axis is known (find_colliding stored it).
+__device__ __forceinline__ void pair_manifold(const CSm& s, int a, int b, int axis, Manifold& m) {
+  const Box Bj = load_box(s, b);
+  if (a < 0) { collide_ground(Bj, m); return; }
+  const Box Bi = load_box(s, a);
+  SatResult sr; sat_axis(Bi, Bj, axis, sr);
+  manifold_boxes(Bi, Bj, sr, m);
+}
+
+// S3, first half: which candidates collide (15-axis SAT / a ground corner below z = 0).  Lane k of a
+// round takes candidate base+k; the colliding ones are compacted in ascending pair index into
+// s.cpair / s.cab.  Returns the number kept (<= pc); sets CONTACT_OVERFLOW.
+__device__ inline int find_colliding(const CSm& s, const Params& P, int n_cand, unsigned* status) {
+  const int lane = lane_id();
+  const unsigned below = (1u << lane) - 1u;
+  int n = 0;
+  for (int base = 0; base < n_cand; base += 32) {
+    const int k = base + lane;
+    bool hit = false; int idx = 0, i = -1, j = 0, axis = JENGA_AXIS_GROUND;
+    if (k < n_cand) {
+      idx = s.cand[k];
+      pair_bodies(P.B, idx, i, j);
+      const Box Bj = load_box(s, j);
+      if (i < 0) hit = ground_hit(Bj);
+      else { const Box Bi = load_box(s, i); SatResult sr; sr.axis = 0; hit = sat_boxes(P.cp, Bi, Bj, sr); axis = sr.axis; }
+    }
+    const unsigned bal = __ballot_sync(kFull, hit);
+    const int rank = n + __popc(bal & below);
+    if (hit && rank < P.pc) { s.cpair[rank] = (unsigned short)idx; s.cab[rank] = pack_ab(s, i, j, axis); }
+    n += __popc(bal);
+  }
+  if (n > P.pc) { *status |= JENGA_ST_CONTACT_OVERFLOW; n = P.pc; }
+  __syncwarp();
+  return n;
+}
+
+// Canonical order (north_star (d), DESIGN §2 S4): visit the colliding pairs in ascending pair index;
+// colour = lowest colour not used by an earlier pair sharing a dynamic body.  The pairs of a colour are then cut
+// into chunks of consecutive lanes of one 32-position block (bin packing, lowest block first: whole if a block has
+// room, else split over the emptiest blocks); s.ph lists the chunks colour by colour = the order the solver visits
+// them, s.pos[r] = 32 block + lane of pair r.  The walk is sequential by definition (lane 0, one 64-bit mask per
+// body).  When the colliding-pair list equals the one the scratch was coloured for, that colouring (the same
+// function of the same input) is kept: the steady state of a standing tower.
+__device__ inline void colour_pairs(const CSm& s, const Params& P, float* scr, const Scratch& L, int n_coll, unsigned* status) {
+  const int lane = lane_id();
+  int* meta = reinterpret_cast<int*>(scr + L.meta);
+  unsigned short* gpos = reinterpret_cast<unsigned short*>(scr + L.pos);
+  unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
+  bool same = meta[MetaMagic] == kMagic && meta[MetaNcoll] == n_coll;
+  if (same)
+    for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
+  same = __all_sync(kFull, same);
+  if (same) {
+    for (int r = lane; r < n_coll; r += 32) s.pos[r] = gpos[r];
+    if (lane == 0) { s.misc[MiNph] = meta[MetaNph]; s.misc[MiNcol] = meta[MetaNcol]; s.misc[MiNblk] = meta[MetaNblk]; }
+    __syncwarp();
+    return;
+  }
+  const int nblk = P.nblk;
+  for (int b = lane; b < P.B; b += 32) s.used[b] = 0ull;
+  for (int c = lane; c < kMaxColours; c += 32) s.ccount[c] = 0;
+  __syncwarp();
+  if (lane == 0) {
+    int ncol = 0; unsigned st = 0;
+    for (int r = 0; r < n_coll; ++r) {
+      const unsigned w = s.cab[r];
+      const int a = ab_a(w), b = ab_b(w);
+      unsigned long long m = 0ull;
+      if (w & (1u << 11)) m |= s.used[a];
+      if (w & (1u << 27)) m |= s.used[b];
+      int c = __ffsll((long long)~m) - 1;
+      if (c < 0) { c = kMaxColours - 1; st |= JENGA_ST_COLOUR_OVERFLOW; }
+      if (a >= 0) s.used[a] |= 1ull << c;
+      s.used[b] |= 1ull << c;
+      s.colour[r] = (unsigned char)c;
+      const int k = s.ccount[c];
+      s.wrank[r] = (unsigned short)k; s.ccount[c] = k + 1;
+      if (c + 1 > ncol) ncol = c + 1;
+    }
+    // bin packing: fill[j] = lanes taken in block j (taken from lane 0 upwards)
+    const SP<int> fill = s.fill;
+    for (int j = 0; j < nblk; ++j) fill[j] = 0;
+    int nph = 0, top = 0;
+    for (int c = 0; c < ncol; ++c) {
+      int n = s.ccount[c], w0 = 0;
+      s.cfirst[c] = nph;
+      while (n > 0) {
+        int take = n > 32 ? 32 : n, jb = -1;
+        for (int j = 0; j < nblk; ++j) if (32 - fill[j] >= take) { jb = j; break; }
+        if (jb < 0) {                                         // no block holds it whole: the emptiest block takes what fits
+          int best = 0;
+          for (int j = 0; j < nblk; ++j) if (32 - fill[j] > best) { best = 32 - fill[j]; jb = j; }
+          take = best;
+        }
+        s.ph[nph] = ph_pack(jb, fill[jb], take); s.chc[nph] = c | (w0 << 8); ++nph;
+        fill[jb] += take; w0 += take; n -= take;
+        if (jb + 1 > top) top = jb + 1;
+      }
+    }
+    s.misc[MiNcol] = ncol; s.misc[MiNph] = nph; s.misc[MiNblk] = top;
+    if (st) *status |= st;
+  }
+  __syncwarp();
+  const int nph = s.misc[MiNph];
+  for (int r = lane; r < n_coll; r += 32) {
+    const int c = s.colour[r], w = s.wrank[r];
+    int j = s.cfirst[c], k = 0;
+    for (; j < nph; ++j) {
+      const int d = s.ph[j], w0 = s.chc[j] >> 8, cnt = (d >> 8) & 0xff;
+      if (w >= w0 && w < w0 + cnt) { k = 32 * (d >> 16) + (d & 0xff) + (w - w0); break; }
+    }
+    s.pos[r] = (unsigned short)k;
+    gpos[r] = (unsigned short)k; gpair[r] = s.cpair[r];
+  }
+  int* gph = reinterpret_cast<int*>(scr + L.ph);
+  for (int j = lane; j < nph; j += 32) gph[j] = s.ph[j];
+  if (lane == 0) {
+    meta[MetaMagic] = kMagic; meta[MetaNcoll] = n_coll; meta[MetaNph] = nph; meta[MetaNcol] = s.misc[MiNcol]; meta[MetaNblk] = s.misc[MiNblk];
+  }
+  __syncwarp();
+}
+
+// ---------------------------------------------------------------- pair slots (solver constants at a position)
+// Header of position k (scratch: hdr[f * npos + k]):
+//   0: ab = (a+1) | b << 16, meta = np | axis << 8 | pair index << 16, rank r of the pair, 1/|e_k - n (n.e_k)|
+//   1: n.x n.y n.z, Baumgarte corr = beta max(0, depth_max - slop) / (imA + imB)     (Eq. 16)
+//   2: t1.x t1.y t1.z, 0
+// Contact constants of position k: 48 words.  ro[9c..9c+8] = p.xyz, (1+e)/K_nn, 1/K_t1t1, 1/K_t2t2,
+// K_n,t1, K_n,t2, K_t1,t2 of contact c (K_dd: Eq. 13, for d = n, t1, t2); lam[3c..3c+2] = jn, jt1, jt2.
+struct PairC { float v[48]; };      // v[0..35] read-only constants, v[36..47] impulses
+constexpr int kLam = 36;
+
+struct Frame { Vec3 n, t1, t2; };
+
+// t1 = normalise(e_k - n (n.e_k)), k = x unless |n_x| > 1/sqrt(2), then y;  t2 = n x t1   (DESIGN §3 R-basis)
+__device__ __forceinline__ void tangent_raw(Vec3 n, Vec3& u) {
+  const bool usey = fabsf(n.x) > 0.70710678118654752f;
+  const float d = usey ? n.y : n.x;
+  u = v3(fmaf(-d, n.x, usey ? 0.0f : 1.0f), fmaf(-d, n.y, usey ? 1.0f : 0.0f), -d * n.z);
+}
+__device__ __forceinline__ Frame make_frame(Vec3 n, float il) {
+  Frame F; F.n = n;
+  Vec3 u; tangent_raw(n, u);
+  F.t1 = il * u;
+  F.t2 = cross(n, F.t1);
+  return F;
+}
+
+struct BodyK { float4 x, i0, i1; };           // x.w = inverse mass (0: static / inactive / ground)
+__device__ __forceinline__ void load_bodyk(const CSm& s, int b, BodyK& o) {
+  if (b >= 0) { o.x = cb4(s, b, 0); o.i0 = cb4(s, b, 4); o.i1 = cb4(s, b, 5); }
+  else o.x = o.i0 = o.i1 = make_float4(0, 0, 0, 0);
+}
+__device__ __forceinline__ Vec3 imul(const BodyK& B, Vec3 a) {      // Iw^-1 a
+  return v3(fmaf(B.i0.z, a.z, fmaf(B.i0.y, a.y, B.i0.x * a.x)),
+            fmaf(B.i1.x, a.z, fmaf(B.i0.w, a.y, B.i0.y * a.x)),
+            fmaf(B.i1.y, a.z, fmaf(B.i1.x, a.y, B.i0.z * a.x)));
+}
+__device__ __forceinline__ Vec3 xyz(float4 v) { return v3(v.x, v.y, v.z); }
+
+// S4 for one colliding pair: header and constants of position k from the pair's manifold, written to the scratch.
+// Warm start (DESIGN §3 R-warm): a new contact inherits (jn,jt1,jt2) of the nearest not yet taken previous contact
+// point of the same pair within match_tol; slots ascending.  The previous pair list is s.cprev (ascending).
+__device__ inline void setup_slot(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int nprev,
+                                  int k, int r, int a, int b, int pair, const Manifold& m) {
+  BodyK A, Bb; load_bodyk(s, a, A); load_bodyk(s, b, Bb);
+  const Vec3 n = m.n;
+  Vec3 u; tangent_raw(n, u);
+  const float il = rsqrtf(dot(u, u));
+  const Frame F = make_frame(n, il);
+  const Vec3 dir[3] = { F.n, F.t1, F.t2 };
+  const float im = A.x.w + Bb.x.w;
+  float lam[4][3]; Vec3 pt[4];
+  float dmax = 0.0f;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) { lam[c][0] = lam[c][1] = lam[c][2] = 0.0f; pt[c] = v3(0, 0, 0); }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) if (c < m.np) { pt[c] = m.p[c]; dmax = fmaxf(dmax, m.d[c]); }
+
+  if (P.warm_start && nprev > 0) {
+    int lo = 0, hi = nprev;
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)s.cprev[mid] < pair) lo = mid + 1; else hi = mid; }
+    if (lo < nprev && (int)s.cprev[lo] == pair) {
+      const int ocnt = P.cache_key[((size_t)env * P.pc + lo) * 2 + 1] & 0xff;
+      const float4* ol4 = reinterpret_cast<const float4*>(P.cache_lam + ((size_t)env * P.pc + lo) * 12);
+      const float4* op4 = reinterpret_cast<const float4*>(P.cache_pt + ((size_t)env * P.pc + lo) * 12);
+      float ol[12], op[12];
+#pragma unroll
+      for (int f = 0; f < 3; ++f) {
+        const float4 a4 = ol4[f], b4 = op4[f];
+        ol[4 * f] = a4.x; ol[4 * f + 1] = a4.y; ol[4 * f + 2] = a4.z; ol[4 * f + 3] = a4.w;
+        op[4 * f] = b4.x; op[4 * f + 1] = b4.y; op[4 * f + 2] = b4.z; op[4 * f + 3] = b4.w;
+      }
+      unsigned taken = 0;
+      const float tol2 = P.match_tol * P.match_tol;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        if (c < m.np) {
+          int bo = -1; float bdist = tol2;
+#pragma unroll
+          for (int o = 0; o < 4; ++o)
+            if (o < ocnt && !((taken >> o) & 1u)) {
+              const Vec3 d = pt[c] - v3(op[3 * o], op[3 * o + 1], op[3 * o + 2]); const float dd = dot(d, d);
+              if (dd < bdist) { bdist = dd; bo = o; }
+            }
+#pragma unroll
+          for (int o = 0; o < 4; ++o)
+            if (o == bo) { taken |= 1u << o; lam[c][0] = ol[3 * o]; lam[c][1] = ol[3 * o + 1]; lam[c][2] = ol[3 * o + 2]; }
+        }
+      }
+    }
+  }
+
+  const int npos = 32 * P.nblk;
+  float4* hdr = reinterpret_cast<float4*>(scr + L.hdr);
+  const int meta = m.np | (m.axis << 8) | (pair << 16);
+  hdr[k] = make_float4(__int_as_float((a + 1) | (b << 16)), __int_as_float(meta), __int_as_float(r), il);
+  hdr[npos + k] = make_float4(n.x, n.y, n.z, im > 0.0f ? P.beta * fmaxf(0.0f, dmax - P.slop) / im : 0.0f);
+  hdr[2 * npos + k] = make_float4(F.t1.x, F.t1.y, F.t1.z, 0.0f);
+  const float e1 = 1.0f + P.restitution;
+  PairC out;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    float ik[3] = { 0, 0, 0 }, ko[3] = { 0, 0, 0 };
+    if (c < m.np) {
+      const Vec3 rA = a >= 0 ? pt[c] - xyz(A.x) : v3(0, 0, 0), rB = pt[c] - xyz(Bb.x);
+      Vec3 uA[3], uB[3], wA[3], wB[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        uA[d] = cross(rA, dir[d]); uB[d] = cross(rB, dir[d]);
+        wA[d] = imul(A, uA[d]); wB[d] = imul(Bb, uB[d]);
+      }
+#pragma unroll
+      for (int d = 0; d < 3; ++d) ik[d] = 1.0f / (im + dot(uA[d], wA[d]) + dot(uB[d], wB[d]));
+      ik[0] *= e1;
+      ko[0] = dot(uA[0], wA[1]) + dot(uB[0], wB[1]);
+      ko[1] = dot(uA[0], wA[2]) + dot(uB[0], wB[2]);
+      ko[2] = dot(uA[1], wA[2]) + dot(uB[1], wB[2]);
+    }
+    float* o = out.v + 9 * c;
+    o[0] = pt[c].x; o[1] = pt[c].y; o[2] = pt[c].z; o[3] = ik[0]; o[4] = ik[1]; o[5] = ik[2]; o[6] = ko[0]; o[7] = ko[1]; o[8] = ko[2];
+    out.v[kLam + 3 * c] = lam[c][0]; out.v[kLam + 3 * c + 1] = lam[c][1]; out.v[kLam + 3 * c + 2] = lam[c][2];
+  }
+  float4* cs = reinterpret_cast<float4*>(scr + L.cs) + (size_t)(k >> 5) * (kCsF4 * 32) + (k & 31);
+#pragma unroll
+  for (int f = 0; f < kCsF4; ++f) cs[f * 32] = make_float4(out.v[4 * f], out.v[4 * f + 1], out.v[4 * f + 2], out.v[4 * f + 3]);
+}
+
+// The warm-start cache's pair list (ascending) into shared memory.
+__device__ inline int load_prev_keys(const CSm& s, const Params& P, int env) {
+  int nprev = P.warm_start ? P.n_cache[env] : 0;
+  nprev = max(0, min(nprev, P.pc));
+  const int* keys = P.cache_key + (size_t)env * P.pc * 2;
+  for (int r = lane_id(); r < nprev; r += 32) s.cprev[r] = (unsigned short)keys[2 * r];
+  __syncwarp();
+  return nprev;
+}
+
+// S3 second half + S4: lane l of a round takes colliding pair r = 32 round + l (ascending pair index), computes its
+// manifold (the SAT axis is known) and writes header and constants at the pair's position.
+__device__ inline void setup_pairs(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_coll, int nprev) {
+  for (int r = lane_id(); r < n_coll; r += 32) {
+    const unsigned w = s.cab[r];
+    const int a = ab_a(w), b = ab_b(w);
+    Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
+    pair_manifold(s, a, b, ab_axis(w), m);
+    setup_slot(s, P, env, scr, L, nprev, s.pos[r], r, a, b, s.cpair[r], m);
+  }
+  __syncwarp();
+}
+
+// ---------------------------------------------------------------- materialised outputs (stage calls / parity)
+__device__ inline void write_pairs(const CSm& s, const Params& P, int env, int n_cand) {
+  int* out = P.pairs + (size_t)env * P.max_pairs;
+  for (int k = lane_id(); k < n_cand; k += 32) out[k] = s.cand[k];
+  if (lane_id() == 0) P.n_pairs[env] = n_cand;
+  __syncwarp();
+}
+
+__device__ inline int load_candidates(const CSm& s, const Params& P, int env) {
+  int n_cand = P.n_pairs[env];
+  n_cand = max(0, min(n_cand, P.max_pairs));
+  for (int k = lane_id(); k < n_cand; k += 32) s.cand[k] = (unsigned short)P.pairs[(size_t)env * P.max_pairs + k];
+  __syncwarp();
+  return n_cand;
+}
+
+__device__ __forceinline__ int warp_excl_scan(int v, int* total) {
+  const int lane = lane_id();
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += t; }
+  *total = __shfl_sync(kFull, inc, 31);
+  return inc - v;
+}
+
+// Contact list in (pair, slot) order: the manifolds are recomputed from the (unchanged) poses in ascending
+// pair order.  Leaves s.wrank[r] = contact offset of pair r (also written to the scratch for the lambda output).
+__device__ inline int write_contacts(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_cand, int n_coll) {
+  const int lane = lane_id();
+  unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
+  int off0 = 0;
+  for (int base = 0; base < n_coll; base += 32) {
+    const int r = base + lane;
+    Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
+    int idx = 0;
+    if (r < n_coll) {
+      const unsigned w = s.cab[r];
+      idx = s.cpair[r];
+      pair_manifold(s, ab_a(w), ab_b(w), ab_axis(w), m);
+    }
+    int tot; const int off = off0 + warp_excl_scan(m.np, &tot);
+    if (r < n_coll) {
+      s.wrank[r] = (unsigned short)off; gcoff[r] = (unsigned short)off;
+      int lo = 0, hi = n_cand;                                   // position of the pair in the candidate list
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)s.cand[mid] < idx) lo = mid + 1; else hi = mid; }
+      float4* out = reinterpret_cast<float4*>(P.contacts + ((size_t)env * P.max_contacts + off) * 8);
+      for (int c = 0; c < m.np; ++c) {
+        const int tag = (lo & 0xffff) | (c << 16) | (m.axis << 20);
+        out[2 * c] = make_float4(m.n.x, m.n.y, m.n.z, m.d[c]);
+        out[2 * c + 1] = make_float4(m.p[c].x, m.p[c].y, m.p[c].z, __int_as_float(tag));
+      }
+    }
+    off0 += tot;
+  }
+  if (lane == 0) { P.n_contacts[env] = off0; reinterpret_cast<int*>(scr + L.meta)[MetaNcont] = off0; }
+  __syncwarp();
+  return off0;
+}
+
+// Rebuild the colliding-pair list from a contact list in global memory (ordered (pair, slot); slot 0 carries
+// the pair's normal): s.cpair, s.cab, s.wrank[r] = offset of the pair's first contact.
+__device__ inline int pairs_from_contacts(const CSm& s, const Params& P, int env, int n_cont, unsigned* status) {
+  const int lane = lane_id();
+  const unsigned below = (1u << lane) - 1u;
+  const float4* in = reinterpret_cast<const float4*>(P.contacts + (size_t)env * P.max_contacts * 8);
+  const int* pairs = P.pairs + (size_t)env * P.max_pairs;
+  int n = 0;
+  for (int base = 0; base < n_cont; base += 32) {
+    const int c = base + lane;
+    bool first = false; int tag = 0;
+    if (c < n_cont) { tag = __float_as_int(in[2 * c + 1].w); first = ((tag >> 16) & 3) == 0; }
+    const unsigned bal = __ballot_sync(kFull, first);
+    const int rank = n + __popc(bal & below);
+    if (first && rank < P.pc) {
+      const int idx = pairs[tag & 0xffff];
+      int i, j; pair_bodies(P.B, idx, i, j);
+      s.cpair[rank] = (unsigned short)idx; s.cab[rank] = pack_ab(s, i, j, (tag >> 20) & 0xf); s.wrank[rank] = (unsigned short)c;
+    }
+    n += __popc(bal);
+  }
+  if (n > P.pc) { *status |= JENGA_ST_CONTACT_OVERFLOW; n = P.pc; }
+  __syncwarp();
+  return n;
+}
+
+// ModeGiven (jenga_pgs_solve): slots from the contact list the caller supplied instead of the narrowphase.
+__device__ inline void setup_given(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_coll, int n_cont, int nprev) {
+  const float4* in = reinterpret_cast<const float4*>(P.contacts + (size_t)env * P.max_contacts * 8);
+  unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
+  for (int r = lane_id(); r < n_coll; r += 32) {
+    const int c0 = gcoff[r], c1 = r + 1 < n_coll ? gcoff[r + 1] : n_cont;
+    const unsigned w = s.cab[r];
+    Manifold m; m.np = min(4, c1 - c0);
+    const float4 f0 = in[2 * c0];
+    m.n = v3(f0.x, f0.y, f0.z);
+    m.axis = (__float_as_int(in[2 * c0 + 1].w) >> 20) & 0xf;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      m.p[c] = v3(0, 0, 0); m.d[c] = 0.0f;
+      if (c < m.np) { const float4 a4 = in[2 * (c0 + c)], b4 = in[2 * (c0 + c) + 1]; m.p[c] = v3(b4.x, b4.y, b4.z); m.d[c] = a4.w; }
+    }
+    setup_slot(s, P, env, scr, L, nprev, s.pos[r], r, ab_a(w), ab_b(w), s.cpair[r], m);
+  }
+  __syncwarp();
+}
+
+// ---------------------------------------------------------------- the kernel
+// mode: ModeStep (fused substep, first half), ModeBroad (jenga_broadphase), ModeNarrow (jenga_narrowphase),
+// ModeGiven (first half of jenga_pgs_solve).  honour_rest: envs whose scratch says "at rest" are skipped
+// (jenga_simulate_until_rest).
+__global__ void __launch_bounds__(128, 4) k_collide(const Params P, const int mode, const int honour_rest) {
+  const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
+  const int env = blockIdx.x * wpc + warp;
+  if (env >= P.E) return;
+  const Scratch L = scratch_layout(P.pc);
+  float* scr = P.scratch + (size_t)env * P.scratch_words;
+  int* meta = reinterpret_cast<int*>(scr + L.meta);
+  if (honour_rest && meta[MetaResting]) return;
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc));
+  unsigned st = 0;
+  load_predict(s, P, env, mode == ModeStep);
+  int n_cand = 0, n_coll = 0;
+  if (mode == ModeStep || mode == ModeBroad) {
+    n_cand = broadphase(s, P, &st);
+    if (mode == ModeBroad || P.materialise) write_pairs(s, P, env, n_cand);
+  } else if (mode == ModeNarrow) {
+    n_cand = load_candidates(s, P, env);
+  }
+  if (mode == ModeStep || mode == ModeNarrow) {
+    n_coll = find_colliding(s, P, n_cand, &st);
+    if (mode == ModeNarrow || P.materialise) write_contacts(s, P, env, scr, L, n_cand, n_coll);
+  }
+  if (mode == ModeStep || mode == ModeGiven) {
+    const int nprev = load_prev_keys(s, P, env);
+    int n_cont = 0;
+    if (mode == ModeGiven) {
+      n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
+      n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
+      unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
+      for (int r = lane; r < n_coll; r += 32) gcoff[r] = s.wrank[r];       // the colouring reuses s.wrank
+      if (lane == 0) meta[MetaNcont] = n_cont;
+      __syncwarp();
+    }
+    colour_pairs(s, P, scr, L, n_coll, &st);
+    if (mode == ModeGiven) setup_given(s, P, env, scr, L, n_coll, n_cont, nprev);
+    else setup_pairs(s, P, env, scr, L, n_coll, nprev);
+    if (P.counters && mode == ModeStep && lane == 0) {
+      const int ncol = s.misc[MiNcol];
+      atomicAdd(P.counters + JENGA_CNT_CANDIDATES, (unsigned long long)n_cand);
+      atomicAdd(P.counters + JENGA_CNT_COLLIDING, (unsigned long long)n_coll);
+      atomicAdd(P.counters + JENGA_CNT_COLOURS, (unsigned long long)ncol);
+      atomicMax(P.counters + JENGA_CNT_MAX_CANDIDATES, (unsigned long long)n_cand);
+      atomicMax(P.counters + JENGA_CNT_MAX_COLLIDING, (unsigned long long)n_coll);
+      atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
+    }
+  }
+  flush_status(P, env, st);
+}
+
+}  // namespace jenga

@@ -1,0 +1,486 @@
+// ksolve.cuh -- second kernel of a substep, one env per warp: S4 warm-start application, S5 coloured PGS sweeps,
+// S6 integration + Baumgarte, S7 warm-start cache, Eq. 18 latch.  Inputs: the state tile and the scratch k_collide wrote.
+//
+// Two flavours (template <bool TM>):
+//   TM = true   CTA = 4 warps = 4 envs; the 48 constant words of the positions of the first `tmb` 32-position blocks
+//               live in tensor memory (tcgen05.ld/st.32x32b: lane = position % 32, block j at columns [48 j, 48 j + 48),
+//               warp w owns TMEM lanes 32 w .. 32 w + 31); tmb = 5: 256 columns per CTA, 2 CTAs per SM (8 envs per SM);
+//               tmb = 10: 512 columns, 1 CTA per SM.  Blocks >= tmb are kept in shared memory.
+//   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers).
+#pragma once
+#include "kcollide.cuh"
+
+namespace jenga {
+
+struct SSm {
+  SP<float> bd;                 // [S][kBd] solver body records
+  SP<float> q;                  // [4][S]
+  SP<float4> hdr;               // [kHdrF4][npos]
+  SP<float4> cs;                // [nblk - tmb][kCsF4][32] blocks kept in shared memory
+  SP<int> ph;                   // [ph_max]
+  int npos, tmb;
+  unsigned tm;                  // TMEM address of this warp's lanes, column 0
+};
+
+__host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb) {
+  const int nblk = n_blocks(pc);
+  size_t w = (size_t)(kBd + 4) * S + 4 * kHdrF4 * 32 * (size_t)nblk;
+  w += (size_t)kBlkWords * (nblk > tmb ? nblk - tmb : 0);
+  w += round_up(ph_max(nblk), 4);
+  return round_up((int)w, 4);
+}
+
+__device__ inline SSm carve_solve(int S, int pc, int tmb, int base) {
+  const int nblk = n_blocks(pc);
+  SSm s; int p = base;
+  s.npos = 32 * nblk; s.tmb = tmb; s.tm = 0;
+  s.hdr.off = p; p += 4 * kHdrF4 * s.npos;
+  s.cs.off = p;  p += kBlkWords * (nblk > tmb ? nblk - tmb : 0);
+  s.bd.off = p;  p += kBd * S;
+  s.q.off = p;   p += 4 * S;
+  s.ph.off = p;
+  return s;
+}
+
+__device__ __forceinline__ float4& bd4(const SSm& s, int b, int k) { return reinterpret_cast<float4*>(smem_f + s.bd.off + b * kBd)[k]; }
+__device__ __forceinline__ float4& hdr4(const SSm& s, int f, int k) { return s.hdr[f * s.npos + k]; }
+
+// ---------------------------------------------------------------- TMEM access
+__device__ __forceinline__ void tm_ld16(unsigned a, float* r) {
+  unsigned* u = reinterpret_cast<unsigned*>(r);
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+               : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]), "=r"(u[6]), "=r"(u[7]),
+                 "=r"(u[8]), "=r"(u[9]), "=r"(u[10]), "=r"(u[11]), "=r"(u[12]), "=r"(u[13]), "=r"(u[14]), "=r"(u[15]) : "r"(a));
+}
+__device__ __forceinline__ void tm_st16(unsigned a, const float* r) {
+  const unsigned* u = reinterpret_cast<const unsigned*>(r);
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+               :: "r"(a), "r"(u[0]), "r"(u[1]), "r"(u[2]), "r"(u[3]), "r"(u[4]), "r"(u[5]), "r"(u[6]), "r"(u[7]),
+                  "r"(u[8]), "r"(u[9]), "r"(u[10]), "r"(u[11]), "r"(u[12]), "r"(u[13]), "r"(u[14]), "r"(u[15]) : "memory");
+}
+__device__ __forceinline__ void tm_st4(unsigned a, const float* r) {
+  const unsigned* u = reinterpret_cast<const unsigned*>(r);
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" :: "r"(a), "r"(u[0]), "r"(u[1]), "r"(u[2]), "r"(u[3]) : "memory");
+}
+__device__ __forceinline__ void tm_st8(unsigned a, const float* r) {
+  const unsigned* u = reinterpret_cast<const unsigned*>(r);
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               :: "r"(a), "r"(u[0]), "r"(u[1]), "r"(u[2]), "r"(u[3]), "r"(u[4]), "r"(u[5]), "r"(u[6]), "r"(u[7]) : "memory");
+}
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// whole block j (all 32 lanes take part; lane l gets position 32 j + l)
+__device__ __forceinline__ void tm_load_block(const SSm& s, int j, PairC& c) {
+  const unsigned a = s.tm + 48u * (unsigned)j;
+  tm_ld16(a, c.v); tm_ld16(a + 16, c.v + 16); tm_ld16(a + 32, c.v + 32);
+}
+__device__ __forceinline__ void tm_store_block(const SSm& s, int j, const PairC& c) {
+  const unsigned a = s.tm + 48u * (unsigned)j;
+  tm_st16(a, c.v); tm_st16(a + 16, c.v + 16); tm_st16(a + 32, c.v + 32);
+}
+__device__ __forceinline__ void tm_store_lam(const SSm& s, int j, const float* lam) {
+  const unsigned a = s.tm + 48u * (unsigned)j + 36u;
+  tm_st8(a, lam); tm_st4(a + 8, lam + 8);
+}
+// shared-memory tier: block j >= tmb, lane l
+__device__ __forceinline__ void sm_load_pair(const SSm& s, int j, int l, PairC& c) {
+  const float4* b = s.cs.ptr() + (j - s.tmb) * (kCsF4 * 32) + l;
+#pragma unroll
+  for (int f = 0; f < kCsF4; ++f) { const float4 t = b[f * 32]; c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
+}
+__device__ __forceinline__ void sm_store_pair(const SSm& s, int j, int l, const PairC& c) {
+  float4* b = s.cs.ptr() + (j - s.tmb) * (kCsF4 * 32) + l;
+#pragma unroll
+  for (int f = 0; f < kCsF4; ++f) b[f * 32] = make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]);
+}
+__device__ __forceinline__ void sm_store_lam(const SSm& s, int j, int l, const float* lam) {
+  float4* b = s.cs.ptr() + (j - s.tmb) * (kCsF4 * 32) + l;
+#pragma unroll
+  for (int f = 0; f < 3; ++f) b[(9 + f) * 32] = make_float4(lam[4 * f], lam[4 * f + 1], lam[4 * f + 2], lam[4 * f + 3]);
+}
+// block j of this env: lane l <-> position 32 j + l.  All lanes call these.
+template <bool TM>
+__device__ __forceinline__ void block_load(const SSm& s, int j, PairC& c) {
+  if (TM && j < s.tmb) { tm_load_block(s, j, c); tm_wait_ld(); }
+  else sm_load_pair(s, j, lane_id(), c);
+}
+
+// ---------------------------------------------------------------- warp / TMEM set-up
+template <bool TM>
+__device__ __forceinline__ SSm begin_solve(const Params& P, int& env) {
+  __shared__ unsigned tm_base_s;
+  const int warp = threadIdx.x >> 5;
+  env = blockIdx.x * (TM ? 4 : 1) + warp;
+  const int tmb = TM ? P.tmb : 0, cols = tmb > 5 ? 512 : 256;
+  SSm s = carve_solve(P.S, P.pc, tmb, warp * (int)solve_smem_words(P.S, P.pc, tmb));
+  if (TM) {
+    if (warp == 0) {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                   :: "r"((unsigned)__cvta_generic_to_shared(&tm_base_s)), "r"(cols) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    s.tm = tm_base_s + ((unsigned)(warp * 32) << 16);
+  }
+  return s;
+}
+
+template <bool TM>
+__device__ __forceinline__ void end_solve(const SSm& s) {
+  if (TM) {
+    const int cols = s.tmb > 5 ? 512 : 256;
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if ((threadIdx.x >> 5) == 0)
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s.tm), "r"(cols) : "memory");   // warp 0: s.tm = base
+  }
+}
+
+// ---------------------------------------------------------------- load
+// Body records from the state tile (lane b reads column b of every row: coalesced); Iw^-1 from q (Eq. 1).
+// Spare words of the record keep the body-frame inverse moments (kinetic energy, Eq. 18).
+__device__ inline void load_bodies(const SSm& s, const Params& P, int env) {
+  const int S = P.S;
+  const float* st = P.state + (size_t)env * kStateRows * S;
+  const float* pr = P.props + (size_t)env * kPropRows * S;
+  for (int b = lane_id(); b < P.B; b += 32) {
+    const float w = st[3 * S + b], x = st[4 * S + b], y = st[5 * S + b], z = st[6 * S + b];
+    const float im = pr[b], i0 = pr[S + b], i1 = pr[2 * S + b], i2 = pr[3 * S + b];
+    const bool dyn = pr[7 * S + b] != 0.0f && im != 0.0f;
+    float R[9]; quat_to_R(w, x, y, z, R);
+    float I6[6];
+    world_inv_inertia(R, dyn ? i0 : 0.0f, dyn ? i1 : 0.0f, dyn ? i2 : 0.0f, I6);
+    bd4(s, b, 0) = make_float4(st[b], st[S + b], st[2 * S + b], dyn ? im : 0.0f);
+    bd4(s, b, 1) = make_float4(st[7 * S + b], st[8 * S + b], st[9 * S + b], i0);
+    bd4(s, b, 2) = make_float4(st[10 * S + b], st[11 * S + b], st[12 * S + b], i1);
+    bd4(s, b, 3) = make_float4(I6[0], I6[1], I6[2], I6[3]);
+    bd4(s, b, 4) = make_float4(I6[4], I6[5], i2, 0.0f);
+    s.q[b] = w; s.q[S + b] = x; s.q[2 * S + b] = y; s.q[3 * S + b] = z;
+  }
+}
+
+__device__ inline void store_bodies(const SSm& s, const Params& P, int env) {
+  const int S = P.S;
+  float* st = P.state + (size_t)env * kStateRows * S;
+  for (int b = lane_id(); b < P.B; b += 32) {
+    const float4 x = bd4(s, b, 0), v = bd4(s, b, 1), w = bd4(s, b, 2);
+    if (x.w == 0.0f) continue;                                   // static / inactive bodies are never written
+    st[b] = x.x; st[S + b] = x.y; st[2 * S + b] = x.z;
+    st[3 * S + b] = s.q[b]; st[4 * S + b] = s.q[S + b]; st[5 * S + b] = s.q[2 * S + b]; st[6 * S + b] = s.q[3 * S + b];
+    st[7 * S + b] = v.x; st[8 * S + b] = v.y; st[9 * S + b] = v.z;
+    st[10 * S + b] = w.x; st[11 * S + b] = w.y; st[12 * S + b] = w.z;
+  }
+}
+
+// Chunk list, headers and constant blocks of this env from the scratch.  Returns the number of chunks.
+template <bool TM>
+__device__ inline int load_slots(const SSm& s, const Params& P, const float* scr, const Scratch& L) {
+  const int lane = lane_id();
+  const int* meta = reinterpret_cast<const int*>(scr + L.meta);
+  const int nph = meta[MetaNph], nblk = meta[MetaNblk];
+  const int* gph = reinterpret_cast<const int*>(scr + L.ph);
+  for (int j = lane; j < nph; j += 32) s.ph[j] = gph[j];
+  const float4* ghdr = reinterpret_cast<const float4*>(scr + L.hdr);
+  for (int f = 0; f < kHdrF4; ++f)
+    for (int k = lane; k < 32 * nblk; k += 32) s.hdr[f * s.npos + k] = ghdr[f * s.npos + k];
+  const float4* gcs = reinterpret_cast<const float4*>(scr + L.cs);
+  for (int j = 0; j < nblk; ++j) {
+    PairC c;
+#pragma unroll
+    for (int f = 0; f < kCsF4; ++f) {
+      const float4 t = gcs[(j * kCsF4 + f) * 32 + lane];
+      c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w;
+    }
+    if (TM && j < s.tmb) tm_store_block(s, j, c);
+    else sm_store_pair(s, j, lane, c);
+  }
+  if (TM) tm_wait_st();
+  __syncwarp();
+  return nph;
+}
+
+struct Body5 { float4 x, v, w, i0, i1; };     // x.w = inverse mass (0: static / inactive / ground)
+
+__device__ __forceinline__ void load_body(const SSm& s, int b, Body5& o) {
+  if (b >= 0) {
+    o.x = bd4(s, b, 0); o.v = bd4(s, b, 1); o.w = bd4(s, b, 2); o.i0 = bd4(s, b, 3); o.i1 = bd4(s, b, 4);
+  } else {
+    o.x = o.v = o.w = o.i0 = o.i1 = make_float4(0, 0, 0, 0);
+  }
+}
+
+// a loses the impulse, b gains it (Listing 1, PAPER.md:335-336 + the angular lines, reading A11)
+__device__ __forceinline__ void apply_impulse(Body5& A, Body5& B, Vec3 rA, Vec3 rB, Vec3 Pi) {
+  A.v.x = fmaf(-A.x.w, Pi.x, A.v.x); A.v.y = fmaf(-A.x.w, Pi.y, A.v.y); A.v.z = fmaf(-A.x.w, Pi.z, A.v.z);
+  B.v.x = fmaf(B.x.w, Pi.x, B.v.x);  B.v.y = fmaf(B.x.w, Pi.y, B.v.y);  B.v.z = fmaf(B.x.w, Pi.z, B.v.z);
+  const Vec3 cA = cross(Pi, rA), cB = cross(rB, Pi);        // -(rA x Pi), +(rB x Pi)
+  A.w.x = fmaf(A.i0.z, cA.z, fmaf(A.i0.y, cA.y, fmaf(A.i0.x, cA.x, A.w.x)));
+  A.w.y = fmaf(A.i1.x, cA.z, fmaf(A.i0.w, cA.y, fmaf(A.i0.y, cA.x, A.w.y)));
+  A.w.z = fmaf(A.i1.y, cA.z, fmaf(A.i1.x, cA.y, fmaf(A.i0.z, cA.x, A.w.z)));
+  B.w.x = fmaf(B.i0.z, cB.z, fmaf(B.i0.y, cB.y, fmaf(B.i0.x, cB.x, B.w.x)));
+  B.w.y = fmaf(B.i1.x, cB.z, fmaf(B.i0.w, cB.y, fmaf(B.i0.y, cB.x, B.w.y)));
+  B.w.z = fmaf(B.i1.y, cB.z, fmaf(B.i1.x, cB.y, fmaf(B.i0.z, cB.x, B.w.z)));
+}
+
+// One chunk visit of the warm-start application (S4) or of a Gauss-Seidel sweep (S5).  The chunk's pairs are lanes
+// [lane0, lane0 + count) of block j; slots ascending; per contact the normal row (Eq. 14, clamp >= 0), then t1, then
+// t2 (Eq. 15, each clipped to +-mu_s jn) -- Listing 1.  The three rows of a contact act on the same
+// two bodies: the relative velocity of the contact point is read once, advanced between rows with the contact-space
+// couplings K_ij (exactly the change the applied impulse causes), and the summed impulse is applied once (DESIGN §3
+// R-couple).  Pairs of one colour share no dynamic body.  TMEM stores are warp-wide: the lanes outside the chunk
+// write back the impulses they loaded.
+template <bool TM, bool WARM>
+__device__ __forceinline__ void solve_chunk(const SSm& s, int d, float mu) {
+  const int lane = lane_id();
+  const int j = d >> 16, lane0 = d & 0xff, count = (d >> 8) & 0xff;
+  const bool active = lane >= lane0 && lane < lane0 + count;
+  const bool in_tm = TM && j < s.tmb;
+  const int k = 32 * j + lane;
+  PairC c;
+  if (in_tm) { tm_load_block(s, j, c); tm_wait_ld(); }
+  else if (active) sm_load_pair(s, j, lane, c);
+  if (active) {
+    const float4 h = hdr4(s, 0, k), nn = hdr4(s, 1, k), tt = hdr4(s, 2, k);
+    const int ab = __float_as_int(h.x), a = (ab & 0xffff) - 1, b = ab >> 16, np = __float_as_int(h.y) & 0xff;
+    Body5 A, B; load_body(s, a, A); load_body(s, b, B);
+    Frame F; F.n = xyz(nn); F.t1 = xyz(tt); F.t2 = cross(F.n, F.t1);
+#pragma unroll
+    for (int ci = 0; ci < 4; ++ci)
+      if (ci < np) {
+        const float* r = c.v + 9 * ci; float* l = c.v + kLam + 3 * ci;
+        const Vec3 p = v3(r[0], r[1], r[2]), rA = p - xyz(A.x), rB = p - xyz(B.x);
+        Vec3 Pi;
+        if (WARM) {
+          Pi = madd(madd(l[0] * F.n, l[1], F.t1), l[2], F.t2);
+        } else {
+          // vr = (vB + wB x rB) - (vA + wA x rA), each component one subtraction and four fused multiply-adds
+          const Vec3 vr = v3(
+            fmaf(A.w.z, rA.y, fmaf(-A.w.y, rA.z, fmaf(-B.w.z, rB.y, fmaf(B.w.y, rB.z, B.v.x - A.v.x)))),
+            fmaf(A.w.x, rA.z, fmaf(-A.w.z, rA.x, fmaf(-B.w.x, rB.z, fmaf(B.w.z, rB.x, B.v.y - A.v.y)))),
+            fmaf(A.w.y, rA.x, fmaf(-A.w.x, rA.y, fmaf(-B.w.y, rB.x, fmaf(B.w.x, rB.y, B.v.z - A.v.z)))));
+          const float u0 = dot(vr, F.n);
+          float u1 = dot(vr, F.t1), u2 = dot(vr, F.t2);
+          const float nw = fmaxf(fmaf(-u0, r[3], l[0]), 0.0f);
+          const float d0 = nw - l[0];
+          u1 = fmaf(r[6], d0, u1); u2 = fmaf(r[7], d0, u2);
+          const float lim = mu * nw;
+          const float n1 = fminf(fmaxf(fmaf(-u1, r[4], l[1]), -lim), lim);
+          const float d1 = n1 - l[1];
+          u2 = fmaf(r[8], d1, u2);
+          const float n2 = fminf(fmaxf(fmaf(-u2, r[5], l[2]), -lim), lim);
+          const float d2 = n2 - l[2];
+          l[0] = nw; l[1] = n1; l[2] = n2;
+          Pi = madd(madd(d0 * F.n, d1, F.t1), d2, F.t2);
+        }
+        apply_impulse(A, B, rA, rB, Pi);
+      }
+    if (a >= 0) { bd4(s, a, 1) = A.v; bd4(s, a, 2) = A.w; }
+    bd4(s, b, 1) = B.v; bd4(s, b, 2) = B.w;
+    if (!WARM && !in_tm) sm_store_lam(s, j, lane, c.v + kLam);
+  }
+  if (!WARM && in_tm) { tm_store_lam(s, j, c.v + kLam); tm_wait_st(); }
+  __syncwarp();
+}
+
+// S4 (warm-start application) + S5: the chunks in canonical order, `iters` sweeps.
+template <bool TM>
+__device__ inline void pgs_sweeps(const SSm& s, const Params& P, int nph, int iters, float mu) {
+  if (P.warm_start)
+    for (int j = 0; j < nph; ++j) solve_chunk<TM, true>(s, s.ph[j], mu);
+  for (int it = 0; it < iters; ++it)
+    for (int j = 0; j < nph; ++j) solve_chunk<TM, false>(s, s.ph[j], mu);
+}
+
+// S6: x += h v (Eq. 6); q <- normalise(q + h/2 [0,w] (x) q) (Eq. 2, world-frame
+// reading A3); then Eq. 16 (reading A14) once per colliding pair, chunk by chunk.
+__device__ inline void integrate(const SSm& s, const Params& P, int nph, unsigned* status) {
+  const int S = P.S, lane = lane_id(); const float h = P.h;
+  for (int b = lane; b < P.B; b += 32) {
+    float4 x = bd4(s, b, 0);
+    if (x.w == 0.0f) continue;                                   // static or inactive
+    const float4 v = bd4(s, b, 1), om = bd4(s, b, 2);
+    x.x += h * v.x; x.y += h * v.y; x.z += h * v.z;
+    bd4(s, b, 0) = x;
+    const float qw = s.q[b], qx = s.q[S + b], qy = s.q[2 * S + b], qz = s.q[3 * S + b];
+    const float dw = -(om.x * qx + om.y * qy + om.z * qz);
+    const float dx = om.x * qw + om.y * qz - om.z * qy;
+    const float dy = om.y * qw + om.z * qx - om.x * qz;
+    const float dz = om.z * qw + om.x * qy - om.y * qx;
+    const float hh = 0.5f * h;
+    const float nw = qw + hh * dw, nx = qx + hh * dx, ny = qy + hh * dy, nz = qz + hh * dz;
+    const float il = 1.0f / sqrtf(nw * nw + nx * nx + ny * ny + nz * nz);
+    s.q[b] = nw * il; s.q[S + b] = nx * il; s.q[2 * S + b] = ny * il; s.q[3 * S + b] = nz * il;
+    const float chk = (x.x + x.y + x.z) + (v.x + v.y + v.z) + (om.x + om.y + om.z) + il;      // any inf/NaN poisons the sum
+    if (!isfinite(chk)) *status |= JENGA_ST_NONFINITE;
+  }
+  __syncwarp();
+  for (int j = 0; j < nph; ++j) {
+    const int d = s.ph[j], lane0 = d & 0xff, count = (d >> 8) & 0xff, k = 32 * (d >> 16) + lane;
+    float4 nn = make_float4(0, 0, 0, 0);
+    if (lane >= lane0 && lane < lane0 + count) nn = hdr4(s, 1, k);
+    if (__any_sync(kFull, nn.w > 0.0f)) {
+      if (nn.w > 0.0f) {
+        const int ab = __float_as_int(hdr4(s, 0, k).x), a = (ab & 0xffff) - 1, b = ab >> 16;
+        float4 xb = bd4(s, b, 0);
+        if (xb.w != 0.0f) {
+          const float f = xb.w * nn.w;
+          xb.x += f * nn.x; xb.y += f * nn.y; xb.z += f * nn.z;
+          bd4(s, b, 0) = xb;
+        }
+        if (a >= 0) {
+          float4 xa = bd4(s, a, 0);
+          if (xa.w != 0.0f) {
+            const float f = xa.w * nn.w;
+            xa.x -= f * nn.x; xa.y -= f * nn.y; xa.z -= f * nn.z;
+            bd4(s, a, 0) = xa;
+          }
+        }
+      }
+      __syncwarp();
+    }
+  }
+}
+
+// Per-body terms of Eq. 18 / PAPER.md:380: kinetic energy 1/2 m |v|^2 + 1/2 w . I w with I in the body frame
+// (R^T w against the principal moments, R from the new q, Eq. 1).
+__device__ __forceinline__ float body_kinetic_energy(const SSm& s, int S, int b, float4 x, float4 v, float4 w, float i2) {
+  const float qw = s.q[b], qx = s.q[S + b], qy = s.q[2 * S + b], qz = s.q[3 * S + b];
+  float R[9]; quat_to_R(qw, qx, qy, qz, R);
+  const float w0 = R[0] * w.x + R[3] * w.y + R[6] * w.z, w1 = R[1] * w.x + R[4] * w.y + R[7] * w.z, w2 = R[2] * w.x + R[5] * w.y + R[8] * w.z;
+  return 0.5f * (v.x * v.x + v.y * v.y + v.z * v.z) / x.w + 0.5f * (w0 * w0 / v.w + w1 * w1 / w.w + w2 * w2 / i2);
+}
+
+// Collapse latch (Eq. 18, reading A17) after a dt advance: dx_max = max_b |x_b - x_b(0)|,
+// theta_max = max_b 2 acos|q_b . q_b(0)|, E_k; collapsed |= all three above their thresholds at this step.
+// Returns E_k (all lanes).
+__device__ inline float collapse_latch(const SSm& s, const Params& P, int env, bool latch) {
+  const int S = P.S, lane = lane_id();
+  const float* ref = latch ? P.ref_pose + (size_t)env * 7 * S : nullptr;
+  float dxm = 0.0f, thm = 0.0f, ek = 0.0f;
+  for (int b = lane; b < P.B; b += 32) {
+    const float4 x = bd4(s, b, 0);
+    if (x.w == 0.0f) continue;
+    const float4 v = bd4(s, b, 1), w = bd4(s, b, 2);
+    ek += body_kinetic_energy(s, S, b, x, v, w, bd4(s, b, 4).z);
+    if (latch) {
+      const float dx = x.x - ref[b], dy = x.y - ref[S + b], dz = x.z - ref[2 * S + b];
+      dxm = fmaxf(dxm, sqrtf(dx * dx + dy * dy + dz * dz));
+      const float c = fminf(fabsf(s.q[b] * ref[3 * S + b] + s.q[S + b] * ref[4 * S + b] + s.q[2 * S + b] * ref[5 * S + b] + s.q[3 * S + b] * ref[6 * S + b]), 1.0f);
+      thm = fmaxf(thm, 2.0f * acosf(c));
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    dxm = fmaxf(dxm, __shfl_xor_sync(kFull, dxm, o)); thm = fmaxf(thm, __shfl_xor_sync(kFull, thm, o));
+    ek += __shfl_xor_sync(kFull, ek, o);
+  }
+  if (latch && lane == 0) {
+    if (dxm > P.collapse_dx && ek > P.collapse_ek && thm > P.collapse_theta) P.collapsed[env] = 1;
+    if (P.collapse_stats) *reinterpret_cast<float4*>(P.collapse_stats + (size_t)env * 4) = make_float4(dxm, ek, thm, 0.0f);
+  }
+  return ek;
+}
+
+// S7: every pair's impulses and contact points become the next substep's warm-start cache, in ascending
+// pair order (cache entry r = pair rank r, from the header).  Returns the lane's (contacts, ground contacts).
+template <bool TM>
+__device__ inline int2 store_cache(const SSm& s, const Params& P, int env, const float* scr, const Scratch& L, int nph, bool cache_out, bool lambda_out) {
+  const int lane = lane_id();
+  const unsigned short* gcoff = reinterpret_cast<const unsigned short*>(scr + L.coff);
+  int nc = 0, ng = 0;
+  for (int j = 0; j < nph; ++j) {
+    const int d = s.ph[j], jb = d >> 16, lane0 = d & 0xff, count = (d >> 8) & 0xff, k = 32 * jb + lane;
+    PairC c; block_load<TM>(s, jb, c);
+    if (lane >= lane0 && lane < lane0 + count) {
+      const float4 hd = hdr4(s, 0, k);
+      const int meta = __float_as_int(hd.y), np = meta & 0xff, r = __float_as_int(hd.z);
+      nc += np; if ((__float_as_int(hd.x) & 0xffff) == 0) ng += np;
+      if (cache_out) {
+        int* key = P.cache_key + ((size_t)env * P.pc + r) * 2;
+        key[0] = (int)((unsigned)meta >> 16); key[1] = meta & 0xfff;
+        float4* ol = reinterpret_cast<float4*>(P.cache_lam + ((size_t)env * P.pc + r) * 12);
+        float4* op = reinterpret_cast<float4*>(P.cache_pt + ((size_t)env * P.pc + r) * 12);
+        float l[12], p[12];
+#pragma unroll
+        for (int ci = 0; ci < 4; ++ci)
+#pragma unroll
+          for (int t = 0; t < 3; ++t) { l[3 * ci + t] = ci < np ? c.v[kLam + 3 * ci + t] : 0.0f; p[3 * ci + t] = c.v[9 * ci + t]; }
+#pragma unroll
+        for (int f = 0; f < 3; ++f) {
+          ol[f] = make_float4(l[4 * f], l[4 * f + 1], l[4 * f + 2], l[4 * f + 3]);
+          op[f] = make_float4(p[4 * f], p[4 * f + 1], p[4 * f + 2], p[4 * f + 3]);
+        }
+      }
+      if (lambda_out) {                                          // lambda in contact order (debug / stage output)
+        float* out = P.lambda + ((size_t)env * P.max_contacts + gcoff[r]) * 3;
+#pragma unroll
+        for (int ci = 0; ci < 4; ++ci)
+          if (ci < np) { out[3 * ci] = c.v[kLam + 3 * ci]; out[3 * ci + 1] = c.v[kLam + 3 * ci + 1]; out[3 * ci + 2] = c.v[kLam + 3 * ci + 2]; }
+      }
+    }
+  }
+  return make_int2(nc, ng);
+}
+
+// ---------------------------------------------------------------- the kernel
+// flags: bit 0 end of a dt step (latch, counters, rest test), bit 1 PGS only (jenga_pgs_solve: no integration, no cache),
+// bit 2 honour / update the per-env rest flag (jenga_simulate_until_rest).
+enum { SolveEndOfStep = 1, SolvePgsOnly = 2, SolveRest = 4 };
+
+template <bool TM>
+__global__ void __launch_bounds__(TM ? 128 : 32, TM ? 2 : 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
+  int env;
+  const SSm s = begin_solve<TM>(P, env);
+  const int lane = lane_id();
+  const Scratch L = scratch_layout(P.pc);
+  float* scr = P.scratch + (size_t)(env < P.E ? env : 0) * P.scratch_words;
+  int* meta = reinterpret_cast<int*>(scr + L.meta);
+  const bool valid = env < P.E && !((flags & SolveRest) && meta[MetaResting]);
+  if (valid) {
+    unsigned st = 0;
+    load_bodies(s, P, env);
+    const int nph = load_slots<TM>(s, P, scr, L);
+    pgs_sweeps<TM>(s, P, nph, iters, P.mu[env]);
+    if (flags & SolvePgsOnly) {
+      store_cache<TM>(s, P, env, scr, L, nph, false, true);      // lambda in contact order only
+      store_bodies(s, P, env);
+    } else {
+      integrate(s, P, nph, &st);
+      const int2 cc = store_cache<TM>(s, P, env, scr, L, nph, true, P.materialise != 0);
+      if (lane == 0) P.n_cache[env] = meta[MetaNcoll];
+      store_bodies(s, P, env);
+      const bool eos = flags & SolveEndOfStep;
+      if (eos && (P.collapsed || (flags & SolveRest))) {
+        const float ek = collapse_latch(s, P, env, P.collapsed != nullptr);
+        if ((flags & SolveRest) && lane == 0) {
+          const int steps = meta[MetaSteps] + 1;
+          meta[MetaSteps] = steps;
+          if (P.rest_steps) P.rest_steps[env] = steps;
+          if (ek < rest_ek) meta[MetaResting] = 1;
+        }
+      }
+      if (P.counters) {
+        const unsigned long long v = warp_sum((unsigned long long)cc.x), vg = warp_sum((unsigned long long)cc.y);
+        int n_active = 0;
+        for (int b = lane; b < P.B; b += 32) n_active += s.bd[b * kBd + 3] != 0.0f ? 1 : 0;
+        n_active = __reduce_add_sync(kFull, n_active);
+        if (lane == 0) {
+          atomicAdd(P.counters + JENGA_CNT_CONTACTS, v);
+          atomicAdd(P.counters + JENGA_CNT_CONTACT_ITERS, v * (unsigned long long)iters);
+          atomicAdd(P.counters + JENGA_CNT_GROUND_CONTACTS, vg);
+          if (eos) {
+            atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, 1ull);
+            atomicAdd(P.counters + JENGA_CNT_BODY_STEPS, (unsigned long long)n_active);
+          }
+        }
+      }
+    }
+    flush_status(P, env, st);
+  }
+  end_solve<TM>(s);
+}
+
+}  // namespace jenga
