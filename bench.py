@@ -235,11 +235,15 @@ def run_cuda(args) -> dict:
         world.jenga_step(min(args.chunk, K))
     reset()
 
+    # ---- roofline denominators measured on this device now (FP32 FFMA issue rate, LDS.128 bandwidth)
+    peaks = binding.jenga_measure_peaks(local)
+
     # ---- device-resident timing: inputs already in HBM, CUDA events on the launching stream
     launches = list(schedule(wl, K, args.chunk))
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(len(launches) + 1)]
     sampler = ClockSampler(local); sampler.start()
     barrier()
+    world.jenga_profile_enable(True)                         # CUDA events around every kernel launch of the step (same stream)
     ev[0].record(stream)
     for i, (s, n, active) in enumerate(launches):
         set_push(active)
@@ -249,6 +253,8 @@ def run_cuda(args) -> dict:
     clocks = sampler.stop()
     ms = ev[0].elapsed_time(ev[-1])
     launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(len(launches))]
+    prof = world.jenga_profile_read()
+    world.jenga_profile_enable(False)
     cnt = world.counters_dict()
     status_or = int(np.bitwise_or.reduce(world.status.cpu().numpy()))
     n_flagged = int((world.status != 0).sum().item())
@@ -304,25 +310,45 @@ def run_cuda(args) -> dict:
     value = total_env_steps / (ms * 1e-3)
     e2e_value = E * Ke * world_size / (ms_e2e * 1e-3)
 
-    # ---- roofline of the (only) kernel, k_step: algorithmic FP32 thread-instructions / launch time vs FP32 issue peak
+    # ---- roofline.  Two kernels per substep: k_collide (S1-S4) and k_solve (S4 warm start, S5, S6, S7), timed
+    # separately with CUDA events on the launching stream (jenga_profile_*).  `roofline` is the dominant kernel
+    # (k_solve): its algorithmic FP32 thread-instructions / its summed launch time vs the FP32 issue rate measured by
+    # jenga_measure_peaks on this device; "step" carries the same ratio for the whole step (both kernels).
     wm = work_model(cnt, wp.n_bodies, wp.pgs_iters)
-    kernel_s = sum(launch_ms) * 1e-3
-    sm_max = clocks.get("sm_max_mhz") or 1965
-    peak = N_SM * FP32_LANES_PER_SM * sm_max * 1e6 / 1e12
-    achieved = wm["total"] / kernel_s / 1e12
+    solve_s, collide_s = prof["solve_ms"] * 1e-3, prof["collide_ms"] * 1e-3
+    peak = peaks["fp32_instr_per_s"] / 1e12
+    w_solve = wm["pgs_rows"] + wm["integrate"]
+    w_collide = wm["total"] - w_solve
+    achieved = w_solve / solve_s / 1e12
+    n_sub = prof["substeps"]
+    smem_model = (cnt["contact_iters"] * 96.0) / solve_s / 1e12       # 96 B of body traffic per contact-iteration
     traffic = None                                           # ncu dram__bytes per env-step (profiles/) x env-steps per launch
-    tpath = os.path.join(ROOT, "profiles", "k_step_traffic.csv")
+    tpath = os.path.join(ROOT, "profiles", "k_solve_traffic.csv")
     if os.path.exists(tpath):
         import csv
         row = next(csv.DictReader(open(tpath)))
-        traffic = float(row["dram_bytes_per_env_step"]) * cnt["env_steps"] / len(launches)
+        traffic = float(row["dram_bytes_per_env_step"]) * cnt["env_steps"] / max(n_sub, 1)
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinstr/s (FP32 thread-instructions, FMA=1)",
+                "frac": achieved / peak, "traffic": traffic, "kernel": "k_solve", "launch_ms_avg": prof["solve_ms"] / max(n_sub, 1),
+                "launches": n_sub, "share_of_step_time": solve_s / (solve_s + collide_s),
+                "peak_source": f"measured now by jenga_measure_peaks: dependent-free FFMA streams on {peaks['n_sm']} SMs "
+                               f"({peaks['fp32_instr_per_s_3reg'] / 1e12:.2f} T/s with three register operands); "
+                               f"LDS.128 {peaks['smem_bytes_per_s'] / 1e12:.2f} TB/s; nominal 148 x 128 x {clocks.get('sm_max_mhz') or 1965} MHz = "
+                               f"{N_SM * FP32_LANES_PER_SM * (clocks.get('sm_max_mhz') or 1965) * 1e6 / 1e12:.2f} T/s",
+                "smem_model_frac": smem_model / (peaks["smem_bytes_per_s"] / 1e12),
+                "algorithmic_instr_per_env_step": wm["total"] / cnt["env_steps"],
+                "shares": {k: round(v / wm["total"], 4) for k, v in wm.items() if k != "total"},
+                "k_collide": {"achieved": w_collide / collide_s / 1e12, "frac": w_collide / collide_s / 1e12 / peak,
+                              "launch_ms_avg": prof["collide_ms"] / max(n_sub, 1)},
+                "step": {"achieved": wm["total"] / (solve_s + collide_s) / 1e12, "frac": wm["total"] / (solve_s + collide_s) / 1e12 / peak,
+                         "kernel_ms": prof["solve_ms"] + prof["collide_ms"], "wall_ms": sum(launch_ms)}}
     out = {
         "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world_size, "steps": K, "warmup": args.warmup,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "cfg5 (BASELINE.json configs[4]): 18-level 54-block towers, mu_s {0.25,0.40,0.60} round-robin, 0-12 removals, "
                                "Ziglar push sweep, dt=1/240, 20 PGS iters, rollout steps 0..K" if args.cfg == CFG else f"cfg{args.cfg} (manual run, not the bench workload)",
-                   "envs_per_gpu": E, "n_bodies": wp.n_bodies, "pgs_iters": wp.pgs_iters, "steps_per_launch": args.chunk,
+                   "envs_per_gpu": E, "n_bodies": wp.n_bodies, "pgs_iters": wp.pgs_iters, "steps_per_call": args.chunk, "kernels_per_substep": 2,
                    "parallelism": f"env-sharded x{world_size}, no data-path collective",
                    "l2": "inputs larger than L2 (state 191 MB + warm-start cache 1.7 GB per step vs 126 MB L2)"},
         "body_steps_per_s": cnt["body_steps"] * world_size / (ms * 1e-3),
@@ -337,12 +363,8 @@ def run_cuda(args) -> dict:
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke,
                 "split": n_split, "launches": e2e_launches},
-        "gpu_launches": len(launches),
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinstr/s (FP32 thread-instructions, FMA=1)",
-                     "frac": achieved / peak, "traffic": traffic, "kernel": "k_step", "launch_ms_avg": sum(launch_ms) / len(launch_ms),
-                     "peak_source": f"{N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x {sm_max} MHz (nominal issue rate; DESIGN.md §7)",
-                     "algorithmic_instr_per_env_step": wm["total"] / cnt["env_steps"],
-                     "shares": {k: round(v / wm["total"], 4) for k, v in wm.items() if k != "total"}},
+        "gpu_launches": 2 * n_sub,
+        "roofline": roofline,
     }
     if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline()

@@ -179,6 +179,13 @@ size_t jenga_scratch_bytes(const jenga_world_desc *desc);
 
 const char *jenga_strerror(int code);
 
+/* Measurement aid (bench.py's roofline): while enabled, every launch of jenga_step / jenga_simulate_until_rest is
+ * bracketed by CUDA events on the caller's stream.  jenga_profile_read synchronises on them and returns, for the launches
+ * since the last enable / read, out[0] = summed device time of the detection + setup kernel [ms], out[1] = of the
+ * solve + integrate kernel [ms], out[2] = out[3] = number of substeps.  `out` is a HOST array of 4 doubles.     */
+int jenga_profile_enable(jenga_world *w, int on);
+int jenga_profile_read(jenga_world *w, double *out);
+
 /* Measured roofline denominators of this device: two micro-benchmarks on all SMs,
  * out[0] = FP32 thread-instructions per second (dependent-free FFMA streams, FMA = 1 instruction),
  * out[1] = shared-memory bytes per second (conflict-free LDS.128 streams), out[2] = SM count,

@@ -69,6 +69,8 @@ def lib():
         L.jenga_smem_bytes.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_smem_bytes.restype = C.c_size_t
         L.jenga_block_threads.argtypes = [C.POINTER(WorldDesc)]
+        L.jenga_profile_enable.argtypes = [C.c_void_p, C.c_int]
+        L.jenga_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.jenga_scratch_bytes.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_scratch_bytes.restype = C.c_size_t
         L.jenga_strerror.argtypes = [C.c_int]
@@ -77,7 +79,8 @@ def lib():
         L.jenga_peaks_scratch_bytes.restype = C.c_size_t
         L.jenga_strerror.restype = C.c_char_p
         for f in ("jenga_world_create", "jenga_world_destroy", "jenga_broadphase", "jenga_narrowphase", "jenga_pgs_solve",
-                  "jenga_step", "jenga_step_host", "jenga_simulate_until_rest", "jenga_set_f_ext", "jenga_block_threads"):
+                  "jenga_step", "jenga_step_host", "jenga_simulate_until_rest", "jenga_set_f_ext", "jenga_block_threads",
+                  "jenga_profile_enable", "jenga_profile_read"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -216,6 +219,14 @@ class World:
             self.f_ext = torch.as_tensor(f_ext, dtype=torch.float32).contiguous().to(self.dev)
             assert self.f_ext.shape == (self.wp.n_envs, 6, self.wp.body_stride)
             _check(lib().jenga_set_f_ext(self.handle, C.c_void_p(self.f_ext.data_ptr())), "jenga_set_f_ext")
+
+    def jenga_profile_enable(self, on: bool = True):
+        _check(lib().jenga_profile_enable(self.handle, int(on)), "jenga_profile_enable")
+
+    def jenga_profile_read(self) -> dict:
+        out = (C.c_double * 4)()
+        _check(lib().jenga_profile_read(self.handle, out), "jenga_profile_read")
+        return dict(collide_ms=out[0], solve_ms=out[1], substeps=int(out[2]))
 
     def jenga_world_destroy(self):
         if self.handle:

@@ -7,9 +7,11 @@
 #include <cuda_runtime.h>
 #include <stdio.h>
 #include <stdlib.h>
+#include <new>
 #include <string.h>
 
 #include <mutex>
+#include <vector>
 
 #include "ksolve.cuh"
 
@@ -37,8 +39,11 @@ struct jenga_world {
   Params P;
   int tmb;                 // TMEM blocks per env of k_solve: 5, 10 or 0 (no TMEM, 1 warp per CTA)
   int wpc_collide;         // warps (= envs) per CTA of k_collide
+  int n_sm;
   size_t smem_solve;       // dynamic shared memory per CTA of k_solve
   size_t smem_collide;     // ... of k_collide
+  bool profiling;          // jenga_profile_enable: events around every launch of the step
+  std::vector<cudaEvent_t> ev;   // e0 k_collide e1 k_solve e2, per substep
 };
 
 static thread_local char g_err[512] = "no error";
@@ -164,14 +169,15 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   e = cudaGetDeviceProperties(&prop, d->device);
   if (e != cudaSuccess) return cuda_fail(e, "cudaGetDeviceProperties");
   if (prop.major != 10) return JENGA_E_DEVICE;
-  jenga_world* w = (jenga_world*)calloc(1, sizeof(jenga_world));
+  jenga_world* w = new (std::nothrow) jenga_world();
   if (!w) return JENGA_E_ARG;
-  w->desc = *d; w->bufs = *b; w->tmb = tmb;
+  w->profiling = false;
+  w->desc = *d; w->bufs = *b; w->tmb = tmb; w->n_sm = prop.multiProcessorCount;
   w->smem_solve = solve_cta_bytes(d, tmb);
   const size_t cb = collide_env_bytes(d);
   w->wpc_collide = 4 * cb <= kSmemMax ? 4 : (2 * cb <= kSmemMax ? 2 : 1);
   w->smem_collide = w->wpc_collide * cb;
-  if (w->smem_solve > (size_t)prop.sharedMemPerBlockOptin || w->smem_collide > (size_t)prop.sharedMemPerBlockOptin) { free(w); return JENGA_E_ARG; }
+  if (w->smem_solve > (size_t)prop.sharedMemPerBlockOptin || w->smem_collide > (size_t)prop.sharedMemPerBlockOptin) { delete w; return JENGA_E_ARG; }
   Params& P = w->P;
   P.E = d->n_envs; P.B = d->n_bodies; P.S = d->body_stride;
   P.h = d->dt / (float)d->n_substeps; P.n_substeps = d->n_substeps; P.iters = d->pgs_iters;
@@ -200,10 +206,47 @@ static int launched(const char* name) {
   return e == cudaSuccess ? JENGA_OK : cuda_fail(e, name);
 }
 
+static void drop_events(jenga_world* w) {
+  for (cudaEvent_t e : w->ev) cudaEventDestroy(e);
+  w->ev.clear();
+}
+
 extern "C" int jenga_world_destroy(jenga_world* w) {
   if (!w) return JENGA_E_ARG;
-  free(w);
+  drop_events(w);
+  delete w;
   return JENGA_OK;
+}
+
+extern "C" int jenga_profile_enable(jenga_world* w, int on) {
+  if (!w) return JENGA_E_ARG;
+  drop_events(w);
+  w->profiling = on != 0;
+  return JENGA_OK;
+}
+
+extern "C" int jenga_profile_read(jenga_world* w, double* out) {
+  if (!w || !out) return JENGA_E_ARG;
+  double ms_c = 0.0, ms_s = 0.0; size_t n = w->ev.size() / 3;
+  for (size_t i = 0; i < n; ++i) {
+    cudaError_t e = cudaEventSynchronize(w->ev[3 * i + 2]);
+    if (e != cudaSuccess) return cuda_fail(e, "jenga_profile_read");
+    float a = 0.0f, b = 0.0f;
+    cudaEventElapsedTime(&a, w->ev[3 * i], w->ev[3 * i + 1]);
+    cudaEventElapsedTime(&b, w->ev[3 * i + 1], w->ev[3 * i + 2]);
+    ms_c += a; ms_s += b;
+  }
+  out[0] = ms_c; out[1] = ms_s; out[2] = (double)n; out[3] = (double)n;
+  drop_events(w);
+  return JENGA_OK;
+}
+
+static void mark(jenga_world* w, cudaStream_t st) {
+  if (!w->profiling) return;
+  cudaEvent_t e;
+  if (cudaEventCreate(&e) != cudaSuccess) return;
+  cudaEventRecord(e, st);
+  w->ev.push_back(e);
 }
 
 extern "C" int jenga_set_f_ext(jenga_world* w, const float* f_ext) {
@@ -223,8 +266,15 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
 static int launch_solve(jenga_world* w, int iters, int flags, float rest_ek, cudaStream_t st) {
   const cudaError_t e = ensure_smem(w->desc.device, w->tmb ? KnSolveTm : KnSolveSm, w->smem_solve);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_solve)");
-  if (w->tmb) jenga::k_solve<true><<<(w->P.E + 3) / 4, 128, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
-  else jenga::k_solve<false><<<w->P.E, 32, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
+  /* persistent CTAs: as many as are resident at once (2 x 4-env CTAs per SM in the 256-column tier), each warp strides
+   * over the envs */
+  if (w->tmb) {
+    const int resident = w->n_sm * (w->tmb > 5 ? 1 : 2), need = (w->P.E + 3) / 4;
+    jenga::k_solve<true><<<need < resident ? need : resident, 128, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
+  } else {
+    const int per_sm = (int)(kSmemMax / (w->smem_solve + 1024)), resident = w->n_sm * (per_sm < 1 ? 1 : (per_sm > 16 ? 16 : per_sm));
+    jenga::k_solve<false><<<w->P.E < resident ? w->P.E : resident, 32, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
+  }
   return launched("k_solve");
 }
 
@@ -249,11 +299,14 @@ static int step_launches(jenga_world* w, int n_steps, int rest, float rest_ek, c
   const int n_sub = w->P.n_substeps;
   for (int s = 0; s < n_steps; ++s)
     for (int sub = 0; sub < n_sub; ++sub) {
+      mark(w, st);
       int rc = launch_collide(w, jenga::ModeStep, rest, st);
       if (rc != JENGA_OK) return rc;
+      mark(w, st);
       const int flags = (sub == n_sub - 1 ? jenga::SolveEndOfStep : 0) | (rest ? jenga::SolveRest : 0);
       rc = launch_solve(w, w->P.iters, flags, rest_ek, st);
       if (rc != JENGA_OK) return rc;
+      mark(w, st);
     }
   return JENGA_OK;
 }

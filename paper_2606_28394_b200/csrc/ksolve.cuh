@@ -225,73 +225,116 @@ __device__ __forceinline__ void apply_impulse(Body5& A, Body5& B, Vec3 rA, Vec3 
   B.w.z = fmaf(B.i1.y, cB.z, fmaf(B.i1.x, cB.y, fmaf(B.i0.z, cB.x, B.w.z)));
 }
 
-// One chunk visit of the warm-start application (S4) or of a Gauss-Seidel sweep (S5).  The chunk's pairs are lanes
-// [lane0, lane0 + count) of block j; slots ascending; per contact the normal row (Eq. 14, clamp >= 0), then t1, then
-// t2 (Eq. 15, each clipped to +-mu_s jn) -- Listing 1.  The three rows of a contact act on the same
-// two bodies: the relative velocity of the contact point is read once, advanced between rows with the contact-space
-// couplings K_ij (exactly the change the applied impulse causes), and the summed impulse is applied once (DESIGN §3
-// R-couple).  Pairs of one colour share no dynamic body.  TMEM stores are warp-wide: the lanes outside the chunk
-// write back the impulses they loaded.
-template <bool TM, bool WARM>
-__device__ __forceinline__ void solve_chunk(const SSm& s, int d, float mu) {
-  const int lane = lane_id();
-  const int j = d >> 16, lane0 = d & 0xff, count = (d >> 8) & 0xff;
-  const bool active = lane >= lane0 && lane < lane0 + count;
-  const bool in_tm = TM && j < s.tmb;
-  const int k = 32 * j + lane;
-  PairC c;
-  if (in_tm) { tm_load_block(s, j, c); tm_wait_ld(); }
-  else if (active) sm_load_pair(s, j, lane, c);
-  if (active) {
-    const float4 h = hdr4(s, 0, k), nn = hdr4(s, 1, k), tt = hdr4(s, 2, k);
-    const int ab = __float_as_int(h.x), a = (ab & 0xffff) - 1, b = ab >> 16, np = __float_as_int(h.y) & 0xff;
-    Body5 A, B; load_body(s, a, A); load_body(s, b, B);
-    Frame F; F.n = xyz(nn); F.t1 = xyz(tt); F.t2 = cross(F.n, F.t1);
+// The contact arithmetic of one pair (both passes).  Slots ascending; per contact the normal row (Eq. 14, clamp >= 0),
+// then t1, then t2 (Eq. 15, each clipped to +-mu_s jn) -- Listing 1.  The three rows of a contact
+// act on the same two bodies: the relative velocity of the contact point is read once, advanced between rows with the
+// contact-space couplings K_ij (exactly the change the applied impulse causes), and the summed impulse is applied
+// once (DESIGN §3 R-couple).  All four slots run unconditionally: an unused slot has zero constants and impulses, so its
+// rows return 0 and it applies +-0 (bit-identical to skipping it, and no divergent branch per contact).
+template <bool WARM>
+__device__ __forceinline__ void solve_pair(PairC& c, Body5& A, Body5& B, const Frame& F, float mu) {
 #pragma unroll
-    for (int ci = 0; ci < 4; ++ci)
-      if (ci < np) {
-        const float* r = c.v + 9 * ci; float* l = c.v + kLam + 3 * ci;
-        const Vec3 p = v3(r[0], r[1], r[2]), rA = p - xyz(A.x), rB = p - xyz(B.x);
-        Vec3 Pi;
-        if (WARM) {
-          Pi = madd(madd(l[0] * F.n, l[1], F.t1), l[2], F.t2);
-        } else {
-          // vr = (vB + wB x rB) - (vA + wA x rA), each component one subtraction and four fused multiply-adds
-          const Vec3 vr = v3(
-            fmaf(A.w.z, rA.y, fmaf(-A.w.y, rA.z, fmaf(-B.w.z, rB.y, fmaf(B.w.y, rB.z, B.v.x - A.v.x)))),
-            fmaf(A.w.x, rA.z, fmaf(-A.w.z, rA.x, fmaf(-B.w.x, rB.z, fmaf(B.w.z, rB.x, B.v.y - A.v.y)))),
-            fmaf(A.w.y, rA.x, fmaf(-A.w.x, rA.y, fmaf(-B.w.y, rB.x, fmaf(B.w.x, rB.y, B.v.z - A.v.z)))));
-          const float u0 = dot(vr, F.n);
-          float u1 = dot(vr, F.t1), u2 = dot(vr, F.t2);
-          const float nw = fmaxf(fmaf(-u0, r[3], l[0]), 0.0f);
-          const float d0 = nw - l[0];
-          u1 = fmaf(r[6], d0, u1); u2 = fmaf(r[7], d0, u2);
-          const float lim = mu * nw;
-          const float n1 = fminf(fmaxf(fmaf(-u1, r[4], l[1]), -lim), lim);
-          const float d1 = n1 - l[1];
-          u2 = fmaf(r[8], d1, u2);
-          const float n2 = fminf(fmaxf(fmaf(-u2, r[5], l[2]), -lim), lim);
-          const float d2 = n2 - l[2];
-          l[0] = nw; l[1] = n1; l[2] = n2;
-          Pi = madd(madd(d0 * F.n, d1, F.t1), d2, F.t2);
-        }
-        apply_impulse(A, B, rA, rB, Pi);
-      }
-    if (a >= 0) { bd4(s, a, 1) = A.v; bd4(s, a, 2) = A.w; }
-    bd4(s, b, 1) = B.v; bd4(s, b, 2) = B.w;
-    if (!WARM && !in_tm) sm_store_lam(s, j, lane, c.v + kLam);
+  for (int ci = 0; ci < 4; ++ci) {
+    const float* r = c.v + 9 * ci; float* l = c.v + kLam + 3 * ci;
+    const Vec3 p = v3(r[0], r[1], r[2]), rA = p - xyz(A.x), rB = p - xyz(B.x);
+    Vec3 Pi;
+    if (WARM) {
+      Pi = madd(madd(l[0] * F.n, l[1], F.t1), l[2], F.t2);
+    } else {
+      // vr = (vB + wB x rB) - (vA + wA x rA), each component one subtraction and four fused multiply-adds
+      const Vec3 vr = v3(
+        fmaf(A.w.z, rA.y, fmaf(-A.w.y, rA.z, fmaf(-B.w.z, rB.y, fmaf(B.w.y, rB.z, B.v.x - A.v.x)))),
+        fmaf(A.w.x, rA.z, fmaf(-A.w.z, rA.x, fmaf(-B.w.x, rB.z, fmaf(B.w.z, rB.x, B.v.y - A.v.y)))),
+        fmaf(A.w.y, rA.x, fmaf(-A.w.x, rA.y, fmaf(-B.w.y, rB.x, fmaf(B.w.x, rB.y, B.v.z - A.v.z)))));
+      const float u0 = dot(vr, F.n);
+      float u1 = dot(vr, F.t1), u2 = dot(vr, F.t2);
+      const float nw = fmaxf(fmaf(-u0, r[3], l[0]), 0.0f);
+      const float d0 = nw - l[0];
+      u1 = fmaf(r[6], d0, u1); u2 = fmaf(r[7], d0, u2);
+      const float lim = mu * nw;
+      const float n1 = fminf(fmaxf(fmaf(-u1, r[4], l[1]), -lim), lim);
+      const float d1 = n1 - l[1];
+      u2 = fmaf(r[8], d1, u2);
+      const float n2 = fminf(fmaxf(fmaf(-u2, r[5], l[2]), -lim), lim);
+      const float d2 = n2 - l[2];
+      l[0] = nw; l[1] = n1; l[2] = n2;
+      Pi = madd(madd(d0 * F.n, d1, F.t1), d2, F.t2);
+    }
+    apply_impulse(A, B, rA, rB, Pi);
   }
-  if (!WARM && in_tm) { tm_store_lam(s, j, c.v + kLam); tm_wait_st(); }
-  __syncwarp();
 }
 
-// S4 (warm-start application) + S5: the chunks in canonical order, `iters` sweeps.
+// What a lane needs of its pair's header during a visit.
+struct Hdr { int a, b; Vec3 n, t1; };
+__device__ __forceinline__ Hdr load_hdr(const SSm& s, int k) {
+  const float4 h = hdr4(s, 0, k), nn = hdr4(s, 1, k), tt = hdr4(s, 2, k);
+  Hdr H; const int ab = __float_as_int(h.x);
+  H.a = (ab & 0xffff) - 1; H.b = ab >> 16; H.n = xyz(nn); H.t1 = xyz(tt);
+  return H;
+}
+__device__ __forceinline__ bool chunk_lane(int d, int lane) { const int l0 = d & 0xff; return lane >= l0 && lane < l0 + ((d >> 8) & 0xff); }
+
+// S4: the cached impulses are applied once, chunk by chunk in canonical order (no impulse changes: nothing is stored).
 template <bool TM>
-__device__ inline void pgs_sweeps(const SSm& s, const Params& P, int nph, int iters, float mu) {
-  if (P.warm_start)
-    for (int j = 0; j < nph; ++j) solve_chunk<TM, true>(s, s.ph[j], mu);
-  for (int it = 0; it < iters; ++it)
-    for (int j = 0; j < nph; ++j) solve_chunk<TM, false>(s, s.ph[j], mu);
+__device__ inline void warm_start_pass(const SSm& s, int nph) {
+  const int lane = lane_id();
+  for (int j = 0; j < nph; ++j) {
+    const int d = s.ph[j], jb = d >> 16;
+    PairC c; block_load<TM>(s, jb, c);
+    if (chunk_lane(d, lane)) {
+      const Hdr H = load_hdr(s, 32 * jb + lane);
+      Body5 A, B; load_body(s, H.a, A); load_body(s, H.b, B);
+      Frame F; F.n = H.n; F.t1 = H.t1; F.t2 = cross(F.n, F.t1);
+      solve_pair<true>(c, A, B, F, 0.0f);
+      if (H.a >= 0) { bd4(s, H.a, 1) = A.v; bd4(s, H.a, 2) = A.w; }
+      bd4(s, H.b, 1) = B.v; bd4(s, H.b, 2) = B.w;
+    }
+    __syncwarp();
+  }
+}
+
+// S5: `iters` Gauss-Seidel sweeps over the chunks in canonical order, as ONE software-pipelined loop over the
+// iters * nph chunk visits.  A visit: the chunk's pairs are lanes [lane0, lane0 + count) of block jb; pairs of one
+// colour share no dynamic body.  While the contacts of visit v run, the header of visit v + 1 is fetched from shared
+// memory, and as soon as the impulses of v are stored the constants of v + 1 are requested from tensor memory, so that
+// the next visit starts with the (dependent) body loads at once.  TMEM accesses are warp-wide: the lanes outside the
+// chunk write back the impulses they loaded.
+template <bool TM>
+__device__ inline void pgs_sweeps(const SSm& s, int nph, int iters, float mu) {
+  const int total = nph * iters, lane = lane_id();
+  if (total <= 0) return;
+  int d = s.ph[0], jn = 0;
+  PairC c;
+  Hdr H; H.a = -1; H.b = 0; H.n = H.t1 = v3(0, 0, 0);
+  if (chunk_lane(d, lane)) H = load_hdr(s, 32 * (d >> 16) + lane);
+  if (TM && (d >> 16) < s.tmb) tm_load_block(s, d >> 16, c);
+  else sm_load_pair(s, d >> 16, lane, c);
+#pragma unroll 1
+  for (int v = 0; v < total; ++v) {
+    const int jb = d >> 16;
+    const bool active = chunk_lane(d, lane), in_tm = TM && jb < s.tmb;
+    jn = jn + 1 == nph ? 0 : jn + 1;
+    const int dn = s.ph[jn];
+    Hdr Hn; Hn.a = -1; Hn.b = 0; Hn.n = Hn.t1 = v3(0, 0, 0);
+    if (in_tm) tm_wait_ld();
+    if (active) {
+      Body5 A, B; load_body(s, H.a, A); load_body(s, H.b, B);
+      if (chunk_lane(dn, lane)) Hn = load_hdr(s, 32 * (dn >> 16) + lane);
+      Frame F; F.n = H.n; F.t1 = H.t1; F.t2 = cross(F.n, F.t1);
+      solve_pair<false>(c, A, B, F, mu);
+      if (H.a >= 0) { bd4(s, H.a, 1) = A.v; bd4(s, H.a, 2) = A.w; }
+      bd4(s, H.b, 1) = B.v; bd4(s, H.b, 2) = B.w;
+      if (!in_tm) sm_store_lam(s, jb, lane, c.v + kLam);
+    } else if (chunk_lane(dn, lane)) {
+      Hn = load_hdr(s, 32 * (dn >> 16) + lane);
+    }
+    if (in_tm) { tm_store_lam(s, jb, c.v + kLam); tm_wait_st(); }
+    __syncwarp();
+    if (TM && (dn >> 16) < s.tmb) tm_load_block(s, dn >> 16, c);
+    else sm_load_pair(s, dn >> 16, lane, c);
+    d = dn; H = Hn;
+  }
+  if (TM) tm_wait_ld();
 }
 
 // S6: x += h v (Eq. 6); q <- normalise(q + h/2 [0,w] (x) q) (Eq. 2, world-frame
@@ -432,18 +475,22 @@ enum { SolveEndOfStep = 1, SolvePgsOnly = 2, SolveRest = 4 };
 
 template <bool TM>
 __global__ void __launch_bounds__(TM ? 128 : 32, TM ? 2 : 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
-  int env;
-  const SSm s = begin_solve<TM>(P, env);
+  int env0;
+  const SSm s = begin_solve<TM>(P, env0);
   const int lane = lane_id();
   const Scratch L = scratch_layout(P.pc);
-  float* scr = P.scratch + (size_t)(env < P.E ? env : 0) * P.scratch_words;
-  int* meta = reinterpret_cast<int*>(scr + L.meta);
-  const bool valid = env < P.E && !((flags & SolveRest) && meta[MetaResting]);
-  if (valid) {
+  const int stride = gridDim.x * (TM ? 4 : 1);
+  // persistent: warp w of CTA c takes envs c * wpc + w, + stride, ... (TMEM is allocated once per CTA; the warps of a CTA
+  // never wait for one another between envs)
+  for (int env = env0; env < P.E; env += stride) {
+    float* scr = P.scratch + (size_t)env * P.scratch_words;
+    int* meta = reinterpret_cast<int*>(scr + L.meta);
+    if ((flags & SolveRest) && meta[MetaResting]) continue;
     unsigned st = 0;
     load_bodies(s, P, env);
     const int nph = load_slots<TM>(s, P, scr, L);
-    pgs_sweeps<TM>(s, P, nph, iters, P.mu[env]);
+    if (P.warm_start) warm_start_pass<TM>(s, nph);
+    pgs_sweeps<TM>(s, nph, iters, P.mu[env]);
     if (flags & SolvePgsOnly) {
       store_cache<TM>(s, P, env, scr, L, nph, false, true);      // lambda in contact order only
       store_bodies(s, P, env);
@@ -479,6 +526,7 @@ __global__ void __launch_bounds__(TM ? 128 : 32, TM ? 2 : 1) k_solve(const Param
       }
     }
     flush_status(P, env, st);
+    __syncwarp();
   }
   end_solve<TM>(s);
 }
