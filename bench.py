@@ -210,7 +210,7 @@ def run_cuda(args) -> dict:
     if args.max_pairs:
         wp.max_pairs = args.max_pairs
     K = min(args.steps, wl.n_steps)
-    world = binding.World(wp, wl.state, wl.props, wl.mu, device=local)
+    world = binding.World(wp, wl.state, wl.props, wl.mu, device=local, tier=args.tier)
     state0 = world.state.clone()
     fext_dev = torch.as_tensor(wl.push_fext).to(dev)
     fext_ptr = binding.C.c_void_p(fext_dev.data_ptr())
@@ -272,7 +272,7 @@ def run_cuda(args) -> dict:
     parts = []
     for lo, hi in bounds:
         wpi = W.WorldParams(**{**wp.__dict__, "n_envs": hi - lo})
-        wi = binding.World(wpi, wl.state[lo:hi], wl.props[lo:hi], wl.mu[lo:hi], device=local)
+        wi = binding.World(wpi, wl.state[lo:hi], wl.props[lo:hi], wl.mu[lo:hi], device=local, tier=args.tier)
         h_a = torch.empty(wi.state.shape, dtype=torch.float32, pin_memory=True)
         h_b = torch.empty_like(h_a, pin_memory=True)
         h_a.copy_(torch.as_tensor(wl.state[lo:hi]))
@@ -385,6 +385,7 @@ def main():
     ap.add_argument("--e2e-split", type=int, default=2, help="worlds (streams) the e2e leg serves the batch with")
     ap.add_argument("--cfg", type=int, default=CFG, help="BASELINE.json config number (5 = the bench workload; others: manual runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tier", default="auto", choices=["auto", "smem", "tmem256", "tmem512"], help="where k_solve keeps the contact constants")
     ap.add_argument("--max-contacts", type=int, default=0, help="override the workload's contact capacity per env")
     ap.add_argument("--max-pairs", type=int, default=0, help="override the workload's candidate capacity per env")
     args = ap.parse_args()

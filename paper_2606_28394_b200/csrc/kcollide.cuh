@@ -13,6 +13,7 @@ struct CSm {
   SP<unsigned long long> used;  // [S]      colour masks per body
   SP<unsigned> cab;             // [pcA]    (a+1) | A dynamic << 11 | axis << 12 | b << 16 | B dynamic << 27
   SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending
+  SP<float> poly;               // [8][3][32] clip polygon of every lane (component-major: lane l <-> bank l)
   SP<unsigned short> cpair;     // [pcA]    colliding pair indices, ascending
   SP<unsigned short> cprev;     // [pcA]    pair indices of the warm-start cache (previous substep), ascending
   SP<unsigned short> pos;       // [pcA]    position of pair r
@@ -31,7 +32,7 @@ __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int p
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc);
   size_t w = (size_t)kCb * S + 3 * S + 2 * S;            // cb, ext, used
   w += pcA;                                              // cab
-  w += mpA / 2;                                          // cand
+  w += mpA / 2 + 768;                                    // cand, poly
   w += 4 * (size_t)(pcA / 2);                            // cpair, cprev, pos, wrank
   w += pcA / 4;                                          // colour
   w += 2 * round_up(ph_max(nblk), 4);                    // ph, chc
@@ -48,6 +49,7 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base) {
   s.used.off = p;   p += 2 * S;
   s.cab.off = p;    p += pcA;
   s.cand.off = p;   p += mpA / 2;
+  s.poly.off = p;   p += 768;
   s.cpair.off = p;  p += pcA / 2;
   s.cprev.off = p;  p += pcA / 2;
   s.pos.off = p;    p += pcA / 2;
@@ -62,6 +64,8 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base) {
   return s;
 }
 
+__device__ __forceinline__ Vec3 xyz(float4 v) { return v3(v.x, v.y, v.z); }
+__device__ __forceinline__ Vec3 xyz4(float4 v) { return v3(v.x, v.y, v.z); }
 __device__ __forceinline__ float4& cb4(const CSm& s, int b, int k) { return reinterpret_cast<float4*>(smem_f + s.cb.off + b * kCb)[k]; }
 
 __device__ __forceinline__ Box load_box(const CSm& s, int b) {
@@ -225,13 +229,218 @@ __device__ __forceinline__ int ab_a(unsigned w) { return (int)(w & 0x7ffu) - 1; 
 __device__ __forceinline__ int ab_b(unsigned w) { return (int)((w >> 16) & 0x7ffu); }
 __device__ __forceinline__ int ab_axis(unsigned w) { return (int)((w >> 12) & 0xfu); }
 
+// ---------------------------------------------------------------- box-box manifold on the shared records
+// The box records are read by dynamic index (axis k of body b = float4 1 + k of its record: axis.xyz, half extent), so
+// the axis choices of the reference / incident faces are address arithmetic, not select chains; the clip polygon of
+// a lane lives in the warp's shared-memory buffer s.poly (8 vertices x 3 floats per lane, component-major so that lane l
+// always hits bank l): no thread-local memory anywhere in the narrowphase.
+__device__ __forceinline__ float4 rec4(int off, int k) { return reinterpret_cast<const float4*>(smem_f + off)[k]; }
+__device__ __forceinline__ Vec3 poly_get(int pb, int k) { return v3(smem_f[pb + (3 * k) * 32], smem_f[pb + (3 * k + 1) * 32], smem_f[pb + (3 * k + 2) * 32]); }
+__device__ __forceinline__ void poly_put(int pb, int k, Vec3 p) { smem_f[pb + (3 * k) * 32] = p.x; smem_f[pb + (3 * k + 1) * 32] = p.y; smem_f[pb + (3 * k + 2) * 32] = p.z; }
+
+// Normal and overlap of ONE axis of a pair that sat_boxes found overlapping with this axis chosen: the same
+// expressions as in sat_boxes (same fused multiply-adds), so the values are identical bit for bit.
+__device__ __forceinline__ void sat_axis(int oA, int oB, int axis, SatResult& r) {
+  const float4 xa = rec4(oA, 0), xb = rec4(oB, 0);
+  const Vec3 t = xyz4(xb) - xyz4(xa);
+  const float4 a0 = rec4(oA, 1), a1 = rec4(oA, 2), a2 = rec4(oA, 3), b0 = rec4(oB, 1), b1 = rec4(oB, 2), b2 = rec4(oB, 3);
+  const float heA[3] = { a0.w, a1.w, a2.w }, heB[3] = { b0.w, b1.w, b2.w };
+  Vec3 n; float delta;
+  if (axis < 3) {
+    const float4 q = rec4(oA, 1 + axis);
+    n = xyz4(q);
+    const float rB = absdot3(heB, dot(n, xyz4(b0)), dot(n, xyz4(b1)), dot(n, xyz4(b2)));
+    delta = q.w + rB - fabsf(dot(t, n));
+  } else if (axis < 6) {
+    const float4 q = rec4(oB, axis - 2);
+    n = xyz4(q);
+    const float rA = absdot3(heA, dot(xyz4(a0), n), dot(xyz4(a1), n), dot(xyz4(a2), n));
+    delta = rA + q.w - fabsf(dot(t, n));
+  } else {
+    const int i = (axis - 6) / 3, j = (axis - 6) - 3 * i;
+    Vec3 u = cross(xyz4(rec4(oA, 1 + i)), xyz4(rec4(oB, 1 + j)));
+    const float inv = 1.0f / sqrtf(dot(u, u));
+    u = inv * u;
+    const float rA = absdot3(heA, dot(xyz4(a0), u), dot(xyz4(a1), u), dot(xyz4(a2), u));
+    const float rB = absdot3(heB, dot(xyz4(b0), u), dot(xyz4(b1), u), dot(xyz4(b2), u));
+    delta = rA + rB - fabsf(dot(t, u));
+    n = u;
+  }
+  if (dot(n, t) < 0.0f) n = -n;
+  r.axis = axis; r.n = n; r.delta = delta;
+}
+
+// Sutherland-Hodgman against the half-space  sgn * ((P - c) . axis) <= e, IN PLACE in the lane's polygon
+// buffer.  Safe: iteration i has read vertices i + 1 and i + 2 before it writes, and it writes at most index i + 2
+// (a convex polygon gains at most one vertex per plane).  At most 8 vertices are kept.
+__device__ inline int clip_halfspace(int pb, int nin, Vec3 c, Vec3 axis, float sgn, float e) {
+  int nout = 0;
+  const Vec3 first = poly_get(pb, 0);
+  Vec3 P = first, Q = nin > 1 ? poly_get(pb, 1) : first;
+  float dP = e - sgn * dot(P - c, axis);
+  for (int i = 0; i < nin; ++i) {
+    const Vec3 R = i + 2 < nin ? poly_get(pb, i + 2) : first;      // the vertex after Q (wraps to vertex 0)
+    const float dQ = e - sgn * dot(Q - c, axis);
+    if (dP >= 0.0f) {
+      if (nout < 8) poly_put(pb, nout++, P);
+      if (dQ < 0.0f && nout < 8) { const float t = dP / (dP - dQ); poly_put(pb, nout++, madd(P, t, Q - P)); }
+    } else if (dQ >= 0.0f && nout < 8) {
+      const float t = dP / (dP - dQ); poly_put(pb, nout++, madd(P, t, Q - P));
+    }
+    P = Q; dP = dQ; Q = R;
+  }
+  return nout;
+}
+
+// Contact manifold for an overlapping pair (PAPER.md:273-280 read as A8): edge case = closest points of the two
+// support edges; face case = incident face clipped against the side planes of the reference face, points below the
+// reference face kept with their depth, <= 4 reduction (DESIGN §2 S3).
+__device__ inline void manifold_boxes(int oA, int oB, const SatResult& sr, int pb, Manifold& m) {
+  const int ax = sr.axis; const Vec3 n = sr.n; const float delta = sr.delta;
+  m.axis = ax; m.n = n; m.np = 0;
+  const Vec3 Ac = xyz4(rec4(oA, 0)), Bc = xyz4(rec4(oB, 0));
+
+  if (ax >= 6) {                            // edge-edge
+    const int i = (ax - 6) / 3, j = (ax - 6) - 3 * i;
+    Vec3 pa = Ac, pb_ = Bc;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const float4 qa = rec4(oA, 1 + k), qb = rec4(oB, 1 + k);
+      const float sa = dot(xyz4(qa), n) >= 0.0f ? 1.0f : -1.0f, sb = dot(xyz4(qb), n) >= 0.0f ? 1.0f : -1.0f;
+      const Vec3 ma = madd(pa, sa * qa.w, xyz4(qa)), mb = madd(pb_, -sb * qb.w, xyz4(qb));
+      if (k != i) pa = ma;
+      if (k != j) pb_ = mb;
+    }
+    const float4 qi = rec4(oA, 1 + i), qj = rec4(oB, 1 + j);
+    const Vec3 ai = xyz4(qi), bj = xyz4(qj), r = pa - pb_;
+    const float hi = qi.w, hj = qj.w;
+    const float bb = dot(ai, bj), cc = dot(ai, r), ff = dot(bj, r), den = 1.0f - bb * bb;
+    float sA = (bb * ff - cc) / den, sB = (ff - bb * cc) / den;
+    sA = fminf(fmaxf(sA, -hi), hi);
+    sB = fminf(fmaxf(sB, -hj), hj);
+    m.p[0] = 0.5f * (madd(pa, sA, ai) + madd(pb_, sB, bj));
+    m.d[0] = delta; m.np = 1;
+    return;
+  }
+
+  // face case: X owns the axis (reference), Y is the other (incident)
+  const bool refA = ax < 3; const int r = refA ? ax : ax - 3;
+  const int oX = refA ? oA : oB, oY = refA ? oB : oA;
+  const Vec3 Xc = refA ? Ac : Bc, Yc = refA ? Bc : Ac;
+  const Vec3 nref = refA ? n : -n;
+  int mi = 0; float sg = -1.0f, best = 3.0e38f;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const float dk = dot(xyz4(rec4(oY, 1 + k)), nref);
+    if (-dk < best) { best = -dk; mi = k; sg = -1.0f; }
+    if (dk < best) { best = dk; mi = k; sg = 1.0f; }
+  }
+  const int iu = (mi == 0) ? 1 : 0, iv = (mi == 2) ? 1 : 2;
+  Vec3 fc, eu, ev;
+  {
+    const float4 qm = rec4(oY, 1 + mi), qu = rec4(oY, 1 + iu), qv = rec4(oY, 1 + iv);
+    fc = madd(Yc, sg * qm.w, xyz4(qm));
+    eu = qu.w * xyz4(qu); ev = qv.w * xyz4(qv);
+    poly_put(pb, 0, fc - eu - ev); poly_put(pb, 1, fc + eu - ev); poly_put(pb, 2, fc + eu + ev); poly_put(pb, 3, fc - eu + ev);
+  }
+  const int u = (r == 0) ? 1 : 0, v = (r == 2) ? 1 : 2;
+  const float4 qxu = rec4(oX, 1 + u), qxv = rec4(oX, 1 + v);
+  const Vec3 xu = xyz4(qxu), xv = xyz4(qxv);
+  const float hu = qxu.w, hv = qxv.w, hr = rec4(oX, 1 + r).w;
+  int np = 4;
+#pragma unroll 1
+  for (int pl = 0; pl < 4 && np; ++pl)        // side planes +u, -u, +v, -v of the reference face (one copy of the clip code)
+    np = clip_halfspace(pb, np, Xc, pl < 2 ? xu : xv, (pl & 1) ? -1.0f : 1.0f, pl < 2 ? hu : hv);
+  // keep the vertices below the reference face (in place: write index <= read index)
+  int nc = 0;
+  for (int k = 0; k < np; ++k) {
+    const Vec3 q = poly_get(pb, k);
+    const float d = hr - dot(q - Xc, nref);
+    if (d >= 0.0f) { poly_put(pb, nc, q); ++nc; }
+  }
+  if (nc == 0) {                            // fallback: deepest incident vertex, SAT depth
+    const Vec3 inc[4] = { fc - eu - ev, fc + eu - ev, fc + eu + ev, fc - eu + ev };
+    Vec3 bp = inc[0]; float bd = -3.0e38f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const float d = hr - dot(inc[k] - Xc, nref);
+      if (d > bd) { bd = d; bp = inc[k]; }
+    }
+    m.p[0] = madd(bp, 0.5f * delta, nref); m.d[0] = delta; m.np = 1;
+    return;
+  }
+  // contact point and depth of kept vertex k: the expressions of the keep test, so the depths are the same bits
+#define CPT(k, P_, D_) { const Vec3 q_ = poly_get(pb, (k)); D_ = hr - dot(q_ - Xc, nref); P_ = madd(q_, 0.5f * D_, nref); }
+  unsigned keep = (1u << nc) - 1u;
+  if (nc > 4) {                             // <= 4 reduction (DESIGN §2 S3)
+    int i0 = 0, i1 = -1, i2 = -1, i3 = -1; float far2 = -1.0f, amax = 0.0f, amin = 0.0f, d0 = 0.0f;
+    Vec3 p0;
+    CPT(0, p0, d0);
+    for (int k = 1; k < nc; ++k) { Vec3 pk; float dk; CPT(k, pk, dk); if (dk > d0) { i0 = k; d0 = dk; p0 = pk; } }
+    Vec3 p1 = p0;
+    for (int k = 0; k < nc; ++k) if (k != i0) {
+      Vec3 pk; float dk; CPT(k, pk, dk);
+      const Vec3 d = pk - p0; const float dd = dot(d, d);
+      if (dd > far2) { far2 = dd; i1 = k; p1 = pk; }
+    }
+    const Vec3 e01 = p1 - p0;
+    for (int k = 0; k < nc; ++k) {
+      if (k == i0 || k == i1) continue;
+      Vec3 pk; float dk; CPT(k, pk, dk);
+      const float area = dot(cross(e01, pk - p0), n);
+      if (area > amax) { amax = area; i2 = k; }
+      if (area < amin) { amin = area; i3 = k; }
+    }
+    keep = (1u << i0) | (1u << i1);
+    if (i2 >= 0) keep |= 1u << i2;
+    if (i3 >= 0) keep |= 1u << i3;
+  }
+  const int no = __popc(keep);              // survivors in ascending clip-output index; static output slots
+#pragma unroll
+  for (int o = 0; o < 4; ++o)
+    if (o < no) { const int k = __fns(keep, 0, o + 1); CPT(k, m.p[o], m.d[o]); }
+#undef CPT
+  m.np = no;
+}
+
+// ---------------------------------------------------------------- ground plane (reading A9)
+// Corners below z = 0 are contacts: n = +z, depth = -z, point at mid-surface (cx, cy, z/2).
+// More than four: drop the shallowest (ties: the higher corner id goes) until four remain; ascending corner id.
+// The corners go through the lane's polygon buffer so that the survivors are fetched by index (no local memory).
+__device__ inline void collide_ground(const Box& b, int pb, Manifold& m) {
+  float cz[8];
+  unsigned ok = 0; int nq = 0;
+#pragma unroll
+  for (int id = 0; id < 8; ++id) {
+    const float sx = (id & 1) ? b.he[0] : -b.he[0], sy = (id & 2) ? b.he[1] : -b.he[1], sz = (id & 4) ? b.he[2] : -b.he[2];
+    const Vec3 o = madd(madd(sx * b.ax[0], sy, b.ax[1]), sz, b.ax[2]);
+    cz[id] = b.c.z + o.z;
+    poly_put(pb, id, v3(b.c.x + o.x, b.c.y + o.y, cz[id]));
+    if (cz[id] < 0.0f) { ok |= 1u << id; ++nq; }
+  }
+  while (nq > 4) {
+    int worst = -1; float wd = 0.0f;
+#pragma unroll
+    for (int id = 0; id < 8; ++id)
+      if ((ok >> id) & 1u) { const float dd = -cz[id]; if (worst < 0 || dd <= wd) { worst = id; wd = dd; } }
+    ok &= ~(1u << worst); --nq;
+  }
+  m.np = nq; m.axis = 15; m.n = v3(0.0f, 0.0f, 1.0f);
+#pragma unroll
+  for (int o = 0; o < 4; ++o)
+    if (o < nq) {
+      const Vec3 c = poly_get(pb, __fns(ok, 0, o + 1));
+      m.p[o] = v3(c.x, c.y, 0.5f * c.z);
+      m.d[o] = -c.z;
+    }
+}
+
 // Manifold of colliding pair (a, b) whose SAT axis is known (find_colliding stored it).
 __device__ __forceinline__ void pair_manifold(const CSm& s, int a, int b, int axis, Manifold& m) {
-  const Box Bj = load_box(s, b);
-  if (a < 0) { collide_ground(Bj, m); return; }
-  const Box Bi = load_box(s, a);
-  SatResult sr; sat_axis(Bi, Bj, axis, sr);
-  manifold_boxes(Bi, Bj, sr, m);
+  if (a < 0) { collide_ground(load_box(s, b), s.poly.off + lane_id(), m); return; }
+  const int oA = s.cb.off + a * kCb, oB = s.cb.off + b * kCb;
+  SatResult sr; sat_axis(oA, oB, axis, sr);
+  manifold_boxes(oA, oB, sr, s.poly.off + lane_id(), m);
 }
 
 // S3, first half: which candidates collide (15-axis SAT / a ground corner below z = 0).  Lane k of a
@@ -383,7 +592,6 @@ __device__ __forceinline__ Vec3 imul(const BodyK& B, Vec3 a) {      // Iw^-1 a
             fmaf(B.i1.x, a.z, fmaf(B.i0.w, a.y, B.i0.y * a.x)),
             fmaf(B.i1.y, a.z, fmaf(B.i1.x, a.y, B.i0.z * a.x)));
 }
-__device__ __forceinline__ Vec3 xyz(float4 v) { return v3(v.x, v.y, v.z); }
 
 // S4 for one colliding pair: header and constants of position k from the pair's manifold, written to the scratch.
 // Warm start (DESIGN §3 R-warm): a new contact inherits (jn,jt1,jt2) of the nearest not yet taken previous contact
@@ -542,11 +750,13 @@ __device__ inline int write_contacts(const CSm& s, const Params& P, int env, flo
       int lo = 0, hi = n_cand;                                   // position of the pair in the candidate list
       while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)s.cand[mid] < idx) lo = mid + 1; else hi = mid; }
       float4* out = reinterpret_cast<float4*>(P.contacts + ((size_t)env * P.max_contacts + off) * 8);
-      for (int c = 0; c < m.np; ++c) {
-        const int tag = (lo & 0xffff) | (c << 16) | (m.axis << 20);
-        out[2 * c] = make_float4(m.n.x, m.n.y, m.n.z, m.d[c]);
-        out[2 * c + 1] = make_float4(m.p[c].x, m.p[c].y, m.p[c].z, __int_as_float(tag));
-      }
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+        if (c < m.np) {
+          const int tag = (lo & 0xffff) | (c << 16) | (m.axis << 20);
+          out[2 * c] = make_float4(m.n.x, m.n.y, m.n.z, m.d[c]);
+          out[2 * c + 1] = make_float4(m.p[c].x, m.p[c].y, m.p[c].z, __int_as_float(tag));
+        }
     }
     off0 += tot;
   }
