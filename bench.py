@@ -359,7 +359,7 @@ def run_cuda(args) -> dict:
         "status": {"or": status_or, "envs_flagged": n_flagged},
         "maxima": {k: cnt[k] for k in ("max_candidates", "max_colliding", "max_colours")},
         "capacity": {"max_pairs": wp.max_pairs, "max_contacts": wp.max_contacts, "smem_bytes_per_cta": linfo["smem_bytes"],
-                     "threads_per_cta": linfo["threads"], "envs_per_cta": linfo["threads"] // 32},
+                     "threads_per_cta": linfo["threads"], "envs_in_flight_per_sm": linfo["threads"] // 32},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke,
                 "split": n_split, "launches": e2e_launches},
@@ -385,7 +385,7 @@ def main():
     ap.add_argument("--e2e-split", type=int, default=2, help="worlds (streams) the e2e leg serves the batch with")
     ap.add_argument("--cfg", type=int, default=CFG, help="BASELINE.json config number (5 = the bench workload; others: manual runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--tier", default="auto", choices=["auto", "smem", "tmem256", "tmem512"], help="where k_solve keeps the contact constants")
+    ap.add_argument("--tier", default="auto", choices=["auto", "smem", "tmem160", "tmem256", "tmem512"], help="where k_solve keeps the contact constants")
     ap.add_argument("--max-contacts", type=int, default=0, help="override the workload's contact capacity per env")
     ap.add_argument("--max-pairs", type=int, default=0, help="override the workload's candidate capacity per env")
     args = ap.parse_args()

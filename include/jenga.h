@@ -84,10 +84,12 @@ typedef struct {
   int32_t  device;                      /* CUDA device ordinal the buffers live on                     */
   float    collapse_length;             /* block length l of Eq. 18; latch off if <= 0 */
   float    collapse_fd, collapse_ek, collapse_theta;   /* f_d = 0.5, eps_k = 5e-5 J, theta_th = 30 deg in rad   */
-  int32_t  solver_tier;                 /* where the PGS kernel keeps the contact constants: 0 = auto (the fastest tier
-                                           that fits), 1 = shared memory only (one warp per CTA), 2 = tensor memory,
-                                           256 columns per 4-env CTA (two CTAs per SM), 3 = tensor memory, 512 columns
-                                           (one CTA per SM).  A tier that does not fit the sizes is JENGA_E_ARG.       */
+  int32_t  solver_tier;                 /* where the PGS kernel keeps the contact constants: 0 = auto (the most envs in
+                                           flight per SM that fit), 1 = shared memory only (one warp per CTA);
+                                           tensor memory, one CTA per SM owning its 512 columns: 4 = 12 envs in flight with
+                                           3 blocks of 32 pairs each in TMEM, 2 = 8 envs with 5 blocks, 3 = 4 envs with 10
+                                           blocks (further blocks are served from the L2-resident scratch).  A tier that
+                                           does not fit the sizes is JENGA_E_ARG.                                     */
 } jenga_world_desc;
 
 /* All DEVICE pointers, caller-owned, 16-byte aligned.  PC = max_contacts/4. */

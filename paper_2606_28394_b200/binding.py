@@ -43,7 +43,7 @@ class Buffers(C.Structure):
                                           "ref_pose", "collapsed", "collapse_stats", "rest_steps", "scratch")] + [("scratch_bytes", C.c_size_t)]
 
 
-TIERS = {"auto": 0, "smem": 1, "tmem256": 2, "tmem512": 3}
+TIERS = {"auto": 0, "smem": 1, "tmem256": 2, "tmem512": 3, "tmem160": 4}
 
 
 def lib():

@@ -30,7 +30,7 @@ __global__ void k_reset_rest(const Params P) {
 // =================================================================== host side / C-ABI
 using jenga::Params;
 
-enum { TierAuto = 0, TierSmem = 1, TierTmem256 = 2, TierTmem512 = 3 };
+enum { TierAuto = 0, TierSmem = 1, TierTmem256 = 2, TierTmem512 = 3, TierTmem160 = 4 };
 static const size_t kSmemMax = 227 * 1024;
 
 struct jenga_world {
@@ -62,32 +62,32 @@ static bool desc_ok(const jenga_world_desc* d) {
   if (d->n_substeps <= 0 || d->n_substeps > 64 || d->pgs_iters < 0 || !(d->dt > 0.0f)) return false;
   if (d->max_pairs <= 0 || d->max_pairs > 65535) return false;
   if (d->max_contacts < 4 || (d->max_contacts & 3) || d->max_contacts > 65532) return false;
-  if (d->solver_tier < TierAuto || d->solver_tier > TierTmem512) return false;
+  if (d->solver_tier < TierAuto || d->solver_tier > TierTmem160) return false;
   if (collide_env_bytes(d) > kSmemMax || solve_env_bytes(d, 0) > kSmemMax) return false;
   return true;
 }
 
-/* TMEM blocks per env of k_solve.  5 (256 columns per 4-env CTA) when two such CTAs fit one SM: 8 envs per SM; else 10
- * (512 columns) when one 4-env CTA fits: 4 envs per SM; else 0: everything in shared memory, one warp per CTA.
- * desc.solver_tier forces one of the three (-1 if it does not fit).                                              */
+/* TMEM blocks per env of k_solve: the CTA (one per SM) has 4 G warps = 4 G envs in flight; each env gets 512 / G columns
+ * = tmb blocks of 48: G = 3 -> 3 blocks (12 envs per SM), G = 2 -> 5, G = 1 -> 10; 0 = everything in shared memory, one
+ * warp per CTA.  Auto takes the largest G whose shared memory (headers + bodies of 4 G envs) fits one SM;
+ * desc.solver_tier forces a tier (-1 if it does not fit).                                                         */
+static int tier_groups(int tmb) { return tmb == 3 ? 3 : (tmb == 5 ? 2 : (tmb == 10 ? 1 : 0)); }
+static bool tier_fits(const jenga_world_desc* d, int tmb) {
+  return 4 * tier_groups(tmb) * solve_env_bytes(d, tmb) + 1024 + 16 <= kSmemMax;
+}
 static int pick_tmb(const jenga_world_desc* d) {
-  const bool fit5 = 2 * (4 * solve_env_bytes(d, 5) + 1024 + 16) <= kSmemMax;
-  const bool fit10 = 4 * solve_env_bytes(d, 10) + 1024 + 16 <= kSmemMax;
   switch (d->solver_tier) {
     case TierSmem: return 0;
-    case TierTmem256: return 4 * solve_env_bytes(d, 5) + 1024 + 16 <= kSmemMax ? 5 : -1;
-    case TierTmem512: return fit10 ? 10 : -1;
-    default: return fit5 ? 5 : (fit10 ? 10 : 0);
+    case TierTmem160: return tier_fits(d, 3) ? 3 : -1;
+    case TierTmem256: return tier_fits(d, 5) ? 5 : -1;
+    case TierTmem512: return tier_fits(d, 10) ? 10 : -1;
+    default: return tier_fits(d, 3) ? 3 : (tier_fits(d, 5) ? 5 : (tier_fits(d, 10) ? 10 : 0));
   }
 }
 
-/* dynamic shared memory of a k_solve CTA.  The 512-column tier must be alone on its SM (a second CTA would wait in
- * tcgen05.alloc holding shared memory and thread slots): its request is padded past half of the SM's shared memory. */
+/* dynamic shared memory of a k_solve CTA */
 static size_t solve_cta_bytes(const jenga_world_desc* d, int tmb) {
-  if (tmb == 0) return solve_env_bytes(d, 0);
-  size_t b = 4 * solve_env_bytes(d, tmb);
-  if (tmb > 5 && b < kSmemMax / 2 + 1024) b = kSmemMax / 2 + 1024;
-  return b;
+  return tmb ? 4 * tier_groups(tmb) * solve_env_bytes(d, tmb) : solve_env_bytes(d, 0);
 }
 
 extern "C" size_t jenga_smem_bytes(const jenga_world_desc* d) {
@@ -99,7 +99,7 @@ extern "C" size_t jenga_smem_bytes(const jenga_world_desc* d) {
 extern "C" int jenga_block_threads(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
   const int tmb = pick_tmb(d);
-  return tmb < 0 ? 0 : (tmb ? 128 : 32);   /* one warp per env; 4 envs per CTA in the TMEM tiers */
+  return tmb < 0 ? 0 : (tmb ? 128 * tier_groups(tmb) : 32);   /* one warp per env; 4, 8 or 12 envs per CTA in the TMEM tiers */
 }
 
 extern "C" size_t jenga_scratch_bytes(const jenga_world_desc* d) {
@@ -266,11 +266,10 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
 static int launch_solve(jenga_world* w, int iters, int flags, float rest_ek, cudaStream_t st) {
   const cudaError_t e = ensure_smem(w->desc.device, w->tmb ? KnSolveTm : KnSolveSm, w->smem_solve);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_solve)");
-  /* persistent CTAs: as many as are resident at once (2 x 4-env CTAs per SM in the 256-column tier), each warp strides
-   * over the envs */
+  /* persistent CTAs: one per SM in the TMEM tiers (it owns all 512 columns), each warp strides over the envs */
   if (w->tmb) {
-    const int resident = w->n_sm * (w->tmb > 5 ? 1 : 2), need = (w->P.E + 3) / 4;
-    jenga::k_solve<true><<<need < resident ? need : resident, 128, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
+    const int wpc = 4 * tier_groups(w->tmb), need = (w->P.E + wpc - 1) / wpc;
+    jenga::k_solve<true><<<need < w->n_sm ? need : w->n_sm, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
   } else {
     const int per_sm = (int)(kSmemMax / (w->smem_solve + 1024)), resident = w->n_sm * (per_sm < 1 ? 1 : (per_sm > 16 ? 16 : per_sm));
     jenga::k_solve<false><<<w->P.E < resident ? w->P.E : resident, 32, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);

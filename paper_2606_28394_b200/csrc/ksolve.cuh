@@ -2,11 +2,13 @@
 // S6 integration + Baumgarte, S7 warm-start cache, Eq. 18 latch.  Inputs: the state tile and the scratch k_collide wrote.
 //
 // Two flavours (template <bool TM>):
-//   TM = true   CTA = 4 warps = 4 envs; the 48 constant words of the positions of the first `tmb` 32-position blocks
-//               live in tensor memory (tcgen05.ld/st.32x32b: lane = position % 32, block j at columns [48 j, 48 j + 48),
-//               warp w owns TMEM lanes 32 w .. 32 w + 31); tmb = 5: 256 columns per CTA, 2 CTAs per SM (8 envs per SM);
-//               tmb = 10: 512 columns, 1 CTA per SM.  Blocks >= tmb are kept in shared memory.
-//   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers).
+//   TM = true   ONE persistent CTA per SM of 4 G warps = 4 G envs in flight (G = 3, 2 or 1) that owns all 512 columns of
+//               tensor memory.  Warp w works in TMEM lanes 32 (w % 4) .. + 31 (its quadrant) and columns
+//               [48 tmb (w / 4), + 48 tmb): the 48 constant words of the positions of the env's first `tmb` 32-position
+//               blocks (tmb = 3, 5, 10 for G = 3, 2, 1; tcgen05.ld/st.32x32b: lane = position % 32, block j at column
+//               offset 48 j).  Blocks >= tmb stay where k_collide wrote them, in the scratch (L2-resident while the env is
+//               in flight): their visits load and store global memory, one visit ahead of use.
+//   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers; test coverage).
 #pragma once
 #include "kcollide.cuh"
 
@@ -16,16 +18,18 @@ struct SSm {
   SP<float> bd;                 // [S][kBd] solver body records
   SP<float> q;                  // [4][S]
   SP<float4> hdr;               // [kHdrF4][npos]
-  SP<float4> cs;                // [nblk - tmb][kCsF4][32] blocks kept in shared memory
+  SP<float4> cs;                // TM = false: [nblk][kCsF4][32] every block in shared memory
   SP<int> ph;                   // [ph_max]
   int npos, tmb;
-  unsigned tm;                  // TMEM address of this warp's lanes, column 0
+  unsigned tm;                  // TMEM address of this warp's lanes, first column of its group
+  float4* gcs;                  // TM = true: the env's constant blocks in the scratch (blocks >= tmb are used in place)
 };
 
+// tmb = 0: the all-shared-memory flavour
 __host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb) {
   const int nblk = n_blocks(pc);
   size_t w = (size_t)(kBd + 4) * S + 4 * kHdrF4 * 32 * (size_t)nblk;
-  w += (size_t)kBlkWords * (nblk > tmb ? nblk - tmb : 0);
+  w += tmb ? 0 : (size_t)kBlkWords * nblk;
   w += round_up(ph_max(nblk), 4);
   return round_up((int)w, 4);
 }
@@ -33,9 +37,9 @@ __host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb) {
 __device__ inline SSm carve_solve(int S, int pc, int tmb, int base) {
   const int nblk = n_blocks(pc);
   SSm s; int p = base;
-  s.npos = 32 * nblk; s.tmb = tmb; s.tm = 0;
+  s.npos = 32 * nblk; s.tmb = tmb; s.tm = 0; s.gcs = nullptr;
   s.hdr.off = p; p += 4 * kHdrF4 * s.npos;
-  s.cs.off = p;  p += kBlkWords * (nblk > tmb ? nblk - tmb : 0);
+  s.cs.off = p;  p += tmb ? 0 : kBlkWords * nblk;
   s.bd.off = p;  p += kBd * S;
   s.q.off = p;   p += 4 * S;
   s.ph.off = p;
@@ -83,19 +87,24 @@ __device__ __forceinline__ void tm_store_lam(const SSm& s, int j, const float* l
   const unsigned a = s.tm + 48u * (unsigned)j + 36u;
   tm_st8(a, lam); tm_st4(a + 8, lam + 8);
 }
-// shared-memory tier: block j >= tmb, lane l
+// blocks outside tensor memory, lane l: shared memory (TM = false) or the scratch itself (TM = true, block j >= tmb)
+template <bool TM>
+__device__ __forceinline__ float4* ov_ptr(const SSm& s, int j, int l) { return (TM ? s.gcs : s.cs.ptr()) + j * (kCsF4 * 32) + l; }
+template <bool TM>
 __device__ __forceinline__ void sm_load_pair(const SSm& s, int j, int l, PairC& c) {
-  const float4* b = s.cs.ptr() + (j - s.tmb) * (kCsF4 * 32) + l;
+  const float4* b = ov_ptr<TM>(s, j, l);
 #pragma unroll
   for (int f = 0; f < kCsF4; ++f) { const float4 t = b[f * 32]; c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
 }
+template <bool TM>
 __device__ __forceinline__ void sm_store_pair(const SSm& s, int j, int l, const PairC& c) {
-  float4* b = s.cs.ptr() + (j - s.tmb) * (kCsF4 * 32) + l;
+  float4* b = ov_ptr<TM>(s, j, l);
 #pragma unroll
   for (int f = 0; f < kCsF4; ++f) b[f * 32] = make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]);
 }
+template <bool TM>
 __device__ __forceinline__ void sm_store_lam(const SSm& s, int j, int l, const float* lam) {
-  float4* b = s.cs.ptr() + (j - s.tmb) * (kCsF4 * 32) + l;
+  float4* b = ov_ptr<TM>(s, j, l);
 #pragma unroll
   for (int f = 0; f < 3; ++f) b[(9 + f) * 32] = make_float4(lam[4 * f], lam[4 * f + 1], lam[4 * f + 2], lam[4 * f + 3]);
 }
@@ -103,27 +112,27 @@ __device__ __forceinline__ void sm_store_lam(const SSm& s, int j, int l, const f
 template <bool TM>
 __device__ __forceinline__ void block_load(const SSm& s, int j, PairC& c) {
   if (TM && j < s.tmb) { tm_load_block(s, j, c); tm_wait_ld(); }
-  else sm_load_pair(s, j, lane_id(), c);
+  else sm_load_pair<TM>(s, j, lane_id(), c);
 }
 
 // ---------------------------------------------------------------- warp / TMEM set-up
 template <bool TM>
 __device__ __forceinline__ SSm begin_solve(const Params& P, int& env) {
   __shared__ unsigned tm_base_s;
-  const int warp = threadIdx.x >> 5;
-  env = blockIdx.x * (TM ? 4 : 1) + warp;
-  const int tmb = TM ? P.tmb : 0, cols = tmb > 5 ? 512 : 256;
+  const int warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+  env = blockIdx.x * wpc + warp;
+  const int tmb = TM ? P.tmb : 0;
   SSm s = carve_solve(P.S, P.pc, tmb, warp * (int)solve_smem_words(P.S, P.pc, tmb));
   if (TM) {
     if (warp == 0) {
       asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                   :: "r"((unsigned)__cvta_generic_to_shared(&tm_base_s)), "r"(cols) : "memory");
+                   :: "r"((unsigned)__cvta_generic_to_shared(&tm_base_s)), "r"(512) : "memory");
       asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    s.tm = tm_base_s + ((unsigned)(warp * 32) << 16);
+    s.tm = tm_base_s + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)(48 * tmb * (warp >> 2));
   }
   return s;
 }
@@ -131,11 +140,10 @@ __device__ __forceinline__ SSm begin_solve(const Params& P, int& env) {
 template <bool TM>
 __device__ __forceinline__ void end_solve(const SSm& s) {
   if (TM) {
-    const int cols = s.tmb > 5 ? 512 : 256;
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if ((threadIdx.x >> 5) == 0)
-      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s.tm), "r"(cols) : "memory");   // warp 0: s.tm = base
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s.tm), "r"(512) : "memory");   // warp 0: s.tm = base
   }
 }
 
@@ -187,15 +195,16 @@ __device__ inline int load_slots(const SSm& s, const Params& P, const float* scr
   for (int f = 0; f < kHdrF4; ++f)
     for (int k = lane; k < 32 * nblk; k += 32) s.hdr[f * s.npos + k] = ghdr[f * s.npos + k];
   const float4* gcs = reinterpret_cast<const float4*>(scr + L.cs);
-  for (int j = 0; j < nblk; ++j) {
+  const int ncopy = TM ? min(nblk, s.tmb) : nblk;              // TM: blocks >= tmb are used in place
+  for (int j = 0; j < ncopy; ++j) {
     PairC c;
 #pragma unroll
     for (int f = 0; f < kCsF4; ++f) {
       const float4 t = gcs[(j * kCsF4 + f) * 32 + lane];
       c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w;
     }
-    if (TM && j < s.tmb) tm_store_block(s, j, c);
-    else sm_store_pair(s, j, lane, c);
+    if (TM) tm_store_block(s, j, c);
+    else sm_store_pair<TM>(s, j, lane, c);
   }
   if (TM) tm_wait_st();
   __syncwarp();
@@ -308,7 +317,7 @@ __device__ inline void pgs_sweeps(const SSm& s, int nph, int iters, float mu) {
   Hdr H; H.a = -1; H.b = 0; H.n = H.t1 = v3(0, 0, 0);
   if (chunk_lane(d, lane)) H = load_hdr(s, 32 * (d >> 16) + lane);
   if (TM && (d >> 16) < s.tmb) tm_load_block(s, d >> 16, c);
-  else sm_load_pair(s, d >> 16, lane, c);
+  else sm_load_pair<TM>(s, d >> 16, lane, c);
 #pragma unroll 1
   for (int v = 0; v < total; ++v) {
     const int jb = d >> 16;
@@ -324,14 +333,14 @@ __device__ inline void pgs_sweeps(const SSm& s, int nph, int iters, float mu) {
       solve_pair<false>(c, A, B, F, mu);
       if (H.a >= 0) { bd4(s, H.a, 1) = A.v; bd4(s, H.a, 2) = A.w; }
       bd4(s, H.b, 1) = B.v; bd4(s, H.b, 2) = B.w;
-      if (!in_tm) sm_store_lam(s, jb, lane, c.v + kLam);
+      if (!in_tm) sm_store_lam<TM>(s, jb, lane, c.v + kLam);
     } else if (chunk_lane(dn, lane)) {
       Hn = load_hdr(s, 32 * (dn >> 16) + lane);
     }
     if (in_tm) { tm_store_lam(s, jb, c.v + kLam); tm_wait_st(); }
     __syncwarp();
     if (TM && (dn >> 16) < s.tmb) tm_load_block(s, dn >> 16, c);
-    else sm_load_pair(s, dn >> 16, lane, c);
+    else sm_load_pair<TM>(s, dn >> 16, lane, c);
     d = dn; H = Hn;
   }
   if (TM) tm_wait_ld();
@@ -474,12 +483,12 @@ __device__ inline int2 store_cache(const SSm& s, const Params& P, int env, const
 enum { SolveEndOfStep = 1, SolvePgsOnly = 2, SolveRest = 4 };
 
 template <bool TM>
-__global__ void __launch_bounds__(TM ? 128 : 32, TM ? 2 : 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
+__global__ void __launch_bounds__(TM ? 384 : 32, 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
   int env0;
-  const SSm s = begin_solve<TM>(P, env0);
+  SSm s = begin_solve<TM>(P, env0);
   const int lane = lane_id();
   const Scratch L = scratch_layout(P.pc);
-  const int stride = gridDim.x * (TM ? 4 : 1);
+  const int stride = gridDim.x * (blockDim.x >> 5);
   // persistent: warp w of CTA c takes envs c * wpc + w, + stride, ... (TMEM is allocated once per CTA; the warps of a CTA
   // never wait for one another between envs)
   for (int env = env0; env < P.E; env += stride) {
@@ -487,6 +496,7 @@ __global__ void __launch_bounds__(TM ? 128 : 32, TM ? 2 : 1) k_solve(const Param
     int* meta = reinterpret_cast<int*>(scr + L.meta);
     if ((flags & SolveRest) && meta[MetaResting]) continue;
     unsigned st = 0;
+    s.gcs = reinterpret_cast<float4*>(scr + L.cs);
     load_bodies(s, P, env);
     const int nph = load_slots<TM>(s, P, scr, L);
     if (P.warm_start) warm_start_pass<TM>(s, nph);
