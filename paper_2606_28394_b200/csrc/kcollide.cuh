@@ -13,7 +13,8 @@ struct CSm {
   SP<unsigned long long> used;  // [S]      colour masks per body
   SP<unsigned> cab;             // [pcA]    (a+1) | A dynamic << 11 | axis << 12 | b << 16 | B dynamic << 27
   SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending
-  SP<float> poly;               // [8][3][32] clip polygon of every lane (component-major: lane l <-> bank l)
+  SP<float> poly;               // [8][3][32] clip polygon of every lane (component-major: lane l <-> bank l); ALIASES cand,
+                                //            which is dead once the colliding-pair list exists
   SP<unsigned short> cpair;     // [pcA]    colliding pair indices, ascending
   SP<unsigned short> cprev;     // [pcA]    pair indices of the warm-start cache (previous substep), ascending
   SP<unsigned short> pos;       // [pcA]    position of pair r
@@ -32,7 +33,7 @@ __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int p
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc);
   size_t w = (size_t)kCb * S + 3 * S + 2 * S;            // cb, ext, used
   w += pcA;                                              // cab
-  w += mpA / 2 + 768;                                    // cand, poly
+  w += mpA / 2 > 768 ? mpA / 2 : 768;                    // cand / poly (aliased)
   w += 4 * (size_t)(pcA / 2);                            // cpair, cprev, pos, wrank
   w += pcA / 4;                                          // colour
   w += 2 * round_up(ph_max(nblk), 4);                    // ph, chc
@@ -48,8 +49,7 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base) {
   if (p & 1) ++p;
   s.used.off = p;   p += 2 * S;
   s.cab.off = p;    p += pcA;
-  s.cand.off = p;   p += mpA / 2;
-  s.poly.off = p;   p += 768;
+  s.cand.off = p;   s.poly.off = p;   p += mpA / 2 > 768 ? mpA / 2 : 768;
   s.cpair.off = p;  p += pcA / 2;
   s.cprev.off = p;  p += pcA / 2;
   s.pos.off = p;    p += pcA / 2;
@@ -747,8 +747,9 @@ __device__ inline int write_contacts(const CSm& s, const Params& P, int env, flo
     int tot; const int off = off0 + warp_excl_scan(m.np, &tot);
     if (r < n_coll) {
       s.wrank[r] = (unsigned short)off; gcoff[r] = (unsigned short)off;
-      int lo = 0, hi = n_cand;                                   // position of the pair in the candidate list
-      while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)s.cand[mid] < idx) lo = mid + 1; else hi = mid; }
+      const int* gp = P.pairs + (size_t)env * P.max_pairs;      // position of the pair in the candidate list (the on-chip
+      int lo = 0, hi = n_cand;                                   // copy is overwritten by the clip polygons)
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if (gp[mid] < idx) lo = mid + 1; else hi = mid; }
       float4* out = reinterpret_cast<float4*>(P.contacts + ((size_t)env * P.max_contacts + off) * 8);
 #pragma unroll
       for (int c = 0; c < 4; ++c)

@@ -15,7 +15,7 @@
 namespace jenga {
 
 struct SSm {
-  SP<float> bd;                 // [S][kBd] solver body records
+  SP<float> bd;                 // [S + 1][kBd] solver body records; record S is the ground: all zeros, never changes
   SP<float> q;                  // [4][S]
   SP<float4> hdr;               // [kHdrF4][npos]
   SP<float4> cs;                // TM = false: [nblk][kCsF4][32] every block in shared memory
@@ -28,7 +28,7 @@ struct SSm {
 // tmb = 0: the all-shared-memory flavour
 __host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb) {
   const int nblk = n_blocks(pc);
-  size_t w = (size_t)(kBd + 4) * S + 4 * kHdrF4 * 32 * (size_t)nblk;
+  size_t w = (size_t)(kBd + 4) * S + kBd + 4 * kHdrF4 * 32 * (size_t)nblk;
   w += tmb ? 0 : (size_t)kBlkWords * nblk;
   w += round_up(ph_max(nblk), 4);
   return round_up((int)w, 4);
@@ -40,7 +40,7 @@ __device__ inline SSm carve_solve(int S, int pc, int tmb, int base) {
   s.npos = 32 * nblk; s.tmb = tmb; s.tm = 0; s.gcs = nullptr;
   s.hdr.off = p; p += 4 * kHdrF4 * s.npos;
   s.cs.off = p;  p += tmb ? 0 : kBlkWords * nblk;
-  s.bd.off = p;  p += kBd * S;
+  s.bd.off = p;  p += kBd * (S + 1);
   s.q.off = p;   p += 4 * S;
   s.ph.off = p;
   return s;
@@ -168,6 +168,7 @@ __device__ inline void load_bodies(const SSm& s, const Params& P, int env) {
     bd4(s, b, 4) = make_float4(I6[4], I6[5], i2, 0.0f);
     s.q[b] = w; s.q[S + b] = x; s.q[2 * S + b] = y; s.q[3 * S + b] = z;
   }
+  if (lane_id() < 5) bd4(s, S, lane_id()) = make_float4(0, 0, 0, 0);      // the ground: inverse mass and inertia 0, at rest
 }
 
 __device__ inline void store_bodies(const SSm& s, const Params& P, int env) {
@@ -214,12 +215,10 @@ __device__ inline int load_slots(const SSm& s, const Params& P, const float* scr
 struct Body5 { float4 x, v, w, i0, i1; };     // x.w = inverse mass (0: static / inactive / ground)
 
 __device__ __forceinline__ void load_body(const SSm& s, int b, Body5& o) {
-  if (b >= 0) {
-    o.x = bd4(s, b, 0); o.v = bd4(s, b, 1); o.w = bd4(s, b, 2); o.i0 = bd4(s, b, 3); o.i1 = bd4(s, b, 4);
-  } else {
-    o.x = o.v = o.w = o.i0 = o.i1 = make_float4(0, 0, 0, 0);
-  }
+  o.x = bd4(s, b, 0); o.v = bd4(s, b, 1); o.w = bd4(s, b, 2); o.i0 = bd4(s, b, 3); o.i1 = bd4(s, b, 4);
 }
+// the ground's velocities stay +-0 (its inverse mass and inertia are 0), so writing them back is harmless
+__device__ __forceinline__ void store_body_vel(const SSm& s, int b, const Body5& o) { bd4(s, b, 1) = o.v; bd4(s, b, 2) = o.w; }
 
 // a loses the impulse, b gains it (Listing 1, PAPER.md:335-336 + the angular lines, reading A11)
 __device__ __forceinline__ void apply_impulse(Body5& A, Body5& B, Vec3 rA, Vec3 rB, Vec3 Pi) {
@@ -275,28 +274,28 @@ __device__ __forceinline__ void solve_pair(PairC& c, Body5& A, Body5& B, const F
 
 // What a lane needs of its pair's header during a visit.
 struct Hdr { int a, b; Vec3 n, t1; };
-__device__ __forceinline__ Hdr load_hdr(const SSm& s, int k) {
+// a = body record of A: the ground (header field 0) is the all-zero record S
+__device__ __forceinline__ Hdr load_hdr(const SSm& s, int S, int k) {
   const float4 h = hdr4(s, 0, k), nn = hdr4(s, 1, k), tt = hdr4(s, 2, k);
-  Hdr H; const int ab = __float_as_int(h.x);
-  H.a = (ab & 0xffff) - 1; H.b = ab >> 16; H.n = xyz(nn); H.t1 = xyz(tt);
+  Hdr H; const int ab = __float_as_int(h.x), a1 = ab & 0xffff;
+  H.a = a1 ? a1 - 1 : S; H.b = ab >> 16; H.n = xyz(nn); H.t1 = xyz(tt);
   return H;
 }
 __device__ __forceinline__ bool chunk_lane(int d, int lane) { const int l0 = d & 0xff; return lane >= l0 && lane < l0 + ((d >> 8) & 0xff); }
 
 // S4: the cached impulses are applied once, chunk by chunk in canonical order (no impulse changes: nothing is stored).
 template <bool TM>
-__device__ inline void warm_start_pass(const SSm& s, int nph) {
+__device__ inline void warm_start_pass(const SSm& s, int S, int nph) {
   const int lane = lane_id();
   for (int j = 0; j < nph; ++j) {
     const int d = s.ph[j], jb = d >> 16;
     PairC c; block_load<TM>(s, jb, c);
     if (chunk_lane(d, lane)) {
-      const Hdr H = load_hdr(s, 32 * jb + lane);
+      const Hdr H = load_hdr(s, S, 32 * jb + lane);
       Body5 A, B; load_body(s, H.a, A); load_body(s, H.b, B);
       Frame F; F.n = H.n; F.t1 = H.t1; F.t2 = cross(F.n, F.t1);
       solve_pair<true>(c, A, B, F, 0.0f);
-      if (H.a >= 0) { bd4(s, H.a, 1) = A.v; bd4(s, H.a, 2) = A.w; }
-      bd4(s, H.b, 1) = B.v; bd4(s, H.b, 2) = B.w;
+      store_body_vel(s, H.a, A); store_body_vel(s, H.b, B);
     }
     __syncwarp();
   }
@@ -309,13 +308,13 @@ __device__ inline void warm_start_pass(const SSm& s, int nph) {
 // the next visit starts with the (dependent) body loads at once.  TMEM accesses are warp-wide: the lanes outside the
 // chunk write back the impulses they loaded.
 template <bool TM>
-__device__ inline void pgs_sweeps(const SSm& s, int nph, int iters, float mu) {
+__device__ inline void pgs_sweeps(const SSm& s, int S, int nph, int iters, float mu) {
   const int total = nph * iters, lane = lane_id();
   if (total <= 0) return;
   int d = s.ph[0], jn = 0;
   PairC c;
-  Hdr H; H.a = -1; H.b = 0; H.n = H.t1 = v3(0, 0, 0);
-  if (chunk_lane(d, lane)) H = load_hdr(s, 32 * (d >> 16) + lane);
+  Hdr H; H.a = S; H.b = S; H.n = H.t1 = v3(0, 0, 0);
+  if (chunk_lane(d, lane)) H = load_hdr(s, S, 32 * (d >> 16) + lane);
   if (TM && (d >> 16) < s.tmb) tm_load_block(s, d >> 16, c);
   else sm_load_pair<TM>(s, d >> 16, lane, c);
 #pragma unroll 1
@@ -324,18 +323,15 @@ __device__ inline void pgs_sweeps(const SSm& s, int nph, int iters, float mu) {
     const bool active = chunk_lane(d, lane), in_tm = TM && jb < s.tmb;
     jn = jn + 1 == nph ? 0 : jn + 1;
     const int dn = s.ph[jn];
-    Hdr Hn; Hn.a = -1; Hn.b = 0; Hn.n = Hn.t1 = v3(0, 0, 0);
     if (in_tm) tm_wait_ld();
+    // every lane fetches the header of its position in the next chunk's block (garbage outside the chunk: never used)
+    const Hdr Hn = load_hdr(s, S, 32 * (dn >> 16) + lane);
     if (active) {
       Body5 A, B; load_body(s, H.a, A); load_body(s, H.b, B);
-      if (chunk_lane(dn, lane)) Hn = load_hdr(s, 32 * (dn >> 16) + lane);
       Frame F; F.n = H.n; F.t1 = H.t1; F.t2 = cross(F.n, F.t1);
       solve_pair<false>(c, A, B, F, mu);
-      if (H.a >= 0) { bd4(s, H.a, 1) = A.v; bd4(s, H.a, 2) = A.w; }
-      bd4(s, H.b, 1) = B.v; bd4(s, H.b, 2) = B.w;
+      store_body_vel(s, H.a, A); store_body_vel(s, H.b, B);
       if (!in_tm) sm_store_lam<TM>(s, jb, lane, c.v + kLam);
-    } else if (chunk_lane(dn, lane)) {
-      Hn = load_hdr(s, 32 * (dn >> 16) + lane);
     }
     if (in_tm) { tm_store_lam(s, jb, c.v + kLam); tm_wait_st(); }
     __syncwarp();
@@ -499,8 +495,8 @@ __global__ void __launch_bounds__(TM ? 384 : 32, 1) k_solve(const Params P, cons
     s.gcs = reinterpret_cast<float4*>(scr + L.cs);
     load_bodies(s, P, env);
     const int nph = load_slots<TM>(s, P, scr, L);
-    if (P.warm_start) warm_start_pass<TM>(s, nph);
-    pgs_sweeps<TM>(s, nph, iters, P.mu[env]);
+    if (P.warm_start) warm_start_pass<TM>(s, P.S, nph);
+    pgs_sweeps<TM>(s, P.S, nph, iters, P.mu[env]);
     if (flags & SolvePgsOnly) {
       store_cache<TM>(s, P, env, scr, L, nph, false, true);      // lambda in contact order only
       store_bodies(s, P, env);
