@@ -132,7 +132,7 @@ class World:
     """
 
     def __init__(self, wp, state, props, mu, materialise: bool = False, device: int = 0, collapse_length: float = 0.0,
-                 tier: str = "auto"):
+                 tier: str = "auto", ref_state=None):
         if not torch.cuda.is_available():
             raise JengaError("no CUDA device: the Jenga step has no CPU path")
         self.wp = wp
@@ -174,7 +174,8 @@ class World:
         b.rest_steps = self.rest_steps.data_ptr()
         b.scratch, b.scratch_bytes = self.scratch.data_ptr(), n_scr
         if collapse_length > 0.0:                      # Eq. 18 latch against the pose the world starts from
-            self.ref_pose = self.state[:, 0:7, :].clone()      # a copy also when E = 1 (contiguous() would alias the live state)
+            src = self.state if ref_state is None else t(ref_state, torch.float32)      # Eq. 18's reference pose
+            self.ref_pose = src[:, 0:7, :].clone()             # a copy also when E = 1 (contiguous() would alias the live state)
             self.collapsed = z((E,), torch.int32)
             self.collapse_stats = z((E, 4), torch.float32)
             b.ref_pose, b.collapsed, b.collapse_stats = self.ref_pose.data_ptr(), self.collapsed.data_ptr(), self.collapse_stats.data_ptr()

@@ -474,6 +474,66 @@ def test_rollout_collapse_agreement(orc, J):
     assert agree[far].mean() >= self_agree[far].mean() - 0.01
 
 
+def load_cache(world, cache):
+    """The oracle's warm-start cache, rounded to fp32, into the GPU buffers (and back into the oracle's own copy)."""
+    import torch
+    cache.lam[:] = cache.lam.astype(np.float32); cache.pt[:] = cache.pt.astype(np.float32)
+    world.cache_key[:, :, :] = torch.as_tensor(np.stack([cache.key_pair, cache.key_meta], axis=-1)).to(world.dev)
+    world.cache_lam[:] = torch.as_tensor(cache.lam.astype(np.float32)).to(world.dev)
+    world.cache_pt[:] = torch.as_tensor(cache.pt.astype(np.float32)).to(world.dev)
+    world.n_cache[:] = torch.as_tensor(cache.n_keys).to(world.dev)
+
+
+def test_collapse_stats_match_oracle(orc, J):
+    """The kernel's Eq. 18 terms (collapse_stats = dx_max, E_k, theta_max of the last step) against the oracle's
+    orc_collapse_test (pinned in tests/test_oracle_collapse.py), element by element, one step from a common mid-collapse
+    state of cfg2 (step 130: the pushes ended at step 84, several towers are falling, others stand)."""
+    import torch
+    E = 16
+    wl = W.make_config(2, n_envs=E)
+    B = wl.params.n_bodies
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(wl.state, wl.props, B)
+    x0, q0 = bod.x.copy(), bod.q.copy()
+    cache = orc.Cache(E, wl.params.max_contacts); f64 = orc.unpack_fext(wl.push_fext, B); mu64 = wl.mu.astype(np.float64)
+    for lo, hi, f in ((0, wl.push_start, None), (wl.push_start, wl.push_end, f64), (wl.push_end, 130, None)):
+        orc.rollout(P, bod, mu64, hi - lo, fext=f, cache=cache)
+    state = orc.pack_state(bod, wl.params.body_stride).astype(np.float32)
+    world = J.World(wl.params, state, wl.props, wl.mu, collapse_length=W.BLOCK_L, ref_state=wl.state)
+    load_cache(world, cache)
+    world.step(1); torch.cuda.synchronize()
+    stats = world.collapse_stats.cpu().numpy().astype(np.float64); flags = world.collapsed.cpu().numpy()
+    bod = orc.unpack_tiles(state, wl.props, B)
+    n_moving = 0
+    for e in range(E):
+        orc.step_env(P, bod, float(wl.mu[e]), e=e, cache=cache)
+        ref_flag, out = orc.collapse_test(bod, x0[e], q0[e], e=e, length=W.BLOCK_L)
+        assert abs(stats[e, 0] - out[0]) < 2e-6, (e, stats[e], out)                       # dx_max [m]
+        assert abs(stats[e, 2] - out[2]) < 5e-4 + 1e-4 * out[2], (e, stats[e], out)       # theta_max [rad]: 2 acos|q.q0| in fp32
+        assert abs(stats[e, 1] - out[1]) <= 2e-3 * out[1] + 1e-9, (e, stats[e], out)      # E_k [J]
+        margin = min(abs(out[0] - 0.5 * W.BLOCK_L) / (0.5 * W.BLOCK_L), abs(out[1] - 5e-5) / 5e-5, abs(out[2] - np.radians(30)) / np.radians(30))
+        if margin > 1e-2:
+            assert bool(flags[e]) == ref_flag
+        n_moving += int(out[1] > 5e-5)
+    print(f"\n[collapse stats] {E} envs one step after step 130: {n_moving} with E_k > 5e-5 J, {int(flags.sum())} latched")
+    assert 0 < n_moving < E
+
+
+def test_single_env_latch_keeps_its_reference_pose(J):
+    """E = 1: the reference pose of Eq. 18 is a copy, not a view of the live state; the displacement is
+    measured from the pose the world was created with across launches."""
+    import torch
+    wl = W.make_custom([dict(pos=(0, 0, 0.04), size=(W.BLOCK_L, W.BLOCK_W, W.BLOCK_H), mass=W.BLOCK_MASS, vel=(1.0, 0, 0), omg=(0, 25.0, 0))], mu=0.6)
+    world = J.World(wl.params, wl.state, wl.props, wl.mu, collapse_length=W.BLOCK_L)
+    assert world.ref_pose.data_ptr() != world.state.data_ptr()
+    for _ in range(30):
+        world.step(12)
+    torch.cuda.synchronize()
+    st = world.collapse_stats.cpu().numpy()[0]
+    x = world.state[0, 0:3, 0].cpu().numpy()
+    assert int(world.collapsed[0].item()) == 1                      # latched while it tumbled
+    assert abs(st[0] - np.linalg.norm(x - wl.state[0, 0:3, 0])) < 1e-5 and st[0] > 0.5 * W.BLOCK_L and st[1] < 5e-5
+
+
 # ----------------------------------------------------------------------------- full size, edge cases, untested parameters
 def test_full_size_cfg5_sampled_envs(orc, J):
     """BASELINE.json configs[4] at its full size, in the launch shape bench.py times (65,536 envs, jenga_step(12) is
@@ -500,6 +560,79 @@ def test_full_size_cfg5_sampled_envs(orc, J):
         assert np.max(np.abs(x - bod.x[0])) < TOL_POS, f"env {e}: position error {np.max(np.abs(x - bod.x[0])):.3e}"
         assert np.max(rotation_angle(q, bod.q[0])) < TOL_ANG
     world.destroy()
+
+
+def test_full_size_cfg5_mid_rollout_sampled_envs(orc, J):
+    """The 65,536-env launch shape again, with the sampled envs in a pushed / collapsing state: the oracle advances 40
+    sampled envs of cfg5 to step 96 (settle, 24 push steps, 12 more); their fp32-rounded states and warm-start caches
+    replace the initial ones inside the full batch, and two more steps (the last one under jenga_step(2), i.e. the
+    multi-step call) are compared env by env."""
+    import torch
+    E, n_s, at = 65536, 40, 96
+    wl = W.make_config(5, n_envs=E)
+    B, S = wl.params.n_bodies, wl.params.body_stride
+    sample = np.unique(np.concatenate([[0, E - 1], np.random.default_rng(12).integers(0, E, n_s - 2)]))
+    sub = W.make_config(5, n_envs=1)
+    P = orc.make_params(sub.params)
+    state = wl.state.copy()
+    caches, bods = [], []
+    for e in sample:
+        one = W.make_config(5, n_envs=1, env_offset=int(e))
+        assert np.array_equal(one.state[0], wl.state[e])
+        bod = orc.unpack_tiles(one.state, one.props, B); cache = orc.Cache(1, one.params.max_contacts)
+        f64 = orc.unpack_fext(one.push_fext, B); mu = one.mu.astype(np.float64)
+        for lo, hi, f in ((0, one.push_start, None), (one.push_start, one.push_end, f64), (one.push_end, at, None)):
+            orc.rollout(P, bod, mu, hi - lo, fext=f, cache=cache)
+        state[e] = orc.pack_state(bod, S).astype(np.float32)[0]
+        cache.lam[:] = cache.lam.astype(np.float32); cache.pt[:] = cache.pt.astype(np.float32)
+        caches.append(cache); bods.append(orc.unpack_tiles(state[e:e + 1], wl.props[e:e + 1], B))
+    world = J.World(wl.params, state, wl.props, wl.mu)
+    idx = torch.as_tensor(sample).to(world.dev)
+    world.cache_key[idx] = torch.as_tensor(np.stack([np.stack([c.key_pair[0], c.key_meta[0]], -1) for c in caches])).to(world.dev)
+    world.cache_lam[idx] = torch.as_tensor(np.stack([c.lam[0] for c in caches]).astype(np.float32)).to(world.dev)
+    world.cache_pt[idx] = torch.as_tensor(np.stack([c.pt[0] for c in caches]).astype(np.float32)).to(world.dev)
+    world.n_cache[idx] = torch.as_tensor(np.array([c.n_keys[0] for c in caches], np.int32)).to(world.dev)
+    world.step(2); torch.cuda.synchronize()
+    assert int(world.status.max().item()) == 0
+    g = world.state[idx].cpu().numpy().astype(np.float64)
+    n_moving = worst = 0
+    for n, e in enumerate(sample):
+        bod = bods[n]
+        for _ in range(2):
+            orc.step_env(P, bod, float(wl.mu[e]), e=0, cache=caches[n])
+        x = np.transpose(g[n, 0:3, :B]); q = np.transpose(g[n, 3:7, :B])
+        err = float(np.max(np.abs(x - bod.x[0])))
+        worst = max(worst, err)
+        assert err < 2 * TOL_POS, f"env {e}: position error {err:.3e} after two steps"
+        assert np.max(rotation_angle(q, bod.q[0])) < 2 * TOL_ANG
+        n_moving += int(np.max(np.abs(bod.v[0])) > 0.05)
+    print(f"\n[cfg5 full size, step {at}] {len(sample)} sampled envs, {n_moving} with a block faster than 5 cm/s; worst position error {worst:.2e} m")
+    assert n_moving >= 3
+    world.destroy()
+
+
+def test_status_nonfinite_and_colour_overflow(orc, J):
+    """The two status bits no config raises.  NONFINITE: a NaN velocity in one env is flagged for that env only, on both
+    sides.  COLOUR_OVERFLOW: a slab carrying 70 small blocks has 70 pairs that share one dynamic body, i.e. needs more than
+    64 colours: both sides set the bit (results are then not comparable: colour 63 is no longer conflict-free)."""
+    import torch
+    wl = W.make_config(2, n_envs=3)
+    st = wl.state.copy(); st[1, 7, 53] = np.nan                 # a top-level block: never among the removed ones
+    world = J.World(wl.params, st, wl.props, wl.mu)
+    world.step(1); torch.cuda.synchronize()
+    got = world.status.cpu().numpy()
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(st, wl.props, wl.params.n_bodies)
+    ref = [orc.step_env(P, bod, float(wl.mu[e]), e=e, cache=orc.Cache(3, wl.params.max_contacts)) for e in range(3)]
+    assert list(got & J.ST_NONFINITE) == [0, J.ST_NONFINITE, 0] and [r & 8 for r in ref] == [0, 8, 0]
+    slab = dict(pos=(0, 0, 0.01 - 1e-4), size=(0.62, 0.56, 0.02), mass=2.0)
+    small = [dict(pos=(-0.27 + 0.06 * (k % 10), -0.21 + 0.07 * (k // 10), 0.02 + 0.01 - 2e-4), size=(0.02, 0.02, 0.02), mass=0.005) for k in range(70)]
+    wl = W.make_custom([slab] + small, max_pairs=512, max_contacts=1024)
+    world = J.World(wl.params, wl.state, wl.props, wl.mu)
+    world.step(1); torch.cuda.synchronize()
+    P = orc.make_params(wl.params); bod = orc.unpack_tiles(wl.state, wl.props, 71)
+    ref = orc.step_env(P, bod, 0.4, e=0, cache=orc.Cache(1, 1024))
+    assert ref & 4 and int(world.status[0].item()) & J.ST_COLOUR_OVERFLOW
+    assert world.counters_dict()["max_colours"] == 64 and bool(torch.isfinite(world.state).all().item())
 
 
 def test_empty_and_single_body_envs(orc, J):
