@@ -156,6 +156,20 @@ int jenga_step(jenga_world *w, int n_steps, void *cuda_stream);
  * as in jenga_step; counters add the steps actually taken.                                                */
 int jenga_simulate_until_rest(jenga_world *w, int max_steps, float ek_rest, void *cuda_stream);
 
+/* Support-polygon margin of every env (Eq. 17, §8.1): the convex hull of the (x, y) of the 8 corners of
+ * every active body resting on the ground (world-AABB bottom <= aabb_margin), the mass-weighted COM_xy of the active
+ * dynamic bodies, and the minimum signed distance from COM_xy to the hull's edges (positive inside).
+ * out: DEVICE [E][4] fp32, 16-byte aligned: margin [m], COM_x, COM_y, number of hull vertices.  Nothing on the ground:
+ * margin = -1e30, 0 vertices; a single point or a segment: minus the distance to it.                    */
+int jenga_support_margin(jenga_world *w, float *out, void *cuda_stream);
+
+/* ziglar_block_analysis() (Table 1, §5.4; Eq. 8-9): class of the move "push body
+ * block[env] along axis[env]" of every env.  axis 0 = along the block's length (the paper's Y axis),
+ * 1 = across it (the paper's X axis); the block's slot follows the tower layout body id = 3 level + slot,
+ * slot 1 = centre block.  block, axis: DEVICE int32 [E].  out: DEVICE [E][4] fp32, 16-byte aligned: class (0 center_xaxis,
+ * 1 side_yaxis, 2 side_xaxis; -1 for an invalid body id), F_min = k mu_s m g [N], torque flag, k (3 or 4).       */
+int jenga_ziglar_block_analysis(jenga_world *w, const int32_t *block, const int32_t *axis, float *out, void *cuda_stream);
+
 /* jenga_step with HOST state buffers (the end-to-end call): enqueues, on `cuda_stream`, a host->device copy
  * of h_state_in ([E][13][S] fp32, same layout as bufs.state; pinned memory recommended, pageable works but
  * serialises) into bufs.state, the fused step, and a device->host copy of bufs.state into h_state_out.

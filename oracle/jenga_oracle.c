@@ -767,6 +767,87 @@ int32_t orc_collapse_test(int32_t B, const double *x, const double *q, const dou
   return dxm > 0.5 * length && ek > 5e-5 && thm > 30.0 * 3.14159265358979323846 / 180.0;
 }
 
+/* ------------------------------------------------------------------ NEXT-4: support polygon, Ziglar move classes */
+/* Eq. 17 (§8.1): support polygon = convex hull of the (x, y) of all 8 corners of every body that rests
+ * on the ground, i.e. whose world-AABB bottom z_b - e'_b,z <= eps (e' = |R| e as in Eq. 10, eps = the AABB margin);
+ * COM_xy = mass-weighted mean over the active dynamic bodies; margin d = minimum signed distance from COM_xy to the
+ * edges of the polygon (positive inside).  Returns d; *n_hull = number of hull vertices (0: nothing on the ground,
+ * d = -1e30; 1 or 2: degenerate support, d = -(distance to the point / segment)).
+ * The hull is Andrew's monotone chain (textbook): sort by (x, y), lower then upper chain, strictly convex turns. */
+static int cmp_xy(const void *a, const void *b) {
+  const double *p = (const double *)a, *q = (const double *)b;
+  if (p[0] != q[0]) return p[0] < q[0] ? -1 : 1;
+  if (p[1] != q[1]) return p[1] < q[1] ? -1 : 1;
+  return 0;
+}
+static double cross2(const double *o, const double *a, const double *b) {
+  return (a[0]-o[0])*(b[1]-o[1]) - (a[1]-o[1])*(b[0]-o[0]);
+}
+double orc_support_margin(int32_t B, const double *x, const double *q, const double *he, const double *inv_m,
+                          const int32_t *active, double eps, double *com_xy, int32_t *n_hull) {
+  double *pts = (double *)malloc(sizeof(double) * 2 * 8 * (size_t)(B > 0 ? B : 1));
+  int n = 0; double msum = 0.0, cx = 0.0, cy = 0.0;
+  for (int b = 0; b < B; ++b) {
+    if (!active[b]) continue;
+    double R[9]; orc_quat_to_R(q + 4*b, R);
+    if (inv_m[b] > 0.0) { double m = 1.0 / inv_m[b]; msum += m; cx += m * x[3*b]; cy += m * x[3*b+1]; }
+    double ez = fabs(R[6])*he[3*b] + fabs(R[7])*he[3*b+1] + fabs(R[8])*he[3*b+2];
+    if (x[3*b+2] - ez > eps) continue;
+    for (int id = 0; id < 8; ++id) {
+      double s[3] = { (id & 1) ? he[3*b] : -he[3*b], (id & 2) ? he[3*b+1] : -he[3*b+1], (id & 4) ? he[3*b+2] : -he[3*b+2] };
+      pts[2*n]   = x[3*b]   + R[0]*s[0] + R[1]*s[1] + R[2]*s[2];
+      pts[2*n+1] = x[3*b+1] + R[3]*s[0] + R[4]*s[1] + R[5]*s[2];
+      ++n;
+    }
+  }
+  if (msum > 0.0) { cx /= msum; cy /= msum; }
+  if (com_xy) { com_xy[0] = cx; com_xy[1] = cy; }
+  if (n == 0) { if (n_hull) *n_hull = 0; free(pts); return -1e30; }
+  qsort(pts, (size_t)n, 2 * sizeof(double), cmp_xy);
+  double *h = (double *)malloc(sizeof(double) * 2 * (size_t)(2 * n + 2));
+  int k = 0;
+  for (int i = 0; i < n; ++i) {                                  /* lower chain */
+    while (k >= 2 && cross2(h + 2*(k-2), h + 2*(k-1), pts + 2*i) <= 0.0) --k;
+    h[2*k] = pts[2*i]; h[2*k+1] = pts[2*i+1]; ++k;
+  }
+  for (int i = n - 2, t = k + 1; i >= 0; --i) {                  /* upper chain */
+    while (k >= t && cross2(h + 2*(k-2), h + 2*(k-1), pts + 2*i) <= 0.0) --k;
+    h[2*k] = pts[2*i]; h[2*k+1] = pts[2*i+1]; ++k;
+  }
+  int nh = k > 1 ? k - 1 : k;                                    /* the last point repeats the first */
+  double c[2] = { cx, cy }, d = 1e300;
+  if (nh >= 3) {
+    for (int i = 0; i < nh; ++i) {                               /* counter-clockwise: inside is to the left of every edge */
+      const double *a = h + 2*i, *b2 = h + 2*((i + 1) % nh);
+      double ex = b2[0]-a[0], ey = b2[1]-a[1], len = sqrt(ex*ex + ey*ey);
+      double sd = cross2(a, b2, c) / len;
+      if (sd < d) d = sd;
+    }
+  } else if (nh == 2) {
+    double ex = h[2]-h[0], ey = h[3]-h[1], l2 = ex*ex + ey*ey;
+    double t = ((cx-h[0])*ex + (cy-h[1])*ey) / l2; if (t < 0) t = 0; if (t > 1) t = 1;
+    double px = h[0] + t*ex - cx, py = h[1] + t*ey - cy;
+    d = -sqrt(px*px + py*py);
+  } else {
+    d = -sqrt((cx-h[0])*(cx-h[0]) + (cy-h[1])*(cy-h[1]));
+  }
+  if (n_hull) *n_hull = nh;
+  free(pts); free(h);
+  return d;
+}
+
+/* Table 1 (§5.4): the move classes of ziglar_block_analysis().  slot: 1 = centre block of its level,
+ * 0 / 2 = side blocks; axis: 0 = along the block's length (the paper's Y), 1 = across it (the paper's X,
+ * PAPER.md:216).  Class 0 center_xaxis (k = 3, no torque; the centre block has one row in the table, whatever the axis),
+ * 1 side_yaxis (k = 3, no torque), 2 side_xaxis (k = 4, torque on the upper layer).  F_min = k mu_s m g (Eq. 8-9). */
+int32_t orc_ziglar_block_analysis(int32_t slot, int32_t axis, double mu_s, double m, double g, double *f_min, int32_t *torque) {
+  int32_t cls = slot == 1 ? 0 : (axis == 0 ? 1 : 2);
+  double k = cls == 2 ? 4.0 : 3.0;
+  if (f_min) *f_min = orc_ziglar_force(k, mu_s, m, g);
+  if (torque) *torque = cls == 2;
+  return cls;
+}
+
 /* ------------------------------------------------------------------ batch rollout */
 /* E envs, arrays [E][...] contiguous; OpenMP over envs only (each env is sequential).
  * f_ext may be NULL; cache arrays are caller-owned and persist between calls:

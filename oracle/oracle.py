@@ -74,6 +74,8 @@ def lib():
         _lib.orc_step_env.restype = C.c_uint32
         _lib.orc_collapse_test.restype = C.c_int32
         _lib.orc_max_threads.restype = C.c_int32
+        _lib.orc_support_margin.restype = C.c_double
+        _lib.orc_ziglar_block_analysis.restype = C.c_int32
     return _lib
 
 
@@ -339,6 +341,22 @@ def collapse_test(bod: Bodies, x0, q0, e=0, length=0.075):
     r = lib().orc_collapse_test(C.c_int32(bod.B), dp(bod.x[e]), dp(bod.q[e]), dp(bod.v[e]), dp(bod.w[e]), dp(x0), dp(q0),
                                 dp(bod.inv_m[e]), dp(bod.inv_I[e]), ip(bod.active[e]), C.c_double(length), dp(out))
     return bool(r), out
+
+
+def support_margin(bod: Bodies, e=0, eps=0.002):
+    """Eq. 17: (margin d, COM_xy, number of hull vertices) of env e."""
+    com = np.zeros(2); nh = C.c_int32(0)
+    d = lib().orc_support_margin(C.c_int32(bod.B), dp(bod.x[e]), dp(bod.q[e]), dp(bod.he[e]), dp(bod.inv_m[e]), ip(bod.active[e]),
+                                 C.c_double(eps), dp(com), C.byref(nh))
+    return d, com, nh.value
+
+
+def ziglar_block_analysis(slot, axis, mu_s, m, g=9.81):
+    """Table 1: (class 0 center_xaxis / 1 side_yaxis / 2 side_xaxis, F_min [N], torque flag)."""
+    f = C.c_double(0); t = C.c_int32(0)
+    c = lib().orc_ziglar_block_analysis(C.c_int32(slot), C.c_int32(axis), C.c_double(mu_s), C.c_double(m), C.c_double(g),
+                                        C.byref(f), C.byref(t))
+    return c, f.value, bool(t.value)
 
 
 def n_threads():

@@ -69,6 +69,8 @@ def lib():
         L.jenga_smem_bytes.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_smem_bytes.restype = C.c_size_t
         L.jenga_block_threads.argtypes = [C.POINTER(WorldDesc)]
+        L.jenga_support_margin.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.jenga_ziglar_block_analysis.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.jenga_profile_enable.argtypes = [C.c_void_p, C.c_int]
         L.jenga_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.jenga_scratch_bytes.argtypes = [C.POINTER(WorldDesc)]
@@ -80,7 +82,7 @@ def lib():
         L.jenga_strerror.restype = C.c_char_p
         for f in ("jenga_world_create", "jenga_world_destroy", "jenga_broadphase", "jenga_narrowphase", "jenga_pgs_solve",
                   "jenga_step", "jenga_step_host", "jenga_simulate_until_rest", "jenga_set_f_ext", "jenga_block_threads",
-                  "jenga_profile_enable", "jenga_profile_read"):
+                  "jenga_profile_enable", "jenga_profile_read", "jenga_support_margin", "jenga_ziglar_block_analysis"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -220,6 +222,22 @@ class World:
             self.f_ext = torch.as_tensor(f_ext, dtype=torch.float32).contiguous().to(self.dev)
             assert self.f_ext.shape == (self.wp.n_envs, 6, self.wp.body_stride)
             _check(lib().jenga_set_f_ext(self.handle, C.c_void_p(self.f_ext.data_ptr())), "jenga_set_f_ext")
+
+    def jenga_support_margin(self):
+        """Eq. 17 per env: tensor [E][4] = margin, COM_x, COM_y, hull vertices (device)."""
+        out = torch.empty((self.wp.n_envs, 4), dtype=torch.float32, device=self.dev)
+        _check(lib().jenga_support_margin(self.handle, C.c_void_p(out.data_ptr()), self._stream()), "jenga_support_margin")
+        return out
+
+    def jenga_ziglar_block_analysis(self, block, axis):
+        """Table 1 per env: block, axis int arrays [E]; tensor [E][4] = class, F_min [N], torque flag, k (device)."""
+        tb = torch.as_tensor(block, dtype=torch.int32).contiguous().to(self.dev)
+        ta = torch.as_tensor(axis, dtype=torch.int32).contiguous().to(self.dev)
+        assert tb.shape == (self.wp.n_envs,) and ta.shape == (self.wp.n_envs,)
+        out = torch.empty((self.wp.n_envs, 4), dtype=torch.float32, device=self.dev)
+        _check(lib().jenga_ziglar_block_analysis(self.handle, C.c_void_p(tb.data_ptr()), C.c_void_p(ta.data_ptr()),
+                                                 C.c_void_p(out.data_ptr()), self._stream()), "jenga_ziglar_block_analysis")
+        return out
 
     def jenga_profile_enable(self, on: bool = True):
         _check(lib().jenga_profile_enable(self.handle, int(on)), "jenga_profile_enable")

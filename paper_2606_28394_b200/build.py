@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libjenga.so")
 SOURCES = ["jenga.cu", "peaks.cu"]
-DEPS = ["jenga.cu", "peaks.cu", "ksolve.cuh", "kcollide.cuh", "layout.cuh", "collide.cuh", os.path.join("..", "..", "include", "jenga.h")]
+DEPS = ["jenga.cu", "peaks.cu", "ksolve.cuh", "kcollide.cuh", "layout.cuh", "collide.cuh", "analysis.cuh", os.path.join("..", "..", "include", "jenga.h")]
 
 
 def _nvcc() -> str:

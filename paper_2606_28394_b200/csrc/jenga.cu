@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "ksolve.cuh"
+#include "analysis.cuh"
 
 namespace jenga {
 
@@ -338,4 +339,21 @@ extern "C" int jenga_step_host(jenga_world* w, const float* h_in, float* h_out, 
     if (e != cudaSuccess) return cuda_fail(e, "jenga_step_host D2H");
   }
   return JENGA_OK;
+}
+
+extern "C" int jenga_support_margin(jenga_world* w, float* out, void* stream) {
+  if (!w || !aligned16(out)) return JENGA_E_ARG;
+  const size_t smem = (size_t)8 * w->P.S * sizeof(float2);
+  if (smem > 48 * 1024) {
+    const cudaError_t e = cudaFuncSetAttribute((const void*)jenga::k_support, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_support)");
+  }
+  jenga::k_support<<<w->P.E, 32, smem, (cudaStream_t)stream>>>(w->P, reinterpret_cast<float4*>(out));
+  return launched("k_support");
+}
+
+extern "C" int jenga_ziglar_block_analysis(jenga_world* w, const int32_t* block, const int32_t* axis, float* out, void* stream) {
+  if (!w || !block || !axis || !aligned16(out)) return JENGA_E_ARG;
+  jenga::k_ziglar<<<(w->P.E + 127) / 128, 128, 0, (cudaStream_t)stream>>>(w->P, block, axis, reinterpret_cast<float4*>(out));
+  return launched("k_ziglar");
 }

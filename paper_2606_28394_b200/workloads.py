@@ -121,7 +121,7 @@ def set_body(state, props, e, b, pos, quat, half, inv_m, inv_I, vel=(0, 0, 0), o
     props[e, 7, b] = active
 
 
-def tower_nominal(levels: int):
+def tower_nominal(levels: int, width: float = BLOCK_W, height: float = BLOCK_H, g_lat: float = G_LAT):
     """Nominal (unjittered) block centres and yaw of an L-level tower.
     body id = 3*level + slot; even levels have the length along world x."""
     n = 3 * levels
@@ -132,8 +132,8 @@ def tower_nominal(levels: int):
         ybody = np.array([-math.sin(psi), math.cos(psi), 0.0])
         for s in range(3):
             b = 3 * lv + s
-            pos[b] = (s - 1) * (BLOCK_W + G_LAT) * ybody
-            pos[b, 2] = BLOCK_H / 2 - DELTA0 + lv * (BLOCK_H - DELTA0)
+            pos[b] = (s - 1) * (width + g_lat) * ybody
+            pos[b, 2] = height / 2 - DELTA0 + lv * (height - DELTA0)
             yaw[b] = psi
     return pos, yaw
 
@@ -144,6 +144,12 @@ _TOWER_CFG = {
     2: dict(E=450, levels=18, iters=20, steps=480, max_rem=12, rem_levels=15, push=(2.0, 5.0), mu="block150"),
     4: dict(E=4096, levels=30, iters=50, steps=480, max_rem=20, rem_levels=27, push=None, mu="draw"),
     5: dict(E=65536, levels=18, iters=20, steps=480, max_rem=12, rem_levels=15, push=(2.5, 4.5), mu="roundrobin"),
+    # cfg6: the paper's own parameter set, App. A Table 6: 81 x 26 x 18 mm blocks of
+    # 19.6 g, e = 0.10, three substeps, 14 PGS iterations; 450 episodes = 150 per friction level, the
+    # removal / push recipe of cfg2.  Lateral play 1.5 mm (81 mm vs 3 x 26 mm); the jitter is halved
+    # (+-0.25 mm, +-0.5 deg) so that neighbours cannot interpenetrate at t = 0 with that play.
+    6: dict(E=450, levels=18, iters=14, steps=480, max_rem=12, rem_levels=15, push=(2.0, 5.0), mu="block150",
+            size=(0.081, 0.026, 0.018), mass=0.0196, g_lat=0.0015, jitter_mm=0.25, jitter_deg=0.5, restitution=0.10, n_substeps=3),
 }
 MU_LEVELS = (0.25, 0.40, 0.60)
 SETTLE_STEPS = 60
@@ -158,9 +164,12 @@ def make_tower(cfg: int, n_envs: Optional[int] = None, env_offset: int = 0, jitt
     levels = c["levels"]
     B = 3 * levels
     state, props, S = empty_tiles(E, B)
-    nom_pos, nom_yaw = tower_nominal(levels)
-    inv_m, inv_I = box_mass_props(BLOCK_L, BLOCK_W, BLOCK_H, BLOCK_MASS)
-    half = (BLOCK_L / 2, BLOCK_W / 2, BLOCK_H / 2)
+    bl, bw, bh = c.get("size", (BLOCK_L, BLOCK_W, BLOCK_H))
+    mass = c.get("mass", BLOCK_MASS)
+    jit_pos, jit_yaw = 1.0e-3 * c.get("jitter_mm", 0.5), math.radians(c.get("jitter_deg", 1.0))
+    nom_pos, nom_yaw = tower_nominal(levels, bw, bh, c.get("g_lat", G_LAT))
+    inv_m, inv_I = box_mass_props(bl, bw, bh, mass)
+    half = (bl / 2, bw / 2, bh / 2)
     mu = np.zeros(E)
     fext = np.zeros((E, FEXT_ROWS, S)) if c["push"] else None
     push_body = np.full(E, -1, dtype=np.int32)
@@ -174,9 +183,9 @@ def make_tower(cfg: int, n_envs: Optional[int] = None, env_offset: int = 0, jitt
         jit = rng.uniform(-1.0, 1.0, size=(B, 3))
         if not jitter:
             jit[:] = 0.0
-        px = nom_pos[:, 0] + 0.5e-3 * jit[:, 0]
-        py = nom_pos[:, 1] + 0.5e-3 * jit[:, 1]
-        yaw = nom_yaw + math.radians(1.0) * jit[:, 2]
+        px = nom_pos[:, 0] + jit_pos * jit[:, 0]
+        py = nom_pos[:, 1] + jit_pos * jit[:, 1]
+        yaw = nom_yaw + jit_yaw * jit[:, 2]
         state[e, 0, :B] = px
         state[e, 1, :B] = py
         state[e, 2, :B] = nom_pos[:, 2]
@@ -219,10 +228,11 @@ def make_tower(cfg: int, n_envs: Optional[int] = None, env_offset: int = 0, jitt
             else:
                 d = across * float(slot - 1)
                 kthr = 4.0
-            F = k * mu[e] * BLOCK_MASS * GRAV
+            F = k * mu[e] * mass * GRAV
             fext[e, 0:3, b] = F * d
             push_body[e], push_k[e], push_kthr[e] = b, k, kthr
     params = WorldParams(n_envs=E, n_bodies=B, body_stride=S, pgs_iters=c["iters"],
+                         restitution=f32(c.get("restitution", 0.0)), n_substeps=c.get("n_substeps", 1),
                          max_pairs=768 if B <= 54 else 1536,       # 54 blocks: <= 570 candidates / 171 colliding pairs seen in
                          max_contacts=704 if B <= 54 else 1216)    # collapses (156 standing); 90 blocks: > 768 / 269 (264 standing)
     return Workload(
@@ -232,7 +242,7 @@ def make_tower(cfg: int, n_envs: Optional[int] = None, env_offset: int = 0, jitt
         push_fext=None if fext is None else fext.astype(np.float32),
         push_start=SETTLE_STEPS, push_end=SETTLE_STEPS + PUSH_STEPS,
         push_body=push_body, push_k=push_k, push_kthr=push_kthr,
-        meta=dict(cfg=cfg, levels=levels, n_removed=n_removed, env_offset=env_offset))
+        meta=dict(cfg=cfg, levels=levels, n_removed=n_removed, env_offset=env_offset, block_length=bl, block_mass=mass))
 
 
 def make_debris(n_envs: int = 4096, env_offset: int = 0, n_bodies: int = 54) -> Workload:
