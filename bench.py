@@ -120,11 +120,21 @@ def schedule(wl, n_steps: int, chunk: int):
 
 
 # ------------------------------------------------------------------------------- oracle arm (CPU)
-def oracle_sample(n_envs: int, env_offset: int = 0):
+# the oracle is timed on cfg1 and cfg2 in full, the first 256 envs of cfg3 / cfg4, the first 1024 of cfg5
+ORACLE_SUBSET = {1: 1, 2: 450, 3: 256, 4: 256, 5: 1024, 6: 450}
+CFG_ENVS = {1: 1, 2: 450, 3: 4096, 4: 4096, 5: 65536, 6: 450}      # BASELINE.json configs[0..4]; 6 = the paper's Table 6 set
+CFG_NAMES = {1: "cfg1 (BASELINE.json configs[0]): 1 env, 3-level tower, 10 PGS iters, 240 steps",
+             2: "cfg2 (BASELINE.json configs[1]): 450 envs of 18-level 54-block towers, removals + push k ~ U(2,5), 20 PGS iters, 480 steps",
+             3: "cfg3 (BASELINE.json configs[2]): 4096 envs of 54-block collapse debris, 20 PGS iters, 720 steps",
+             4: "cfg4 (BASELINE.json configs[3]): 4096 envs of 30-level 90-block towers, 0-20 removals, 50 PGS iters, 480 steps",
+             6: "cfg6 (SURVEY §8(f) NEXT-3): 450 envs of 54-block towers with the paper's Table 6 parameters (81x26x18 mm, 19.6 g, e = 0.10, 3 substeps, 14 PGS iters)"}
+
+
+def oracle_sample(n_envs: int, env_offset: int = 0, cfg: int = CFG):
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import oracle as O                                     # test infrastructure; allowed here (cpu_baseline / --impl reference)
     from paper_2606_28394_b200 import workloads as W
-    wl = W.make_config(CFG, n_envs=n_envs, env_offset=env_offset)
+    wl = W.make_config(cfg, n_envs=n_envs, env_offset=env_offset)
     P = O.make_params(wl.params)
     bod = O.unpack_tiles(wl.state, wl.props, wl.params.n_bodies)
     cache = O.Cache(bod.E, wl.params.max_contacts)
@@ -144,21 +154,23 @@ def oracle_advance(O, wl, P, bod, cache, fext, first: int, n: int):
     return time.perf_counter() - t0
 
 
-def cpu_baseline(budget_s: float = 15.0) -> dict:
-    """The oracle as it stands on the host cores, on a bounded sample of the same workload:
-    the whole 480-step rollout of the first n envs, n sized from a probe so that the run takes ~budget_s."""
+def cpu_baseline(budget_s: float = 15.0, cfg: int = CFG) -> dict:
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload: the whole rollout of the
+    first n envs of the config, n sized from a probe so that the run takes ~budget_s, at most SURVEY §8(d)'s subset."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import oracle as O
     cores = int(O.n_threads())
-    O, wl, P, bod, cache, fext = oracle_sample(2 * cores)
+    cap = ORACLE_SUBSET.get(cfg, 1024)
+    n_probe = min(2 * cores, cap)
+    O, wl, P, bod, cache, fext = oracle_sample(n_probe, cfg=cfg)
     oracle_advance(O, wl, P, bod, cache, fext, 0, 2)                      # page in, spin up the OpenMP team
     t_probe = oracle_advance(O, wl, P, bod, cache, fext, 2, 10)
-    rate = 2 * cores * 10 / t_probe                                        # env-steps/s
-    n_envs = int(min(4096, max(cores, round(budget_s * rate / wl.n_steps / cores) * cores)))
-    O, wl, P, bod, cache, fext = oracle_sample(n_envs)
+    rate = n_probe * 10 / t_probe                                          # env-steps/s
+    n_envs = int(min(cap, max(min(cores, cap), round(budget_s * rate / wl.n_steps / cores) * cores)))
+    O, wl, P, bod, cache, fext = oracle_sample(n_envs, cfg=cfg)
     t = oracle_advance(O, wl, P, bod, cache, fext, 0, wl.n_steps)
     return {"value": n_envs * wl.n_steps / t, "unit": METRIC, "cores": cores, "kind": "oracle",
-            "sample": f"first {n_envs} envs of cfg5, all {wl.n_steps} steps of the rollout (fp64, OpenMP over envs), {t:.1f} s"}
+            "sample": f"first {n_envs} envs of cfg{cfg}, all {wl.n_steps} steps of the rollout (fp64, OpenMP over envs), {t:.1f} s"}
 
 
 def run_reference(args) -> dict:
@@ -184,6 +196,24 @@ def run_reference(args) -> dict:
             "gpu_launches": 0}
 
 
+def run_dry(args):
+    """The multi-rank plumbing of the CUDA arm without a GPU: process group, env ranges, max-over-ranks timing."""
+    import torch.distributed as dist
+    from paper_2606_28394_b200 import shard
+    rank, world_size = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world_size > 1:
+        dist.init_process_group(args.backend)
+    lo, hi = shard.env_range(rank, world_size, args.envs)
+    ms = shard.max_over_ranks(100.0 + rank)                       # stands in for the device time of this rank
+    total = shard.sum_over_ranks(hi - lo)
+    if world_size > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return None
+    return {"dry_run": True, "n_gpus": world_size, "env_ranges_rank0": [lo, hi], "total_envs": total, "ms_max_over_ranks": ms,
+            "scaling": "weak"}
+
+
 # ------------------------------------------------------------------------------- CUDA arm
 def run_cuda(args) -> dict:
     import torch
@@ -197,10 +227,10 @@ def run_cuda(args) -> dict:
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world_size > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        dist.init_process_group(args.backend, device_id=dev)
     binding.lib()                                            # fail loudly if libjenga.so is missing
 
-    E = args.envs
+    E = args.envs or CFG_ENVS[args.cfg]
     wl = W.make_config(args.cfg, n_envs=E, env_offset=shard.env_range(rank, world_size, E)[0])
     if wl.push_fext is None:
         wl.push_fext = np.zeros((E, 6, wl.params.body_stride), np.float32); wl.push_start = wl.push_end = 0   # weak scaling: every rank has its own E envs
@@ -240,19 +270,26 @@ def run_cuda(args) -> dict:
 
     # ---- device-resident timing: inputs already in HBM, CUDA events on the launching stream
     launches = list(schedule(wl, K, args.chunk))
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(len(launches) + 1)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in launches]
+    # inputs far larger than L2 (cfg3-5) need no flush; the small configs rewrite a 256 MB buffer between the timed calls
+    scratch_per_env = world.scratch.numel() // E
+    small = E * (scratch_per_env + 13 * wp.body_stride * 4) < 2 * 126e6
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if small else None
     sampler = ClockSampler(local); sampler.start()
     barrier()
     world.jenga_profile_enable(True)                         # CUDA events around every kernel launch of the step (same stream)
-    ev[0].record(stream)
     for i, (s, n, active) in enumerate(launches):
         set_push(active)
+        if flush is not None:
+            flush.zero_()
+        ev[i][0].record(stream)
         world.jenga_step(n)
-        ev[i + 1].record(stream)
+        ev[i][1].record(stream)
     barrier()
     clocks = sampler.stop()
-    ms = ev[0].elapsed_time(ev[-1])
-    launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(len(launches))]
+    launch_ms = [a.elapsed_time(b) for a, b in ev]
+    ms = sum(launch_ms)                                      # the timed region = the jenga_step calls (back to back when there is no flush)
+    del flush
     prof = world.jenga_profile_read()
     world.jenga_profile_enable(False)
     cnt = world.counters_dict()
@@ -265,6 +302,7 @@ def run_cuda(args) -> dict:
     # envs on their own streams, so that one part's copies overlap the other part's kernel (what a user of the
     # library would do with a PCIe-bound call); the result of step s is the host input of step s+1.
     linfo = world.launch_info()
+    linfo_scratch = world.scratch.numel() // E
     world.destroy(); del world
     torch.cuda.empty_cache()
     n_split = max(1, min(args.e2e_split, E))
@@ -347,10 +385,12 @@ def run_cuda(args) -> dict:
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "cfg5 (BASELINE.json configs[4]): 18-level 54-block towers, mu_s {0.25,0.40,0.60} round-robin, 0-12 removals, "
-                               "Ziglar push sweep, dt=1/240, 20 PGS iters, rollout steps 0..K" if args.cfg == CFG else f"cfg{args.cfg} (manual run, not the bench workload)",
+                               "Ziglar push sweep, dt=1/240, 20 PGS iters, rollout steps 0..K" if args.cfg == CFG else CFG_NAMES[args.cfg] + " (not the headline workload)",
                    "envs_per_gpu": E, "n_bodies": wp.n_bodies, "pgs_iters": wp.pgs_iters, "steps_per_call": args.chunk, "kernels_per_substep": 2,
                    "parallelism": f"env-sharded x{world_size}, no data-path collective",
-                   "l2": "inputs larger than L2 (state 191 MB + warm-start cache 1.7 GB per step vs 126 MB L2)"},
+                   "l2": (f"inputs larger than L2: state {E * 13 * wp.body_stride * 4 / 1e6:.0f} MB + scratch {E * linfo_scratch / 1e6:.0f} MB + warm-start cache "
+                          f"{E * (wp.max_contacts // 4) * 104 / 1e6:.0f} MB per step vs 126 MB L2") if not small else
+                         "working set smaller than L2 (small config): an 8 x 32 MB buffer is rewritten between the timed launches"},
         "body_steps_per_s": cnt["body_steps"] * world_size / (ms * 1e-3),
         "contacts_per_s": cnt["contacts"] * world_size / (ms * 1e-3),
         "contact_iters_per_s": cnt["contact_iters"] * world_size / (ms * 1e-3),
@@ -367,10 +407,22 @@ def run_cuda(args) -> dict:
         "roofline": roofline,
     }
     if rank == 0 and world_size == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline()
+        out["cpu_baseline"] = cpu_baseline(cfg=args.cfg)
     if world_size > 1:
         dist.destroy_process_group()
     return out if rank == 0 else None
+
+
+def spawn_ranks(n: int, argv) -> int:
+    """`python bench.py --gpus N` without a launcher: re-exec this script under torch.distributed.run, one rank per GPU
+    (envs are independent episodes: each rank owns its own env range)."""
+    import socket
+    import subprocess
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    env = dict(os.environ, NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "WARN"))
+    return subprocess.call(cmd, env=env)
 
 
 def main():
@@ -379,7 +431,7 @@ def main():
     ap.add_argument("--steps", type=int, default=480, help="dt advances timed (default: the config's full 480-step rollout)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
-    ap.add_argument("--envs", type=int, default=65536, help="envs per GPU (cfg5: 65,536)")
+    ap.add_argument("--envs", type=int, default=0, help="envs per GPU (default: the config's own count; cfg5: 65,536)")
     ap.add_argument("--chunk", type=int, default=12, help="dt advances per jenga_step launch")
     ap.add_argument("--e2e-steps", type=int, default=96, help="steps of the end-to-end (host buffers) leg; 0 = K")
     ap.add_argument("--e2e-split", type=int, default=2, help="worlds (streams) the e2e leg serves the batch with")
@@ -388,7 +440,16 @@ def main():
     ap.add_argument("--tier", default="auto", choices=["auto", "smem", "tmem160", "tmem256", "tmem512"], help="where k_solve keeps the contact constants")
     ap.add_argument("--max-contacts", type=int, default=0, help="override the workload's contact capacity per env")
     ap.add_argument("--max-pairs", type=int, default=0, help="override the workload's candidate capacity per env")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="torch.distributed backend (gloo: the CPU test of the launch path)")
+    ap.add_argument("--dry-run", action="store_true", help="rendezvous, shard bookkeeping and the timing reduction only (no GPU work): the CPU test of --gpus N")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "cuda":
+        sys.exit(spawn_ranks(args.gpus, sys.argv[1:]))
+    if args.dry_run:
+        out = run_dry(args)
+        if out is not None:
+            print(json.dumps(out), flush=True)
+        return
     if args.impl == "reference":
         args.steps = min(args.steps, 60)                     # bounded: the oracle is slow by design
         out = run_reference(args)

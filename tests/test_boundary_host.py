@@ -136,3 +136,21 @@ def test_env_sharding_two_ranks_gloo(tmp_path):
              for r in range(2)]
     outs = [p.communicate(timeout=240)[0] for p in procs]
     assert all(p.returncode == 0 for p in procs), outs
+
+
+def test_bench_gpus_n_launches_its_own_ranks():
+    """`python bench.py --gpus 2` with no launcher re-execs under torch.distributed.run: the dry run
+    (gloo, no GPU work) shows two ranks, rank-owned env ranges and the max-over-ranks reduction."""
+    import json
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--envs", "64", "--steps", "4", "--dry-run", "--backend", "gloo"],
+                         capture_output=True, text=True, timeout=300, env={k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")})
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = [l for l in out.stdout.splitlines() if l.startswith("{")][-1]
+    d = json.loads(line)
+    assert d["n_gpus"] == 2 and d["total_envs"] == 128 and d["env_ranges_rank0"] == [0, 64] and d["ms_max_over_ranks"] == 101.0
+    # without --dry-run the two spawned ranks fail only where the GPU is needed
+    import torch
+    if not torch.cuda.is_available():
+        out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--envs", "64", "--steps", "4"],
+                             capture_output=True, text=True, timeout=300, env={k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")})
+        assert out.returncode != 0 and "bench.py needs a CUDA device" in out.stderr
