@@ -9,7 +9,8 @@ namespace jenga {
 // ---------------------------------------------------------------- shared-memory arena of one env
 struct CSm {
   SP<float> cb;                 // [S][kCb] collision body records
-  SP<float> ext;                // [3][S]   world AABB half extents
+  SP<float4> ext;               // [S]      world AABB half extents e'_x e'_y e'_z, flags (1 active | 2 dynamic)
+  SP<unsigned> hitw;            // [ceil(S/32)][32] broadphase hit words of the current block of 32 rows; ALIASES used
   SP<unsigned long long> used;  // [S]      colour masks per body
   SP<unsigned> cab;             // [pcA]    (a+1) | A dynamic << 11 | axis << 12 | b << 16 | B dynamic << 27
   SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending
@@ -31,7 +32,8 @@ enum { MiNph = 0, MiNcol = 1, MiNblk = 2 };
 
 __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc);
-  size_t w = (size_t)kCb * S + 3 * S + 2 * S;            // cb, ext, used
+  const int uh = 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
+  size_t w = (size_t)kCb * S + 4 * S + uh;               // cb, ext, used / hitw (aliased)
   w += pcA;                                              // cab
   w += mpA / 2 > 768 ? mpA / 2 : 768;                    // cand / poly (aliased)
   w += 4 * (size_t)(pcA / 2);                            // cpair, cprev, pos, wrank
@@ -45,9 +47,8 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc), phw = round_up(ph_max(nblk), 4);
   CSm s; int p = base;
   s.cb.off = p;     p += kCb * S;
-  s.ext.off = p;    p += 3 * S;
-  if (p & 1) ++p;
-  s.used.off = p;   p += 2 * S;
+  s.ext.off = p;    p += 4 * S;
+  s.hitw.off = p;   s.used.off = p;   p += 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
   s.cab.off = p;    p += pcA;
   s.cand.off = p;   s.poly.off = p;   p += mpA / 2 > 768 ? mpA / 2 : 768;
   s.cpair.off = p;  p += pcA / 2;
@@ -92,9 +93,11 @@ __device__ inline void load_predict(const CSm& s, const Params& P, int env, bool
     const float hx = pr[4 * S + b], hy = pr[5 * S + b], hz = pr[6 * S + b];
     const bool act = pr[7 * S + b] != 0.0f, dyn = act && im != 0.0f;
     float R[9]; quat_to_R(w, x, y, z, R);
+    float e3[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k)
-      s.ext[k * S + b] = fabsf(R[3 * k]) * hx + fabsf(R[3 * k + 1]) * hy + fabsf(R[3 * k + 2]) * hz;
+      e3[k] = fabsf(R[3 * k]) * hx + fabsf(R[3 * k + 1]) * hy + fabsf(R[3 * k + 2]) * hz;
+    s.ext[b] = make_float4(e3[0], e3[1], e3[2], (act ? 1.0f : 0.0f) + (dyn ? 2.0f : 0.0f));
     float I6[6];
     world_inv_inertia(R, dyn ? i0r : 0.0f, dyn ? i1r : 0.0f, dyn ? i2r : 0.0f, I6);
     cb4(s, b, 0) = make_float4(px, py, pz, dyn ? im : 0.0f);
@@ -127,6 +130,15 @@ __device__ inline void load_predict(const CSm& s, const Params& P, int env, bool
     st[10 * S + b] = wv.x + P.h * dw.x; st[11 * S + b] = wv.y + P.h * dw.y; st[12 * S + b] = wv.z + P.h * dw.z;
   }
   __syncwarp();
+}
+
+__device__ __forceinline__ int warp_excl_scan(int v, int* total) {
+  const int lane = lane_id();
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += t; }
+  *total = __shfl_sync(kFull, inc, 31);
+  return inc - v;
 }
 
 // fp64 re-evaluation of one Eq. 10 test, every operation rounded separately (no FMA), in the order
@@ -168,11 +180,14 @@ __device__ __noinline__ bool aabb_test_f64(const CSm& s, const Params& P, int i,
 #undef DA
 #undef DS
 
-// S2: ground tests, then all body pairs, in ascending canonical pair index; 32 tests per round, hits
-// compacted with __ballot_sync/__popc into s.cand (Eq. 10; ground test reading A6).
-// Returns the number of candidates kept (<= max_pairs); sets PAIR_OVERFLOW in *status.
+// S2: ground tests, then all body pairs, in ascending canonical pair index (Eq. 10; ground test
+// reading A6).  Body pairs: lane = row i of a block of 32 rows, its AABB in registers; the warp walks the columns j
+// together (every lane reads body j: a shared-memory broadcast) and each lane collects its row's hits in 32-bit words;
+// __popc / a warp scan of the row counts give every row its offset in the ascending list, which the lane then fills from
+// its words (__ffs).  Ground candidates: __ballot_sync / __popc.  Returns the number of candidates kept (<= max_pairs);
+// sets PAIR_OVERFLOW in *status.
 __device__ inline int broadphase(const CSm& s, const Params& P, unsigned* status) {
-  const int B = P.B, S = P.S, lane = lane_id();
+  const int B = P.B, lane = lane_id();
   const float eps = P.aabb_margin;
   const unsigned below = (1u << lane) - 1u;
   int n = 0;
@@ -180,7 +195,7 @@ __device__ inline int broadphase(const CSm& s, const Params& P, unsigned* status
     const int j = base + lane;
     bool hit = false;
     if (j < B && cb4(s, j, 5).w != 0.0f) {
-      const float sl = eps - (cb4(s, j, 0).z - s.ext[2 * S + j]);
+      const float sl = eps - (cb4(s, j, 0).z - s.ext[j].z);
       hit = sl >= 0.0f;
       if (fabsf(sl) < 1.0e-5f) hit = aabb_test_f64(s, P, -1, j);
     }
@@ -189,29 +204,43 @@ __device__ inline int broadphase(const CSm& s, const Params& P, unsigned* status
     if (hit && rank < P.max_pairs) s.cand[rank] = (unsigned short)j;
     n += __popc(bal);
   }
-  const int n_bp = B * (B - 1) / 2;
-  int i = 0, col = lane;                                   // lane's pair: row i, column col (j = i + 1 + col)
-  for (int base = 0; base < n_bp; base += 32) {
-    while (i < B - 1 && col >= B - 1 - i) { col -= B - 1 - i; ++i; }
-    bool hit = false;
-    const int j = i + 1 + col;
-    if (i < B - 1) {
-      const float4 xi = cb4(s, i, 0), xj = cb4(s, j, 0);
-      const bool consider = cb4(s, i, 5).z != 0.0f && cb4(s, j, 5).z != 0.0f && (xi.w != 0.0f || xj.w != 0.0f);
-      if (consider) {
-        const float s0 = (s.ext[i] + s.ext[j] + eps) - fabsf(xi.x - xj.x);
-        const float s1 = (s.ext[S + i] + s.ext[S + j] + eps) - fabsf(xi.y - xj.y);
-        const float s2 = (s.ext[2 * S + i] + s.ext[2 * S + j] + eps) - fabsf(xi.z - xj.z);
+  const int nW = (B + 31) >> 5;
+  for (int ib = 0; ib < nW; ++ib) {
+    const int i = 32 * ib + lane;
+    const bool row = i < B - 1;
+    float4 xi = make_float4(0, 0, 0, 0), ei = make_float4(0, 0, 0, 0);
+    if (i < B) { xi = cb4(s, i, 0); ei = s.ext[i]; }
+    const int fi = (int)ei.w;                               // 1 active | 2 dynamic
+    for (int jb = ib; jb < nW; ++jb) {
+      unsigned word = 0;
+      const int j0 = 32 * jb, j1 = min(B, j0 + 32);
+      for (int j = max(j0, 32 * ib + 1); j < j1; ++j) {     // uniform j: broadcast loads
+        const float4 xj = cb4(s, j, 0), ej = s.ext[j];
+        const int fj = (int)ej.w;
+        const float s0 = (ei.x + ej.x + eps) - fabsf(xi.x - xj.x);
+        const float s1 = (ei.y + ej.y + eps) - fabsf(xi.y - xj.y);
+        const float s2 = (ei.z + ej.z + eps) - fabsf(xi.z - xj.z);
         const float smin = fminf(s0, fminf(s1, s2));
-        hit = smin >= 0.0f;
-        if (fabsf(smin) < 1.0e-5f) hit = aabb_test_f64(s, P, i, j);
+        bool hit = smin >= 0.0f;
+        const bool consider = row && j > i && (fi & fj & 1) && ((fi | fj) & 2);
+        if (consider && fabsf(smin) < 1.0e-5f) hit = aabb_test_f64(s, P, i, j);
+        if (hit && consider) word |= 1u << (j - j0);
+      }
+      s.hitw[jb * 32 + lane] = word;
+    }
+    int cnt = 0;
+    for (int jb = ib; jb < nW; ++jb) cnt += __popc(s.hitw[jb * 32 + lane]);
+    int tot; int off = n + warp_excl_scan(cnt, &tot);
+    for (int jb = ib; jb < nW; ++jb) {
+      unsigned word = s.hitw[jb * 32 + lane];
+      const int rowbase = B + i * (2 * B - i - 1) / 2 - i - 1 + 32 * jb;      // pair index of (i, j) = rowbase + (j - 32 jb)
+      while (word) {
+        const int bit = __ffs(word) - 1; word &= word - 1;
+        if (off < P.max_pairs) s.cand[off] = (unsigned short)(rowbase + bit);
+        ++off;
       }
     }
-    const unsigned bal = __ballot_sync(kFull, hit);
-    const int rank = n + __popc(bal & below);
-    if (hit && rank < P.max_pairs) s.cand[rank] = (unsigned short)(B + i * (2 * B - i - 1) / 2 + col);
-    n += __popc(bal);
-    col += 32;
+    n += tot;
   }
   if (n > P.max_pairs) { *status |= JENGA_ST_PAIR_OVERFLOW; n = P.max_pairs; }
   __syncwarp();
@@ -718,15 +747,6 @@ __device__ inline int load_candidates(const CSm& s, const Params& P, int env) {
   for (int k = lane_id(); k < n_cand; k += 32) s.cand[k] = (unsigned short)P.pairs[(size_t)env * P.max_pairs + k];
   __syncwarp();
   return n_cand;
-}
-
-__device__ __forceinline__ int warp_excl_scan(int v, int* total) {
-  const int lane = lane_id();
-  int inc = v;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += t; }
-  *total = __shfl_sync(kFull, inc, 31);
-  return inc - v;
 }
 
 // Contact list in (pair, slot) order: the manifolds are recomputed from the (unchanged) poses in ascending
