@@ -105,7 +105,7 @@ extern "C" int jenga_block_threads(const jenga_world_desc* d) {
 
 extern "C" size_t jenga_scratch_bytes(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
-  return (size_t)d->n_envs * jenga::scratch_layout(d->max_contacts / 4).total * sizeof(float);
+  return ((size_t)d->n_envs * jenga::scratch_layout(d->max_contacts / 4).total + jenga::kScratchHead) * sizeof(float);
 }
 
 extern "C" const char* jenga_strerror(int code) {
@@ -197,7 +197,8 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.collapse_stats = latch ? b->collapse_stats : nullptr;
   P.rest_steps = b->rest_steps;
   P.collapse_dx = d->collapse_fd * d->collapse_length; P.collapse_ek = d->collapse_ek; P.collapse_theta = d->collapse_theta;
-  P.scratch = (float*)b->scratch; P.scratch_words = jenga::scratch_layout(P.pc).total;
+  P.work_counter = (int*)b->scratch;
+  P.scratch = (float*)b->scratch + jenga::kScratchHead; P.scratch_words = jenga::scratch_layout(P.pc).total;
   *out = w;
   return JENGA_OK;
 }

@@ -840,6 +840,7 @@ __device__ inline void setup_given(const CSm& s, const Params& P, int env, float
 __global__ void __launch_bounds__(128, 4) k_collide(const Params P, const int mode, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
   const int env = blockIdx.x * wpc + warp;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *P.work_counter = 0;      // k_solve of this substep starts its env queue at 0
   if (env >= P.E) return;
   const Scratch L = scratch_layout(P.pc);
   float* scr = P.scratch + (size_t)env * P.scratch_words;

@@ -484,10 +484,15 @@ __global__ void __launch_bounds__(TM ? 384 : 32, 1) k_solve(const Params P, cons
   SSm s = begin_solve<TM>(P, env0);
   const int lane = lane_id();
   const Scratch L = scratch_layout(P.pc);
-  const int stride = gridDim.x * (blockDim.x >> 5);
-  // persistent: warp w of CTA c takes envs c * wpc + w, + stride, ... (TMEM is allocated once per CTA; the warps of a CTA
-  // never wait for one another between envs)
-  for (int env = env0; env < P.E; env += stride) {
+  // persistent: every warp takes the next env of a global queue (an atomic counter that k_collide reset): envs differ in
+  // cost by the number of colliding pairs, so a static split would leave warps idle at the end.  TMEM is allocated once
+  // per CTA; the warps of a CTA never wait for one another between envs.
+  (void)env0;
+  for (;;) {
+    int env = 0;
+    if (lane == 0) env = atomicAdd(P.work_counter, 1);
+    env = __shfl_sync(kFull, env, 0);
+    if (env >= P.E) break;
     float* scr = P.scratch + (size_t)env * P.scratch_words;
     int* meta = reinterpret_cast<int*>(scr + L.meta);
     if ((flags & SolveRest) && meta[MetaResting]) continue;

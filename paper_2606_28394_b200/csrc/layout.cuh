@@ -30,6 +30,7 @@ constexpr int kHdrF4 = 3;      // float4 per pair header: (ab, meta, rank, 1/|t1
 constexpr int kCsF4 = 12;      // float4 of contact constants per pair: 36 read-only words + 12 impulses
 constexpr int kBlkWords = kCsF4 * 4 * 32;   // words of one 32-position constant block in the scratch / shared tier
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kScratchHead = 64;             // global words in front of the per-env scratch: [0] = k_solve's work counter
 constexpr int kMagic = 0x4a454e47;          // "JENG": scratch meta stamp of a valid colouring
 
 enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaWords = 16 };
@@ -52,7 +53,8 @@ struct Params {
   unsigned* status; unsigned long long* counters;
   const float* ref_pose; int* collapsed; float* collapse_stats; int* rest_steps;
   float collapse_dx, collapse_ek, collapse_theta;           // f_d * l, eps_k, theta_th
-  float* scratch; long long scratch_words;                  // per env
+  int* work_counter;                                        // next env of the running k_solve (reset by every k_collide)
+  float* scratch; long long scratch_words;                  // per env (the first kScratchHead words of the buffer are global)
 };
 
 __host__ __device__ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
