@@ -127,13 +127,16 @@ static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; 
 
 /* cudaFuncAttributeMaxDynamicSharedMemorySize is per kernel and process-wide: it is only ever raised (running maximum
  * per device), immediately before the launch that needs it, so worlds of different sizes can be used in any order.   */
-enum { KnCollide = 0, KnSolveTm, KnSolveSm, KnCount };
+enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnSolveTm, KnSolveSm, KnCount };
 static std::mutex g_attr_mutex;
 static size_t g_attr_max[16][KnCount];
 
 static const void* kernel_ptr(int kn) {
   switch (kn) {
-    case KnCollide: return (const void*)jenga::k_collide;
+    case KnCollide: return (const void*)jenga::k_collide<jenga::ModeStep>;
+    case KnCollideBroad: return (const void*)jenga::k_collide<jenga::ModeBroad>;
+    case KnCollideNarrow: return (const void*)jenga::k_collide<jenga::ModeNarrow>;
+    case KnCollideGiven: return (const void*)jenga::k_collide<jenga::ModeGiven>;
     case KnSolveTm: return (const void*)jenga::k_solve<true>;
     default: return (const void*)jenga::k_solve<false>;
   }
@@ -258,10 +261,15 @@ extern "C" int jenga_set_f_ext(jenga_world* w, const float* f_ext) {
 }
 
 static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_t st) {
-  const cudaError_t e = ensure_smem(w->desc.device, KnCollide, w->smem_collide);
+  const cudaError_t e = ensure_smem(w->desc.device, KnCollide + mode, w->smem_collide);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_collide)");
-  const int wpc = w->wpc_collide;
-  jenga::k_collide<<<(w->P.E + wpc - 1) / wpc, 32 * wpc, w->smem_collide, st>>>(w->P, mode, honour_rest);
+  const int wpc = w->wpc_collide, grid = (w->P.E + wpc - 1) / wpc, thr = 32 * wpc;
+  switch (mode) {
+    case jenga::ModeStep: jenga::k_collide<jenga::ModeStep><<<grid, thr, w->smem_collide, st>>>(w->P, honour_rest); break;
+    case jenga::ModeBroad: jenga::k_collide<jenga::ModeBroad><<<grid, thr, w->smem_collide, st>>>(w->P, honour_rest); break;
+    case jenga::ModeNarrow: jenga::k_collide<jenga::ModeNarrow><<<grid, thr, w->smem_collide, st>>>(w->P, honour_rest); break;
+    default: jenga::k_collide<jenga::ModeGiven><<<grid, thr, w->smem_collide, st>>>(w->P, honour_rest); break;
+  }
   return launched("k_collide");
 }
 

@@ -837,44 +837,55 @@ __device__ inline void setup_given(const CSm& s, const Params& P, int env, float
 // mode: ModeStep (fused substep, first half), ModeBroad (jenga_broadphase), ModeNarrow (jenga_narrowphase),
 // ModeGiven (first half of jenga_pgs_solve).  honour_rest: envs whose scratch says "at rest" are skipped
 // (jenga_simulate_until_rest).
-__global__ void __launch_bounds__(128, 4) k_collide(const Params P, const int mode, const int honour_rest) {
+template <int mode>
+__global__ void __launch_bounds__(128, 4) k_collide(const Params P, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
   const int env = blockIdx.x * wpc + warp;
   if (blockIdx.x == 0 && threadIdx.x == 0) *P.work_counter = 0;      // k_solve of this substep starts its env queue at 0
-  if (env >= P.E) return;
   const Scratch L = scratch_layout(P.pc);
-  float* scr = P.scratch + (size_t)env * P.scratch_words;
+  float* scr = P.scratch + (size_t)(env < P.E ? env : 0) * P.scratch_words;
   int* meta = reinterpret_cast<int*>(scr + L.meta);
-  if (honour_rest && meta[MetaResting]) return;
+  // The warps of a CTA meet at a CTA barrier between the stages (ModeStep): an SM then executes as many code regions at a
+  // time as it has CTAs, not as it has warps, which keeps the hot instructions in the 32 KB instruction cache.
+  const bool valid = env < P.E && !(honour_rest && meta[MetaResting]);
+#define STAGE_SYNC() do { if (mode == ModeStep) __syncthreads(); } while (0)
+  if (mode != ModeStep && !valid) return;
   const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc));
   unsigned st = 0;
-  load_predict(s, P, env, mode == ModeStep);
-  int n_cand = 0, n_coll = 0;
-  if (mode == ModeStep || mode == ModeBroad) {
-    n_cand = broadphase(s, P, &st);
-    if (mode == ModeBroad || P.materialise) write_pairs(s, P, env, n_cand);
-  } else if (mode == ModeNarrow) {
-    n_cand = load_candidates(s, P, env);
+  int n_cand = 0, n_coll = 0, nprev = 0;
+  if (valid) {
+    load_predict(s, P, env, mode == ModeStep);
+    if (mode == ModeStep || mode == ModeBroad) {
+      n_cand = broadphase(s, P, &st);
+      if (mode == ModeBroad || P.materialise) write_pairs(s, P, env, n_cand);
+    } else if (mode == ModeNarrow) {
+      n_cand = load_candidates(s, P, env);
+    }
   }
-  if (mode == ModeStep || mode == ModeNarrow) {
+  STAGE_SYNC();
+  if (valid && (mode == ModeStep || mode == ModeNarrow)) {
     n_coll = find_colliding(s, P, n_cand, &st);
     if (mode == ModeNarrow || P.materialise) write_contacts(s, P, env, scr, L, n_cand, n_coll);
   }
-  if (mode == ModeStep || mode == ModeGiven) {
-    const int nprev = load_prev_keys(s, P, env);
-    int n_cont = 0;
+  if (valid && (mode == ModeStep || mode == ModeGiven)) {
+    nprev = load_prev_keys(s, P, env);
     if (mode == ModeGiven) {
-      n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
+      const int n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
       n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
       unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
       for (int r = lane; r < n_coll; r += 32) gcoff[r] = s.wrank[r];       // the colouring reuses s.wrank
       if (lane == 0) meta[MetaNcont] = n_cont;
       __syncwarp();
+      colour_pairs(s, P, scr, L, n_coll, &st);
+      setup_given(s, P, env, scr, L, n_coll, n_cont, nprev);
+    } else {
+      colour_pairs(s, P, scr, L, n_coll, &st);
     }
-    colour_pairs(s, P, scr, L, n_coll, &st);
-    if (mode == ModeGiven) setup_given(s, P, env, scr, L, n_coll, n_cont, nprev);
-    else setup_pairs(s, P, env, scr, L, n_coll, nprev);
-    if (P.counters && mode == ModeStep && lane == 0) {
+  }
+  STAGE_SYNC();
+  if (valid && mode == ModeStep) {
+    setup_pairs(s, P, env, scr, L, n_coll, nprev);
+    if (P.counters && lane == 0) {
       const int ncol = s.misc[MiNcol];
       atomicAdd(P.counters + JENGA_CNT_CANDIDATES, (unsigned long long)n_cand);
       atomicAdd(P.counters + JENGA_CNT_COLLIDING, (unsigned long long)n_coll);
@@ -884,7 +895,8 @@ __global__ void __launch_bounds__(128, 4) k_collide(const Params P, const int mo
       atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
     }
   }
-  flush_status(P, env, st);
+#undef STAGE_SYNC
+  if (valid) flush_status(P, env, st);
 }
 
 }  // namespace jenga
