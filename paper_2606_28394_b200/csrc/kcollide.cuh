@@ -625,7 +625,23 @@ __device__ __forceinline__ Vec3 imul(const BodyK& B, Vec3 a) {      // Iw^-1 a
 // S4 for one colliding pair: header and constants of position k from the pair's manifold, written to the scratch.
 // Warm start (DESIGN §3 R-warm): a new contact inherits (jn,jt1,jt2) of the nearest not yet taken previous contact
 // point of the same pair within match_tol; slots ascending.  The previous pair list is s.cprev (ascending).
-__device__ inline void setup_slot(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int nprev,
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
+
+// Entry of pair index `pair` in the warm-start cache (ascending list s.cprev), or -1; its impulses and points are
+// prefetched into L2 (k_solve of the previous step wrote them a whole batch ago: they come from HBM) so that the loads of
+// setup_slot, issued after the manifold arithmetic, do not wait for DRAM.
+__device__ __forceinline__ int cache_lookup(const CSm& s, const Params& P, int env, int nprev, int pair) {
+  if (!P.warm_start || nprev <= 0) return -1;
+  int lo = 0, hi = nprev;
+  while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)s.cprev[mid] < pair) lo = mid + 1; else hi = mid; }
+  if (lo >= nprev || (int)s.cprev[lo] != pair) return -1;
+  prefetch_l2(P.cache_lam + ((size_t)env * P.pc + lo) * 12);
+  prefetch_l2(P.cache_pt + ((size_t)env * P.pc + lo) * 12);
+  prefetch_l2(P.cache_key + ((size_t)env * P.pc + lo) * 2);
+  return lo;
+}
+
+__device__ inline void setup_slot(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int lo,
                                   int k, int r, int a, int b, int pair, const Manifold& m) {
   BodyK A, Bb; load_bodyk(s, a, A); load_bodyk(s, b, Bb);
   const Vec3 n = m.n;
@@ -641,10 +657,8 @@ __device__ inline void setup_slot(const CSm& s, const Params& P, int env, float*
 #pragma unroll
   for (int c = 0; c < 4; ++c) if (c < m.np) { pt[c] = m.p[c]; dmax = fmaxf(dmax, m.d[c]); }
 
-  if (P.warm_start && nprev > 0) {
-    int lo = 0, hi = nprev;
-    while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)s.cprev[mid] < pair) lo = mid + 1; else hi = mid; }
-    if (lo < nprev && (int)s.cprev[lo] == pair) {
+  {
+    if (lo >= 0) {
       const int ocnt = P.cache_key[((size_t)env * P.pc + lo) * 2 + 1] & 0xff;
       const float4* ol4 = reinterpret_cast<const float4*>(P.cache_lam + ((size_t)env * P.pc + lo) * 12);
       const float4* op4 = reinterpret_cast<const float4*>(P.cache_pt + ((size_t)env * P.pc + lo) * 12);
@@ -725,10 +739,11 @@ __device__ inline int load_prev_keys(const CSm& s, const Params& P, int env) {
 __device__ inline void setup_pairs(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_coll, int nprev) {
   for (int r = lane_id(); r < n_coll; r += 32) {
     const unsigned w = s.cab[r];
-    const int a = ab_a(w), b = ab_b(w);
+    const int a = ab_a(w), b = ab_b(w), pair = s.cpair[r];
+    const int lo = cache_lookup(s, P, env, nprev, pair);
     Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
     pair_manifold(s, a, b, ab_axis(w), m);
-    setup_slot(s, P, env, scr, L, nprev, s.pos[r], r, a, b, s.cpair[r], m);
+    setup_slot(s, P, env, scr, L, lo, s.pos[r], r, a, b, pair, m);
   }
   __syncwarp();
 }
@@ -828,7 +843,7 @@ __device__ inline void setup_given(const CSm& s, const Params& P, int env, float
       m.p[c] = v3(0, 0, 0); m.d[c] = 0.0f;
       if (c < m.np) { const float4 a4 = in[2 * (c0 + c)], b4 = in[2 * (c0 + c) + 1]; m.p[c] = v3(b4.x, b4.y, b4.z); m.d[c] = a4.w; }
     }
-    setup_slot(s, P, env, scr, L, nprev, s.pos[r], r, ab_a(w), ab_b(w), s.cpair[r], m);
+    setup_slot(s, P, env, scr, L, cache_lookup(s, P, env, nprev, s.cpair[r]), s.pos[r], r, ab_a(w), ab_b(w), s.cpair[r], m);
   }
   __syncwarp();
 }
