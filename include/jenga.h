@@ -144,7 +144,7 @@ int jenga_narrowphase(jenga_world *w, void *cuda_stream);
  * (read only) when desc.warm_start = 1 and n_cache[env] > 0.  Eq. 13-15, Listing 1.                   */
 int jenga_pgs_solve(jenga_world *w, int iters, void *cuda_stream);
 
-/* n_steps advances of dt (each n_substeps substeps S1..S7 = two kernel launches: detection + setup, then solve +
+/* n_steps advances of dt (each n_substeps substeps S1..S7 = three kernel launches: detection, contact setup, solve +
  * integrate), all enqueued by this one call; state, cache, status and counters are updated in place.  */
 int jenga_step(jenga_world *w, int n_steps, void *cuda_stream);
 
@@ -197,8 +197,9 @@ const char *jenga_strerror(int code);
 
 /* Measurement aid (bench.py's roofline): while enabled, every launch of jenga_step / jenga_simulate_until_rest is
  * bracketed by CUDA events on the caller's stream.  jenga_profile_read synchronises on them and returns, for the launches
- * since the last enable / read, out[0] = summed device time of the detection + setup kernel [ms], out[1] = of the
- * solve + integrate kernel [ms], out[2] = out[3] = number of substeps.  `out` is a HOST array of 4 doubles.     */
+ * since the last enable / read, the summed device time [ms] of out[0] = the detection kernel (S1, S2, SAT, colouring),
+ * out[1] = the setup kernel (manifolds, effective masses), out[2] = the solve + integrate kernel; out[3] = number of
+ * substeps.  `out` is a HOST array of 4 doubles.                                                           */
 int jenga_profile_enable(jenga_world *w, int on);
 int jenga_profile_read(jenga_world *w, double *out);
 

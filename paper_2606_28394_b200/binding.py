@@ -245,7 +245,7 @@ class World:
     def jenga_profile_read(self) -> dict:
         out = (C.c_double * 4)()
         _check(lib().jenga_profile_read(self.handle, out), "jenga_profile_read")
-        return dict(collide_ms=out[0], solve_ms=out[1], substeps=int(out[2]))
+        return dict(detect_ms=out[0], setup_ms=out[1], collide_ms=out[0] + out[1], solve_ms=out[2], substeps=int(out[3]))
 
     def jenga_world_destroy(self):
         if self.handle:

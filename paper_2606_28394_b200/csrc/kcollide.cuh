@@ -1,6 +1,8 @@
-// kcollide.cuh -- first kernel of a substep, one env per warp: S1 predict, S2 broadphase, S3 narrowphase, S4 contact
-// setup (effective masses, warm-start lookup) and the canonical colouring; its products go to the scratch buffer
-// (layout.cuh) for k_solve.
+// kcollide.cuh -- the two collision kernels of a substep, one env per warp.  k_detect: S1 predict, S2 broadphase, S3 SAT
+// (which candidates collide), S4 canonical colouring + chunk packing.  k_setup: S3 manifolds, S4 contact setup (effective
+// masses, warm-start lookup).  Their products go to the scratch buffer (layout.cuh) for k_solve.  They are separate
+// kernels because each one's hot code then fits the 32 KB instruction cache (as one kernel: 70 KB, and `no_instruction`
+// was the top stall with 16 warps per SM at different places in it).
 #pragma once
 #include "layout.cuh"
 
@@ -14,8 +16,7 @@ struct CSm {
   SP<unsigned long long> used;  // [S]      colour masks per body
   SP<unsigned> cab;             // [pcA]    (a+1) | A dynamic << 11 | axis << 12 | b << 16 | B dynamic << 27
   SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending
-  SP<float> poly;               // [8][3][32] clip polygon of every lane (component-major: lane l <-> bank l); ALIASES cand,
-                                //            which is dead once the colliding-pair list exists
+  SP<float> poly;               // [8][3][32] clip polygon of every lane (component-major: lane l <-> bank l)
   SP<unsigned short> cpair;     // [pcA]    colliding pair indices, ascending
   SP<unsigned short> cprev;     // [pcA]    pair indices of the warm-start cache (previous substep), ascending
   SP<unsigned short> pos;       // [pcA]    position of pair r
@@ -30,38 +31,51 @@ struct CSm {
 };
 enum { MiNph = 0, MiNcol = 1, MiNblk = 2 };
 
-__host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc) {
+enum { ArenaDetect = 0, ArenaSetup = 1 };
+
+// k_detect: records, extents, masks / hit words, candidate list, colliding list, colouring products.
+// k_setup: records, colliding list (copied from the scratch), cache keys, contact offsets, per-lane clip polygons.
+__host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc, int arena) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc);
-  const int uh = 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
-  size_t w = (size_t)kCb * S + 4 * S + uh;               // cb, ext, used / hitw (aliased)
-  w += pcA;                                              // cab
-  w += mpA / 2 > 768 ? mpA / 2 : 768;                    // cand / poly (aliased)
-  w += 4 * (size_t)(pcA / 2);                            // cpair, cprev, pos, wrank
-  w += pcA / 4;                                          // colour
-  w += 2 * round_up(ph_max(nblk), 4);                    // ph, chc
-  w += 2 * kMaxColours + round_up(nblk, 4) + 8;          // ccount, cfirst, fill, misc
+  size_t w = (size_t)kCb * S + pcA;                        // cb, cab
+  w += 3 * (size_t)(pcA / 2);                              // cpair, pos, wrank
+  if (arena == ArenaDetect) {
+    const int uh = 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
+    w += 4 * S + uh + mpA / 2 + pcA / 4;                   // ext, used / hitw, cand, colour
+    w += 2 * round_up(ph_max(nblk), 4);                    // ph, chc
+    w += 2 * kMaxColours + round_up(nblk, 4) + 8;          // ccount, cfirst, fill, misc
+  } else {
+    w += pcA / 2 + 768;                                    // cprev, poly
+  }
   return round_up((int)w, 4);
 }
 
-__device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base) {
+__device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int arena) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc), phw = round_up(ph_max(nblk), 4);
   CSm s; int p = base;
   s.cb.off = p;     p += kCb * S;
-  s.ext.off = p;    p += 4 * S;
-  s.hitw.off = p;   s.used.off = p;   p += 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
   s.cab.off = p;    p += pcA;
-  s.cand.off = p;   s.poly.off = p;   p += mpA / 2 > 768 ? mpA / 2 : 768;
   s.cpair.off = p;  p += pcA / 2;
-  s.cprev.off = p;  p += pcA / 2;
   s.pos.off = p;    p += pcA / 2;
   s.wrank.off = p;  p += pcA / 2;
-  s.colour.off = p; p += pcA / 4;
-  s.ph.off = p;     p += phw;
-  s.chc.off = p;    p += phw;
-  s.ccount.off = p; p += kMaxColours;
-  s.cfirst.off = p; p += kMaxColours;
-  s.fill.off = p;   p += round_up(nblk, 4);
-  s.misc.off = p;
+  // the arrays of the other arena get offset 0 (never touched by this kernel)
+  s.ext.off = s.hitw.off = s.used.off = s.cand.off = s.colour.off = s.ph.off = s.chc.off = 0;
+  s.ccount.off = s.cfirst.off = s.fill.off = s.misc.off = s.cprev.off = s.poly.off = 0;
+  if (arena == ArenaDetect) {
+    s.ext.off = p;    p += 4 * S;
+    s.hitw.off = p;   s.used.off = p;   p += 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
+    s.cand.off = p;   p += mpA / 2;
+    s.colour.off = p; p += pcA / 4;
+    s.ph.off = p;     p += phw;
+    s.chc.off = p;    p += phw;
+    s.ccount.off = p; p += kMaxColours;
+    s.cfirst.off = p; p += kMaxColours;
+    s.fill.off = p;   p += round_up(nblk, 4);
+    s.misc.off = p;
+  } else {
+    s.cprev.off = p;  p += pcA / 2;
+    s.poly.off = p;
+  }
   return s;
 }
 
@@ -82,7 +96,7 @@ __device__ __forceinline__ Box load_box(const CSm& s, int b) {
 // state [13][S] and props [8][S] of one env are contiguous in HBM; lane b reads column b of every row (coalesced).
 // Eq. 1, I_world^-1 = R diag(I_body^-1) R^T, e'_k = sum_j |R_kj| e_j;
 // v += h (g + f/m), w += h Iw^-1 (tau [- w x Iw w]) (Eq. 5; reading A2): written back to `state`.
-__device__ inline void load_predict(const CSm& s, const Params& P, int env, bool predict) {
+__device__ inline void load_predict(const CSm& s, const Params& P, int env, bool predict, bool want_ext = true) {
   const int S = P.S;
   float* st = P.state + (size_t)env * kStateRows * S;
   const float* pr = P.props + (size_t)env * kPropRows * S;
@@ -97,7 +111,7 @@ __device__ inline void load_predict(const CSm& s, const Params& P, int env, bool
 #pragma unroll
     for (int k = 0; k < 3; ++k)
       e3[k] = fabsf(R[3 * k]) * hx + fabsf(R[3 * k + 1]) * hy + fabsf(R[3 * k + 2]) * hz;
-    s.ext[b] = make_float4(e3[0], e3[1], e3[2], (act ? 1.0f : 0.0f) + (dyn ? 2.0f : 0.0f));
+    if (want_ext) s.ext[b] = make_float4(e3[0], e3[1], e3[2], (act ? 1.0f : 0.0f) + (dyn ? 2.0f : 0.0f));
     float I6[6];
     world_inv_inertia(R, dyn ? i0r : 0.0f, dyn ? i1r : 0.0f, dyn ? i2r : 0.0f, I6);
     cb4(s, b, 0) = make_float4(px, py, pz, dyn ? im : 0.0f);
@@ -511,12 +525,13 @@ __device__ inline void colour_pairs(const CSm& s, const Params& P, float* scr, c
   int* meta = reinterpret_cast<int*>(scr + L.meta);
   unsigned short* gpos = reinterpret_cast<unsigned short*>(scr + L.pos);
   unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
+  unsigned* gcab = reinterpret_cast<unsigned*>(scr + L.cab);
+  for (int r = lane; r < n_coll; r += 32) gcab[r] = s.cab[r];             // bodies + SAT axis of every pair, for k_setup
   bool same = meta[MetaMagic] == kMagic && meta[MetaNcoll] == n_coll;
   if (same)
     for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
   same = __all_sync(kFull, same);
   if (same) {
-    for (int r = lane; r < n_coll; r += 32) s.pos[r] = gpos[r];
     if (lane == 0) { s.misc[MiNph] = meta[MetaNph]; s.misc[MiNcol] = meta[MetaNcol]; s.misc[MiNblk] = meta[MetaNblk]; }
     __syncwarp();
     return;
@@ -852,55 +867,53 @@ __device__ inline void setup_given(const CSm& s, const Params& P, int env, float
 // mode: ModeStep (fused substep, first half), ModeBroad (jenga_broadphase), ModeNarrow (jenga_narrowphase),
 // ModeGiven (first half of jenga_pgs_solve).  honour_rest: envs whose scratch says "at rest" are skipped
 // (jenga_simulate_until_rest).
+// The colliding-pair list of this env from the scratch (k_detect wrote it) into the arena of k_setup.
+__device__ inline int load_colliding(const CSm& s, const float* scr, const Scratch& L) {
+  const int n_coll = reinterpret_cast<const int*>(scr + L.meta)[MetaNcoll];
+  const unsigned* gcab = reinterpret_cast<const unsigned*>(scr + L.cab);
+  const unsigned short* gpos = reinterpret_cast<const unsigned short*>(scr + L.pos);
+  const unsigned short* gpair = reinterpret_cast<const unsigned short*>(scr + L.cpair);
+  for (int r = lane_id(); r < n_coll; r += 32) { s.cab[r] = gcab[r]; s.pos[r] = gpos[r]; s.cpair[r] = gpair[r]; }
+  __syncwarp();
+  return n_coll;
+}
+
+// ---------------------------------------------------------------- the kernels
+// mode: ModeStep (a substep of jenga_step), ModeBroad (jenga_broadphase: k_detect only), ModeNarrow (jenga_narrowphase),
+// ModeGiven (first half of jenga_pgs_solve: the caller's contact list instead of the narrowphase).  honour_rest: envs whose
+// scratch says "at rest" are skipped (jenga_simulate_until_rest).
 template <int mode>
-__global__ void __launch_bounds__(128, 4) k_collide(const Params P, const int honour_rest) {
+__global__ void __launch_bounds__(128, 4) k_detect(const Params P, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
   const int env = blockIdx.x * wpc + warp;
   if (blockIdx.x == 0 && threadIdx.x == 0) *P.work_counter = 0;      // k_solve of this substep starts its env queue at 0
+  if (env >= P.E) return;
   const Scratch L = scratch_layout(P.pc);
-  float* scr = P.scratch + (size_t)(env < P.E ? env : 0) * P.scratch_words;
+  float* scr = P.scratch + (size_t)env * P.scratch_words;
   int* meta = reinterpret_cast<int*>(scr + L.meta);
-  // The warps of a CTA meet at a CTA barrier between the stages (ModeStep): an SM then executes as many code regions at a
-  // time as it has CTAs, not as it has warps, which keeps the hot instructions in the 32 KB instruction cache.
-  const bool valid = env < P.E && !(honour_rest && meta[MetaResting]);
-#define STAGE_SYNC() do { if (mode == ModeStep) __syncthreads(); } while (0)
-  if (mode != ModeStep && !valid) return;
-  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc));
+  if (honour_rest && meta[MetaResting]) return;
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaDetect), ArenaDetect);
   unsigned st = 0;
-  int n_cand = 0, n_coll = 0, nprev = 0;
-  if (valid) {
-    load_predict(s, P, env, mode == ModeStep);
-    if (mode == ModeStep || mode == ModeBroad) {
-      n_cand = broadphase(s, P, &st);
-      if (mode == ModeBroad || P.materialise) write_pairs(s, P, env, n_cand);
-    } else if (mode == ModeNarrow) {
-      n_cand = load_candidates(s, P, env);
-    }
+  int n_cand = 0, n_coll = 0;
+  load_predict(s, P, env, mode == ModeStep);
+  if (mode == ModeStep || mode == ModeBroad) {
+    n_cand = broadphase(s, P, &st);
+    if (mode == ModeBroad || P.materialise) write_pairs(s, P, env, n_cand);
+  } else if (mode == ModeNarrow) {
+    n_cand = load_candidates(s, P, env);
   }
-  STAGE_SYNC();
-  if (valid && (mode == ModeStep || mode == ModeNarrow)) {
-    n_coll = find_colliding(s, P, n_cand, &st);
-    if (mode == ModeNarrow || P.materialise) write_contacts(s, P, env, scr, L, n_cand, n_coll);
+  if (mode == ModeStep || mode == ModeNarrow) n_coll = find_colliding(s, P, n_cand, &st);
+  if (mode == ModeGiven) {
+    const int n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
+    n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
+    unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
+    for (int r = lane; r < n_coll; r += 32) gcoff[r] = s.wrank[r];       // the colouring reuses s.wrank
+    if (lane == 0) meta[MetaNcont] = n_cont;
+    __syncwarp();
   }
-  if (valid && (mode == ModeStep || mode == ModeGiven)) {
-    nprev = load_prev_keys(s, P, env);
-    if (mode == ModeGiven) {
-      const int n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
-      n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
-      unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
-      for (int r = lane; r < n_coll; r += 32) gcoff[r] = s.wrank[r];       // the colouring reuses s.wrank
-      if (lane == 0) meta[MetaNcont] = n_cont;
-      __syncwarp();
-      colour_pairs(s, P, scr, L, n_coll, &st);
-      setup_given(s, P, env, scr, L, n_coll, n_cont, nprev);
-    } else {
-      colour_pairs(s, P, scr, L, n_coll, &st);
-    }
-  }
-  STAGE_SYNC();
-  if (valid && mode == ModeStep) {
-    setup_pairs(s, P, env, scr, L, n_coll, nprev);
-    if (P.counters && lane == 0) {
+  if (mode != ModeBroad) {
+    colour_pairs(s, P, scr, L, n_coll, &st);
+    if (P.counters && mode == ModeStep && lane == 0) {
       const int ncol = s.misc[MiNcol];
       atomicAdd(P.counters + JENGA_CNT_CANDIDATES, (unsigned long long)n_cand);
       atomicAdd(P.counters + JENGA_CNT_COLLIDING, (unsigned long long)n_coll);
@@ -910,8 +923,30 @@ __global__ void __launch_bounds__(128, 4) k_collide(const Params P, const int ho
       atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
     }
   }
-#undef STAGE_SYNC
-  if (valid) flush_status(P, env, st);
+  flush_status(P, env, st);
+}
+
+template <int mode>
+__global__ void __launch_bounds__(128, 4) k_setup(const Params P, const int honour_rest) {
+  const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
+  const int env = blockIdx.x * wpc + warp;
+  if (env >= P.E) return;
+  const Scratch L = scratch_layout(P.pc);
+  float* scr = P.scratch + (size_t)env * P.scratch_words;
+  int* meta = reinterpret_cast<int*>(scr + L.meta);
+  if (honour_rest && meta[MetaResting]) return;
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaSetup), ArenaSetup);
+  load_predict(s, P, env, false, false);                                 // the records again (k_detect changed v, w only)
+  const int n_coll = load_colliding(s, scr, L);
+  if (mode == ModeNarrow || (mode == ModeStep && P.materialise)) {
+    const int n_cand = max(0, min(P.n_pairs[env], P.max_pairs));
+    write_contacts(s, P, env, scr, L, n_cand, n_coll);
+  }
+  if (mode == ModeStep || mode == ModeGiven) {
+    const int nprev = load_prev_keys(s, P, env);
+    if (mode == ModeGiven) setup_given(s, P, env, scr, L, n_coll, meta[MetaNcont], nprev);
+    else setup_pairs(s, P, env, scr, L, n_coll, nprev);
+  }
 }
 
 }  // namespace jenga
