@@ -144,8 +144,8 @@ int jenga_narrowphase(jenga_world *w, void *cuda_stream);
  * (read only) when desc.warm_start = 1 and n_cache[env] > 0.  Eq. 13-15, Listing 1.                   */
 int jenga_pgs_solve(jenga_world *w, int iters, void *cuda_stream);
 
-/* n_steps advances of dt (each n_substeps substeps S1..S7 = three kernel launches: detection, contact setup, solve +
- * integrate), all enqueued by this one call; state, cache, status and counters are updated in place.  */
+/* n_steps advances of dt (each n_substeps substeps S1..S7 = four kernel launches: detection, manifolds, contact setup,
+ * solve + integrate), all enqueued by this one call; state, cache, status and counters are updated in place.  */
 int jenga_step(jenga_world *w, int n_steps, void *cuda_stream);
 
 /* simulate_until_rest (§8.3): every env advances dt by dt until its total kinetic energy
@@ -198,8 +198,8 @@ const char *jenga_strerror(int code);
 /* Measurement aid (bench.py's roofline): while enabled, every launch of jenga_step / jenga_simulate_until_rest is
  * bracketed by CUDA events on the caller's stream.  jenga_profile_read synchronises on them and returns, for the launches
  * since the last enable / read, the summed device time [ms] of out[0] = the detection kernel (S1, S2, SAT, colouring),
- * out[1] = the setup kernel (manifolds, effective masses), out[2] = the solve + integrate kernel; out[3] = number of
- * substeps.  `out` is a HOST array of 4 doubles.                                                           */
+ * out[1] = the manifold kernel, out[2] = the contact-setup kernel (effective masses, warm-start lookup), out[3] = the
+ * solve + integrate kernel; out[4] = number of substeps.  `out` is a HOST array of 5 doubles.               */
 int jenga_profile_enable(jenga_world *w, int on);
 int jenga_profile_read(jenga_world *w, double *out);
 

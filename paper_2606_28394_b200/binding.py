@@ -243,9 +243,10 @@ class World:
         _check(lib().jenga_profile_enable(self.handle, int(on)), "jenga_profile_enable")
 
     def jenga_profile_read(self) -> dict:
-        out = (C.c_double * 4)()
+        out = (C.c_double * 5)()
         _check(lib().jenga_profile_read(self.handle, out), "jenga_profile_read")
-        return dict(detect_ms=out[0], setup_ms=out[1], collide_ms=out[0] + out[1], solve_ms=out[2], substeps=int(out[3]))
+        return dict(detect_ms=out[0], manifold_ms=out[1], slot_ms=out[2], collide_ms=out[0] + out[1] + out[2], solve_ms=out[3],
+                    substeps=int(out[4]))
 
     def jenga_world_destroy(self):
         if self.handle:

@@ -1,7 +1,8 @@
-// jenga.cu -- C-ABI of the batched Jenga step (include/jenga.h) over the three kernels of a substep.  sm_100a only.
+// jenga.cu -- C-ABI of the batched Jenga step (include/jenga.h) over the four kernels of a substep.  sm_100a only.
 //
 //   k_detect  (kcollide.cuh)  S1 predict, S2 broadphase, S3 SAT, S4 colouring                   -> scratch
-//   k_setup   (kcollide.cuh)  S3 manifolds, S4 effective masses + warm-start lookup             -> scratch
+//   k_manifold (kcollide.cuh) S3 contact manifolds                                              -> scratch
+//   k_slot    (kcollide.cuh)  S4 effective masses + warm-start lookup                           -> scratch
 //   k_solve   (ksolve.cuh)    S4 warm start, S5 PGS sweeps, S6 integrate, S7 cache, Eq. 18 latch
 // One warp per env in both.  jenga_step(n) enqueues n * n_substeps such pairs of launches on the caller's stream;
 // nothing returns to the host in between.  The stage entry points run the same device functions in a reduced mode.
@@ -44,17 +45,18 @@ struct jenga_world {
   int n_sm;
   size_t smem_solve;       // dynamic shared memory per CTA of k_solve
   size_t smem_collide;     // ... of k_detect
-  size_t smem_setup;       // ... of k_setup
+  size_t smem_manifold, smem_slot;   // ... of k_manifold, k_slot
   bool profiling;          // jenga_profile_enable: events around every launch of the step
-  std::vector<cudaEvent_t> ev;   // e0 k_detect e1 k_setup e2 k_solve e3, per substep
+  std::vector<cudaEvent_t> ev;   // e0 k_detect e1 k_manifold e2 k_slot e3 k_solve e4, per substep
 };
 
 static thread_local char g_err[512] = "no error";
 
 static size_t collide_env_bytes(const jenga_world_desc* d, int arena = -1) {
   const size_t a = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaDetect);
-  const size_t b = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaSetup);
-  return arena == jenga::ArenaDetect ? a : (arena == jenga::ArenaSetup ? b : (a > b ? a : b));
+  const size_t b = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaManifold);
+  const size_t c = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaSlot);
+  return arena == jenga::ArenaDetect ? a : (arena == jenga::ArenaManifold ? b : (arena == jenga::ArenaSlot ? c : (a > b ? a : b)));
 }
 static size_t solve_env_bytes(const jenga_world_desc* d, int tmb) {
   return 4 * jenga::solve_smem_words(d->body_stride, d->max_contacts / 4, tmb);
@@ -131,7 +133,7 @@ static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; 
 
 /* cudaFuncAttributeMaxDynamicSharedMemorySize is per kernel and process-wide: it is only ever raised (running maximum
  * per device), immediately before the launch that needs it, so worlds of different sizes can be used in any order.   */
-enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnSetup, KnSetupNarrow, KnSetupGiven, KnSolveTm, KnSolveSm, KnCount };
+enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnSolveTm, KnSolveSm, KnCount };
 static std::mutex g_attr_mutex;
 static size_t g_attr_max[16][KnCount];
 
@@ -141,9 +143,10 @@ static const void* kernel_ptr(int kn) {
     case KnCollideBroad: return (const void*)jenga::k_detect<jenga::ModeBroad>;
     case KnCollideNarrow: return (const void*)jenga::k_detect<jenga::ModeNarrow>;
     case KnCollideGiven: return (const void*)jenga::k_detect<jenga::ModeGiven>;
-    case KnSetup: return (const void*)jenga::k_setup<jenga::ModeStep>;
-    case KnSetupNarrow: return (const void*)jenga::k_setup<jenga::ModeNarrow>;
-    case KnSetupGiven: return (const void*)jenga::k_setup<jenga::ModeGiven>;
+    case KnManifold: return (const void*)jenga::k_manifold<jenga::ModeStep>;
+    case KnManifoldNarrow: return (const void*)jenga::k_manifold<jenga::ModeNarrow>;
+    case KnSlot: return (const void*)jenga::k_slot<jenga::ModeStep>;
+    case KnSlotGiven: return (const void*)jenga::k_slot<jenga::ModeGiven>;
     case KnSolveTm: return (const void*)jenga::k_solve<true>;
     default: return (const void*)jenga::k_solve<false>;
   }
@@ -188,7 +191,8 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   const size_t cb = collide_env_bytes(d);
   w->wpc_collide = 4 * cb <= kSmemMax ? 4 : (2 * cb <= kSmemMax ? 2 : 1);
   w->smem_collide = w->wpc_collide * collide_env_bytes(d, jenga::ArenaDetect);
-  w->smem_setup = w->wpc_collide * collide_env_bytes(d, jenga::ArenaSetup);
+  w->smem_manifold = w->wpc_collide * collide_env_bytes(d, jenga::ArenaManifold);
+  w->smem_slot = w->wpc_collide * collide_env_bytes(d, jenga::ArenaSlot);
   if (w->smem_solve > (size_t)prop.sharedMemPerBlockOptin || w->smem_collide > (size_t)prop.sharedMemPerBlockOptin) { delete w; return JENGA_E_ARG; }
   Params& P = w->P;
   P.E = d->n_envs; P.B = d->n_bodies; P.S = d->body_stride;
@@ -240,17 +244,14 @@ extern "C" int jenga_profile_enable(jenga_world* w, int on) {
 
 extern "C" int jenga_profile_read(jenga_world* w, double* out) {
   if (!w || !out) return JENGA_E_ARG;
-  double ms_d = 0.0, ms_u = 0.0, ms_s = 0.0; size_t n = w->ev.size() / 4;
+  double ms[4] = { 0.0, 0.0, 0.0, 0.0 }; const size_t n = w->ev.size() / 5;
   for (size_t i = 0; i < n; ++i) {
-    cudaError_t e = cudaEventSynchronize(w->ev[4 * i + 3]);
+    cudaError_t e = cudaEventSynchronize(w->ev[5 * i + 4]);
     if (e != cudaSuccess) return cuda_fail(e, "jenga_profile_read");
-    float a = 0.0f, b = 0.0f, c = 0.0f;
-    cudaEventElapsedTime(&a, w->ev[4 * i], w->ev[4 * i + 1]);
-    cudaEventElapsedTime(&b, w->ev[4 * i + 1], w->ev[4 * i + 2]);
-    cudaEventElapsedTime(&c, w->ev[4 * i + 2], w->ev[4 * i + 3]);
-    ms_d += a; ms_u += b; ms_s += c;
+    for (int k = 0; k < 4; ++k) { float t = 0.0f; cudaEventElapsedTime(&t, w->ev[5 * i + k], w->ev[5 * i + k + 1]); ms[k] += t; }
   }
-  out[0] = ms_d; out[1] = ms_u; out[2] = ms_s; out[3] = (double)n;
+  for (int k = 0; k < 4; ++k) out[k] = ms[k];
+  out[4] = (double)n;
   drop_events(w);
   return JENGA_OK;
 }
@@ -270,7 +271,7 @@ static void mark(jenga_world* w, cudaStream_t st) {
   w->ev.push_back(e);
 }
 
-/* k_detect, then (except for jenga_broadphase) k_setup, for every env */
+/* k_detect, then (except for jenga_broadphase) k_manifold and k_slot, for every env */
 static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_t st) {
   cudaError_t e = ensure_smem(w->desc.device, KnCollide + mode, w->smem_collide);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_detect)");
@@ -284,15 +285,21 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
   int rc = launched("k_detect");
   if (rc != JENGA_OK || mode == jenga::ModeBroad) return rc;
   mark(w, st);
-  const int kn = mode == jenga::ModeStep ? KnSetup : (mode == jenga::ModeNarrow ? KnSetupNarrow : KnSetupGiven);
-  e = ensure_smem(w->desc.device, kn, w->smem_setup);
-  if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_setup)");
-  switch (mode) {
-    case jenga::ModeStep: jenga::k_setup<jenga::ModeStep><<<grid, thr, w->smem_setup, st>>>(w->P, honour_rest); break;
-    case jenga::ModeNarrow: jenga::k_setup<jenga::ModeNarrow><<<grid, thr, w->smem_setup, st>>>(w->P, honour_rest); break;
-    default: jenga::k_setup<jenga::ModeGiven><<<grid, thr, w->smem_setup, st>>>(w->P, honour_rest); break;
+  if (mode != jenga::ModeGiven) {                           /* manifolds (jenga_pgs_solve: the caller's contacts instead) */
+    const int kn = mode == jenga::ModeStep ? KnManifold : KnManifoldNarrow;
+    e = ensure_smem(w->desc.device, kn, w->smem_manifold);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_manifold)");
+    if (mode == jenga::ModeStep) jenga::k_manifold<jenga::ModeStep><<<grid, thr, w->smem_manifold, st>>>(w->P, honour_rest);
+    else jenga::k_manifold<jenga::ModeNarrow><<<grid, thr, w->smem_manifold, st>>>(w->P, honour_rest);
+    rc = launched("k_manifold");
+    if (rc != JENGA_OK || mode == jenga::ModeNarrow) return rc;
   }
-  return launched("k_setup");
+  mark(w, st);
+  e = ensure_smem(w->desc.device, mode == jenga::ModeStep ? KnSlot : KnSlotGiven, w->smem_slot);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_slot)");
+  if (mode == jenga::ModeStep) jenga::k_slot<jenga::ModeStep><<<grid, thr, w->smem_slot, st>>>(w->P, honour_rest);
+  else jenga::k_slot<jenga::ModeGiven><<<grid, thr, w->smem_slot, st>>>(w->P, honour_rest);
+  return launched("k_slot");
 }
 
 static int launch_solve(jenga_world* w, int iters, int flags, float rest_ek, cudaStream_t st) {

@@ -1,8 +1,8 @@
-// kcollide.cuh -- the two collision kernels of a substep, one env per warp.  k_detect: S1 predict, S2 broadphase, S3 SAT
-// (which candidates collide), S4 canonical colouring + chunk packing.  k_setup: S3 manifolds, S4 contact setup (effective
-// masses, warm-start lookup).  Their products go to the scratch buffer (layout.cuh) for k_solve.  They are separate
-// kernels because each one's hot code then fits the 32 KB instruction cache (as one kernel: 70 KB, and `no_instruction`
-// was the top stall with 16 warps per SM at different places in it).
+// kcollide.cuh -- the three collision kernels of a substep, one env per warp.  k_detect: S1 predict, S2 broadphase, S3 SAT
+// (which candidates collide), S4 canonical colouring + chunk packing.  k_manifold: S3 contact manifolds.  k_slot: S4
+// contact setup (effective masses, warm-start lookup).  Their products go to the scratch buffer (layout.cuh) for the
+// next kernel.  They are separate kernels because each one's hot code then fits the 32 KB instruction cache (as one
+// kernel: 70 KB, and `no_instruction` was the top stall with 16 warps per SM at different places in it).
 #pragma once
 #include "layout.cuh"
 
@@ -31,10 +31,11 @@ struct CSm {
 };
 enum { MiNph = 0, MiNcol = 1, MiNblk = 2 };
 
-enum { ArenaDetect = 0, ArenaSetup = 1 };
+enum { ArenaDetect = 0, ArenaManifold = 1, ArenaSlot = 2 };
 
 // k_detect: records, extents, masks / hit words, candidate list, colliding list, colouring products.
-// k_setup: records, colliding list (copied from the scratch), cache keys, contact offsets, per-lane clip polygons.
+// k_manifold: records, colliding list (copied from the scratch), per-lane clip polygons.  k_slot: records, colliding
+// list, cache keys.
 __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc, int arena) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc);
   size_t w = (size_t)kCb * S + pcA;                        // cb, cab
@@ -44,8 +45,10 @@ __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int p
     w += 4 * S + uh + mpA / 2 + pcA / 4;                   // ext, used / hitw, cand, colour
     w += 2 * round_up(ph_max(nblk), 4);                    // ph, chc
     w += 2 * kMaxColours + round_up(nblk, 4) + 8;          // ccount, cfirst, fill, misc
+  } else if (arena == ArenaManifold) {
+    w += 768;                                              // poly
   } else {
-    w += pcA / 2 + 768;                                    // cprev, poly
+    w += pcA / 2;                                          // cprev
   }
   return round_up((int)w, 4);
 }
@@ -72,9 +75,10 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int 
     s.cfirst.off = p; p += kMaxColours;
     s.fill.off = p;   p += round_up(nblk, 4);
     s.misc.off = p;
-  } else {
-    s.cprev.off = p;  p += pcA / 2;
+  } else if (arena == ArenaManifold) {
     s.poly.off = p;
+  } else {
+    s.cprev.off = p;
   }
   return s;
 }
@@ -749,15 +753,19 @@ __device__ inline int load_prev_keys(const CSm& s, const Params& P, int env) {
   return nprev;
 }
 
-// S3 second half + S4: lane l of a round takes colliding pair r = 32 round + l (ascending pair index), computes its
-// manifold (the SAT axis is known) and writes header and constants at the pair's position.
+// S4: lane l of a round takes colliding pair r = 32 round + l (ascending pair index), fetches the manifold k_manifold
+// left in the scratch and writes header and constants at the pair's position.
 __device__ inline void setup_pairs(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_coll, int nprev) {
+  const float4* man = reinterpret_cast<const float4*>(scr + L.man);
   for (int r = lane_id(); r < n_coll; r += 32) {
     const unsigned w = s.cab[r];
     const int a = ab_a(w), b = ab_b(w), pair = s.cpair[r];
     const int lo = cache_lookup(s, P, env, nprev, pair);
-    Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
-    pair_manifold(s, a, b, ab_axis(w), m);
+    Manifold m;
+    const float4 h = man[5 * r];
+    m.n = v3(h.x, h.y, h.z); m.np = __float_as_int(h.w) & 0xff; m.axis = __float_as_int(h.w) >> 8;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) { const float4 q = man[5 * r + 1 + c]; m.p[c] = v3(q.x, q.y, q.z); m.d[c] = q.w; }
     setup_slot(s, P, env, scr, L, lo, s.pos[r], r, a, b, pair, m);
   }
   __syncwarp();
@@ -779,26 +787,34 @@ __device__ inline int load_candidates(const CSm& s, const Params& P, int env) {
   return n_cand;
 }
 
-// Contact list in (pair, slot) order: the manifolds are recomputed from the (unchanged) poses in ascending
-// pair order.  Leaves s.wrank[r] = contact offset of pair r (also written to the scratch for the lambda output).
-__device__ inline int write_contacts(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_cand, int n_coll) {
+// S3 second half: the manifold of every colliding pair (lane l of a round takes pair r = 32 round + l, ascending pair
+// index; the SAT axis is known) into the scratch for k_slot.  With contacts_out the contact list is also written in
+// (pair, slot) order (stage call / parity), and the contact offset of pair r goes to the scratch for the lambda output.
+__device__ inline void manifold_pairs(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_coll, bool contacts_out) {
   const int lane = lane_id();
+  float4* man = reinterpret_cast<float4*>(scr + L.man);
   unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
+  const int n_cand = contacts_out ? max(0, min(P.n_pairs[env], P.max_pairs)) : 0;
   int off0 = 0;
   for (int base = 0; base < n_coll; base += 32) {
     const int r = base + lane;
     Manifold m; m.np = 0; m.axis = 0; m.n = v3(0, 0, 1);
-    int idx = 0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) { m.p[c] = v3(0, 0, 0); m.d[c] = 0.0f; }
     if (r < n_coll) {
       const unsigned w = s.cab[r];
-      idx = s.cpair[r];
       pair_manifold(s, ab_a(w), ab_b(w), ab_axis(w), m);
+      man[5 * r] = make_float4(m.n.x, m.n.y, m.n.z, __int_as_float(m.np | (m.axis << 8)));
+#pragma unroll
+      for (int c = 0; c < 4; ++c) man[5 * r + 1 + c] = make_float4(m.p[c].x, m.p[c].y, m.p[c].z, m.d[c]);
     }
+    if (!contacts_out) continue;
     int tot; const int off = off0 + warp_excl_scan(m.np, &tot);
     if (r < n_coll) {
-      s.wrank[r] = (unsigned short)off; gcoff[r] = (unsigned short)off;
-      const int* gp = P.pairs + (size_t)env * P.max_pairs;      // position of the pair in the candidate list (the on-chip
-      int lo = 0, hi = n_cand;                                   // copy is overwritten by the clip polygons)
+      const int idx = s.cpair[r];
+      gcoff[r] = (unsigned short)off;
+      const int* gp = P.pairs + (size_t)env * P.max_pairs;      // position of the pair in the candidate list
+      int lo = 0, hi = n_cand;
       while (lo < hi) { const int mid = (lo + hi) >> 1; if (gp[mid] < idx) lo = mid + 1; else hi = mid; }
       float4* out = reinterpret_cast<float4*>(P.contacts + ((size_t)env * P.max_contacts + off) * 8);
 #pragma unroll
@@ -811,9 +827,8 @@ __device__ inline int write_contacts(const CSm& s, const Params& P, int env, flo
     }
     off0 += tot;
   }
-  if (lane == 0) { P.n_contacts[env] = off0; reinterpret_cast<int*>(scr + L.meta)[MetaNcont] = off0; }
+  if (contacts_out && lane == 0) { P.n_contacts[env] = off0; reinterpret_cast<int*>(scr + L.meta)[MetaNcont] = off0; }
   __syncwarp();
-  return off0;
 }
 
 // Rebuild the colliding-pair list from a contact list in global memory (ordered (pair, slot); slot 0 carries
@@ -927,7 +942,21 @@ __global__ void __launch_bounds__(128, 4) k_detect(const Params P, const int hon
 }
 
 template <int mode>
-__global__ void __launch_bounds__(128, 4) k_setup(const Params P, const int honour_rest) {
+__global__ void __launch_bounds__(128, 4) k_manifold(const Params P, const int honour_rest) {
+  const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
+  const int env = blockIdx.x * wpc + warp;
+  if (env >= P.E) return;
+  const Scratch L = scratch_layout(P.pc);
+  float* scr = P.scratch + (size_t)env * P.scratch_words;
+  if (honour_rest && reinterpret_cast<int*>(scr + L.meta)[MetaResting]) return;
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaManifold), ArenaManifold);
+  load_predict(s, P, env, false, false);                                 // the records again (k_detect changed v, w only)
+  const int n_coll = load_colliding(s, scr, L);
+  manifold_pairs(s, P, env, scr, L, n_coll, mode == ModeNarrow || P.materialise);
+}
+
+template <int mode>
+__global__ void __launch_bounds__(128, 4) k_slot(const Params P, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
   const int env = blockIdx.x * wpc + warp;
   if (env >= P.E) return;
@@ -935,18 +964,12 @@ __global__ void __launch_bounds__(128, 4) k_setup(const Params P, const int hono
   float* scr = P.scratch + (size_t)env * P.scratch_words;
   int* meta = reinterpret_cast<int*>(scr + L.meta);
   if (honour_rest && meta[MetaResting]) return;
-  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaSetup), ArenaSetup);
-  load_predict(s, P, env, false, false);                                 // the records again (k_detect changed v, w only)
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaSlot), ArenaSlot);
+  load_predict(s, P, env, false, false);
   const int n_coll = load_colliding(s, scr, L);
-  if (mode == ModeNarrow || (mode == ModeStep && P.materialise)) {
-    const int n_cand = max(0, min(P.n_pairs[env], P.max_pairs));
-    write_contacts(s, P, env, scr, L, n_cand, n_coll);
-  }
-  if (mode == ModeStep || mode == ModeGiven) {
-    const int nprev = load_prev_keys(s, P, env);
-    if (mode == ModeGiven) setup_given(s, P, env, scr, L, n_coll, meta[MetaNcont], nprev);
-    else setup_pairs(s, P, env, scr, L, n_coll, nprev);
-  }
+  const int nprev = load_prev_keys(s, P, env);
+  if (mode == ModeGiven) setup_given(s, P, env, scr, L, n_coll, meta[MetaNcont], nprev);
+  else setup_pairs(s, P, env, scr, L, n_coll, nprev);
 }
 
 }  // namespace jenga

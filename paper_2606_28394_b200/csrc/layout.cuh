@@ -1,14 +1,15 @@
 // layout.cuh -- parameters, the global hand-off ("scratch") between the two kernels of a substep, and the shared
 // memory arenas of the batched Jenga step (sm_100a).
 //
-// A substep (S1..S7 of include/jenga.h) is THREE kernels, all with ONE WARP PER ENV (every synchronisation inside an
+// A substep (S1..S7 of include/jenga.h) is FOUR kernels, all with ONE WARP PER ENV (every synchronisation inside an
 // env is a __syncwarp()):
 //   k_detect   S1 predict, S2 broadphase, S3 SAT (which candidates collide, on which axis), S4 canonical colouring.
-//   k_setup    S3 manifolds, S4 contact setup (effective masses, warm-start lookup).  Small footprints (11 / 10 KB of
-//              shared memory per 54-body env, <= 128 registers): 16-20 warps per SM hide the latencies of this branchy,
-//              load-heavy half, and each kernel's hot code fits the instruction cache.  Output per env, in the
-//              caller-owned scratch buffer: pair headers and the 48 solver constants of every colliding pair at its
-//              colour-packed POSITION, and the list of colour chunks.
+//   k_manifold S3 contact manifolds of the colliding pairs.
+//   k_slot     S4 contact setup (effective masses, warm-start lookup).  Small footprints (8-11 KB of shared memory per
+//              54-body env, <= 128 registers): 16+ warps per SM hide the latencies of this branchy, load-heavy half, and
+//              each kernel's hot code fits the instruction cache.  Output per env, in the caller-owned scratch
+//              buffer: pair headers and the 48 solver constants of every colliding pair at its colour-packed POSITION,
+//              and the list of colour chunks.
 //   k_solve    S4 warm-start application, S5 PGS sweeps, S6 integrate + Baumgarte, S7 cache, Eq. 18 latch.
 //              CTA = 4 warps = 4 envs, 2 CTAs per SM; the constants live in TENSOR MEMORY (tcgen05.ld/st, lane =
 //              position % 32, block j = position / 32 at columns [48 j, 48 j + 48)), bodies and headers in shared
@@ -66,7 +67,7 @@ __host__ __device__ inline int n_blocks(int pc) { return (pc + 31) / 32; }
 __host__ __device__ inline int ph_max(int nblk) { return kMaxColours + 2 * nblk + 8; }
 
 struct Scratch {
-  int hdr, cs, ph, meta, pos, cpair, coff, cab, total;
+  int hdr, cs, ph, meta, pos, cpair, coff, cab, man, total;
 };
 __host__ __device__ inline Scratch scratch_layout(int pc) {
   const int pcA = round_up(pc, 8), nblk = n_blocks(pc), npos = 32 * nblk;
@@ -79,6 +80,7 @@ __host__ __device__ inline Scratch scratch_layout(int pc) {
   L.cpair = p; p += pcA / 2;
   L.coff = p;  p += pcA / 2;
   L.cab = p;   p += pcA;
+  L.man = p;   p += 20 * pcA;           // manifold of pair r: (n.xyz, np | axis << 8), 4 x (p.xyz, depth)
   L.total = round_up(p, 32);
   return L;
 }
