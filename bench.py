@@ -438,7 +438,7 @@ def main():
     ap.add_argument("--e2e-split", type=int, default=2, help="worlds (streams) the e2e leg serves the batch with")
     ap.add_argument("--cfg", type=int, default=CFG, help="BASELINE.json config number (5 = the bench workload; others: manual runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--tier", default="auto", choices=["auto", "smem", "tmem160", "tmem256", "tmem512"], help="where k_solve keeps the contact constants")
+    ap.add_argument("--tier", default="auto", choices=["auto", "smem", "tmem128", "tmem160", "tmem256", "tmem512"], help="where k_solve keeps the contact constants")
     ap.add_argument("--max-contacts", type=int, default=0, help="override the workload's contact capacity per env")
     ap.add_argument("--max-pairs", type=int, default=0, help="override the workload's candidate capacity per env")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="torch.distributed backend (gloo: the CPU test of the launch path)")

@@ -207,7 +207,9 @@ int jenga_profile_read(jenga_world *w, double *out);
  * out[0] = FP32 thread-instructions per second (dependent-free FFMA streams, FMA = 1 instruction),
  * out[1] = shared-memory bytes per second (conflict-free LDS.128 streams), out[2] = SM count,
  * out[3], out[4] = seconds of the two timed runs, out[5] = the FFMA rate with three register operands (out[0] has
- * one uniform-register operand).  `out` is a HOST array of 6 doubles; `scratch` a DEVICE
+ * one uniform-register operand), out[6] = the FFMA rate when all three source registers change from one instruction to the
+ * next (no operand-reuse hits: the solver's shape), out[7] = FMAs per second of the packed form fma.rn.f32x2 (two FMAs per
+ * instruction) under the same no-reuse pattern.  `out` is a HOST array of 8 doubles; `scratch` a DEVICE
  * buffer of jenga_peaks_scratch_bytes() bytes.  Unlike the step calls this one synchronises the stream.  */
 int jenga_measure_peaks(double *out, void *scratch, void *cuda_stream);
 size_t jenga_peaks_scratch_bytes(void);

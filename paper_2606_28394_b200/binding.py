@@ -43,7 +43,7 @@ class Buffers(C.Structure):
                                           "ref_pose", "collapsed", "collapse_stats", "rest_steps", "scratch")] + [("scratch_bytes", C.c_size_t)]
 
 
-TIERS = {"auto": 0, "smem": 1, "tmem256": 2, "tmem512": 3, "tmem160": 4}
+TIERS = {"auto": 0, "smem": 1, "tmem256": 2, "tmem512": 3, "tmem160": 4, "tmem128": 5}
 
 
 def lib():
@@ -119,11 +119,11 @@ def jenga_measure_peaks(device: int = 0) -> dict:
     L = lib()
     dev = torch.device("cuda", device)
     scratch = torch.empty(L.jenga_peaks_scratch_bytes(), dtype=torch.uint8, device=dev)
-    out = (C.c_double * 6)()
+    out = (C.c_double * 8)()
     with torch.cuda.device(dev):
         _check(L.jenga_measure_peaks(out, C.c_void_p(scratch.data_ptr()), C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)),
                "jenga_measure_peaks")
-    return dict(fp32_instr_per_s=out[0], smem_bytes_per_s=out[1], n_sm=int(out[2]), ffma_s=out[3], lds_s=out[4], fp32_instr_per_s_3reg=out[5])
+    return dict(fp32_instr_per_s=out[0], smem_bytes_per_s=out[1], n_sm=int(out[2]), ffma_s=out[3], lds_s=out[4], fp32_instr_per_s_3reg=out[5], fp32_instr_per_s_noreuse=out[6], fp32_fma_per_s_packed_noreuse=out[7])
 
 
 class World:

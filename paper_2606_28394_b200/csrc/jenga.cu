@@ -33,7 +33,7 @@ __global__ void k_reset_rest(const Params P) {
 // =================================================================== host side / C-ABI
 using jenga::Params;
 
-enum { TierAuto = 0, TierSmem = 1, TierTmem256 = 2, TierTmem512 = 3, TierTmem160 = 4 };
+enum { TierAuto = 0, TierSmem = 1, TierTmem256 = 2, TierTmem512 = 3, TierTmem160 = 4, TierTmem128 = 5 };
 static const size_t kSmemMax = 227 * 1024;
 
 struct jenga_world {
@@ -69,7 +69,7 @@ static bool desc_ok(const jenga_world_desc* d) {
   if (d->n_substeps <= 0 || d->n_substeps > 64 || d->pgs_iters < 0 || !(d->dt > 0.0f)) return false;
   if (d->max_pairs <= 0 || d->max_pairs > 65535) return false;
   if (d->max_contacts < 4 || (d->max_contacts & 3) || d->max_contacts > 65532) return false;
-  if (d->solver_tier < TierAuto || d->solver_tier > TierTmem160) return false;
+  if (d->solver_tier < TierAuto || d->solver_tier > TierTmem128) return false;
   if (collide_env_bytes(d) > kSmemMax || solve_env_bytes(d, 0) > kSmemMax) return false;
   return true;
 }
@@ -78,17 +78,18 @@ static bool desc_ok(const jenga_world_desc* d) {
  * = tmb blocks of 48: G = 3 -> 3 blocks (12 envs per SM), G = 2 -> 5, G = 1 -> 10; 0 = everything in shared memory, one
  * warp per CTA.  Auto takes the largest G whose shared memory (headers + bodies of 4 G envs) fits one SM;
  * desc.solver_tier forces a tier (-1 if it does not fit).                                                         */
-static int tier_groups(int tmb) { return tmb == 3 ? 3 : (tmb == 5 ? 2 : (tmb == 10 ? 1 : 0)); }
+static int tier_groups(int tmb) { return tmb == 2 ? 4 : (tmb == 3 ? 3 : (tmb == 5 ? 2 : (tmb == 10 ? 1 : 0))); }
 static bool tier_fits(const jenga_world_desc* d, int tmb) {
   return 4 * tier_groups(tmb) * solve_env_bytes(d, tmb) + 1024 + 16 <= kSmemMax;
 }
 static int pick_tmb(const jenga_world_desc* d) {
   switch (d->solver_tier) {
     case TierSmem: return 0;
+    case TierTmem128: return tier_fits(d, 2) ? 2 : -1;
     case TierTmem160: return tier_fits(d, 3) ? 3 : -1;
     case TierTmem256: return tier_fits(d, 5) ? 5 : -1;
     case TierTmem512: return tier_fits(d, 10) ? 10 : -1;
-    default: return tier_fits(d, 3) ? 3 : (tier_fits(d, 5) ? 5 : (tier_fits(d, 10) ? 10 : 0));
+    default: return tier_fits(d, 2) ? 2 : (tier_fits(d, 3) ? 3 : (tier_fits(d, 5) ? 5 : (tier_fits(d, 10) ? 10 : 0)));
   }
 }
 

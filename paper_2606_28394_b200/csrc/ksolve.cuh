@@ -5,7 +5,7 @@
 //   TM = true   ONE persistent CTA per SM of 4 G warps = 4 G envs in flight (G = 3, 2 or 1) that owns all 512 columns of
 //               tensor memory.  Warp w works in TMEM lanes 32 (w % 4) .. + 31 (its quadrant) and columns
 //               [48 tmb (w / 4), + 48 tmb): the 48 constant words of the positions of the env's first `tmb` 32-position
-//               blocks (tmb = 3, 5, 10 for G = 3, 2, 1; tcgen05.ld/st.32x32b: lane = position % 32, block j at column
+//               blocks (tmb = 2, 3, 5, 10 for G = 4, 3, 2, 1; tcgen05.ld/st.32x32b: lane = position % 32, block j at column
 //               offset 48 j).  Blocks >= tmb stay where k_collide wrote them, in the scratch (L2-resident while the env is
 //               in flight): their visits load and store global memory, one visit ahead of use.
 //   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers; test coverage).
@@ -17,7 +17,7 @@ namespace jenga {
 struct SSm {
   SP<float> bd;                 // [S + 1][kBd] solver body records; record S is the ground: all zeros, never changes
   SP<float> q;                  // [4][S]
-  SP<float4> hdr;               // [kHdrF4][npos]
+  SP<float4> hdr;               // [2][npos] the first two float4 of the pair headers (t1 is recomputed from n)
   SP<float4> cs;                // TM = false: [nblk][kCsF4][32] every block in shared memory
   SP<int> ph;                   // [ph_max]
   int npos, tmb;
@@ -28,7 +28,7 @@ struct SSm {
 // tmb = 0: the all-shared-memory flavour
 __host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb) {
   const int nblk = n_blocks(pc);
-  size_t w = (size_t)(kBd + 4) * S + kBd + 4 * kHdrF4 * 32 * (size_t)nblk;
+  size_t w = (size_t)(kBd + 4) * S + kBd + 4 * 2 * 32 * (size_t)nblk;
   w += tmb ? 0 : (size_t)kBlkWords * nblk;
   w += round_up(ph_max(nblk), 4);
   return round_up((int)w, 4);
@@ -38,7 +38,7 @@ __device__ inline SSm carve_solve(int S, int pc, int tmb, int base) {
   const int nblk = n_blocks(pc);
   SSm s; int p = base;
   s.npos = 32 * nblk; s.tmb = tmb; s.tm = 0; s.gcs = nullptr;
-  s.hdr.off = p; p += 4 * kHdrF4 * s.npos;
+  s.hdr.off = p; p += 4 * 2 * s.npos;
   s.cs.off = p;  p += tmb ? 0 : kBlkWords * nblk;
   s.bd.off = p;  p += kBd * (S + 1);
   s.q.off = p;   p += 4 * S;
@@ -77,7 +77,13 @@ __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sy
 // whole block j (all 32 lanes take part; lane l gets position 32 j + l)
 __device__ __forceinline__ void tm_load_block(const SSm& s, int j, PairC& c) {
   const unsigned a = s.tm + 48u * (unsigned)j;
+#ifdef EXP_SKIP_LDTM
+  tm_ld16(a + 32, c.v + 32);
+#pragma unroll
+  for (int t = 0; t < 32; ++t) c.v[t] = c.v[32 + (t & 15)];
+#else
   tm_ld16(a, c.v); tm_ld16(a + 16, c.v + 16); tm_ld16(a + 32, c.v + 32);
+#endif
 }
 __device__ __forceinline__ void tm_store_block(const SSm& s, int j, const PairC& c) {
   const unsigned a = s.tm + 48u * (unsigned)j;
@@ -149,7 +155,9 @@ __device__ __forceinline__ void end_solve(const SSm& s) {
 
 // ---------------------------------------------------------------- load
 // Body records from the state tile (lane b reads column b of every row: coalesced); Iw^-1 from q (Eq. 1).
-// Spare words of the record keep the body-frame inverse moments (kinetic energy, Eq. 18).
+// Record (5 float4, stride 20 words: an odd number of 16-byte words, so 8 consecutive bodies cover all bank groups):
+// x y z im | v.xyz Ixx | w.xyz Ixy | Ixz Iyy Iyz Izz | body-frame inverse moments.  The solver reads the first four and
+// writes back the second and third (the inertia words ride along unchanged).
 __device__ inline void load_bodies(const SSm& s, const Params& P, int env) {
   const int S = P.S;
   const float* st = P.state + (size_t)env * kStateRows * S;
@@ -162,10 +170,10 @@ __device__ inline void load_bodies(const SSm& s, const Params& P, int env) {
     float I6[6];
     world_inv_inertia(R, dyn ? i0 : 0.0f, dyn ? i1 : 0.0f, dyn ? i2 : 0.0f, I6);
     bd4(s, b, 0) = make_float4(st[b], st[S + b], st[2 * S + b], dyn ? im : 0.0f);
-    bd4(s, b, 1) = make_float4(st[7 * S + b], st[8 * S + b], st[9 * S + b], i0);
-    bd4(s, b, 2) = make_float4(st[10 * S + b], st[11 * S + b], st[12 * S + b], i1);
-    bd4(s, b, 3) = make_float4(I6[0], I6[1], I6[2], I6[3]);
-    bd4(s, b, 4) = make_float4(I6[4], I6[5], i2, 0.0f);
+    bd4(s, b, 1) = make_float4(st[7 * S + b], st[8 * S + b], st[9 * S + b], I6[0]);       // v, Ixx
+    bd4(s, b, 2) = make_float4(st[10 * S + b], st[11 * S + b], st[12 * S + b], I6[1]);    // w, Ixy
+    bd4(s, b, 3) = make_float4(I6[2], I6[3], I6[4], I6[5]);                                // Ixz Iyy Iyz Izz
+    bd4(s, b, 4) = make_float4(i0, i1, i2, 0.0f);                                          // body-frame inverse moments (Eq. 18)
     s.q[b] = w; s.q[S + b] = x; s.q[2 * S + b] = y; s.q[3 * S + b] = z;
   }
   if (lane_id() < 5) bd4(s, S, lane_id()) = make_float4(0, 0, 0, 0);      // the ground: inverse mass and inertia 0, at rest
@@ -193,7 +201,7 @@ __device__ inline int load_slots(const SSm& s, const Params& P, const float* scr
   const int* gph = reinterpret_cast<const int*>(scr + L.ph);
   for (int j = lane; j < nph; j += 32) s.ph[j] = gph[j];
   const float4* ghdr = reinterpret_cast<const float4*>(scr + L.hdr);
-  for (int f = 0; f < kHdrF4; ++f)
+  for (int f = 0; f < 2; ++f)
     for (int k = lane; k < 32 * nblk; k += 32) s.hdr[f * s.npos + k] = ghdr[f * s.npos + k];
   const float4* gcs = reinterpret_cast<const float4*>(scr + L.cs);
   const int ncopy = TM ? min(nblk, s.tmb) : nblk;              // TM: blocks >= tmb are used in place
@@ -212,10 +220,10 @@ __device__ inline int load_slots(const SSm& s, const Params& P, const float* scr
   return nph;
 }
 
-struct Body5 { float4 x, v, w, i0, i1; };     // x.w = inverse mass (0: static / inactive / ground)
+struct Body5 { float4 x, v, w, i; };           // x.w = inverse mass (0: static / inactive / ground); v.w = Ixx, w.w = Ixy, i = Ixz Iyy Iyz Izz
 
 __device__ __forceinline__ void load_body(const SSm& s, int b, Body5& o) {
-  o.x = bd4(s, b, 0); o.v = bd4(s, b, 1); o.w = bd4(s, b, 2); o.i0 = bd4(s, b, 3); o.i1 = bd4(s, b, 4);
+  o.x = bd4(s, b, 0); o.v = bd4(s, b, 1); o.w = bd4(s, b, 2); o.i = bd4(s, b, 3);
 }
 // the ground's velocities stay +-0 (its inverse mass and inertia are 0), so writing them back is harmless
 __device__ __forceinline__ void store_body_vel(const SSm& s, int b, const Body5& o) { bd4(s, b, 1) = o.v; bd4(s, b, 2) = o.w; }
@@ -225,12 +233,12 @@ __device__ __forceinline__ void apply_impulse(Body5& A, Body5& B, Vec3 rA, Vec3 
   A.v.x = fmaf(-A.x.w, Pi.x, A.v.x); A.v.y = fmaf(-A.x.w, Pi.y, A.v.y); A.v.z = fmaf(-A.x.w, Pi.z, A.v.z);
   B.v.x = fmaf(B.x.w, Pi.x, B.v.x);  B.v.y = fmaf(B.x.w, Pi.y, B.v.y);  B.v.z = fmaf(B.x.w, Pi.z, B.v.z);
   const Vec3 cA = cross(Pi, rA), cB = cross(rB, Pi);        // -(rA x Pi), +(rB x Pi)
-  A.w.x = fmaf(A.i0.z, cA.z, fmaf(A.i0.y, cA.y, fmaf(A.i0.x, cA.x, A.w.x)));
-  A.w.y = fmaf(A.i1.x, cA.z, fmaf(A.i0.w, cA.y, fmaf(A.i0.y, cA.x, A.w.y)));
-  A.w.z = fmaf(A.i1.y, cA.z, fmaf(A.i1.x, cA.y, fmaf(A.i0.z, cA.x, A.w.z)));
-  B.w.x = fmaf(B.i0.z, cB.z, fmaf(B.i0.y, cB.y, fmaf(B.i0.x, cB.x, B.w.x)));
-  B.w.y = fmaf(B.i1.x, cB.z, fmaf(B.i0.w, cB.y, fmaf(B.i0.y, cB.x, B.w.y)));
-  B.w.z = fmaf(B.i1.y, cB.z, fmaf(B.i1.x, cB.y, fmaf(B.i0.z, cB.x, B.w.z)));
+  A.w.x = fmaf(A.i.x, cA.z, fmaf(A.w.w, cA.y, fmaf(A.v.w, cA.x, A.w.x)));
+  A.w.y = fmaf(A.i.z, cA.z, fmaf(A.i.y, cA.y, fmaf(A.w.w, cA.x, A.w.y)));
+  A.w.z = fmaf(A.i.w, cA.z, fmaf(A.i.z, cA.y, fmaf(A.i.x, cA.x, A.w.z)));
+  B.w.x = fmaf(B.i.x, cB.z, fmaf(B.w.w, cB.y, fmaf(B.v.w, cB.x, B.w.x)));
+  B.w.y = fmaf(B.i.z, cB.z, fmaf(B.i.y, cB.y, fmaf(B.w.w, cB.x, B.w.y)));
+  B.w.z = fmaf(B.i.w, cB.z, fmaf(B.i.z, cB.y, fmaf(B.i.x, cB.x, B.w.z)));
 }
 
 // The contact arithmetic of one pair (both passes).  Slots ascending; per contact the normal row (Eq. 14, clamp >= 0),
@@ -273,12 +281,12 @@ __device__ __forceinline__ void solve_pair(PairC& c, Body5& A, Body5& B, const F
 }
 
 // What a lane needs of its pair's header during a visit.
-struct Hdr { int a, b; Vec3 n, t1; };
+struct Hdr { int a, b; Vec3 n; float il; };
 // a = body record of A: the ground (header field 0) is the all-zero record S
 __device__ __forceinline__ Hdr load_hdr(const SSm& s, int S, int k) {
-  const float4 h = hdr4(s, 0, k), nn = hdr4(s, 1, k), tt = hdr4(s, 2, k);
+  const float4 h = hdr4(s, 0, k), nn = hdr4(s, 1, k);
   Hdr H; const int ab = __float_as_int(h.x), a1 = ab & 0xffff;
-  H.a = a1 ? a1 - 1 : S; H.b = ab >> 16; H.n = xyz(nn); H.t1 = xyz(tt);
+  H.a = a1 ? a1 - 1 : S; H.b = ab >> 16; H.n = xyz(nn); H.il = h.w;
   return H;
 }
 __device__ __forceinline__ bool chunk_lane(int d, int lane) { const int l0 = d & 0xff; return lane >= l0 && lane < l0 + ((d >> 8) & 0xff); }
@@ -293,7 +301,7 @@ __device__ inline void warm_start_pass(const SSm& s, int S, int nph) {
     if (chunk_lane(d, lane)) {
       const Hdr H = load_hdr(s, S, 32 * jb + lane);
       Body5 A, B; load_body(s, H.a, A); load_body(s, H.b, B);
-      Frame F; F.n = H.n; F.t1 = H.t1; F.t2 = cross(F.n, F.t1);
+      const Frame F = make_frame(H.n, H.il);
       solve_pair<true>(c, A, B, F, 0.0f);
       store_body_vel(s, H.a, A); store_body_vel(s, H.b, B);
     }
@@ -313,7 +321,7 @@ __device__ inline void pgs_sweeps(const SSm& s, int S, int nph, int iters, float
   if (total <= 0) return;
   int d = s.ph[0], jn = 0;
   PairC c;
-  Hdr H; H.a = S; H.b = S; H.n = H.t1 = v3(0, 0, 0);
+  Hdr H; H.a = S; H.b = S; H.n = v3(0, 0, 0); H.il = 0.0f;
   if (chunk_lane(d, lane)) H = load_hdr(s, S, 32 * (d >> 16) + lane);
   if (TM && (d >> 16) < s.tmb) tm_load_block(s, d >> 16, c);
   else sm_load_pair<TM>(s, d >> 16, lane, c);
@@ -328,7 +336,7 @@ __device__ inline void pgs_sweeps(const SSm& s, int S, int nph, int iters, float
     const Hdr Hn = load_hdr(s, S, 32 * (dn >> 16) + lane);
     if (active) {
       Body5 A, B; load_body(s, H.a, A); load_body(s, H.b, B);
-      Frame F; F.n = H.n; F.t1 = H.t1; F.t2 = cross(F.n, F.t1);
+      const Frame F = make_frame(H.n, H.il);
       solve_pair<false>(c, A, B, F, mu);
       store_body_vel(s, H.a, A); store_body_vel(s, H.b, B);
       if (!in_tm) sm_store_lam<TM>(s, jb, lane, c.v + kLam);
@@ -394,11 +402,11 @@ __device__ inline void integrate(const SSm& s, const Params& P, int nph, unsigne
 
 // Per-body terms of Eq. 18 / PAPER.md:380: kinetic energy 1/2 m |v|^2 + 1/2 w . I w with I in the body frame
 // (R^T w against the principal moments, R from the new q, Eq. 1).
-__device__ __forceinline__ float body_kinetic_energy(const SSm& s, int S, int b, float4 x, float4 v, float4 w, float i2) {
+__device__ __forceinline__ float body_kinetic_energy(const SSm& s, int S, int b, float4 x, float4 v, float4 w, float4 ib) {
   const float qw = s.q[b], qx = s.q[S + b], qy = s.q[2 * S + b], qz = s.q[3 * S + b];
   float R[9]; quat_to_R(qw, qx, qy, qz, R);
   const float w0 = R[0] * w.x + R[3] * w.y + R[6] * w.z, w1 = R[1] * w.x + R[4] * w.y + R[7] * w.z, w2 = R[2] * w.x + R[5] * w.y + R[8] * w.z;
-  return 0.5f * (v.x * v.x + v.y * v.y + v.z * v.z) / x.w + 0.5f * (w0 * w0 / v.w + w1 * w1 / w.w + w2 * w2 / i2);
+  return 0.5f * (v.x * v.x + v.y * v.y + v.z * v.z) / x.w + 0.5f * (w0 * w0 / ib.x + w1 * w1 / ib.y + w2 * w2 / ib.z);
 }
 
 // Collapse latch (Eq. 18, reading A17) after a dt advance: dx_max = max_b |x_b - x_b(0)|,
@@ -412,7 +420,7 @@ __device__ inline float collapse_latch(const SSm& s, const Params& P, int env, b
     const float4 x = bd4(s, b, 0);
     if (x.w == 0.0f) continue;
     const float4 v = bd4(s, b, 1), w = bd4(s, b, 2);
-    ek += body_kinetic_energy(s, S, b, x, v, w, bd4(s, b, 4).z);
+    ek += body_kinetic_energy(s, S, b, x, v, w, bd4(s, b, 4));
     if (latch) {
       const float dx = x.x - ref[b], dy = x.y - ref[S + b], dz = x.z - ref[2 * S + b];
       dxm = fmaxf(dxm, sqrtf(dx * dx + dy * dy + dz * dz));
@@ -473,13 +481,30 @@ __device__ inline int2 store_cache(const SSm& s, const Params& P, int env, const
   return make_int2(nc, ng);
 }
 
+// L2 prefetch of what load_bodies / load_slots will read of env e (128-byte lines, lanes strided).
+__device__ inline void prefetch_env(const Params& P, const Scratch& L, int e) {
+  const int lane = lane_id();
+  const char* st = reinterpret_cast<const char*>(P.state + (size_t)e * kStateRows * P.S);
+  for (int o = 128 * lane; o < kStateRows * P.S * 4; o += 4096) prefetch_l2(st + o);
+  const char* pr = reinterpret_cast<const char*>(P.props + (size_t)e * kPropRows * P.S);
+  for (int o = 128 * lane; o < 4 * P.S * 4; o += 4096) prefetch_l2(pr + o);
+  const float* scr = P.scratch + (size_t)e * P.scratch_words;
+  const int nblk = reinterpret_cast<const int*>(scr + L.meta)[MetaNblk];
+  const char* hd = reinterpret_cast<const char*>(scr + L.hdr);
+  for (int f = 0; f < 2; ++f)
+    for (int o = 128 * lane; o < 32 * nblk * 16; o += 4096) prefetch_l2(hd + (size_t)f * 32 * P.nblk * 16 + o);
+  const char* cs = reinterpret_cast<const char*>(scr + L.cs);
+  for (int o = 128 * lane; o < nblk * kBlkWords * 4; o += 4096) prefetch_l2(cs + o);
+  prefetch_l2(scr + L.ph + 32 * (lane & 1));
+}
+
 // ---------------------------------------------------------------- the kernel
 // flags: bit 0 end of a dt step (latch, counters, rest test), bit 1 PGS only (jenga_pgs_solve: no integration, no cache),
 // bit 2 honour / update the per-env rest flag (jenga_simulate_until_rest).
 enum { SolveEndOfStep = 1, SolvePgsOnly = 2, SolveRest = 4 };
 
 template <bool TM>
-__global__ void __launch_bounds__(TM ? 384 : 32, 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
+__global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
   int env0;
   SSm s = begin_solve<TM>(P, env0);
   const int lane = lane_id();
@@ -487,12 +512,18 @@ __global__ void __launch_bounds__(TM ? 384 : 32, 1) k_solve(const Params P, cons
   // persistent: every warp takes the next env of a global queue (an atomic counter that k_collide reset): envs differ in
   // cost by the number of colliding pairs, so a static split would leave warps idle at the end.  TMEM is allocated once
   // per CTA; the warps of a CTA never wait for one another between envs.
+  // The queue is read one env ahead: while env e is solved, the state tile, the headers and the used constant blocks of
+  // the warp's next env are prefetched into L2 (they were written a whole batch ago, i.e. they come from HBM).
   (void)env0;
+  int env_next = 0;
+  if (lane == 0) env_next = atomicAdd(P.work_counter, 1);
+  env_next = __shfl_sync(kFull, env_next, 0);
   for (;;) {
-    int env = 0;
-    if (lane == 0) env = atomicAdd(P.work_counter, 1);
-    env = __shfl_sync(kFull, env, 0);
+    const int env = env_next;
     if (env >= P.E) break;
+    if (lane == 0) env_next = atomicAdd(P.work_counter, 1);
+    env_next = __shfl_sync(kFull, env_next, 0);
+    if (env_next < P.E) prefetch_env(P, L, env_next);
     float* scr = P.scratch + (size_t)env * P.scratch_words;
     int* meta = reinterpret_cast<int*>(scr + L.meta);
     if ((flags & SolveRest) && meta[MetaResting]) continue;

@@ -49,6 +49,49 @@ __global__ void __launch_bounds__(kThreads) k_ffma3(float* out, int outer) {
   out[(size_t)blockIdx.x * kThreads + threadIdx.x] = s;
 }
 
+// FFMAs whose three source registers all change from one instruction to the next (no operand-reuse hits): the shape of
+// the solver's cross products and matrix-vector products.  16 accumulators, 8 + 8 multiplicands per thread.
+__global__ void __launch_bounds__(kThreads) k_ffma_nr(float* out, int outer) {
+  float x[16], y[8], z[8];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) x[k] = (float)(threadIdx.x + k) * 1.0e-3f;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { y[k] = 0.999f + (float)(threadIdx.x + k) * 1.0e-7f; z[k] = 1.0e-3f + (float)(threadIdx.x * 8 + k) * 1.0e-9f; }
+  for (int it = 0; it < outer; ++it) {
+#pragma unroll
+    for (int j = 0; j < kInner / 2; ++j)
+#pragma unroll
+      for (int k = 0; k < 16; ++k) x[k] = fmaf(y[(k + j) & 7], z[(k + 3 * j + 1) & 7], x[k]);
+  }
+  float s = 0.0f;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += x[k];
+  out[(size_t)blockIdx.x * kThreads + threadIdx.x] = s;
+}
+
+// The packed form of sm_100 (fma.rn.f32x2, SASS FFMA2): two FMAs per thread per instruction on 64-bit register pairs, again
+// with no operand reuse.  Counted as two FP32 thread-instructions each.
+__global__ void __launch_bounds__(kThreads) k_ffma2_nr(float* out, int outer) {
+  float2 x[8], y[4], z[4];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) x[k] = make_float2((float)(threadIdx.x + k) * 1.0e-3f, (float)(threadIdx.x + k) * 2.0e-3f);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    y[k] = make_float2(0.999f + (float)(threadIdx.x + k) * 1.0e-7f, 0.998f + (float)(threadIdx.x + k) * 1.0e-7f);
+    z[k] = make_float2(1.0e-3f + (float)(threadIdx.x * 8 + k) * 1.0e-9f, 2.0e-3f + (float)(threadIdx.x * 8 + k) * 1.0e-9f);
+  }
+  for (int it = 0; it < outer; ++it) {
+#pragma unroll
+    for (int j = 0; j < kInner / 2; ++j)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = __ffma2_rn(y[(k + j) & 3], z[(k + 3 * j + 1) & 3], x[k]);
+  }
+  float s = 0.0f;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += x[k].x + x[k].y;
+  out[(size_t)blockIdx.x * kThreads + threadIdx.x] = s;
+}
+
 // Every lane reads consecutive 16-byte words (conflict-free LDS.128, 4 wavefronts of 128 B per instruction);
 // 8 loads in flight per thread per inner step; the sums keep the loads alive.
 __global__ void __launch_bounds__(kThreads) k_lds(float* out, int outer) {
@@ -73,7 +116,8 @@ __global__ void __launch_bounds__(kThreads) k_lds(float* out, int outer) {
 
 // out[0] = FP32 thread-instructions per second (FFMA, all SMs), out[1] = shared-memory bytes per second (LDS.128),
 // out[2] = SM count, out[3] = seconds of the FFMA run, out[4] = seconds of the LDS run, out[5] = FP32 thread-instructions
-// per second of the three-register-operand FFMA form.
+// per second of the three-register-operand FFMA form, out[6] = the same with three source registers that all change from
+// one instruction to the next (no operand-reuse hits).
 // `scratch` is a caller-owned device buffer of at least jenga_peaks_scratch_bytes(); the call synchronises the
 // stream (it is a measurement, not a step of the path).
 extern "C" size_t jenga_peaks_scratch_bytes(void) { return (size_t)148 * 8 * 8 * jenga_peaks::kThreads * sizeof(float); }
@@ -109,6 +153,24 @@ extern "C" int jenga_measure_peaks(double* out, void* scratch, void* cuda_stream
     float ms; cudaEventElapsedTime(&ms, e0, e1);
     if (rep && ms < ms_f3) ms_f3 = ms;
   }
+  float ms_nr = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, st);
+    k_ffma_nr<<<grid, kThreads, 0, st>>>(o, outer_f);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) return JENGA_E_CUDA;
+    float ms; cudaEventElapsedTime(&ms, e0, e1);
+    if (rep && ms < ms_nr) ms_nr = ms;
+  }
+  float ms_p2 = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, st);
+    k_ffma2_nr<<<grid, kThreads, 0, st>>>(o, outer_f);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) return JENGA_E_CUDA;
+    float ms; cudaEventElapsedTime(&ms, e0, e1);
+    if (rep && ms < ms_p2) ms_p2 = ms;
+  }
   const int grid_l = n_sm * 6;                                // 6 x 32 KB of shared memory per SM
   for (int rep = 0; rep < 4; ++rep) {
     cudaEventRecord(e0, st);
@@ -124,5 +186,7 @@ extern "C" int jenga_measure_peaks(double* out, void* scratch, void* cuda_stream
   const double n_bytes = (double)grid_l * kThreads * (double)outer_l * 8 * 16;
   out[0] = n_ffma / (ms_f * 1e-3); out[1] = n_bytes / (ms_l * 1e-3); out[2] = (double)n_sm;
   out[3] = ms_f * 1e-3; out[4] = ms_l * 1e-3; out[5] = n_ffma / (ms_f3 * 1e-3);
+  out[6] = n_ffma / (ms_nr * 1e-3);
+  out[7] = n_ffma / (ms_p2 * 1e-3);
   return JENGA_OK;
 }

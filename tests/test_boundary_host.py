@@ -47,7 +47,7 @@ def test_descriptor_validation_and_launch_shape(L):
     from paper_2606_28394_b200 import binding, workloads as W
     wp = W.make_config(2, n_envs=2).params
     d = binding.make_desc(wp)
-    assert L.jenga_block_threads(C.byref(d)) in (32, 128, 256, 384)   # one warp per env; 4, 8 or 12 envs per CTA in the TMEM tiers
+    assert L.jenga_block_threads(C.byref(d)) in (32, 128, 256, 384, 512)   # one warp per env; 4, 8, 12 or 16 envs per CTA in the TMEM tiers
     smem = L.jenga_smem_bytes(C.byref(d))
     assert 0 < smem <= 227 * 1024
     bad = binding.make_desc(wp); bad.body_stride = wp.n_bodies + 1          # not a multiple of 4

@@ -341,7 +341,7 @@ def test_solver_tiers_bit_identical(J, cfg, E):
     wl = W.make_config(cfg, n_envs=E)
     ref = None
     used = []
-    for tier in ("smem", "tmem160", "tmem256", "tmem512", "auto"):
+    for tier in ("smem", "tmem128", "tmem160", "tmem256", "tmem512", "auto"):
         try:
             w = J.World(wl.params, wl.state, wl.props, wl.mu, tier=tier)
         except J.JengaError:
@@ -574,7 +574,7 @@ def test_full_size_cfg5_sampled_envs(orc, J):
     E = 65536
     wl = W.make_config(5, n_envs=E)
     world = J.World(wl.params, wl.state, wl.props, wl.mu)
-    assert world.launch_info()["threads"] in (32, 128, 256, 384)
+    assert world.launch_info()["threads"] in (32, 128, 256, 384, 512)
     world.step(1); torch.cuda.synchronize()
     assert int(world.status.max().item()) == 0 and bool(torch.isfinite(world.state).all().item())
     cnt = world.counters_dict()
