@@ -121,7 +121,7 @@ typedef struct {
   float       *collapse_stats; /* [E][4] of the last step: dx_max [m], E_k [J], theta_max [rad], 0     */
   int32_t     *rest_steps; /* [E]  steps taken by the last jenga_simulate_until_rest; may be NULL      */
   void        *scratch;    /* jenga_scratch_bytes(desc) bytes, 16-byte aligned, ZERO-FILLED by the caller before the
-                              first call: the hand-off between the two kernels of a substep (pair headers, solver
+                              first call: the hand-off between the four kernels of a substep (pair headers, solver
                               constants and colour chunks of every env) plus per-env bookkeeping (the colouring of the
                               last pair list, the rest flag).  Contents are private to the library.              */
   size_t       scratch_bytes;

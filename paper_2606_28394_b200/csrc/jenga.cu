@@ -41,7 +41,7 @@ struct jenga_world {
   jenga_buffers bufs;
   Params P;
   int tmb;                 // TMEM blocks per env of k_solve: 5, 10 or 0 (no TMEM, 1 warp per CTA)
-  int wpc_collide;         // warps (= envs) per CTA of k_collide
+  int wpc_collide;         // warps (= envs) per CTA of the collision kernels
   int n_sm;
   size_t smem_solve;       // dynamic shared memory per CTA of k_solve
   size_t smem_collide;     // ... of k_detect
@@ -308,8 +308,9 @@ static int launch_solve(jenga_world* w, int iters, int flags, float rest_ek, cud
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_solve)");
   /* persistent CTAs: one per SM in the TMEM tiers (it owns all 512 columns), each warp strides over the envs */
   if (w->tmb) {
-    const int wpc = 4 * tier_groups(w->tmb), need = (w->P.E + wpc - 1) / wpc;
-    jenga::k_solve<true><<<need < w->n_sm ? need : w->n_sm, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
+    /* small batches are spread over all SMs (the warps of every CTA pull envs from the same queue) */
+    const int wpc = 4 * tier_groups(w->tmb), grid = w->P.E < w->n_sm ? w->P.E : w->n_sm;
+    jenga::k_solve<true><<<grid, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
   } else {
     const int per_sm = (int)(kSmemMax / (w->smem_solve + 1024)), resident = w->n_sm * (per_sm < 1 ? 1 : (per_sm > 16 ? 16 : per_sm));
     jenga::k_solve<false><<<w->P.E < resident ? w->P.E : resident, 32, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);

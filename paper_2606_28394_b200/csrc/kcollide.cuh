@@ -530,7 +530,7 @@ __device__ inline void colour_pairs(const CSm& s, const Params& P, float* scr, c
   unsigned short* gpos = reinterpret_cast<unsigned short*>(scr + L.pos);
   unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
   unsigned* gcab = reinterpret_cast<unsigned*>(scr + L.cab);
-  for (int r = lane; r < n_coll; r += 32) gcab[r] = s.cab[r];             // bodies + SAT axis of every pair, for k_setup
+  for (int r = lane; r < n_coll; r += 32) gcab[r] = s.cab[r];             // bodies + SAT axis of every pair, for k_manifold / k_slot
   bool same = meta[MetaMagic] == kMagic && meta[MetaNcoll] == n_coll;
   if (same)
     for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
@@ -882,7 +882,7 @@ __device__ inline void setup_given(const CSm& s, const Params& P, int env, float
 // mode: ModeStep (fused substep, first half), ModeBroad (jenga_broadphase), ModeNarrow (jenga_narrowphase),
 // ModeGiven (first half of jenga_pgs_solve).  honour_rest: envs whose scratch says "at rest" are skipped
 // (jenga_simulate_until_rest).
-// The colliding-pair list of this env from the scratch (k_detect wrote it) into the arena of k_setup.
+// The colliding-pair list of this env from the scratch (k_detect wrote it) into the arena of k_manifold / k_slot.
 __device__ inline int load_colliding(const CSm& s, const float* scr, const Scratch& L) {
   const int n_coll = reinterpret_cast<const int*>(scr + L.meta)[MetaNcoll];
   const unsigned* gcab = reinterpret_cast<const unsigned*>(scr + L.cab);

@@ -1,12 +1,12 @@
 // ksolve.cuh -- second kernel of a substep, one env per warp: S4 warm-start application, S5 coloured PGS sweeps,
-// S6 integration + Baumgarte, S7 warm-start cache, Eq. 18 latch.  Inputs: the state tile and the scratch k_collide wrote.
+// S6 integration + Baumgarte, S7 warm-start cache, Eq. 18 latch.  Inputs: the state tile and the scratch k_slot wrote.
 //
 // Two flavours (template <bool TM>):
 //   TM = true   ONE persistent CTA per SM of 4 G warps = 4 G envs in flight (G = 3, 2 or 1) that owns all 512 columns of
 //               tensor memory.  Warp w works in TMEM lanes 32 (w % 4) .. + 31 (its quadrant) and columns
 //               [48 tmb (w / 4), + 48 tmb): the 48 constant words of the positions of the env's first `tmb` 32-position
 //               blocks (tmb = 2, 3, 5, 10 for G = 4, 3, 2, 1; tcgen05.ld/st.32x32b: lane = position % 32, block j at column
-//               offset 48 j).  Blocks >= tmb stay where k_collide wrote them, in the scratch (L2-resident while the env is
+//               offset 48 j).  Blocks >= tmb stay where k_slot wrote them, in the scratch (L2-resident while the env is
 //               in flight): their visits load and store global memory, one visit ahead of use.
 //   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers; test coverage).
 #pragma once
@@ -509,7 +509,7 @@ __global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, cons
   SSm s = begin_solve<TM>(P, env0);
   const int lane = lane_id();
   const Scratch L = scratch_layout(P.pc);
-  // persistent: every warp takes the next env of a global queue (an atomic counter that k_collide reset): envs differ in
+  // persistent: every warp takes the next env of a global queue (an atomic counter that k_detect reset): envs differ in
   // cost by the number of colliding pairs, so a static split would leave warps idle at the end.  TMEM is allocated once
   // per CTA; the warps of a CTA never wait for one another between envs.
   // The queue is read one env ahead: while env e is solved, the state tile, the headers and the used constant blocks of

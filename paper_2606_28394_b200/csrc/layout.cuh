@@ -1,4 +1,4 @@
-// layout.cuh -- parameters, the global hand-off ("scratch") between the two kernels of a substep, and the shared
+// layout.cuh -- parameters, the global hand-off ("scratch") between the four kernels of a substep, and the shared
 // memory arenas of the batched Jenga step (sm_100a).
 //
 // A substep (S1..S7 of include/jenga.h) is FOUR kernels, all with ONE WARP PER ENV (every synchronisation inside an
@@ -37,7 +37,7 @@ constexpr int kMagic = 0x4a454e47;          // "JENG": scratch meta stamp of a v
 
 enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaWords = 16 };
 
-// k_collide modes
+// modes of the collision kernels
 enum { ModeStep = 0, ModeBroad = 1, ModeNarrow = 2, ModeGiven = 3 };
 
 struct Params {
@@ -55,7 +55,7 @@ struct Params {
   unsigned* status; unsigned long long* counters;
   const float* ref_pose; int* collapsed; float* collapse_stats; int* rest_steps;
   float collapse_dx, collapse_ek, collapse_theta;           // f_d * l, eps_k, theta_th
-  int* work_counter;                                        // next env of the running k_solve (reset by every k_collide)
+  int* work_counter;                                        // next env of the running k_solve (reset by every k_detect)
   float* scratch; long long scratch_words;                  // per env (the first kScratchHead words of the buffer are global)
 };
 
