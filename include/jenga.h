@@ -77,8 +77,9 @@ typedef struct {
   int32_t  warm_start;                  /* 1: carry (jn,jt1,jt2) between steps                         */
   int32_t  gyroscopic;                  /* 1: add -h Iw^-1 (w x Iw w) in S1 (Eq. 4); default 0         */
   int32_t  max_pairs;                   /* candidate-pair capacity per env                             */
-  int32_t  max_contacts;                /* contact capacity per env; colliding pairs <= max_contacts/4;
-                                           32 <= max_contacts/4 <= 512                                 */
+  int32_t  max_contacts;                /* contact capacity per env, a multiple of 4 in 4..65532; colliding pairs <=
+                                           max_contacts/4.  Sizes whose per-env shared-memory arenas exceed 227 KB
+                                           are rejected (jenga_scratch_bytes / jenga_smem_bytes return 0)       */
   int32_t  materialise;                 /* 1: jenga_step also writes pairs/contacts/lambda of its last
                                            substep (debug / parity); 0: they stay on chip              */
   int32_t  device;                      /* CUDA device ordinal the buffers live on                     */
