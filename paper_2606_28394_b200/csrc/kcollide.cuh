@@ -942,7 +942,7 @@ __global__ void __launch_bounds__(128, 4) k_detect(const Params P, const int hon
 }
 
 template <int mode>
-__global__ void __launch_bounds__(128, 4) k_manifold(const Params P, const int honour_rest) {
+__global__ void __launch_bounds__(128, 5) k_manifold(const Params P, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
   const int env = blockIdx.x * wpc + warp;
   if (env >= P.E) return;

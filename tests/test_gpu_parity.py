@@ -902,6 +902,30 @@ def test_in_rollout_block_removal(orc, J):
 
 
 
+# ----------------------------------------------------------------------------- measurement aids of the C-ABI
+def test_measured_peaks_and_kernel_timers(J):
+    """jenga_measure_peaks: the FP32 issue rate and the LDS bandwidth of the device are within 10 % of the B200's nominal
+    148 x 128 lanes x clock, and a FFMA stream without operand reuse is slower than one with.  jenga_profile_*: every
+    substep of jenga_step is timed kernel by kernel on the caller's stream."""
+    import torch
+    pk = J.jenga_measure_peaks()
+    mhz = torch.cuda.clock_rate() / 1e3 if hasattr(torch.cuda, "clock_rate") else 1965.0
+    nominal = pk["n_sm"] * 128 * 1.965e9
+    assert pk["n_sm"] == 148 and 0.80 * nominal < pk["fp32_instr_per_s"] < 1.05 * nominal
+    assert 0.80 * nominal < pk["smem_bytes_per_s"] < 1.05 * nominal
+    assert 0.4 * pk["fp32_instr_per_s"] < pk["fp32_instr_per_s_noreuse"] < 0.9 * pk["fp32_instr_per_s"]
+    wl = W.make_config(6, n_envs=64)                               # 3 substeps per step
+    world = J.World(wl.params, wl.state, wl.props, wl.mu)
+    world.jenga_profile_enable(True)
+    world.step(2); world.step(1)
+    t = world.jenga_profile_read()
+    assert t["substeps"] == 9 and min(t["detect_ms"], t["manifold_ms"], t["slot_ms"], t["solve_ms"]) > 0.0
+    assert world.jenga_profile_read()["substeps"] == 0              # read drops the events
+    world.jenga_profile_enable(False)
+    world.step(1); torch.cuda.synchronize()
+    assert world.counters_dict()["env_steps"] == 64 * 4
+
+
 # ----------------------------------------------------------------------------- north_star's rollout bar, as stated (kept LAST in the file)
 @pytest.mark.xfail(strict=False, reason="north_star's raw bar: towers at their own stability limit flip under any rounding-level change; the "
                                         "fp64 oracle disagrees with itself at the same rate (DESIGN.md §6)")
