@@ -85,12 +85,14 @@ typedef struct {
   int32_t  device;                      /* CUDA device ordinal the buffers live on                     */
   float    collapse_length;             /* block length l of Eq. 18; latch off if <= 0 */
   float    collapse_fd, collapse_ek, collapse_theta;   /* f_d = 0.5, eps_k = 5e-5 J, theta_th = 30 deg in rad   */
-  int32_t  solver_tier;                 /* where the PGS kernel keeps the contact constants: 0 = auto (the most envs in
-                                           flight per SM that fit), 1 = shared memory only (one warp per CTA);
-                                           tensor memory, one CTA per SM owning its 512 columns: 4 = 12 envs in flight with
-                                           3 blocks of 32 pairs each in TMEM, 2 = 8 envs with 5 blocks, 3 = 4 envs with 10
-                                           blocks (further blocks are served from the L2-resident scratch).  A tier that
-                                           does not fit the sizes is JENGA_E_ARG.                                     */
+  int32_t  solver_tier;                 /* where the PGS kernel keeps the contact constants.  0 = auto: the most envs in
+                                           flight per SM that fit, or, for a batch that does not fill 148 SMs, the tier
+                                           with the fewest envs per SM that still holds the batch at once (n_envs <= 592:
+                                           tier 1).  1 = shared memory only (one warp per CTA).  Tensor memory, one CTA per
+                                           SM owning its 512 columns: 5 = 16 envs in flight with 2 blocks of 32 pairs each
+                                           in TMEM, 4 = 12 envs with 3 blocks, 2 = 8 envs with 5 blocks, 3 = 4 envs with 10
+                                           blocks (further blocks are served from the L2-resident scratch).  Every tier
+                                           computes the same bits.  A tier that does not fit the sizes is JENGA_E_ARG. */
 } jenga_world_desc;
 
 /* All DEVICE pointers, caller-owned, 16-byte aligned.  PC = max_contacts/4. */

@@ -35,6 +35,7 @@ using jenga::Params;
 
 enum { TierAuto = 0, TierSmem = 1, TierTmem256 = 2, TierTmem512 = 3, TierTmem160 = 4, TierTmem128 = 5 };
 static const size_t kSmemMax = 227 * 1024;
+static const int kSmNominal = 148;     /* SMs of a B200: used by the tier heuristic only (helpers answer without a device) */
 
 struct jenga_world {
   jenga_world_desc desc;
@@ -89,7 +90,17 @@ static int pick_tmb(const jenga_world_desc* d) {
     case TierTmem160: return tier_fits(d, 3) ? 3 : -1;
     case TierTmem256: return tier_fits(d, 5) ? 5 : -1;
     case TierTmem512: return tier_fits(d, 10) ? 10 : -1;
-    default: return tier_fits(d, 2) ? 2 : (tier_fits(d, 3) ? 3 : (tier_fits(d, 5) ? 5 : (tier_fits(d, 10) ? 10 : 0)));
+    default: {
+      /* auto.  A batch that does not fill the machine (148 SMs x 4 G envs in flight) takes the tier with the fewest envs
+         per SM that still holds it at once: more of every env's constant blocks are then in tensor memory, and below
+         4 envs per SM the shared-memory tier (lowest latency per chunk visit) is the quickest.  All tiers give the same bits. */
+      const long long E = d->n_envs;
+      if (E <= 4ll * kSmNominal && solve_env_bytes(d, 0) + 1024 <= kSmemMax) return 0;
+      const int by_size[3] = { 10, 5, 3 };
+      for (int k = 0; k < 3; ++k)
+        if (E <= 4ll * tier_groups(by_size[k]) * kSmNominal && tier_fits(d, by_size[k])) return by_size[k];
+      return tier_fits(d, 2) ? 2 : (tier_fits(d, 3) ? 3 : (tier_fits(d, 5) ? 5 : (tier_fits(d, 10) ? 10 : 0)));
+    }
   }
 }
 

@@ -10,7 +10,8 @@ namespace jenga {
 
 // ---------------------------------------------------------------- shared-memory arena of one env
 struct CSm {
-  SP<float> cb;                 // [S][kCb] collision body records
+  SP<float> cb;                 // [S][cbw] collision body records: x y z im | a0 h0 | a1 h1 | a2 h2 | then q (k_detect) or Iw^-1 (k_slot)
+  int cbw;                      // words per record: 20 (k_detect, k_manifold) or kCb = 28 (k_slot); a multiple of 4, odd in float4
   SP<float4> ext;               // [S]      world AABB half extents e'_x e'_y e'_z, flags (1 active | 2 dynamic)
   SP<unsigned> hitw;            // [ceil(S/32)][32] broadphase hit words of the current block of 32 rows; ALIASES used
   SP<unsigned long long> used;  // [S]      colour masks per body
@@ -36,10 +37,12 @@ enum { ArenaDetect = 0, ArenaManifold = 1, ArenaSlot = 2 };
 // k_detect: records, extents, masks / hit words, candidate list, colliding list, colouring products.
 // k_manifold: records, colliding list (copied from the scratch), per-lane clip polygons.  k_slot: records, colliding
 // list, cache keys.
+__host__ __device__ inline int cb_words(int arena) { return arena == ArenaSlot ? kCb : 20; }
+
 __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc, int arena) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc);
-  size_t w = (size_t)kCb * S + pcA;                        // cb, cab
-  w += 3 * (size_t)(pcA / 2);                              // cpair, pos, wrank
+  size_t w = (size_t)cb_words(arena) * S + pcA + pcA / 2;  // cb, cab, cpair
+  if (arena != ArenaManifold) w += 2 * (size_t)(pcA / 2);  // pos, wrank
   if (arena == ArenaDetect) {
     const int uh = 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
     w += 4 * S + uh + mpA / 2 + pcA / 4;                   // ext, used / hitw, cand, colour
@@ -56,11 +59,12 @@ __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int p
 __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int arena) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc), phw = round_up(ph_max(nblk), 4);
   CSm s; int p = base;
-  s.cb.off = p;     p += kCb * S;
+  s.cbw = cb_words(arena);
+  s.cb.off = p;     p += s.cbw * S;
   s.cab.off = p;    p += pcA;
   s.cpair.off = p;  p += pcA / 2;
-  s.pos.off = p;    p += pcA / 2;
-  s.wrank.off = p;  p += pcA / 2;
+  s.pos.off = s.wrank.off = 0;
+  if (arena != ArenaManifold) { s.pos.off = p; p += pcA / 2; s.wrank.off = p; p += pcA / 2; }
   // the arrays of the other arena get offset 0 (never touched by this kernel)
   s.ext.off = s.hitw.off = s.used.off = s.cand.off = s.colour.off = s.ph.off = s.chc.off = 0;
   s.ccount.off = s.cfirst.off = s.fill.off = s.misc.off = s.cprev.off = s.poly.off = 0;
@@ -85,7 +89,7 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int 
 
 __device__ __forceinline__ Vec3 xyz(float4 v) { return v3(v.x, v.y, v.z); }
 __device__ __forceinline__ Vec3 xyz4(float4 v) { return v3(v.x, v.y, v.z); }
-__device__ __forceinline__ float4& cb4(const CSm& s, int b, int k) { return reinterpret_cast<float4*>(smem_f + s.cb.off + b * kCb)[k]; }
+__device__ __forceinline__ float4& cb4(const CSm& s, int b, int k) { return reinterpret_cast<float4*>(smem_f + s.cb.off + b * s.cbw)[k]; }
 
 __device__ __forceinline__ Box load_box(const CSm& s, int b) {
   Box X;
@@ -122,9 +126,12 @@ __device__ inline void load_predict(const CSm& s, const Params& P, int env, bool
     cb4(s, b, 1) = make_float4(R[0], R[3], R[6], hx);        // body axis k = column k of R
     cb4(s, b, 2) = make_float4(R[1], R[4], R[7], hy);
     cb4(s, b, 3) = make_float4(R[2], R[5], R[8], hz);
-    cb4(s, b, 4) = make_float4(I6[0], I6[1], I6[2], I6[3]);
-    cb4(s, b, 5) = make_float4(I6[4], I6[5], act ? 1.0f : 0.0f, dyn ? 1.0f : 0.0f);
-    cb4(s, b, 6) = make_float4(w, x, y, z);
+    if (s.cbw == kCb) {                                      // k_slot: the effective masses need Iw^-1
+      cb4(s, b, 4) = make_float4(I6[0], I6[1], I6[2], I6[3]);
+      cb4(s, b, 5) = make_float4(I6[4], I6[5], 0.0f, 0.0f);
+    } else if (want_ext) {
+      cb4(s, b, 4) = make_float4(w, x, y, z);                // k_detect: the fp64 re-check of threshold AABB tests
+    }
     if (!predict || !dyn) continue;
     float f[6] = { 0, 0, 0, 0, 0, 0 };
     if (P.f_ext) {
@@ -166,7 +173,7 @@ __device__ __forceinline__ int warp_excl_scan(int v, int* total) {
 #define DA(a, b) __dadd_rn((a), (b))
 #define DS(a, b) __dsub_rn((a), (b))
 __device__ __noinline__ void ext_f64(const CSm& s, int b, double* e3) {
-  const float4 q4 = cb4(s, b, 6);
+  const float4 q4 = cb4(s, b, 4);
   const double w = q4.x, x = q4.y, y = q4.z, z = q4.w;
   const double hx = cb4(s, b, 1).w, hy = cb4(s, b, 2).w, hz = cb4(s, b, 3).w;
   double R[9];
@@ -212,7 +219,7 @@ __device__ inline int broadphase(const CSm& s, const Params& P, unsigned* status
   for (int base = 0; base < B; base += 32) {               // ground: pair index = b
     const int j = base + lane;
     bool hit = false;
-    if (j < B && cb4(s, j, 5).w != 0.0f) {
+    if (j < B && cb4(s, j, 0).w != 0.0f) {
       const float sl = eps - (cb4(s, j, 0).z - s.ext[j].z);
       hit = sl >= 0.0f;
       if (fabsf(sl) < 1.0e-5f) hit = aabb_test_f64(s, P, -1, j);
@@ -485,7 +492,7 @@ __device__ inline void collide_ground(const Box& b, int pb, Manifold& m) {
 // Manifold of colliding pair (a, b) whose SAT axis is known (find_colliding stored it).
 __device__ __forceinline__ void pair_manifold(const CSm& s, int a, int b, int axis, Manifold& m) {
   if (a < 0) { collide_ground(load_box(s, b), s.poly.off + lane_id(), m); return; }
-  const int oA = s.cb.off + a * kCb, oB = s.cb.off + b * kCb;
+  const int oA = s.cb.off + a * s.cbw, oB = s.cb.off + b * s.cbw;
   SatResult sr; sat_axis(oA, oB, axis, sr);
   manifold_boxes(oA, oB, sr, s.poly.off + lane_id(), m);
 }
@@ -883,12 +890,15 @@ __device__ inline void setup_given(const CSm& s, const Params& P, int env, float
 // ModeGiven (first half of jenga_pgs_solve).  honour_rest: envs whose scratch says "at rest" are skipped
 // (jenga_simulate_until_rest).
 // The colliding-pair list of this env from the scratch (k_detect wrote it) into the arena of k_manifold / k_slot.
-__device__ inline int load_colliding(const CSm& s, const float* scr, const Scratch& L) {
+__device__ inline int load_colliding(const CSm& s, const float* scr, const Scratch& L, bool want_pos) {
   const int n_coll = reinterpret_cast<const int*>(scr + L.meta)[MetaNcoll];
   const unsigned* gcab = reinterpret_cast<const unsigned*>(scr + L.cab);
   const unsigned short* gpos = reinterpret_cast<const unsigned short*>(scr + L.pos);
   const unsigned short* gpair = reinterpret_cast<const unsigned short*>(scr + L.cpair);
-  for (int r = lane_id(); r < n_coll; r += 32) { s.cab[r] = gcab[r]; s.pos[r] = gpos[r]; s.cpair[r] = gpair[r]; }
+  for (int r = lane_id(); r < n_coll; r += 32) {
+    s.cab[r] = gcab[r]; s.cpair[r] = gpair[r];
+    if (want_pos) s.pos[r] = gpos[r];
+  }
   __syncwarp();
   return n_coll;
 }
@@ -898,7 +908,7 @@ __device__ inline int load_colliding(const CSm& s, const float* scr, const Scrat
 // ModeGiven (first half of jenga_pgs_solve: the caller's contact list instead of the narrowphase).  honour_rest: envs whose
 // scratch says "at rest" are skipped (jenga_simulate_until_rest).
 template <int mode>
-__global__ void __launch_bounds__(128, 4) k_detect(const Params P, const int honour_rest) {
+__global__ void __launch_bounds__(128, 5) k_detect(const Params P, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
   const int env = blockIdx.x * wpc + warp;
   if (blockIdx.x == 0 && threadIdx.x == 0) *P.work_counter = 0;      // k_solve of this substep starts its env queue at 0
@@ -951,7 +961,7 @@ __global__ void __launch_bounds__(128, 5) k_manifold(const Params P, const int h
   if (honour_rest && reinterpret_cast<int*>(scr + L.meta)[MetaResting]) return;
   const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaManifold), ArenaManifold);
   load_predict(s, P, env, false, false);                                 // the records again (k_detect changed v, w only)
-  const int n_coll = load_colliding(s, scr, L);
+  const int n_coll = load_colliding(s, scr, L, false);
   manifold_pairs(s, P, env, scr, L, n_coll, mode == ModeNarrow || P.materialise);
 }
 
@@ -966,7 +976,7 @@ __global__ void __launch_bounds__(128, 4) k_slot(const Params P, const int honou
   if (honour_rest && meta[MetaResting]) return;
   const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaSlot), ArenaSlot);
   load_predict(s, P, env, false, false);
-  const int n_coll = load_colliding(s, scr, L);
+  const int n_coll = load_colliding(s, scr, L, true);
   const int nprev = load_prev_keys(s, P, env);
   if (mode == ModeGiven) setup_given(s, P, env, scr, L, n_coll, meta[MetaNcont], nprev);
   else setup_pairs(s, P, env, scr, L, n_coll, nprev);

@@ -514,9 +514,12 @@ __global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, cons
   // per CTA; the warps of a CTA never wait for one another between envs.
   // The queue is read one env ahead: while env e is solved, the state tile, the headers and the used constant blocks of
   // the warp's next env are prefetched into L2 (they were written a whole batch ago, i.e. they come from HBM).
+  // A batch smaller than the machine (E < warps in the grid) is spread evenly: only the first ceil(E / CTAs) warps of
+  // every CTA draw from the queue, so that no SM solves 16 envs while others idle.
   (void)env0;
-  int env_next = 0;
-  if (lane == 0) env_next = atomicAdd(P.work_counter, 1);
+  const bool draws = (int)(threadIdx.x >> 5) < (P.E + (int)gridDim.x - 1) / (int)gridDim.x;
+  int env_next = P.E;
+  if (draws && lane == 0) env_next = atomicAdd(P.work_counter, 1);
   env_next = __shfl_sync(kFull, env_next, 0);
   for (;;) {
     const int env = env_next;

@@ -27,7 +27,7 @@ namespace jenga {
 constexpr int kStateRows = 13, kPropRows = 8, kFextRows = 6;
 constexpr int kMaxColours = 64;
 constexpr int kBd = 20;        // solver body record (floats): x y z im | vx vy vz - | wx wy wz - | Ixx Ixy Ixz Iyy | Iyz Izz - -
-constexpr int kCb = 28;        // collision body record: x y z im | a0.xyz h0 | a1.xyz h1 | a2.xyz h2 | Ixx Ixy Ixz Iyy | Iyz Izz act dyn | pad 4
+constexpr int kCb = 28;        // collision body record of k_slot: x y z im | a0.xyz h0 | a1.xyz h1 | a2.xyz h2 | Ixx Ixy Ixz Iyy | Iyz Izz - - | pad 4 (k_detect, k_manifold: 20 words, kcollide.cuh)
 constexpr int kHdrF4 = 3;      // float4 per pair header: (ab, meta, rank, 1/|t1 raw|), (n.xyz, Baumgarte corr), (t1.xyz, 0)
 constexpr int kCsF4 = 12;      // float4 of contact constants per pair: 36 read-only words + 12 impulses
 constexpr int kBlkWords = kCsF4 * 4 * 32;   // words of one 32-position constant block in the scratch / shared tier
