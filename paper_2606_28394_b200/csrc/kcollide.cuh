@@ -722,7 +722,14 @@ __device__ inline void setup_slot(const CSm& s, const Params& P, int env, float*
   hdr[npos + k] = make_float4(n.x, n.y, n.z, im > 0.0f ? P.beta * fmaxf(0.0f, dmax - P.slop) / im : 0.0f);
   hdr[2 * npos + k] = make_float4(F.t1.x, F.t1.y, F.t1.z, 0.0f);
   const float e1 = 1.0f + P.restitution;
+  // the 12 float4 of the pair are stored as soon as their words are complete (the impulses first), so that the whole
+  // record is never live in registers at once
+  float4* cs = reinterpret_cast<float4*>(scr + L.cs) + (size_t)(k >> 5) * (kCsF4 * 32) + (k & 31);
   PairC out;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) { out.v[kLam + 3 * c] = lam[c][0]; out.v[kLam + 3 * c + 1] = lam[c][1]; out.v[kLam + 3 * c + 2] = lam[c][2]; }
+#pragma unroll
+  for (int f = kLam / 4; f < kCsF4; ++f) cs[f * 32] = make_float4(out.v[4 * f], out.v[4 * f + 1], out.v[4 * f + 2], out.v[4 * f + 3]);
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     float ik[3] = { 0, 0, 0 }, ko[3] = { 0, 0, 0 };
@@ -743,11 +750,9 @@ __device__ inline void setup_slot(const CSm& s, const Params& P, int env, float*
     }
     float* o = out.v + 9 * c;
     o[0] = pt[c].x; o[1] = pt[c].y; o[2] = pt[c].z; o[3] = ik[0]; o[4] = ik[1]; o[5] = ik[2]; o[6] = ko[0]; o[7] = ko[1]; o[8] = ko[2];
-    out.v[kLam + 3 * c] = lam[c][0]; out.v[kLam + 3 * c + 1] = lam[c][1]; out.v[kLam + 3 * c + 2] = lam[c][2];
-  }
-  float4* cs = reinterpret_cast<float4*>(scr + L.cs) + (size_t)(k >> 5) * (kCsF4 * 32) + (k & 31);
 #pragma unroll
-  for (int f = 0; f < kCsF4; ++f) cs[f * 32] = make_float4(out.v[4 * f], out.v[4 * f + 1], out.v[4 * f + 2], out.v[4 * f + 3]);
+    for (int f = 9 * c / 4; f < 9 * (c + 1) / 4; ++f) cs[f * 32] = make_float4(out.v[4 * f], out.v[4 * f + 1], out.v[4 * f + 2], out.v[4 * f + 3]);
+  }
 }
 
 // The warm-start cache's pair list (ascending) into shared memory.
@@ -966,7 +971,7 @@ __global__ void __launch_bounds__(128, 5) k_manifold(const Params P, const int h
 }
 
 template <int mode>
-__global__ void __launch_bounds__(128, 4) k_slot(const Params P, const int honour_rest) {
+__global__ void __launch_bounds__(128, 2) k_slot(const Params P, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
   const int env = blockIdx.x * wpc + warp;
   if (env >= P.E) return;

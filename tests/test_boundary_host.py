@@ -50,6 +50,12 @@ def test_descriptor_validation_and_launch_shape(L):
     assert L.jenga_block_threads(C.byref(d)) in (32, 128, 256, 384, 512)   # one warp per env; 4, 8, 12 or 16 envs per CTA in the TMEM tiers
     smem = L.jenga_smem_bytes(C.byref(d))
     assert 0 < smem <= 227 * 1024
+    # auto tier by batch size: a batch that does not fill 148 SMs runs fewer envs per SM (header, solver_tier)
+    shape = {}
+    for E in (2, 592, 593, 1184, 1185, 1776, 1777, 65536):
+        de = binding.make_desc(wp); de.n_envs = E
+        shape[E] = L.jenga_block_threads(C.byref(de))
+    assert shape == {2: 32, 592: 32, 593: 256, 1184: 256, 1185: 384, 1776: 384, 1777: 512, 65536: 512}
     bad = binding.make_desc(wp); bad.body_stride = wp.n_bodies + 1          # not a multiple of 4
     assert L.jenga_smem_bytes(C.byref(bad)) == 0 and L.jenga_block_threads(C.byref(bad)) == 0
     bad = binding.make_desc(wp); bad.struct_size = 4
