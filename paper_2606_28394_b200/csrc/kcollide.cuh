@@ -593,6 +593,20 @@ __device__ inline void colour_pairs(const CSm& s, const Params& P, float* scr, c
   }
   __syncwarp();
   const int nph = s.misc[MiNph];
+  // Blocks are renumbered by the number of chunks they hold (= solver visits per sweep), most first: the first blocks
+  // are the ones k_solve keeps in tensor memory, the rest are used in place in the L2-resident scratch.  Lane j = block j.
+  if (const int top = s.misc[MiNblk]; top > 1 && top <= 32) {
+    int cj = 0;
+    for (int i = 0; i < nph; ++i) cj += (s.ph[i] >> 16) == lane ? 1 : 0;
+    int id = 0;
+    for (int k = 0; k < top; ++k) { const int ck = __shfl_sync(kFull, cj, k); id += (ck > cj || (ck == cj && k < lane)) ? 1 : 0; }
+    for (int base = 0; base < nph; base += 32) {            // lane = chunk
+      const int i = base + lane, d = i < nph ? s.ph[i] : 0;
+      const int nid = __shfl_sync(kFull, id, (d >> 16) & 31);
+      if (i < nph) s.ph[i] = (d & 0xffff) | (nid << 16);
+    }
+    __syncwarp();
+  }
   for (int r = lane; r < n_coll; r += 32) {
     const int c = s.colour[r], w = s.wrank[r];
     int j = s.cfirst[c], k = 0;
