@@ -240,7 +240,7 @@ def run_cuda(args) -> dict:
     if args.max_pairs:
         wp.max_pairs = args.max_pairs
     K = min(args.steps, wl.n_steps) if args.steps > 0 else wl.n_steps
-    world = binding.World(wp, wl.state, wl.props, wl.mu, device=local, tier=args.tier)
+    world = binding.World(wp, wl.state, wl.props, wl.mu, device=local, tier=args.tier, group=args.group)
     state0 = world.state.clone()
     fext_dev = torch.as_tensor(wl.push_fext).to(dev)
     fext_ptr = binding.C.c_void_p(fext_dev.data_ptr())
@@ -310,7 +310,7 @@ def run_cuda(args) -> dict:
     parts = []
     for lo, hi in bounds:
         wpi = W.WorldParams(**{**wp.__dict__, "n_envs": hi - lo})
-        wi = binding.World(wpi, wl.state[lo:hi], wl.props[lo:hi], wl.mu[lo:hi], device=local, tier=args.tier)
+        wi = binding.World(wpi, wl.state[lo:hi], wl.props[lo:hi], wl.mu[lo:hi], device=local, tier=args.tier, group=args.group)
         h_a = torch.empty(wi.state.shape, dtype=torch.float32, pin_memory=True)
         h_b = torch.empty_like(h_a, pin_memory=True)
         h_a.copy_(torch.as_tensor(wl.state[lo:hi]))
@@ -403,7 +403,8 @@ def run_cuda(args) -> dict:
         "status": {"or": status_or, "envs_flagged": n_flagged},
         "maxima": {k: cnt[k] for k in ("max_candidates", "max_colliding", "max_colours")},
         "capacity": {"max_pairs": wp.max_pairs, "max_contacts": wp.max_contacts, "smem_bytes_per_cta": linfo["smem_bytes"],
-                     "threads_per_cta": linfo["threads"], "envs_in_flight_per_sm": linfo["threads"] // 32},
+                     "threads_per_cta": linfo["threads"], "envs_per_warp": linfo["env_group"],
+                     "envs_in_flight_per_sm": linfo["threads"] // 32 * linfo["env_group"]},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke,
                 "split": n_split, "launches": e2e_launches},
@@ -441,6 +442,7 @@ def main():
     ap.add_argument("--e2e-split", type=int, default=2, help="worlds (streams) the e2e leg serves the batch with")
     ap.add_argument("--cfg", type=int, default=CFG, help="BASELINE.json config number (5 = the bench workload; others: manual runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--group", type=int, default=0, choices=[0, 1, 2], help="envs per k_solve warp (0 = auto)")
     ap.add_argument("--tier", default="auto", choices=["auto", "smem", "tmem128", "tmem160", "tmem256", "tmem512"], help="where k_solve keeps the contact constants")
     ap.add_argument("--max-contacts", type=int, default=0, help="override the workload's contact capacity per env")
     ap.add_argument("--max-pairs", type=int, default=0, help="override the workload's candidate capacity per env")

@@ -85,14 +85,19 @@ typedef struct {
   int32_t  device;                      /* CUDA device ordinal the buffers live on                     */
   float    collapse_length;             /* block length l of Eq. 18; latch off if <= 0 */
   float    collapse_fd, collapse_ek, collapse_theta;   /* f_d = 0.5, eps_k = 5e-5 J, theta_th = 30 deg in rad   */
-  int32_t  solver_tier;                 /* where the PGS kernel keeps the contact constants.  0 = auto: the most envs in
+  int32_t  solver_tier;                 /* where the PGS kernel keeps the contact constants.  0 = auto: the most groups in
                                            flight per SM that fit, or, for a batch that does not fill 148 SMs, the tier
-                                           with the fewest envs per SM that still holds the batch at once (n_envs <= 592:
+                                           with the fewest groups per SM that still holds the batch at once (<= 592 groups:
                                            tier 1).  1 = shared memory only (one warp per CTA).  Tensor memory, one CTA per
-                                           SM owning its 512 columns: 5 = 16 envs in flight with 2 blocks of 32 pairs each
-                                           in TMEM, 4 = 12 envs with 3 blocks, 2 = 8 envs with 5 blocks, 3 = 4 envs with 10
-                                           blocks (further blocks are served from the L2-resident scratch).  Every tier
+                                           SM owning its 512 columns: 5 = 16 groups in flight with 2 blocks of 32 pairs each
+                                           in TMEM, 4 = 12 groups with 3 blocks, 2 = 8 groups with 4 blocks, 3 = 4 groups with
+                                           9 blocks (further blocks are served from the L2-resident scratch).  Every tier
                                            computes the same bits.  A tier that does not fit the sizes is JENGA_E_ARG. */
+  int32_t  env_group;                   /* envs per warp of the PGS kernel (a "group"): 1, 2, or 0 = auto (2 when
+                                           n_envs >= 4736 = 2 x 16 x 148, so that the batch still fills every SM).  With 2,
+                                           a solver visit takes pairs of the current colour of BOTH envs (they share no
+                                           body), so the warp's 32 lanes are filled better; each env's Gauss-Seidel order,
+                                           and so its result, is the canonical one bit for bit whatever the grouping.    */
 } jenga_world_desc;
 
 /* All DEVICE pointers, caller-owned, 16-byte aligned.  PC = max_contacts/4. */
@@ -124,9 +129,9 @@ typedef struct {
   float       *collapse_stats; /* [E][4] of the last step: dx_max [m], E_k [J], theta_max [rad], 0     */
   int32_t     *rest_steps; /* [E]  steps taken by the last jenga_simulate_until_rest; may be NULL      */
   void        *scratch;    /* jenga_scratch_bytes(desc) bytes, 16-byte aligned, ZERO-FILLED by the caller before the
-                              first call: the hand-off between the four kernels of a substep (pair headers, solver
-                              constants and colour chunks of every env) plus per-env bookkeeping (the colouring of the
-                              last pair list, the rest flag).  Contents are private to the library.              */
+                              first call: the hand-off between the four kernels of a substep (solver constants,
+                              pair headers and visit chunks of every group of envs) plus per-env bookkeeping (the
+                              colouring of the last pair list, the rest flag).  Contents are private to the library. */
   size_t       scratch_bytes;
 } jenga_buffers;
 
@@ -190,8 +195,11 @@ int jenga_world_destroy(jenga_world *w);
 /* Dynamic shared memory per CTA of the PGS kernel for this descriptor (0 if invalid). */
 size_t jenga_smem_bytes(const jenga_world_desc *desc);
 
-/* Threads per CTA of the PGS kernel (one warp per env: 128 = 4 envs per CTA in the tensor-memory tiers, 32 else). */
+/* Threads per CTA of the PGS kernel (one warp per group of envs: 128 Q threads in the tensor-memory tiers, 32 else). */
 int jenga_block_threads(const jenga_world_desc *desc);
+
+/* Envs per warp of the PGS kernel that this descriptor gets (desc.env_group, or what auto chooses; 0 if invalid). */
+int jenga_env_group(const jenga_world_desc *desc);
 
 /* Size of jenga_buffers.scratch for this descriptor (0 if invalid). */
 size_t jenga_scratch_bytes(const jenga_world_desc *desc);

@@ -34,7 +34,7 @@ class WorldDesc(C.Structure):
                 ("match_tol", C.c_float), ("warm_start", C.c_int32), ("gyroscopic", C.c_int32), ("max_pairs", C.c_int32),
                 ("max_contacts", C.c_int32), ("materialise", C.c_int32), ("device", C.c_int32),
                 ("collapse_length", C.c_float), ("collapse_fd", C.c_float), ("collapse_ek", C.c_float), ("collapse_theta", C.c_float),
-                ("solver_tier", C.c_int32)]
+                ("solver_tier", C.c_int32), ("env_group", C.c_int32)]
 
 
 class Buffers(C.Structure):
@@ -69,6 +69,7 @@ def lib():
         L.jenga_smem_bytes.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_smem_bytes.restype = C.c_size_t
         L.jenga_block_threads.argtypes = [C.POINTER(WorldDesc)]
+        L.jenga_env_group.argtypes = [C.POINTER(WorldDesc)]
         L.jenga_support_margin.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.jenga_ziglar_block_analysis.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.jenga_profile_enable.argtypes = [C.c_void_p, C.c_int]
@@ -81,7 +82,7 @@ def lib():
         L.jenga_peaks_scratch_bytes.restype = C.c_size_t
         L.jenga_strerror.restype = C.c_char_p
         for f in ("jenga_world_create", "jenga_world_destroy", "jenga_broadphase", "jenga_narrowphase", "jenga_pgs_solve",
-                  "jenga_step", "jenga_step_host", "jenga_simulate_until_rest", "jenga_set_f_ext", "jenga_block_threads",
+                  "jenga_step", "jenga_step_host", "jenga_simulate_until_rest", "jenga_set_f_ext", "jenga_block_threads", "jenga_env_group",
                   "jenga_profile_enable", "jenga_profile_read", "jenga_support_margin", "jenga_ziglar_block_analysis"):
             getattr(L, f).restype = C.c_int
         _lib = L
@@ -93,7 +94,7 @@ def _check(code: int, what: str):
         raise JengaError(f"{what} failed ({code}): {lib().jenga_strerror(code).decode()}")
 
 
-def make_desc(wp, materialise: bool = False, device: int = 0, tier: str = "auto") -> WorldDesc:
+def make_desc(wp, materialise: bool = False, device: int = 0, tier: str = "auto", group: int = 0) -> WorldDesc:
     """wp: any object with the fields of workloads.WorldParams."""
     d = WorldDesc()
     d.struct_size = C.sizeof(WorldDesc)
@@ -109,6 +110,7 @@ def make_desc(wp, materialise: bool = False, device: int = 0, tier: str = "auto"
     d.collapse_length = getattr(wp, "collapse_length", 0.0)
     d.collapse_fd, d.collapse_ek, d.collapse_theta = 0.5, 5.0e-5, 0.5235987755982988      # Eq. 18: f_d, eps_k [J], 30 deg
     d.solver_tier = TIERS[tier]
+    d.env_group = int(group)
     return d
 
 
@@ -134,7 +136,7 @@ class World:
     """
 
     def __init__(self, wp, state, props, mu, materialise: bool = False, device: int = 0, collapse_length: float = 0.0,
-                 tier: str = "auto", ref_state=None):
+                 tier: str = "auto", ref_state=None, group: int = 0):
         if not torch.cuda.is_available():
             raise JengaError("no CUDA device: the Jenga step has no CPU path")
         self.wp = wp
@@ -159,7 +161,7 @@ class World:
         self.n_cache = z((E,), torch.int32)
         self.status = z((E,), torch.int32)
         self.counters = z((N_COUNTERS,), torch.int64)
-        self.desc = make_desc(wp, materialise, device, tier)
+        self.desc = make_desc(wp, materialise, device, tier, group)
         self.desc.collapse_length = float(collapse_length)
         n_scr = lib().jenga_scratch_bytes(C.byref(self.desc))
         if n_scr == 0:
@@ -271,4 +273,5 @@ class World:
         return dict(zip(COUNTER_NAMES, self.counters.tolist()))
 
     def launch_info(self):
-        return dict(threads=lib().jenga_block_threads(C.byref(self.desc)), smem_bytes=lib().jenga_smem_bytes(C.byref(self.desc)))
+        return dict(threads=lib().jenga_block_threads(C.byref(self.desc)), smem_bytes=lib().jenga_smem_bytes(C.byref(self.desc)),
+                    env_group=lib().jenga_env_group(C.byref(self.desc)))

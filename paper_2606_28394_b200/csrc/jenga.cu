@@ -1,11 +1,12 @@
 // jenga.cu -- C-ABI of the batched Jenga step (include/jenga.h) over the four kernels of a substep.  sm_100a only.
 //
-//   k_detect  (kcollide.cuh)  S1 predict, S2 broadphase, S3 SAT, S4 colouring                   -> scratch
+//   k_detect  (kcollide.cuh)  S1 predict, S2 broadphase, S3 SAT, S4 colouring + visit plan      -> scratch
 //   k_manifold (kcollide.cuh) S3 contact manifolds                                              -> scratch
 //   k_slot    (kcollide.cuh)  S4 effective masses + warm-start lookup                           -> scratch
 //   k_solve   (ksolve.cuh)    S4 warm start, S5 PGS sweeps, S6 integrate, S7 cache, Eq. 18 latch
-// One warp per env in both.  jenga_step(n) enqueues n * n_substeps such pairs of launches on the caller's stream;
-// nothing returns to the host in between.  The stage entry points run the same device functions in a reduced mode.
+// One warp per env in the first three, one warp per group of G envs in k_solve (layout.cuh).  jenga_step(n) enqueues
+// n * n_substeps such quadruples of launches on the caller's stream; nothing returns to the host in between.  The stage
+// entry points run the same device functions in a reduced mode.
 #include <cuda_runtime.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -24,7 +25,7 @@ namespace jenga {
 __global__ void k_reset_rest(const Params P) {
   const int env = blockIdx.x * blockDim.x + threadIdx.x;
   if (env >= P.E) return;
-  int* meta = reinterpret_cast<int*>(P.scratch + (size_t)env * P.scratch_words + scratch_layout(P.pc).meta);
+  int* meta = reinterpret_cast<int*>(P.scratch + (size_t)env * P.scratch_words + scratch_layout(P.pc, P.G).meta);
   meta[MetaResting] = 0; meta[MetaSteps] = 0;
 }
 
@@ -41,7 +42,8 @@ struct jenga_world {
   jenga_world_desc desc;
   jenga_buffers bufs;
   Params P;
-  int tmb;                 // TMEM blocks per env of k_solve: 5, 10 or 0 (no TMEM, 1 warp per CTA)
+  int tmb;                 // TMEM blocks per group of k_solve: 2, 3, 4, 9 or 0 (no TMEM, 1 warp per CTA)
+  int G;                   // envs per group (= per k_solve warp)
   int wpc_collide;         // warps (= envs) per CTA of the collision kernels
   int n_sm;
   size_t smem_solve;       // dynamic shared memory per CTA of k_solve
@@ -53,14 +55,15 @@ struct jenga_world {
 
 static thread_local char g_err[512] = "no error";
 
-static size_t collide_env_bytes(const jenga_world_desc* d, int arena = -1) {
-  const size_t a = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaDetect);
-  const size_t b = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaManifold);
-  const size_t c = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaSlot);
+static size_t collide_env_bytes(const jenga_world_desc* d, int G, int arena = -1) {
+  const size_t a = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaDetect, G);
+  const size_t b = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaManifold, G);
+  const size_t c = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaSlot, G);
   return arena == jenga::ArenaDetect ? a : (arena == jenga::ArenaManifold ? b : (arena == jenga::ArenaSlot ? c : (a > b ? a : b)));
 }
-static size_t solve_env_bytes(const jenga_world_desc* d, int tmb) {
-  return 4 * jenga::solve_smem_words(d->body_stride, d->max_contacts / 4, tmb);
+/* shared memory of one k_solve warp (= one group of G envs) */
+static size_t solve_group_bytes(const jenga_world_desc* d, int tmb, int G) {
+  return 4 * jenga::solve_smem_words(d->body_stride, d->max_contacts / 4, tmb, G);
 }
 
 static bool desc_ok(const jenga_world_desc* d) {
@@ -71,59 +74,91 @@ static bool desc_ok(const jenga_world_desc* d) {
   if (d->max_pairs <= 0 || d->max_pairs > 65535) return false;
   if (d->max_contacts < 4 || (d->max_contacts & 3) || d->max_contacts > 65532) return false;
   if (d->solver_tier < TierAuto || d->solver_tier > TierTmem128) return false;
-  if (collide_env_bytes(d) > kSmemMax || solve_env_bytes(d, 0) > kSmemMax) return false;
+  if (d->env_group < 0 || d->env_group > jenga::kMaxGroup) return false;
+  if (collide_env_bytes(d, 1) > kSmemMax || solve_group_bytes(d, 0, 1) > kSmemMax) return false;
   return true;
 }
 
-/* TMEM blocks per env of k_solve: the CTA (one per SM) has 4 G warps = 4 G envs in flight; each env gets 512 / G columns
- * = tmb blocks of 48: G = 3 -> 3 blocks (12 envs per SM), G = 2 -> 5, G = 1 -> 10; 0 = everything in shared memory, one
- * warp per CTA.  Auto takes the largest G whose shared memory (headers + bodies of 4 G envs) fits one SM;
- * desc.solver_tier forces a tier (-1 if it does not fit).                                                         */
-static int tier_groups(int tmb) { return tmb == 2 ? 4 : (tmb == 3 ? 3 : (tmb == 5 ? 2 : (tmb == 10 ? 1 : 0))); }
-static bool tier_fits(const jenga_world_desc* d, int tmb) {
-  return 4 * tier_groups(tmb) * solve_env_bytes(d, tmb) + 1024 + 16 <= kSmemMax;
+/* Envs per k_solve warp.  Two envs share a warp when the batch still fills the machine that way (every SM gets 16 groups),
+ * when two collision warps fit one CTA (the two warps of a group plan their visits together in k_detect), and when the
+ * widest tensor-memory tier holds the doubled records; desc.env_group forces it (-1 if it does not fit).           */
+static size_t solve_group_bytes(const jenga_world_desc* d, int tmb, int G);
+static bool group_fits(const jenga_world_desc* d, int G) {
+  if (G == 1) return true;
+  return 2 * collide_env_bytes(d, G) <= kSmemMax && solve_group_bytes(d, 0, G) + 1024 <= kSmemMax;
 }
-static int pick_tmb(const jenga_world_desc* d) {
+static int pick_group(const jenga_world_desc* d) {
+  if (d->env_group) return group_fits(d, d->env_group) ? d->env_group : -1;
+  return (long long)d->n_envs >= 2ll * 16 * kSmNominal && group_fits(d, 2) ? 2 : 1;
+}
+
+/* TMEM blocks per group of k_solve: the CTA (one per SM) has 4 Q warps = 4 Q groups in flight; each group gets 512 / Q
+ * columns = tmb blocks of 56: Q = 4 -> 2 blocks (16 groups per SM), Q = 3 -> 3, Q = 2 -> 4, Q = 1 -> 9; 0 = everything in
+ * shared memory, one warp per CTA.  Auto takes the largest Q whose shared memory (body records of 4 Q groups) fits one
+ * SM; desc.solver_tier forces a tier (-1 if it does not fit).                                                      */
+static int tier_groups(int tmb) { return tmb == 2 ? 4 : (tmb == 3 ? 3 : (tmb == 4 ? 2 : (tmb == 9 ? 1 : 0))); }
+static bool tier_fits(const jenga_world_desc* d, int tmb, int G) {
+  return 4 * tier_groups(tmb) * solve_group_bytes(d, tmb, G) + 1024 + 16 <= kSmemMax;
+}
+/* The blocks of a group beyond its tensor-memory share are re-read from the scratch in every sweep: they must stay in L2
+ * while the group is in flight, or every visit goes to HBM (measured at cfg5 with two envs per warp: 16 groups per SM =
+ * 166 MB of blocks in flight, k_solve 6.9 ms; 12 groups per SM = 112 MB, 4.8 ms).  Capacity-based bound, 126 MB of L2. */
+static bool tier_in_l2(const jenga_world_desc* d, int tmb, int G) {
+  const long long nblk = jenga::n_blocks(d->max_contacts / 4, G), out = nblk > tmb ? nblk - tmb : 0;
+  return (long long)kSmNominal * 4 * tier_groups(tmb) * out * jenga::kBlkWords * 4 <= 120ll << 20;
+}
+static int pick_tmb(const jenga_world_desc* d, int G) {
   switch (d->solver_tier) {
-    case TierSmem: return 0;
-    case TierTmem128: return tier_fits(d, 2) ? 2 : -1;
-    case TierTmem160: return tier_fits(d, 3) ? 3 : -1;
-    case TierTmem256: return tier_fits(d, 5) ? 5 : -1;
-    case TierTmem512: return tier_fits(d, 10) ? 10 : -1;
+    case TierSmem: return solve_group_bytes(d, 0, G) + 1024 <= kSmemMax ? 0 : -1;
+    case TierTmem128: return tier_fits(d, 2, G) ? 2 : -1;
+    case TierTmem160: return tier_fits(d, 3, G) ? 3 : -1;
+    case TierTmem256: return tier_fits(d, 4, G) ? 4 : -1;
+    case TierTmem512: return tier_fits(d, 9, G) ? 9 : -1;
     default: {
-      /* auto.  A batch that does not fill the machine (148 SMs x 4 G envs in flight) takes the tier with the fewest envs
-         per SM that still holds it at once: more of every env's constant blocks are then in tensor memory, and below
-         4 envs per SM the shared-memory tier (lowest latency per chunk visit) is the quickest.  All tiers give the same bits. */
-      const long long E = d->n_envs;
-      if (E <= 4ll * kSmNominal && solve_env_bytes(d, 0) + 1024 <= kSmemMax) return 0;
-      const int by_size[3] = { 10, 5, 3 };
+      /* auto.  A batch that does not fill the machine (148 SMs x 4 Q groups in flight) takes the tier with the fewest groups
+         per SM that still holds it at once: more of every group's blocks are then in tensor memory, and below
+         4 groups per SM the shared-memory tier (lowest latency per chunk visit) is the quickest.  All tiers give the same bits. */
+      const long long NG = ((long long)d->n_envs + G - 1) / G;
+      if (NG <= 4ll * kSmNominal && solve_group_bytes(d, 0, G) + 1024 <= kSmemMax) return 0;
+      const int by_size[3] = { 9, 4, 3 };
       for (int k = 0; k < 3; ++k)
-        if (E <= 4ll * tier_groups(by_size[k]) * kSmNominal && tier_fits(d, by_size[k])) return by_size[k];
-      return tier_fits(d, 2) ? 2 : (tier_fits(d, 3) ? 3 : (tier_fits(d, 5) ? 5 : (tier_fits(d, 10) ? 10 : 0)));
+        if (NG <= 4ll * tier_groups(by_size[k]) * kSmNominal && tier_fits(d, by_size[k], G)) return by_size[k];
+      const int by_width[4] = { 2, 3, 4, 9 };
+      for (int k = 0; k < 4; ++k)
+        if (tier_fits(d, by_width[k], G) && (tier_in_l2(d, by_width[k], G) || k == 3)) return by_width[k];
+      return 0;
     }
   }
 }
 
 /* dynamic shared memory of a k_solve CTA */
-static size_t solve_cta_bytes(const jenga_world_desc* d, int tmb) {
-  return tmb ? 4 * tier_groups(tmb) * solve_env_bytes(d, tmb) : solve_env_bytes(d, 0);
+static size_t solve_cta_bytes(const jenga_world_desc* d, int tmb, int G) {
+  return tmb ? 4 * tier_groups(tmb) * solve_group_bytes(d, tmb, G) : solve_group_bytes(d, 0, G);
 }
 
 extern "C" size_t jenga_smem_bytes(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
-  const int tmb = pick_tmb(d);
-  return tmb < 0 ? 0 : solve_cta_bytes(d, tmb);
+  const int G = pick_group(d), tmb = G < 0 ? -1 : pick_tmb(d, G);
+  return tmb < 0 ? 0 : solve_cta_bytes(d, tmb, G);
 }
 
 extern "C" int jenga_block_threads(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
-  const int tmb = pick_tmb(d);
-  return tmb < 0 ? 0 : (tmb ? 128 * tier_groups(tmb) : 32);   /* one warp per env; 4, 8 or 12 envs per CTA in the TMEM tiers */
+  const int G = pick_group(d), tmb = G < 0 ? -1 : pick_tmb(d, G);
+  return tmb < 0 ? 0 : (tmb ? 128 * tier_groups(tmb) : 32);   /* one warp per group; 4, 8, 12 or 16 groups per CTA in the TMEM tiers */
+}
+
+extern "C" int jenga_env_group(const jenga_world_desc* d) {
+  if (!desc_ok(d)) return 0;
+  const int G = pick_group(d);
+  return G < 0 ? 0 : G;
 }
 
 extern "C" size_t jenga_scratch_bytes(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
-  return ((size_t)d->n_envs * jenga::scratch_layout(d->max_contacts / 4).total + jenga::kScratchHead) * sizeof(float);
+  const int G = pick_group(d);
+  if (G < 0) return 0;
+  return ((size_t)d->n_envs * jenga::scratch_layout(d->max_contacts / 4, G).total + jenga::kScratchHead) * sizeof(float);
 }
 
 extern "C" const char* jenga_strerror(int code) {
@@ -185,7 +220,9 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
     return JENGA_E_ARG;
   if (b->f_ext && !aligned16(b->f_ext)) return JENGA_E_ARG;
   if (b->scratch_bytes < jenga_scratch_bytes(d)) return JENGA_E_ARG;
-  const int tmb = pick_tmb(d);
+  const int G = pick_group(d);
+  if (G < 0) return JENGA_E_ARG;
+  const int tmb = pick_tmb(d, G);
   if (tmb < 0) return JENGA_E_ARG;
   int cur = -1;
   cudaError_t e = cudaGetDevice(&cur);
@@ -198,13 +235,13 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   jenga_world* w = new (std::nothrow) jenga_world();
   if (!w) return JENGA_E_ARG;
   w->profiling = false;
-  w->desc = *d; w->bufs = *b; w->tmb = tmb; w->n_sm = prop.multiProcessorCount;
-  w->smem_solve = solve_cta_bytes(d, tmb);
-  const size_t cb = collide_env_bytes(d);
-  w->wpc_collide = 4 * cb <= kSmemMax ? 4 : (2 * cb <= kSmemMax ? 2 : 1);
-  w->smem_collide = w->wpc_collide * collide_env_bytes(d, jenga::ArenaDetect);
-  w->smem_manifold = w->wpc_collide * collide_env_bytes(d, jenga::ArenaManifold);
-  w->smem_slot = w->wpc_collide * collide_env_bytes(d, jenga::ArenaSlot);
+  w->desc = *d; w->bufs = *b; w->tmb = tmb; w->G = G; w->n_sm = prop.multiProcessorCount;
+  w->smem_solve = solve_cta_bytes(d, tmb, G);
+  const size_t cb = collide_env_bytes(d, G);
+  w->wpc_collide = 4 * cb <= kSmemMax ? 4 : (2 * cb <= kSmemMax ? 2 : 1);       /* G = 2: group_fits made sure of two */
+  w->smem_collide = w->wpc_collide * collide_env_bytes(d, G, jenga::ArenaDetect);
+  w->smem_manifold = w->wpc_collide * collide_env_bytes(d, G, jenga::ArenaManifold);
+  w->smem_slot = w->wpc_collide * collide_env_bytes(d, G, jenga::ArenaSlot);
   if (w->smem_solve > (size_t)prop.sharedMemPerBlockOptin || w->smem_collide > (size_t)prop.sharedMemPerBlockOptin) { delete w; return JENGA_E_ARG; }
   Params& P = w->P;
   P.E = d->n_envs; P.B = d->n_bodies; P.S = d->body_stride;
@@ -214,7 +251,7 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.cp.edge_bias_rel = d->edge_bias_rel; P.cp.edge_bias_abs = d->edge_bias_abs; P.cp.par_eps = d->par_eps; P.cp.tie_eps = d->tie_eps;
   P.match_tol = d->match_tol; P.warm_start = d->warm_start; P.gyroscopic = d->gyroscopic;
   P.max_pairs = d->max_pairs; P.max_contacts = d->max_contacts; P.pc = d->max_contacts / 4; P.materialise = d->materialise;
-  P.tmb = tmb; P.nblk = jenga::n_blocks(P.pc);
+  P.tmb = tmb; P.G = G; P.nblk = jenga::n_blocks(P.pc, G);
   P.state = b->state; P.props = b->props; P.mu = b->mu; P.f_ext = b->f_ext;
   P.pairs = b->pairs; P.n_pairs = b->n_pairs; P.contacts = b->contacts; P.n_contacts = b->n_contacts; P.lambda = b->lambda;
   P.cache_key = b->cache_key; P.cache_lam = b->cache_lam; P.cache_pt = b->cache_pt; P.n_cache = b->n_cache;
@@ -225,7 +262,7 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.rest_steps = b->rest_steps;
   P.collapse_dx = d->collapse_fd * d->collapse_length; P.collapse_ek = d->collapse_ek; P.collapse_theta = d->collapse_theta;
   P.work_counter = (int*)b->scratch;
-  P.scratch = (float*)b->scratch + jenga::kScratchHead; P.scratch_words = jenga::scratch_layout(P.pc).total;
+  P.scratch = (float*)b->scratch + jenga::kScratchHead; P.scratch_words = jenga::scratch_layout(P.pc, G).total;
   *out = w;
   return JENGA_OK;
 }
@@ -317,14 +354,15 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
 static int launch_solve(jenga_world* w, int iters, int flags, float rest_ek, cudaStream_t st) {
   const cudaError_t e = ensure_smem(w->desc.device, w->tmb ? KnSolveTm : KnSolveSm, w->smem_solve);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_solve)");
-  /* persistent CTAs: one per SM in the TMEM tiers (it owns all 512 columns), each warp strides over the envs */
+  /* persistent CTAs: one per SM in the TMEM tiers (it owns all 512 columns), each warp takes groups from a global queue */
+  const int n_groups = (w->P.E + w->G - 1) / w->G;
   if (w->tmb) {
-    /* small batches are spread over all SMs (the warps of every CTA pull envs from the same queue) */
-    const int wpc = 4 * tier_groups(w->tmb), grid = w->P.E < w->n_sm ? w->P.E : w->n_sm;
+    /* small batches are spread over all SMs (the warps of every CTA pull groups from the same queue) */
+    const int wpc = 4 * tier_groups(w->tmb), grid = n_groups < w->n_sm ? n_groups : w->n_sm;
     jenga::k_solve<true><<<grid, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
   } else {
     const int per_sm = (int)(kSmemMax / (w->smem_solve + 1024)), resident = w->n_sm * (per_sm < 1 ? 1 : (per_sm > 16 ? 16 : per_sm));
-    jenga::k_solve<false><<<w->P.E < resident ? w->P.E : resident, 32, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
+    jenga::k_solve<false><<<n_groups < resident ? n_groups : resident, 32, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
   }
   return launched("k_solve");
 }

@@ -1,5 +1,5 @@
 // kcollide.cuh -- the three collision kernels of a substep, one env per warp.  k_detect: S1 predict, S2 broadphase, S3 SAT
-// (which candidates collide), S4 canonical colouring + chunk packing.  k_manifold: S3 contact manifolds.  k_slot: S4
+// (which candidates collide), S4 canonical colouring + the group's visit plan.  k_manifold: S3 contact manifolds.  k_slot: S4
 // contact setup (effective masses, warm-start lookup).  Their products go to the scratch buffer (layout.cuh) for the
 // next kernel.  They are separate kernels because each one's hot code then fits the 32 KB instruction cache (as one
 // kernel: 70 KB, and `no_instruction` was the top stall with 16 warps per SM at different places in it).
@@ -16,21 +16,21 @@ struct CSm {
   SP<unsigned> hitw;            // [ceil(S/32)][32] broadphase hit words of the current block of 32 rows; ALIASES used
   SP<unsigned long long> used;  // [S]      colour masks per body
   SP<unsigned> cab;             // [pcA]    (a+1) | A dynamic << 11 | axis << 12 | b << 16 | B dynamic << 27
-  SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending
+  SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending; ALIASES chm
   SP<float> poly;               // [8][3][32] clip polygon of every lane (component-major: lane l <-> bank l)
   SP<unsigned short> cpair;     // [pcA]    colliding pair indices, ascending
   SP<unsigned short> cprev;     // [pcA]    pair indices of the warm-start cache (previous substep), ascending
   SP<unsigned short> pos;       // [pcA]    position of pair r
   SP<unsigned short> wrank;     // [pcA]    rank inside its colour / contact offset
   SP<unsigned char> colour;     // [pcA]
-  SP<int> ph;                   // [ph_max] chunk descriptors in canonical order
-  SP<int> chc;                  // [ph_max] colour | first rank-in-colour << 8 of each chunk
-  SP<int> ccount;               // [64]
-  SP<int> cfirst;               // [64] first chunk of the colour
+  SP<int> ph;                   // [ph_max] chunk descriptors of the GROUP in the order the solver visits them
+  SP<int> chm;                  // [kMaxGroup][ph_max] per member: colour | first rank-in-colour << 6 | pairs << 20 of each chunk
+  SP<int> ccount;               // [64] pairs of each colour of this env (the sibling warp reads it)
+  SP<int> cfirst;               // [64] first chunk with pairs of the colour (this env's)
   SP<int> fill;                 // [nblk] lanes taken in each block (packing)
   SP<int> misc;                 // [8]
 };
-enum { MiNph = 0, MiNcol = 1, MiNblk = 2 };
+enum { MiNph = 0, MiNcol = 1, MiNblk = 2, MiSame = 3 };
 
 enum { ArenaDetect = 0, ArenaManifold = 1, ArenaSlot = 2 };
 
@@ -39,14 +39,16 @@ enum { ArenaDetect = 0, ArenaManifold = 1, ArenaSlot = 2 };
 // list, cache keys.
 __host__ __device__ inline int cb_words(int arena) { return arena == ArenaSlot ? kCb : 20; }
 
-__host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc, int arena) {
-  const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc);
+__host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc, int arena, int G) {
+  const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc, G);
   size_t w = (size_t)cb_words(arena) * S + pcA + pcA / 2;  // cb, cab, cpair
   if (arena != ArenaManifold) w += 2 * (size_t)(pcA / 2);  // pos, wrank
   if (arena == ArenaDetect) {
     const int uh = 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
-    w += 4 * S + uh + mpA / 2 + pcA / 4;                   // ext, used / hitw, cand, colour
-    w += 2 * round_up(ph_max(nblk), 4);                    // ph, chc
+    const int phw = round_up(ph_max(nblk, G), 4);
+    w += 4 * S + uh + pcA / 4;                             // ext, used / hitw, colour
+    w += mpA / 2 > kMaxGroup * phw ? mpA / 2 : kMaxGroup * phw;   // cand; chm aliases it (the candidates are dead by then)
+    w += phw;                                              // ph
     w += 2 * kMaxColours + round_up(nblk, 4) + 8;          // ccount, cfirst, fill, misc
   } else if (arena == ArenaManifold) {
     w += 768;                                              // poly
@@ -56,8 +58,8 @@ __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int p
   return round_up((int)w, 4);
 }
 
-__device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int arena) {
-  const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc), phw = round_up(ph_max(nblk), 4);
+__device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int arena, int G) {
+  const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc, G), phw = round_up(ph_max(nblk, G), 4);
   CSm s; int p = base;
   s.cbw = cb_words(arena);
   s.cb.off = p;     p += s.cbw * S;
@@ -66,15 +68,14 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int 
   s.pos.off = s.wrank.off = 0;
   if (arena != ArenaManifold) { s.pos.off = p; p += pcA / 2; s.wrank.off = p; p += pcA / 2; }
   // the arrays of the other arena get offset 0 (never touched by this kernel)
-  s.ext.off = s.hitw.off = s.used.off = s.cand.off = s.colour.off = s.ph.off = s.chc.off = 0;
+  s.ext.off = s.hitw.off = s.used.off = s.cand.off = s.colour.off = s.ph.off = s.chm.off = 0;
   s.ccount.off = s.cfirst.off = s.fill.off = s.misc.off = s.cprev.off = s.poly.off = 0;
   if (arena == ArenaDetect) {
     s.ext.off = p;    p += 4 * S;
     s.hitw.off = p;   s.used.off = p;   p += 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
-    s.cand.off = p;   p += mpA / 2;
+    s.cand.off = p;   s.chm.off = p;    p += mpA / 2 > kMaxGroup * phw ? mpA / 2 : kMaxGroup * phw;
     s.colour.off = p; p += pcA / 4;
     s.ph.off = p;     p += phw;
-    s.chc.off = p;    p += phw;
     s.ccount.off = p; p += kMaxColours;
     s.cfirst.off = p; p += kMaxColours;
     s.fill.off = p;   p += round_up(nblk, 4);
@@ -525,29 +526,11 @@ __device__ inline int find_colliding(const CSm& s, const Params& P, int n_cand, 
 }
 
 // Canonical order (north_star (d), DESIGN §2 S4): visit the colliding pairs in ascending pair index;
-// colour = lowest colour not used by an earlier pair sharing a dynamic body.  The pairs of a colour are then cut
-// into chunks of consecutive lanes of one 32-position block (bin packing, lowest block first: whole if a block has
-// room, else split over the emptiest blocks); s.ph lists the chunks colour by colour = the order the solver visits
-// them, s.pos[r] = 32 block + lane of pair r.  The walk is sequential by definition (lane 0, one 64-bit mask per
-// body).  When the colliding-pair list equals the one the scratch was coloured for, that colouring (the same
-// function of the same input) is kept: the steady state of a standing tower.
-__device__ inline void colour_pairs(const CSm& s, const Params& P, float* scr, const Scratch& L, int n_coll, unsigned* status) {
+// colour = lowest colour not used by an earlier pair sharing a dynamic body.  The walk is sequential by definition
+// (lane 0, one 64-bit mask per body).  Products: s.colour[r], s.wrank[r] = rank of pair r inside its colour,
+// s.ccount[c], s.misc[MiNcol].
+__device__ inline void colour_walk(const CSm& s, const Params& P, int n_coll, unsigned* status) {
   const int lane = lane_id();
-  int* meta = reinterpret_cast<int*>(scr + L.meta);
-  unsigned short* gpos = reinterpret_cast<unsigned short*>(scr + L.pos);
-  unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
-  unsigned* gcab = reinterpret_cast<unsigned*>(scr + L.cab);
-  for (int r = lane; r < n_coll; r += 32) gcab[r] = s.cab[r];             // bodies + SAT axis of every pair, for k_manifold / k_slot
-  bool same = meta[MetaMagic] == kMagic && meta[MetaNcoll] == n_coll;
-  if (same)
-    for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
-  same = __all_sync(kFull, same);
-  if (same) {
-    if (lane == 0) { s.misc[MiNph] = meta[MetaNph]; s.misc[MiNcol] = meta[MetaNcol]; s.misc[MiNblk] = meta[MetaNblk]; }
-    __syncwarp();
-    return;
-  }
-  const int nblk = P.nblk;
   for (int b = lane; b < P.B; b += 32) s.used[b] = 0ull;
   for (int c = lane; c < kMaxColours; c += 32) s.ccount[c] = 0;
   __syncwarp();
@@ -568,29 +551,131 @@ __device__ inline void colour_pairs(const CSm& s, const Params& P, float* scr, c
       s.wrank[r] = (unsigned short)k; s.ccount[c] = k + 1;
       if (c + 1 > ncol) ncol = c + 1;
     }
-    // bin packing: fill[j] = lanes taken in block j (taken from lane 0 upwards)
-    const SP<int> fill = s.fill;
-    for (int j = 0; j < nblk; ++j) fill[j] = 0;
-    int nph = 0, top = 0;
-    for (int c = 0; c < ncol; ++c) {
-      int n = s.ccount[c], w0 = 0;
-      s.cfirst[c] = nph;
-      while (n > 0) {
-        int take = n > 32 ? 32 : n, jb = -1;
-        for (int j = 0; j < nblk; ++j) if (32 - fill[j] >= take) { jb = j; break; }
-        if (jb < 0) {                                         // no block holds it whole: the emptiest block takes what fits
-          int best = 0;
-          for (int j = 0; j < nblk; ++j) if (32 - fill[j] > best) { best = 32 - fill[j]; jb = j; }
-          take = best;
-        }
-        s.ph[nph] = ph_pack(jb, fill[jb], take); s.chc[nph] = c | (w0 << 8); ++nph;
-        fill[jb] += take; w0 += take; n -= take;
-        if (jb + 1 > top) top = jb + 1;
-      }
-    }
-    s.misc[MiNcol] = ncol; s.misc[MiNph] = nph; s.misc[MiNblk] = top;
+    s.misc[MiNcol] = ncol;
     if (st) *status |= st;
   }
+  __syncwarp();
+}
+
+// chunk word of a member: colour | first rank-in-colour << 6 | pairs << 20
+__device__ __forceinline__ int chm_pack(int colour, int w0, int cnt) { return cnt ? (colour | (w0 << 6) | (cnt << 20)) : 0; }
+
+// The visit plan of a group (warp-uniform: every lane runs the same steps, lane j looks after the fill of blocks j, j + 32,
+// ...; both warps of the group compute the same plan from the members' colour counts).
+// A visit takes pairs of the CURRENT colour of every member, at most 32 in all: first of the member with the most colours
+// left (ties: the most pairs left), then of the other as far as lanes remain; a member moves to its next colour in the
+// visit after its current one is used up.  So a member's colours are visited in ascending order, every pair once per
+// sweep, and the pairs of one visit share no dynamic body (same colour, or different envs).  A visit becomes one chunk =
+// consecutive lanes of one 32-position block, member 0's pairs first (bin packing, lowest block first: whole if a block
+// has room, else cut over the emptiest blocks).  s.ph lists the chunks in visiting order; s.chm[m] says which pairs of
+// member m a chunk holds; s.cfirst[c] = first chunk with pairs of colour c of member `me`.
+__device__ inline void plan_group(const CSm& s, const CSm& s0, const CSm& s1, int nm, int me, int nblk, int phw, unsigned* status) {
+  const int lane = lane_id();
+  const SP<int> fill = s.fill;
+  for (int j = lane; j < nblk; j += 32) fill[j] = 0;
+  const int ncol0 = s0.misc[MiNcol], ncol1 = nm > 1 ? s1.misc[MiNcol] : 0;
+  int work0 = 0, work1 = 0;
+  for (int c = lane; c < ncol0; c += 32) work0 += s0.ccount[c];
+  for (int c = lane; c < ncol1; c += 32) work1 += s1.ccount[c];
+  work0 = __reduce_add_sync(kFull, work0); work1 = __reduce_add_sync(kFull, work1);
+  int ci0 = 0, ci1 = 0, rem0 = 0, rem1 = 0, nph = 0, top = 0;
+  __syncwarp();
+  for (;;) {
+    // the current colour of each member (empty colours are skipped)
+    while (ci0 < ncol0 && rem0 == 0) { rem0 = s0.ccount[ci0]; if (rem0 == 0) ++ci0; }
+    while (ci1 < ncol1 && rem1 == 0) { rem1 = s1.ccount[ci1]; if (rem1 == 0) ++ci1; }
+    const int left0 = ncol0 - ci0, left1 = ncol1 - ci1;
+    if (left0 <= 0 && left1 <= 0) break;
+    int t0, t1;
+    if (left1 > left0 || (left1 == left0 && work1 > work0)) { t1 = min(rem1, 32); t0 = min(rem0, 32 - t1); }
+    else { t0 = min(rem0, 32); t1 = min(rem1, 32 - t0); }
+    const int w00 = left0 > 0 ? s0.ccount[ci0] - rem0 : 0, w01 = left1 > 0 ? s1.ccount[ci1] - rem1 : 0;
+    int n = t0 + t1, done = 0;
+    while (n > 0) {
+      int take = n, jb = -1;
+      for (int base = 0; base < nblk && jb < 0; base += 32) {            // lowest block that holds it whole
+        const int j = base + lane, room = j < nblk ? 32 - fill[j] : 0;
+        const unsigned bal = __ballot_sync(kFull, room >= take);
+        if (bal) jb = base + __ffs(bal) - 1;
+      }
+      if (jb < 0) {                                           // none: the emptiest block (lowest on ties) takes what fits
+        int best = 0;
+        for (int base = 0; base < nblk; base += 32) {
+          const int j = base + lane, room = j < nblk ? 32 - fill[j] : 0;
+          const int mx = __reduce_max_sync(kFull, room);
+          if (mx > best) { best = mx; jb = base + __ffs(__ballot_sync(kFull, room == mx)) - 1; }
+        }
+        take = best;
+      }
+      if (jb < 0 || take <= 0 || nph >= phw) { *status |= JENGA_ST_CONTACT_OVERFLOW; break; }     // cannot happen: 32 nblk >= G pc
+      const int f = fill[jb], hi = done + take;
+      const int c0 = max(0, min(hi, t0) - done), lo1 = max(done, t0), c1 = max(0, hi - lo1);
+      const int st0 = w00 + done, st1 = w01 + lo1 - t0;
+      __syncwarp();
+      if (lane == 0) {
+        s.ph[nph] = ph_pack(jb, f, take);
+        s.chm[nph] = chm_pack(ci0, st0, c0); s.chm[phw + nph] = chm_pack(ci1, st1, c1);
+        if (me == 0 ? (c0 > 0 && st0 == 0) : (c1 > 0 && st1 == 0)) s.cfirst[me ? ci1 : ci0] = nph;
+        fill[jb] = f + take;
+      }
+      __syncwarp();
+      done += take; n -= take; ++nph;
+      if (jb + 1 > top) top = jb + 1;
+    }
+    rem0 -= t0; work0 -= t0; if (t0 > 0 && rem0 == 0) ++ci0;
+    rem1 -= t1; work1 -= t1; if (t1 > 0 && rem1 == 0) ++ci1;
+  }
+  if (lane == 0) { s.misc[MiNph] = nph; s.misc[MiNblk] = top; }
+}
+
+// Does the colliding-pair list of this env equal the one its scratch was coloured for?  (the steady state of a standing
+// tower: colouring and plan are functions of the lists alone and are kept).  Also hands the bodies + SAT axis of every pair
+// to k_manifold / k_slot.
+__device__ inline bool colouring_is_current(const CSm& s, float* scr, const Scratch& L, int n_coll) {
+  const int lane = lane_id();
+  const int* meta = reinterpret_cast<const int*>(scr + L.meta);
+  const unsigned short* gpair = reinterpret_cast<const unsigned short*>(scr + L.cpair);
+  unsigned* gcab = reinterpret_cast<unsigned*>(scr + L.cab);
+  for (int r = lane; r < n_coll; r += 32) gcab[r] = s.cab[r];
+  bool same = meta[MetaMagic] == kMagic && meta[MetaNcoll] == n_coll;
+  if (same)
+    for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
+  return __all_sync(kFull, same);
+}
+
+__device__ __forceinline__ void pair_barrier(int id) {
+  if (id == 1) asm volatile("bar.sync 1, 64;" ::: "memory"); else asm volatile("bar.sync 2, 64;" ::: "memory");
+}
+
+// S4 colouring + plan of the group this env belongs to.  `present`: the env exists (env < E); an env that exists but is
+// skipped (at rest) takes part with n_coll = 0.  With G = 2 the two warps of a group are neighbours in the CTA and meet at
+// two named barriers (ids 1 + warp / 2); both always take this path, whatever their env does.
+__device__ inline void colour_pairs(const CSm& s, const Params& P, int env, bool present, int n_coll, unsigned* status) {
+  const int lane = lane_id(), warp = threadIdx.x >> 5, G = P.G;
+  const Scratch L = scratch_layout(P.pc, G);
+  const int me = G == 2 ? (env & 1) : 0;
+  float* scr = P.scratch + (size_t)env * P.scratch_words;                    // touched only if present
+  float* scr0 = P.scratch + (size_t)(env - me) * P.scratch_words;            // the group's first env always exists
+  int* meta = reinterpret_cast<int*>(scr + L.meta);
+  int* meta0 = reinterpret_cast<int*>(scr0 + L.meta);
+  const int arena = (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaDetect, G);
+  const CSm sib = carve_collide(P.S, P.max_pairs, P.pc, (warp ^ 1) * arena, ArenaDetect, G);
+  bool same = present ? colouring_is_current(s, scr, L, n_coll) : true;
+  if (G == 2) {
+    if (lane == 0) s.misc[MiSame] = same ? 1 : 0;
+    pair_barrier(1 + (warp >> 1));
+    same = same && sib.misc[MiSame] != 0;
+  }
+  if (same) {
+    if (lane == 0) { s.misc[MiNph] = meta0[MetaNph]; s.misc[MiNblk] = meta0[MetaNblk]; s.misc[MiNcol] = present ? meta[MetaNcol] : 0; }
+    __syncwarp();
+    return;
+  }
+  colour_walk(s, P, present ? n_coll : 0, status);
+  if (G == 2) pair_barrier(1 + (warp >> 1));
+  const int nblk = P.nblk, phw = round_up(ph_max(nblk, G), 4);
+  const int nm = G == 2 && (env | 1) < P.E ? 2 : 1;              // members that exist
+  plan_group(s, me ? sib : s, me ? s : sib, nm, me, nblk, phw, status);
   __syncwarp();
   const int nph = s.misc[MiNph];
   // Blocks are renumbered by the number of chunks they hold (= solver visits per sweep), most first: the first blocks
@@ -607,33 +692,45 @@ __device__ inline void colour_pairs(const CSm& s, const Params& P, float* scr, c
     }
     __syncwarp();
   }
-  for (int r = lane; r < n_coll; r += 32) {
-    const int c = s.colour[r], w = s.wrank[r];
-    int j = s.cfirst[c], k = 0;
-    for (; j < nph; ++j) {
-      const int d = s.ph[j], w0 = s.chc[j] >> 8, cnt = (d >> 8) & 0xff;
-      if (w >= w0 && w < w0 + cnt) { k = 32 * (d >> 16) + (d & 0xff) + (w - w0); break; }
+  if (present) {
+    unsigned short* gpos = reinterpret_cast<unsigned short*>(scr + L.pos);
+    unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
+    for (int r = lane; r < n_coll; r += 32) {
+      const int c = s.colour[r], w = s.wrank[r];
+      int k = 0;
+      for (int j = s.cfirst[c]; j < nph; ++j) {
+        const int cm = s.chm[me * phw + j], cnt = cm >> 20, w0 = (cm >> 6) & 0x3fff;
+        if (cnt && (cm & 63) == c && w >= w0 && w < w0 + cnt) {
+          const int d = s.ph[j], off = me ? (s.chm[j] >> 20) : 0;
+          k = 32 * (d >> 16) + (d & 0xff) + off + (w - w0);
+          break;
+        }
+      }
+      s.pos[r] = (unsigned short)k;
+      gpos[r] = (unsigned short)k; gpair[r] = s.cpair[r];
     }
-    s.pos[r] = (unsigned short)k;
-    gpos[r] = (unsigned short)k; gpair[r] = s.cpair[r];
+    if (lane == 0) { meta[MetaMagic] = kMagic; meta[MetaNcoll] = n_coll; meta[MetaNcol] = s.misc[MiNcol]; }
   }
-  int* gph = reinterpret_cast<int*>(scr + L.ph);
-  for (int j = lane; j < nph; j += 32) gph[j] = s.ph[j];
-  if (lane == 0) {
-    meta[MetaMagic] = kMagic; meta[MetaNcoll] = n_coll; meta[MetaNph] = nph; meta[MetaNcol] = s.misc[MiNcol]; meta[MetaNblk] = s.misc[MiNblk];
+  if (me == 0) {                                              // group data: in the region of the group's first env
+    int* gph = reinterpret_cast<int*>(scr0 + L.ph);
+    for (int j = lane; j < nph; j += 32) gph[j] = s.ph[j];
+    if (lane == 0) { meta0[MetaNph] = nph; meta0[MetaNblk] = s.misc[MiNblk]; }
   }
   __syncwarp();
 }
 
 // ---------------------------------------------------------------- pair slots (solver constants at a position)
-// Header of position k (scratch: hdr[f * npos + k]):
-//   0: ab = (a+1) | b << 16, meta = np | axis << 8 | pair index << 16, rank r of the pair, 1/|e_k - n (n.e_k)|
-//   1: n.x n.y n.z, Baumgarte corr = beta max(0, depth_max - slop) / (imA + imB)     (Eq. 16)
-//   2: t1.x t1.y t1.z, 0
-// Contact constants of position k: 48 words.  ro[9c..9c+8] = p.xyz, (1+e)/K_nn, 1/K_t1t1, 1/K_t2t2,
-// K_n,t1, K_n,t2, K_t1,t2 of contact c (K_dd: Eq. 13, for d = n, t1, t2); lam[3c..3c+2] = jn, jt1, jt2.
-struct PairC { float v[48]; };      // v[0..35] read-only constants, v[36..47] impulses
-constexpr int kLam = 36;
+// The 56 words of position k (block k / 32, lane k % 32; float4 f of the pair at [block][f][lane]):
+//   v[9c..9c+8], c = 0..3   p.xyz, (1+e)/K_nn, 1/K_t1t1, 1/K_t2t2, K_n,t1, K_n,t2, K_t1,t2 of contact c (K_dd: Eq. 13,
+//                           PAPER.md:296, for d = n, t1, t2)
+//   v[36 + 3c..], c = 0..3  the impulses jn, jt1, jt2 of contact c
+//   v[48..51]               ab = record of A | record of B << 16 (solver body records of the GROUP: member m's body b is
+//                           record m S + b, the ground is record G S), meta = np | axis << 8 | member << 12 | A is the
+//                           ground << 13 | pair index << 16, rank r of the pair in its env's list, 1/|e_k - n (n.e_k)|
+//   v[52..55]               n.x n.y n.z, Baumgarte corr = beta max(0, depth_max - slop) / (imA + imB)     (Eq. 16)
+struct PairC { float v[56]; };      // v[0..35] read-only constants, v[36..47] impulses, v[48..55] header
+constexpr int kLam = 36, kHdr = 48;
+constexpr int kMetaMember = 1 << 12, kMetaGround = 1 << 13;
 
 struct Frame { Vec3 n, t1, t2; };
 
@@ -681,7 +778,7 @@ __device__ __forceinline__ int cache_lookup(const CSm& s, const Params& P, int e
   return lo;
 }
 
-__device__ inline void setup_slot(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int lo,
+__device__ inline void setup_slot(const CSm& s, const Params& P, int env, float* scr0, const Scratch& L, int lo,
                                   int k, int r, int a, int b, int pair, const Manifold& m) {
   BodyK A, Bb; load_bodyk(s, a, A); load_bodyk(s, b, Bb);
   const Vec3 n = m.n;
@@ -729,21 +826,20 @@ __device__ inline void setup_slot(const CSm& s, const Params& P, int env, float*
     }
   }
 
-  const int npos = 32 * P.nblk;
-  float4* hdr = reinterpret_cast<float4*>(scr + L.hdr);
-  const int meta = m.np | (m.axis << 8) | (pair << 16);
-  hdr[k] = make_float4(__int_as_float((a + 1) | (b << 16)), __int_as_float(meta), __int_as_float(r), il);
-  hdr[npos + k] = make_float4(n.x, n.y, n.z, im > 0.0f ? P.beta * fmaxf(0.0f, dmax - P.slop) / im : 0.0f);
-  hdr[2 * npos + k] = make_float4(F.t1.x, F.t1.y, F.t1.z, 0.0f);
+  // the 14 float4 of the pair (in the blocks of the env's group) are stored as soon as their words are complete (header
+  // and impulses first), so that the whole record is never live in registers at once
+  float4* cs = reinterpret_cast<float4*>(scr0 + L.cs) + (size_t)(k >> 5) * (kCsF4 * 32) + (k & 31);
+  const int mem = P.G == 2 ? (env & 1) : 0;
+  const int meta = m.np | (m.axis << 8) | (mem ? kMetaMember : 0) | (a < 0 ? kMetaGround : 0) | (pair << 16);
+  const int ab = (a >= 0 ? mem * P.S + a : P.G * P.S) | ((mem * P.S + b) << 16);
+  cs[(kHdr / 4) * 32] = make_float4(__int_as_float(ab), __int_as_float(meta), __int_as_float(r), il);
+  cs[(kHdr / 4 + 1) * 32] = make_float4(n.x, n.y, n.z, im > 0.0f ? P.beta * fmaxf(0.0f, dmax - P.slop) / im : 0.0f);
   const float e1 = 1.0f + P.restitution;
-  // the 12 float4 of the pair are stored as soon as their words are complete (the impulses first), so that the whole
-  // record is never live in registers at once
-  float4* cs = reinterpret_cast<float4*>(scr + L.cs) + (size_t)(k >> 5) * (kCsF4 * 32) + (k & 31);
   PairC out;
 #pragma unroll
   for (int c = 0; c < 4; ++c) { out.v[kLam + 3 * c] = lam[c][0]; out.v[kLam + 3 * c + 1] = lam[c][1]; out.v[kLam + 3 * c + 2] = lam[c][2]; }
 #pragma unroll
-  for (int f = kLam / 4; f < kCsF4; ++f) cs[f * 32] = make_float4(out.v[4 * f], out.v[4 * f + 1], out.v[4 * f + 2], out.v[4 * f + 3]);
+  for (int f = kLam / 4; f < kHdr / 4; ++f) cs[f * 32] = make_float4(out.v[4 * f], out.v[4 * f + 1], out.v[4 * f + 2], out.v[4 * f + 3]);
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     float ik[3] = { 0, 0, 0 }, ko[3] = { 0, 0, 0 };
@@ -781,7 +877,7 @@ __device__ inline int load_prev_keys(const CSm& s, const Params& P, int env) {
 
 // S4: lane l of a round takes colliding pair r = 32 round + l (ascending pair index), fetches the manifold k_manifold
 // left in the scratch and writes header and constants at the pair's position.
-__device__ inline void setup_pairs(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_coll, int nprev) {
+__device__ inline void setup_pairs(const CSm& s, const Params& P, int env, float* scr, float* scr0, const Scratch& L, int n_coll, int nprev) {
   const float4* man = reinterpret_cast<const float4*>(scr + L.man);
   for (int r = lane_id(); r < n_coll; r += 32) {
     const unsigned w = s.cab[r];
@@ -792,7 +888,7 @@ __device__ inline void setup_pairs(const CSm& s, const Params& P, int env, float
     m.n = v3(h.x, h.y, h.z); m.np = __float_as_int(h.w) & 0xff; m.axis = __float_as_int(h.w) >> 8;
 #pragma unroll
     for (int c = 0; c < 4; ++c) { const float4 q = man[5 * r + 1 + c]; m.p[c] = v3(q.x, q.y, q.z); m.d[c] = q.w; }
-    setup_slot(s, P, env, scr, L, lo, s.pos[r], r, a, b, pair, m);
+    setup_slot(s, P, env, scr0, L, lo, s.pos[r], r, a, b, pair, m);
   }
   __syncwarp();
 }
@@ -884,7 +980,7 @@ __device__ inline int pairs_from_contacts(const CSm& s, const Params& P, int env
 }
 
 // ModeGiven (jenga_pgs_solve): slots from the contact list the caller supplied instead of the narrowphase.
-__device__ inline void setup_given(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_coll, int n_cont, int nprev) {
+__device__ inline void setup_given(const CSm& s, const Params& P, int env, float* scr, float* scr0, const Scratch& L, int n_coll, int n_cont, int nprev) {
   const float4* in = reinterpret_cast<const float4*>(P.contacts + (size_t)env * P.max_contacts * 8);
   unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
   for (int r = lane_id(); r < n_coll; r += 32) {
@@ -899,7 +995,7 @@ __device__ inline void setup_given(const CSm& s, const Params& P, int env, float
       m.p[c] = v3(0, 0, 0); m.d[c] = 0.0f;
       if (c < m.np) { const float4 a4 = in[2 * (c0 + c)], b4 = in[2 * (c0 + c) + 1]; m.p[c] = v3(b4.x, b4.y, b4.z); m.d[c] = a4.w; }
     }
-    setup_slot(s, P, env, scr, L, cache_lookup(s, P, env, nprev, s.cpair[r]), s.pos[r], r, ab_a(w), ab_b(w), s.cpair[r], m);
+    setup_slot(s, P, env, scr0, L, cache_lookup(s, P, env, nprev, s.cpair[r]), s.pos[r], r, ab_a(w), ab_b(w), s.cpair[r], m);
   }
   __syncwarp();
 }
@@ -930,33 +1026,39 @@ template <int mode>
 __global__ void __launch_bounds__(128, 5) k_detect(const Params P, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
   const int env = blockIdx.x * wpc + warp;
-  if (blockIdx.x == 0 && threadIdx.x == 0) *P.work_counter = 0;      // k_solve of this substep starts its env queue at 0
-  if (env >= P.E) return;
-  const Scratch L = scratch_layout(P.pc);
+  if (blockIdx.x == 0 && threadIdx.x == 0) *P.work_counter = 0;      // k_solve of this substep starts its group queue at 0
+  if (env - (P.G == 2 ? (env & 1) : 0) >= P.E) return;              // no env of this warp's group exists (the whole group leaves)
+  const bool present = env < P.E;
+  const Scratch L = scratch_layout(P.pc, P.G);
   float* scr = P.scratch + (size_t)env * P.scratch_words;
   int* meta = reinterpret_cast<int*>(scr + L.meta);
-  if (honour_rest && meta[MetaResting]) return;
-  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaDetect), ArenaDetect);
+  // an env at rest (jenga_simulate_until_rest) is skipped, but its warp still takes part in the group's plan (with no pairs)
+  const bool live = present && !(honour_rest && meta[MetaResting]);
+  if (mode == ModeBroad && !live) return;
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaDetect, P.G), ArenaDetect, P.G);
   unsigned st = 0;
   int n_cand = 0, n_coll = 0;
-  load_predict(s, P, env, mode == ModeStep);
-  if (mode == ModeStep || mode == ModeBroad) {
-    n_cand = broadphase(s, P, &st);
-    if (mode == ModeBroad || P.materialise) write_pairs(s, P, env, n_cand);
-  } else if (mode == ModeNarrow) {
-    n_cand = load_candidates(s, P, env);
-  }
-  if (mode == ModeStep || mode == ModeNarrow) n_coll = find_colliding(s, P, n_cand, &st);
-  if (mode == ModeGiven) {
-    const int n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
-    n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
-    unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
-    for (int r = lane; r < n_coll; r += 32) gcoff[r] = s.wrank[r];       // the colouring reuses s.wrank
-    if (lane == 0) meta[MetaNcont] = n_cont;
-    __syncwarp();
+  if (live) {
+    load_predict(s, P, env, mode == ModeStep);
+    if (mode == ModeStep || mode == ModeBroad) {
+      n_cand = broadphase(s, P, &st);
+      if (mode == ModeBroad || P.materialise) write_pairs(s, P, env, n_cand);
+    } else if (mode == ModeNarrow) {
+      n_cand = load_candidates(s, P, env);
+    }
+    if (mode == ModeStep || mode == ModeNarrow) n_coll = find_colliding(s, P, n_cand, &st);
+    if (mode == ModeGiven) {
+      const int n_cont = max(0, min(P.n_contacts[env], P.max_contacts));
+      n_coll = pairs_from_contacts(s, P, env, n_cont, &st);
+      unsigned short* gcoff = reinterpret_cast<unsigned short*>(scr + L.coff);
+      for (int r = lane; r < n_coll; r += 32) gcoff[r] = s.wrank[r];       // the colouring reuses s.wrank
+      if (lane == 0) meta[MetaNcont] = n_cont;
+      __syncwarp();
+    }
   }
   if (mode != ModeBroad) {
-    colour_pairs(s, P, scr, L, n_coll, &st);
+    colour_pairs(s, P, env, present, n_coll, &st);
+    if (!live) return;
     if (P.counters && mode == ModeStep && lane == 0) {
       const int ncol = s.misc[MiNcol];
       atomicAdd(P.counters + JENGA_CNT_CANDIDATES, (unsigned long long)n_cand);
@@ -967,7 +1069,7 @@ __global__ void __launch_bounds__(128, 5) k_detect(const Params P, const int hon
       atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
     }
   }
-  flush_status(P, env, st);
+  if (live) flush_status(P, env, st);
 }
 
 template <int mode>
@@ -975,10 +1077,10 @@ __global__ void __launch_bounds__(128, 5) k_manifold(const Params P, const int h
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
   const int env = blockIdx.x * wpc + warp;
   if (env >= P.E) return;
-  const Scratch L = scratch_layout(P.pc);
+  const Scratch L = scratch_layout(P.pc, P.G);
   float* scr = P.scratch + (size_t)env * P.scratch_words;
   if (honour_rest && reinterpret_cast<int*>(scr + L.meta)[MetaResting]) return;
-  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaManifold), ArenaManifold);
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaManifold, P.G), ArenaManifold, P.G);
   load_predict(s, P, env, false, false);                                 // the records again (k_detect changed v, w only)
   const int n_coll = load_colliding(s, scr, L, false);
   manifold_pairs(s, P, env, scr, L, n_coll, mode == ModeNarrow || P.materialise);
@@ -989,16 +1091,17 @@ __global__ void __launch_bounds__(128, 2) k_slot(const Params P, const int honou
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
   const int env = blockIdx.x * wpc + warp;
   if (env >= P.E) return;
-  const Scratch L = scratch_layout(P.pc);
+  const Scratch L = scratch_layout(P.pc, P.G);
   float* scr = P.scratch + (size_t)env * P.scratch_words;
   int* meta = reinterpret_cast<int*>(scr + L.meta);
   if (honour_rest && meta[MetaResting]) return;
-  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaSlot), ArenaSlot);
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaSlot, P.G), ArenaSlot, P.G);
   load_predict(s, P, env, false, false);
   const int n_coll = load_colliding(s, scr, L, true);
   const int nprev = load_prev_keys(s, P, env);
-  if (mode == ModeGiven) setup_given(s, P, env, scr, L, n_coll, meta[MetaNcont], nprev);
-  else setup_pairs(s, P, env, scr, L, n_coll, nprev);
+  float* scr0 = P.scratch + (size_t)(env - (P.G == 2 ? (env & 1) : 0)) * P.scratch_words;      // the group's blocks
+  if (mode == ModeGiven) setup_given(s, P, env, scr, scr0, L, n_coll, meta[MetaNcont], nprev);
+  else setup_pairs(s, P, env, scr, scr0, L, n_coll, nprev);
 }
 
 }  // namespace jenga

@@ -1,53 +1,50 @@
-// ksolve.cuh -- second kernel of a substep, one env per warp: S4 warm-start application, S5 coloured PGS sweeps,
-// S6 integration + Baumgarte, S7 warm-start cache, Eq. 18 latch.  Inputs: the state tile and the scratch k_slot wrote.
+// ksolve.cuh -- fourth kernel of a substep, one GROUP of G envs per warp (layout.cuh): S4 warm-start application, S5
+// coloured PGS sweeps, S6 integration + Baumgarte, S7 warm-start cache, Eq. 18 latch.  Inputs: the state tiles of the
+// group's envs and the blocks + chunk list k_detect / k_slot left in the scratch of the group's first env.
 //
 // Two flavours (template <bool TM>):
-//   TM = true   ONE persistent CTA per SM of 4 G warps = 4 G envs in flight (G = 3, 2 or 1) that owns all 512 columns of
-//               tensor memory.  Warp w works in TMEM lanes 32 (w % 4) .. + 31 (its quadrant) and columns
-//               [48 tmb (w / 4), + 48 tmb): the 48 constant words of the positions of the env's first `tmb` 32-position
-//               blocks (tmb = 2, 3, 5, 10 for G = 4, 3, 2, 1; tcgen05.ld/st.32x32b: lane = position % 32, block j at column
-//               offset 48 j).  Blocks >= tmb stay where k_slot wrote them, in the scratch (L2-resident while the env is
+//   TM = true   ONE persistent CTA per SM of 4 Q warps = 4 Q groups in flight (Q = 4, 3, 2 or 1) that owns all 512 columns
+//               of tensor memory.  Warp w works in TMEM lanes 32 (w % 4) .. + 31 (its quadrant) and columns
+//               [56 tmb (w / 4), + 56 tmb): the 56 words of the positions of the group's first `tmb` 32-position blocks
+//               (tmb = 2, 3, 4, 9 for Q = 4, 3, 2, 1; tcgen05.ld/st.32x32b: lane = position % 32, block j at column
+//               offset 56 j).  Blocks >= tmb stay where k_slot wrote them, in the scratch (L2-resident while the group is
 //               in flight): their visits load and store global memory, one visit ahead of use.
-//   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers; test coverage).
+//   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers; small batches).
 #pragma once
 #include "kcollide.cuh"
 
 namespace jenga {
 
 struct SSm {
-  SP<float> bd;                 // [S + 1][kBd] solver body records; record S is the ground: all zeros, never changes
-  SP<float> q;                  // [4][S]
-  SP<float4> hdr;               // [2][npos] the first two float4 of the pair headers (t1 is recomputed from n)
+  SP<float> bd;                 // [G S + 1][kBd] solver body records of the group (member m's body b: record m S + b);
+                                // the last record is the ground: all zeros, never changes
   SP<float4> cs;                // TM = false: [nblk][kCsF4][32] every block in shared memory
   SP<int> ph;                   // [ph_max]
-  int npos, tmb;
+  int tmb;
   unsigned tm;                  // TMEM address of this warp's lanes, first column of its group
-  float4* gcs;                  // TM = true: the env's constant blocks in the scratch (blocks >= tmb are used in place)
+  float4* gcs;                  // TM = true: the group's blocks in the scratch (blocks >= tmb are used in place)
 };
 
 // tmb = 0: the all-shared-memory flavour
-__host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb) {
-  const int nblk = n_blocks(pc);
-  size_t w = (size_t)(kBd + 4) * S + kBd + 4 * 2 * 32 * (size_t)nblk;
+__host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb, int G) {
+  const int nblk = n_blocks(pc, G);
+  size_t w = (size_t)kBd * (G * S + 1);
   w += tmb ? 0 : (size_t)kBlkWords * nblk;
-  w += round_up(ph_max(nblk), 4);
+  w += round_up(ph_max(nblk, G), 4);
   return round_up((int)w, 4);
 }
 
-__device__ inline SSm carve_solve(int S, int pc, int tmb, int base) {
-  const int nblk = n_blocks(pc);
+__device__ inline SSm carve_solve(int S, int pc, int tmb, int G, int base) {
+  const int nblk = n_blocks(pc, G);
   SSm s; int p = base;
-  s.npos = 32 * nblk; s.tmb = tmb; s.tm = 0; s.gcs = nullptr;
-  s.hdr.off = p; p += 4 * 2 * s.npos;
+  s.tmb = tmb; s.tm = 0; s.gcs = nullptr;
   s.cs.off = p;  p += tmb ? 0 : kBlkWords * nblk;
-  s.bd.off = p;  p += kBd * (S + 1);
-  s.q.off = p;   p += 4 * S;
+  s.bd.off = p;  p += kBd * (G * S + 1);
   s.ph.off = p;
   return s;
 }
 
 __device__ __forceinline__ float4& bd4(const SSm& s, int b, int k) { return reinterpret_cast<float4*>(smem_f + s.bd.off + b * kBd)[k]; }
-__device__ __forceinline__ float4& hdr4(const SSm& s, int f, int k) { return s.hdr[f * s.npos + k]; }
 
 // ---------------------------------------------------------------- TMEM access
 __device__ __forceinline__ void tm_ld16(unsigned a, float* r) {
@@ -55,6 +52,11 @@ __device__ __forceinline__ void tm_ld16(unsigned a, float* r) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
                : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]), "=r"(u[6]), "=r"(u[7]),
                  "=r"(u[8]), "=r"(u[9]), "=r"(u[10]), "=r"(u[11]), "=r"(u[12]), "=r"(u[13]), "=r"(u[14]), "=r"(u[15]) : "r"(a));
+}
+__device__ __forceinline__ void tm_ld8(unsigned a, float* r) {
+  unsigned* u = reinterpret_cast<unsigned*>(r);
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]), "=r"(u[6]), "=r"(u[7]) : "r"(a));
 }
 __device__ __forceinline__ void tm_st16(unsigned a, const float* r) {
   const unsigned* u = reinterpret_cast<const unsigned*>(r);
@@ -76,21 +78,15 @@ __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sy
 
 // whole block j (all 32 lanes take part; lane l gets position 32 j + l)
 __device__ __forceinline__ void tm_load_block(const SSm& s, int j, PairC& c) {
-  const unsigned a = s.tm + 48u * (unsigned)j;
-#ifdef EXP_SKIP_LDTM
-  tm_ld16(a + 32, c.v + 32);
-#pragma unroll
-  for (int t = 0; t < 32; ++t) c.v[t] = c.v[32 + (t & 15)];
-#else
-  tm_ld16(a, c.v); tm_ld16(a + 16, c.v + 16); tm_ld16(a + 32, c.v + 32);
-#endif
+  const unsigned a = s.tm + (unsigned)kTmCols * (unsigned)j;
+  tm_ld16(a, c.v); tm_ld16(a + 16, c.v + 16); tm_ld16(a + 32, c.v + 32); tm_ld8(a + 48, c.v + 48);
 }
 __device__ __forceinline__ void tm_store_block(const SSm& s, int j, const PairC& c) {
-  const unsigned a = s.tm + 48u * (unsigned)j;
-  tm_st16(a, c.v); tm_st16(a + 16, c.v + 16); tm_st16(a + 32, c.v + 32);
+  const unsigned a = s.tm + (unsigned)kTmCols * (unsigned)j;
+  tm_st16(a, c.v); tm_st16(a + 16, c.v + 16); tm_st16(a + 32, c.v + 32); tm_st8(a + 48, c.v + 48);
 }
 __device__ __forceinline__ void tm_store_lam(const SSm& s, int j, const float* lam) {
-  const unsigned a = s.tm + 48u * (unsigned)j + 36u;
+  const unsigned a = s.tm + (unsigned)kTmCols * (unsigned)j + (unsigned)kLam;
   tm_st8(a, lam); tm_st4(a + 8, lam + 8);
 }
 // blocks outside tensor memory, lane l: shared memory (TM = false) or the scratch itself (TM = true, block j >= tmb)
@@ -112,23 +108,27 @@ template <bool TM>
 __device__ __forceinline__ void sm_store_lam(const SSm& s, int j, int l, const float* lam) {
   float4* b = ov_ptr<TM>(s, j, l);
 #pragma unroll
-  for (int f = 0; f < 3; ++f) b[(9 + f) * 32] = make_float4(lam[4 * f], lam[4 * f + 1], lam[4 * f + 2], lam[4 * f + 3]);
+  for (int f = 0; f < 3; ++f) b[(kLam / 4 + f) * 32] = make_float4(lam[4 * f], lam[4 * f + 1], lam[4 * f + 2], lam[4 * f + 3]);
 }
-// block j of this env: lane l <-> position 32 j + l.  All lanes call these.
+// The lane whose pair lane `lane` loads from a block outside tensor memory: its own inside the chunk d, the chunk's first
+// lane otherwise (a block in the scratch costs L2 bandwidth per sector touched; the duplicate addresses cost nothing and
+// there is no divergent branch around the 14 loads).
+__device__ __forceinline__ int load_lane(int d, int lane) { const int l0 = d & 0xff; return lane >= l0 && lane < l0 + ((d >> 8) & 0xff) ? lane : l0; }
+// block of chunk d of this group: lane l <-> position 32 j + l.  All lanes call this.
 template <bool TM>
-__device__ __forceinline__ void block_load(const SSm& s, int j, PairC& c) {
+__device__ __forceinline__ void block_load(const SSm& s, int d, PairC& c) {
+  const int j = d >> 16;
   if (TM && j < s.tmb) { tm_load_block(s, j, c); tm_wait_ld(); }
-  else sm_load_pair<TM>(s, j, lane_id(), c);
+  else sm_load_pair<TM>(s, j, load_lane(d, lane_id()), c);
 }
 
 // ---------------------------------------------------------------- warp / TMEM set-up
 template <bool TM>
-__device__ __forceinline__ SSm begin_solve(const Params& P, int& env) {
+__device__ __forceinline__ SSm begin_solve(const Params& P) {
   __shared__ unsigned tm_base_s;
-  const int warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
-  env = blockIdx.x * wpc + warp;
+  const int warp = threadIdx.x >> 5;
   const int tmb = TM ? P.tmb : 0;
-  SSm s = carve_solve(P.S, P.pc, tmb, warp * (int)solve_smem_words(P.S, P.pc, tmb));
+  SSm s = carve_solve(P.S, P.pc, tmb, P.G, warp * (int)solve_smem_words(P.S, P.pc, tmb, P.G));
   if (TM) {
     if (warp == 0) {
       asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
@@ -138,7 +138,7 @@ __device__ __forceinline__ SSm begin_solve(const Params& P, int& env) {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    s.tm = tm_base_s + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)(48 * tmb * (warp >> 2));
+    s.tm = tm_base_s + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)(kTmCols * tmb * (warp >> 2));
   }
   return s;
 }
@@ -154,12 +154,12 @@ __device__ __forceinline__ void end_solve(const SSm& s) {
 }
 
 // ---------------------------------------------------------------- load
-// Body records from the state tile (lane b reads column b of every row: coalesced); Iw^-1 from q (Eq. 1).
-// Record (5 float4, stride 20 words: an odd number of 16-byte words, so 8 consecutive bodies cover all bank groups):
-// x y z im | v.xyz Ixx | w.xyz Ixy | Ixz Iyy Iyz Izz | body-frame inverse moments.  The solver reads the first four and
-// writes back the second and third (the inertia words ride along unchanged).
-__device__ inline void load_bodies(const SSm& s, const Params& P, int env) {
-  const int S = P.S;
+// Body records of member m from its state tile (lane b reads column b of every row: coalesced); Iw^-1 from q (Eq. 1,
+// PAPER.md:168).  Record (5 float4, stride 20 words: an odd number of 16-byte words, so 8 consecutive bodies cover all
+// bank groups): x y z im | v.xyz Ixx | w.xyz Ixy | Ixz Iyy Iyz Izz | q.  The solver reads the first four and writes back
+// the second and third (the inertia words ride along unchanged).
+__device__ inline void load_bodies(const SSm& s, const Params& P, int env, int m) {
+  const int S = P.S, r0 = m * S;
   const float* st = P.state + (size_t)env * kStateRows * S;
   const float* pr = P.props + (size_t)env * kPropRows * S;
   for (int b = lane_id(); b < P.B; b += 32) {
@@ -169,41 +169,36 @@ __device__ inline void load_bodies(const SSm& s, const Params& P, int env) {
     float R[9]; quat_to_R(w, x, y, z, R);
     float I6[6];
     world_inv_inertia(R, dyn ? i0 : 0.0f, dyn ? i1 : 0.0f, dyn ? i2 : 0.0f, I6);
-    bd4(s, b, 0) = make_float4(st[b], st[S + b], st[2 * S + b], dyn ? im : 0.0f);
-    bd4(s, b, 1) = make_float4(st[7 * S + b], st[8 * S + b], st[9 * S + b], I6[0]);       // v, Ixx
-    bd4(s, b, 2) = make_float4(st[10 * S + b], st[11 * S + b], st[12 * S + b], I6[1]);    // w, Ixy
-    bd4(s, b, 3) = make_float4(I6[2], I6[3], I6[4], I6[5]);                                // Ixz Iyy Iyz Izz
-    bd4(s, b, 4) = make_float4(i0, i1, i2, 0.0f);                                          // body-frame inverse moments (Eq. 18)
-    s.q[b] = w; s.q[S + b] = x; s.q[2 * S + b] = y; s.q[3 * S + b] = z;
+    bd4(s, r0 + b, 0) = make_float4(st[b], st[S + b], st[2 * S + b], dyn ? im : 0.0f);
+    bd4(s, r0 + b, 1) = make_float4(st[7 * S + b], st[8 * S + b], st[9 * S + b], I6[0]);       // v, Ixx
+    bd4(s, r0 + b, 2) = make_float4(st[10 * S + b], st[11 * S + b], st[12 * S + b], I6[1]);    // w, Ixy
+    bd4(s, r0 + b, 3) = make_float4(I6[2], I6[3], I6[4], I6[5]);                                // Ixz Iyy Iyz Izz
+    bd4(s, r0 + b, 4) = make_float4(w, x, y, z);
   }
-  if (lane_id() < 5) bd4(s, S, lane_id()) = make_float4(0, 0, 0, 0);      // the ground: inverse mass and inertia 0, at rest
 }
 
-__device__ inline void store_bodies(const SSm& s, const Params& P, int env) {
-  const int S = P.S;
+__device__ inline void store_bodies(const SSm& s, const Params& P, int env, int m) {
+  const int S = P.S, r0 = m * S;
   float* st = P.state + (size_t)env * kStateRows * S;
   for (int b = lane_id(); b < P.B; b += 32) {
-    const float4 x = bd4(s, b, 0), v = bd4(s, b, 1), w = bd4(s, b, 2);
+    const float4 x = bd4(s, r0 + b, 0), v = bd4(s, r0 + b, 1), w = bd4(s, r0 + b, 2), q = bd4(s, r0 + b, 4);
     if (x.w == 0.0f) continue;                                   // static / inactive bodies are never written
     st[b] = x.x; st[S + b] = x.y; st[2 * S + b] = x.z;
-    st[3 * S + b] = s.q[b]; st[4 * S + b] = s.q[S + b]; st[5 * S + b] = s.q[2 * S + b]; st[6 * S + b] = s.q[3 * S + b];
+    st[3 * S + b] = q.x; st[4 * S + b] = q.y; st[5 * S + b] = q.z; st[6 * S + b] = q.w;
     st[7 * S + b] = v.x; st[8 * S + b] = v.y; st[9 * S + b] = v.z;
     st[10 * S + b] = w.x; st[11 * S + b] = w.y; st[12 * S + b] = w.z;
   }
 }
 
-// Chunk list, headers and constant blocks of this env from the scratch.  Returns the number of chunks.
+// Chunk list and blocks of this group from the scratch of its first env.  Returns the number of chunks.
 template <bool TM>
-__device__ inline int load_slots(const SSm& s, const Params& P, const float* scr, const Scratch& L) {
+__device__ inline int load_slots(const SSm& s, const float* scr0, const Scratch& L) {
   const int lane = lane_id();
-  const int* meta = reinterpret_cast<const int*>(scr + L.meta);
+  const int* meta = reinterpret_cast<const int*>(scr0 + L.meta);
   const int nph = meta[MetaNph], nblk = meta[MetaNblk];
-  const int* gph = reinterpret_cast<const int*>(scr + L.ph);
+  const int* gph = reinterpret_cast<const int*>(scr0 + L.ph);
   for (int j = lane; j < nph; j += 32) s.ph[j] = gph[j];
-  const float4* ghdr = reinterpret_cast<const float4*>(scr + L.hdr);
-  for (int f = 0; f < 2; ++f)
-    for (int k = lane; k < 32 * nblk; k += 32) s.hdr[f * s.npos + k] = ghdr[f * s.npos + k];
-  const float4* gcs = reinterpret_cast<const float4*>(scr + L.cs);
+  const float4* gcs = reinterpret_cast<const float4*>(scr0 + L.cs);
   const int ncopy = TM ? min(nblk, s.tmb) : nblk;              // TM: blocks >= tmb are used in place
   for (int j = 0; j < ncopy; ++j) {
     PairC c;
@@ -280,51 +275,45 @@ __device__ __forceinline__ void solve_pair(PairC& c, Body5& A, Body5& B, const F
   }
 }
 
-// What a lane needs of its pair's header during a visit.
-struct Hdr { int a, b; Vec3 n; float il; };
-// a = body record of A: the ground (header field 0) is the all-zero record S
-__device__ __forceinline__ Hdr load_hdr(const SSm& s, int S, int k) {
-  const float4 h = hdr4(s, 0, k), nn = hdr4(s, 1, k);
-  Hdr H; const int ab = __float_as_int(h.x), a1 = ab & 0xffff;
-  H.a = a1 ? a1 - 1 : S; H.b = ab >> 16; H.n = xyz(nn); H.il = h.w;
-  return H;
-}
+// header words of a loaded pair
+__device__ __forceinline__ int hdr_ab(const PairC& c) { return __float_as_int(c.v[kHdr]); }
+__device__ __forceinline__ int hdr_meta(const PairC& c) { return __float_as_int(c.v[kHdr + 1]); }
+__device__ __forceinline__ int hdr_rank(const PairC& c) { return __float_as_int(c.v[kHdr + 2]); }
+__device__ __forceinline__ Frame hdr_frame(const PairC& c) { return make_frame(v3(c.v[kHdr + 4], c.v[kHdr + 5], c.v[kHdr + 6]), c.v[kHdr + 3]); }
 __device__ __forceinline__ bool chunk_lane(int d, int lane) { const int l0 = d & 0xff; return lane >= l0 && lane < l0 + ((d >> 8) & 0xff); }
 
-// S4: the cached impulses are applied once, chunk by chunk in canonical order (no impulse changes: nothing is stored).
+// S4: the cached impulses are applied once, chunk by chunk in visiting order (no impulse changes: nothing is stored).
 template <bool TM>
-__device__ inline void warm_start_pass(const SSm& s, int S, int nph) {
+__device__ inline void warm_start_pass(const SSm& s, int nph) {
   const int lane = lane_id();
   for (int j = 0; j < nph; ++j) {
     const int d = s.ph[j], jb = d >> 16;
-    PairC c; block_load<TM>(s, jb, c);
+    PairC c; block_load<TM>(s, d, c);
     if (chunk_lane(d, lane)) {
-      const Hdr H = load_hdr(s, S, 32 * jb + lane);
-      Body5 A, B; load_body(s, H.a, A); load_body(s, H.b, B);
-      const Frame F = make_frame(H.n, H.il);
+      const int ab = hdr_ab(c), a = ab & 0xffff, b = ab >> 16;
+      Body5 A, B; load_body(s, a, A); load_body(s, b, B);
+      const Frame F = hdr_frame(c);
       solve_pair<true>(c, A, B, F, 0.0f);
-      store_body_vel(s, H.a, A); store_body_vel(s, H.b, B);
+      store_body_vel(s, a, A); store_body_vel(s, b, B);
     }
     __syncwarp();
   }
 }
 
-// S5: `iters` Gauss-Seidel sweeps over the chunks in canonical order, as ONE software-pipelined loop over the
-// iters * nph chunk visits.  A visit: the chunk's pairs are lanes [lane0, lane0 + count) of block jb; pairs of one
-// colour share no dynamic body.  While the contacts of visit v run, the header of visit v + 1 is fetched from shared
-// memory, and as soon as the impulses of v are stored the constants of v + 1 are requested from tensor memory, so that
-// the next visit starts with the (dependent) body loads at once.  TMEM accesses are warp-wide: the lanes outside the
-// chunk write back the impulses they loaded.
+// S5: `iters` Gauss-Seidel sweeps over the chunks in visiting order, as ONE software-pipelined loop over the
+// iters * nph chunk visits.  A visit: the chunk's pairs are lanes [lane0, lane0 + count) of block jb; they share no
+// dynamic body.  As soon as the impulses of visit v are stored the block of visit v + 1 (constants, impulses, header) is
+// requested from tensor memory / the scratch, so that the next visit starts with its (dependent) body loads at once.
+// TMEM accesses are warp-wide: the lanes outside the chunk write back the impulses they loaded.  mu0 / mu1: the friction
+// coefficients of the group's members (the pair's member is a header bit).
 template <bool TM>
-__device__ inline void pgs_sweeps(const SSm& s, int S, int nph, int iters, float mu) {
+__device__ inline void pgs_sweeps(const SSm& s, int nph, int iters, float mu0, float mu1) {
   const int total = nph * iters, lane = lane_id();
   if (total <= 0) return;
   int d = s.ph[0], jn = 0;
   PairC c;
-  Hdr H; H.a = S; H.b = S; H.n = v3(0, 0, 0); H.il = 0.0f;
-  if (chunk_lane(d, lane)) H = load_hdr(s, S, 32 * (d >> 16) + lane);
   if (TM && (d >> 16) < s.tmb) tm_load_block(s, d >> 16, c);
-  else sm_load_pair<TM>(s, d >> 16, lane, c);
+  else sm_load_pair<TM>(s, d >> 16, load_lane(d, lane), c);
 #pragma unroll 1
   for (int v = 0; v < total; ++v) {
     const int jb = d >> 16;
@@ -332,35 +321,34 @@ __device__ inline void pgs_sweeps(const SSm& s, int S, int nph, int iters, float
     jn = jn + 1 == nph ? 0 : jn + 1;
     const int dn = s.ph[jn];
     if (in_tm) tm_wait_ld();
-    // every lane fetches the header of its position in the next chunk's block (garbage outside the chunk: never used)
-    const Hdr Hn = load_hdr(s, S, 32 * (dn >> 16) + lane);
     if (active) {
-      Body5 A, B; load_body(s, H.a, A); load_body(s, H.b, B);
-      const Frame F = make_frame(H.n, H.il);
-      solve_pair<false>(c, A, B, F, mu);
-      store_body_vel(s, H.a, A); store_body_vel(s, H.b, B);
+      const int ab = hdr_ab(c), a = ab & 0xffff, b = ab >> 16;
+      Body5 A, B; load_body(s, a, A); load_body(s, b, B);
+      const Frame F = hdr_frame(c);
+      solve_pair<false>(c, A, B, F, (hdr_meta(c) & kMetaMember) ? mu1 : mu0);
+      store_body_vel(s, a, A); store_body_vel(s, b, B);
       if (!in_tm) sm_store_lam<TM>(s, jb, lane, c.v + kLam);
     }
     if (in_tm) { tm_store_lam(s, jb, c.v + kLam); tm_wait_st(); }
     __syncwarp();
     if (TM && (dn >> 16) < s.tmb) tm_load_block(s, dn >> 16, c);
-    else sm_load_pair<TM>(s, dn >> 16, lane, c);
-    d = dn; H = Hn;
+    else sm_load_pair<TM>(s, dn >> 16, load_lane(dn, lane), c);
+    d = dn;
   }
   if (TM) tm_wait_ld();
 }
 
-// S6: x += h v (Eq. 6); q <- normalise(q + h/2 [0,w] (x) q) (Eq. 2, world-frame
-// reading A3); then Eq. 16 (reading A14) once per colliding pair, chunk by chunk.
-__device__ inline void integrate(const SSm& s, const Params& P, int nph, unsigned* status) {
-  const int S = P.S, lane = lane_id(); const float h = P.h;
-  for (int b = lane; b < P.B; b += 32) {
-    float4 x = bd4(s, b, 0);
+// S6, bodies of member m: x += h v (Eq. 6); q <- normalise(q + h/2 [0,w] (x) q) (Eq. 2, PAPER.md:151,
+// world-frame reading A3).
+__device__ inline void integrate_bodies(const SSm& s, const Params& P, int m, unsigned* status) {
+  const int r0 = m * P.S; const float h = P.h;
+  for (int b = lane_id(); b < P.B; b += 32) {
+    float4 x = bd4(s, r0 + b, 0);
     if (x.w == 0.0f) continue;                                   // static or inactive
-    const float4 v = bd4(s, b, 1), om = bd4(s, b, 2);
+    const float4 v = bd4(s, r0 + b, 1), om = bd4(s, r0 + b, 2), q = bd4(s, r0 + b, 4);
     x.x += h * v.x; x.y += h * v.y; x.z += h * v.z;
-    bd4(s, b, 0) = x;
-    const float qw = s.q[b], qx = s.q[S + b], qy = s.q[2 * S + b], qz = s.q[3 * S + b];
+    bd4(s, r0 + b, 0) = x;
+    const float qw = q.x, qx = q.y, qy = q.z, qz = q.w;
     const float dw = -(om.x * qx + om.y * qy + om.z * qz);
     const float dx = om.x * qw + om.y * qz - om.z * qy;
     const float dy = om.y * qw + om.z * qx - om.x * qz;
@@ -368,63 +356,37 @@ __device__ inline void integrate(const SSm& s, const Params& P, int nph, unsigne
     const float hh = 0.5f * h;
     const float nw = qw + hh * dw, nx = qx + hh * dx, ny = qy + hh * dy, nz = qz + hh * dz;
     const float il = 1.0f / sqrtf(nw * nw + nx * nx + ny * ny + nz * nz);
-    s.q[b] = nw * il; s.q[S + b] = nx * il; s.q[2 * S + b] = ny * il; s.q[3 * S + b] = nz * il;
+    bd4(s, r0 + b, 4) = make_float4(nw * il, nx * il, ny * il, nz * il);
     const float chk = (x.x + x.y + x.z) + (v.x + v.y + v.z) + (om.x + om.y + om.z) + il;      // any inf/NaN poisons the sum
     if (!isfinite(chk)) *status |= JENGA_ST_NONFINITE;
-  }
-  __syncwarp();
-  for (int j = 0; j < nph; ++j) {
-    const int d = s.ph[j], lane0 = d & 0xff, count = (d >> 8) & 0xff, k = 32 * (d >> 16) + lane;
-    float4 nn = make_float4(0, 0, 0, 0);
-    if (lane >= lane0 && lane < lane0 + count) nn = hdr4(s, 1, k);
-    if (__any_sync(kFull, nn.w > 0.0f)) {
-      if (nn.w > 0.0f) {
-        const int ab = __float_as_int(hdr4(s, 0, k).x), a = (ab & 0xffff) - 1, b = ab >> 16;
-        float4 xb = bd4(s, b, 0);
-        if (xb.w != 0.0f) {
-          const float f = xb.w * nn.w;
-          xb.x += f * nn.x; xb.y += f * nn.y; xb.z += f * nn.z;
-          bd4(s, b, 0) = xb;
-        }
-        if (a >= 0) {
-          float4 xa = bd4(s, a, 0);
-          if (xa.w != 0.0f) {
-            const float f = xa.w * nn.w;
-            xa.x -= f * nn.x; xa.y -= f * nn.y; xa.z -= f * nn.z;
-            bd4(s, a, 0) = xa;
-          }
-        }
-      }
-      __syncwarp();
-    }
   }
 }
 
 // Per-body terms of Eq. 18 / PAPER.md:380: kinetic energy 1/2 m |v|^2 + 1/2 w . I w with I in the body frame
-// (R^T w against the principal moments, R from the new q, Eq. 1).
-__device__ __forceinline__ float body_kinetic_energy(const SSm& s, int S, int b, float4 x, float4 v, float4 w, float4 ib) {
-  const float qw = s.q[b], qx = s.q[S + b], qy = s.q[2 * S + b], qz = s.q[3 * S + b];
-  float R[9]; quat_to_R(qw, qx, qy, qz, R);
+// (R^T w against the principal moments, R from the new q, Eq. 1).  ib: body-frame inverse moments.
+__device__ __forceinline__ float body_kinetic_energy(float4 q, float4 x, float4 v, float4 w, float ib0, float ib1, float ib2) {
+  float R[9]; quat_to_R(q.x, q.y, q.z, q.w, R);
   const float w0 = R[0] * w.x + R[3] * w.y + R[6] * w.z, w1 = R[1] * w.x + R[4] * w.y + R[7] * w.z, w2 = R[2] * w.x + R[5] * w.y + R[8] * w.z;
-  return 0.5f * (v.x * v.x + v.y * v.y + v.z * v.z) / x.w + 0.5f * (w0 * w0 / ib.x + w1 * w1 / ib.y + w2 * w2 / ib.z);
+  return 0.5f * (v.x * v.x + v.y * v.y + v.z * v.z) / x.w + 0.5f * (w0 * w0 / ib0 + w1 * w1 / ib1 + w2 * w2 / ib2);
 }
 
-// Collapse latch (Eq. 18, reading A17) after a dt advance: dx_max = max_b |x_b - x_b(0)|,
+// Collapse latch (Eq. 18, reading A17) of member m after a dt advance: dx_max = max_b |x_b - x_b(0)|,
 // theta_max = max_b 2 acos|q_b . q_b(0)|, E_k; collapsed |= all three above their thresholds at this step.
 // Returns E_k (all lanes).
-__device__ inline float collapse_latch(const SSm& s, const Params& P, int env, bool latch) {
-  const int S = P.S, lane = lane_id();
+__device__ inline float collapse_latch(const SSm& s, const Params& P, int env, int m, bool latch) {
+  const int S = P.S, lane = lane_id(), r0 = m * S;
   const float* ref = latch ? P.ref_pose + (size_t)env * 7 * S : nullptr;
+  const float* pr = P.props + (size_t)env * kPropRows * S;
   float dxm = 0.0f, thm = 0.0f, ek = 0.0f;
   for (int b = lane; b < P.B; b += 32) {
-    const float4 x = bd4(s, b, 0);
+    const float4 x = bd4(s, r0 + b, 0);
     if (x.w == 0.0f) continue;
-    const float4 v = bd4(s, b, 1), w = bd4(s, b, 2);
-    ek += body_kinetic_energy(s, S, b, x, v, w, bd4(s, b, 4));
+    const float4 v = bd4(s, r0 + b, 1), w = bd4(s, r0 + b, 2), q = bd4(s, r0 + b, 4);
+    ek += body_kinetic_energy(q, x, v, w, pr[S + b], pr[2 * S + b], pr[3 * S + b]);
     if (latch) {
       const float dx = x.x - ref[b], dy = x.y - ref[S + b], dz = x.z - ref[2 * S + b];
       dxm = fmaxf(dxm, sqrtf(dx * dx + dy * dy + dz * dz));
-      const float c = fminf(fabsf(s.q[b] * ref[3 * S + b] + s.q[S + b] * ref[4 * S + b] + s.q[2 * S + b] * ref[5 * S + b] + s.q[3 * S + b] * ref[6 * S + b]), 1.0f);
+      const float c = fminf(fabsf(q.x * ref[3 * S + b] + q.y * ref[4 * S + b] + q.z * ref[5 * S + b] + q.w * ref[6 * S + b]), 1.0f);
       thm = fmaxf(thm, 2.0f * acosf(c));
     }
   }
@@ -440,20 +402,45 @@ __device__ inline float collapse_latch(const SSm& s, const Params& P, int env, b
   return ek;
 }
 
-// S7: every pair's impulses and contact points become the next substep's warm-start cache, in ascending
-// pair order (cache entry r = pair rank r, from the header).  Returns the lane's (contacts, ground contacts).
+// One pass over the chunks in visiting order after the sweeps.  `baumgarte`: Eq. 16 (reading A14) once per
+// colliding pair (after the bodies were integrated; pairs of a chunk share no dynamic body).  S7 (`cache_out`): every
+// pair's impulses and contact points become the next substep's warm-start cache of its env (cache entry r = the pair's
+// rank in the env's ascending pair list, from the header).  `lambda_out`: the impulses in contact order (stage output).
+// Returns the lane's (contacts, ground contacts).
 template <bool TM>
-__device__ inline int2 store_cache(const SSm& s, const Params& P, int env, const float* scr, const Scratch& L, int nph, bool cache_out, bool lambda_out) {
+__device__ inline int2 finish_pairs(const SSm& s, const Params& P, int env0, const Scratch& L, int nph, bool baumgarte, bool cache_out, bool lambda_out) {
   const int lane = lane_id();
-  const unsigned short* gcoff = reinterpret_cast<const unsigned short*>(scr + L.coff);
   int nc = 0, ng = 0;
   for (int j = 0; j < nph; ++j) {
-    const int d = s.ph[j], jb = d >> 16, lane0 = d & 0xff, count = (d >> 8) & 0xff, k = 32 * jb + lane;
-    PairC c; block_load<TM>(s, jb, c);
-    if (lane >= lane0 && lane < lane0 + count) {
-      const float4 hd = hdr4(s, 0, k);
-      const int meta = __float_as_int(hd.y), np = meta & 0xff, r = __float_as_int(hd.z);
-      nc += np; if ((__float_as_int(hd.x) & 0xffff) == 0) ng += np;
+    const int d = s.ph[j], jb = d >> 16;
+    const bool active = chunk_lane(d, lane);
+    PairC c; block_load<TM>(s, d, c);
+    if (baumgarte) {
+      const float corr = active ? c.v[kHdr + 7] : 0.0f;
+      if (__any_sync(kFull, corr > 0.0f)) {
+        if (corr > 0.0f) {
+          const int ab = hdr_ab(c), a = ab & 0xffff, b = ab >> 16;
+          const Vec3 n = v3(c.v[kHdr + 4], c.v[kHdr + 5], c.v[kHdr + 6]);
+          float4 xb = bd4(s, b, 0);
+          if (xb.w != 0.0f) {
+            const float f = xb.w * corr;
+            xb.x += f * n.x; xb.y += f * n.y; xb.z += f * n.z;
+            bd4(s, b, 0) = xb;
+          }
+          float4 xa = bd4(s, a, 0);                              // the ground's record has inverse mass 0
+          if (xa.w != 0.0f) {
+            const float f = xa.w * corr;
+            xa.x -= f * n.x; xa.y -= f * n.y; xa.z -= f * n.z;
+            bd4(s, a, 0) = xa;
+          }
+        }
+        __syncwarp();
+      }
+    }
+    if (active) {
+      const int meta = hdr_meta(c), np = meta & 0xff, r = hdr_rank(c);
+      const int env = env0 + ((meta & kMetaMember) ? 1 : 0);
+      nc += np; if (meta & kMetaGround) ng += np;
       if (cache_out) {
         int* key = P.cache_key + ((size_t)env * P.pc + r) * 2;
         key[0] = (int)((unsigned)meta >> 16); key[1] = meta & 0xfff;
@@ -471,6 +458,7 @@ __device__ inline int2 store_cache(const SSm& s, const Params& P, int env, const
         }
       }
       if (lambda_out) {                                          // lambda in contact order (debug / stage output)
+        const unsigned short* gcoff = reinterpret_cast<const unsigned short*>(P.scratch + (size_t)env * P.scratch_words + L.coff);
         float* out = P.lambda + ((size_t)env * P.max_contacts + gcoff[r]) * 3;
 #pragma unroll
         for (int ci = 0; ci < 4; ++ci)
@@ -481,21 +469,22 @@ __device__ inline int2 store_cache(const SSm& s, const Params& P, int env, const
   return make_int2(nc, ng);
 }
 
-// L2 prefetch of what load_bodies / load_slots will read of env e (128-byte lines, lanes strided).
-__device__ inline void prefetch_env(const Params& P, const Scratch& L, int e) {
+// L2 prefetch of what the warp will read of group g (128-byte lines, lanes strided).
+__device__ inline void prefetch_group(const Params& P, const Scratch& L, int g) {
   const int lane = lane_id();
-  const char* st = reinterpret_cast<const char*>(P.state + (size_t)e * kStateRows * P.S);
-  for (int o = 128 * lane; o < kStateRows * P.S * 4; o += 4096) prefetch_l2(st + o);
-  const char* pr = reinterpret_cast<const char*>(P.props + (size_t)e * kPropRows * P.S);
-  for (int o = 128 * lane; o < 4 * P.S * 4; o += 4096) prefetch_l2(pr + o);
-  const float* scr = P.scratch + (size_t)e * P.scratch_words;
-  const int nblk = reinterpret_cast<const int*>(scr + L.meta)[MetaNblk];
-  const char* hd = reinterpret_cast<const char*>(scr + L.hdr);
-  for (int f = 0; f < 2; ++f)
-    for (int o = 128 * lane; o < 32 * nblk * 16; o += 4096) prefetch_l2(hd + (size_t)f * 32 * P.nblk * 16 + o);
-  const char* cs = reinterpret_cast<const char*>(scr + L.cs);
+  for (int m = 0; m < P.G; ++m) {
+    const int e = g * P.G + m;
+    if (e >= P.E) break;
+    const char* st = reinterpret_cast<const char*>(P.state + (size_t)e * kStateRows * P.S);
+    for (int o = 128 * lane; o < kStateRows * P.S * 4; o += 4096) prefetch_l2(st + o);
+    const char* pr = reinterpret_cast<const char*>(P.props + (size_t)e * kPropRows * P.S);
+    for (int o = 128 * lane; o < 4 * P.S * 4; o += 4096) prefetch_l2(pr + o);
+  }
+  const float* scr0 = P.scratch + (size_t)g * P.G * P.scratch_words;
+  const int nblk = reinterpret_cast<const int*>(scr0 + L.meta)[MetaNblk];
+  const char* cs = reinterpret_cast<const char*>(scr0 + L.cs);
   for (int o = 128 * lane; o < nblk * kBlkWords * 4; o += 4096) prefetch_l2(cs + o);
-  prefetch_l2(scr + L.ph + 32 * (lane & 1));
+  prefetch_l2(scr0 + L.ph + 32 * (lane & 3));
 }
 
 // ---------------------------------------------------------------- the kernel
@@ -505,72 +494,93 @@ enum { SolveEndOfStep = 1, SolvePgsOnly = 2, SolveRest = 4 };
 
 template <bool TM>
 __global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
-  int env0;
-  SSm s = begin_solve<TM>(P, env0);
-  const int lane = lane_id();
-  const Scratch L = scratch_layout(P.pc);
-  // persistent: every warp takes the next env of a global queue (an atomic counter that k_detect reset): envs differ in
-  // cost by the number of colliding pairs, so a static split would leave warps idle at the end.  TMEM is allocated once
-  // per CTA; the warps of a CTA never wait for one another between envs.
-  // The queue is read one env ahead: while env e is solved, the state tile, the headers and the used constant blocks of
-  // the warp's next env are prefetched into L2 (they were written a whole batch ago, i.e. they come from HBM).
-  // A batch smaller than the machine (E < warps in the grid) is spread evenly: only the first ceil(E / CTAs) warps of
-  // every CTA draw from the queue, so that no SM solves 16 envs while others idle.
-  (void)env0;
-  const bool draws = (int)(threadIdx.x >> 5) < (P.E + (int)gridDim.x - 1) / (int)gridDim.x;
-  int env_next = P.E;
-  if (draws && lane == 0) env_next = atomicAdd(P.work_counter, 1);
-  env_next = __shfl_sync(kFull, env_next, 0);
+  SSm s = begin_solve<TM>(P);
+  const int lane = lane_id(), G = P.G;
+  const Scratch L = scratch_layout(P.pc, G);
+  const int n_groups = (P.E + G - 1) / G;
+  // persistent: every warp takes the next group of a global queue (an atomic counter that k_detect reset): groups differ
+  // in cost by the number of colliding pairs, so a static split would leave warps idle at the end.  TMEM is allocated once
+  // per CTA; the warps of a CTA never wait for one another between groups.
+  // The queue is read one group ahead: while group g is solved, the state tiles and the used blocks of the warp's next
+  // group are prefetched into L2 (they were written a whole batch ago, i.e. they come from HBM).
+  // A batch smaller than the machine (fewer groups than warps in the grid) is spread evenly: only the first
+  // ceil(groups / CTAs) warps of every CTA draw from the queue, so that no SM solves 16 groups while others idle.
+  const bool draws = (int)(threadIdx.x >> 5) < (n_groups + (int)gridDim.x - 1) / (int)gridDim.x;
+  int g_next = n_groups;
+  if (draws && lane == 0) g_next = atomicAdd(P.work_counter, 1);
+  g_next = __shfl_sync(kFull, g_next, 0);
   for (;;) {
-    const int env = env_next;
-    if (env >= P.E) break;
-    if (lane == 0) env_next = atomicAdd(P.work_counter, 1);
-    env_next = __shfl_sync(kFull, env_next, 0);
-    if (env_next < P.E) prefetch_env(P, L, env_next);
-    float* scr = P.scratch + (size_t)env * P.scratch_words;
-    int* meta = reinterpret_cast<int*>(scr + L.meta);
-    if ((flags & SolveRest) && meta[MetaResting]) continue;
-    unsigned st = 0;
-    s.gcs = reinterpret_cast<float4*>(scr + L.cs);
-    load_bodies(s, P, env);
-    const int nph = load_slots<TM>(s, P, scr, L);
-    if (P.warm_start) warm_start_pass<TM>(s, P.S, nph);
-    pgs_sweeps<TM>(s, P.S, nph, iters, P.mu[env]);
+    const int g = g_next;
+    if (g >= n_groups) break;
+    if (lane == 0) g_next = atomicAdd(P.work_counter, 1);
+    g_next = __shfl_sync(kFull, g_next, 0);
+    if (g_next < n_groups) prefetch_group(P, L, g_next);
+    const int env0 = g * G, nm = min(G, P.E - env0);
+    float* scr0 = P.scratch + (size_t)env0 * P.scratch_words;
+    bool act[kMaxGroup]; bool any = false;
+#pragma unroll
+    for (int m = 0; m < kMaxGroup; ++m) {
+      act[m] = m < nm;
+      if (act[m] && (flags & SolveRest)) act[m] = reinterpret_cast<const int*>(scr0 + (size_t)m * P.scratch_words + L.meta)[MetaResting] == 0;
+      any = any || act[m];
+    }
+    if (!any) continue;
+    s.gcs = reinterpret_cast<float4*>(scr0 + L.cs);
+#pragma unroll
+    for (int m = 0; m < kMaxGroup; ++m) if (act[m]) load_bodies(s, P, env0 + m, m);
+    if (lane < 5) bd4(s, G * P.S, lane) = make_float4(0, 0, 0, 0);      // the ground: inverse mass and inertia 0, at rest
+    const int nph = load_slots<TM>(s, scr0, L);
+    if (P.warm_start) warm_start_pass<TM>(s, nph);
+    pgs_sweeps<TM>(s, nph, iters, P.mu[env0], act[kMaxGroup - 1] ? P.mu[env0 + kMaxGroup - 1] : 0.0f);
     if (flags & SolvePgsOnly) {
-      store_cache<TM>(s, P, env, scr, L, nph, false, true);      // lambda in contact order only
-      store_bodies(s, P, env);
+      finish_pairs<TM>(s, P, env0, L, nph, false, false, true);  // lambda in contact order only
+#pragma unroll
+      for (int m = 0; m < kMaxGroup; ++m) if (act[m]) store_bodies(s, P, env0 + m, m);
     } else {
-      integrate(s, P, nph, &st);
-      const int2 cc = store_cache<TM>(s, P, env, scr, L, nph, true, P.materialise != 0);
-      if (lane == 0) P.n_cache[env] = meta[MetaNcoll];
-      store_bodies(s, P, env);
+      unsigned st[kMaxGroup];
+#pragma unroll
+      for (int m = 0; m < kMaxGroup; ++m) { st[m] = 0; if (act[m]) integrate_bodies(s, P, m, &st[m]); }
+      __syncwarp();
+      const int2 cc = finish_pairs<TM>(s, P, env0, L, nph, true, true, P.materialise != 0);
+      __syncwarp();
       const bool eos = flags & SolveEndOfStep;
-      if (eos && (P.collapsed || (flags & SolveRest))) {
-        const float ek = collapse_latch(s, P, env, P.collapsed != nullptr);
-        if ((flags & SolveRest) && lane == 0) {
-          const int steps = meta[MetaSteps] + 1;
-          meta[MetaSteps] = steps;
-          if (P.rest_steps) P.rest_steps[env] = steps;
-          if (ek < rest_ek) meta[MetaResting] = 1;
+      int n_active = 0, n_steps = 0;
+#pragma unroll
+      for (int m = 0; m < kMaxGroup; ++m) {
+        if (!act[m]) continue;
+        const int env = env0 + m;
+        int* meta = reinterpret_cast<int*>(scr0 + (size_t)m * P.scratch_words + L.meta);
+        if (lane == 0) P.n_cache[env] = meta[MetaNcoll];
+        store_bodies(s, P, env, m);
+        if (eos && (P.collapsed || (flags & SolveRest))) {
+          const float ek = collapse_latch(s, P, env, m, P.collapsed != nullptr);
+          if ((flags & SolveRest) && lane == 0) {
+            const int steps = meta[MetaSteps] + 1;
+            meta[MetaSteps] = steps;
+            if (P.rest_steps) P.rest_steps[env] = steps;
+            if (ek < rest_ek) meta[MetaResting] = 1;
+          }
         }
+        if (P.counters) {
+          ++n_steps;
+          for (int b = lane; b < P.B; b += 32) n_active += s.bd[(m * P.S + b) * kBd + 3] != 0.0f ? 1 : 0;
+        }
+        flush_status(P, env, st[m]);
       }
       if (P.counters) {
         const unsigned long long v = warp_sum((unsigned long long)cc.x), vg = warp_sum((unsigned long long)cc.y);
-        int n_active = 0;
-        for (int b = lane; b < P.B; b += 32) n_active += s.bd[b * kBd + 3] != 0.0f ? 1 : 0;
         n_active = __reduce_add_sync(kFull, n_active);
         if (lane == 0) {
           atomicAdd(P.counters + JENGA_CNT_CONTACTS, v);
           atomicAdd(P.counters + JENGA_CNT_CONTACT_ITERS, v * (unsigned long long)iters);
           atomicAdd(P.counters + JENGA_CNT_GROUND_CONTACTS, vg);
           if (eos) {
-            atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, 1ull);
+            atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, (unsigned long long)n_steps);
             atomicAdd(P.counters + JENGA_CNT_BODY_STEPS, (unsigned long long)n_active);
           }
         }
       }
     }
-    flush_status(P, env, st);
     __syncwarp();
   }
   end_solve<TM>(s);

@@ -1,23 +1,28 @@
 // layout.cuh -- parameters, the global hand-off ("scratch") between the four kernels of a substep, and the shared
 // memory arenas of the batched Jenga step (sm_100a).
 //
-// A substep (S1..S7 of include/jenga.h) is FOUR kernels, all with ONE WARP PER ENV (every synchronisation inside an
-// env is a __syncwarp()):
-//   k_detect   S1 predict, S2 broadphase, S3 SAT (which candidates collide, on which axis), S4 canonical colouring.
-//   k_manifold S3 contact manifolds of the colliding pairs.
-//   k_slot     S4 contact setup (effective masses, warm-start lookup).  Small footprints (8-11 KB of shared memory per
-//              54-body env, <= 128 registers): 16+ warps per SM hide the latencies of this branchy, load-heavy half, and
-//              each kernel's hot code fits the instruction cache.  Output per env, in the caller-owned scratch
-//              buffer: pair headers and the 48 solver constants of every colliding pair at its colour-packed POSITION,
-//              and the list of colour chunks.
-//   k_solve    S4 warm-start application, S5 PGS sweeps, S6 integrate + Baumgarte, S7 cache, Eq. 18 latch.
-//              CTA = 4 warps = 4 envs, 2 CTAs per SM; the constants live in TENSOR MEMORY (tcgen05.ld/st, lane =
-//              position % 32, block j = position / 32 at columns [48 j, 48 j + 48)), bodies and headers in shared
-//              memory.
-// Positions.  The colliding pairs of a colour are cut into chunks of consecutive lanes of ONE 32-position block
-// (never across a block boundary), bin-packed into the blocks: a chunk visit of the solver is then three warp-wide
-// TMEM loads, the contact arithmetic of the chunk's lanes, and one warp-wide store of the impulses (lanes outside the
-// chunk write back what they loaded).
+// A substep (S1..S7 of include/jenga.h) is FOUR kernels:
+//   k_detect   S1 predict, S2 broadphase, S3 SAT (which candidates collide, on which axis), S4 canonical colouring and
+//              the visit plan of the env GROUP.  One warp per env.
+//   k_manifold S3 contact manifolds of the colliding pairs.  One warp per env.
+//   k_slot     S4 contact setup (effective masses, warm-start lookup).  One warp per env.  Small footprints (8-11 KB of
+//              shared memory per 54-body env, <= 128 registers): 16+ warps per SM hide the latencies of this branchy,
+//              load-heavy half, and each kernel's hot code fits the instruction cache.  Output, in the caller-owned
+//              scratch buffer: the 56 solver words (36 constants, 12 impulses, 8 header words) of every colliding pair at
+//              its POSITION in the group's blocks, and the list of chunks.
+//   k_solve    S4 warm-start application, S5 PGS sweeps, S6 integrate + Baumgarte, S7 cache, Eq. 18 latch.  ONE WARP PER
+//              GROUP of G envs (G = 1 or 2); the blocks live in TENSOR MEMORY (tcgen05.ld/st, lane = position % 32,
+//              block j = position / 32 at columns [56 j, 56 j + 56)) or are used in place in the scratch; body records
+//              in shared memory.
+// Groups and positions.  Envs are independent, and a warp that sweeps the colours of ONE env runs half empty (a 54-block
+// tower has 7 colours of 1..27 pairs).  So G consecutive envs form a group that one solver warp owns, and the solver's
+// unit of work, the VISIT, takes pairs of the current colour of EVERY member: up to 32 pairs that share no dynamic body
+// (same colour within an env; different envs share nothing).  A member's colours stay in ascending order and each of
+// its pairs is visited once per sweep after every pair of a lower colour: the Gauss-Seidel result of every env is the
+// canonical one bit for bit (pairs of one colour commute).  A visit is a chunk of consecutive lanes of ONE 32-position
+// block (bin-packed; a visit that fits no block whole is cut over the emptiest blocks): a chunk visit of the solver is
+// four warp-wide TMEM loads, the contact arithmetic of the chunk's lanes, and one warp-wide store of the impulses
+// (lanes outside the chunk write back what they loaded).
 #pragma once
 #include "../../include/jenga.h"
 #include "collide.cuh"
@@ -28,9 +33,10 @@ constexpr int kStateRows = 13, kPropRows = 8, kFextRows = 6;
 constexpr int kMaxColours = 64;
 constexpr int kBd = 20;        // solver body record (floats): x y z im | vx vy vz - | wx wy wz - | Ixx Ixy Ixz Iyy | Iyz Izz - -
 constexpr int kCb = 28;        // collision body record of k_slot: x y z im | a0.xyz h0 | a1.xyz h1 | a2.xyz h2 | Ixx Ixy Ixz Iyy | Iyz Izz - - | pad 4 (k_detect, k_manifold: 20 words, kcollide.cuh)
-constexpr int kHdrF4 = 3;      // float4 per pair header: (ab, meta, rank, 1/|t1 raw|), (n.xyz, Baumgarte corr), (t1.xyz, 0)
-constexpr int kCsF4 = 12;      // float4 of contact constants per pair: 36 read-only words + 12 impulses
-constexpr int kBlkWords = kCsF4 * 4 * 32;   // words of one 32-position constant block in the scratch / shared tier
+constexpr int kCsF4 = 14;      // float4 per pair: 36 read-only words + 12 impulses + 8 header words (kcollide.cuh PairC)
+constexpr int kTmCols = 4 * kCsF4;          // tensor-memory columns of one block
+constexpr int kBlkWords = kCsF4 * 4 * 32;   // words of one 32-position block in the scratch / shared tier
+constexpr int kMaxGroup = 2;                // envs per solver warp
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kScratchHead = 64;             // global words in front of the per-env scratch: [0] = k_solve's work counter
 constexpr int kMagic = 0x4a454e47;          // "JENG": scratch meta stamp of a valid colouring
@@ -48,7 +54,8 @@ struct Params {
   float restitution, aabb_margin, beta, slop;
   CollideParams cp;
   float match_tol;
-  int warm_start, gyroscopic, max_pairs, max_contacts, pc, materialise, tmb, nblk;
+  int warm_start, gyroscopic, max_pairs, max_contacts, pc, materialise, tmb, nblk;   // nblk: blocks of a GROUP
+  int G;                    // envs per group (one k_solve warp): env = G * group + member
   float* state; const float* props; const float* mu; const float* f_ext;
   int* pairs; int* n_pairs; float* contacts; int* n_contacts; float* lambda;
   int* cache_key; float* cache_lam; float* cache_pt; int* n_cache;
@@ -62,19 +69,20 @@ struct Params {
 __host__ __device__ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
 // ---------------------------------------------------------------- scratch (global, per env), word offsets
-// 32-position blocks: enough for pc pairs (capacity beyond the pairs actually colliding is the packing's slack).
-__host__ __device__ inline int n_blocks(int pc) { return (pc + 31) / 32; }
-__host__ __device__ inline int ph_max(int nblk) { return kMaxColours + 2 * nblk + 8; }
+// Every env has the same region; the blocks (cs), the chunk list (ph) and MetaNph / MetaNblk are GROUP data and live in
+// the region of the group's first env (those of the other members stay untouched).
+// 32-position blocks of a group: enough for G pc pairs (capacity beyond the pairs actually colliding is the packing's slack).
+__host__ __device__ inline int n_blocks(int pc, int G) { return G * ((pc + 31) / 32); }
+__host__ __device__ inline int ph_max(int nblk, int G) { return G * kMaxColours + 2 * nblk + 8; }
 
 struct Scratch {
-  int hdr, cs, ph, meta, pos, cpair, coff, cab, man, total;
+  int cs, ph, meta, pos, cpair, coff, cab, man, total;
 };
-__host__ __device__ inline Scratch scratch_layout(int pc) {
-  const int pcA = round_up(pc, 8), nblk = n_blocks(pc), npos = 32 * nblk;
+__host__ __device__ inline Scratch scratch_layout(int pc, int G) {
+  const int pcA = round_up(pc, 8), nblk = n_blocks(pc, G);
   Scratch L; int p = 0;
-  L.hdr = p;   p += 4 * kHdrF4 * npos;
   L.cs = p;    p += kBlkWords * nblk;
-  L.ph = p;    p += round_up(ph_max(nblk), 4);
+  L.ph = p;    p += round_up(ph_max(nblk, G), 4);
   L.meta = p;  p += MetaWords;
   L.pos = p;   p += pcA / 2;
   L.cpair = p; p += pcA / 2;

@@ -238,7 +238,7 @@ def test_narrowphase_box_soup(orc, J):
 
 
 # ----------------------------------------------------------------------------- S4+S5 PGS
-@pytest.mark.parametrize("tier", ["auto", "smem", "tmem256", "tmem512"])
+@pytest.mark.parametrize("tier", ["auto", "smem", "tmem256", "tmem512", "auto+2", "tmem128+2"])
 @pytest.mark.parametrize("name,cfg,E,steps,warm", [("cfg1", 1, 1, 30, True), ("cfg2", 2, 6, 70, True), ("cfg2cold", 2, 3, 40, False),
                                                    ("cfg3", 3, 4, 300, True), ("cfg4", 4, 2, 30, True), ("cfg6", 6, 6, 25, True)])
 def test_pgs_matches_oracle(orc, J, name, cfg, E, steps, warm, tier):
@@ -252,8 +252,12 @@ def test_pgs_matches_oracle(orc, J, name, cfg, E, steps, warm, tier):
     dyn = (wl.props[:, 7, :] != 0) & (wl.props[:, 0, :] != 0)
     state[:, 9, :] += np.float32(h * wl.params.gravity[2]) * dyn           # pre-add h*g (S1)
     if tier != "auto" and name not in ("cfg2", "cfg4"):
-        pytest.skip("the explicit tiers are exercised on cfg2 and cfg4")
-    world = J.World(wl.params, state, wl.props, wl.mu, tier=tier)
+        pytest.skip("the explicit tiers and the two-env groups are exercised on cfg2 and cfg4")
+    tier, _, group = tier.partition("+")
+    try:
+        world = J.World(wl.params, state, wl.props, wl.mu, tier=tier, group=int(group or 0))
+    except J.JengaError:
+        pytest.skip("this tier does not fit the config's shared-memory footprint")
     P = orc.make_params(wl.params); bod = orc.unpack_tiles(state, wl.props, wl.params.n_bodies)
     if warm:
         # the cache the GPU sees is the oracle's, rounded to fp32; the oracle re-reads the rounded values
@@ -333,29 +337,32 @@ def test_single_step_pose(orc, J, name, cfg, E, steps):
 
 @pytest.mark.parametrize("cfg,E", [(2, 9), (4, 5), (3, 6)])
 def test_solver_tiers_bit_identical(J, cfg, E):
-    """Every tier of the solve kernel (shared memory only; tensor memory with 12 / 8 / 4 envs in flight per SM, the
-    blocks beyond the TMEM share served from the scratch) runs the same arithmetic in the same order: 8 steps from the
-    seeded initial state give bit-identical states, caches and counters.  cfg4 (304 pair slots = 10 blocks) puts most
-    blocks of the 12- and 8-env tiers outside tensor memory."""
+    """Every tier of the solve kernel (shared memory only; tensor memory with 16 / 12 / 8 / 4 groups in flight per SM, the
+    blocks beyond the TMEM share served from the scratch) and both group sizes (one env per solver warp; two envs whose
+    colours share the warp's visits -- E is odd, so the last group has one member) run every env's arithmetic in the same
+    order: 8 steps from the seeded initial state give bit-identical states, caches and counters.  cfg4 (304 pair slots =
+    10 blocks per env) puts most blocks of the wider tiers outside tensor memory."""
     import torch
     wl = W.make_config(cfg, n_envs=E)
     ref = None
     used = []
-    for tier in ("smem", "tmem128", "tmem160", "tmem256", "tmem512", "auto"):
-        try:
-            w = J.World(wl.params, wl.state, wl.props, wl.mu, tier=tier)
-        except J.JengaError:
-            continue                                               # a tier that does not fit this config
-        used.append((tier, w.launch_info()["threads"]))
-        w.step(5); w.step(3); torch.cuda.synchronize()
-        got = (w.state.clone(), w.cache_lam.clone(), w.cache_key.clone(), w.counters.clone(), w.status.clone())
-        if ref is None:
-            ref = got
-        else:
-            assert all(torch.equal(a, b) for a, b in zip(ref, got)), f"tier {tier} differs"
-        w.destroy()
+    for group in (1, 2):
+        for tier in ("smem", "tmem128", "tmem160", "tmem256", "tmem512", "auto"):
+            try:
+                w = J.World(wl.params, wl.state, wl.props, wl.mu, tier=tier, group=group)
+            except J.JengaError:
+                continue                                               # a tier that does not fit this config
+            assert w.launch_info()["env_group"] == group
+            used.append((group, tier, w.launch_info()["threads"]))
+            w.step(5); w.step(3); torch.cuda.synchronize()
+            got = (w.state.clone(), w.cache_lam.clone(), w.cache_key.clone(), w.counters.clone(), w.status.clone())
+            if ref is None:
+                ref = got
+            else:
+                assert all(torch.equal(a, b) for a, b in zip(ref, got)), f"group {group} tier {tier} differs"
+            w.destroy()
     print(f"\n[tiers] cfg{cfg}: {used}")
-    assert len(used) >= 4 and int(ref[4].max().item()) == 0
+    assert len([u for u in used if u[0] == 1]) >= 4 and len([u for u in used if u[0] == 2]) >= 3 and int(ref[4].max().item()) == 0
 
 
 def test_worlds_of_different_sizes_in_any_order(J):
@@ -826,6 +833,7 @@ def test_until_rest_matches_oracle(orc, J):
     world.cache_lam[:] = torch.as_tensor(cache.lam.astype(np.float32)).to(world.dev)
     world.cache_pt[:] = torch.as_tensor(cache.pt.astype(np.float32)).to(world.dev)
     world.n_cache[:] = torch.as_tensor(cache.n_keys).to(world.dev)
+    cache0 = (cache.key_pair.copy(), cache.key_meta.copy(), cache.lam.astype(np.float32), cache.pt.astype(np.float32), cache.n_keys.copy())
     world.simulate_until_rest(400, 1e-7); torch.cuda.synchronize()
     bod = orc.unpack_tiles(state, wl.props, wl.params.n_bodies)
     ref, ek_ref, _ = orc.rollout_until_rest(P, bod, mu64, 400, 1e-7, cache=cache)
@@ -839,6 +847,13 @@ def test_until_rest_matches_oracle(orc, J):
     # the step at which E_k crosses 1e-7 J depends on rounding for towers that are still rocking: measured on B200
     # 71 % equal, 92 % within 5 steps
     assert np.mean(d == 0) >= 0.5 and np.mean(d <= 5) >= 0.8
+    # two envs per solver warp: an env at rest leaves its group's visits; the other member's result is unchanged bit for bit
+    w2 = J.World(wl.params, state, wl.props, wl.mu, collapse_length=W.BLOCK_L, group=2, tier="tmem128")
+    w2.cache_key[:] = torch.as_tensor(np.stack([cache0[0], cache0[1]], axis=-1)).to(w2.dev)
+    w2.cache_lam[:] = torch.as_tensor(cache0[2]).to(w2.dev); w2.cache_pt[:] = torch.as_tensor(cache0[3]).to(w2.dev)
+    w2.n_cache[:] = torch.as_tensor(cache0[4]).to(w2.dev)
+    w2.simulate_until_rest(400, 1e-7); torch.cuda.synchronize()
+    assert torch.equal(w2.rest_steps, world.rest_steps) and torch.equal(w2.state, world.state)
 
 
 def test_step_host_equals_step(J):
