@@ -1,6 +1,7 @@
 // jenga.cu -- C-ABI of the batched Jenga step (include/jenga.h) over the four kernels of a substep.  sm_100a only.
 //
-//   k_detect  (kcollide.cuh)  S1 predict, S2 broadphase, S3 SAT, S4 colouring + visit plan      -> scratch
+//   k_detect  (kcollide.cuh)  S1 predict, S2 broadphase, S3 SAT                                -> scratch
+//   k_plan    (kcollide.cuh)  S4 colouring + visit plan of the groups whose pair lists changed  -> scratch
 //   k_manifold (kcollide.cuh) S3 contact manifolds                                              -> scratch
 //   k_slot    (kcollide.cuh)  S4 effective masses + warm-start lookup                           -> scratch
 //   k_solve   (ksolve.cuh)    S4 warm start, S5 PGS sweeps, S6 integrate, S7 cache, Eq. 18 latch
@@ -48,7 +49,7 @@ struct jenga_world {
   int n_sm;
   size_t smem_solve;       // dynamic shared memory per CTA of k_solve
   size_t smem_collide;     // ... of k_detect
-  size_t smem_manifold, smem_slot;   // ... of k_manifold, k_slot
+  size_t smem_manifold, smem_slot, smem_plan;   // ... of k_manifold, k_slot, k_plan
   bool profiling;          // jenga_profile_enable: events around every launch of the step
   std::vector<cudaEvent_t> ev;   // e0 k_detect e1 k_manifold e2 k_slot e3 k_solve e4, per substep
 };
@@ -59,7 +60,10 @@ static size_t collide_env_bytes(const jenga_world_desc* d, int G, int arena = -1
   const size_t a = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaDetect, G);
   const size_t b = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaManifold, G);
   const size_t c = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaSlot, G);
-  return arena == jenga::ArenaDetect ? a : (arena == jenga::ArenaManifold ? b : (arena == jenga::ArenaSlot ? c : (a > b ? a : b)));
+  const size_t p = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaPlan, G);
+  if (arena == jenga::ArenaPlan) return p;
+  const size_t ab = a > b ? a : b, cp = c > p ? c : p;
+  return arena == jenga::ArenaDetect ? a : (arena == jenga::ArenaManifold ? b : (arena == jenga::ArenaSlot ? c : (ab > cp ? ab : cp)));
 }
 /* shared memory of one k_solve warp (= one group of G envs) */
 static size_t solve_group_bytes(const jenga_world_desc* d, int tmb, int G) {
@@ -180,7 +184,7 @@ static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; 
 
 /* cudaFuncAttributeMaxDynamicSharedMemorySize is per kernel and process-wide: it is only ever raised (running maximum
  * per device), immediately before the launch that needs it, so worlds of different sizes can be used in any order.   */
-enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnSolveTm, KnSolveSm, KnCount };
+enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnPlan, KnSolveTm, KnSolveSm, KnCount };
 static std::mutex g_attr_mutex;
 static size_t g_attr_max[16][KnCount];
 
@@ -194,6 +198,7 @@ static const void* kernel_ptr(int kn) {
     case KnManifoldNarrow: return (const void*)jenga::k_manifold<jenga::ModeNarrow>;
     case KnSlot: return (const void*)jenga::k_slot<jenga::ModeStep>;
     case KnSlotGiven: return (const void*)jenga::k_slot<jenga::ModeGiven>;
+    case KnPlan: return (const void*)jenga::k_plan;
     case KnSolveTm: return (const void*)jenga::k_solve<true>;
     default: return (const void*)jenga::k_solve<false>;
   }
@@ -242,6 +247,7 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   w->smem_collide = w->wpc_collide * collide_env_bytes(d, G, jenga::ArenaDetect);
   w->smem_manifold = w->wpc_collide * collide_env_bytes(d, G, jenga::ArenaManifold);
   w->smem_slot = w->wpc_collide * collide_env_bytes(d, G, jenga::ArenaSlot);
+  w->smem_plan = w->wpc_collide * collide_env_bytes(d, G, jenga::ArenaPlan);
   if (w->smem_solve > (size_t)prop.sharedMemPerBlockOptin || w->smem_collide > (size_t)prop.sharedMemPerBlockOptin) { delete w; return JENGA_E_ARG; }
   Params& P = w->P;
   P.E = d->n_envs; P.B = d->n_bodies; P.S = d->body_stride;
@@ -320,7 +326,7 @@ static void mark(jenga_world* w, cudaStream_t st) {
   w->ev.push_back(e);
 }
 
-/* k_detect, then (except for jenga_broadphase) k_manifold and k_slot, for every env */
+/* k_detect, then (except for jenga_broadphase) k_plan, k_manifold and k_slot, for every env */
 static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_t st) {
   cudaError_t e = ensure_smem(w->desc.device, KnCollide + mode, w->smem_collide);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_detect)");
@@ -333,6 +339,11 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
   }
   int rc = launched("k_detect");
   if (rc != JENGA_OK || mode == jenga::ModeBroad) return rc;
+  e = ensure_smem(w->desc.device, KnPlan, w->smem_plan);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_plan)");
+  jenga::k_plan<<<grid, thr, w->smem_plan, st>>>(w->P, mode == jenga::ModeStep ? 1 : 0);
+  rc = launched("k_plan");
+  if (rc != JENGA_OK) return rc;
   mark(w, st);
   if (mode != jenga::ModeGiven) {                           /* manifolds (jenga_pgs_solve: the caller's contacts instead) */
     const int kn = mode == jenga::ModeStep ? KnManifold : KnManifoldNarrow;

@@ -1,8 +1,9 @@
-// kcollide.cuh -- the three collision kernels of a substep, one env per warp.  k_detect: S1 predict, S2 broadphase, S3 SAT
-// (which candidates collide), S4 canonical colouring + the group's visit plan.  k_manifold: S3 contact manifolds.  k_slot: S4
-// contact setup (effective masses, warm-start lookup).  Their products go to the scratch buffer (layout.cuh) for the
-// next kernel.  They are separate kernels because each one's hot code then fits the 32 KB instruction cache (as one
-// kernel: 70 KB, and `no_instruction` was the top stall with 16 warps per SM at different places in it).
+// kcollide.cuh -- the collision kernels of a substep, one env per warp.  k_detect: S1 predict, S2 broadphase, S3 SAT
+// (which candidates collide).  k_plan: S4 canonical colouring + the group's visit plan (only for groups whose pair lists
+// changed).  k_manifold: S3 contact manifolds.  k_slot: S4 contact setup (effective masses, warm-start lookup).  Their
+// products go to the scratch buffer (layout.cuh) for the next kernel.  They are separate kernels because each one's hot
+// code then fits the 32 KB instruction cache (as one kernel: 70 KB, and `no_instruction` was the top stall with 16 warps
+// per SM at different places in it).
 #pragma once
 #include "layout.cuh"
 
@@ -13,10 +14,10 @@ struct CSm {
   SP<float> cb;                 // [S][cbw] collision body records: x y z im | a0 h0 | a1 h1 | a2 h2 | then q (k_detect) or Iw^-1 (k_slot)
   int cbw;                      // words per record: 20 (k_detect, k_manifold) or kCb = 28 (k_slot); a multiple of 4, odd in float4
   SP<float4> ext;               // [S]      world AABB half extents e'_x e'_y e'_z, flags (1 active | 2 dynamic)
-  SP<unsigned> hitw;            // [ceil(S/32)][32] broadphase hit words of the current block of 32 rows; ALIASES used
-  SP<unsigned long long> used;  // [S]      colour masks per body
+  SP<unsigned> hitw;            // [ceil(S/32)][32] broadphase hit words of the current block of 32 rows
+  SP<unsigned long long> used;  // [S]      colour masks per body (k_plan)
   SP<unsigned> cab;             // [pcA]    (a+1) | A dynamic << 11 | axis << 12 | b << 16 | B dynamic << 27
-  SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending; ALIASES chm
+  SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending
   SP<float> poly;               // [8][3][32] clip polygon of every lane (component-major: lane l <-> bank l)
   SP<unsigned short> cpair;     // [pcA]    colliding pair indices, ascending
   SP<unsigned short> cprev;     // [pcA]    pair indices of the warm-start cache (previous substep), ascending
@@ -32,23 +33,24 @@ struct CSm {
 };
 enum { MiNph = 0, MiNcol = 1, MiNblk = 2, MiSame = 3 };
 
-enum { ArenaDetect = 0, ArenaManifold = 1, ArenaSlot = 2 };
+enum { ArenaDetect = 0, ArenaManifold = 1, ArenaSlot = 2, ArenaPlan = 3 };
 
-// k_detect: records, extents, masks / hit words, candidate list, colliding list, colouring products.
-// k_manifold: records, colliding list (copied from the scratch), per-lane clip polygons.  k_slot: records, colliding
-// list, cache keys.
-__host__ __device__ inline int cb_words(int arena) { return arena == ArenaSlot ? kCb : 20; }
+// k_detect: records, extents, hit words, candidate list, colliding list.  k_plan: colliding list, masks, colouring and
+// plan products (no body records).  k_manifold: records, colliding list (copied from the scratch), per-lane clip
+// polygons.  k_slot: records, colliding list, cache keys.
+__host__ __device__ inline int cb_words(int arena) { return arena == ArenaSlot ? kCb : (arena == ArenaPlan ? 0 : 20); }
 
 __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc, int arena, int G) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc, G);
   size_t w = (size_t)cb_words(arena) * S + pcA + pcA / 2;  // cb, cab, cpair
   if (arena != ArenaManifold) w += 2 * (size_t)(pcA / 2);  // pos, wrank
   if (arena == ArenaDetect) {
-    const int uh = 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
+    const int uh = 32 * ((S + 31) / 32);
+    w += 4 * S + uh + mpA / 2 + 8;                         // ext, hitw, cand, misc
+  } else if (arena == ArenaPlan) {
     const int phw = round_up(ph_max(nblk, G), 4);
-    w += 4 * S + uh + pcA / 4;                             // ext, used / hitw, colour
-    w += mpA / 2 > kMaxGroup * phw ? mpA / 2 : kMaxGroup * phw;   // cand; chm aliases it (the candidates are dead by then)
-    w += phw;                                              // ph
+    w += 2 * S + pcA / 4;                                  // used, colour
+    w += (1 + kMaxGroup) * phw;                            // ph, chm
     w += 2 * kMaxColours + round_up(nblk, 4) + 8;          // ccount, cfirst, fill, misc
   } else if (arena == ArenaManifold) {
     w += 768;                                              // poly
@@ -72,10 +74,14 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int 
   s.ccount.off = s.cfirst.off = s.fill.off = s.misc.off = s.cprev.off = s.poly.off = 0;
   if (arena == ArenaDetect) {
     s.ext.off = p;    p += 4 * S;
-    s.hitw.off = p;   s.used.off = p;   p += 2 * S > 32 * ((S + 31) / 32) ? 2 * S : 32 * ((S + 31) / 32);
-    s.cand.off = p;   s.chm.off = p;    p += mpA / 2 > kMaxGroup * phw ? mpA / 2 : kMaxGroup * phw;
+    s.hitw.off = p;   p += 32 * ((S + 31) / 32);
+    s.cand.off = p;   p += mpA / 2;
+    s.misc.off = p;
+  } else if (arena == ArenaPlan) {
+    s.used.off = p;   p += 2 * S;
     s.colour.off = p; p += pcA / 4;
     s.ph.off = p;     p += phw;
+    s.chm.off = p;    p += kMaxGroup * phw;
     s.ccount.off = p; p += kMaxColours;
     s.cfirst.off = p; p += kMaxColours;
     s.fill.off = p;   p += round_up(nblk, 4);
@@ -628,54 +634,83 @@ __device__ inline void plan_group(const CSm& s, const CSm& s0, const CSm& s1, in
   if (lane == 0) { s.misc[MiNph] = nph; s.misc[MiNblk] = top; }
 }
 
-// Does the colliding-pair list of this env equal the one its scratch was coloured for?  (the steady state of a standing
-// tower: colouring and plan are functions of the lists alone and are kept).  Also hands the bodies + SAT axis of every pair
-// to k_manifold / k_slot.
-__device__ inline bool colouring_is_current(const CSm& s, float* scr, const Scratch& L, int n_coll) {
+// k_detect's hand-over to k_plan: does the colliding-pair list of this env equal the one its scratch was coloured for?
+// (the steady state of a standing tower: colouring and plan are functions of the lists alone and are kept).  The bodies
+// + SAT axis of every pair go to the scratch for k_manifold / k_slot; a changed list replaces the stored one and
+// invalidates the stamp until k_plan has re-planned the group.  meta[MetaSame] tells k_plan.
+__device__ inline void publish_pairs(const CSm& s, float* scr, const Scratch& L, int n_coll) {
   const int lane = lane_id();
-  const int* meta = reinterpret_cast<const int*>(scr + L.meta);
-  const unsigned short* gpair = reinterpret_cast<const unsigned short*>(scr + L.cpair);
+  int* meta = reinterpret_cast<int*>(scr + L.meta);
+  unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
   unsigned* gcab = reinterpret_cast<unsigned*>(scr + L.cab);
   for (int r = lane; r < n_coll; r += 32) gcab[r] = s.cab[r];
   bool same = meta[MetaMagic] == kMagic && meta[MetaNcoll] == n_coll;
   if (same)
     for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
-  return __all_sync(kFull, same);
+  same = __all_sync(kFull, same);
+  if (!same) for (int r = lane; r < n_coll; r += 32) gpair[r] = s.cpair[r];
+  if (lane == 0) {
+    meta[MetaSame] = same ? 1 : 0;
+    if (!same) { meta[MetaMagic] = 0; meta[MetaNcoll] = n_coll; }
+  }
 }
 
 __device__ __forceinline__ void pair_barrier(int id) {
   if (id == 1) asm volatile("bar.sync 1, 64;" ::: "memory"); else asm volatile("bar.sync 2, 64;" ::: "memory");
 }
 
-// S4 colouring + plan of the group this env belongs to.  `present`: the env exists (env < E); an env that exists but is
-// skipped (at rest) takes part with n_coll = 0.  With G = 2 the two warps of a group are neighbours in the CTA and meet at
-// two named barriers (ids 1 + warp / 2); both always take this path, whatever their env does.
-__device__ inline void colour_pairs(const CSm& s, const Params& P, int env, bool present, int n_coll, unsigned* status) {
-  const int lane = lane_id(), warp = threadIdx.x >> 5, G = P.G;
-  const Scratch L = scratch_layout(P.pc, G);
+// k_plan: S4 colouring + visit plan of the group this env belongs to, when the pair list of one of its members changed.
+// One warp per env; with G = 2 the two warps of a group are neighbours in the CTA, exchange their colour counts through
+// shared memory and meet at a named barrier (id 1 + warp / 2); both take the same path (the decision depends on the
+// group's MetaSame flags only).  A member whose own list did not change reloads its colouring from the scratch.
+__global__ void __launch_bounds__(128) k_plan(const Params P, const int count_colours) {
+  const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id(), G = P.G;
+  const int env = blockIdx.x * wpc + warp;
   const int me = G == 2 ? (env & 1) : 0;
+  if (env - me >= P.E) return;                                   // no env of this warp's group exists (both warps leave)
+  const bool present = env < P.E, sib_present = G == 2 && (env ^ 1) < P.E;
+  const Scratch L = scratch_layout(P.pc, G);
   float* scr = P.scratch + (size_t)env * P.scratch_words;                    // touched only if present
   float* scr0 = P.scratch + (size_t)(env - me) * P.scratch_words;            // the group's first env always exists
   int* meta = reinterpret_cast<int*>(scr + L.meta);
   int* meta0 = reinterpret_cast<int*>(scr0 + L.meta);
-  const int arena = (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaDetect, G);
-  const CSm sib = carve_collide(P.S, P.max_pairs, P.pc, (warp ^ 1) * arena, ArenaDetect, G);
-  bool same = present ? colouring_is_current(s, scr, L, n_coll) : true;
-  if (G == 2) {
-    if (lane == 0) s.misc[MiSame] = same ? 1 : 0;
-    pair_barrier(1 + (warp >> 1));
-    same = same && sib.misc[MiSame] != 0;
-  }
-  if (same) {
-    if (lane == 0) { s.misc[MiNph] = meta0[MetaNph]; s.misc[MiNblk] = meta0[MetaNblk]; s.misc[MiNcol] = present ? meta[MetaNcol] : 0; }
-    __syncwarp();
+  const bool same_me = present ? meta[MetaSame] != 0 : true;
+  const bool same_sib = sib_present ? reinterpret_cast<const int*>(P.scratch + (size_t)(env ^ 1) * P.scratch_words + L.meta)[MetaSame] != 0 : true;
+  if (same_me && same_sib) {
+    if (present && count_colours && P.counters && lane == 0) {
+      const int ncol = meta[MetaNcol];
+      atomicAdd(P.counters + JENGA_CNT_COLOURS, (unsigned long long)ncol);
+      atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
+    }
     return;
   }
-  colour_walk(s, P, present ? n_coll : 0, status);
+  const int arena = (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaPlan, G);
+  const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * arena, ArenaPlan, G);
+  const CSm sib = carve_collide(P.S, P.max_pairs, P.pc, (warp ^ 1) * arena, ArenaPlan, G);
+  unsigned st = 0;
+  const int n_coll = present ? meta[MetaNcoll] : 0;
+  unsigned char* gcol = reinterpret_cast<unsigned char*>(scr + L.col);
+  unsigned short* gwrk = reinterpret_cast<unsigned short*>(scr + L.wrk);
+  int* gcnt = reinterpret_cast<int*>(scr + L.ccnt);
+  if (!same_me) {                                              // colour the new list, keep the colouring
+    const unsigned* gcab = reinterpret_cast<const unsigned*>(scr + L.cab);
+    for (int r = lane; r < n_coll; r += 32) s.cab[r] = gcab[r];
+    __syncwarp();
+    colour_walk(s, P, n_coll, &st);
+    for (int r = lane; r < n_coll; r += 32) { gcol[r] = s.colour[r]; gwrk[r] = s.wrank[r]; }
+    for (int c = lane; c < kMaxColours; c += 32) gcnt[c] = s.ccount[c];
+  } else {                                                     // the list is the one coloured last time
+    if (present) {
+      for (int r = lane; r < n_coll; r += 32) { s.colour[r] = gcol[r]; s.wrank[r] = gwrk[r]; }
+      for (int c = lane; c < kMaxColours; c += 32) s.ccount[c] = gcnt[c];
+    }
+    if (lane == 0) s.misc[MiNcol] = present ? meta[MetaNcol] : 0;
+    __syncwarp();
+  }
   if (G == 2) pair_barrier(1 + (warp >> 1));
   const int nblk = P.nblk, phw = round_up(ph_max(nblk, G), 4);
-  const int nm = G == 2 && (env | 1) < P.E ? 2 : 1;              // members that exist
-  plan_group(s, me ? sib : s, me ? s : sib, nm, me, nblk, phw, status);
+  const int nm = sib_present || me == 1 ? 2 : 1;                 // members that exist
+  plan_group(s, me ? sib : s, me ? s : sib, nm, me, nblk, phw, &st);
   __syncwarp();
   const int nph = s.misc[MiNph];
   // Blocks are renumbered by the number of chunks they hold (= solver visits per sweep), most first: the first blocks
@@ -694,7 +729,6 @@ __device__ inline void colour_pairs(const CSm& s, const Params& P, int env, bool
   }
   if (present) {
     unsigned short* gpos = reinterpret_cast<unsigned short*>(scr + L.pos);
-    unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
     for (int r = lane; r < n_coll; r += 32) {
       const int c = s.colour[r], w = s.wrank[r];
       int k = 0;
@@ -706,17 +740,23 @@ __device__ inline void colour_pairs(const CSm& s, const Params& P, int env, bool
           break;
         }
       }
-      s.pos[r] = (unsigned short)k;
-      gpos[r] = (unsigned short)k; gpair[r] = s.cpair[r];
+      gpos[r] = (unsigned short)k;
     }
-    if (lane == 0) { meta[MetaMagic] = kMagic; meta[MetaNcoll] = n_coll; meta[MetaNcol] = s.misc[MiNcol]; }
+    if (lane == 0) {
+      const int ncol = s.misc[MiNcol];
+      meta[MetaMagic] = kMagic; meta[MetaNcol] = ncol;
+      if (count_colours && P.counters) {
+        atomicAdd(P.counters + JENGA_CNT_COLOURS, (unsigned long long)ncol);
+        atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
+      }
+    }
+    flush_status(P, env, st);
   }
   if (me == 0) {                                              // group data: in the region of the group's first env
     int* gph = reinterpret_cast<int*>(scr0 + L.ph);
     for (int j = lane; j < nph; j += 32) gph[j] = s.ph[j];
     if (lane == 0) { meta0[MetaNph] = nph; meta0[MetaNblk] = s.misc[MiNblk]; }
   }
-  __syncwarp();
 }
 
 // ---------------------------------------------------------------- pair slots (solver constants at a position)
@@ -1027,13 +1067,12 @@ __global__ void __launch_bounds__(128, 5) k_detect(const Params P, const int hon
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
   const int env = blockIdx.x * wpc + warp;
   if (blockIdx.x == 0 && threadIdx.x == 0) *P.work_counter = 0;      // k_solve of this substep starts its group queue at 0
-  if (env - (P.G == 2 ? (env & 1) : 0) >= P.E) return;              // no env of this warp's group exists (the whole group leaves)
-  const bool present = env < P.E;
+  if (env >= P.E) return;
   const Scratch L = scratch_layout(P.pc, P.G);
   float* scr = P.scratch + (size_t)env * P.scratch_words;
   int* meta = reinterpret_cast<int*>(scr + L.meta);
-  // an env at rest (jenga_simulate_until_rest) is skipped, but its warp still takes part in the group's plan (with no pairs)
-  const bool live = present && !(honour_rest && meta[MetaResting]);
+  // an env at rest (jenga_simulate_until_rest) is skipped: it takes part in its group's plan with an empty pair list
+  const bool live = !(honour_rest && meta[MetaResting]);
   if (mode == ModeBroad && !live) return;
   const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaDetect, P.G), ArenaDetect, P.G);
   unsigned st = 0;
@@ -1057,19 +1096,16 @@ __global__ void __launch_bounds__(128, 5) k_detect(const Params P, const int hon
     }
   }
   if (mode != ModeBroad) {
-    colour_pairs(s, P, env, present, n_coll, &st);
+    publish_pairs(s, scr, L, n_coll);                          // an env at rest: an empty list
     if (!live) return;
     if (P.counters && mode == ModeStep && lane == 0) {
-      const int ncol = s.misc[MiNcol];
       atomicAdd(P.counters + JENGA_CNT_CANDIDATES, (unsigned long long)n_cand);
       atomicAdd(P.counters + JENGA_CNT_COLLIDING, (unsigned long long)n_coll);
-      atomicAdd(P.counters + JENGA_CNT_COLOURS, (unsigned long long)ncol);
       atomicMax(P.counters + JENGA_CNT_MAX_CANDIDATES, (unsigned long long)n_cand);
       atomicMax(P.counters + JENGA_CNT_MAX_COLLIDING, (unsigned long long)n_coll);
-      atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
     }
   }
-  if (live) flush_status(P, env, st);
+  flush_status(P, env, st);
 }
 
 template <int mode>

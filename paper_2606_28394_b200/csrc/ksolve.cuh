@@ -287,7 +287,7 @@ template <bool TM>
 __device__ inline void warm_start_pass(const SSm& s, int nph) {
   const int lane = lane_id();
   for (int j = 0; j < nph; ++j) {
-    const int d = s.ph[j], jb = d >> 16;
+    const int d = s.ph[j];
     PairC c; block_load<TM>(s, d, c);
     if (chunk_lane(d, lane)) {
       const int ab = hdr_ab(c), a = ab & 0xffff, b = ab >> 16;
@@ -412,7 +412,7 @@ __device__ inline int2 finish_pairs(const SSm& s, const Params& P, int env0, con
   const int lane = lane_id();
   int nc = 0, ng = 0;
   for (int j = 0; j < nph; ++j) {
-    const int d = s.ph[j], jb = d >> 16;
+    const int d = s.ph[j];
     const bool active = chunk_lane(d, lane);
     PairC c; block_load<TM>(s, d, c);
     if (baumgarte) {

@@ -1,9 +1,9 @@
 // layout.cuh -- parameters, the global hand-off ("scratch") between the four kernels of a substep, and the shared
 // memory arenas of the batched Jenga step (sm_100a).
 //
-// A substep (S1..S7 of include/jenga.h) is FOUR kernels:
-//   k_detect   S1 predict, S2 broadphase, S3 SAT (which candidates collide, on which axis), S4 canonical colouring and
-//              the visit plan of the env GROUP.  One warp per env.
+// A substep (S1..S7 of include/jenga.h) is FIVE kernels:
+//   k_detect   S1 predict, S2 broadphase, S3 SAT (which candidates collide, on which axis).  One warp per env.
+//   k_plan     S4 canonical colouring and the visit plan of the env GROUP, for the groups whose pair lists changed.
 //   k_manifold S3 contact manifolds of the colliding pairs.  One warp per env.
 //   k_slot     S4 contact setup (effective masses, warm-start lookup).  One warp per env.  Small footprints (8-11 KB of
 //              shared memory per 54-body env, <= 128 registers): 16+ warps per SM hide the latencies of this branchy,
@@ -41,7 +41,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr int kScratchHead = 64;             // global words in front of the per-env scratch: [0] = k_solve's work counter
 constexpr int kMagic = 0x4a454e47;          // "JENG": scratch meta stamp of a valid colouring
 
-enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaWords = 16 };
+enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaSame, MetaWords = 16 };
 
 // modes of the collision kernels
 enum { ModeStep = 0, ModeBroad = 1, ModeNarrow = 2, ModeGiven = 3 };
@@ -76,7 +76,7 @@ __host__ __device__ inline int n_blocks(int pc, int G) { return G * ((pc + 31) /
 __host__ __device__ inline int ph_max(int nblk, int G) { return G * kMaxColours + 2 * nblk + 8; }
 
 struct Scratch {
-  int cs, ph, meta, pos, cpair, coff, cab, man, total;
+  int cs, ph, meta, pos, cpair, coff, cab, col, wrk, ccnt, man, total;
 };
 __host__ __device__ inline Scratch scratch_layout(int pc, int G) {
   const int pcA = round_up(pc, 8), nblk = n_blocks(pc, G);
@@ -88,6 +88,9 @@ __host__ __device__ inline Scratch scratch_layout(int pc, int G) {
   L.cpair = p; p += pcA / 2;
   L.coff = p;  p += pcA / 2;
   L.cab = p;   p += pcA;
+  L.col = p;   p += pcA / 4;            // colour of pair r, rank inside its colour, pairs per colour: the colouring of
+  L.wrk = p;   p += pcA / 2;            // the env's current pair list (k_plan re-plans a group without re-colouring a
+  L.ccnt = p;  p += kMaxColours;        // member whose list did not change)
   L.man = p;   p += 20 * pcA;           // manifold of pair r: (n.xyz, np | axis << 8), 4 x (p.xyz, depth)
   L.total = round_up(p, 32);
   return L;

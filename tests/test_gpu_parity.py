@@ -848,7 +848,7 @@ def test_until_rest_matches_oracle(orc, J):
     # 71 % equal, 92 % within 5 steps
     assert np.mean(d == 0) >= 0.5 and np.mean(d <= 5) >= 0.8
     # two envs per solver warp: an env at rest leaves its group's visits; the other member's result is unchanged bit for bit
-    w2 = J.World(wl.params, state, wl.props, wl.mu, collapse_length=W.BLOCK_L, group=2, tier="tmem128")
+    w2 = J.World(wl.params, state, wl.props, wl.mu, collapse_length=W.BLOCK_L, group=2, tier="tmem160")
     w2.cache_key[:] = torch.as_tensor(np.stack([cache0[0], cache0[1]], axis=-1)).to(w2.dev)
     w2.cache_lam[:] = torch.as_tensor(cache0[2]).to(w2.dev); w2.cache_pt[:] = torch.as_tensor(cache0[3]).to(w2.dev)
     w2.n_cache[:] = torch.as_tensor(cache0[4]).to(w2.dev)
