@@ -1063,7 +1063,7 @@ __device__ inline int load_colliding(const CSm& s, const float* scr, const Scrat
 // ModeGiven (first half of jenga_pgs_solve: the caller's contact list instead of the narrowphase).  honour_rest: envs whose
 // scratch says "at rest" are skipped (jenga_simulate_until_rest).
 template <int mode>
-__global__ void __launch_bounds__(128, 5) k_detect(const Params P, const int honour_rest) {
+__global__ void __launch_bounds__(128, 6) k_detect(const Params P, const int honour_rest) {
   const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
   const int env = blockIdx.x * wpc + warp;
   if (blockIdx.x == 0 && threadIdx.x == 0) *P.work_counter = 0;      // k_solve of this substep starts its group queue at 0
