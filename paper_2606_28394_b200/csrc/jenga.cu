@@ -65,9 +65,9 @@ static size_t collide_env_bytes(const jenga_world_desc* d, int G, int arena = -1
   const size_t ab = a > b ? a : b, cp = c > p ? c : p;
   return arena == jenga::ArenaDetect ? a : (arena == jenga::ArenaManifold ? b : (arena == jenga::ArenaSlot ? c : (ab > cp ? ab : cp)));
 }
-/* shared memory of one k_solve warp (= one group of G envs) */
-static size_t solve_group_bytes(const jenga_world_desc* d, int tmb, int G) {
-  return 4 * jenga::solve_smem_words(d->body_stride, d->max_contacts / 4, tmb, G);
+/* shared memory of one k_solve warp (= one group of G envs), without / with smb blocks of spare shared memory */
+static size_t solve_group_bytes(const jenga_world_desc* d, int tmb, int G, int smb = 0) {
+  return 4 * jenga::solve_smem_words(d->body_stride, d->max_contacts / 4, tmb, smb, G);
 }
 
 static bool desc_ok(const jenga_world_desc* d) {
@@ -86,7 +86,6 @@ static bool desc_ok(const jenga_world_desc* d) {
 /* Envs per k_solve warp.  Two envs share a warp when the batch still fills the machine that way (every SM gets 16 groups),
  * when two collision warps fit one CTA (the two warps of a group plan their visits together in k_detect), and when the
  * widest tensor-memory tier holds the doubled records; desc.env_group forces it (-1 if it does not fit).           */
-static size_t solve_group_bytes(const jenga_world_desc* d, int tmb, int G);
 static bool group_fits(const jenga_world_desc* d, int G) {
   if (G == 1) return true;
   return 2 * collide_env_bytes(d, G) <= kSmemMax && solve_group_bytes(d, 0, G) + 1024 <= kSmemMax;
@@ -106,9 +105,10 @@ static bool tier_fits(const jenga_world_desc* d, int tmb, int G) {
 }
 /* The blocks of a group beyond its tensor-memory share are re-read from the scratch in every sweep: they must stay in L2
  * while the group is in flight, or every visit goes to HBM (measured at cfg5 with two envs per warp: 16 groups per SM =
- * 166 MB of blocks in flight, k_solve 6.9 ms; 12 groups per SM = 112 MB, 4.8 ms).  Capacity-based bound, 126 MB of L2. */
+ * 133 MB of blocks in flight, k_solve 6.9 ms; 12 groups per SM = 87 MB, 4.8 ms).  Capacity-based estimate, 126 MB of L2. */
 static bool tier_in_l2(const jenga_world_desc* d, int tmb, int G) {
-  const long long nblk = jenga::n_blocks(d->max_contacts / 4, G), out = nblk > tmb ? nblk - tmb : 0;
+  /* blocks a group uses: about 4/5 of its capacity (cfg5: 10 of 12 with two envs per group; cfg4: 8 of 10) */
+  const long long nblk = (4 * jenga::n_blocks(d->max_contacts / 4, G) + 4) / 5, out = nblk > tmb ? nblk - tmb : 0;
   return (long long)kSmNominal * 4 * tier_groups(tmb) * out * jenga::kBlkWords * 4 <= 120ll << 20;
 }
 static int pick_tmb(const jenga_world_desc* d, int G) {
@@ -135,9 +135,18 @@ static int pick_tmb(const jenga_world_desc* d, int G) {
   }
 }
 
+/* Blocks per group that a tensor-memory tier also keeps in shared memory: what the CTA's 227 KB leave per warp, at most
+ * the blocks beyond the TMEM share. */
+static int pick_smb(const jenga_world_desc* d, int tmb, int G) {
+  if (!tmb) return 0;
+  const long long warps = 4 * tier_groups(tmb), spare = (long long)kSmemMax - 1024 - 16 - warps * (long long)solve_group_bytes(d, tmb, G);
+  const long long nblk = jenga::n_blocks(d->max_contacts / 4, G), smb = spare / (warps * jenga::kBlkWords * 4);
+  return (int)(smb < 0 ? 0 : (smb > nblk - tmb ? (nblk > tmb ? nblk - tmb : 0) : smb));
+}
+
 /* dynamic shared memory of a k_solve CTA */
 static size_t solve_cta_bytes(const jenga_world_desc* d, int tmb, int G) {
-  return tmb ? 4 * tier_groups(tmb) * solve_group_bytes(d, tmb, G) : solve_group_bytes(d, 0, G);
+  return tmb ? 4 * tier_groups(tmb) * solve_group_bytes(d, tmb, G, pick_smb(d, tmb, G)) : solve_group_bytes(d, 0, G);
 }
 
 extern "C" size_t jenga_smem_bytes(const jenga_world_desc* d) {
@@ -162,7 +171,7 @@ extern "C" size_t jenga_scratch_bytes(const jenga_world_desc* d) {
   if (!desc_ok(d)) return 0;
   const int G = pick_group(d);
   if (G < 0) return 0;
-  return ((size_t)d->n_envs * jenga::scratch_layout(d->max_contacts / 4, G).total + jenga::kScratchHead) * sizeof(float);
+  return ((size_t)d->n_envs * jenga::scratch_layout(d->max_contacts / 4, G).total + jenga::kScratchHead + jenga::round_up(d->n_envs, 32)) * sizeof(float);
 }
 
 extern "C" const char* jenga_strerror(int code) {
@@ -257,7 +266,7 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.cp.edge_bias_rel = d->edge_bias_rel; P.cp.edge_bias_abs = d->edge_bias_abs; P.cp.par_eps = d->par_eps; P.cp.tie_eps = d->tie_eps;
   P.match_tol = d->match_tol; P.warm_start = d->warm_start; P.gyroscopic = d->gyroscopic;
   P.max_pairs = d->max_pairs; P.max_contacts = d->max_contacts; P.pc = d->max_contacts / 4; P.materialise = d->materialise;
-  P.tmb = tmb; P.G = G; P.nblk = jenga::n_blocks(P.pc, G);
+  P.tmb = tmb; P.G = G; P.nblk = jenga::n_blocks(P.pc, G); P.smb = pick_smb(d, tmb, G);
   P.state = b->state; P.props = b->props; P.mu = b->mu; P.f_ext = b->f_ext;
   P.pairs = b->pairs; P.n_pairs = b->n_pairs; P.contacts = b->contacts; P.n_contacts = b->n_contacts; P.lambda = b->lambda;
   P.cache_key = b->cache_key; P.cache_lam = b->cache_lam; P.cache_pt = b->cache_pt; P.n_cache = b->n_cache;
@@ -268,7 +277,8 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   P.rest_steps = b->rest_steps;
   P.collapse_dx = d->collapse_fd * d->collapse_length; P.collapse_ek = d->collapse_ek; P.collapse_theta = d->collapse_theta;
   P.work_counter = (int*)b->scratch;
-  P.scratch = (float*)b->scratch + jenga::kScratchHead; P.scratch_words = jenga::scratch_layout(P.pc, G).total;
+  P.same_flag = (int*)b->scratch + jenga::kScratchHead;
+  P.scratch = (float*)b->scratch + jenga::kScratchHead + jenga::round_up(d->n_envs, 32); P.scratch_words = jenga::scratch_layout(P.pc, G).total;
   *out = w;
   return JENGA_OK;
 }
@@ -341,7 +351,7 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
   if (rc != JENGA_OK || mode == jenga::ModeBroad) return rc;
   e = ensure_smem(w->desc.device, KnPlan, w->smem_plan);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_plan)");
-  jenga::k_plan<<<grid, thr, w->smem_plan, st>>>(w->P, mode == jenga::ModeStep ? 1 : 0);
+  jenga::k_plan<<<grid, thr, w->smem_plan, st>>>(w->P);
   rc = launched("k_plan");
   if (rc != JENGA_OK) return rc;
   mark(w, st);

@@ -637,8 +637,9 @@ __device__ inline void plan_group(const CSm& s, const CSm& s0, const CSm& s1, in
 // k_detect's hand-over to k_plan: does the colliding-pair list of this env equal the one its scratch was coloured for?
 // (the steady state of a standing tower: colouring and plan are functions of the lists alone and are kept).  The bodies
 // + SAT axis of every pair go to the scratch for k_manifold / k_slot; a changed list replaces the stored one and
-// invalidates the stamp until k_plan has re-planned the group.  meta[MetaSame] tells k_plan.
-__device__ inline void publish_pairs(const CSm& s, float* scr, const Scratch& L, int n_coll) {
+// invalidates the stamp until k_plan has re-planned the group.  same_flag[env] (a dense array: k_plan's warps read it
+// coalesced and most of them leave at once) tells k_plan.
+__device__ inline void publish_pairs(const CSm& s, const Params& P, int env, float* scr, const Scratch& L, int n_coll) {
   const int lane = lane_id();
   int* meta = reinterpret_cast<int*>(scr + L.meta);
   unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
@@ -650,7 +651,7 @@ __device__ inline void publish_pairs(const CSm& s, float* scr, const Scratch& L,
   same = __all_sync(kFull, same);
   if (!same) for (int r = lane; r < n_coll; r += 32) gpair[r] = s.cpair[r];
   if (lane == 0) {
-    meta[MetaSame] = same ? 1 : 0;
+    P.same_flag[env] = same ? 1 : 0;
     if (!same) { meta[MetaMagic] = 0; meta[MetaNcoll] = n_coll; }
   }
 }
@@ -662,28 +663,20 @@ __device__ __forceinline__ void pair_barrier(int id) {
 // k_plan: S4 colouring + visit plan of the group this env belongs to, when the pair list of one of its members changed.
 // One warp per env; with G = 2 the two warps of a group are neighbours in the CTA, exchange their colour counts through
 // shared memory and meet at a named barrier (id 1 + warp / 2); both take the same path (the decision depends on the
-// group's MetaSame flags only).  A member whose own list did not change reloads its colouring from the scratch.
-__global__ void __launch_bounds__(128) k_plan(const Params P, const int count_colours) {
-  const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id(), G = P.G;
-  const int env = blockIdx.x * wpc + warp;
+// group's same_flag entries only).  A member whose own list did not change reloads its colouring from the scratch.
+__device__ inline void plan_env(const Params& P, const int env) {
+  const int warp = threadIdx.x >> 5, lane = lane_id(), G = P.G;
   const int me = G == 2 ? (env & 1) : 0;
   if (env - me >= P.E) return;                                   // no env of this warp's group exists (both warps leave)
   const bool present = env < P.E, sib_present = G == 2 && (env ^ 1) < P.E;
+  const bool same_me = present ? P.same_flag[env] != 0 : true;
+  const bool same_sib = sib_present ? P.same_flag[env ^ 1] != 0 : true;
+  if (same_me && same_sib) return;
   const Scratch L = scratch_layout(P.pc, G);
   float* scr = P.scratch + (size_t)env * P.scratch_words;                    // touched only if present
   float* scr0 = P.scratch + (size_t)(env - me) * P.scratch_words;            // the group's first env always exists
   int* meta = reinterpret_cast<int*>(scr + L.meta);
   int* meta0 = reinterpret_cast<int*>(scr0 + L.meta);
-  const bool same_me = present ? meta[MetaSame] != 0 : true;
-  const bool same_sib = sib_present ? reinterpret_cast<const int*>(P.scratch + (size_t)(env ^ 1) * P.scratch_words + L.meta)[MetaSame] != 0 : true;
-  if (same_me && same_sib) {
-    if (present && count_colours && P.counters && lane == 0) {
-      const int ncol = meta[MetaNcol];
-      atomicAdd(P.counters + JENGA_CNT_COLOURS, (unsigned long long)ncol);
-      atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
-    }
-    return;
-  }
   const int arena = (int)collide_smem_words(P.S, P.max_pairs, P.pc, ArenaPlan, G);
   const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * arena, ArenaPlan, G);
   const CSm sib = carve_collide(P.S, P.max_pairs, P.pc, (warp ^ 1) * arena, ArenaPlan, G);
@@ -711,6 +704,7 @@ __global__ void __launch_bounds__(128) k_plan(const Params P, const int count_co
   const int nblk = P.nblk, phw = round_up(ph_max(nblk, G), 4);
   const int nm = sib_present || me == 1 ? 2 : 1;                 // members that exist
   plan_group(s, me ? sib : s, me ? s : sib, nm, me, nblk, phw, &st);
+  if (G == 2) pair_barrier(1 + (warp >> 1));                    // the sibling has read this warp's colour counts (k_plan's loop reuses them)
   __syncwarp();
   const int nph = s.misc[MiNph];
   // Blocks are renumbered by the number of chunks they hold (= solver visits per sweep), most first: the first blocks
@@ -742,20 +736,24 @@ __global__ void __launch_bounds__(128) k_plan(const Params P, const int count_co
       }
       gpos[r] = (unsigned short)k;
     }
-    if (lane == 0) {
-      const int ncol = s.misc[MiNcol];
-      meta[MetaMagic] = kMagic; meta[MetaNcol] = ncol;
-      if (count_colours && P.counters) {
-        atomicAdd(P.counters + JENGA_CNT_COLOURS, (unsigned long long)ncol);
-        atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)ncol);
-      }
-    }
+    if (lane == 0) { meta[MetaMagic] = kMagic; meta[MetaNcol] = s.misc[MiNcol]; }
     flush_status(P, env, st);
   }
   if (me == 0) {                                              // group data: in the region of the group's first env
     int* gph = reinterpret_cast<int*>(scr0 + L.ph);
     for (int j = lane; j < nph; j += 32) gph[j] = s.ph[j];
     if (lane == 0) { meta0[MetaNph] = nph; meta0[MetaNblk] = s.misc[MiNblk]; }
+  }
+}
+
+// One CTA per wpc envs like the other collision kernels (a persistent grid of 8 or 16 CTAs per SM measured slower: 1.13 -
+// 1.16 vs 1.09 ms for detection + plan at cfg5); the loop only matters for grids the host caps.  The two warps of a group
+// stay side by side (wpc is even when G = 2) and make the same decisions, so the pair barriers match.
+__global__ void __launch_bounds__(128) k_plan(const Params P) {
+  const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
+  for (int base = blockIdx.x * wpc; base < P.E; base += gridDim.x * wpc) {
+    plan_env(P, base + warp);
+    __syncwarp();
   }
 }
 
@@ -1096,7 +1094,7 @@ __global__ void __launch_bounds__(128, 6) k_detect(const Params P, const int hon
     }
   }
   if (mode != ModeBroad) {
-    publish_pairs(s, scr, L, n_coll);                          // an env at rest: an empty list
+    publish_pairs(s, P, env, scr, L, n_coll);                  // an env at rest: an empty list
     if (!live) return;
     if (P.counters && mode == ModeStep && lane == 0) {
       atomicAdd(P.counters + JENGA_CNT_CANDIDATES, (unsigned long long)n_cand);

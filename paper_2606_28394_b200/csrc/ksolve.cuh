@@ -7,8 +7,9 @@
 //               of tensor memory.  Warp w works in TMEM lanes 32 (w % 4) .. + 31 (its quadrant) and columns
 //               [56 tmb (w / 4), + 56 tmb): the 56 words of the positions of the group's first `tmb` 32-position blocks
 //               (tmb = 2, 3, 4, 9 for Q = 4, 3, 2, 1; tcgen05.ld/st.32x32b: lane = position % 32, block j at column
-//               offset 56 j).  Blocks >= tmb stay where k_slot wrote them, in the scratch (L2-resident while the group is
-//               in flight): their visits load and store global memory, one visit ahead of use.
+//               offset 56 j).  The next `smb` blocks are copied to the warp's share of the CTA's spare shared memory.
+//               Blocks >= tmb + smb stay where k_slot wrote them, in the scratch (L2-resident while the group is in
+//               flight): their visits load and store global memory, one visit ahead of use.
 //   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers; small batches).
 #pragma once
 #include "kcollide.cuh"
@@ -18,27 +19,27 @@ namespace jenga {
 struct SSm {
   SP<float> bd;                 // [G S + 1][kBd] solver body records of the group (member m's body b: record m S + b);
                                 // the last record is the ground: all zeros, never changes
-  SP<float4> cs;                // TM = false: [nblk][kCsF4][32] every block in shared memory
+  SP<float4> cs;                // [smb][kCsF4][32] blocks tmb .. tmb + smb - 1 (TM = false: tmb = 0, smb = nblk: every block)
   SP<int> ph;                   // [ph_max]
-  int tmb;
+  int tmb, smb;
   unsigned tm;                  // TMEM address of this warp's lanes, first column of its group
   float4* gcs;                  // TM = true: the group's blocks in the scratch (blocks >= tmb are used in place)
 };
 
-// tmb = 0: the all-shared-memory flavour
-__host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb, int G) {
+// tmb = 0: the all-shared-memory flavour (smb is then the group's block capacity)
+__host__ __device__ inline size_t solve_smem_words(int S, int pc, int tmb, int smb, int G) {
   const int nblk = n_blocks(pc, G);
   size_t w = (size_t)kBd * (G * S + 1);
-  w += tmb ? 0 : (size_t)kBlkWords * nblk;
+  w += (size_t)kBlkWords * (tmb ? smb : nblk);
   w += round_up(ph_max(nblk, G), 4);
   return round_up((int)w, 4);
 }
 
-__device__ inline SSm carve_solve(int S, int pc, int tmb, int G, int base) {
+__device__ inline SSm carve_solve(int S, int pc, int tmb, int smb, int G, int base) {
   const int nblk = n_blocks(pc, G);
   SSm s; int p = base;
-  s.tmb = tmb; s.tm = 0; s.gcs = nullptr;
-  s.cs.off = p;  p += tmb ? 0 : kBlkWords * nblk;
+  s.tmb = tmb; s.smb = tmb ? smb : nblk; s.tm = 0; s.gcs = nullptr;
+  s.cs.off = p;  p += kBlkWords * s.smb;
   s.bd.off = p;  p += kBd * (G * S + 1);
   s.ph.off = p;
   return s;
@@ -89,26 +90,24 @@ __device__ __forceinline__ void tm_store_lam(const SSm& s, int j, const float* l
   const unsigned a = s.tm + (unsigned)kTmCols * (unsigned)j + (unsigned)kLam;
   tm_st8(a, lam); tm_st4(a + 8, lam + 8);
 }
-// blocks outside tensor memory, lane l: shared memory (TM = false) or the scratch itself (TM = true, block j >= tmb)
-template <bool TM>
-__device__ __forceinline__ float4* ov_ptr(const SSm& s, int j, int l) { return (TM ? s.gcs : s.cs.ptr()) + j * (kCsF4 * 32) + l; }
+// blocks outside tensor memory (j >= tmb), lane l: the warp's shared-memory copy (j < tmb + smb) or the scratch itself
+__device__ __forceinline__ float4* sm_ptr(const SSm& s, int j, int l) { return s.cs.ptr() + (j - s.tmb) * (kCsF4 * 32) + l; }
+__device__ __forceinline__ float4* gl_ptr(const SSm& s, int j, int l) { return s.gcs + j * (kCsF4 * 32) + l; }
+#define JENGA_ROWS_LOAD(b) _Pragma("unroll") for (int f = 0; f < kCsF4; ++f) { const float4 t = (b)[f * 32]; c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
+#define JENGA_ROWS_STORE(b, f0, f1) _Pragma("unroll") for (int f = (f0); f < (f1); ++f) (b)[f * 32] = make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]);
 template <bool TM>
 __device__ __forceinline__ void sm_load_pair(const SSm& s, int j, int l, PairC& c) {
-  const float4* b = ov_ptr<TM>(s, j, l);
-#pragma unroll
-  for (int f = 0; f < kCsF4; ++f) { const float4 t = b[f * 32]; c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
+  if (!TM || j < s.tmb + s.smb) { const float4* b = sm_ptr(s, j, l); JENGA_ROWS_LOAD(b) }
+  else { const float4* b = gl_ptr(s, j, l); JENGA_ROWS_LOAD(b) }
 }
 template <bool TM>
 __device__ __forceinline__ void sm_store_pair(const SSm& s, int j, int l, const PairC& c) {
-  float4* b = ov_ptr<TM>(s, j, l);
-#pragma unroll
-  for (int f = 0; f < kCsF4; ++f) b[f * 32] = make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]);
+  float4* b = sm_ptr(s, j, l); JENGA_ROWS_STORE(b, 0, kCsF4)
 }
 template <bool TM>
-__device__ __forceinline__ void sm_store_lam(const SSm& s, int j, int l, const float* lam) {
-  float4* b = ov_ptr<TM>(s, j, l);
-#pragma unroll
-  for (int f = 0; f < 3; ++f) b[(kLam / 4 + f) * 32] = make_float4(lam[4 * f], lam[4 * f + 1], lam[4 * f + 2], lam[4 * f + 3]);
+__device__ __forceinline__ void sm_store_lam(const SSm& s, int j, int l, const PairC& c) {
+  if (!TM || j < s.tmb + s.smb) { float4* b = sm_ptr(s, j, l); JENGA_ROWS_STORE(b, kLam / 4, kHdr / 4) }
+  else { float4* b = gl_ptr(s, j, l); JENGA_ROWS_STORE(b, kLam / 4, kHdr / 4) }
 }
 // The lane whose pair lane `lane` loads from a block outside tensor memory: its own inside the chunk d, the chunk's first
 // lane otherwise (a block in the scratch costs L2 bandwidth per sector touched; the duplicate addresses cost nothing and
@@ -128,7 +127,7 @@ __device__ __forceinline__ SSm begin_solve(const Params& P) {
   __shared__ unsigned tm_base_s;
   const int warp = threadIdx.x >> 5;
   const int tmb = TM ? P.tmb : 0;
-  SSm s = carve_solve(P.S, P.pc, tmb, P.G, warp * (int)solve_smem_words(P.S, P.pc, tmb, P.G));
+  SSm s = carve_solve(P.S, P.pc, tmb, P.smb, P.G, warp * (int)solve_smem_words(P.S, P.pc, tmb, P.smb, P.G));
   if (TM) {
     if (warp == 0) {
       asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
@@ -199,7 +198,7 @@ __device__ inline int load_slots(const SSm& s, const float* scr0, const Scratch&
   const int* gph = reinterpret_cast<const int*>(scr0 + L.ph);
   for (int j = lane; j < nph; j += 32) s.ph[j] = gph[j];
   const float4* gcs = reinterpret_cast<const float4*>(scr0 + L.cs);
-  const int ncopy = TM ? min(nblk, s.tmb) : nblk;              // TM: blocks >= tmb are used in place
+  const int ncopy = min(nblk, s.tmb + s.smb);                  // blocks beyond are used in place
   for (int j = 0; j < ncopy; ++j) {
     PairC c;
 #pragma unroll
@@ -207,7 +206,7 @@ __device__ inline int load_slots(const SSm& s, const float* scr0, const Scratch&
       const float4 t = gcs[(j * kCsF4 + f) * 32 + lane];
       c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w;
     }
-    if (TM) tm_store_block(s, j, c);
+    if (TM && j < s.tmb) tm_store_block(s, j, c);
     else sm_store_pair<TM>(s, j, lane, c);
   }
   if (TM) tm_wait_st();
@@ -327,7 +326,7 @@ __device__ inline void pgs_sweeps(const SSm& s, int nph, int iters, float mu0, f
       const Frame F = hdr_frame(c);
       solve_pair<false>(c, A, B, F, (hdr_meta(c) & kMetaMember) ? mu1 : mu0);
       store_body_vel(s, a, A); store_body_vel(s, b, B);
-      if (!in_tm) sm_store_lam<TM>(s, jb, lane, c.v + kLam);
+      if (!in_tm) sm_store_lam<TM>(s, jb, lane, c);
     }
     if (in_tm) { tm_store_lam(s, jb, c.v + kLam); tm_wait_st(); }
     __syncwarp();
@@ -544,7 +543,7 @@ __global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, cons
       const int2 cc = finish_pairs<TM>(s, P, env0, L, nph, true, true, P.materialise != 0);
       __syncwarp();
       const bool eos = flags & SolveEndOfStep;
-      int n_active = 0, n_steps = 0;
+      int n_active = 0, n_steps = 0, n_colours = 0, max_colours = 0;
 #pragma unroll
       for (int m = 0; m < kMaxGroup; ++m) {
         if (!act[m]) continue;
@@ -563,6 +562,8 @@ __global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, cons
         }
         if (P.counters) {
           ++n_steps;
+          const int ncol = meta[MetaNcol];
+          n_colours += ncol; max_colours = max(max_colours, ncol);
           for (int b = lane; b < P.B; b += 32) n_active += s.bd[(m * P.S + b) * kBd + 3] != 0.0f ? 1 : 0;
         }
         flush_status(P, env, st[m]);
@@ -574,6 +575,8 @@ __global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, cons
           atomicAdd(P.counters + JENGA_CNT_CONTACTS, v);
           atomicAdd(P.counters + JENGA_CNT_CONTACT_ITERS, v * (unsigned long long)iters);
           atomicAdd(P.counters + JENGA_CNT_GROUND_CONTACTS, vg);
+          atomicAdd(P.counters + JENGA_CNT_COLOURS, (unsigned long long)n_colours);
+          atomicMax(P.counters + JENGA_CNT_MAX_COLOURS, (unsigned long long)max_colours);
           if (eos) {
             atomicAdd(P.counters + JENGA_CNT_ENV_STEPS, (unsigned long long)n_steps);
             atomicAdd(P.counters + JENGA_CNT_BODY_STEPS, (unsigned long long)n_active);

@@ -41,7 +41,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr int kScratchHead = 64;             // global words in front of the per-env scratch: [0] = k_solve's work counter
 constexpr int kMagic = 0x4a454e47;          // "JENG": scratch meta stamp of a valid colouring
 
-enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaSame, MetaWords = 16 };
+enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaWords = 16 };
 
 // modes of the collision kernels
 enum { ModeStep = 0, ModeBroad = 1, ModeNarrow = 2, ModeGiven = 3 };
@@ -56,13 +56,15 @@ struct Params {
   float match_tol;
   int warm_start, gyroscopic, max_pairs, max_contacts, pc, materialise, tmb, nblk;   // nblk: blocks of a GROUP
   int G;                    // envs per group (one k_solve warp): env = G * group + member
+  int smb;                  // blocks per group that the tensor-memory tiers of k_solve keep in spare shared memory
   float* state; const float* props; const float* mu; const float* f_ext;
   int* pairs; int* n_pairs; float* contacts; int* n_contacts; float* lambda;
   int* cache_key; float* cache_lam; float* cache_pt; int* n_cache;
   unsigned* status; unsigned long long* counters;
   const float* ref_pose; int* collapsed; float* collapse_stats; int* rest_steps;
   float collapse_dx, collapse_ek, collapse_theta;           // f_d * l, eps_k, theta_th
-  int* work_counter;                                        // next env of the running k_solve (reset by every k_detect)
+  int* work_counter;                                        // next group of the running k_solve (reset by every k_detect)
+  int* same_flag;                                           // [E] k_detect -> k_plan: 1 = the env's pair list is the one its colouring was made for
   float* scratch; long long scratch_words;                  // per env (the first kScratchHead words of the buffer are global)
 };
 
