@@ -51,11 +51,18 @@ def test_descriptor_validation_and_launch_shape(L):
     smem = L.jenga_smem_bytes(C.byref(d))
     assert 0 < smem <= 227 * 1024
     # auto tier by batch size: a batch that does not fill 148 SMs runs fewer envs per SM (header, solver_tier)
+    # and a batch that still fills every SM with two envs per solver warp (>= 2 x 16 x 148 envs) gets groups of two, in the
+    # tier whose blocks in flight fit the L2 (12 warps per SM)
     shape = {}
-    for E in (2, 592, 593, 1184, 1185, 1776, 1777, 65536):
+    for E in (2, 592, 593, 1184, 1185, 1776, 1777, 4735, 4736, 65536):
         de = binding.make_desc(wp); de.n_envs = E
-        shape[E] = L.jenga_block_threads(C.byref(de))
-    assert shape == {2: 32, 592: 32, 593: 256, 1184: 256, 1185: 384, 1776: 384, 1777: 512, 65536: 512}
+        shape[E] = (L.jenga_block_threads(C.byref(de)), L.jenga_env_group(C.byref(de)))
+    assert shape == {2: (32, 1), 592: (32, 1), 593: (256, 1), 1184: (256, 1), 1185: (384, 1), 1776: (384, 1), 1777: (512, 1),
+                     4735: (512, 1), 4736: (384, 2), 65536: (384, 2)}
+    forced = binding.make_desc(wp, group=2); forced.n_envs = 9
+    assert L.jenga_env_group(C.byref(forced)) == 2 and L.jenga_scratch_bytes(C.byref(forced)) > L.jenga_scratch_bytes(C.byref(binding.make_desc(wp)))
+    bad = binding.make_desc(wp); bad.env_group = 3
+    assert L.jenga_env_group(C.byref(bad)) == 0 and L.jenga_scratch_bytes(C.byref(bad)) == 0
     bad = binding.make_desc(wp); bad.body_stride = wp.n_bodies + 1          # not a multiple of 4
     assert L.jenga_smem_bytes(C.byref(bad)) == 0 and L.jenga_block_threads(C.byref(bad)) == 0
     bad = binding.make_desc(wp); bad.struct_size = 4
