@@ -297,11 +297,13 @@ def test_pgs_matches_oracle(orc, J, name, cfg, E, steps, warm, tier):
 @pytest.mark.parametrize("name,cfg,E,steps", [("cfg1", 1, 1, 20), ("cfg2", 2, 6, 60), ("cfg3", 3, 4, 250), ("cfg4", 4, 2, 10), ("cfg6", 6, 6, 20),
                                               ("cfg6push", 6, 6, 70)])
 def test_single_step_pose(orc, J, name, cfg, E, steps):
-    """One fused jenga_step from a common fp32 state and warm-start cache vs one oracle step."""
+    """One fused jenga_step from a common fp32 state and warm-start cache vs one oracle step.  The 54-block configs run
+    the headline launch shape (two envs per solver warp, tensor-memory tier), the others what auto gives them."""
     import torch
     wl = W.make_config(cfg, n_envs=E)
     state, cache = oracle_mid_state(orc, wl, steps)
-    world = J.World(wl.params, state, wl.props, wl.mu, materialise=True)
+    shape = dict(tier="tmem160", group=2) if name in ("cfg2", "cfg3", "cfg6push") else {}
+    world = J.World(wl.params, state, wl.props, wl.mu, materialise=True, **shape)
     cache.lam[:] = cache.lam.astype(np.float32); cache.pt[:] = cache.pt.astype(np.float32)
     world.cache_key[:, :, :] = torch.as_tensor(np.stack([cache.key_pair, cache.key_meta], axis=-1)).to(world.dev)
     world.cache_lam[:] = torch.as_tensor(cache.lam.astype(np.float32)).to(world.dev)
