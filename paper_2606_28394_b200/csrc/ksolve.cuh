@@ -93,12 +93,28 @@ __device__ __forceinline__ void tm_store_lam(const SSm& s, int j, const float* l
 // blocks outside tensor memory (j >= tmb), lane l: the warp's shared-memory copy (j < tmb + smb) or the scratch itself
 __device__ __forceinline__ float4* sm_ptr(const SSm& s, int j, int l) { return s.cs.ptr() + (j - s.tmb) * (kCsF4 * 32) + l; }
 __device__ __forceinline__ float4* gl_ptr(const SSm& s, int j, int l) { return s.gcs + j * (kCsF4 * 32) + l; }
+// L2 eviction priorities: the rows of the in-place blocks are re-read in every sweep (keep: evict_last); what a group
+// reads or writes once (tiles, blocks on their way into tensor / shared memory, the cache) should not push them out.
+__device__ __forceinline__ unsigned long long l2_policy_keep() { unsigned long long p; asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p; }
+__device__ __forceinline__ unsigned long long l2_policy_once() { unsigned long long p; asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p; }
+__device__ __forceinline__ float4 ldg_hint(const float4* a, unsigned long long pol) {
+  float4 t;
+  asm volatile("ld.global.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;" : "=f"(t.x), "=f"(t.y), "=f"(t.z), "=f"(t.w) : "l"(a), "l"(pol) : "memory");
+  return t;
+}
+__device__ __forceinline__ void stg_hint(float4* a, float4 t, unsigned long long pol) {
+  asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" :: "l"(a), "f"(t.x), "f"(t.y), "f"(t.z), "f"(t.w), "l"(pol) : "memory");
+}
 #define JENGA_ROWS_LOAD(b) _Pragma("unroll") for (int f = 0; f < kCsF4; ++f) { const float4 t = (b)[f * 32]; c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
 #define JENGA_ROWS_STORE(b, f0, f1) _Pragma("unroll") for (int f = (f0); f < (f1); ++f) (b)[f * 32] = make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]);
 template <bool TM>
 __device__ __forceinline__ void sm_load_pair(const SSm& s, int j, int l, PairC& c) {
   if (!TM || j < s.tmb + s.smb) { const float4* b = sm_ptr(s, j, l); JENGA_ROWS_LOAD(b) }
-  else { const float4* b = gl_ptr(s, j, l); JENGA_ROWS_LOAD(b) }
+  else {
+    const float4* b = gl_ptr(s, j, l); const unsigned long long pol = l2_policy_keep();
+#pragma unroll
+    for (int f = 0; f < kCsF4; ++f) { const float4 t = ldg_hint(b + f * 32, pol); c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
+  }
 }
 template <bool TM>
 __device__ __forceinline__ void sm_store_pair(const SSm& s, int j, int l, const PairC& c) {
@@ -107,7 +123,11 @@ __device__ __forceinline__ void sm_store_pair(const SSm& s, int j, int l, const 
 template <bool TM>
 __device__ __forceinline__ void sm_store_lam(const SSm& s, int j, int l, const PairC& c) {
   if (!TM || j < s.tmb + s.smb) { float4* b = sm_ptr(s, j, l); JENGA_ROWS_STORE(b, kLam / 4, kHdr / 4) }
-  else { float4* b = gl_ptr(s, j, l); JENGA_ROWS_STORE(b, kLam / 4, kHdr / 4) }
+  else {
+    float4* b = gl_ptr(s, j, l); const unsigned long long pol = l2_policy_keep();
+#pragma unroll
+    for (int f = kLam / 4; f < kHdr / 4; ++f) stg_hint(b + f * 32, make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]), pol);
+  }
 }
 // The lane whose pair lane `lane` loads from a block outside tensor memory: its own inside the chunk d, the chunk's first
 // lane otherwise (a block in the scratch costs L2 bandwidth per sector touched; the duplicate addresses cost nothing and
@@ -199,11 +219,12 @@ __device__ inline int load_slots(const SSm& s, const float* scr0, const Scratch&
   for (int j = lane; j < nph; j += 32) s.ph[j] = gph[j];
   const float4* gcs = reinterpret_cast<const float4*>(scr0 + L.cs);
   const int ncopy = min(nblk, s.tmb + s.smb);                  // blocks beyond are used in place
+  const unsigned long long once = l2_policy_once();
   for (int j = 0; j < ncopy; ++j) {
     PairC c;
 #pragma unroll
     for (int f = 0; f < kCsF4; ++f) {
-      const float4 t = gcs[(j * kCsF4 + f) * 32 + lane];
+      const float4 t = ldg_hint(gcs + (j * kCsF4 + f) * 32 + lane, once);
       c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w;
     }
     if (TM && j < s.tmb) tm_store_block(s, j, c);
@@ -409,6 +430,7 @@ __device__ inline float collapse_latch(const SSm& s, const Params& P, int env, i
 template <bool TM>
 __device__ inline int2 finish_pairs(const SSm& s, const Params& P, int env0, const Scratch& L, int nph, bool baumgarte, bool cache_out, bool lambda_out) {
   const int lane = lane_id();
+  const unsigned long long once = l2_policy_once();
   int nc = 0, ng = 0;
   for (int j = 0; j < nph; ++j) {
     const int d = s.ph[j];
@@ -452,8 +474,8 @@ __device__ inline int2 finish_pairs(const SSm& s, const Params& P, int env0, con
           for (int t = 0; t < 3; ++t) { l[3 * ci + t] = ci < np ? c.v[kLam + 3 * ci + t] : 0.0f; p[3 * ci + t] = c.v[9 * ci + t]; }
 #pragma unroll
         for (int f = 0; f < 3; ++f) {
-          ol[f] = make_float4(l[4 * f], l[4 * f + 1], l[4 * f + 2], l[4 * f + 3]);
-          op[f] = make_float4(p[4 * f], p[4 * f + 1], p[4 * f + 2], p[4 * f + 3]);
+          stg_hint(ol + f, make_float4(l[4 * f], l[4 * f + 1], l[4 * f + 2], l[4 * f + 3]), once);
+          stg_hint(op + f, make_float4(p[4 * f], p[4 * f + 1], p[4 * f + 2], p[4 * f + 3]), once);
         }
       }
       if (lambda_out) {                                          // lambda in contact order (debug / stage output)
