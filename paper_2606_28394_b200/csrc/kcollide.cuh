@@ -534,15 +534,29 @@ __device__ inline int find_colliding(const CSm& s, const Params& P, int n_cand, 
 // Canonical order (north_star (d), DESIGN §2 S4): visit the colliding pairs in ascending pair index;
 // colour = lowest colour not used by an earlier pair sharing a dynamic body.  The walk is sequential by definition
 // (lane 0, one 64-bit mask per body).  Products: s.colour[r], s.wrank[r] = rank of pair r inside its colour,
-// s.ccount[c], s.misc[MiNcol].
-__device__ inline void colour_walk(const CSm& s, const Params& P, int n_coll, unsigned* status) {
+// s.ccount[c], s.misc[MiNcol].  The colour of a pair depends on the pairs before it only: when the first r0 pairs are the
+// ones of the list coloured last time (gcol, gwrk: that colouring), their colours are kept -- masks and counts are rebuilt
+// from them by all lanes -- and the walk starts at r0.
+__device__ inline void colour_walk(const CSm& s, const Params& P, int n_coll, int r0, const unsigned char* gcol, const unsigned short* gwrk, unsigned* status) {
   const int lane = lane_id();
   for (int b = lane; b < P.B; b += 32) s.used[b] = 0ull;
   for (int c = lane; c < kMaxColours; c += 32) s.ccount[c] = 0;
   __syncwarp();
+  int ncol0 = 0;
+  for (int r = lane; r < r0; r += 32) {
+    const unsigned w = s.cab[r];
+    const int a = ab_a(w), b = ab_b(w), c = gcol[r];
+    s.colour[r] = (unsigned char)c; s.wrank[r] = gwrk[r];
+    if (a >= 0) atomicOr(&s.used[a], 1ull << c);
+    atomicOr(&s.used[b], 1ull << c);
+    atomicAdd(&s.ccount[c], 1);
+    ncol0 = max(ncol0, c + 1);
+  }
+  ncol0 = __reduce_max_sync(kFull, ncol0);
+  __syncwarp();
   if (lane == 0) {
-    int ncol = 0; unsigned st = 0;
-    for (int r = 0; r < n_coll; ++r) {
+    int ncol = ncol0; unsigned st = 0;
+    for (int r = r0; r < n_coll; ++r) {
       const unsigned w = s.cab[r];
       const int a = ab_a(w), b = ab_b(w);
       unsigned long long m = 0ull;
@@ -649,7 +663,16 @@ __device__ inline void publish_pairs(const CSm& s, const Params& P, int env, flo
   if (same)
     for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
   same = __all_sync(kFull, same);
-  if (!same) for (int r = lane; r < n_coll; r += 32) gpair[r] = s.cpair[r];
+  if (!same) {
+    // the first position at which the new list differs from the one coloured last time (0 if there is no such colouring)
+    const int n_old = meta[MetaMagic] == kMagic ? meta[MetaNcoll] : 0, n_min = min(n_old, n_coll);
+    int first = n_min;
+    for (int r = lane; r < n_min; r += 32) if (s.cpair[r] != gpair[r]) { first = r; break; }
+    first = __reduce_min_sync(kFull, first);
+    __syncwarp();
+    for (int r = lane; r < n_coll; r += 32) gpair[r] = s.cpair[r];
+    if (lane == 0) meta[MetaFirst] = first;
+  }
   if (lane == 0) {
     P.same_flag[env] = same ? 1 : 0;
     if (!same) { meta[MetaMagic] = 0; meta[MetaNcoll] = n_coll; }
@@ -689,8 +712,9 @@ __device__ inline void plan_env(const Params& P, const int env) {
     const unsigned* gcab = reinterpret_cast<const unsigned*>(scr + L.cab);
     for (int r = lane; r < n_coll; r += 32) s.cab[r] = gcab[r];
     __syncwarp();
-    colour_walk(s, P, n_coll, &st);
-    for (int r = lane; r < n_coll; r += 32) { gcol[r] = s.colour[r]; gwrk[r] = s.wrank[r]; }
+    const int r0 = max(0, min(meta[MetaFirst], n_coll));
+    colour_walk(s, P, n_coll, r0, gcol, gwrk, &st);
+    for (int r = lane + (r0 & ~31); r < n_coll; r += 32) if (r >= r0) { gcol[r] = s.colour[r]; gwrk[r] = s.wrank[r]; }
     for (int c = lane; c < kMaxColours; c += 32) gcnt[c] = s.ccount[c];
   } else {                                                     // the list is the one coloured last time
     if (present) {

@@ -41,7 +41,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr int kScratchHead = 64;             // global words in front of the per-env scratch: [0] = k_solve's work counter
 constexpr int kMagic = 0x4a454e47;          // "JENG": scratch meta stamp of a valid colouring
 
-enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaWords = 16 };
+enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaFirst, MetaWords = 16 };
 
 // modes of the collision kernels
 enum { ModeStep = 0, ModeBroad = 1, ModeNarrow = 2, ModeGiven = 3 };

@@ -396,6 +396,38 @@ def test_counters_and_multi_step_equivalence(J):
     assert ca["body_steps"] == 12 * active
 
 
+def test_kept_colouring_and_plan_equal_a_fresh_one(J):
+    """k_plan keeps what did not change: the whole plan when neither member's pair list changed, a member's colouring when
+    only its sibling's list changed, and the colours of the pairs in front of the first changed one.  A world that has
+    been stepping (towers standing, pushed, collapsing) must therefore continue exactly like a world created from its
+    state and warm-start cache (empty scratch: everything coloured and planned from scratch), bit for bit."""
+    import torch
+    wl = W.make_config(2, n_envs=13)
+    a = J.World(wl.params, wl.state, wl.props, wl.mu, tier="tmem160", group=2)
+    changed = 0
+    for step in range(0, 110):
+        if step == wl.push_start:
+            a.set_f_ext(wl.push_fext)
+        if step == wl.push_end:
+            a.set_f_ext(None)
+        if step % 7 == 3 or wl.push_start <= step < wl.push_start + 3:
+            torch.cuda.synchronize()
+            b = J.World(wl.params, a.state.cpu().numpy(), wl.props, wl.mu, tier="tmem160", group=2)
+            for name in ("cache_key", "cache_lam", "cache_pt", "n_cache"):
+                getattr(b, name).copy_(getattr(a, name))
+            if wl.push_start <= step < wl.push_end:
+                b.set_f_ext(wl.push_fext)
+            flags = a.scratch.view(torch.int32)[64:64 + 13]
+            a.step(1); b.step(1); torch.cuda.synchronize()
+            changed += int((flags == 0).sum().item())
+            assert torch.equal(a.state, b.state) and torch.equal(a.cache_lam, b.cache_lam) and torch.equal(a.cache_key, b.cache_key), f"step {step}"
+            b.destroy()
+        else:
+            a.step(1)
+    assert changed > 10                                   # pair lists did change at the compared steps
+    assert int(a.status.max().item()) == 0
+
+
 # ----------------------------------------------------------------------------- rollouts
 def collapse_flags(state, state0, props, B, length=W.BLOCK_L):
     """Eq. 18 (reading A17) on [E][13][S] tiles, restated in NumPy for the harness:
