@@ -12,6 +12,7 @@
 //               flight): their visits load and store global memory, one visit ahead of use.
 //   TM = false  CTA = 1 warp; every block in shared memory (configs too large for the TMEM tiers; small batches).
 #pragma once
+#include <type_traits>
 #include "kcollide.cuh"
 
 namespace jenga {
@@ -97,14 +98,18 @@ __device__ __forceinline__ float4* gl_ptr(const SSm& s, int j, int l) { return s
 // reads or writes once (tiles, blocks on their way into tensor / shared memory, the cache) should not push them out.
 __device__ __forceinline__ unsigned long long l2_policy_keep() { unsigned long long p; asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p; }
 __device__ __forceinline__ unsigned long long l2_policy_once() { unsigned long long p; asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p; }
+// OFF: a compile-time byte offset (an immediate of the instruction: the rows of a pair are 512 bytes apart)
+template <int OFF>
 __device__ __forceinline__ float4 ldg_hint(const float4* a, unsigned long long pol) {
   float4 t;
-  asm volatile("ld.global.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;" : "=f"(t.x), "=f"(t.y), "=f"(t.z), "=f"(t.w) : "l"(a), "l"(pol) : "memory");
+  asm volatile("ld.global.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4 + %6], %5;" : "=f"(t.x), "=f"(t.y), "=f"(t.z), "=f"(t.w) : "l"(a), "l"(pol), "n"(OFF) : "memory");
   return t;
 }
+template <int OFF>
 __device__ __forceinline__ void stg_hint(float4* a, float4 t, unsigned long long pol) {
-  asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" :: "l"(a), "f"(t.x), "f"(t.y), "f"(t.z), "f"(t.w), "l"(pol) : "memory");
+  asm volatile("st.global.L2::cache_hint.v4.f32 [%0 + %6], {%1, %2, %3, %4}, %5;" :: "l"(a), "f"(t.x), "f"(t.y), "f"(t.z), "f"(t.w), "l"(pol), "n"(OFF) : "memory");
 }
+template <int F, int F1, class Fn> __device__ __forceinline__ void static_rows(Fn fn) { if constexpr (F < F1) { fn(std::integral_constant<int, F>()); static_rows<F + 1, F1>(fn); } }
 #define JENGA_ROWS_LOAD(b) _Pragma("unroll") for (int f = 0; f < kCsF4; ++f) { const float4 t = (b)[f * 32]; c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
 #define JENGA_ROWS_STORE(b, f0, f1) _Pragma("unroll") for (int f = (f0); f < (f1); ++f) (b)[f * 32] = make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]);
 template <bool TM>
@@ -112,8 +117,7 @@ __device__ __forceinline__ void sm_load_pair(const SSm& s, int j, int l, PairC& 
   if (!TM || j < s.tmb + s.smb) { const float4* b = sm_ptr(s, j, l); JENGA_ROWS_LOAD(b) }
   else {
     const float4* b = gl_ptr(s, j, l); const unsigned long long pol = l2_policy_keep();
-#pragma unroll
-    for (int f = 0; f < kCsF4; ++f) { const float4 t = ldg_hint(b + f * 32, pol); c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; }
+    static_rows<0, kCsF4>([&](auto F) { constexpr int f = decltype(F)::value; const float4 t = ldg_hint<f * 512>(b, pol); c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w; });
   }
 }
 template <bool TM>
@@ -125,8 +129,7 @@ __device__ __forceinline__ void sm_store_lam(const SSm& s, int j, int l, const P
   if (!TM || j < s.tmb + s.smb) { float4* b = sm_ptr(s, j, l); JENGA_ROWS_STORE(b, kLam / 4, kHdr / 4) }
   else {
     float4* b = gl_ptr(s, j, l); const unsigned long long pol = l2_policy_keep();
-#pragma unroll
-    for (int f = kLam / 4; f < kHdr / 4; ++f) stg_hint(b + f * 32, make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]), pol);
+    static_rows<kLam / 4, kHdr / 4>([&](auto F) { constexpr int f = decltype(F)::value; stg_hint<f * 512>(b, make_float4(c.v[4 * f], c.v[4 * f + 1], c.v[4 * f + 2], c.v[4 * f + 3]), pol); });
   }
 }
 // The lane whose pair lane `lane` loads from a block outside tensor memory: its own inside the chunk d, the chunk's first
@@ -224,7 +227,7 @@ __device__ inline int load_slots(const SSm& s, const float* scr0, const Scratch&
     PairC c;
 #pragma unroll
     for (int f = 0; f < kCsF4; ++f) {
-      const float4 t = ldg_hint(gcs + (j * kCsF4 + f) * 32 + lane, once);
+      const float4 t = ldg_hint<0>(gcs + (j * kCsF4 + f) * 32 + lane, once);
       c.v[4 * f] = t.x; c.v[4 * f + 1] = t.y; c.v[4 * f + 2] = t.z; c.v[4 * f + 3] = t.w;
     }
     if (TM && j < s.tmb) tm_store_block(s, j, c);
@@ -474,8 +477,8 @@ __device__ inline int2 finish_pairs(const SSm& s, const Params& P, int env0, con
           for (int t = 0; t < 3; ++t) { l[3 * ci + t] = ci < np ? c.v[kLam + 3 * ci + t] : 0.0f; p[3 * ci + t] = c.v[9 * ci + t]; }
 #pragma unroll
         for (int f = 0; f < 3; ++f) {
-          stg_hint(ol + f, make_float4(l[4 * f], l[4 * f + 1], l[4 * f + 2], l[4 * f + 3]), once);
-          stg_hint(op + f, make_float4(p[4 * f], p[4 * f + 1], p[4 * f + 2], p[4 * f + 3]), once);
+          stg_hint<0>(ol + f, make_float4(l[4 * f], l[4 * f + 1], l[4 * f + 2], l[4 * f + 3]), once);
+          stg_hint<0>(op + f, make_float4(p[4 * f], p[4 * f + 1], p[4 * f + 2], p[4 * f + 3]), once);
         }
       }
       if (lambda_out) {                                          // lambda in contact order (debug / stage output)
