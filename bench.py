@@ -348,7 +348,7 @@ def run_cuda(args) -> dict:
     value = total_env_steps / (ms * 1e-3)
     e2e_value = E * Ke * world_size / (ms_e2e * 1e-3)
 
-    # ---- roofline.  Five kernels per substep: k_detect, k_plan (timed together), k_manifold, k_slot (S1-S4) and k_solve (S4 warm
+    # ---- roofline.  Six kernels per substep: k_detect, k_walk, k_plan (timed together), k_manifold, k_slot (S1-S4) and k_solve (S4 warm
     # start, S5, S6, S7), timed with CUDA events on the launching stream (jenga_profile_*).  `roofline` is the dominant kernel
     # (k_solve): its algorithmic FP32 thread-instructions / its summed launch time vs the FP32 issue rate measured by
     # jenga_measure_peaks on this device; "step" carries the same ratio for the whole step (both kernels).
@@ -390,7 +390,7 @@ def run_cuda(args) -> dict:
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "cfg5 (BASELINE.json configs[4]): 18-level 54-block towers, mu_s {0.25,0.40,0.60} round-robin, 0-12 removals, "
                                "Ziglar push sweep, dt=1/240, 20 PGS iters, rollout steps 0..K" if args.cfg == CFG else CFG_NAMES[args.cfg] + " (not the headline workload)",
-                   "envs_per_gpu": E, "n_bodies": wp.n_bodies, "pgs_iters": wp.pgs_iters, "steps_per_call": args.chunk, "kernels_per_substep": 5,
+                   "envs_per_gpu": E, "n_bodies": wp.n_bodies, "pgs_iters": wp.pgs_iters, "steps_per_call": args.chunk, "kernels_per_substep": 6,
                    "parallelism": f"env-sharded x{world_size}, no data-path collective",
                    "l2": (f"inputs larger than L2: state {E * 13 * wp.body_stride * 4 / 1e6:.0f} MB + scratch {E * linfo_scratch / 1e6:.0f} MB + warm-start cache "
                           f"{E * (wp.max_contacts // 4) * 104 / 1e6:.0f} MB per step vs 126 MB L2") if not small else
@@ -408,7 +408,7 @@ def run_cuda(args) -> dict:
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke,
                 "split": n_split, "launches": e2e_launches},
-        "gpu_launches": 5 * n_sub,
+        "gpu_launches": 6 * n_sub,
         "roofline": roofline,
     }
     if rank == 0 and world_size == 1 and not args.no_cpu_baseline:

@@ -129,7 +129,7 @@ typedef struct {
   float       *collapse_stats; /* [E][4] of the last step: dx_max [m], E_k [J], theta_max [rad], 0     */
   int32_t     *rest_steps; /* [E]  steps taken by the last jenga_simulate_until_rest; may be NULL      */
   void        *scratch;    /* jenga_scratch_bytes(desc) bytes, 16-byte aligned, ZERO-FILLED by the caller before the
-                              first call: the hand-off between the five kernels of a substep (solver constants,
+                              first call: the hand-off between the six kernels of a substep (solver constants,
                               pair headers and visit chunks of every group of envs) plus per-env bookkeeping (the
                               colouring of the last pair list, the rest flag).  Contents are private to the library. */
   size_t       scratch_bytes;
@@ -152,7 +152,7 @@ int jenga_narrowphase(jenga_world *w, void *cuda_stream);
  * (read only) when desc.warm_start = 1 and n_cache[env] > 0.  Eq. 13-15, Listing 1.                   */
 int jenga_pgs_solve(jenga_world *w, int iters, void *cuda_stream);
 
-/* n_steps advances of dt (each n_substeps substeps S1..S7 = five kernel launches: detection, colouring + visit plan, manifolds, contact setup,
+/* n_steps advances of dt (each n_substeps substeps S1..S7 = six kernel launches: detection, colouring, visit plan, manifolds, contact setup,
  * solve + integrate), all enqueued by this one call; state, cache, status and counters are updated in place.  */
 int jenga_step(jenga_world *w, int n_steps, void *cuda_stream);
 
@@ -208,7 +208,7 @@ const char *jenga_strerror(int code);
 
 /* Measurement aid (bench.py's roofline): while enabled, every launch of jenga_step / jenga_simulate_until_rest is
  * bracketed by CUDA events on the caller's stream.  jenga_profile_read synchronises on them and returns, for the launches
- * since the last enable / read, the summed device time [ms] of out[0] = the detection and plan kernels (S1, S2, SAT; colouring),
+ * since the last enable / read, the summed device time [ms] of out[0] = the detection, colouring and plan kernels (S1, S2, SAT; S4 order),
  * out[1] = the manifold kernel, out[2] = the contact-setup kernel (effective masses, warm-start lookup), out[3] = the
  * solve + integrate kernel; out[4] = number of substeps.  `out` is a HOST array of 5 doubles.               */
 int jenga_profile_enable(jenga_world *w, int on);

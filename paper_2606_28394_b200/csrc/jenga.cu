@@ -1,7 +1,8 @@
 // jenga.cu -- C-ABI of the batched Jenga step (include/jenga.h) over the four kernels of a substep.  sm_100a only.
 //
 //   k_detect  (kcollide.cuh)  S1 predict, S2 broadphase, S3 SAT                                -> scratch
-//   k_plan    (kcollide.cuh)  S4 colouring + visit plan of the groups whose pair lists changed  -> scratch
+//   k_walk    (kcollide.cuh)  S4 greedy colouring of the envs whose pair list changed          -> scratch
+//   k_plan    (kcollide.cuh)  S4 visit plan of the groups with such an env                      -> scratch
 //   k_manifold (kcollide.cuh) S3 contact manifolds                                              -> scratch
 //   k_slot    (kcollide.cuh)  S4 effective masses + warm-start lookup                           -> scratch
 //   k_solve   (ksolve.cuh)    S4 warm start, S5 PGS sweeps, S6 integrate, S7 cache, Eq. 18 latch
@@ -193,7 +194,7 @@ static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; 
 
 /* cudaFuncAttributeMaxDynamicSharedMemorySize is per kernel and process-wide: it is only ever raised (running maximum
  * per device), immediately before the launch that needs it, so worlds of different sizes can be used in any order.   */
-enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnPlan, KnSolveTm, KnSolveSm, KnCount };
+enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnPlan, KnWalk, KnSolveTm, KnSolveSm, KnCount };
 static std::mutex g_attr_mutex;
 static size_t g_attr_max[16][KnCount];
 
@@ -208,6 +209,7 @@ static const void* kernel_ptr(int kn) {
     case KnSlot: return (const void*)jenga::k_slot<jenga::ModeStep>;
     case KnSlotGiven: return (const void*)jenga::k_slot<jenga::ModeGiven>;
     case KnPlan: return (const void*)jenga::k_plan;
+    case KnWalk: return (const void*)jenga::k_walk;
     case KnSolveTm: return (const void*)jenga::k_solve<true>;
     default: return (const void*)jenga::k_solve<false>;
   }
@@ -336,7 +338,7 @@ static void mark(jenga_world* w, cudaStream_t st) {
   w->ev.push_back(e);
 }
 
-/* k_detect, then (except for jenga_broadphase) k_plan, k_manifold and k_slot, for every env */
+/* k_detect, then (except for jenga_broadphase) k_walk, k_plan, k_manifold and k_slot, for every env */
 static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_t st) {
   cudaError_t e = ensure_smem(w->desc.device, KnCollide + mode, w->smem_collide);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_detect)");
@@ -349,6 +351,12 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
   }
   int rc = launched("k_detect");
   if (rc != JENGA_OK || mode == jenga::ModeBroad) return rc;
+  const size_t smem_walk = (size_t)jenga::kWalkThreads * w->P.B * sizeof(unsigned long long);
+  e = ensure_smem(w->desc.device, KnWalk, smem_walk);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_walk)");
+  jenga::k_walk<<<(w->P.E + jenga::kWalkThreads - 1) / jenga::kWalkThreads, jenga::kWalkThreads, smem_walk, st>>>(w->P);
+  rc = launched("k_walk");
+  if (rc != JENGA_OK) return rc;
   e = ensure_smem(w->desc.device, KnPlan, w->smem_plan);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_plan)");
   jenga::k_plan<<<grid, thr, w->smem_plan, st>>>(w->P);

@@ -1,6 +1,6 @@
 // kcollide.cuh -- the collision kernels of a substep, one env per warp.  k_detect: S1 predict, S2 broadphase, S3 SAT
-// (which candidates collide).  k_plan: S4 canonical colouring + the group's visit plan (only for groups whose pair lists
-// changed).  k_manifold: S3 contact manifolds.  k_slot: S4 contact setup (effective masses, warm-start lookup).  Their
+// (which candidates collide).  k_walk: S4 canonical greedy colouring (one env per thread; only envs whose pair list
+// changed).  k_plan: the group's visit plan (only for groups with such an env).  k_manifold: S3 contact manifolds.  k_slot: S4 contact setup (effective masses, warm-start lookup).  Their
 // products go to the scratch buffer (layout.cuh) for the next kernel.  They are separate kernels because each one's hot
 // code then fits the 32 KB instruction cache (as one kernel: 70 KB, and `no_instruction` was the top stall with 16 warps
 // per SM at different places in it).
@@ -15,7 +15,7 @@ struct CSm {
   int cbw;                      // words per record: 20 (k_detect, k_manifold) or kCb = 28 (k_slot); a multiple of 4, odd in float4
   SP<float4> ext;               // [S]      world AABB half extents e'_x e'_y e'_z, flags (1 active | 2 dynamic)
   SP<unsigned> hitw;            // [ceil(S/32)][32] broadphase hit words of the current block of 32 rows
-  SP<unsigned long long> used;  // [S]      colour masks per body (k_plan)
+  SP<unsigned long long> used;  // unused (k_walk keeps the colour masks per body in its own layout)
   SP<unsigned> cab;             // [pcA]    (a+1) | A dynamic << 11 | axis << 12 | b << 16 | B dynamic << 27
   SP<unsigned short> cand;      // [mpA]    candidate pair indices, ascending
   SP<float> poly;               // [8][3][32] clip polygon of every lane (component-major: lane l <-> bank l)
@@ -35,23 +35,22 @@ enum { MiNph = 0, MiNcol = 1, MiNblk = 2, MiSame = 3 };
 
 enum { ArenaDetect = 0, ArenaManifold = 1, ArenaSlot = 2, ArenaPlan = 3 };
 
-// k_detect: records, extents, hit words, candidate list, colliding list.  k_plan: colliding list, masks, colouring and
+// k_detect: records, extents, hit words, candidate list, colliding list.  k_plan: colouring and
 // plan products (no body records).  k_manifold: records, colliding list (copied from the scratch), per-lane clip
 // polygons.  k_slot: records, colliding list, cache keys.
 __host__ __device__ inline int cb_words(int arena) { return arena == ArenaSlot ? kCb : (arena == ArenaPlan ? 0 : 20); }
 
 __host__ __device__ inline size_t collide_smem_words(int S, int max_pairs, int pc, int arena, int G) {
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc, G);
+  if (arena == ArenaPlan) {                                // wrank, colour, ph, chm, ccount, cfirst, fill, misc
+    const int phw = round_up(ph_max(nblk, G), 4);
+    return round_up(pcA / 2 + pcA / 4 + (1 + kMaxGroup) * phw + 2 * kMaxColours + round_up(nblk, 4) + 8, 4);
+  }
   size_t w = (size_t)cb_words(arena) * S + pcA + pcA / 2;  // cb, cab, cpair
   if (arena != ArenaManifold) w += 2 * (size_t)(pcA / 2);  // pos, wrank
   if (arena == ArenaDetect) {
     const int uh = 32 * ((S + 31) / 32);
     w += 4 * S + uh + mpA / 2 + 8;                         // ext, hitw, cand, misc
-  } else if (arena == ArenaPlan) {
-    const int phw = round_up(ph_max(nblk, G), 4);
-    w += 2 * S + pcA / 4;                                  // used, colour
-    w += (1 + kMaxGroup) * phw;                            // ph, chm
-    w += 2 * kMaxColours + round_up(nblk, 4) + 8;          // ccount, cfirst, fill, misc
   } else if (arena == ArenaManifold) {
     w += 768;                                              // poly
   } else {
@@ -64,6 +63,18 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int 
   const int pcA = round_up(pc, 8), mpA = round_up(max_pairs, 8), nblk = n_blocks(pc, G), phw = round_up(ph_max(nblk, G), 4);
   CSm s; int p = base;
   s.cbw = cb_words(arena);
+  if (arena == ArenaPlan) {
+    s.cb.off = s.cab.off = s.cpair.off = s.pos.off = s.ext.off = s.hitw.off = s.used.off = s.cand.off = s.cprev.off = s.poly.off = 0;
+    s.wrank.off = p;  p += pcA / 2;
+    s.colour.off = p; p += pcA / 4;
+    s.ph.off = p;     p += phw;
+    s.chm.off = p;    p += kMaxGroup * phw;
+    s.ccount.off = p; p += kMaxColours;
+    s.cfirst.off = p; p += kMaxColours;
+    s.fill.off = p;   p += round_up(nblk, 4);
+    s.misc.off = p;
+    return s;
+  }
   s.cb.off = p;     p += s.cbw * S;
   s.cab.off = p;    p += pcA;
   s.cpair.off = p;  p += pcA / 2;
@@ -76,15 +87,6 @@ __device__ inline CSm carve_collide(int S, int max_pairs, int pc, int base, int 
     s.ext.off = p;    p += 4 * S;
     s.hitw.off = p;   p += 32 * ((S + 31) / 32);
     s.cand.off = p;   p += mpA / 2;
-    s.misc.off = p;
-  } else if (arena == ArenaPlan) {
-    s.used.off = p;   p += 2 * S;
-    s.colour.off = p; p += pcA / 4;
-    s.ph.off = p;     p += phw;
-    s.chm.off = p;    p += kMaxGroup * phw;
-    s.ccount.off = p; p += kMaxColours;
-    s.cfirst.off = p; p += kMaxColours;
-    s.fill.off = p;   p += round_up(nblk, 4);
     s.misc.off = p;
   } else if (arena == ArenaManifold) {
     s.poly.off = p;
@@ -531,50 +533,40 @@ __device__ inline int find_colliding(const CSm& s, const Params& P, int n_cand, 
   return n;
 }
 
-// Canonical order (north_star (d), DESIGN §2 S4): visit the colliding pairs in ascending pair index;
-// colour = lowest colour not used by an earlier pair sharing a dynamic body.  The walk is sequential by definition
-// (lane 0, one 64-bit mask per body).  Products: s.colour[r], s.wrank[r] = rank of pair r inside its colour,
-// s.ccount[c], s.misc[MiNcol].  The colour of a pair depends on the pairs before it only: when the first r0 pairs are the
-// ones of the list coloured last time (gcol, gwrk: that colouring), their colours are kept -- masks and counts are rebuilt
-// from them by all lanes -- and the walk starts at r0.
-__device__ inline void colour_walk(const CSm& s, const Params& P, int n_coll, int r0, const unsigned char* gcol, const unsigned short* gwrk, unsigned* status) {
-  const int lane = lane_id();
-  for (int b = lane; b < P.B; b += 32) s.used[b] = 0ull;
-  for (int c = lane; c < kMaxColours; c += 32) s.ccount[c] = 0;
-  __syncwarp();
-  int ncol0 = 0;
-  for (int r = lane; r < r0; r += 32) {
-    const unsigned w = s.cab[r];
-    const int a = ab_a(w), b = ab_b(w), c = gcol[r];
-    s.colour[r] = (unsigned char)c; s.wrank[r] = gwrk[r];
-    if (a >= 0) atomicOr(&s.used[a], 1ull << c);
-    atomicOr(&s.used[b], 1ull << c);
-    atomicAdd(&s.ccount[c], 1);
-    ncol0 = max(ncol0, c + 1);
+// k_walk.  Canonical order (north_star (d), DESIGN §2 S4): visit the colliding pairs in ascending pair index;
+// colour = lowest colour not used by an earlier pair sharing a dynamic body.  The walk of ONE env is sequential by
+// definition, so a THREAD walks an env (one 64-bit colour mask per body in shared memory, [body][thread]: conflict-free)
+// and the 32 lanes of a warp walk 32 envs at once -- only envs whose pair list changed (same_flag) take part.  Products, in
+// the env's scratch: the colour of every pair (bytes, four per store) and meta[MetaNcol]; k_plan derives ranks and counts.
+constexpr int kWalkThreads = 64;
+__global__ void __launch_bounds__(kWalkThreads) k_walk(const Params P) {
+  const int env = blockIdx.x * kWalkThreads + threadIdx.x, t = threadIdx.x;
+  if (env >= P.E || P.same_flag[env] != 0) return;
+  unsigned long long* used = reinterpret_cast<unsigned long long*>(smem_f);
+  const Scratch L = scratch_layout(P.pc, P.G);
+  float* scr = P.scratch + (size_t)env * P.scratch_words;
+  int* meta = reinterpret_cast<int*>(scr + L.meta);
+  const unsigned* gcab = reinterpret_cast<const unsigned*>(scr + L.cab);
+  unsigned* gcol4 = reinterpret_cast<unsigned*>(scr + L.col);
+  const int n = meta[MetaNcoll];
+  for (int b = 0; b < P.B; ++b) used[b * kWalkThreads + t] = 0ull;
+  int ncol = 0; unsigned st = 0, pack = 0;
+  for (int r = 0; r < n; ++r) {
+    const unsigned w = gcab[r];
+    const int a = ab_a(w), b = ab_b(w);
+    unsigned long long m = 0ull;
+    if (w & (1u << 11)) m |= used[a * kWalkThreads + t];
+    if (w & (1u << 27)) m |= used[b * kWalkThreads + t];
+    int c = __ffsll((long long)~m) - 1;
+    if (c < 0) { c = kMaxColours - 1; st |= JENGA_ST_COLOUR_OVERFLOW; }
+    if (a >= 0) used[a * kWalkThreads + t] |= 1ull << c;
+    used[b * kWalkThreads + t] |= 1ull << c;
+    pack |= (unsigned)c << (8 * (r & 3));
+    if ((r & 3) == 3 || r == n - 1) { gcol4[r >> 2] = pack; pack = 0; }
+    if (c + 1 > ncol) ncol = c + 1;
   }
-  ncol0 = __reduce_max_sync(kFull, ncol0);
-  __syncwarp();
-  if (lane == 0) {
-    int ncol = ncol0; unsigned st = 0;
-    for (int r = r0; r < n_coll; ++r) {
-      const unsigned w = s.cab[r];
-      const int a = ab_a(w), b = ab_b(w);
-      unsigned long long m = 0ull;
-      if (w & (1u << 11)) m |= s.used[a];
-      if (w & (1u << 27)) m |= s.used[b];
-      int c = __ffsll((long long)~m) - 1;
-      if (c < 0) { c = kMaxColours - 1; st |= JENGA_ST_COLOUR_OVERFLOW; }
-      if (a >= 0) s.used[a] |= 1ull << c;
-      s.used[b] |= 1ull << c;
-      s.colour[r] = (unsigned char)c;
-      const int k = s.ccount[c];
-      s.wrank[r] = (unsigned short)k; s.ccount[c] = k + 1;
-      if (c + 1 > ncol) ncol = c + 1;
-    }
-    s.misc[MiNcol] = ncol;
-    if (st) *status |= st;
-  }
-  __syncwarp();
+  meta[MetaNcol] = ncol;
+  if (st) atomicOr(P.status + env, st);
 }
 
 // chunk word of a member: colour | first rank-in-colour << 6 | pairs << 20
@@ -663,16 +655,7 @@ __device__ inline void publish_pairs(const CSm& s, const Params& P, int env, flo
   if (same)
     for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
   same = __all_sync(kFull, same);
-  if (!same) {
-    // the first position at which the new list differs from the one coloured last time (0 if there is no such colouring)
-    const int n_old = meta[MetaMagic] == kMagic ? meta[MetaNcoll] : 0, n_min = min(n_old, n_coll);
-    int first = n_min;
-    for (int r = lane; r < n_min; r += 32) if (s.cpair[r] != gpair[r]) { first = r; break; }
-    first = __reduce_min_sync(kFull, first);
-    __syncwarp();
-    for (int r = lane; r < n_coll; r += 32) gpair[r] = s.cpair[r];
-    if (lane == 0) meta[MetaFirst] = first;
-  }
+  if (!same) for (int r = lane; r < n_coll; r += 32) gpair[r] = s.cpair[r];
   if (lane == 0) {
     P.same_flag[env] = same ? 1 : 0;
     if (!same) { meta[MetaMagic] = 0; meta[MetaNcoll] = n_coll; }
@@ -683,10 +666,11 @@ __device__ __forceinline__ void pair_barrier(int id) {
   if (id == 1) asm volatile("bar.sync 1, 64;" ::: "memory"); else asm volatile("bar.sync 2, 64;" ::: "memory");
 }
 
-// k_plan: S4 colouring + visit plan of the group this env belongs to, when the pair list of one of its members changed.
+// k_plan: S4 visit plan of the group this env belongs to, when the pair list of one of its members changed (k_walk has
+// coloured the changed lists).
 // One warp per env; with G = 2 the two warps of a group are neighbours in the CTA, exchange their colour counts through
 // shared memory and meet at a named barrier (id 1 + warp / 2); both take the same path (the decision depends on the
-// group's same_flag entries only).  A member whose own list did not change reloads its colouring from the scratch.
+// group's same_flag entries only).  A member whose own list did not change reloads ranks and counts from the scratch.
 __device__ inline void plan_env(const Params& P, const int env) {
   const int warp = threadIdx.x >> 5, lane = lane_id(), G = P.G;
   const int me = G == 2 ? (env & 1) : 0;
@@ -708,14 +692,24 @@ __device__ inline void plan_env(const Params& P, const int env) {
   unsigned char* gcol = reinterpret_cast<unsigned char*>(scr + L.col);
   unsigned short* gwrk = reinterpret_cast<unsigned short*>(scr + L.wrk);
   int* gcnt = reinterpret_cast<int*>(scr + L.ccnt);
-  if (!same_me) {                                              // colour the new list, keep the colouring
-    const unsigned* gcab = reinterpret_cast<const unsigned*>(scr + L.cab);
-    for (int r = lane; r < n_coll; r += 32) s.cab[r] = gcab[r];
+  if (!same_me) {                                              // k_walk coloured the new list: ranks and counts, kept with it
+    for (int c = lane; c < kMaxColours; c += 32) s.ccount[c] = 0;
     __syncwarp();
-    const int r0 = max(0, min(meta[MetaFirst], n_coll));
-    colour_walk(s, P, n_coll, r0, gcol, gwrk, &st);
-    for (int r = lane + (r0 & ~31); r < n_coll; r += 32) if (r >= r0) { gcol[r] = s.colour[r]; gwrk[r] = s.wrank[r]; }
+    const unsigned below = (1u << lane) - 1u;
+    for (int base = 0; base < n_coll; base += 32) {            // rank of pair r inside its colour = pairs of that colour before it
+      const int r = base + lane, c = r < n_coll ? gcol[r] : 255;
+      const unsigned peers = __match_any_sync(kFull, c);
+      if (r < n_coll) {
+        const int k = s.ccount[c] + __popc(peers & below);
+        s.colour[r] = (unsigned char)c; s.wrank[r] = (unsigned short)k; gwrk[r] = (unsigned short)k;
+      }
+      __syncwarp();
+      if (r < n_coll && (peers & below) == 0) s.ccount[c] += __popc(peers);
+      __syncwarp();
+    }
     for (int c = lane; c < kMaxColours; c += 32) gcnt[c] = s.ccount[c];
+    if (lane == 0) s.misc[MiNcol] = meta[MetaNcol];
+    __syncwarp();
   } else {                                                     // the list is the one coloured last time
     if (present) {
       for (int r = lane; r < n_coll; r += 32) { s.colour[r] = gcol[r]; s.wrank[r] = gwrk[r]; }
@@ -760,7 +754,7 @@ __device__ inline void plan_env(const Params& P, const int env) {
       }
       gpos[r] = (unsigned short)k;
     }
-    if (lane == 0) { meta[MetaMagic] = kMagic; meta[MetaNcol] = s.misc[MiNcol]; }
+    if (lane == 0) meta[MetaMagic] = kMagic;
     flush_status(P, env, st);
   }
   if (me == 0) {                                              // group data: in the region of the group's first env

@@ -1,9 +1,10 @@
 // layout.cuh -- parameters, the global hand-off ("scratch") between the four kernels of a substep, and the shared
 // memory arenas of the batched Jenga step (sm_100a).
 //
-// A substep (S1..S7 of include/jenga.h) is FIVE kernels:
+// A substep (S1..S7 of include/jenga.h) is SIX kernels:
 //   k_detect   S1 predict, S2 broadphase, S3 SAT (which candidates collide, on which axis).  One warp per env.
-//   k_plan     S4 canonical colouring and the visit plan of the env GROUP, for the groups whose pair lists changed.
+//   k_walk     S4 canonical greedy colouring of the envs whose pair list changed.  One THREAD per env.
+//   k_plan     S4 visit plan of the env GROUP, for the groups with such an env.  One warp per env.
 //   k_manifold S3 contact manifolds of the colliding pairs.  One warp per env.
 //   k_slot     S4 contact setup (effective masses, warm-start lookup).  One warp per env.  Small footprints (8-11 KB of
 //              shared memory per 54-body env, <= 128 registers): 16+ warps per SM hide the latencies of this branchy,
@@ -41,7 +42,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr int kScratchHead = 64;             // global words in front of the per-env scratch: [0] = k_solve's work counter
 constexpr int kMagic = 0x4a454e47;          // "JENG": scratch meta stamp of a valid colouring
 
-enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaFirst, MetaWords = 16 };
+enum { MetaMagic = 0, MetaNcoll, MetaNph, MetaNcol, MetaNblk, MetaResting, MetaSteps, MetaNcont, MetaWords = 16 };
 
 // modes of the collision kernels
 enum { ModeStep = 0, ModeBroad = 1, ModeNarrow = 2, ModeGiven = 3 };
