@@ -538,7 +538,6 @@ __global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, cons
     if (g >= n_groups) break;
     if (lane == 0) g_next = atomicAdd(P.work_counter, 1);
     g_next = __shfl_sync(kFull, g_next, 0);
-    if (g_next < n_groups) prefetch_group(P, L, g_next);
     const int env0 = g * G, nm = min(G, P.E - env0);
     float* scr0 = P.scratch + (size_t)env0 * P.scratch_words;
     bool act[kMaxGroup]; bool any = false;
@@ -556,6 +555,9 @@ __global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, cons
     const int nph = load_slots<TM>(s, scr0, L);
     if (P.warm_start) warm_start_pass<TM>(s, nph);
     pgs_sweeps<TM>(s, nph, iters, P.mu[env0], act[kMaxGroup - 1] ? P.mu[env0 + kMaxGroup - 1] : 0.0f);
+    // the next group into L2 now: requested when this group was taken (a whole group's duration ago, during which the
+    // GPU streams twice the L2's size through it) the lines would be gone again by the time they are used
+    if (g_next < n_groups) prefetch_group(P, L, g_next);
     if (flags & SolvePgsOnly) {
       finish_pairs<TM>(s, P, env0, L, nph, false, false, true);  // lambda in contact order only
 #pragma unroll
