@@ -1,4 +1,4 @@
-// jenga.cu -- C-ABI of the batched Jenga step (include/jenga.h) over the four kernels of a substep.  sm_100a only.
+// jenga.cu -- C-ABI of the batched Jenga step (include/jenga.h) over the six kernels of a substep.  sm_100a only.
 //
 //   k_detect  (kcollide.cuh)  S1 predict, S2 broadphase, S3 SAT                                -> scratch
 //   k_walk    (kcollide.cuh)  S4 greedy colouring of the envs whose pair list changed          -> scratch

@@ -1,4 +1,4 @@
-// layout.cuh -- parameters, the global hand-off ("scratch") between the four kernels of a substep, and the shared
+// layout.cuh -- parameters, the global hand-off ("scratch") between the six kernels of a substep, and the shared
 // memory arenas of the batched Jenga step (sm_100a).
 //
 // A substep (S1..S7 of include/jenga.h) is SIX kernels:
