@@ -194,7 +194,7 @@ static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; 
 
 /* cudaFuncAttributeMaxDynamicSharedMemorySize is per kernel and process-wide: it is only ever raised (running maximum
  * per device), immediately before the launch that needs it, so worlds of different sizes can be used in any order.   */
-enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnPlan, KnWalk, KnSolveTm, KnSolveSm, KnCount };
+enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnPlan, KnWalk, KnSolveTm, KnSolveTm384, KnSolveTm256, KnSolveTm128, KnSolveSm, KnCount };
 static std::mutex g_attr_mutex;
 static size_t g_attr_max[16][KnCount];
 
@@ -210,8 +210,11 @@ static const void* kernel_ptr(int kn) {
     case KnSlotGiven: return (const void*)jenga::k_slot<jenga::ModeGiven>;
     case KnPlan: return (const void*)jenga::k_plan;
     case KnWalk: return (const void*)jenga::k_walk;
-    case KnSolveTm: return (const void*)jenga::k_solve<true>;
-    default: return (const void*)jenga::k_solve<false>;
+    case KnSolveTm: return (const void*)jenga::k_solve<true, 512>;
+    case KnSolveTm384: return (const void*)jenga::k_solve<true, 384>;
+    case KnSolveTm256: return (const void*)jenga::k_solve<true, 256>;
+    case KnSolveTm128: return (const void*)jenga::k_solve<true, 128>;
+    default: return (const void*)jenga::k_solve<false, 32>;
   }
 }
 
@@ -381,17 +384,24 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
 }
 
 static int launch_solve(jenga_world* w, int iters, int flags, float rest_ek, cudaStream_t st) {
-  const cudaError_t e = ensure_smem(w->desc.device, w->tmb ? KnSolveTm : KnSolveSm, w->smem_solve);
+  const int q = tier_groups(w->tmb);
+  const int kn = !w->tmb ? KnSolveSm : (q == 4 ? KnSolveTm : (q == 3 ? KnSolveTm384 : (q == 2 ? KnSolveTm256 : KnSolveTm128)));
+  const cudaError_t e = ensure_smem(w->desc.device, kn, w->smem_solve);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_solve)");
   /* persistent CTAs: one per SM in the TMEM tiers (it owns all 512 columns), each warp takes groups from a global queue */
   const int n_groups = (w->P.E + w->G - 1) / w->G;
   if (w->tmb) {
     /* small batches are spread over all SMs (the warps of every CTA pull groups from the same queue) */
     const int wpc = 4 * tier_groups(w->tmb), grid = n_groups < w->n_sm ? n_groups : w->n_sm;
-    jenga::k_solve<true><<<grid, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
+    switch (q) {
+      case 4: jenga::k_solve<true, 512><<<grid, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek); break;
+      case 3: jenga::k_solve<true, 384><<<grid, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek); break;
+      case 2: jenga::k_solve<true, 256><<<grid, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek); break;
+      default: jenga::k_solve<true, 128><<<grid, 32 * wpc, w->smem_solve, st>>>(w->P, iters, flags, rest_ek); break;
+    }
   } else {
     const int per_sm = (int)(kSmemMax / (w->smem_solve + 1024)), resident = w->n_sm * (per_sm < 1 ? 1 : (per_sm > 16 ? 16 : per_sm));
-    jenga::k_solve<false><<<n_groups < resident ? n_groups : resident, 32, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
+    jenga::k_solve<false, 32><<<n_groups < resident ? n_groups : resident, 32, w->smem_solve, st>>>(w->P, iters, flags, rest_ek);
   }
   return launched("k_solve");
 }

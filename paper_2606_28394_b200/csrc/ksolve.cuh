@@ -516,8 +516,9 @@ __device__ inline void prefetch_group(const Params& P, const Scratch& L, int g) 
 // bit 2 honour / update the per-env rest flag (jenga_simulate_until_rest).
 enum { SolveEndOfStep = 1, SolvePgsOnly = 2, SolveRest = 4 };
 
-template <bool TM>
-__global__ void __launch_bounds__(TM ? 512 : 32, 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
+// THREADS: the CTA size of the tier (the register budget follows it: 128 per thread with 16 warps, 168 with 12).
+template <bool TM, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1) k_solve(const Params P, const int iters, const int flags, const float rest_ek) {
   SSm s = begin_solve<TM>(P);
   const int lane = lane_id(), G = P.G;
   const Scratch L = scratch_layout(P.pc, G);
