@@ -203,7 +203,7 @@ def run_dry(args):
     rank, world_size = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     if world_size > 1:
         dist.init_process_group(args.backend)
-    lo, hi = shard.env_range(rank, world_size, args.envs)
+    lo, hi = shard.env_range(rank, world_size, args.envs or CFG_ENVS[args.cfg])
     ms = shard.max_over_ranks(100.0 + rank)                       # stands in for the device time of this rank
     total = shard.sum_over_ranks(hi - lo)
     if world_size > 1:
