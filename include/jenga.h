@@ -204,6 +204,41 @@ int jenga_env_group(const jenga_world_desc *desc);
 /* Size of jenga_buffers.scratch for this descriptor (0 if invalid). */
 size_t jenga_scratch_bytes(const jenga_world_desc *desc);
 
+/* S3 for callers that have no device memory to lend the library as scratch.  Who that is: a plug-in inside a host program
+ * whose memory pool was carved up at start-up and is closed to further requests; a control loop that must not meet the
+ * device-wide stall a cudaMalloc / cudaFree implies; a thread that is inside a region of its own where the CUDA allocator
+ * may not be called at all.  Such a caller can still own state / props / pairs / contacts (they are its data), but it
+ * cannot size, obtain and zero a jenga_buffers.scratch, so it cannot create a jenga_world.  This ONE call does without:
+ * the same narrowphase as jenga_narrowphase (§6.2: 15-axis SAT, face / edge / ground manifolds of at
+ * most 4 points), bit for bit, as a single kernel launch whose hand-off area is an array built into the library image.
+ *
+ *   desc  the fields n_envs, n_bodies, body_stride, max_pairs, max_contacts, edge_bias_rel, edge_bias_abs, par_eps,
+ *         tie_eps and device are used (struct_size is checked); everything else is ignored.
+ *   IN    state [E][13][S], props [E][8][S], pairs [E][max_pairs], n_pairs [E]     (layouts as in jenga_buffers)
+ *   OUT   contacts [E][max_contacts][8], n_contacts [E]; status [E] gets JENGA_ST_CONTACT_OVERFLOW OR-ed in.
+ *   All seven are DEVICE pointers owned by the caller; state, props, pairs and contacts 16-byte aligned.
+ *
+ * Limit.  The built-in array has JENGA_STATIC_SCRATCH_BYTES (8 MiB); an env takes jenga_narrowphase_static_env_bytes(desc)
+ * of it (15,616 B at max_contacts = 704: up to 537 envs per call).  A larger batch is refused with JENGA_E_STATIC_CAPACITY
+ * and nothing is launched: split it into several calls on the same stream (env ranges are independent).
+ * Cost.  Every GPU on which a process uses libjenga.so carries these 8 MiB from the moment the library's device code is
+ * loaded there until the process exits, whether this call is ever made or not.
+ * No allocation: the call makes no cudaMalloc / cudaFree / cudaMallocAsync, no host allocation of its own, and calls no
+ * library routine that allocates.  The FIRST call on each device looks up the array's device address
+ * (cudaGetSymbolAddress) and raises the kernel's shared-memory limit; make that first call outside any stream capture.
+ * Later calls only enqueue the kernel on `cuda_stream` and return (asynchronous like the other stage calls).
+ * Sharing.  There is one array per device, shared by every call from every thread and stream, and it keeps what the last
+ * call left in it.  The kernel reads back only words that the same launch wrote earlier, so nothing needs to start at zero
+ * and nothing is cleared -- but two calls whose kernels may run at the same time on one device (different streams, or
+ * different host threads with their own streams) overwrite each other's hand-off and produce garbage without any error.
+ * Keep all calls of a device on one stream, or order them with events.                                                  */
+#define JENGA_STATIC_SCRATCH_BYTES (8u << 20)
+#define JENGA_E_STATIC_CAPACITY -4   /* jenga_narrowphase_static: n_envs x per-env bytes exceeds JENGA_STATIC_SCRATCH_BYTES */
+int jenga_narrowphase_static(const jenga_world_desc *desc, const float *state, const float *props, const int32_t *pairs,
+                             const int32_t *n_pairs, float *contacts, int32_t *n_contacts, uint32_t *status, void *cuda_stream);
+/* Bytes of the built-in array that one env of this descriptor takes (0 if the descriptor is out of range). */
+size_t jenga_narrowphase_static_env_bytes(const jenga_world_desc *desc);
+
 const char *jenga_strerror(int code);
 
 /* Measurement aid (bench.py's roofline): while enabled, every launch of jenga_step / jenga_simulate_until_rest is

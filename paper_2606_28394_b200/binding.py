@@ -81,6 +81,10 @@ def lib():
         L.jenga_measure_peaks.restype = C.c_int
         L.jenga_peaks_scratch_bytes.restype = C.c_size_t
         L.jenga_strerror.restype = C.c_char_p
+        L.jenga_narrowphase_static.argtypes = [C.POINTER(WorldDesc)] + [C.c_void_p] * 8
+        L.jenga_narrowphase_static.restype = C.c_int
+        L.jenga_narrowphase_static_env_bytes.argtypes = [C.POINTER(WorldDesc)]
+        L.jenga_narrowphase_static_env_bytes.restype = C.c_size_t
         for f in ("jenga_world_create", "jenga_world_destroy", "jenga_broadphase", "jenga_narrowphase", "jenga_pgs_solve",
                   "jenga_step", "jenga_step_host", "jenga_simulate_until_rest", "jenga_set_f_ext", "jenga_block_threads", "jenga_env_group",
                   "jenga_profile_enable", "jenga_profile_read", "jenga_support_margin", "jenga_ziglar_block_analysis"):
@@ -126,6 +130,33 @@ def jenga_measure_peaks(device: int = 0) -> dict:
         _check(L.jenga_measure_peaks(out, C.c_void_p(scratch.data_ptr()), C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)),
                "jenga_measure_peaks")
     return dict(fp32_instr_per_s=out[0], smem_bytes_per_s=out[1], n_sm=int(out[2]), ffma_s=out[3], lds_s=out[4], fp32_instr_per_s_3reg=out[5], fp32_instr_per_s_noreuse=out[6], fp32_fma_per_s_packed_noreuse=out[7])
+
+
+STATIC_SCRATCH_BYTES = 8 << 20
+E_STATIC_CAPACITY = -4
+
+
+def jenga_narrowphase_static(desc: WorldDesc, state, props, pairs, n_pairs, contacts, n_contacts, status):
+    """jenga_narrowphase for a caller that has no device memory to give the library as scratch (include/jenga.h).
+
+    Every argument after `desc` is a CUDA tensor the caller already owns (inputs state, props, pairs, n_pairs; outputs
+    contacts, n_contacts, status); this function only passes their addresses and torch's current stream on.  Neither it
+    nor the library allocates: the kernel's hand-off area is an 8 MiB array inside libjenga.so (STATIC_SCRATCH_BYTES),
+    one per device, shared by all calls -- so a batch must fit it (JengaError with code E_STATIC_CAPACITY otherwise;
+    jenga_narrowphase_static_env_bytes(desc) is the share of one env) and calls on one device must not overlap in time.
+    The first call on a device does a one-off set-up and belongs outside stream capture."""
+    dev = state.device
+    for t in (state, props, pairs, n_pairs, contacts, n_contacts, status):
+        assert t.is_cuda and t.device == dev and t.is_contiguous()
+    p = lambda t: C.c_void_p(t.data_ptr())
+    with torch.cuda.device(dev):
+        _check(lib().jenga_narrowphase_static(C.byref(desc), p(state), p(props), p(pairs), p(n_pairs), p(contacts), p(n_contacts),
+                                              p(status), C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)),
+               "jenga_narrowphase_static")
+
+
+def jenga_narrowphase_static_env_bytes(desc: WorldDesc) -> int:
+    return int(lib().jenga_narrowphase_static_env_bytes(C.byref(desc)))
 
 
 class World:

@@ -181,6 +181,8 @@ extern "C" const char* jenga_strerror(int code) {
     case JENGA_E_ARG: return "bad argument (NULL or misaligned pointer, size or capacity out of range)";
     case JENGA_E_CUDA: return g_err;
     case JENGA_E_DEVICE: return "device is not sm_100 or not the current device (kernels are built for sm_100a only)";
+    case JENGA_E_STATIC_CAPACITY: return "jenga_narrowphase_static: n_envs x jenga_narrowphase_static_env_bytes(desc) exceeds the built-in "
+                                         "scratch (JENGA_STATIC_SCRATCH_BYTES = 8 MiB); split the batch into smaller calls";
     default: return "unknown error";
   }
 }
@@ -484,4 +486,149 @@ extern "C" int jenga_ziglar_block_analysis(jenga_world* w, const int32_t* block,
   if (!w || !block || !axis || !aligned16(out)) return JENGA_E_ARG;
   jenga::k_ziglar<<<(w->P.E + 127) / 128, 128, 0, (cudaStream_t)stream>>>(w->P, block, axis, reinterpret_cast<float4*>(out));
   return launched("k_ziglar");
+}
+
+// =================================================================== jenga_narrowphase_static: S3 with no caller scratch
+// For callers that cannot hand the library device memory of their own to work in (include/jenga.h says who): the
+// narrowphase as ONE kernel whose hand-off area is the array below, part of the library image on every device that
+// loads it.  Nothing above this line is touched by it; it has its own per-device set-up and its own shared-memory bookkeeping.
+
+/* The built-in hand-off area.  In HOST code this name is only a stand-in for the symbol -- its host address is not where the
+ * array lives on the GPU -- so the host never passes it to a kernel: static_scratch_of() asks the runtime for the device
+ * address once per device (cudaGetSymbolAddress, with that device current) and the launch passes that pointer.            */
+static __device__ __align__(256) float g_static_scratch[JENGA_STATIC_SCRATCH_BYTES / sizeof(float)];
+
+namespace jenga {
+
+// Per-env region of the built-in area: only what the narrowphase hands from its first half to its second (the solver
+// blocks, chunk list and colouring of the full layout are left out: 15.6 KB per 54-block env instead of 103 KB).
+// Regions are multiples of 256 bytes; every array starts on a 16-byte boundary.
+__host__ __device__ inline Scratch static_layout(int pc) {
+  const int pcA = round_up(pc, 8);
+  Scratch L; int p = 0;
+  L.cs = L.ph = L.pos = L.col = L.wrk = L.ccnt = 0;      // not part of this layout, never addressed
+  L.meta = p;  p += MetaWords;
+  L.cpair = p; p += pcA / 2;
+  L.coff = p;  p += pcA / 2;
+  L.cab = p;   p += pcA;
+  L.man = p;   p += 20 * pcA;
+  L.total = round_up(p, 64);
+  return L;
+}
+
+// One warp per env.  First half = k_detect<ModeNarrow> without the colouring hand-over: body records, the caller's candidate
+// list, SAT -> colliding pairs (index, bodies, axis) into the env's region of the area.  Second half = k_manifold<ModeNarrow>:
+// the records again in the manifold arena (it re-carves the same shared memory), the colliding list read back from the
+// area, manifolds -> contacts / n_contacts in (pair, slot) order.  Same device functions, same order of arithmetic as the
+// two kernels of jenga_narrowphase, so the contact list is the same bit for bit.  A warp reads back only what it wrote
+// itself in this launch (ordered by __syncwarp), so the area's previous contents never matter.
+// arena_words: shared-memory words per warp = the larger of the two arenas (the second must not reach into a neighbour's first).
+__global__ void __launch_bounds__(128) k_narrow_static(const Params P, const int arena_words) {
+  const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = lane_id();
+  const int env = blockIdx.x * wpc + warp;
+  if (env >= P.E) return;
+  const Scratch L = static_layout(P.pc);
+  float* scr = P.scratch + (size_t)env * P.scratch_words;
+  int* meta = reinterpret_cast<int*>(scr + L.meta);
+  unsigned st = 0;
+  {
+    const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * arena_words, ArenaDetect, 1);
+    load_predict(s, P, env, false);
+    const int n_cand = load_candidates(s, P, env);
+    const int n_coll = find_colliding(s, P, n_cand, &st);
+    unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
+    unsigned* gcab = reinterpret_cast<unsigned*>(scr + L.cab);
+    for (int r = lane; r < n_coll; r += 32) { gcab[r] = s.cab[r]; gpair[r] = s.cpair[r]; }
+    if (lane == 0) meta[MetaNcoll] = n_coll;
+    __syncwarp();                                            // the lanes' global writes are visible to the warp from here on
+  }
+  {
+    const CSm s = carve_collide(P.S, P.max_pairs, P.pc, warp * arena_words, ArenaManifold, 1);
+    load_predict(s, P, env, false, false);
+    const int n_coll = load_colliding(s, scr, L, false);
+    manifold_pairs(s, P, env, scr, L, n_coll, true);
+  }
+  flush_status(P, env, st);
+}
+
+}  // namespace jenga
+
+static size_t static_arena_bytes(const jenga_world_desc* d) {
+  const size_t a = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaDetect, 1);
+  const size_t b = 4 * jenga::collide_smem_words(d->body_stride, d->max_pairs, d->max_contacts / 4, jenga::ArenaManifold, 1);
+  return a > b ? a : b;
+}
+
+/* the fields jenga_narrowphase_static reads (the rest of the descriptor is ignored) */
+static bool static_desc_ok(const jenga_world_desc* d) {
+  if (!d || d->struct_size != sizeof(jenga_world_desc)) return false;
+  if (d->n_envs <= 0 || d->n_bodies <= 0 || d->n_bodies > 360) return false;
+  if (d->body_stride < d->n_bodies || (d->body_stride & 3)) return false;
+  if (d->max_pairs <= 0 || d->max_pairs > 65535) return false;
+  if (d->max_contacts < 4 || (d->max_contacts & 3) || d->max_contacts > 65532) return false;
+  if (d->device < 0 || d->device >= 64) return false;
+  return static_arena_bytes(d) <= kSmemMax;
+}
+
+extern "C" size_t jenga_narrowphase_static_env_bytes(const jenga_world_desc* d) {
+  return static_desc_ok(d) ? (size_t)jenga::static_layout(d->max_contacts / 4).total * sizeof(float) : 0;
+}
+
+/* Per-device set-up, done by the first call on that device and kept: the device address of g_static_scratch and the
+ * shared-memory limit the kernel has been given there.  No allocation: two runtime queries and one attribute.          */
+struct static_dev { float* ptr; size_t smem_max; bool ready; };
+static static_dev g_static_dev[64];
+static std::mutex g_static_mutex;
+
+static int static_scratch_of(int device, size_t smem, float** out) {
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  static_dev& sd = g_static_dev[device];
+  if (!sd.ready) {
+    int major = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+    if (major != 10) return JENGA_E_DEVICE;
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_scratch);          /* answers for the CURRENT device: the caller checked it is `device` */
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_static_scratch)");
+    if (!p || (((uintptr_t)p) & 255u)) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_static_scratch): unaligned");
+    sd.ptr = (float*)p; sd.smem_max = 48 * 1024; sd.ready = true;
+  }
+  if (smem > sd.smem_max) {
+    const cudaError_t e = cudaFuncSetAttribute((const void*)jenga::k_narrow_static, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_narrow_static)");
+    sd.smem_max = smem;
+  }
+  *out = sd.ptr;
+  return JENGA_OK;
+}
+
+extern "C" int jenga_narrowphase_static(const jenga_world_desc* d, const float* state, const float* props, const int32_t* pairs,
+                                        const int32_t* n_pairs, float* contacts, int32_t* n_contacts, uint32_t* status, void* stream) {
+  if (!static_desc_ok(d)) return JENGA_E_ARG;
+  if (!aligned16(state) || !aligned16(props) || !aligned16(pairs) || !n_pairs || !aligned16(contacts) || !n_contacts || !status)
+    return JENGA_E_ARG;
+  const jenga::Scratch L = jenga::static_layout(d->max_contacts / 4);
+  if ((unsigned long long)d->n_envs * (unsigned long long)L.total * sizeof(float) > JENGA_STATIC_SCRATCH_BYTES)
+    return JENGA_E_STATIC_CAPACITY;                            /* beyond the built-in area: nothing is launched */
+  int cur = -1;
+  const cudaError_t e = cudaGetDevice(&cur);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+  if (cur != d->device) return JENGA_E_DEVICE;                 /* the address below is the current device's copy of the array */
+  const size_t arena = static_arena_bytes(d);
+  const int wpc = 4 * arena <= kSmemMax ? 4 : (2 * arena <= kSmemMax ? 2 : 1);
+  float* area = nullptr;
+  const int rc = static_scratch_of(d->device, wpc * arena, &area);
+  if (rc != JENGA_OK) return rc;
+  Params P;
+  memset(&P, 0, sizeof(P));                                    /* every pointer the narrowphase does not use stays NULL */
+  P.E = d->n_envs; P.B = d->n_bodies; P.S = d->body_stride; P.G = 1;
+  P.cp.edge_bias_rel = d->edge_bias_rel; P.cp.edge_bias_abs = d->edge_bias_abs; P.cp.par_eps = d->par_eps; P.cp.tie_eps = d->tie_eps;
+  P.max_pairs = d->max_pairs; P.max_contacts = d->max_contacts; P.pc = d->max_contacts / 4;
+  P.state = const_cast<float*>(state);                         /* read only here: load_predict(predict = false) */
+  P.props = props; P.pairs = const_cast<int*>(pairs); P.n_pairs = const_cast<int*>(n_pairs);
+  P.contacts = contacts; P.n_contacts = n_contacts; P.status = status;
+  P.scratch = area; P.scratch_words = L.total;
+  jenga::k_narrow_static<<<(P.E + wpc - 1) / wpc, 32 * wpc, wpc * arena, (cudaStream_t)stream>>>(P, (int)(arena / 4));
+  return launched("k_narrow_static");
 }
