@@ -7,8 +7,10 @@
 Workload: BASELINE.json configs[4] ("cfg5", the throughput headline): 65,536 envs of 18-level, 54-block
 towers per GPU, mu_s round-robin, 0-12 removals, Ziglar push sweep, dt = 1/240, 20 PGS iterations, fp32;
 seeded synthetic inputs from paper_2606_28394_b200/workloads.py.  A "step" is one dt
-advance of every env of the batch through the whole hot path (S1..S7, one fused kernel).  The timed region
-starts at step 0 of the rollout (cold warm-start cache, settle window, push at steps 60-83) and covers K steps.
+advance of every env of the batch through the whole hot path (S1..S7, six kernels per substep).  With no --steps the
+timed region is the whole 480-step rollout (cold warm-start cache, settle window, push at steps 60-83, collapse);
+with --steps K below that, the K timed steps are spread evenly over the rollout and the steps in between run untimed
+(config.window says which), so a short run still measures the rollout's mix and not only its standing towers.
 Weak scaling: each rank owns its own 65,536 envs (env ids rank*E ..), no collective on the data path.
 
 One JSON line on stdout (rank 0).  See DESIGN.md §7 for the work model behind "roofline".
@@ -117,6 +119,20 @@ def schedule(wl, n_steps: int, chunk: int):
         n = min(chunk, nxt - s)
         yield s, n, active
         s += n
+
+
+def timed_plan(wl, K: int, chunk: int):
+    """The launches of the timed pass: (first_step, n, push_active, timed).  K = the whole rollout: every launch is timed
+    (chunks of `chunk` steps).  K below the rollout length (the driver's --steps 20): the K timed steps are spread evenly
+    over the WHOLE rollout -- step round(i N / K), one step per call -- and the steps in between run untimed, so that the
+    figure is the rollout's (settle window, push, collapse, debris), not that of its first K steps of standing towers."""
+    N = wl.n_steps
+    if K >= N:
+        return [(s, n, a, True) for s, n, a in schedule(wl, N, chunk)]
+    picked = sorted({int(i * N / K) for i in range(K)})
+    assert len(picked) == K
+    pset = set(picked)
+    return [(s, 1, a, s in pset) for s, _, a in schedule(wl, picked[-1] + 1, 1)]
 
 
 # ------------------------------------------------------------------------------- oracle arm (CPU)
@@ -240,7 +256,8 @@ def run_cuda(args) -> dict:
     if args.max_pairs:
         wp.max_pairs = args.max_pairs
     K = min(args.steps, wl.n_steps) if args.steps > 0 else wl.n_steps
-    world = binding.World(wp, wl.state, wl.props, wl.mu, device=local, tier=args.tier, group=args.group)
+    # a world that only steps: no pairs / contacts / lambda buffers (2.3 GB at 65,536 envs that nothing would write)
+    world = binding.World(wp, wl.state, wl.props, wl.mu, device=local, tier=args.tier, group=args.group, stage_buffers=False)
     state0 = world.state.clone()
     fext_dev = torch.as_tensor(wl.push_fext).to(dev)
     fext_ptr = binding.C.c_void_p(fext_dev.data_ptr())
@@ -268,34 +285,65 @@ def run_cuda(args) -> dict:
     # ---- roofline denominators measured on this device now (FP32 FFMA issue rate, LDS.128 bandwidth)
     peaks = binding.jenga_measure_peaks(local)
 
-    # ---- device-resident timing: inputs already in HBM, CUDA events on the launching stream
-    launches = list(schedule(wl, K, args.chunk))
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in launches]
+    # ---- device-resident timing: inputs already in HBM, CUDA events on the launching stream.  Two passes over the same
+    # launches: pass 1 is the headline (no per-kernel events, the shipping configuration); pass 2 repeats it with
+    # jenga_profile_* on and gives the per-kernel split for the roofline (its own total is reported as "profiled_ms").
+    launches = timed_plan(wl, K, args.chunk)
+    n_timed = sum(1 for l in launches if l[3])
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for l in launches if l[3]]
     # inputs far larger than L2 (cfg3-5) need no flush; the small configs rewrite a 256 MB buffer between the timed calls
     scratch_per_env = world.scratch.numel() // E
     small = E * (scratch_per_env + 13 * wp.body_stride * 4) < 2 * 126e6
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if small else None
+    ACC = ("env_steps", "body_steps", "candidates", "colliding", "contacts", "contact_iters", "colours", "ground_contacts")
     sampler = ClockSampler(local); sampler.start()
     barrier()
-    world.jenga_profile_enable(True)                         # CUDA events around every kernel launch of the step (same stream)
-    for i, (s, n, active) in enumerate(launches):
+    snaps, k = [], 0
+    for s, n, active, timed in launches:
         set_push(active)
+        if not timed:
+            world.jenga_step(n)
+            continue
         if flush is not None:
             flush.zero_()
-        ev[i][0].record(stream)
+        c0 = world.counters.clone()                          # counters of the timed launches only (device-side copies, no sync)
+        ev[k][0].record(stream)
         world.jenga_step(n)
-        ev[i][1].record(stream)
+        ev[k][1].record(stream)
+        snaps.append((c0, world.counters.clone())); k += 1
     barrier()
     clocks = sampler.stop()
     launch_ms = [a.elapsed_time(b) for a, b in ev]
-    ms = sum(launch_ms)                                      # the timed region = the jenga_step calls (back to back when there is no flush)
-    del flush
-    prof = world.jenga_profile_read()
-    world.jenga_profile_enable(False)
-    cnt = world.counters_dict()
+    ms = sum(launch_ms)                                      # the timed region = the timed jenga_step calls
+    cnt = world.counters_dict()                              # running maxima: of the whole pass
+    acc = sum((b - a for a, b in snaps), torch.zeros_like(world.counters)).tolist()
+    for name in ACC:
+        cnt[name] = int(acc[binding.COUNTER_NAMES.index(name)])
     status_or = int(np.bitwise_or.reduce(world.status.cpu().numpy()))
     n_flagged = int((world.status != 0).sum().item())
     assert cnt["env_steps"] == E * K, (cnt, E, K)
+    # pass 2: the same launches with events around every kernel of the timed ones
+    reset()
+    prof = dict(detect_ms=0.0, manifold_ms=0.0, slot_ms=0.0, collide_ms=0.0, solve_ms=0.0, substeps=0)
+    barrier()
+    for s, n, active, timed in launches:
+        set_push(active)
+        if not timed:
+            world.jenga_step(n)
+            continue
+        if flush is not None:
+            flush.zero_()
+        world.jenga_profile_enable(True)
+        world.jenga_step(n)
+        for key, v in world.jenga_profile_read().items():    # synchronises on this launch's events
+            prof[key] += v
+        world.jenga_profile_enable(False)
+    barrier()
+    del flush
+    first_timed, last_timed = min(l[0] for l in launches if l[3]), max(l[0] + l[1] - 1 for l in launches if l[3])
+    window = (f"all {K} steps of the rollout, {args.chunk} per call" if K >= wl.n_steps else
+              f"{K} timed steps spread over rollout steps {first_timed}..{last_timed} of {wl.n_steps} (every {wl.n_steps / K:.0f}th step, one per call; "
+              f"the steps in between run untimed)")
 
     # ---- end to end through the C-ABI with HOST buffers: every step, for every env, H2D of the state tile (pinned
     # memory), the step, D2H of the result (jenga_step_host).  The batch is served as `--e2e-split` worlds of E/split
@@ -310,7 +358,7 @@ def run_cuda(args) -> dict:
     parts = []
     for lo, hi in bounds:
         wpi = W.WorldParams(**{**wp.__dict__, "n_envs": hi - lo})
-        wi = binding.World(wpi, wl.state[lo:hi], wl.props[lo:hi], wl.mu[lo:hi], device=local, tier=args.tier, group=args.group)
+        wi = binding.World(wpi, wl.state[lo:hi], wl.props[lo:hi], wl.mu[lo:hi], device=local, tier=args.tier, group=args.group, stage_buffers=False)
         h_a = torch.empty(wi.state.shape, dtype=torch.float32, pin_memory=True)
         h_b = torch.empty_like(h_a, pin_memory=True)
         h_a.copy_(torch.as_tensor(wl.state[lo:hi]))
@@ -360,14 +408,21 @@ def run_cuda(args) -> dict:
     achieved = w_solve / solve_s / 1e12
     n_sub = prof["substeps"]
     smem_model = (cnt["contact_iters"] * 96.0) / solve_s / 1e12       # 96 B of body traffic per contact-iteration
-    traffic = None                                           # ncu dram__bytes per env-step (profiles/) x env-steps per launch
+    # traffic is NOT measured by this run: it is the committed ncu figure (dram__bytes_read + write per env-step of one
+    # --set full capture of k_solve at cfg5, profiles/k_solve_traffic.csv) scaled to the env-steps of one launch
+    traffic = traffic_src = step_dram = None
     tpath = os.path.join(ROOT, "profiles", "k_solve_traffic.csv")
     if os.path.exists(tpath):
         import csv
         row = next(csv.DictReader(open(tpath)))
         traffic = float(row["dram_bytes_per_env_step"]) * cnt["env_steps"] / max(n_sub, 1)
+        traffic_src = "profiles/k_solve_traffic.csv (ncu --set full of k_solve at cfg5, not this run) x env-steps per launch"
+        step_dram = float(row["step_dram_bytes_per_env_step"]) if row.get("step_dram_bytes_per_env_step") else None
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinstr/s (FP32 thread-instructions, FMA=1)",
-                "frac": achieved / peak, "traffic": traffic, "kernel": "k_solve", "launch_ms_avg": prof["solve_ms"] / max(n_sub, 1),
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+                "step_dram_bytes_per_env_step": step_dram,            # all six kernels, ncu (profiles/), cfg5
+                "algorithmic_bytes_per_env_step": 25e3,               # state in + out, props, warm-start cache <= 25 KB
+                "kernel": "k_solve", "launch_ms_avg": prof["solve_ms"] / max(n_sub, 1),
                 "launches": n_sub, "share_of_step_time": solve_s / (solve_s + collide_s),
                 "peak_source": f"measured now by jenga_measure_peaks: dependent-free FFMA streams on {peaks['n_sm']} SMs "
                                f"({peaks['fp32_instr_per_s_noreuse'] / 1e12:.2f} T/s when no source register is reused, {peaks['fp32_fma_per_s_packed_noreuse'] / 1e12:.2f} T FMA/s packed f32x2); "
@@ -383,13 +438,16 @@ def run_cuda(args) -> dict:
                                       "k_detect_ms_avg": prof["detect_ms"] / max(n_sub, 1), "k_manifold_ms_avg": prof["manifold_ms"] / max(n_sub, 1),
                                       "k_slot_ms_avg": prof["slot_ms"] / max(n_sub, 1)},
                 "step": {"achieved": wm["total"] / (solve_s + collide_s) / 1e12, "frac": wm["total"] / (solve_s + collide_s) / 1e12 / peak,
-                         "kernel_ms": prof["solve_ms"] + prof["collide_ms"], "wall_ms": sum(launch_ms)}}
+                         "kernel_ms": prof["solve_ms"] + prof["collide_ms"], "wall_ms": sum(launch_ms)},
+                "timing": "value / ms_per_step: pass 1, CUDA events around the timed jenga_step calls, no per-kernel events; "
+                          "kernel times and fractions: pass 2 over the same steps with jenga_profile_* events around every kernel"}
     out = {
         "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world_size, "steps": K, "warmup": args.warmup,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "cfg5 (BASELINE.json configs[4]): 18-level 54-block towers, mu_s {0.25,0.40,0.60} round-robin, 0-12 removals, "
-                               "Ziglar push sweep, dt=1/240, 20 PGS iters, rollout steps 0..K" if args.cfg == CFG else CFG_NAMES[args.cfg] + " (not the headline workload)",
+                               "Ziglar push sweep, dt=1/240, 20 PGS iters" if args.cfg == CFG else CFG_NAMES[args.cfg] + " (not the headline workload)",
+                   "window": window,
                    "envs_per_gpu": E, "n_bodies": wp.n_bodies, "pgs_iters": wp.pgs_iters, "steps_per_call": args.chunk, "kernels_per_substep": 6,
                    "parallelism": f"env-sharded x{world_size}, no data-path collective",
                    "l2": (f"inputs larger than L2: state {E * 13 * wp.body_stride * 4 / 1e6:.0f} MB + scratch {E * linfo_scratch / 1e6:.0f} MB + warm-start cache "
@@ -407,7 +465,7 @@ def run_cuda(args) -> dict:
                      "envs_in_flight_per_sm": linfo["threads"] // 32 * linfo["env_group"]},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke, "steps": Ke,
-                "split": n_split, "launches": e2e_launches},
+                "split": n_split, "launches": e2e_launches, "window": f"rollout steps 0..{Ke - 1}, contiguous (every step's state goes through the host)"},
         "gpu_launches": 6 * n_sub,
         "roofline": roofline,
     }

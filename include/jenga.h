@@ -38,7 +38,7 @@ extern "C" {
 #define JENGA_OK            0
 #define JENGA_E_ARG        -1   /* bad argument: NULL / misaligned pointer, capacity out of range */
 #define JENGA_E_CUDA       -2   /* CUDA error on launch; text via jenga_strerror(JENGA_E_CUDA) */
-#define JENGA_E_DEVICE     -3   /* device is not sm_100 (the kernels are compiled for sm_100a only) */
+#define JENGA_E_DEVICE     -3   /* device is not sm_100 (the kernels are sm_100a only), or desc.device is not the current device */
 
 /* status[env] bit flags */
 #define JENGA_ST_PAIR_OVERFLOW    1u   /* more broadphase candidates than max_pairs          */
@@ -100,7 +100,11 @@ typedef struct {
                                            and so its result, is the canonical one bit for bit whatever the grouping.    */
 } jenga_world_desc;
 
-/* All DEVICE pointers, caller-owned, 16-byte aligned.  PC = max_contacts/4. */
+/* All DEVICE pointers, caller-owned, 16-byte aligned.  PC = max_contacts/4.
+ * pairs, n_pairs, contacts, n_contacts and lambda (the "stage buffers") are only written by jenga_broadphase /
+ * jenga_narrowphase / jenga_pgs_solve and, when desc.materialise = 1, by jenga_step.  A world that only steps with
+ * materialise = 0 may pass all five as NULL (all or none; 36 KB per 54-block env): the three stage calls then return
+ * JENGA_E_ARG on that handle.                                                                            */
 typedef struct {
   float       *state;      /* [E][13][S]  px py pz qw qx qy qz vx vy vz wx wy wz  */
   const float *props;      /* [E][8][S]   inv_m invIx invIy invIz hx hy hz active(0/1); I_body diagonal,

@@ -167,7 +167,9 @@ class World:
     """
 
     def __init__(self, wp, state, props, mu, materialise: bool = False, device: int = 0, collapse_length: float = 0.0,
-                 tier: str = "auto", ref_state=None, group: int = 0):
+                 tier: str = "auto", ref_state=None, group: int = 0, stage_buffers: bool = True):
+        """stage_buffers=False: pairs / contacts / lambda are not allocated (2.3 GB at 65,536 envs); such a world steps
+        (materialise must be off) but refuses jenga_broadphase / jenga_narrowphase / jenga_pgs_solve."""
         if not torch.cuda.is_available():
             raise JengaError("no CUDA device: the Jenga step has no CPU path")
         self.wp = wp
@@ -181,11 +183,14 @@ class World:
         assert self.state.shape == (E, 13, S) and self.props.shape == (E, 8, S) and self.mu.shape == (E,)
         z = lambda shape, dt: torch.zeros(shape, dtype=dt, device=self.dev)
         self.f_ext = None
-        self.pairs = z((E, wp.max_pairs), torch.int32)
-        self.n_pairs = z((E,), torch.int32)
-        self.contacts = z((E, wp.max_contacts, 8), torch.float32)
-        self.n_contacts = z((E,), torch.int32)
-        self.lam = z((E, wp.max_contacts, 3), torch.float32)
+        if stage_buffers:
+            self.pairs = z((E, wp.max_pairs), torch.int32)
+            self.n_pairs = z((E,), torch.int32)
+            self.contacts = z((E, wp.max_contacts, 8), torch.float32)
+            self.n_contacts = z((E,), torch.int32)
+            self.lam = z((E, wp.max_contacts, 3), torch.float32)
+        else:
+            self.pairs = self.n_pairs = self.contacts = self.n_contacts = self.lam = None
         self.cache_key = z((E, pc, 2), torch.int32)
         self.cache_lam = z((E, pc, 4, 3), torch.float32)
         self.cache_pt = z((E, pc, 4, 3), torch.float32)
@@ -200,8 +205,9 @@ class World:
         self.scratch = z((n_scr,), torch.uint8)
         b = Buffers()
         b.state, b.props, b.mu, b.f_ext = self.state.data_ptr(), self.props.data_ptr(), self.mu.data_ptr(), None
-        b.pairs, b.n_pairs = self.pairs.data_ptr(), self.n_pairs.data_ptr()
-        b.contacts, b.n_contacts, b.lambda_ = self.contacts.data_ptr(), self.n_contacts.data_ptr(), self.lam.data_ptr()
+        if stage_buffers:
+            b.pairs, b.n_pairs = self.pairs.data_ptr(), self.n_pairs.data_ptr()
+            b.contacts, b.n_contacts, b.lambda_ = self.contacts.data_ptr(), self.n_contacts.data_ptr(), self.lam.data_ptr()
         b.cache_key, b.cache_lam, b.cache_pt = self.cache_key.data_ptr(), self.cache_lam.data_ptr(), self.cache_pt.data_ptr()
         b.n_cache, b.status, b.counters = self.n_cache.data_ptr(), self.status.data_ptr(), self.counters.data_ptr()
         self.ref_pose = self.collapsed = self.collapse_stats = None

@@ -6,9 +6,9 @@
 //   k_manifold (kcollide.cuh) S3 contact manifolds                                              -> scratch
 //   k_slot    (kcollide.cuh)  S4 effective masses + warm-start lookup                           -> scratch
 //   k_solve   (ksolve.cuh)    S4 warm start, S5 PGS sweeps, S6 integrate, S7 cache, Eq. 18 latch
-// One warp per env in the first three, one warp per group of G envs in k_solve (layout.cuh).  jenga_step(n) enqueues
-// n * n_substeps such quadruples of launches on the caller's stream; nothing returns to the host in between.  The stage
-// entry points run the same device functions in a reduced mode.
+// One warp per env in k_detect, k_plan, k_manifold and k_slot, one thread per env in k_walk, one warp per group of G envs
+// in k_solve (layout.cuh).  jenga_step(n) enqueues n * n_substeps such sextuples of launches on the caller's stream; nothing
+// returns to the host in between.  The stage entry points run the same device functions in a reduced mode.
 #include <cuda_runtime.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -51,8 +51,11 @@ struct jenga_world {
   size_t smem_solve;       // dynamic shared memory per CTA of k_solve
   size_t smem_collide;     // ... of k_detect
   size_t smem_manifold, smem_slot, smem_plan;   // ... of k_manifold, k_slot, k_plan
+  bool stage_bufs;         // pairs / contacts / lambda were given: the stage calls are available
   bool profiling;          // jenga_profile_enable: events around every launch of the step
   std::vector<cudaEvent_t> ev;   // e0 k_detect e1 k_manifold e2 k_slot e3 k_solve e4, per substep
+  std::vector<cudaEvent_t> ev_pool;   // events of earlier reads, reused by the next marks (no create / destroy per substep)
+  bool ev_broken;          // an event could not be created or recorded: the groups of five no longer line up
 };
 
 static thread_local char g_err[512] = "no error";
@@ -196,9 +199,9 @@ static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; 
 
 /* cudaFuncAttributeMaxDynamicSharedMemorySize is per kernel and process-wide: it is only ever raised (running maximum
  * per device), immediately before the launch that needs it, so worlds of different sizes can be used in any order.   */
-enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnPlan, KnWalk, KnSolveTm, KnSolveTm384, KnSolveTm256, KnSolveTm128, KnSolveSm, KnCount };
+enum { KnCollide = 0, KnCollideBroad, KnCollideNarrow, KnCollideGiven, KnManifold, KnManifoldNarrow, KnSlot, KnSlotGiven, KnPlan, KnWalk, KnSolveTm, KnSolveTm384, KnSolveTm256, KnSolveTm128, KnSolveSm, KnSupport, KnCount };
 static std::mutex g_attr_mutex;
-static size_t g_attr_max[16][KnCount];
+static size_t g_attr_max[16][KnCount];   /* bytes already granted; 0 = the 48 KB every kernel has without opting in */
 
 static const void* kernel_ptr(int kn) {
   switch (kn) {
@@ -216,6 +219,7 @@ static const void* kernel_ptr(int kn) {
     case KnSolveTm384: return (const void*)jenga::k_solve<true, 384>;
     case KnSolveTm256: return (const void*)jenga::k_solve<true, 256>;
     case KnSolveTm128: return (const void*)jenga::k_solve<true, 128>;
+    case KnSupport: return (const void*)jenga::k_support;
     default: return (const void*)jenga::k_solve<false, 32>;
   }
 }
@@ -235,11 +239,18 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   if (!out) return JENGA_E_ARG;
   *out = nullptr;
   if (!desc_ok(d) || !b) return JENGA_E_ARG;
-  if (!aligned16(b->state) || !aligned16(b->props) || !b->mu || !aligned16(b->pairs) || !b->n_pairs ||
-      !aligned16(b->contacts) || !b->n_contacts || !b->lambda || !b->cache_key || !aligned16(b->cache_lam) || !aligned16(b->cache_pt) ||
+  if (!aligned16(b->state) || !aligned16(b->props) || !b->mu || !b->cache_key || !aligned16(b->cache_lam) || !aligned16(b->cache_pt) ||
       !b->n_cache || !b->status || !aligned16(b->scratch))
     return JENGA_E_ARG;
+  /* the stage buffers (pairs .. lambda) are written by the stage calls and by jenga_step only with materialise = 1: a world
+     that only steps may leave all five NULL (all or none) and then refuses the stage calls */
+  const bool any_stage = b->pairs || b->n_pairs || b->contacts || b->n_contacts || b->lambda;
+  const bool all_stage = aligned16(b->pairs) && b->n_pairs && aligned16(b->contacts) && b->n_contacts && b->lambda;
+  if ((any_stage || d->materialise) && !all_stage) return JENGA_E_ARG;
   if (b->f_ext && !aligned16(b->f_ext)) return JENGA_E_ARG;
+  if (d->collapse_length > 0.0f && b->ref_pose && b->collapsed &&      /* latch on: ref_pose rows and the float4 stats */
+      (!aligned16(b->ref_pose) || (b->collapse_stats && !aligned16(b->collapse_stats))))
+    return JENGA_E_ARG;
   if (b->scratch_bytes < jenga_scratch_bytes(d)) return JENGA_E_ARG;
   const int G = pick_group(d);
   if (G < 0) return JENGA_E_ARG;
@@ -255,7 +266,8 @@ extern "C" int jenga_world_create(const jenga_world_desc* d, const jenga_buffers
   if (prop.major != 10) return JENGA_E_DEVICE;
   jenga_world* w = new (std::nothrow) jenga_world();
   if (!w) return JENGA_E_ARG;
-  w->profiling = false;
+  w->profiling = false; w->ev_broken = false;
+  w->stage_bufs = all_stage;
   w->desc = *d; w->bufs = *b; w->tmb = tmb; w->G = G; w->n_sm = prop.multiProcessorCount;
   w->smem_solve = solve_cta_bytes(d, tmb, G);
   const size_t cb = collide_env_bytes(d, G);
@@ -295,14 +307,29 @@ static int launched(const char* name) {
   return e == cudaSuccess ? JENGA_OK : cuda_fail(e, name);
 }
 
-static void drop_events(jenga_world* w) {
-  for (cudaEvent_t e : w->ev) cudaEventDestroy(e);
+/* Every launch goes to the CURRENT device with pointers that belong to desc.device: on any other device the kernels would
+ * fault on foreign addresses (a sticky error that ends the context), and the shared-memory opt-in below would be recorded
+ * for the wrong device.  Checked at the top of every call that launches or copies. */
+static int on_device(const jenga_world* w) {
+  int cur = -1;
+  const cudaError_t e = cudaGetDevice(&cur);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+  return cur == w->desc.device ? JENGA_OK : JENGA_E_DEVICE;
+}
+
+/* recorded events go back to the pool for the next marks; `destroy` (jenga_world_destroy) frees them all */
+static void drop_events(jenga_world* w, bool destroy = false) {
+  for (cudaEvent_t e : w->ev) w->ev_pool.push_back(e);
   w->ev.clear();
+  w->ev_broken = false;
+  if (!destroy) return;
+  for (cudaEvent_t e : w->ev_pool) cudaEventDestroy(e);
+  w->ev_pool.clear();
 }
 
 extern "C" int jenga_world_destroy(jenga_world* w) {
   if (!w) return JENGA_E_ARG;
-  drop_events(w);
+  drop_events(w, true);
   delete w;
   return JENGA_OK;
 }
@@ -316,11 +343,21 @@ extern "C" int jenga_profile_enable(jenga_world* w, int on) {
 
 extern "C" int jenga_profile_read(jenga_world* w, double* out) {
   if (!w || !out) return JENGA_E_ARG;
+  /* five marks per substep, recorded by step_launches only; a mark that failed would shift every later group */
+  if (w->ev_broken || w->ev.size() % 5 != 0) {
+    drop_events(w);
+    return cuda_fail(cudaErrorUnknown, "jenga_profile_read (an event of this interval could not be created or recorded)");
+  }
   double ms[4] = { 0.0, 0.0, 0.0, 0.0 }; const size_t n = w->ev.size() / 5;
   for (size_t i = 0; i < n; ++i) {
     cudaError_t e = cudaEventSynchronize(w->ev[5 * i + 4]);
     if (e != cudaSuccess) return cuda_fail(e, "jenga_profile_read");
-    for (int k = 0; k < 4; ++k) { float t = 0.0f; cudaEventElapsedTime(&t, w->ev[5 * i + k], w->ev[5 * i + k + 1]); ms[k] += t; }
+    for (int k = 0; k < 4; ++k) {
+      float t = 0.0f;
+      e = cudaEventElapsedTime(&t, w->ev[5 * i + k], w->ev[5 * i + k + 1]);
+      if (e != cudaSuccess) { drop_events(w); return cuda_fail(e, "jenga_profile_read (cudaEventElapsedTime)"); }
+      ms[k] += t;
+    }
   }
   for (int k = 0; k < 4; ++k) out[k] = ms[k];
   out[4] = (double)n;
@@ -338,13 +375,16 @@ extern "C" int jenga_set_f_ext(jenga_world* w, const float* f_ext) {
 static void mark(jenga_world* w, cudaStream_t st) {
   if (!w->profiling) return;
   cudaEvent_t e;
-  if (cudaEventCreate(&e) != cudaSuccess) return;
-  cudaEventRecord(e, st);
+  if (!w->ev_pool.empty()) { e = w->ev_pool.back(); w->ev_pool.pop_back(); }
+  else if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); w->ev_broken = true; return; }
+  if (cudaEventRecord(e, st) != cudaSuccess) { cudaGetLastError(); w->ev_broken = true; }
   w->ev.push_back(e);
 }
 
 /* k_detect, then (except for jenga_broadphase) k_walk, k_plan, k_manifold and k_slot, for every env */
 static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_t st) {
+  int rc = on_device(w);
+  if (rc != JENGA_OK) return rc;
   cudaError_t e = ensure_smem(w->desc.device, KnCollide + mode, w->smem_collide);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_detect)");
   const int wpc = w->wpc_collide, grid = (w->P.E + wpc - 1) / wpc, thr = 32 * wpc;
@@ -354,7 +394,7 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
     case jenga::ModeNarrow: jenga::k_detect<jenga::ModeNarrow><<<grid, thr, w->smem_collide, st>>>(w->P, honour_rest); break;
     default: jenga::k_detect<jenga::ModeGiven><<<grid, thr, w->smem_collide, st>>>(w->P, honour_rest); break;
   }
-  int rc = launched("k_detect");
+  rc = launched("k_detect");
   if (rc != JENGA_OK || mode == jenga::ModeBroad) return rc;
   const size_t smem_walk = (size_t)jenga::kWalkThreads * w->P.B * sizeof(unsigned long long);
   e = ensure_smem(w->desc.device, KnWalk, smem_walk);
@@ -367,7 +407,7 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
   jenga::k_plan<<<grid, thr, w->smem_plan, st>>>(w->P);
   rc = launched("k_plan");
   if (rc != JENGA_OK) return rc;
-  mark(w, st);
+  if (mode == jenga::ModeStep) mark(w, st);
   if (mode != jenga::ModeGiven) {                           /* manifolds (jenga_pgs_solve: the caller's contacts instead) */
     const int kn = mode == jenga::ModeStep ? KnManifold : KnManifoldNarrow;
     e = ensure_smem(w->desc.device, kn, w->smem_manifold);
@@ -377,7 +417,7 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
     rc = launched("k_manifold");
     if (rc != JENGA_OK || mode == jenga::ModeNarrow) return rc;
   }
-  mark(w, st);
+  if (mode == jenga::ModeStep) mark(w, st);
   e = ensure_smem(w->desc.device, mode == jenga::ModeStep ? KnSlot : KnSlotGiven, w->smem_slot);
   if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_slot)");
   if (mode == jenga::ModeStep) jenga::k_slot<jenga::ModeStep><<<grid, thr, w->smem_slot, st>>>(w->P, honour_rest);
@@ -386,6 +426,8 @@ static int launch_collide(jenga_world* w, int mode, int honour_rest, cudaStream_
 }
 
 static int launch_solve(jenga_world* w, int iters, int flags, float rest_ek, cudaStream_t st) {
+  const int dev_rc = on_device(w);
+  if (dev_rc != JENGA_OK) return dev_rc;
   const int q = tier_groups(w->tmb);
   const int kn = !w->tmb ? KnSolveSm : (q == 4 ? KnSolveTm : (q == 3 ? KnSolveTm384 : (q == 2 ? KnSolveTm256 : KnSolveTm128)));
   const cudaError_t e = ensure_smem(w->desc.device, kn, w->smem_solve);
@@ -409,17 +451,17 @@ static int launch_solve(jenga_world* w, int iters, int flags, float rest_ek, cud
 }
 
 extern "C" int jenga_broadphase(jenga_world* w, void* stream) {
-  if (!w) return JENGA_E_ARG;
+  if (!w || !w->stage_bufs) return JENGA_E_ARG;
   return launch_collide(w, jenga::ModeBroad, 0, (cudaStream_t)stream);
 }
 
 extern "C" int jenga_narrowphase(jenga_world* w, void* stream) {
-  if (!w) return JENGA_E_ARG;
+  if (!w || !w->stage_bufs) return JENGA_E_ARG;
   return launch_collide(w, jenga::ModeNarrow, 0, (cudaStream_t)stream);
 }
 
 extern "C" int jenga_pgs_solve(jenga_world* w, int iters, void* stream) {
-  if (!w || iters < 0) return JENGA_E_ARG;
+  if (!w || iters < 0 || !w->stage_bufs) return JENGA_E_ARG;
   const int rc = launch_collide(w, jenga::ModeGiven, 0, (cudaStream_t)stream);
   if (rc != JENGA_OK) return rc;
   return launch_solve(w, iters > 0 ? iters : w->P.iters, jenga::SolvePgsOnly, 0.0f, (cudaStream_t)stream);
@@ -448,6 +490,8 @@ extern "C" int jenga_step(jenga_world* w, int n_steps, void* stream) {
 
 extern "C" int jenga_simulate_until_rest(jenga_world* w, int max_steps, float ek_rest, void* stream) {
   if (!w || max_steps <= 0 || max_steps > (1 << 20) || !(ek_rest > 0.0f)) return JENGA_E_ARG;
+  const int dev_rc = on_device(w);
+  if (dev_rc != JENGA_OK) return dev_rc;
   jenga::k_reset_rest<<<(w->P.E + 255) / 256, 256, 0, (cudaStream_t)stream>>>(w->P);
   const int rc = launched("k_reset_rest");
   if (rc != JENGA_OK) return rc;
@@ -456,6 +500,8 @@ extern "C" int jenga_simulate_until_rest(jenga_world* w, int max_steps, float ek
 
 extern "C" int jenga_step_host(jenga_world* w, const float* h_in, float* h_out, int n_steps, void* stream) {
   if (!w || n_steps < 0) return JENGA_E_ARG;
+  const int dev_rc = on_device(w);
+  if (dev_rc != JENGA_OK) return dev_rc;
   const size_t bytes = (size_t)w->P.E * jenga::kStateRows * w->P.S * sizeof(float);
   cudaStream_t st = (cudaStream_t)stream;
   if (h_in) {
@@ -473,9 +519,11 @@ extern "C" int jenga_step_host(jenga_world* w, const float* h_in, float* h_out, 
 
 extern "C" int jenga_support_margin(jenga_world* w, float* out, void* stream) {
   if (!w || !aligned16(out)) return JENGA_E_ARG;
+  const int dev_rc = on_device(w);
+  if (dev_rc != JENGA_OK) return dev_rc;
   const size_t smem = (size_t)8 * w->P.S * sizeof(float2);
   if (smem > 48 * 1024) {
-    const cudaError_t e = cudaFuncSetAttribute((const void*)jenga::k_support, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const cudaError_t e = ensure_smem(w->desc.device, KnSupport, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_support)");
   }
   jenga::k_support<<<w->P.E, 32, smem, (cudaStream_t)stream>>>(w->P, reinterpret_cast<float4*>(out));
@@ -484,6 +532,8 @@ extern "C" int jenga_support_margin(jenga_world* w, float* out, void* stream) {
 
 extern "C" int jenga_ziglar_block_analysis(jenga_world* w, const int32_t* block, const int32_t* axis, float* out, void* stream) {
   if (!w || !block || !axis || !aligned16(out)) return JENGA_E_ARG;
+  const int dev_rc = on_device(w);
+  if (dev_rc != JENGA_OK) return dev_rc;
   jenga::k_ziglar<<<(w->P.E + 127) / 128, 128, 0, (cudaStream_t)stream>>>(w->P, block, axis, reinterpret_cast<float4*>(out));
   return launched("k_ziglar");
 }

@@ -650,11 +650,15 @@ __device__ inline void publish_pairs(const CSm& s, const Params& P, int env, flo
   int* meta = reinterpret_cast<int*>(scr + L.meta);
   unsigned short* gpair = reinterpret_cast<unsigned short*>(scr + L.cpair);
   unsigned* gcab = reinterpret_cast<unsigned*>(scr + L.cab);
-  for (int r = lane; r < n_coll; r += 32) gcab[r] = s.cab[r];
+  // The colouring is a function of the pair indices AND of which bodies are dynamic (two pairs that share only a pinned
+  // body may share a colour): props is the caller's and may change between calls with the pair list unchanged, so the
+  // dynamic bits of the stored words are part of the comparison (the SAT axis bits are not: they do not colour anything).
+  constexpr unsigned kDynBits = (1u << 11) | (1u << 27);
   bool same = meta[MetaMagic] == kMagic && meta[MetaNcoll] == n_coll;
   if (same)
-    for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]);
+    for (int r = lane; r < n_coll; r += 32) same = same && (s.cpair[r] == gpair[r]) && (((s.cab[r] ^ gcab[r]) & kDynBits) == 0u);
   same = __all_sync(kFull, same);
+  for (int r = lane; r < n_coll; r += 32) gcab[r] = s.cab[r];
   if (!same) for (int r = lane; r < n_coll; r += 32) gpair[r] = s.cpair[r];
   if (lane == 0) {
     P.same_flag[env] = same ? 1 : 0;

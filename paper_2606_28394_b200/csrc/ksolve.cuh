@@ -1,4 +1,4 @@
-// ksolve.cuh -- fourth kernel of a substep, one GROUP of G envs per warp (layout.cuh): S4 warm-start application, S5
+// ksolve.cuh -- sixth and last kernel of a substep, one GROUP of G envs per warp (layout.cuh): S4 warm-start application, S5
 // coloured PGS sweeps, S6 integration + Baumgarte, S7 warm-start cache, Eq. 18 latch.  Inputs: the state tiles of the
 // group's envs and the blocks + chunk list k_detect / k_slot left in the scratch of the group's first env.
 //

@@ -32,7 +32,7 @@ namespace jenga {
 
 constexpr int kStateRows = 13, kPropRows = 8, kFextRows = 6;
 constexpr int kMaxColours = 64;
-constexpr int kBd = 20;        // solver body record (floats): x y z im | vx vy vz - | wx wy wz - | Ixx Ixy Ixz Iyy | Iyz Izz - -
+constexpr int kBd = 20;        // solver body record (floats): x y z im | vx vy vz Ixx | wx wy wz Ixy | Ixz Iyy Iyz Izz | qw qx qy qz   (ksolve.cuh load_bodies)
 constexpr int kCb = 28;        // collision body record of k_slot: x y z im | a0.xyz h0 | a1.xyz h1 | a2.xyz h2 | Ixx Ixy Ixz Iyy | Iyz Izz - - | pad 4 (k_detect, k_manifold: 20 words, kcollide.cuh)
 constexpr int kCsF4 = 14;      // float4 per pair: 36 read-only words + 12 impulses + 8 header words (kcollide.cuh PairC)
 constexpr int kTmCols = 4 * kCsF4;          // tensor-memory columns of one block

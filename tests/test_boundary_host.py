@@ -75,6 +75,37 @@ def test_descriptor_validation_and_launch_shape(L):
     assert b"bad argument" in L.jenga_strerror(-1) and L.jenga_strerror(0) == b"ok"
 
 
+def test_stage_buffers_are_optional_for_a_world_that_only_steps(L):
+    """pairs / n_pairs / contacts / n_contacts / lambda: all five or none, and none only with materialise = 0.  The checks
+    run before the first CUDA call, so without a device a descriptor that passes them fails later (not with -1); with a
+    device it gives a handle (no kernel is launched by create / destroy)."""
+    from paper_2606_28394_b200 import binding, workloads as W
+    wp = W.make_config(2, n_envs=2).params
+
+    def create(materialise, stage, **override):
+        d = binding.make_desc(wp, materialise=materialise)
+        b = binding.Buffers()
+        names = ["state", "props", "mu", "cache_key", "cache_lam", "cache_pt", "n_cache", "status", "scratch"]
+        names += stage
+        for k, n in enumerate(names):
+            setattr(b, n, 4096 * (k + 1))                      # aligned, never dereferenced on the host
+        for n, v in override.items():
+            setattr(b, n, v)
+        b.scratch_bytes = L.jenga_scratch_bytes(C.byref(d))
+        h = C.c_void_p()
+        rc = L.jenga_world_create(C.byref(d), C.byref(b), C.byref(h))
+        if rc == 0:
+            L.jenga_world_destroy(h)
+        return rc
+
+    all_five = ["pairs", "n_pairs", "contacts", "n_contacts", "lambda_"]
+    assert create(False, all_five) != -1 and create(True, all_five) != -1 and create(False, []) != -1
+    assert create(True, []) == -1                              # materialise writes them
+    assert create(False, ["pairs", "n_pairs"]) == -1           # some but not all
+    assert create(False, all_five, contacts=4096 + 4) == -1    # misaligned
+    assert create(False, [], state=None) == -1
+
+
 def test_python_struct_matches_c_layout():
     """sizeof / field order of the ctypes mirror vs the header, via a tiny C program."""
     from paper_2606_28394_b200 import binding

@@ -428,6 +428,80 @@ def test_kept_colouring_and_plan_equal_a_fresh_one(J):
     assert int(a.status.max().item()) == 0
 
 
+@pytest.mark.parametrize("unpin_first", [True, False])
+def test_kept_colouring_sees_a_body_becoming_dynamic_or_pinned(J, unpin_first):
+    """props is the caller's buffer and may be edited between calls.  Pinning (inv_m = 0) or releasing a body leaves the
+    colliding-pair list of a standing tower as it was, but not its colouring: pairs that share only a pinned body may share
+    a colour, pairs that share a dynamic one may not (they would update the same body record in one visit).  The kept
+    colouring must therefore be dropped when a body's dynamic flag changes: the stepping world continues exactly like a
+    world created from its state, cache and the edited props."""
+    import torch
+    wl = W.make_config(2, n_envs=5)
+    body = 3 * 7 + 1                                      # the centre block of level 7: three pairs below it, three above
+    pinned = wl.props.copy()
+    pinned[:, 0:4, body] = 0.0                            # inv_m and inv_I: a static body
+    first, second = (pinned, wl.props) if unpin_first else (wl.props, pinned)
+    a = J.World(wl.params, wl.state, first, wl.mu, tier="tmem160", group=2)
+    a.step(6); torch.cuda.synchronize()
+    a.props.copy_(torch.as_tensor(second).to(a.dev))      # the edit: same poses, same pair list, other dynamic flags
+    b = J.World(wl.params, a.state.cpu().numpy(), second, wl.mu, tier="tmem160", group=2)
+    for name in ("cache_key", "cache_lam", "cache_pt", "n_cache"):
+        getattr(b, name).copy_(getattr(a, name))
+    flags = a.scratch.view(torch.int32)[64:64 + 5]
+    for k in range(4):
+        a.step(1); b.step(1); torch.cuda.synchronize()
+        if k == 0:
+            assert int((flags == 0).sum().item()) == 5    # every env re-coloured although no pair index changed
+        assert torch.equal(a.state, b.state) and torch.equal(a.cache_lam, b.cache_lam), f"step {k} after the edit"
+    assert int(a.status.max().item()) == 0
+    a.destroy(); b.destroy()
+
+
+def test_world_without_stage_buffers_steps_and_refuses_stage_calls(J):
+    """jenga_buffers: a world that only steps (materialise = 0) may leave pairs / contacts / lambda NULL.  It steps to the
+    same bits as a world that has them; the three stage calls answer JENGA_E_ARG on it."""
+    import ctypes as C
+    import torch
+    wl = W.make_config(2, n_envs=6)
+    a = J.World(wl.params, wl.state, wl.props, wl.mu)
+    b = J.World(wl.params, wl.state, wl.props, wl.mu, stage_buffers=False)
+    a.step(5); b.step(5); torch.cuda.synchronize()
+    assert torch.equal(a.state, b.state) and torch.equal(a.cache_lam, b.cache_lam)
+    L, st = J.lib(), C.c_void_p(torch.cuda.current_stream(b.dev).cuda_stream)
+    assert L.jenga_broadphase(b.handle, st) == -1 and L.jenga_narrowphase(b.handle, st) == -1 and L.jenga_pgs_solve(b.handle, 0, st) == -1
+    with pytest.raises(J.JengaError):
+        J.World(wl.params, wl.state, wl.props, wl.mu, materialise=True, stage_buffers=False)
+    a.destroy(); b.destroy()
+
+
+def test_calls_on_another_device_are_refused(J):
+    """include/jenga.h: desc.device must be the current device in every call on the handle.  A launch from another device
+    would hand that device's kernels foreign pointers (a sticky fault); every launching call answers JENGA_E_DEVICE (-3)
+    instead, launches nothing, and the handle keeps working once the right device is current again."""
+    import ctypes as C
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    wl = W.make_config(1)
+    world = J.World(wl.params, wl.state, wl.props, wl.mu, device=0)
+    L, st0 = J.lib(), world.state.clone()
+    out = torch.empty((1, 4), dtype=torch.float32, device=world.dev)
+    with torch.cuda.device(1):
+        stream = C.c_void_p(torch.cuda.current_stream(torch.device("cuda", 1)).cuda_stream)
+        assert L.jenga_step(world.handle, 1, stream) == -3
+        assert L.jenga_broadphase(world.handle, stream) == -3 and L.jenga_narrowphase(world.handle, stream) == -3
+        assert L.jenga_pgs_solve(world.handle, 0, stream) == -3
+        assert L.jenga_simulate_until_rest(world.handle, 2, C.c_float(1e-7), stream) == -3
+        assert L.jenga_step_host(world.handle, None, None, 1, stream) == -3
+        assert L.jenga_support_margin(world.handle, C.c_void_p(out.data_ptr()), stream) == -3
+        torch.cuda.synchronize()
+    torch.cuda.synchronize()
+    assert torch.equal(world.state, st0)
+    world.step(1); torch.cuda.synchronize()
+    assert not torch.equal(world.state, st0)
+    world.destroy()
+
+
 # ----------------------------------------------------------------------------- rollouts
 def collapse_flags(state, state0, props, B, length=W.BLOCK_L):
     """Eq. 18 (reading A17) on [E][13][S] tiles, restated in NumPy for the harness:
@@ -544,6 +618,16 @@ def test_rollout_agreement_on_decided_episodes(orc, J, cfg, E):
     print(f"\n[rollout cfg{cfg}] {E} episodes, {int(r['far'].sum())} far from the threshold, of those {nd and int(r['decided'][r['far']].sum())} decided "
           f"({pd:.3f} +- {sd:.3f}); CUDA vs oracle on the decided far episodes: {p:.4f} +- {sig:.4f} (n = {n})")
     assert n > 0.8 * r["far"].sum() and p >= 0.99
+    # and a hard floor on the RAW figure (every far episode, decided or not): not below what the fp64 oracle reaches against
+    # itself from inputs moved by <= 1e-7 m, less one point.  north_star's absolute 0.99 stays the xfail at the end of the file.
+    raw, _, _ = rate(agree[r["far"]])
+    self_rates = [rate((q == r["ref"])[r["far"]])[0] for q in r["pert"]]
+    assert raw >= min(self_rates) - 0.01, f"raw agreement {raw:.4f} fell below the oracle's own noise floor {min(self_rates):.4f} - 0.01"
+
+
+def flips(a, ref, far):
+    """(stands -> collapses, collapses -> stands) among the far episodes, `ref` being the fp64 oracle's answer"""
+    return int((a & ~ref & far).sum()), int((~a & ref & far).sum())
 
 
 def load_cache(world, cache):
@@ -991,4 +1075,13 @@ def test_rollout_agreement_north_star(orc, J, cfg, E):
     print(f"\n[rollout cfg{cfg}] north_star figure: CUDA vs oracle on the {n} far episodes {p:.4f} +- {sig:.4f} (all {E}: {pa:.4f}); "
           f"oracle collapses {int(r['ref'][far].sum())}, CUDA {int(r['cuda'][far].sum())}; "
           f"oracle vs oracle moved by <= 1e-7 m ({N_PERTURBED} seeds): {min(self_rates):.4f} .. {max(self_rates):.4f}")
+    # direction of the disagreements (is fp32 biased towards collapse, or is it the oracle's own chaos?)
+    up, down = flips(r["cuda"], r["ref"], far)
+    print(f"  flips vs the oracle, stands->collapses / collapses->stands: CUDA {up} / {down}; perturbed oracles "
+          + ", ".join("%d / %d" % flips(q, r["ref"], far) for q in r["pert"]))
+    mu = r["wl"].mu
+    for m in np.unique(mu):
+        sel = far & (mu == m)
+        print(f"    mu_s {m:.2f}: {int(sel.sum())} far episodes, CUDA flips {flips(r['cuda'], r['ref'], sel)}, perturbed oracles "
+              + ", ".join("%d / %d" % flips(q, r["ref"], sel) for q in r["pert"]))
     assert p >= 0.99
