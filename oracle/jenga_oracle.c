@@ -20,6 +20,10 @@
  *   orc_solve            P7  single contact closed form, active-set LCP enumeration,
  *                            in-colour permutation invariance, KE monotone
  *   whole step           P8  incline stick/slip, P9 Ziglar rigs, P10 resting tower drift
+ *   substep details      Eq. 16 above the slop (rise = beta (delta - slop); inverse-mass split, once per pair),
+ *                        Eq. 14 with e > 0 ((-e)^k v_n after k iterations), external torque (n h tau / I_xx about a
+ *                        principal axis; R diag(1/I) R^T tau in general), gyroscopic = 1 (first-step closed form,
+ *                        angular momentum conserved), KE never rising in a row update: tests/test_oracle_pins_r3.py
  *   PARITY UNPINNED by anything in the paper (fixed by SURVEY §8(c) / DESIGN.md only):
  *   the >4-point reduction rule, the face-preference and tie constants, the tangent-basis
  *   rule, the warm-start match rule, the load split in statically indeterminate stacks.

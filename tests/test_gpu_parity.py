@@ -95,8 +95,6 @@ def test_broadphase_bit_exact(orc, J, steps):
     """Pair lists bit-exact, no exclusions (north_star), on step-0 and mid-rollout states."""
     import torch
     for name, wl, _ in workloads_small() + [("cfg3b", W.make_config(3, n_envs=3, env_offset=100), 0)]:
-        if steps and name == "cfg4":
-            continue
         state = wl.state if steps == 0 else oracle_mid_state(orc, wl, steps if name != "cfg3b" else 260)[0]
         world = J.World(wl.params, state, wl.props, wl.mu)
         world.broadphase(); torch.cuda.synchronize()
@@ -184,7 +182,7 @@ def compare_contacts(orc, world, P, bod, e, pairs, stats):
 
 
 @pytest.mark.parametrize("name,cfg,E,steps", [("cfg1", 1, 1, 30), ("cfg2", 2, 6, 40), ("cfg3", 3, 4, 200), ("cfg3late", 3, 3, 420),
-                                              ("cfg4", 4, 2, 20), ("cfg6", 6, 6, 30)])
+                                              ("cfg4", 4, 2, 20), ("cfg4late", 4, 8, 110), ("cfg6", 6, 6, 30)])
 def test_narrowphase_matches_oracle(orc, J, name, cfg, E, steps):
     import torch
     wl = W.make_config(cfg, n_envs=E)
@@ -295,7 +293,7 @@ def test_pgs_matches_oracle(orc, J, name, cfg, E, steps, warm, tier):
 
 # ----------------------------------------------------------------------------- whole step
 @pytest.mark.parametrize("name,cfg,E,steps", [("cfg1", 1, 1, 20), ("cfg2", 2, 6, 60), ("cfg3", 3, 4, 250), ("cfg4", 4, 2, 10), ("cfg6", 6, 6, 20),
-                                              ("cfg6push", 6, 6, 70)])
+                                              ("cfg6push", 6, 6, 70), ("cfg4late", 4, 8, 110)])
 def test_single_step_pose(orc, J, name, cfg, E, steps):
     """One fused jenga_step from a common fp32 state and warm-start cache vs one oracle step.  The 54-block configs run
     the headline launch shape (two envs per solver warp, tensor-memory tier), the others what auto gives them."""
@@ -317,11 +315,25 @@ def test_single_step_pose(orc, J, name, cfg, E, steps):
     f64 = orc.unpack_fext(fext, wl.params.n_bodies)
     g = world.state.cpu().numpy().astype(np.float64)
     n_ok = 0
+    bod0 = bod.copy()                                            # the poses both narrowphases saw (S1 changes velocities only)
     for e in range(E):
         tr = orc.step_env(P, bod, float(wl.mu[e]), e=e, fext=f64, cache=cache, trace=True)
         B = wl.params.n_bodies
         if int(world.n_contacts[e].item()) != tr["contacts"].n:
-            assert near_threshold(tr["margins"]), (name, e, tr["margins"])   # a manifold decision sat on its threshold
+            # excused only if a pair whose contacts DIFFER has a discrete decision on its threshold (its own margins)
+            gc = gpu_contacts(world, e); rc = tr["contacts"].trimmed()
+            got_pairs = world.pairs[e, :int(world.n_pairs[e].item())].cpu().numpy()[gc["cand"]]
+            differing = [int(p) for p in np.union1d(np.unique(rc["pair"]), np.unique(got_pairs))
+                         if (rc["pair"] == p).sum() != (got_pairs == p).sum()]
+            assert differing
+            for p in differing:
+                i, j = orc.pair_bodies(B, p)
+                pm = orc.OrcMargins(); pm.reset()
+                if i < 0:
+                    orc.collide_ground(bod0.x[e, j], bod0.q[e, j], bod0.he[e, j], margins=pm)
+                else:
+                    orc.collide_boxes(P, bod0.x[e, i], bod0.q[e, i], bod0.he[e, i], bod0.x[e, j], bod0.q[e, j], bod0.he[e, j], margins=pm)
+                assert near_threshold(pm.as_dict()), (name, e, p, pm.as_dict())
             continue
         n_ok += 1
         assert int(world.n_pairs[e].item()) == len(tr["pairs"])
@@ -334,7 +346,73 @@ def test_single_step_pose(orc, J, name, cfg, E, steps):
         assert np.max(ang) < TOL_ANG, f"{name} env {e}: orientation error {ang.max():.3e} rad"
         assert int(world.status[e].item()) == tr["status"]
     print(f"\n[{name}] single-step pose parity on {n_ok}/{E} envs (rest: a contact-count decision on its threshold)")
-    assert n_ok >= max(1, (3 * E) // 4)
+    assert n_ok >= (int(0.9 * E) if E >= 6 else max(1, E - 1))    # at least 90 % of the envs compared (whole envs)
+
+
+def test_single_step_gyroscopic_and_deep_contacts(orc, J):
+    """The parts of the step that the configs leave idle, on a tower: every level interface overlaps by
+    0.7 mm > slop (Eq. 16 moves every block), the bodies spin (the gyroscopic term of Eq. 4 acts, gyroscopic = 1), a
+    world torque and a force load a few blocks (the torque rows of f_ext), and e = 0.1.  One step against the oracle at
+    north_star's pose tolerance, plus the velocities; and the oracle itself moves by far more than the tolerance when the
+    gyroscopic term, the torque or the deep-contact correction is taken away, so agreeing means having them."""
+    import torch
+    E = 6
+    wl = W.make_config(2, n_envs=E)
+    wl.params.gyroscopic = 1
+    wl.params.restitution = float(np.float32(0.1))
+    B, S = wl.params.n_bodies, wl.params.body_stride
+    rng = np.random.default_rng(31)
+    state = wl.state.copy()
+    level = np.arange(B) // 3
+    state[:, 2, :B] -= np.float32(0.6e-3) * (level + 1)               # 0.1 mm initial overlap + 0.6 mm per interface
+    state[:, 10:13, :B] = rng.uniform(-6.0, 6.0, (E, 3, B)).astype(np.float32)
+    fext = np.zeros((E, 6, S), np.float32)
+    top = B - 3 + np.arange(3)
+    fext[:, 3:6, top] = rng.uniform(-2e-3, 2e-3, (E, 3, 3)).astype(np.float32)      # N m on the top level
+    fext[:, 0, top] = 0.05
+    world = J.World(wl.params, state, wl.props, wl.mu, materialise=True, tier="tmem160", group=2)
+    world.set_f_ext(fext)
+    world.step(1); torch.cuda.synchronize()
+    g = world.state.cpu().numpy().astype(np.float64)
+    f64 = orc.unpack_fext(fext, B)
+
+    def oracle_step(gyro=1, torque=True, slop=None):
+        wp = W.WorldParams(**{**wl.params.__dict__, "gyroscopic": gyro})
+        if slop is not None:
+            wp.slop = slop
+        P = orc.make_params(wp); bod = orc.unpack_tiles(state, wl.props, B)
+        f = f64.copy()
+        if not torque:
+            f[:, :, 3:6] = 0.0
+        traces = [orc.step_env(P, bod, float(wl.mu[e]), e=e, fext=f, trace=True) for e in range(E)]
+        return bod, traces
+
+    bod, traces = oracle_step()
+    deep = n_ok = 0
+    for e in range(E):
+        tr = traces[e]
+        if int(world.n_contacts[e].item()) != tr["contacts"].n:
+            assert near_threshold(tr["margins"]), (e, tr["margins"])           # a manifold decision sat on its threshold
+            continue
+        n_ok += 1
+        assert int(world.status[e].item()) == tr["status"]
+        deep += int((tr["contacts"].trimmed()["depth"] > wl.params.slop).sum())
+        act = wl.props[e, 7, :B] != 0
+        x = np.transpose(g[e, 0:3, :B]); q = np.transpose(g[e, 3:7, :B])
+        v = np.transpose(g[e, 7:10, :B]); w = np.transpose(g[e, 10:13, :B])
+        assert np.max(np.abs(x - bod.x[e])[act]) < TOL_POS, f"env {e}: position error {np.max(np.abs(x - bod.x[e])[act]):.3e}"
+        assert np.max(rotation_angle(q, bod.q[e])[act]) < TOL_ANG
+        assert np.max(np.abs(v - bod.v[e])[act]) < 2e-5 and np.max(np.abs(w - bod.w[e])[act]) < 2e-3, \
+            (np.max(np.abs(v - bod.v[e])[act]), np.max(np.abs(w - bod.w[e])[act]))
+    assert n_ok >= 5 and deep > 100 * n_ok                                      # the Baumgarte branch ran on every interface
+    # what the oracle does without each part: far outside the tolerances above
+    no_gyro, _ = oracle_step(gyro=0)
+    no_tau, _ = oracle_step(torque=False)
+    no_push, _ = oracle_step(slop=1.0)                                          # slop above every depth: Eq. 16 idle
+    ang = lambda a, b: max(np.max(rotation_angle(a.q[e], b.q[e])) for e in range(E))
+    assert ang(no_gyro, bod) > 10 * TOL_ANG and ang(no_tau, bod) > 100 * TOL_ANG
+    assert np.max(np.abs(no_push.x - bod.x)) > 100 * TOL_POS
+    world.destroy()
 
 
 @pytest.mark.parametrize("cfg,E", [(2, 9), (4, 5), (3, 6)])
@@ -1057,6 +1135,56 @@ def test_measured_peaks_and_kernel_timers(J):
     world.jenga_profile_enable(False)
     world.step(1); torch.cuda.synchronize()
     assert world.counters_dict()["env_steps"] == 64 * 4
+
+
+@pytest.mark.parametrize("EK", [1.0e-7, 2.0e-5])
+def test_until_rest_equals_single_steps_with_a_host_energy_test(J, EK):
+    """jenga_simulate_until_rest against its definition on the SAME CUDA trajectory: a second world
+    advances with jenga_step(1), the host reads E_k after every step and notes the first step with E_k < 1e-7 J.  Step
+    counts must be equal and the state an env was frozen with must be, bit for bit, the state of the stepping world at that
+    step -- also for an env that rests after its first step (the looser threshold: standing towers), one that never rests
+    within max_steps (the paper's 1e-7 J: towers still settling), and an env whose group sibling went to rest before it (two
+    envs per solver warp)."""
+    import torch
+    E, MAX = 14, 70
+    wl = W.make_config(2, n_envs=E)
+    lead = J.World(wl.params, wl.state, wl.props, wl.mu, tier="tmem160", group=2)
+    for lo, hi, f in ((0, wl.push_start, None), (wl.push_start, wl.push_end, wl.push_fext), (wl.push_end, 170, None)):
+        lead.set_f_ext(f); lead.step(hi - lo)
+    torch.cuda.synchronize()
+    start = lead.state.cpu().numpy()
+
+    def fresh():
+        w = J.World(wl.params, start, wl.props, wl.mu, collapse_length=W.BLOCK_L, tier="tmem160", group=2, ref_state=wl.state)
+        for name in ("cache_key", "cache_lam", "cache_pt", "n_cache"):
+            getattr(w, name).copy_(getattr(lead, name))
+        return w
+
+    a, b = fresh(), fresh()
+    a.simulate_until_rest(MAX, EK); torch.cuda.synchronize()
+    got = a.rest_steps.cpu().numpy()
+    want = np.full(E, MAX, np.int32); done = np.zeros(E, bool)
+    frozen = torch.zeros_like(b.state)
+    for s in range(1, MAX + 1):
+        b.step(1); torch.cuda.synchronize()
+        ek = b.collapse_stats[:, 1].cpu().numpy()
+        newly = (~done) & ((ek < EK) | (s == MAX))
+        want[newly] = s
+        sel = torch.as_tensor(newly).to(b.dev)
+        frozen[sel] = b.state[sel]
+        done |= newly
+    print(f"\n[until rest, exact] steps per env: {got.tolist()}")
+    assert np.array_equal(got, want)
+    assert torch.equal(a.state, frozen)
+    if EK > 1e-6:
+        assert (got == 1).any() and (got > 1).any()              # standing towers rest at once, falling ones later
+    else:
+        assert (got == MAX).any() and (got < MAX).any()
+    pairs = got.reshape(-1, 2)
+    assert (pairs[:, 0] != pairs[:, 1]).any()                    # a group whose members stopped at different steps
+    assert a.counters_dict()["env_steps"] == int(got.sum())
+    for w in (lead, a, b):
+        w.destroy()
 
 
 # ----------------------------------------------------------------------------- north_star's rollout bar, as stated (kept LAST in the file)
