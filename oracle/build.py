@@ -14,14 +14,22 @@ SRC = os.path.join(HERE, "jenga_oracle.c")
 LIB = os.path.join(HERE, "libjenga_oracle.so")
 
 
-def build(force: bool = False) -> str:
-    if (not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
-        return LIB
+LIB32 = os.path.join(HERE, "libjenga_oracle32.so")
+
+
+def build(force: bool = False, bits: int = 64) -> str:
+    """bits = 32: the fp32 build of the same source (control experiment of oracle/oracle32.py only)."""
+    lib = LIB if bits == 64 else LIB32
+    if (not force and os.path.exists(lib) and os.path.getmtime(lib) >= os.path.getmtime(SRC)):
+        return lib
     cmd = ["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
-           "-Wall", "-Wno-misleading-indentation", "-o", LIB, SRC, "-lm"]
+           "-Wall", "-Wno-misleading-indentation", "-o", lib, SRC, "-lm"]
+    if bits == 32:
+        cmd[1:1] = ["-DORC_REAL_FLOAT", "-fsingle-precision-constant", "-Wno-overflow"]
     subprocess.check_call(cmd)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv))
+    print(build(force="--force" in sys.argv, bits=32))

@@ -36,6 +36,15 @@
 #include <stdlib.h>
 #include <string.h>
 
+/* Control experiment only (oracle/oracle32.py, DESIGN.md §6 "rollout agreement"): the SAME source, same order of
+ * operations, with every floating-point variable, array and struct field in fp32 (build.py adds
+ * -DORC_REAL_FLOAT -fsingle-precision-constant; sqrt / fabs / acos are still libm's double routines, rounded on
+ * assignment).  It answers one question -- how often does a rollout of this method flip between fp64 and fp32 arithmetic,
+ * and in which direction -- and is never a parity reference.  The fp64 build does not see this line. */
+#ifdef ORC_REAL_FLOAT
+#define double float
+#endif
+
 #define ORC_PAIR_OVERFLOW    1u
 #define ORC_CONTACT_OVERFLOW 2u
 #define ORC_COLOUR_OVERFLOW  4u
